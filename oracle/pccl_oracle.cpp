@@ -1,0 +1,486 @@
+// =====================================================================================
+//  oracle/pccl_oracle.cpp  --  TEST INFRASTRUCTURE ONLY.  NOT PART OF THE PRODUCT PATH.
+//
+//  A plain, slow, single-threaded CPU statement of the greedy link-chunk matching
+//  synthesizer, written from /root/reference/PAPER.md and the readings listed in
+//  DESIGN.md (section "Readings of the paper", Q1..Q17).  It shares no code with the CUDA
+//  path under paper_2606_07019_b200/csrc (no headers, no helpers, no tables), and nothing
+//  in the product imports, links or executes it.  Only tests/, __graft_entry__.smoke()
+//  and bench.py's cpu_baseline / --impl reference legs may call it.
+//
+//  Representation: per-node holdings and wants are sorted std::vector<uint32_t> chunk-id
+//  lists; the candidate set of a link is std::set_intersection of two such lists.  There
+//  is no blocking, no bitmap, no fusion: each lettered step below is the step of the same
+//  letter in DESIGN.md "The procedure (steps R, A..F)".
+//
+//  What the paper fixes (and where):
+//    conditions (chunk: src -> dests) ............ PAPER.md:168-172  (section 4.1)
+//    a TEN link carries one chunk ................ PAPER.md:308      (section 4.4)
+//    alpha-beta link time  alpha + m*beta ........ PAPER.md:334      (section 4.6)
+//    forward only after arrival .................. PAPER.md:338      (section 4.6)
+//    a used link is busy for its whole interval .. PAPER.md:340      (section 4.6, Fig. 10)
+//    non-group NPUs are intermediates only ....... PAPER.md:298-300, :320
+//    Reduce = reversed Broadcast, RS = reversed AG, AR = RS then AG .. PAPER.md:324-330
+//    c.dist = shortest path, used for ordering ... PAPER.md:276, :310 (Alg. 3)
+//  What the paper does not fix (tie-break, conflict order, relay rule, rounding) follows
+//  the readings in DESIGN.md; the pick rule (step E2) is "parity unpinned" by the paper:
+//  it is pinned only by the Philox known-answer vectors, by brute-force enumeration of
+//  the k-th candidate in tests, and by the closed forms / invariants that any valid pick
+//  must satisfy.
+// =====================================================================================
+#include <algorithm>
+#include <cstdint>
+#include <cstring>
+#include <functional>
+#include <limits>
+#include <queue>
+#include <set>
+#include <utility>
+#include <vector>
+
+namespace {
+
+constexpr uint64_t INF = std::numeric_limits<uint64_t>::max();
+constexpr uint32_t NONE = 0xFFFFFFFFu;
+
+enum {
+    OR_OK = 0,
+    OR_ERR_INVALID = -1,
+    OR_ERR_UNSUPPORTED = -2,
+    OR_ERR_UNREACHABLE = -3,
+    OR_ERR_INTERNAL = -6
+};
+
+struct Link { uint32_t src, dst; uint64_t alpha_ps, bytes_per_ps; };
+struct Pair { uint32_t npu, chunk; };
+struct Rec  { uint32_t chunk, src, dst, link; uint64_t t_start_ps, t_end_ps; };
+struct Cond { uint32_t src; std::vector<uint32_t> dests; bool present = false; };
+
+// -------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw: "Parallel random numbers: as easy as 1, 2,
+// 3", SC'11).  10 rounds; multipliers 0xD2511F53 (on ctr[0]) and 0xCD9E8D57 (on ctr[2]);
+// Weyl key bumps 0x9E3779B9 / 0xBB67AE85.  Pinned by the published known-answer vectors
+// in tests/golden/philox_kat.txt.
+// -------------------------------------------------------------------------------------
+void philox4x32_10(const uint32_t ctr_in[4], const uint32_t key_in[2], uint32_t out[4]) {
+    uint32_t c0 = ctr_in[0], c1 = ctr_in[1], c2 = ctr_in[2], c3 = ctr_in[3];
+    uint32_t k0 = key_in[0], k1 = key_in[1];
+    for (int round = 0; round < 10; ++round) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n1 = (uint32_t)p1;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        const uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// first output word of Philox with key = (seed mod 2^32, seed >> 32)
+uint32_t draw(uint64_t seed, uint32_t a, uint32_t b, uint32_t c, uint32_t tag) {
+    const uint32_t ctr[4] = {a, b, c, tag};
+    const uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32)};
+    uint32_t out[4];
+    philox4x32_10(ctr, key, out);
+    return out[0];
+}
+
+// uniform index in [0, n) from a 32-bit draw:  (r * n) >> 32   (reading Q5)
+uint32_t scale(uint32_t r, uint64_t n) { return (uint32_t)(((uint64_t)r * n) >> 32); }
+
+// -------------------------------------------------------------------------------------
+// Step A.  alpha-beta link cost: alpha + m*beta with beta = 1/bandwidth.
+// Reading Q7: integer ceiling of m / bytes_per_ps, alpha added after.
+// -------------------------------------------------------------------------------------
+uint64_t link_cost(const Link& l, uint64_t chunk_bytes) {
+    return l.alpha_ps + (chunk_bytes + l.bytes_per_ps - 1) / l.bytes_per_ps;
+}
+
+// -------------------------------------------------------------------------------------
+// Step B.  ShortestPath(c.src, .) of Alg. 3, metric = alpha-beta cost
+// (reading Q3).  Textbook Dijkstra; only the distance values are used.
+// -------------------------------------------------------------------------------------
+std::vector<uint64_t> dijkstra(uint32_t n, const std::vector<Link>& links,
+                               const std::vector<uint64_t>& w, uint32_t s) {
+    std::vector<std::vector<uint32_t>> out(n);
+    for (uint32_t l = 0; l < links.size(); ++l) out[links[l].src].push_back(l);
+    std::vector<uint64_t> D(n, INF);
+    using QE = std::pair<uint64_t, uint32_t>;
+    std::priority_queue<QE, std::vector<QE>, std::greater<QE>> pq;
+    D[s] = 0;
+    pq.push({0, s});
+    while (!pq.empty()) {
+        auto [d, u] = pq.top();
+        pq.pop();
+        if (d != D[u]) continue;
+        for (uint32_t l : out[u]) {
+            const uint32_t v = links[l].dst;
+            if (d + w[l] < D[v]) { D[v] = d + w[l]; pq.push({D[v], v}); }
+        }
+    }
+    return D;
+}
+
+struct CopyResult {
+    std::vector<Rec> recs;   // canonical order: (t_start, link id)
+    uint64_t T = 0;          // max t_end, 0 if empty
+    uint64_t events = 0;     // number of event times processed (including t = 0)
+    uint64_t wants_total = 0;// popcount(wants) after step C
+};
+
+// sorted-vector set helpers
+bool contains(const std::vector<uint32_t>& v, uint32_t x) {
+    return std::binary_search(v.begin(), v.end(), x);
+}
+void insert_sorted(std::vector<uint32_t>& v, uint32_t x) {
+    auto it = std::lower_bound(v.begin(), v.end(), x);
+    if (it == v.end() || *it != x) v.insert(it, x);
+}
+void erase_sorted(std::vector<uint32_t>& v, uint32_t x) {
+    auto it = std::lower_bound(v.begin(), v.end(), x);
+    if (it != v.end() && *it == x) v.erase(it);
+}
+
+// -------------------------------------------------------------------------------------
+// synth_copy: steps A..F for non-reduction conditions (one source per chunk).
+// conds[c] is the condition of chunk c; chunks with !present or no dests need nothing.
+// -------------------------------------------------------------------------------------
+int synth_copy(uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& conds,
+               uint64_t chunk_bytes, uint64_t seed, CopyResult& res,
+               std::vector<std::vector<uint32_t>>* wants_out = nullptr) {
+    const uint32_t L = (uint32_t)links.size();
+    const uint32_t C = (uint32_t)conds.size();
+
+    // A. cost
+    std::vector<uint64_t> w(L);
+    for (uint32_t l = 0; l < L; ++l) w[l] = link_cost(links[l], chunk_bytes);
+
+    // in-links of every node in ascending link id
+    std::vector<std::vector<uint32_t>> inl(n);
+    for (uint32_t l = 0; l < L; ++l) inl[links[l].dst].push_back(l);
+
+    // B. distances from every distinct source
+    std::vector<std::vector<uint64_t>> D(n);
+    for (uint32_t c = 0; c < C; ++c) {
+        if (!conds[c].present || conds[c].dests.empty()) continue;
+        const uint32_t s = conds[c].src;
+        if (D[s].empty()) D[s] = dijkstra(n, links, w, s);
+        for (uint32_t d : conds[c].dests)
+            if (D[s][d] == INF) return OR_ERR_UNREACHABLE;
+    }
+
+    // C. wants = thin relay tree per chunk (reading Q4), have = the source
+    std::vector<std::vector<uint32_t>> have(n), wants(n);
+    for (uint32_t c = 0; c < C; ++c) {
+        if (!conds[c].present) continue;
+        const uint32_t s = conds[c].src;
+        insert_sorted(have[s], c);
+        if (conds[c].dests.empty()) continue;
+        const std::vector<uint64_t>& Ds = D[s];
+        std::set<uint32_t> marked;
+        for (uint32_t d : conds[c].dests) {
+            uint32_t cur = d;
+            while (cur != s && !marked.count(cur)) {
+                marked.insert(cur);
+                std::vector<uint32_t> tight;
+                for (uint32_t l : inl[cur]) {
+                    const uint32_t u = links[l].src;
+                    if (Ds[u] != INF && Ds[u] + w[l] == Ds[cur]) tight.push_back(l);
+                }
+                if (tight.empty()) return OR_ERR_INTERNAL;
+                const uint32_t j = scale(draw(seed, c, cur, 0, 1), tight.size());
+                cur = links[tight[j]].src;
+            }
+        }
+        for (uint32_t v : marked) insert_sorted(wants[v], c);
+    }
+    res.wants_total = 0;
+    for (uint32_t v = 0; v < n; ++v) res.wants_total += wants[v].size();
+    if (wants_out) *wants_out = wants;
+
+    // D. init
+    std::vector<uint64_t> free_t(L, 0);
+    std::vector<uint32_t> inflight(L, NONE);
+    uint64_t t = 0;
+    res.recs.clear();
+    res.events = 0;
+
+    // E. loop over event times
+    std::vector<uint32_t> cand;
+    for (;;) {
+        ++res.events;
+        // E1. arrivals: a chunk that arrives at t may be forwarded at t
+        for (uint32_t l = 0; l < L; ++l) {
+            if (inflight[l] != NONE && free_t[l] == t) {
+                insert_sorted(have[links[l].dst], inflight[l]);
+                inflight[l] = NONE;
+            }
+        }
+        // E2. match: destinations are independent; in-links of one destination are taken
+        //     in ascending link id, each seeing the claims of the earlier ones (reading Q6)
+        for (uint32_t v = 0; v < n; ++v) {
+            for (uint32_t l : inl[v]) {
+                if (free_t[l] > t) continue;           // link busy
+                if (wants[v].empty()) continue;
+                const std::vector<uint32_t>& hs = have[links[l].src];
+                cand.clear();
+                std::set_intersection(hs.begin(), hs.end(), wants[v].begin(), wants[v].end(),
+                                      std::back_inserter(cand));
+                if (cand.empty()) continue;            // link stays free
+                const uint32_t r = draw(seed, (uint32_t)(t & 0xFFFFFFFFull),
+                                        (uint32_t)(t >> 32), l, 0);
+                const uint32_t k = scale(r, cand.size());
+                const uint32_t c = cand[k];            // k-th smallest chunk id
+                erase_sorted(wants[v], c);
+                inflight[l] = c;
+                free_t[l] = t + w[l];
+                res.recs.push_back(Rec{c, links[l].src, v, l, t, t + w[l]});
+            }
+        }
+        // E3. advance to the next event time
+        uint64_t tn = INF;
+        for (uint32_t l = 0; l < L; ++l)
+            if (free_t[l] > t && free_t[l] < tn) tn = free_t[l];
+        if (tn == INF) break;
+        t = tn;
+    }
+
+    // F. finish
+    for (uint32_t v = 0; v < n; ++v)
+        if (!wants[v].empty()) return OR_ERR_INTERNAL;
+    for (uint32_t c = 0; c < C; ++c) {
+        if (!conds[c].present) continue;
+        for (uint32_t d : conds[c].dests)
+            if (!contains(have[d], c)) return OR_ERR_INTERNAL;
+    }
+    std::sort(res.recs.begin(), res.recs.end(), [](const Rec& a, const Rec& b) {
+        if (a.t_start_ps != b.t_start_ps) return a.t_start_ps < b.t_start_ps;
+        return a.link < b.link;
+    });
+    res.T = 0;
+    for (const Rec& r : res.recs) res.T = std::max(res.T, r.t_end_ps);
+    return OR_OK;
+}
+
+// -------------------------------------------------------------------------------------
+// REDUCE mode (reading Q10): synthesize the broadcast root -> holders on
+// the TRANSPOSED topology, then reverse every transfer in direction and in time.
+// -------------------------------------------------------------------------------------
+int synth_reduce(uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& bcast,
+                 uint64_t chunk_bytes, uint64_t seed, CopyResult& res) {
+    std::vector<Link> tr(links);
+    for (Link& l : tr) std::swap(l.src, l.dst);
+    CopyResult b;
+    const int rc = synth_copy(n, tr, bcast, chunk_bytes, seed, b);
+    if (rc != OR_OK) return rc;
+    res.recs.clear();
+    for (const Rec& r : b.recs)   // (c, a, b, l, ts, te) -> (c, src=b, dst=a, l, T-te, T-ts)
+        res.recs.push_back(Rec{r.chunk, r.dst, r.src, r.link, b.T - r.t_end_ps, b.T - r.t_start_ps});
+    std::sort(res.recs.begin(), res.recs.end(), [](const Rec& a, const Rec& b2) {
+        if (a.t_start_ps != b2.t_start_ps) return a.t_start_ps < b2.t_start_ps;
+        return a.link < b2.link;
+    });
+    res.T = b.T;
+    res.events = b.events;
+    res.wants_total = b.wants_total;
+    return OR_OK;
+}
+
+struct Result {
+    std::vector<Rec> recs;
+    uint64_t T = 0;
+    uint64_t events = 0;
+    uint64_t wants_total = 0;
+    uint64_t T_phase1 = 0;   // all-reduce: time of the reduce phase
+    int mode = 0;            // 0 copy, 1 reduce, 2 all-reduce
+};
+
+// -------------------------------------------------------------------------------------
+// Step R + dispatch.  Pre/postcondition (NPU-centric) -> conditions
+// (chunk-centric).  |pre(c)| > 1 marks a reduction chunk (reading Q12).
+// -------------------------------------------------------------------------------------
+int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uint32_t* group,
+               uint32_t n_members, uint32_t n_chunks, const Pair* pre_p, uint64_t n_pre,
+               const Pair* post_p, uint64_t n_post, uint64_t chunk_bytes, uint64_t seed,
+               Result& out) {
+    if (n_links && !links_p) return OR_ERR_INVALID;
+    if (n_members && !group) return OR_ERR_INVALID;
+    if ((n_pre && !pre_p) || (n_post && !post_p)) return OR_ERR_INVALID;
+    if (chunk_bytes == 0) return OR_ERR_INVALID;
+    std::vector<Link> links(links_p, links_p + n_links);
+    for (const Link& l : links) {
+        if (l.src >= n_npus || l.dst >= n_npus || l.src == l.dst || l.bytes_per_ps == 0)
+            return OR_ERR_INVALID;
+    }
+    std::vector<char> member(n_npus, 0);
+    for (uint32_t i = 0; i < n_members; ++i) {
+        if (group[i] >= n_npus || member[group[i]]) return OR_ERR_INVALID;
+        member[group[i]] = 1;
+    }
+    std::vector<std::set<uint32_t>> pre(n_chunks), post(n_chunks);
+    for (uint64_t i = 0; i < n_pre; ++i) {
+        if (pre_p[i].chunk >= n_chunks || pre_p[i].npu >= n_npus || !member[pre_p[i].npu])
+            return OR_ERR_INVALID;
+        pre[pre_p[i].chunk].insert(pre_p[i].npu);
+    }
+    for (uint64_t i = 0; i < n_post; ++i) {
+        if (post_p[i].chunk >= n_chunks || post_p[i].npu >= n_npus || !member[post_p[i].npu])
+            return OR_ERR_INVALID;
+        post[post_p[i].chunk].insert(post_p[i].npu);
+    }
+    bool all_single = true, all_multi_one = true, all_multi_many = true;
+    for (uint32_t c = 0; c < n_chunks; ++c) {
+        if (pre[c].empty() || post[c].empty()) return OR_ERR_INVALID;
+        const bool single = pre[c].size() == 1;
+        all_single &= single;
+        all_multi_one &= (!single && post[c].size() == 1);
+        all_multi_many &= (!single && post[c].size() > 1);
+    }
+
+    out = Result{};
+    if (all_single) {                                        // COPY
+        std::vector<Cond> conds(n_chunks);
+        for (uint32_t c = 0; c < n_chunks; ++c) {
+            conds[c].present = true;
+            conds[c].src = *pre[c].begin();
+            for (uint32_t d : post[c]) if (d != conds[c].src) conds[c].dests.push_back(d);
+        }
+        CopyResult r;
+        const int rc = synth_copy(n_npus, links, conds, chunk_bytes, seed, r);
+        if (rc != OR_OK) return rc;
+        out.recs = std::move(r.recs); out.T = r.T; out.events = r.events;
+        out.wants_total = r.wants_total; out.mode = 0;
+        return OR_OK;
+    }
+    if (all_multi_one) {                                     // REDUCE / Reduce-Scatter
+        std::vector<Cond> bc(n_chunks);
+        for (uint32_t c = 0; c < n_chunks; ++c) {
+            bc[c].present = true;
+            bc[c].src = *post[c].begin();
+            for (uint32_t d : pre[c]) if (d != bc[c].src) bc[c].dests.push_back(d);
+        }
+        CopyResult r;
+        const int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r);
+        if (rc != OR_OK) return rc;
+        out.recs = std::move(r.recs); out.T = r.T; out.events = r.events;
+        out.wants_total = r.wants_total; out.mode = 1; out.T_phase1 = r.T;
+        return OR_OK;
+    }
+    if (all_multi_many) {                                    // ALL-REDUCE = RS then AG (Q11)
+        std::vector<Cond> bc(n_chunks), cp(n_chunks);
+        for (uint32_t c = 0; c < n_chunks; ++c) {
+            std::vector<uint32_t> I;
+            for (uint32_t v : pre[c]) if (post[c].count(v)) I.push_back(v);
+            if (I.empty()) I.assign(post[c].begin(), post[c].end());
+            const uint32_t root = I[c % I.size()];           // std::set iterates ascending
+            bc[c].present = cp[c].present = true;
+            bc[c].src = cp[c].src = root;
+            for (uint32_t d : pre[c]) if (d != root) bc[c].dests.push_back(d);
+            for (uint32_t d : post[c]) if (d != root) cp[c].dests.push_back(d);
+        }
+        CopyResult r1, r2;
+        int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r1);
+        if (rc != OR_OK) return rc;
+        rc = synth_copy(n_npus, links, cp, chunk_bytes, seed, r2);
+        if (rc != OR_OK) return rc;
+        out.recs = std::move(r1.recs);
+        for (const Rec& r : r2.recs)
+            out.recs.push_back(Rec{r.chunk, r.src, r.dst, r.link, r.t_start_ps + r1.T, r.t_end_ps + r1.T});
+        std::sort(out.recs.begin(), out.recs.end(), [](const Rec& a, const Rec& b) {
+            if (a.t_start_ps != b.t_start_ps) return a.t_start_ps < b.t_start_ps;
+            return a.link < b.link;
+        });
+        out.T_phase1 = r1.T;
+        out.T = r1.T + r2.T;
+        out.events = r1.events + r2.events;
+        out.wants_total = r1.wants_total + r2.wants_total;
+        out.mode = 2;
+        return OR_OK;
+    }
+    return OR_ERR_UNSUPPORTED;
+}
+
+}  // namespace
+
+// =====================================================================================
+// C interface for ctypes (tests, smoke, bench cpu_baseline).  Host pointers only.
+// =====================================================================================
+extern "C" {
+
+struct oracle_link { uint32_t src, dst; uint64_t alpha_ps, bytes_per_ps; };
+struct oracle_pair { uint32_t npu, chunk; };
+struct oracle_rec  { uint32_t chunk, src, dst, link; uint64_t t_start_ps, t_end_ps; };
+static_assert(sizeof(oracle_link) == sizeof(Link), "layout");
+static_assert(sizeof(oracle_pair) == sizeof(Pair), "layout");
+static_assert(sizeof(oracle_rec) == sizeof(Rec) && sizeof(Rec) == 32, "layout");
+
+void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    philox4x32_10(ctr, key, out);
+}
+
+uint64_t oracle_link_cost(uint64_t alpha_ps, uint64_t bytes_per_ps, uint64_t chunk_bytes) {
+    return link_cost(Link{0, 1, alpha_ps, bytes_per_ps}, chunk_bytes);
+}
+
+// distances from s under the alpha-beta cost; out[n_npus], UINT64_MAX = unreachable
+int oracle_distances(uint32_t n_npus, const oracle_link* links, uint32_t n_links,
+                     uint64_t chunk_bytes, uint32_t s, uint64_t* out) {
+    std::vector<Link> ls((const Link*)links, (const Link*)links + n_links);
+    std::vector<uint64_t> w(n_links);
+    for (uint32_t l = 0; l < n_links; ++l) w[l] = link_cost(ls[l], chunk_bytes);
+    std::vector<uint64_t> D = dijkstra(n_npus, ls, w, s);
+    std::copy(D.begin(), D.end(), out);
+    return OR_OK;
+}
+
+int oracle_synthesize(uint32_t n_npus, const oracle_link* links, uint32_t n_links,
+                      const uint32_t* group, uint32_t n_members, uint32_t n_chunks,
+                      const oracle_pair* pre, uint64_t n_pre, const oracle_pair* post,
+                      uint64_t n_post, uint64_t chunk_bytes, uint64_t seed, void** handle) {
+    if (!handle) return OR_ERR_INVALID;
+    Result* r = new Result();
+    const int rc = synthesize(n_npus, (const Link*)links, n_links, group, n_members, n_chunks,
+                              (const Pair*)pre, n_pre, (const Pair*)post, n_post, chunk_bytes,
+                              seed, *r);
+    if (rc != OR_OK) { delete r; return rc; }
+    *handle = r;
+    return OR_OK;
+}
+
+// wants relation of step C for a COPY-mode problem given directly as conditions:
+// cond_src[c], dests CSR (dest_off[c]..dest_off[c+1]).  Writes pairs (node, chunk) sorted
+// by (node, chunk) to out (capacity cap); returns the number of pairs or a negative error.
+int64_t oracle_wants(uint32_t n_npus, const oracle_link* links, uint32_t n_links,
+                     uint32_t n_chunks, const uint32_t* cond_src, const uint64_t* dest_off,
+                     const uint32_t* dests, uint64_t chunk_bytes, uint64_t seed,
+                     oracle_pair* out, uint64_t cap) {
+    std::vector<Link> ls((const Link*)links, (const Link*)links + n_links);
+    std::vector<Cond> conds(n_chunks);
+    for (uint32_t c = 0; c < n_chunks; ++c) {
+        conds[c].present = true;
+        conds[c].src = cond_src[c];
+        conds[c].dests.assign(dests + dest_off[c], dests + dest_off[c + 1]);
+    }
+    CopyResult r;
+    std::vector<std::vector<uint32_t>> wants;
+    const int rc = synth_copy(n_npus, ls, conds, chunk_bytes, seed, r, &wants);
+    if (rc != OR_OK) return rc;
+    uint64_t k = 0;
+    for (uint32_t v = 0; v < n_npus; ++v)
+        for (uint32_t c : wants[v]) { if (k < cap) out[k] = oracle_pair{v, c}; ++k; }
+    return (int64_t)k;
+}
+
+uint64_t oracle_size(const void* h) { return ((const Result*)h)->recs.size(); }
+const oracle_rec* oracle_records(const void* h) { return (const oracle_rec*)((const Result*)h)->recs.data(); }
+uint64_t oracle_time(const void* h) { return ((const Result*)h)->T; }
+uint64_t oracle_events(const void* h) { return ((const Result*)h)->events; }
+uint64_t oracle_wants_total(const void* h) { return ((const Result*)h)->wants_total; }
+uint64_t oracle_time_phase1(const void* h) { return ((const Result*)h)->T_phase1; }
+int oracle_mode(const void* h) { return ((const Result*)h)->mode; }
+void oracle_free(void* h) { delete (Result*)h; }
+
+}  // extern "C"
