@@ -1,0 +1,223 @@
+/* =========================================================================================
+ * pccl.h -- C-ABI boundary of the B200-native link-chunk matching synthesizer.
+ *
+ * What the library computes: a collective-communication schedule for one or several
+ * process groups on an arbitrary topology, by per-event link-chunk matching over the
+ * time-expanded network (TEN).  The problem statement is the paper's:
+ *   - topology with per-link latency alpha and bandwidth 1/beta ...... PAPER.md:334 (sec 4.6)
+ *   - collective as NPU-centric pre/postcondition ...................... PAPER.md:76  (sec 2.1)
+ *   - process group = the NPUs that take part; others only relay ...... PAPER.md:84  (sec 2.2),
+ *                                                                        :298-300, :320, :422
+ *   - result: which chunk crosses which link during which interval .... PAPER.md:149-156 (sec 3.5)
+ * The matching procedure itself (steps R, A..F) is written out in DESIGN.md.
+ *
+ * Conventions
+ *   - Every function that returns int returns PCCL_OK (0) or a negative pccl_error; on error
+ *     every `out` pointer is left untouched.  No function throws or aborts.
+ *   - "host" / "device" in a parameter comment says which address space the pointer is in.
+ *     Input arrays are BORROWED for the duration of the call only.
+ *   - Handles are opaque, owned by the library, released by the matching *_destroy
+ *     (NULL is accepted and ignored).
+ *   - All times are unsigned 64-bit integer picoseconds.  No floating point anywhere.
+ *   - n_npus counts ALL nodes of the network: NPUs and switch nodes alike (PAPER.md:256,
+ *     :348).  A switch is a node that is never listed in group_members.
+ *   - Link id = index into the `links` array.  Parallel links are legal.
+ *   - Several concurrent process groups go in ONE call: group_members is their union, chunk
+ *     ids are globally unique.
+ *   - Device work is enqueued on the stream set with pccl_set_stream (default: the legacy
+ *     default stream) of the CUDA device that is current when the handle is created, and is
+ *     synchronised before a function returns host-visible results.
+ *   - Calls on distinct handles are independent; a single handle must not be used from two
+ *     threads at once.  The process-wide settings (stream, allocator) are not thread-safe.
+ *   - There is NO CPU fallback: without a CUDA device every compute entry point returns
+ *     PCCL_ERR_CUDA.
+ * ========================================================================================= */
+#ifndef PCCL_H_
+#define PCCL_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PCCL_VERSION 100 /* 0.1.0 */
+
+typedef enum pccl_error {
+    PCCL_OK = 0,
+    PCCL_ERR_INVALID = -1,     /* null pointer; src/dst >= n_npus; self-loop; bytes_per_ps == 0;
+                                  chunk_bytes == 0; duplicate or out-of-range group member; a
+                                  pair whose NPU is not a group member; chunk id >= n_chunks; a
+                                  chunk with no pre-holder or no post-holder; pre.n_chunks !=
+                                  post.n_chunks */
+    PCCL_ERR_UNSUPPORTED = -2, /* copy and reduction chunks mixed in one call (DESIGN.md step R);
+                                  sizes beyond the limits listed in DESIGN.md */
+    PCCL_ERR_UNREACHABLE = -3, /* some destination cannot be reached from its chunk's source */
+    PCCL_ERR_CUDA = -4,        /* any CUDA runtime failure, including "no device" */
+    PCCL_ERR_NOMEM = -5,       /* host or device allocation failed */
+    PCCL_ERR_INTERNAL = -6     /* a post-run invariant failed (never expected) */
+} pccl_error;
+
+/* A directed physical link, cost alpha_ps + ceil(chunk_bytes / bytes_per_ps) picoseconds
+ * (alpha-beta model; integer ceiling = DESIGN.md reading Q7). */
+typedef struct pccl_link {
+    uint32_t src, dst;
+    uint64_t alpha_ps, bytes_per_ps;
+} pccl_link_t;
+
+/* "npu holds chunk" -- one element of an NPU-centric pre- or postcondition. */
+typedef struct pccl_pair {
+    uint32_t npu, chunk;
+} pccl_pair_t;
+
+typedef struct pccl_condition {
+    uint32_t n_chunks;        /* chunk ids are 0 .. n_chunks-1 */
+    uint64_t n_pairs;
+    const pccl_pair_t* pairs; /* host; any order; duplicates are ignored */
+} pccl_condition_t;
+
+/* One transfer of the schedule: `chunk` occupies physical link `link` (src -> dst) during
+ * [t_start_ps, t_end_ps).  32 bytes, no padding. */
+typedef struct pccl_transfer {
+    uint32_t chunk, src, dst, link;
+    uint64_t t_start_ps, t_end_ps;
+} pccl_transfer_t;
+
+typedef struct pccl_topology pccl_topology_t;
+typedef struct pccl_problem pccl_problem_t;
+typedef struct pccl_schedule pccl_schedule_t;
+
+/* ---------------------------------------------------------------------------------------
+ * Process-wide plumbing (PyTorch supplies these through the Python binding).
+ * ------------------------------------------------------------------------------------- */
+
+/* cuda_stream: a cudaStream_t (NULL = legacy default stream).  All later device work of the
+ * library is enqueued on it. */
+void pccl_set_stream(void* cuda_stream);
+
+/* Device allocator hooks.  alloc(bytes, cuda_stream, user) returns a device pointer aligned
+ * to >= 256 bytes or NULL; release(ptr, user) gives it back.  Both NULL restores the
+ * built-in stream-ordered allocator (cudaMallocAsync / cudaFreeAsync).  The library makes
+ * O(1) allocations per call (one workspace, one result buffer). */
+typedef void* (*pccl_alloc_fn)(size_t bytes, void* cuda_stream, void* user);
+typedef void (*pccl_free_fn)(void* device_ptr, void* user);
+void pccl_set_allocator(pccl_alloc_fn alloc, pccl_free_fn release, void* user);
+
+const char* pccl_strerror(int err);
+int pccl_version(void);
+
+/* ---------------------------------------------------------------------------------------
+ * Topology store (DESIGN.md row a0 and the link/in-link tables).
+ * links: host array of n_links directed links.  Validates endpoints, builds the per-node
+ * in-link and out-link tables in ascending link id on the host; the device copy is made on
+ * first use.  Errors: INVALID, NOMEM.
+ * ------------------------------------------------------------------------------------- */
+int pccl_topology_create(uint32_t n_npus, const pccl_link_t* links, uint32_t n_links,
+                         pccl_topology_t** out);
+void pccl_topology_destroy(pccl_topology_t* topo);
+uint32_t pccl_topology_n_npus(const pccl_topology_t* topo);
+uint32_t pccl_topology_n_links(const pccl_topology_t* topo);
+
+/* ---------------------------------------------------------------------------------------
+ * pccl_synthesize -- the whole path with HOST buffers (the paper's problem statement,
+ * PAPER.md:149-156): normalise (step R), upload, run steps A..F on the GPU, download.
+ * group_members: host, n_members distinct node ids.  precondition / postcondition: which
+ * group NPU holds which chunk before / after.  |pre(c)| = 1 for every chunk
+ * means a copy collective (All-Gather, All-to-All(v), Broadcast ...); |pre(c)| > 1 with
+ * |post(c)| = 1 a reduction (Reduce, Reduce-Scatter); |pre(c)| > 1 with |post(c)| > 1
+ * All-Reduce = Reduce-Scatter then All-Gather.  seed keys the
+ * deterministic tie-breaks (Philox4x32-10).  The schedule's transfers are in host memory
+ * on return.  Errors: INVALID, UNSUPPORTED, UNREACHABLE, CUDA, NOMEM, INTERNAL.
+ * ------------------------------------------------------------------------------------- */
+int pccl_synthesize(const pccl_topology_t* topo, const uint32_t* group_members,
+                    uint32_t n_members, const pccl_condition_t* precondition,
+                    const pccl_condition_t* postcondition, uint64_t chunk_bytes, uint64_t seed,
+                    pccl_schedule_t** out);
+
+/* ---------------------------------------------------------------------------------------
+ * Prepared problem: step R done once (host), conditions resident in HBM; then any number of
+ * seeds can be synthesized with no host input traffic (best-of-K seed sweeps).
+ * pccl_problem_create borrows topo for the lifetime of the problem (destroy the problem
+ * first).  It validates and normalises on the host only; the device copy is made by the
+ * first pccl_problem_synthesize (or pccl_problem_upload).
+ * ------------------------------------------------------------------------------------- */
+int pccl_problem_create(const pccl_topology_t* topo, const uint32_t* group_members,
+                        uint32_t n_members, const pccl_condition_t* precondition,
+                        const pccl_condition_t* postcondition, uint64_t chunk_bytes,
+                        pccl_problem_t** out);
+void pccl_problem_destroy(pccl_problem_t* problem);
+int pccl_problem_upload(pccl_problem_t* problem); /* Errors: CUDA, NOMEM */
+
+/* 0 copy, 1 reduce / reduce-scatter, 2 all-reduce (DESIGN.md step R) */
+int pccl_problem_mode(const pccl_problem_t* problem);
+uint32_t pccl_problem_n_chunks(const pccl_problem_t* problem);
+/* Chunk-centric condition of `chunk` in `phase` (0: the only phase of a
+ * copy or reduce problem, or the reduce phase of all-reduce; 1: the copy phase of
+ * all-reduce).  *src = the source (copy) or root (reduce); returns the number of dests and
+ * writes up to cap of them, ascending, to dests (host; may be NULL when cap == 0).
+ * Returns a negative pccl_error for a bad chunk / phase. */
+int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, uint32_t chunk,
+                               uint32_t* src, uint32_t* dests, uint64_t cap);
+
+/* flags for pccl_problem_synthesize */
+#define PCCL_FLAG_KEEP_ON_DEVICE 1u /* do not download the transfers until they are asked for */
+#define PCCL_FLAG_NO_IDLE_SKIP 2u   /* rescan idle links every event (debug / measurement) */
+#define PCCL_FLAG_TIME_LOOP 4u      /* record CUDA events around the event loop (stats) */
+
+/* Steps A..F on the GPU for one seed.  Errors: UNREACHABLE, CUDA, NOMEM, INTERNAL. */
+int pccl_problem_synthesize(pccl_problem_t* problem, uint64_t seed, uint32_t flags,
+                            pccl_schedule_t** out);
+
+/* ---------------------------------------------------------------------------------------
+ * Schedule.  Transfers are in canonical order: ascending (t_start_ps, link).
+ * ------------------------------------------------------------------------------------- */
+uint64_t pccl_schedule_time(const pccl_schedule_t* s); /* max t_end_ps; 0 if empty */
+uint64_t pccl_schedule_size(const pccl_schedule_t* s); /* number of transfers */
+/* host pointer, valid until the schedule is destroyed; downloads on first use when the
+ * schedule was kept on the device; NULL if empty or on a CUDA failure */
+const pccl_transfer_t* pccl_schedule_transfers(pccl_schedule_t* s);
+/* device pointer to the same records (NULL once released or if empty) */
+const pccl_transfer_t* pccl_schedule_transfers_device(const pccl_schedule_t* s);
+void pccl_schedule_destroy(pccl_schedule_t* s);
+
+/* Counters of the run that produced the schedule. */
+typedef struct pccl_stats {
+    uint64_t events;         /* event times processed (both phases of an all-reduce summed) */
+    uint64_t wants_total;    /* popcount(wants) after step C == number of transfers */
+    uint64_t rows_scanned;   /* bitmap rows the match kernel requested (have + wants rows) */
+    uint64_t row_bytes;      /* bytes of one (padded) bitmap row */
+    uint64_t links_scanned;  /* active in-links whose candidates were counted */
+    uint64_t slow_picks;     /* picks that took the serial re-pick path */
+    uint64_t time_phase1_ps; /* all-reduce: time of the reduce phase */
+    float loop_ms;           /* event-loop kernel time (PCCL_FLAG_TIME_LOOP), else 0 */
+    float setup_ms;          /* steps A..D kernels (PCCL_FLAG_TIME_LOOP), else 0 */
+    float emit_ms;           /* emitter kernels (PCCL_FLAG_TIME_LOOP), else 0 */
+    uint32_t mode;           /* 0 copy, 1 reduce, 2 all-reduce */
+    uint32_t grid_blocks;    /* CTAs of the persistent event-loop kernel */
+} pccl_stats_t;
+int pccl_schedule_stats(const pccl_schedule_t* s, pccl_stats_t* out);
+
+/* ---------------------------------------------------------------------------------------
+ * Single rows of the path, exposed for parity tests against the oracle.  Each runs the
+ * same device code the full path uses.
+ * ------------------------------------------------------------------------------------- */
+/* a6: Philox4x32-10 evaluated on the GPU for n counters.  ctr: host n*4 u32, key: host 2
+ * u32, out: host n*4 u32. */
+int pccl_device_philox(const uint32_t* ctr, uint64_t n, const uint32_t key[2], uint32_t* out);
+/* a0: link costs, out: host n_links u64. */
+int pccl_device_link_costs(pccl_topology_t* topo, uint64_t chunk_bytes, uint64_t* out);
+/* a1: alpha-beta shortest distances from src (transposed != 0: on the reversed links),
+ * out: host n_npus u64, UINT64_MAX = unreachable. */
+int pccl_device_distances(pccl_topology_t* topo, uint64_t chunk_bytes, uint32_t src,
+                          int transposed, uint64_t* out);
+/* a2: wants relation of `phase` after step C for `seed`, as (node, chunk) pairs sorted by
+ * (node, chunk).  Returns the pair count (may exceed cap; only cap are written) or a
+ * negative pccl_error.  out: host. */
+int64_t pccl_device_wants(pccl_problem_t* problem, uint32_t phase, uint64_t seed,
+                          pccl_pair_t* out, uint64_t cap);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PCCL_H_ */

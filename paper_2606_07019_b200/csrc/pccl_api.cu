@@ -1,0 +1,917 @@
+// =========================================================================================
+// pccl_api.cu -- host side of libpccl.so: the C-ABI of include/pccl.h, the normaliser
+// (DESIGN.md step R), device-memory layout and kernel orchestration.  All arithmetic of
+// steps A..F runs in the kernels of pccl_device.cuh; this file only validates, lays out
+// memory, launches and copies.
+// =========================================================================================
+#include "../../include/pccl.h"
+
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <vector>
+
+#include "pccl_device.cuh"
+
+using namespace pccl;
+
+static_assert(sizeof(pccl_transfer_t) == sizeof(Rec), "record layout");
+static_assert(sizeof(pccl_link_t) == 24 && sizeof(pccl_pair_t) == 8, "abi layout");
+
+// -----------------------------------------------------------------------------------------
+// process-wide plumbing
+// -----------------------------------------------------------------------------------------
+namespace {
+
+struct Globals {
+    cudaStream_t stream = nullptr;
+    pccl_alloc_fn alloc = nullptr;
+    pccl_free_fn release = nullptr;
+    void* user = nullptr;
+    std::mutex mu;
+    // pinned host memory: a small mailbox for control blocks and a free-list of result buffers
+    void* mailbox = nullptr;
+    struct Pinned { void* p; size_t bytes; };
+    std::vector<Pinned> pinned_free;
+    int sm_count = 0;
+    int dev = -1;
+} G;
+
+#define CU(call)                                   \
+    do {                                           \
+        cudaError_t e__ = (call);                  \
+        if (e__ != cudaSuccess) {                  \
+            (void)cudaGetLastError();              \
+            return PCCL_ERR_CUDA;                  \
+        }                                          \
+    } while (0)
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+int dev_alloc(size_t bytes, void** out) {
+    if (bytes == 0) bytes = 256;
+    void* p = nullptr;
+    if (G.alloc) {
+        p = G.alloc(bytes, (void*)G.stream, G.user);
+        if (!p) return PCCL_ERR_NOMEM;
+    } else {
+        cudaError_t e = cudaMallocAsync(&p, bytes, G.stream);
+        if (e == cudaErrorMemoryAllocation) { (void)cudaGetLastError(); return PCCL_ERR_NOMEM; }
+        if (e != cudaSuccess) { (void)cudaGetLastError(); return PCCL_ERR_CUDA; }
+    }
+    *out = p;
+    return PCCL_OK;
+}
+
+void dev_free(void* p) {
+    if (!p) return;
+    if (G.release) G.release(p, G.user);
+    else if (cudaFreeAsync(p, G.stream) != cudaSuccess) (void)cudaGetLastError();
+}
+
+int ensure_device() {
+    if (G.dev >= 0) return PCCL_OK;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    int sms = 0;
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    int coop = 0;
+    CU(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    if (!coop) return PCCL_ERR_CUDA;
+    void* mb = nullptr;
+    CU(cudaHostAlloc(&mb, 4096, cudaHostAllocDefault));
+    G.mailbox = mb;
+    G.sm_count = sms;
+    G.dev = dev;
+    return PCCL_OK;
+}
+
+void* pinned_get(size_t bytes) {
+    {
+        std::lock_guard<std::mutex> lk(G.mu);
+        size_t best = (size_t)-1;
+        for (size_t i = 0; i < G.pinned_free.size(); ++i)
+            if (G.pinned_free[i].bytes >= bytes && (best == (size_t)-1 || G.pinned_free[i].bytes < G.pinned_free[best].bytes)) best = i;
+        if (best != (size_t)-1 && G.pinned_free[best].bytes <= 2 * bytes + (1u << 20)) {
+            void* p = G.pinned_free[best].p;
+            G.pinned_free.erase(G.pinned_free.begin() + best);
+            return p;
+        }
+    }
+    void* p = nullptr;
+    if (cudaHostAlloc(&p, bytes ? bytes : 32, cudaHostAllocDefault) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+    return p;
+}
+
+void pinned_put(void* p, size_t bytes) {
+    if (!p) return;
+    std::lock_guard<std::mutex> lk(G.mu);
+    if (G.pinned_free.size() >= 4) {   // keep the cache small: drop the smallest
+        size_t s = 0;
+        for (size_t i = 1; i < G.pinned_free.size(); ++i) if (G.pinned_free[i].bytes < G.pinned_free[s].bytes) s = i;
+        if (G.pinned_free[s].bytes < bytes) {
+            (void)cudaFreeHost(G.pinned_free[s].p);
+            G.pinned_free[s] = {p, bytes};
+        } else {
+            (void)cudaFreeHost(p);
+        }
+        return;
+    }
+    G.pinned_free.push_back({p, bytes});
+}
+
+}  // namespace
+
+// -----------------------------------------------------------------------------------------
+// handles
+// -----------------------------------------------------------------------------------------
+struct pccl_topology {
+    uint32_t N = 0, L = 0;
+    std::vector<pccl_link_t> links;
+    std::vector<uint32_t> in_off, in_link, out_off, out_link;   // ascending link id per node
+    // device copy (one blob)
+    void* blob = nullptr;
+    uint32_t *d_src = nullptr, *d_dst = nullptr, *d_in_off = nullptr, *d_in_link = nullptr,
+             *d_out_off = nullptr, *d_out_link = nullptr;
+    uint64_t *d_alpha = nullptr, *d_bpp = nullptr;
+};
+
+namespace {
+
+struct Phase {
+    bool transposed = false;          // run on the reversed links (reductions, Q10)
+    std::vector<uint32_t> cond_src;   // [C] source (copy) or root (reduce) of each chunk
+    std::vector<uint64_t> dest_off;   // [C+1]
+    std::vector<uint32_t> dests;      // ascending per chunk
+    std::vector<uint32_t> dchunk;     // [n_dests] chunk of each (chunk, dest) pair
+    std::vector<uint32_t> sources;    // distinct sources, ascending
+    std::vector<uint32_t> sidx;       // [N] node -> row of D, NONE32 if not a source
+    void* blob = nullptr;
+    uint32_t *d_cond_src = nullptr, *d_dests = nullptr, *d_dchunk = nullptr, *d_sources = nullptr,
+             *d_sidx = nullptr;
+};
+
+}  // namespace
+
+struct pccl_problem {
+    const pccl_topology* topo = nullptr;
+    uint32_t C = 0;
+    uint64_t chunk_bytes = 0;
+    int mode = 0;
+    std::vector<Phase> phases;
+    bool uploaded = false;
+};
+
+struct pccl_schedule {
+    uint64_t M = 0, T = 0;
+    Rec* d_recs = nullptr;
+    void* h_recs = nullptr;
+    size_t h_bytes = 0;
+    bool downloaded = false;
+    pccl_stats_t stats;
+};
+
+// -----------------------------------------------------------------------------------------
+// plumbing entry points
+// -----------------------------------------------------------------------------------------
+extern "C" void pccl_set_stream(void* s) { G.stream = (cudaStream_t)s; }
+extern "C" void pccl_set_allocator(pccl_alloc_fn a, pccl_free_fn f, void* user) {
+    if (a && f) { G.alloc = a; G.release = f; G.user = user; }
+    else { G.alloc = nullptr; G.release = nullptr; G.user = nullptr; }
+}
+extern "C" int pccl_version(void) { return PCCL_VERSION; }
+extern "C" const char* pccl_strerror(int err) {
+    switch (err) {
+        case PCCL_OK: return "ok";
+        case PCCL_ERR_INVALID: return "invalid argument";
+        case PCCL_ERR_UNSUPPORTED: return "unsupported problem (mixed copy/reduction chunks or size limit)";
+        case PCCL_ERR_UNREACHABLE: return "a destination is unreachable from its chunk's source";
+        case PCCL_ERR_CUDA: return "CUDA failure (no device, launch or copy error)";
+        case PCCL_ERR_NOMEM: return "out of memory";
+        case PCCL_ERR_INTERNAL: return "internal invariant violated";
+        default: return "unknown error";
+    }
+}
+
+// -----------------------------------------------------------------------------------------
+// topology store
+// -----------------------------------------------------------------------------------------
+extern "C" int pccl_topology_create(uint32_t n_npus, const pccl_link_t* links, uint32_t n_links,
+                                    pccl_topology_t** out) {
+    if (!out || (n_links && !links)) return PCCL_ERR_INVALID;
+    for (uint32_t l = 0; l < n_links; ++l) {
+        const pccl_link_t& k = links[l];
+        if (k.src >= n_npus || k.dst >= n_npus || k.src == k.dst || k.bytes_per_ps == 0) return PCCL_ERR_INVALID;
+    }
+    pccl_topology* t = new (std::nothrow) pccl_topology();
+    if (!t) return PCCL_ERR_NOMEM;
+    try {
+        t->N = n_npus;
+        t->L = n_links;
+        t->links.assign(links, links + n_links);
+        t->in_off.assign((size_t)n_npus + 1, 0);
+        t->out_off.assign((size_t)n_npus + 1, 0);
+        for (uint32_t l = 0; l < n_links; ++l) { ++t->in_off[links[l].dst + 1]; ++t->out_off[links[l].src + 1]; }
+        for (uint32_t v = 0; v < n_npus; ++v) { t->in_off[v + 1] += t->in_off[v]; t->out_off[v + 1] += t->out_off[v]; }
+        t->in_link.resize(n_links);
+        t->out_link.resize(n_links);
+        std::vector<uint32_t> ci(t->in_off.begin(), t->in_off.end() - 1), co(t->out_off.begin(), t->out_off.end() - 1);
+        for (uint32_t l = 0; l < n_links; ++l) {   // ascending l => each node's list is ascending
+            t->in_link[ci[links[l].dst]++] = l;
+            t->out_link[co[links[l].src]++] = l;
+        }
+    } catch (const std::bad_alloc&) {
+        delete t;
+        return PCCL_ERR_NOMEM;
+    }
+    *out = t;
+    return PCCL_OK;
+}
+
+extern "C" void pccl_topology_destroy(pccl_topology_t* t) {
+    if (!t) return;
+    dev_free(t->blob);
+    delete t;
+}
+extern "C" uint32_t pccl_topology_n_npus(const pccl_topology_t* t) { return t ? t->N : 0; }
+extern "C" uint32_t pccl_topology_n_links(const pccl_topology_t* t) { return t ? t->L : 0; }
+
+namespace {
+
+// carve a blob: returns offset, advances cursor (256-byte aligned pieces)
+struct Carver {
+    size_t cur = 0;
+    size_t take(size_t bytes) { const size_t o = cur; cur = align_up(cur + bytes, 256); return o; }
+};
+
+int topo_upload(pccl_topology* t) {
+    if (t->blob) return PCCL_OK;
+    int rc = ensure_device();
+    if (rc) return rc;
+    const size_t N = t->N, L = t->L;
+    Carver c;
+    const size_t o_src = c.take(L * 4), o_dst = c.take(L * 4), o_alpha = c.take(L * 8), o_bpp = c.take(L * 8),
+                 o_ino = c.take((N + 1) * 4), o_inl = c.take(L * 4), o_outo = c.take((N + 1) * 4), o_outl = c.take(L * 4);
+    std::vector<unsigned char> h(c.cur ? c.cur : 256, 0);
+    for (size_t l = 0; l < L; ++l) {
+        ((uint32_t*)(h.data() + o_src))[l] = t->links[l].src;
+        ((uint32_t*)(h.data() + o_dst))[l] = t->links[l].dst;
+        ((uint64_t*)(h.data() + o_alpha))[l] = t->links[l].alpha_ps;
+        ((uint64_t*)(h.data() + o_bpp))[l] = t->links[l].bytes_per_ps;
+    }
+    memcpy(h.data() + o_ino, t->in_off.data(), (N + 1) * 4);
+    memcpy(h.data() + o_outo, t->out_off.data(), (N + 1) * 4);
+    if (L) {
+        memcpy(h.data() + o_inl, t->in_link.data(), L * 4);
+        memcpy(h.data() + o_outl, t->out_link.data(), L * 4);
+    }
+    void* blob = nullptr;
+    rc = dev_alloc(h.size(), &blob);
+    if (rc) return rc;
+    if (cudaMemcpyAsync(blob, h.data(), h.size(), cudaMemcpyHostToDevice, G.stream) != cudaSuccess ||
+        cudaStreamSynchronize(G.stream) != cudaSuccess) {
+        (void)cudaGetLastError();
+        dev_free(blob);
+        return PCCL_ERR_CUDA;
+    }
+    unsigned char* b = (unsigned char*)blob;
+    t->blob = blob;
+    t->d_src = (uint32_t*)(b + o_src); t->d_dst = (uint32_t*)(b + o_dst);
+    t->d_alpha = (uint64_t*)(b + o_alpha); t->d_bpp = (uint64_t*)(b + o_bpp);
+    t->d_in_off = (uint32_t*)(b + o_ino); t->d_in_link = (uint32_t*)(b + o_inl);
+    t->d_out_off = (uint32_t*)(b + o_outo); t->d_out_link = (uint32_t*)(b + o_outl);
+    return PCCL_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// step R: NPU-centric pre/postcondition -> chunk-centric conditions
+// (PAPER.md:170-172); |pre(c)| > 1 marks a reduction chunk (Q12).
+// ---------------------------------------------------------------------------------------
+// per-chunk ascending, duplicate-free NPU lists
+int group_pairs(const pccl_condition_t* cnd, uint32_t C, uint32_t N, const std::vector<char>& member,
+                std::vector<uint64_t>& off, std::vector<uint32_t>& npus) {
+    off.assign((size_t)C + 1, 0);
+    for (uint64_t i = 0; i < cnd->n_pairs; ++i) {
+        const pccl_pair_t& p = cnd->pairs[i];
+        if (p.chunk >= C || p.npu >= N || !member[p.npu]) return PCCL_ERR_INVALID;
+        ++off[p.chunk + 1];
+    }
+    for (uint32_t c = 0; c < C; ++c) off[c + 1] += off[c];
+    std::vector<uint32_t> tmp(cnd->n_pairs);
+    std::vector<uint64_t> cur(off.begin(), off.end() - 1);
+    for (uint64_t i = 0; i < cnd->n_pairs; ++i) tmp[cur[cnd->pairs[i].chunk]++] = cnd->pairs[i].npu;
+    // sort + unique each list, compacting in place
+    npus.clear();
+    npus.reserve(cnd->n_pairs);
+    std::vector<uint64_t> noff((size_t)C + 1, 0);
+    for (uint32_t c = 0; c < C; ++c) {
+        uint32_t* b = tmp.data() + off[c];
+        uint32_t* e = tmp.data() + off[c + 1];
+        if (e - b > 1) { std::sort(b, e); e = std::unique(b, e); }
+        npus.insert(npus.end(), b, e);
+        noff[c + 1] = npus.size();
+    }
+    off.swap(noff);
+    return PCCL_OK;
+}
+
+void finish_phase(Phase& ph, uint32_t N) {
+    const uint32_t C = (uint32_t)ph.cond_src.size();
+    ph.dchunk.resize(ph.dests.size());
+    std::vector<char> is_src(N, 0);
+    for (uint32_t c = 0; c < C; ++c) {
+        for (uint64_t i = ph.dest_off[c]; i < ph.dest_off[c + 1]; ++i) ph.dchunk[i] = c;
+        if (ph.dest_off[c + 1] > ph.dest_off[c]) is_src[ph.cond_src[c]] = 1;
+    }
+    ph.sidx.assign(N, NONE32);
+    for (uint32_t v = 0; v < N; ++v)
+        if (is_src[v]) { ph.sidx[v] = (uint32_t)ph.sources.size(); ph.sources.push_back(v); }
+}
+
+int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_members,
+              const pccl_condition_t* pre, const pccl_condition_t* post, uint64_t chunk_bytes,
+              pccl_problem& P) {
+    if (!topo || !pre || !post || (n_members && !group)) return PCCL_ERR_INVALID;
+    if ((pre->n_pairs && !pre->pairs) || (post->n_pairs && !post->pairs)) return PCCL_ERR_INVALID;
+    if (chunk_bytes == 0 || pre->n_chunks != post->n_chunks) return PCCL_ERR_INVALID;
+    const uint32_t N = topo->N, C = pre->n_chunks;
+    std::vector<char> member(N, 0);
+    for (uint32_t i = 0; i < n_members; ++i) {
+        if (group[i] >= N || member[group[i]]) return PCCL_ERR_INVALID;
+        member[group[i]] = 1;
+    }
+    std::vector<uint64_t> pre_off, post_off;
+    std::vector<uint32_t> pre_n, post_n;
+    int rc = group_pairs(pre, C, N, member, pre_off, pre_n);
+    if (rc) return rc;
+    rc = group_pairs(post, C, N, member, post_off, post_n);
+    if (rc) return rc;
+    bool all_single = true, all_multi_one = true, all_multi_many = true;
+    for (uint32_t c = 0; c < C; ++c) {
+        const uint64_t np = pre_off[c + 1] - pre_off[c], nq = post_off[c + 1] - post_off[c];
+        if (np == 0 || nq == 0) return PCCL_ERR_INVALID;
+        const bool single = np == 1;
+        all_single &= single;
+        all_multi_one &= (!single && nq == 1);
+        all_multi_many &= (!single && nq > 1);
+    }
+    P.topo = topo;
+    P.C = C;
+    P.chunk_bytes = chunk_bytes;
+    P.phases.clear();
+    auto fill = [&](Phase& ph, uint32_t c, uint32_t src, const uint32_t* b, const uint32_t* e) {
+        ph.cond_src[c] = src;
+        for (const uint32_t* p = b; p != e; ++p) if (*p != src) ph.dests.push_back(*p);
+        ph.dest_off[c + 1] = ph.dests.size();
+    };
+    if (all_single) {   // COPY: the one pre-holder is the source
+        P.mode = 0;
+        P.phases.resize(1);
+        Phase& ph = P.phases[0];
+        ph.cond_src.resize(C);
+        ph.dest_off.assign((size_t)C + 1, 0);
+        for (uint32_t c = 0; c < C; ++c)
+            fill(ph, c, pre_n[pre_off[c]], post_n.data() + post_off[c], post_n.data() + post_off[c + 1]);
+    } else if (all_multi_one) {   // REDUCE: broadcast root -> holders on the transposed links
+        P.mode = 1;
+        P.phases.resize(1);
+        Phase& ph = P.phases[0];
+        ph.transposed = true;
+        ph.cond_src.resize(C);
+        ph.dest_off.assign((size_t)C + 1, 0);
+        for (uint32_t c = 0; c < C; ++c)
+            fill(ph, c, post_n[post_off[c]], pre_n.data() + pre_off[c], pre_n.data() + pre_off[c + 1]);
+    } else if (all_multi_many) {   // ALL-REDUCE = reduce to root(c), then copy from root(c)
+        P.mode = 2;
+        P.phases.resize(2);
+        Phase &r = P.phases[0], &g = P.phases[1];
+        r.transposed = true;
+        r.cond_src.resize(C); g.cond_src.resize(C);
+        r.dest_off.assign((size_t)C + 1, 0); g.dest_off.assign((size_t)C + 1, 0);
+        std::vector<uint32_t> I;
+        for (uint32_t c = 0; c < C; ++c) {
+            const uint32_t *pb = pre_n.data() + pre_off[c], *pe = pre_n.data() + pre_off[c + 1];
+            const uint32_t *qb = post_n.data() + post_off[c], *qe = post_n.data() + post_off[c + 1];
+            I.clear();
+            std::set_intersection(pb, pe, qb, qe, std::back_inserter(I));
+            if (I.empty()) I.assign(qb, qe);
+            const uint32_t root = I[c % I.size()];
+            fill(r, c, root, pb, pe);
+            fill(g, c, root, qb, qe);
+        }
+    } else {
+        return PCCL_ERR_UNSUPPORTED;
+    }
+    for (Phase& ph : P.phases) finish_phase(ph, N);
+    return PCCL_OK;
+}
+
+int phase_upload(Phase& ph, uint32_t N) {
+    if (ph.blob) return PCCL_OK;
+    const size_t C = ph.cond_src.size(), ND = ph.dests.size(), NS = ph.sources.size();
+    Carver c;
+    const size_t o_cs = c.take(C * 4), o_d = c.take(ND * 4), o_dc = c.take(ND * 4), o_s = c.take(NS * 4), o_si = c.take((size_t)N * 4);
+    std::vector<unsigned char> h(c.cur ? c.cur : 256, 0);
+    if (C) memcpy(h.data() + o_cs, ph.cond_src.data(), C * 4);
+    if (ND) { memcpy(h.data() + o_d, ph.dests.data(), ND * 4); memcpy(h.data() + o_dc, ph.dchunk.data(), ND * 4); }
+    if (NS) memcpy(h.data() + o_s, ph.sources.data(), NS * 4);
+    if (N) memcpy(h.data() + o_si, ph.sidx.data(), (size_t)N * 4);
+    void* blob = nullptr;
+    int rc = dev_alloc(h.size(), &blob);
+    if (rc) return rc;
+    if (cudaMemcpyAsync(blob, h.data(), h.size(), cudaMemcpyHostToDevice, G.stream) != cudaSuccess ||
+        cudaStreamSynchronize(G.stream) != cudaSuccess) {
+        (void)cudaGetLastError();
+        dev_free(blob);
+        return PCCL_ERR_CUDA;
+    }
+    unsigned char* b = (unsigned char*)blob;
+    ph.blob = blob;
+    ph.d_cond_src = (uint32_t*)(b + o_cs); ph.d_dests = (uint32_t*)(b + o_d); ph.d_dchunk = (uint32_t*)(b + o_dc);
+    ph.d_sources = (uint32_t*)(b + o_s); ph.d_sidx = (uint32_t*)(b + o_si);
+    return PCCL_OK;
+}
+
+}  // namespace
+
+extern "C" int pccl_problem_create(const pccl_topology_t* topo, const uint32_t* group_members,
+                                   uint32_t n_members, const pccl_condition_t* pre,
+                                   const pccl_condition_t* post, uint64_t chunk_bytes,
+                                   pccl_problem_t** out) {
+    if (!out) return PCCL_ERR_INVALID;
+    pccl_problem* P = new (std::nothrow) pccl_problem();
+    if (!P) return PCCL_ERR_NOMEM;
+    int rc;
+    try {
+        rc = normalise(topo, group_members, n_members, pre, post, chunk_bytes, *P);
+    } catch (const std::bad_alloc&) {
+        rc = PCCL_ERR_NOMEM;
+    }
+    if (rc) { delete P; return rc; }
+    *out = P;
+    return PCCL_OK;
+}
+
+extern "C" void pccl_problem_destroy(pccl_problem_t* P) {
+    if (!P) return;
+    for (Phase& ph : P->phases) dev_free(ph.blob);
+    delete P;
+}
+
+extern "C" int pccl_problem_upload(pccl_problem_t* P) {
+    if (!P) return PCCL_ERR_INVALID;
+    if (P->uploaded) return PCCL_OK;
+    int rc = topo_upload(const_cast<pccl_topology*>(P->topo));
+    if (rc) return rc;
+    try {
+        for (Phase& ph : P->phases) { rc = phase_upload(ph, P->topo->N); if (rc) return rc; }
+    } catch (const std::bad_alloc&) {
+        return PCCL_ERR_NOMEM;
+    }
+    P->uploaded = true;
+    return PCCL_OK;
+}
+
+extern "C" int pccl_problem_mode(const pccl_problem_t* P) { return P ? P->mode : PCCL_ERR_INVALID; }
+extern "C" uint32_t pccl_problem_n_chunks(const pccl_problem_t* P) { return P ? P->C : 0; }
+extern "C" int64_t pccl_problem_condition(const pccl_problem_t* P, uint32_t phase, uint32_t chunk,
+                                          uint32_t* src, uint32_t* dests, uint64_t cap) {
+    if (!P || phase >= P->phases.size() || chunk >= P->C) return PCCL_ERR_INVALID;
+    const Phase& ph = P->phases[phase];
+    if (src) *src = ph.cond_src[chunk];
+    const uint64_t b = ph.dest_off[chunk], e = ph.dest_off[chunk + 1];
+    for (uint64_t i = b; i < e && (i - b) < cap && dests; ++i) dests[i - b] = ph.dests[i];
+    return (int64_t)(e - b);
+}
+
+// -----------------------------------------------------------------------------------------
+// one phase on the device: steps A..E (setup kernels + the persistent event loop)
+// -----------------------------------------------------------------------------------------
+namespace {
+
+struct Work {   // device workspace of one phase
+    void* blob = nullptr;
+    uint64_t *w = nullptr, *D = nullptr, *have = nullptr, *wants = nullptr, *free_t = nullptr, *matchbits = nullptr;
+    uint32_t *wants_cnt = nullptr, *inflight = nullptr, *have_epoch = nullptr, *empty_epoch = nullptr;
+    LoopCtrl* ctrl = nullptr;
+    uint32_t Wp = 0, S = 0, nLw = 0;
+    size_t zero_off = 0, zero_bytes = 0;   // have + wants + wants_cnt + ctrl are cleared per run
+};
+
+int work_alloc(const pccl_problem& P, Work& W) {
+    const size_t N = P.topo->N, L = P.topo->L, C = P.C;
+    size_t max_sources = 0;   // one workspace serves every phase
+    for (const Phase& ph : P.phases) max_sources = std::max(max_sources, ph.sources.size());
+    const size_t words = (C + 63) / 64;
+    W.Wp = (uint32_t)std::max<size_t>(16, align_up(words, 16));   // rows are multiples of 128 bytes
+    W.S = (W.Wp / 2 + SEG_U4 - 1) / SEG_U4;
+    W.nLw = (uint32_t)((L + 63) / 64);
+    if ((size_t)NB * W.S * 4 > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+    Carver c;
+    const size_t o_w = c.take(L * 8), o_D = c.take(max_sources * N * 8), o_free = c.take(L * 8),
+                 o_mb = c.take((size_t)2 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4);
+    W.zero_off = c.cur;
+    const size_t o_have = c.take(N * W.Wp * 8), o_wants = c.take(N * W.Wp * 8), o_wc = c.take(N * 4), o_ctrl = c.take(sizeof(LoopCtrl));
+    W.zero_bytes = c.cur - W.zero_off;
+    int rc = dev_alloc(c.cur, &W.blob);
+    if (rc) return rc;
+    unsigned char* b = (unsigned char*)W.blob;
+    W.w = (uint64_t*)(b + o_w); W.D = (uint64_t*)(b + o_D); W.free_t = (uint64_t*)(b + o_free);
+    W.matchbits = (uint64_t*)(b + o_mb); W.inflight = (uint32_t*)(b + o_inf); W.have_epoch = (uint32_t*)(b + o_he);
+    W.empty_epoch = (uint32_t*)(b + o_ee); W.have = (uint64_t*)(b + o_have); W.wants = (uint64_t*)(b + o_wants);
+    W.wants_cnt = (uint32_t*)(b + o_wc); W.ctrl = (LoopCtrl*)(b + o_ctrl);
+    return PCCL_OK;
+}
+
+struct PhaseView {   // link tables in the synthesized direction
+    const uint32_t *esrc, *edst, *in_off, *in_link;
+};
+PhaseView view_of(const pccl_topology* t, bool transposed) {
+    if (!transposed) return {t->d_src, t->d_dst, t->d_in_off, t->d_in_link};
+    return {t->d_dst, t->d_src, t->d_out_off, t->d_out_link};
+}
+
+// steps A..C; on return the wants total is in *M (synchronises the stream)
+int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint64_t* M) {
+    const pccl_topology* t = P.topo;
+    const uint32_t N = t->N, L = t->L, C = P.C;
+    const PhaseView pv = view_of(t, ph.transposed);
+    const uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
+    cudaStream_t st = G.stream;
+    CU(cudaMemsetAsync((unsigned char*)W.blob + W.zero_off, 0, W.zero_bytes, st));
+    if (L) k_link_cost<<<(L + 255) / 256, 256, 0, st>>>(t->d_alpha, t->d_bpp, L, P.chunk_bytes, W.w);
+    const uint32_t NS = (uint32_t)ph.sources.size();
+    if (NS) {
+        const size_t smem = (size_t)N * 8;
+        if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+        if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        k_distances<<<NS, 256, smem, st>>>(pv.esrc, pv.edst, W.w, N, L, ph.d_sources, W.D);
+    }
+    if (C) k_have<<<(C + 255) / 256, 256, 0, st>>>(ph.d_cond_src, C, W.Wp, W.have);
+    const uint64_t ND = ph.dests.size();
+    if (ND) {
+        k_wants<<<(unsigned)((ND + 127) / 128), 128, 0, st>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, ND, pv.esrc, pv.in_off,
+                                                          pv.in_link, W.w, ph.d_sidx, W.D, N, W.Wp, k0, k1, W.wants,
+                                                          W.wants_cnt, &W.ctrl->err);
+    }
+    k_sum_u32<<<1, 1024, 0, st>>>(W.wants_cnt, N, &W.ctrl->wants_total);
+    CU(cudaGetLastError());
+    LoopCtrl* mb = (LoopCtrl*)G.mailbox;
+    CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (mb->err & 1u) return PCCL_ERR_UNREACHABLE;
+    if (mb->err) return PCCL_ERR_INTERNAL;
+    *M = mb->wants_total;
+    return PCCL_OK;
+}
+
+struct LoopResult {
+    uint64_t total, tmax, events, rows, links, slow;
+    uint32_t grid;
+};
+
+// steps D..E: the event loop; records go to `out` (capacity M) in canonical order
+int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint32_t flags, Rec* out,
+               uint64_t t_offset, LoopResult* res) {
+    const pccl_topology* t = P.topo;
+    const PhaseView pv = view_of(t, ph.transposed);
+    LoopArgs a;
+    a.N = t->N; a.L = t->L; a.Wp = W.Wp; a.S = W.S; a.nLw = W.nLw; a.flags = flags;
+    a.k0 = (uint32_t)(seed & 0xFFFFFFFFull); a.k1 = (uint32_t)(seed >> 32);
+    a.esrc = pv.esrc; a.edst = pv.edst; a.psrc = t->d_src; a.pdst = t->d_dst;
+    a.in_off = pv.in_off; a.in_link = pv.in_link; a.w = W.w; a.have = W.have; a.wants = W.wants;
+    a.wants_cnt = W.wants_cnt; a.free_t = W.free_t; a.inflight = W.inflight; a.have_epoch = W.have_epoch;
+    a.empty_epoch = W.empty_epoch; a.matchbits = W.matchbits; a.ctrl = W.ctrl; a.out = out; a.t_offset = t_offset;
+    cudaStream_t st = G.stream;
+    const uint32_t n_init = std::max(std::max(a.L, a.N), std::max(2 * a.nLw, 1u));
+    k_loop_init<<<(n_init + 255) / 256, 256, 0, st>>>(a);
+    const size_t smem = (size_t)NB * W.S * 4;
+    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_loop, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_loop, LOOP_THREADS, smem));
+    if (occ < 1) return PCCL_ERR_CUDA;
+    const uint32_t max_grid = (uint32_t)occ * (uint32_t)G.sm_count;
+    const uint32_t want = std::max(std::max(a.N, (a.L + LOOP_THREADS - 1) / LOOP_THREADS), 1u);
+    const uint32_t grid = std::min(max_grid, want);
+    void* args[] = {(void*)&a};
+    CU(cudaLaunchCooperativeKernel((const void*)k_loop, dim3(grid), dim3(LOOP_THREADS), args, smem, st));
+    LoopCtrl* mb = (LoopCtrl*)G.mailbox;
+    CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (mb->err) return PCCL_ERR_INTERNAL;
+    res->total = mb->total; res->tmax = mb->tmax; res->events = mb->events;
+    res->rows = mb->rows_scanned; res->links = mb->links_scanned; res->slow = mb->slow_picks;
+    res->grid = grid;
+    return PCCL_OK;
+}
+
+// a9 for reductions: raw (transposed-broadcast) records -> reversed, sorted by (t_start, link), into out
+int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out) {
+    if (M == 0) return PCCL_OK;
+    cudaStream_t st = G.stream;
+    uint32_t link_bits = 1;
+    while ((1ull << link_bits) < (uint64_t)L) ++link_bits;
+    uint32_t t_bits = 1;
+    while (t_bits < 64 && (T >> t_bits)) ++t_bits;
+    if (t_bits + link_bits > 64 || M > 0xFFFFFFFFull) return PCCL_ERR_UNSUPPORTED;
+    const uint32_t nblocks = (uint32_t)((M + SORT_TILE - 1) / SORT_TILE);
+    Carver c;
+    const size_t o_k0 = c.take(M * 8), o_k1 = c.take(M * 8), o_v0 = c.take(M * 4), o_v1 = c.take(M * 4),
+                 o_h = c.take((size_t)256 * nblocks * 4);
+    void* blob = nullptr;
+    int rc = dev_alloc(c.cur, &blob);
+    if (rc) return rc;
+    unsigned char* b = (unsigned char*)blob;
+    uint64_t* keys[2] = {(uint64_t*)(b + o_k0), (uint64_t*)(b + o_k1)};
+    uint32_t* vals[2] = {(uint32_t*)(b + o_v0), (uint32_t*)(b + o_v1)};
+    uint32_t* ghist = (uint32_t*)(b + o_h);
+    const unsigned g256 = (unsigned)((M + 255) / 256);
+    k_reverse_keys<<<g256, 256, 0, st>>>(raw, M, T, link_bits, keys[0], vals[0]);
+    int cur = 0;
+    for (uint32_t shift = 0; shift < t_bits + link_bits; shift += 8) {
+        k_sort_hist<<<nblocks, SORT_THREADS, 0, st>>>(keys[cur], M, shift, ghist, nblocks);
+        k_sort_scan<<<1, 1024, 0, st>>>(ghist, (uint64_t)256 * nblocks);
+        k_sort_scatter<<<nblocks, SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], M, shift, ghist, nblocks);
+        cur ^= 1;
+    }
+    k_gather_shift<<<g256, 256, 0, st>>>(raw, vals[cur], M, 0, out);
+    cudaError_t e = cudaGetLastError();
+    dev_free(blob);   // stream-ordered: freed after the kernels above
+    return e == cudaSuccess ? PCCL_OK : PCCL_ERR_CUDA;
+}
+
+struct Timer {
+    cudaEvent_t a = nullptr, b = nullptr;
+    bool on = false;
+    float acc = 0.f;
+    void init(bool enable) {
+        on = enable && cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess;
+    }
+    void start() { if (on) cudaEventRecord(a, G.stream); }
+    void stop() {   // call after the stream was synchronised or right before a sync
+        if (!on) return;
+        cudaEventRecord(b, G.stream);
+        cudaEventSynchronize(b);
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) acc += ms;
+    }
+    ~Timer() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+};
+
+}  // namespace
+
+extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_t flags, pccl_schedule_t** out) {
+    if (!P || !out) return PCCL_ERR_INVALID;
+    int rc = pccl_problem_upload(P);
+    if (rc) return rc;
+    pccl_schedule* S = new (std::nothrow) pccl_schedule();
+    if (!S) return PCCL_ERR_NOMEM;
+    memset(&S->stats, 0, sizeof(S->stats));
+    S->stats.mode = (uint32_t)P->mode;
+    Timer t_setup, t_loop, t_emit;
+    const bool timed = (flags & PCCL_FLAG_TIME_LOOP) != 0;
+    t_setup.init(timed); t_loop.init(timed); t_emit.init(timed);
+
+    Work W;
+    Rec* out_recs = nullptr;   // final records
+    Rec* raw = nullptr;        // raw records of a reduce phase
+    Rec* stage1 = nullptr;     // sorted phase-1 records of an all-reduce
+    uint64_t M1 = 0, T1 = 0;
+    auto fail = [&](int code) {
+        dev_free(W.blob); dev_free(out_recs); dev_free(raw); dev_free(stage1);
+        if (cudaStreamSynchronize(G.stream) != cudaSuccess) (void)cudaGetLastError();
+        delete S;
+        return code;
+    };
+    const uint32_t L = P->topo->L;
+    for (size_t pi = 0; pi < P->phases.size(); ++pi) {
+        const Phase& ph = P->phases[pi];
+        const bool last = pi + 1 == P->phases.size();
+        if (!W.blob) { rc = work_alloc(*P, W); if (rc) return fail(rc); }
+        uint64_t M = 0;
+        t_setup.start();
+        rc = phase_setup(*P, ph, W, seed, &M);
+        if (rc) return fail(rc);
+        t_setup.stop();
+        S->stats.wants_total += M;
+        LoopResult lr;
+        if (ph.transposed) {
+            rc = dev_alloc(M * sizeof(Rec), (void**)&raw);
+            if (rc) return fail(rc);
+            t_loop.start();
+            rc = phase_loop(*P, ph, W, seed, flags, raw, 0, &lr);
+            if (rc) return fail(rc);
+            t_loop.stop();
+            if (lr.total != M) return fail(PCCL_ERR_INTERNAL);
+            Rec* dst = nullptr;
+            rc = dev_alloc(M * sizeof(Rec), (void**)&dst);
+            if (rc) return fail(rc);
+            if (last) out_recs = dst; else stage1 = dst;
+            t_emit.start();
+            rc = reverse_sorted(raw, M, lr.tmax, L, dst);
+            if (rc) return fail(rc);
+            t_emit.stop();
+            dev_free(raw);
+            raw = nullptr;
+            M1 = M; T1 = lr.tmax;
+            if (last) { S->M = M; S->T = lr.tmax; }
+            S->stats.time_phase1_ps = lr.tmax;
+        } else {
+            const uint64_t base = (pi == 0) ? 0 : M1;
+            const uint64_t toff = (pi == 0) ? 0 : T1;
+            rc = dev_alloc((base + M) * sizeof(Rec), (void**)&out_recs);
+            if (rc) return fail(rc);
+            if (base) {
+                if (cudaMemcpyAsync(out_recs, stage1, base * sizeof(Rec), cudaMemcpyDeviceToDevice, G.stream) != cudaSuccess) {
+                    (void)cudaGetLastError();
+                    return fail(PCCL_ERR_CUDA);
+                }
+            }
+            t_loop.start();
+            rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, toff, &lr);
+            if (rc) return fail(rc);
+            t_loop.stop();
+            if (lr.total != M) return fail(PCCL_ERR_INTERNAL);
+            S->M = base + M;
+            S->T = toff + lr.tmax;
+        }
+        S->stats.events += lr.events;
+        S->stats.rows_scanned += lr.rows;
+        S->stats.links_scanned += lr.links;
+        S->stats.slow_picks += lr.slow;
+        S->stats.grid_blocks = lr.grid;
+        S->stats.row_bytes = (uint64_t)W.Wp * 8;
+    }
+    dev_free(W.blob); W.blob = nullptr;
+    dev_free(stage1); stage1 = nullptr;
+    S->d_recs = out_recs;
+    S->stats.loop_ms = t_loop.acc; S->stats.setup_ms = t_setup.acc; S->stats.emit_ms = t_emit.acc;
+    if (!(flags & PCCL_FLAG_KEEP_ON_DEVICE)) {
+        if (S->M && !pccl_schedule_transfers(S)) { pccl_schedule_destroy(S); return PCCL_ERR_CUDA; }
+    }
+    *out = S;
+    return PCCL_OK;
+}
+
+extern "C" int pccl_synthesize(const pccl_topology_t* topo, const uint32_t* group_members, uint32_t n_members,
+                               const pccl_condition_t* pre, const pccl_condition_t* post, uint64_t chunk_bytes,
+                               uint64_t seed, pccl_schedule_t** out) {
+    if (!out) return PCCL_ERR_INVALID;
+    pccl_problem_t* P = nullptr;
+    int rc = pccl_problem_create(topo, group_members, n_members, pre, post, chunk_bytes, &P);
+    if (rc) return rc;
+    pccl_schedule_t* S = nullptr;
+    rc = pccl_problem_synthesize(P, seed, 0, &S);
+    pccl_problem_destroy(P);
+    if (rc) return rc;
+    *out = S;
+    return PCCL_OK;
+}
+
+// -----------------------------------------------------------------------------------------
+// schedule accessors
+// -----------------------------------------------------------------------------------------
+extern "C" uint64_t pccl_schedule_time(const pccl_schedule_t* s) { return s ? s->T : 0; }
+extern "C" uint64_t pccl_schedule_size(const pccl_schedule_t* s) { return s ? s->M : 0; }
+extern "C" const pccl_transfer_t* pccl_schedule_transfers(pccl_schedule_t* s) {
+    if (!s || s->M == 0) return nullptr;
+    if (!s->downloaded) {
+        if (!s->d_recs) return nullptr;
+        const size_t bytes = s->M * sizeof(Rec);
+        if (!s->h_recs) { s->h_recs = pinned_get(bytes); s->h_bytes = bytes; }
+        if (!s->h_recs) return nullptr;
+        if (cudaMemcpyAsync(s->h_recs, s->d_recs, bytes, cudaMemcpyDeviceToHost, G.stream) != cudaSuccess ||
+            cudaStreamSynchronize(G.stream) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return nullptr;
+        }
+        s->downloaded = true;
+    }
+    return (const pccl_transfer_t*)s->h_recs;
+}
+extern "C" const pccl_transfer_t* pccl_schedule_transfers_device(const pccl_schedule_t* s) {
+    return s ? (const pccl_transfer_t*)s->d_recs : nullptr;
+}
+extern "C" void pccl_schedule_destroy(pccl_schedule_t* s) {
+    if (!s) return;
+    dev_free(s->d_recs);
+    pinned_put(s->h_recs, s->h_bytes);
+    delete s;
+}
+extern "C" int pccl_schedule_stats(const pccl_schedule_t* s, pccl_stats_t* out) {
+    if (!s || !out) return PCCL_ERR_INVALID;
+    *out = s->stats;
+    return PCCL_OK;
+}
+
+// -----------------------------------------------------------------------------------------
+// single rows for parity tests
+// -----------------------------------------------------------------------------------------
+extern "C" int pccl_device_philox(const uint32_t* ctr, uint64_t n, const uint32_t key[2], uint32_t* out) {
+    if ((n && (!ctr || !out)) || !key) return PCCL_ERR_INVALID;
+    if (n == 0) return PCCL_OK;
+    int rc = ensure_device();
+    if (rc) return rc;
+    void* d = nullptr;
+    rc = dev_alloc(n * 32, &d);
+    if (rc) return rc;
+    uint32_t* dc = (uint32_t*)d;
+    uint32_t* dout = dc + 4 * n;
+    cudaStream_t st = G.stream;
+    cudaError_t e = cudaMemcpyAsync(dc, ctr, n * 16, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        k_philox<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(dc, n, key[0], key[1], dout);
+        e = cudaMemcpyAsync(out, dout, n * 16, cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    dev_free(d);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return PCCL_ERR_CUDA; }
+    return PCCL_OK;
+}
+
+extern "C" int pccl_device_link_costs(pccl_topology_t* t, uint64_t chunk_bytes, uint64_t* out) {
+    if (!t || !out || chunk_bytes == 0) return PCCL_ERR_INVALID;
+    int rc = topo_upload(t);
+    if (rc) return rc;
+    if (t->L == 0) return PCCL_OK;
+    void* d = nullptr;
+    rc = dev_alloc((size_t)t->L * 8, &d);
+    if (rc) return rc;
+    cudaStream_t st = G.stream;
+    k_link_cost<<<(t->L + 255) / 256, 256, 0, st>>>(t->d_alpha, t->d_bpp, t->L, chunk_bytes, (uint64_t*)d);
+    cudaError_t e = cudaMemcpyAsync(out, d, (size_t)t->L * 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    dev_free(d);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return PCCL_ERR_CUDA; }
+    return PCCL_OK;
+}
+
+extern "C" int pccl_device_distances(pccl_topology_t* t, uint64_t chunk_bytes, uint32_t src, int transposed,
+                                     uint64_t* out) {
+    if (!t || !out || chunk_bytes == 0 || src >= t->N) return PCCL_ERR_INVALID;
+    int rc = topo_upload(t);
+    if (rc) return rc;
+    const size_t N = t->N, L = t->L;
+    if (N * 8 > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+    Carver c;
+    const size_t o_w = c.take(L * 8), o_D = c.take(N * 8), o_s = c.take(4);
+    void* d = nullptr;
+    rc = dev_alloc(c.cur, &d);
+    if (rc) return rc;
+    unsigned char* b = (unsigned char*)d;
+    cudaStream_t st = G.stream;
+    const PhaseView pv = view_of(t, transposed != 0);
+    cudaError_t e = cudaMemcpyAsync(b + o_s, &src, 4, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && N * 8 > 48 * 1024)
+        e = cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(N * 8));
+    if (e == cudaSuccess) {
+        if (L) k_link_cost<<<(unsigned)((L + 255) / 256), 256, 0, st>>>(t->d_alpha, t->d_bpp, (uint32_t)L, chunk_bytes, (uint64_t*)(b + o_w));
+        k_distances<<<1, 256, N * 8, st>>>(pv.esrc, pv.edst, (uint64_t*)(b + o_w), (uint32_t)N, (uint32_t)L, (uint32_t*)(b + o_s), (uint64_t*)(b + o_D));
+        e = cudaMemcpyAsync(out, b + o_D, N * 8, cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    dev_free(d);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return PCCL_ERR_CUDA; }
+    return PCCL_OK;
+}
+
+extern "C" int64_t pccl_device_wants(pccl_problem_t* P, uint32_t phase, uint64_t seed, pccl_pair_t* out, uint64_t cap) {
+    if (!P || phase >= P->phases.size() || (cap && !out)) return PCCL_ERR_INVALID;
+    int rc = pccl_problem_upload(P);
+    if (rc) return rc;
+    const Phase& ph = P->phases[phase];
+    Work W;
+    rc = work_alloc(*P, W);
+    if (rc) return rc;
+    uint64_t M = 0;
+    rc = phase_setup(*P, ph, W, seed, &M);
+    if (rc) { dev_free(W.blob); return rc; }
+    const uint32_t N = P->topo->N;
+    // node bases from wants_cnt (host exclusive scan; accessor only)
+    std::vector<uint32_t> wc(N);
+    std::vector<uint64_t> base((size_t)N + 1, 0);
+    cudaStream_t st = G.stream;
+    cudaError_t e = cudaMemcpyAsync(wc.data(), W.wants_cnt, (size_t)N * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); dev_free(W.blob); return PCCL_ERR_CUDA; }
+    for (uint32_t v = 0; v < N; ++v) base[v + 1] = base[v] + wc[v];
+    const uint64_t n_out = std::min<uint64_t>(M, cap);
+    void* d = nullptr;
+    Carver c;
+    const size_t o_b = c.take(((size_t)N + 1) * 8), o_p = c.take(n_out * 8);
+    rc = dev_alloc(c.cur, &d);
+    if (rc) { dev_free(W.blob); return rc; }
+    unsigned char* b = (unsigned char*)d;
+    e = cudaMemcpyAsync(b + o_b, base.data(), ((size_t)N + 1) * 8, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && N) {
+        k_wants_pairs<<<(N + 3) / 4, 128, 0, st>>>(W.wants, N, W.Wp, (const uint64_t*)(b + o_b), (uint32_t*)(b + o_p), n_out);
+        if (n_out) e = cudaMemcpyAsync(out, b + o_p, n_out * 8, cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    dev_free(d);
+    dev_free(W.blob);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return PCCL_ERR_CUDA; }
+    return (int64_t)M;
+}

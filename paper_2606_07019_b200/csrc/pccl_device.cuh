@@ -1,0 +1,704 @@
+// =========================================================================================
+// pccl_device.cuh -- device code of the link-chunk matching synthesizer (sm_100a).
+//
+// Rows of DESIGN.md's hot-path table implemented here:
+//   a0 k_link_cost      alpha-beta link cost
+//   a1 k_distances      per-source shortest alpha-beta distances    (Alg. 3)
+//   a2 k_have/k_wants   holdings + thin-relay-tree wants bitmaps
+//   a3 loop phase P1    arrivals
+//   a4 loop phase P2    active in-link compaction per destination   (Alg. 1)
+//   a5 loop phase P2    candidate bitmap  have[src] & wants[dst]
+//   a6 loop phase P2    Philox-keyed k-th-candidate pick
+//   a7 loop phase P2    serial conflict resolve among in-links of one destination
+//   a8 loop phase P2/P1 free-time advance, next-event min, ordered emit
+//   a9 k_reverse + radix sort   reversal for reductions
+//
+// Nothing here is shared with oracle/ (the oracle is set-based C++ with its own Philox).
+// =========================================================================================
+#pragma once
+#include <cooperative_groups.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace cg = cooperative_groups;
+
+namespace pccl {
+
+constexpr uint64_t T_INF = 0xFFFFFFFFFFFFFFFFull;
+constexpr uint32_t NONE32 = 0xFFFFFFFFu;
+constexpr int LOOP_THREADS = 512;  // threads per CTA of the event-loop kernel
+constexpr int NB = 8;              // in-links of one destination counted in one sweep
+constexpr int SEG_U4 = 32;         // uint4 per segment (one warp-wide load) = 64 words = 4096 chunks
+
+struct Rec {  // == pccl_transfer_t
+    uint32_t chunk, src, dst, link;
+    uint64_t t_start, t_end;
+};
+static_assert(sizeof(Rec) == 32, "layout");
+
+// ---- cache-bypassing accessors: all mutable state is read from / written to L2 ------------
+// (the loop kernel is persistent, so L1 lines could otherwise outlive a grid barrier)
+__device__ __forceinline__ uint64_t ldcg64(const uint64_t* p) { return __ldcg((const unsigned long long*)p); }
+__device__ __forceinline__ uint32_t ldcg32(const uint32_t* p) { return __ldcg(p); }
+__device__ __forceinline__ uint4 ldcg128(const uint4* p) { return __ldcg(p); }
+__device__ __forceinline__ void stcg64(uint64_t* p, uint64_t v) { __stcg((unsigned long long*)p, (unsigned long long)v); }
+__device__ __forceinline__ void stcg32(uint32_t* p, uint32_t v) { __stcg(p, v); }
+
+__device__ __forceinline__ int popc128(uint4 a) { return __popc(a.x) + __popc(a.y) + __popc(a.z) + __popc(a.w); }
+__device__ __forceinline__ uint4 and128(uint4 a, uint4 b) { return make_uint4(a.x & b.x, a.y & b.y, a.z & b.z, a.w & b.w); }
+
+// ---- a6: Philox4x32-10 (Salmon et al., SC'11), first output word only ----------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t out[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ k0;
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ k1;
+        c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+__device__ __forceinline__ uint32_t philox_draw(uint32_t a, uint32_t b, uint32_t c, uint32_t tag,
+                                                uint32_t k0, uint32_t k1) {
+    uint32_t o[4];
+    philox4x32_10(a, b, c, tag, k0, k1, o);
+    return o[0];
+}
+
+__global__ void k_philox(const uint32_t* ctr, uint64_t n, uint32_t k0, uint32_t k1, uint32_t* out) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t o[4];
+    philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], k0, k1, o);
+    out[4 * i] = o[0]; out[4 * i + 1] = o[1]; out[4 * i + 2] = o[2]; out[4 * i + 3] = o[3];
+}
+
+// ---- a0: link cost ---------------------------------------------------------------------------
+__global__ void k_link_cost(const uint64_t* __restrict__ alpha, const uint64_t* __restrict__ bpp,
+                            uint32_t L, uint64_t chunk_bytes, uint64_t* __restrict__ w) {
+    const uint32_t l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= L) return;
+    const uint64_t b = bpp[l];
+    w[l] = alpha[l] + chunk_bytes / b + (chunk_bytes % b != 0);
+}
+
+// ---- a1: shortest alpha-beta distances, one CTA per distinct source (Bellman-Ford in smem) ---
+// esrc/edst: link endpoints in the direction being synthesized (swapped for the transposed run).
+__global__ void k_distances(const uint32_t* __restrict__ esrc, const uint32_t* __restrict__ edst,
+                            const uint64_t* __restrict__ w, uint32_t N, uint32_t L,
+                            const uint32_t* __restrict__ sources, uint64_t* __restrict__ D) {
+    extern __shared__ unsigned long long sdist[];
+    __shared__ int s_changed;
+    const uint32_t s = sources[blockIdx.x];
+    for (uint32_t v = threadIdx.x; v < N; v += blockDim.x) sdist[v] = (v == s) ? 0ull : T_INF;
+    __syncthreads();
+    for (;;) {
+        if (threadIdx.x == 0) s_changed = 0;
+        __syncthreads();
+        int changed = 0;
+        for (uint32_t l = threadIdx.x; l < L; l += blockDim.x) {
+            const unsigned long long du = ((volatile unsigned long long*)sdist)[esrc[l]];
+            if (du == T_INF) continue;
+            const unsigned long long nd = du + w[l];
+            const uint32_t v = edst[l];
+            if (nd < ((volatile unsigned long long*)sdist)[v]) {
+                atomicMin(&sdist[v], nd);
+                changed = 1;
+            }
+        }
+        if (changed) s_changed = 1;
+        __syncthreads();
+        const int any = s_changed;
+        __syncthreads();
+        if (!any) break;
+    }
+    uint64_t* row = D + (size_t)blockIdx.x * N;
+    for (uint32_t v = threadIdx.x; v < N; v += blockDim.x) row[v] = sdist[v];
+}
+
+// ---- a2: holdings ------------------------------------------------------------------------------
+__global__ void k_have(const uint32_t* __restrict__ cond_src, uint32_t C, uint32_t Wp,
+                       uint64_t* __restrict__ have) {
+    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= C) return;
+    atomicOr((unsigned long long*)&have[(size_t)cond_src[c] * Wp + (c >> 6)], 1ull << (c & 63));
+}
+
+// ---- a2: wants = thin relay tree, one thread per (chunk, dest) pair ----------------------------
+// Walk from the dest towards the source; at node `cur` the predecessor is the j-th tight
+// in-link (ascending link id), j = (Philox(c, cur, 0, 1)[0] * |tight|) >> 32.  The choice is
+// keyed on (c, cur) only, so walks of one chunk merge into a tree whatever order they run in;
+// a walk stops at the first node already marked for its chunk.
+__global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* __restrict__ dests,
+                        const uint32_t* __restrict__ dchunk, uint64_t n_pairs,
+                        const uint32_t* __restrict__ esrc, const uint32_t* __restrict__ in_off,
+                        const uint32_t* __restrict__ in_link, const uint64_t* __restrict__ w,
+                        const uint32_t* __restrict__ sidx, const uint64_t* __restrict__ D, uint32_t N,
+                        uint32_t Wp, uint32_t k0, uint32_t k1, uint64_t* __restrict__ wants,
+                        uint32_t* __restrict__ wants_cnt, uint32_t* __restrict__ err) {
+    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_pairs) return;
+    const uint32_t c = dchunk[p];
+    const uint32_t s = cond_src[c];
+    const uint64_t* Ds = D + (size_t)sidx[s] * N;
+    uint32_t cur = dests[p];
+    if (Ds[cur] == T_INF) { atomicOr(err, 1u); return; }
+    const unsigned long long bit = 1ull << (c & 63);
+    while (cur != s) {
+        const unsigned long long old = atomicOr((unsigned long long*)&wants[(size_t)cur * Wp + (c >> 6)], bit);
+        if (old & bit) break;
+        atomicAdd(&wants_cnt[cur], 1u);
+        const uint64_t dcur = Ds[cur];
+        const uint32_t e0 = in_off[cur], e1 = in_off[cur + 1];
+        uint32_t ntight = 0;
+        for (uint32_t e = e0; e < e1; ++e) {
+            const uint32_t l = in_link[e];
+            const uint64_t du = Ds[esrc[l]];
+            ntight += (du != T_INF && du + w[l] == dcur);
+        }
+        if (ntight == 0) { atomicOr(err, 2u); return; }
+        uint32_t j = __umulhi(philox_draw(c, cur, 0u, 1u, k0, k1), ntight);
+        uint32_t nxt = cur;
+        for (uint32_t e = e0; e < e1; ++e) {
+            const uint32_t l = in_link[e];
+            const uint32_t u = esrc[l];
+            const uint64_t du = Ds[u];
+            if (du != T_INF && du + w[l] == dcur) {
+                if (j == 0) { nxt = u; break; }
+                --j;
+            }
+        }
+        cur = nxt;
+    }
+}
+
+// sum of wants_cnt -> ctrl (one block)
+__global__ void k_sum_u32(const uint32_t* __restrict__ x, uint32_t n, unsigned long long* out) {
+    __shared__ unsigned long long s[32];
+    unsigned long long acc = 0;
+    for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) acc += x[i];
+    for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        acc = (threadIdx.x < (blockDim.x >> 5)) ? s[threadIdx.x] : 0;
+        for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+        if (threadIdx.x == 0) *out = acc;
+    }
+}
+
+// wants bitmap -> (node, chunk) pairs in (node, chunk) order (parity-test accessor for row a2)
+__global__ void k_wants_pairs(const uint64_t* __restrict__ wants, uint32_t N, uint32_t Wp,
+                              const uint64_t* __restrict__ node_base, uint32_t* __restrict__ out_pairs,
+                              uint64_t cap) {
+    // one warp per node, sequential over the row
+    const uint32_t v = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (v >= N) return;
+    const uint32_t lane = threadIdx.x & 31;
+    uint64_t pos = node_base[v];
+    for (uint32_t wb = 0; wb < Wp; wb += 32) {
+        const uint32_t wi = wb + lane;
+        const uint64_t word = (wi < Wp) ? wants[(size_t)v * Wp + wi] : 0ull;
+        const uint32_t pc = __popcll(word);
+        uint32_t incl = pc;
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if ((int)lane >= o) incl += y;
+        }
+        uint64_t my = pos + incl - pc;
+        uint64_t x = word;
+        while (x) {
+            const int b = __ffsll((long long)x) - 1;
+            x &= x - 1;
+            if (my < cap) { out_pairs[2 * my] = v; out_pairs[2 * my + 1] = wi * 64 + b; }
+            ++my;
+        }
+        pos += __shfl_sync(0xFFFFFFFFu, incl, 31);
+    }
+}
+
+// ==================================================================================================
+//  The event loop: one persistent cooperative kernel, two grid barriers per event time.
+// ==================================================================================================
+struct LoopCtrl {                 // device-resident control block (zeroed / initialised by k_loop_init)
+    unsigned long long tnext[3];  // ring: next event time candidates
+    unsigned long long total;     // transfers emitted so far
+    unsigned long long tmax;      // max t_end
+    unsigned long long events;    // event times processed
+    unsigned long long rows_scanned;
+    unsigned long long links_scanned;
+    unsigned long long slow_picks;
+    unsigned long long wants_total;
+    uint32_t err;
+    uint32_t pad;
+};
+
+struct LoopArgs {
+    uint32_t N, L, Wp, S;   // nodes, links, words per padded row, segments per row
+    uint32_t nLw;           // words of the per-event matched-link bitmap
+    uint32_t flags;
+    uint32_t k0, k1;        // Philox key
+    const uint32_t* esrc;   // link endpoints in the synthesized direction
+    const uint32_t* edst;
+    const uint32_t* psrc;   // physical endpoints (what a record reports)
+    const uint32_t* pdst;
+    const uint32_t* in_off; // per-destination in-link table, ascending link id
+    const uint32_t* in_link;
+    const uint64_t* w;
+    uint64_t* have;
+    uint64_t* wants;
+    uint32_t* wants_cnt;
+    uint64_t* free_t;
+    uint32_t* inflight;
+    uint32_t* have_epoch;
+    uint32_t* empty_epoch;
+    uint64_t* matchbits;    // [2][nLw]
+    LoopCtrl* ctrl;
+    Rec* out;
+    uint64_t t_offset;      // added to the emitted times (phase 2 of all-reduce)
+};
+
+__global__ void k_loop_init(LoopArgs a) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < a.L) {
+        a.free_t[i] = 0;
+        a.inflight[i] = NONE32;
+        a.empty_epoch[i] = 0;
+    }
+    if (i < a.N) a.have_epoch[i] = 0;
+    if (i < 2 * a.nLw) a.matchbits[i] = 0;
+    if (i == 0) {
+        a.ctrl->tnext[0] = 0;
+        a.ctrl->tnext[1] = T_INF;
+        a.ctrl->tnext[2] = T_INF;
+        a.ctrl->total = 0;
+        a.ctrl->tmax = 0;
+        a.ctrl->events = 0;
+        a.ctrl->rows_scanned = 0;
+        a.ctrl->links_scanned = 0;
+        a.ctrl->slow_picks = 0;
+    }
+}
+
+__device__ __forceinline__ uint32_t warp_incl_scan(uint32_t x, uint32_t lane) {
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, x, o);
+        if ((int)lane >= o) x += y;
+    }
+    return x;
+}
+
+// position of the k-th (0-based) set bit of a 128-bit value in ascending bit order
+__device__ __forceinline__ uint32_t kth_bit128(uint4 m, uint32_t k) {
+    uint32_t part[4] = {m.x, m.y, m.z, m.w};
+    uint32_t base = 0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t pc = __popc(part[i]);
+        if (k < pc) return base + __fns(part[i], 0, (int)k + 1);
+        k -= pc;
+        base += 32;
+    }
+    return 0xFFFFFFFFu;
+}
+
+// ---- P1: ordered emit of the previous event's matches (a8) + arrivals at time t (a3) ---------------
+__device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t step, uint64_t t,
+                                                 uint64_t emit_base) {
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const uint32_t nW = (gridDim.x * blockDim.x) >> 5;
+    const uint64_t* mbprev = a.matchbits + (size_t)((step + 1) & 1) * a.nLw;
+    for (uint32_t lb = gw * 32; lb < a.L; lb += nW * 32) {
+        const uint32_t l = lb + lane;
+        const bool ok = l < a.L;
+        uint32_t c = NONE32;
+        uint64_t f = 0;
+        if (ok) {
+            c = ldcg32(a.inflight + l);
+            f = ldcg64(a.free_t + l);
+        }
+        if (step > 0) {
+            const uint32_t wq = lb >> 6;
+            const uint64_t word = ldcg64(mbprev + wq);
+            const uint32_t mine = (uint32_t)(word >> (lb & 32));   // this warp's 32 links
+            if (mine != 0) {                                        // warp-uniform
+                uint32_t pre = 0;
+                for (uint32_t i = lane; i < wq; i += 32) pre += __popcll(ldcg64(mbprev + i));
+                pre = __reduce_add_sync(0xFFFFFFFFu, pre);
+                if (lb & 32) pre += __popc((uint32_t)word);
+                if ((mine >> lane) & 1u) {
+                    const uint64_t rank = pre + __popc(mine & ((1u << lane) - 1u));
+                    const uint64_t wl = a.w[l];
+                    uint4* o = reinterpret_cast<uint4*>(a.out + emit_base + rank);
+                    const uint64_t ts = f - wl + a.t_offset, te = f + a.t_offset;
+                    o[0] = make_uint4(c, a.psrc[l], a.pdst[l], l);
+                    o[1] = make_uint4((uint32_t)ts, (uint32_t)(ts >> 32), (uint32_t)te, (uint32_t)(te >> 32));
+                }
+            }
+        }
+        if (ok && c != NONE32 && f == t) {   // arrival: forwardable from t on
+            const uint32_t d = a.edst[l];
+            atomicOr((unsigned long long*)&a.have[(size_t)d * a.Wp + (c >> 6)], 1ull << (c & 63));
+            stcg32(a.inflight + l, NONE32);
+            stcg32(a.have_epoch + d, step + 1);
+        }
+    }
+    // clear the bitmap the coming match phase writes; re-arm the ring slot after next
+    uint64_t* mbcur = a.matchbits + (size_t)(step & 1) * a.nLw;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < a.nLw; i += gridDim.x * blockDim.x) stcg64(mbcur + i, 0);
+    if (blockIdx.x == 0 && threadIdx.x == 0) stcg64((uint64_t*)&a.ctrl->tnext[(step + 2) % 3], T_INF);
+}
+
+// ---- P2: match one destination (a4..a8) -----------------------------------------------------------------
+struct CtaScratch {
+    uint32_t act[32];   // active in-links of the current window, ascending link id
+    uint32_t nact;
+    uint32_t wc;        // chunks this destination still wants
+};
+
+struct LoopStats {
+    unsigned long long rows, links, slow;
+};
+
+__device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v, uint32_t step, uint64_t t,
+                                                  uint32_t* cnt, CtaScratch& sh, LoopStats& st) {
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t Q = a.Wp >> 1;  // uint4 per row
+    const uint32_t S = a.S;
+    const uint4* wrow = reinterpret_cast<const uint4*>(a.wants + (size_t)v * a.Wp);
+    const uint32_t e0 = a.in_off[v], e1 = a.in_off[v + 1];
+    if (tid == 0) sh.wc = ldcg32(a.wants_cnt + v);
+    __syncthreads();
+    const uint32_t wc_start = sh.wc;
+    uint64_t mymin = T_INF, mymax = 0;   // meaningful in warp 0 only
+    const bool idle_skip = !(a.flags & 2u);
+
+    for (uint32_t eb = e0; eb < e1; eb += 32) {
+        // a4: active in-links of this window, ascending link id
+        if (warp == 0) {
+            const uint32_t e = eb + lane;
+            const uint32_t wc = sh.wc;
+            bool active = false;
+            uint32_t l = 0;
+            if (e < e1) {
+                l = a.in_link[e];
+                const uint64_t f = ldcg64(a.free_t + l);
+                if (f > t) {
+                    mymin = min(mymin, f);
+                } else if (wc > 0) {
+                    active = true;
+                    if (idle_skip) {   // nothing arrived at the source since this link last found no candidate
+                        const uint32_t ee = ldcg32(a.empty_epoch + l);
+                        if (ee != 0 && ee >= ldcg32(a.have_epoch + a.esrc[l])) active = false;
+                    }
+                }
+            }
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, active);
+            if (active) sh.act[__popc(m & ((1u << lane) - 1u))] = l;
+            if (lane == 0) sh.nact = __popc(m);
+        }
+        __syncthreads();
+        const uint32_t nact = sh.nact;
+        for (uint32_t b0 = 0; b0 < nact; b0 += NB) {
+            if (sh.wc == 0) break;   // CTA-uniform: sh.wc only changes between the two barriers below
+            const uint32_t nb = min((uint32_t)NB, nact - b0);
+            // a5: candidate counts per 64-word segment for nb in-links in one sweep of wants[v]
+            const uint4* hrow[NB];
+#pragma unroll
+            for (int j = 0; j < NB; ++j)
+                hrow[j] = reinterpret_cast<const uint4*>(a.have + (size_t)a.esrc[sh.act[b0 + (j < (int)nb ? j : 0)]] * a.Wp);
+            for (uint32_t qb = warp * 32; qb < Q; qb += blockDim.x) {
+                const uint32_t q = qb + lane;
+                const bool ok = q < Q;
+                uint4 wv = make_uint4(0, 0, 0, 0);
+                uint4 h[NB];
+                if (ok) wv = ldcg128(wrow + q);
+#pragma unroll
+                for (int j = 0; j < NB; ++j) {
+                    h[j] = make_uint4(0, 0, 0, 0);
+                    if (j < (int)nb && ok) h[j] = ldcg128(hrow[j] + q);
+                }
+#pragma unroll
+                for (int j = 0; j < NB; ++j) {
+                    if (j < (int)nb) {
+                        const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)popc128(and128(h[j], wv)));
+                        if (lane == 0) cnt[j * S + (qb >> 5)] = tot;
+                    }
+                }
+            }
+            __syncthreads();
+            // a6 + a7: serial picks in ascending link id, each seeing the earlier claims
+            if (warp == 0) {
+                st.rows += nb + 1;
+                st.links += nb;
+                uint32_t wc = sh.wc;
+                uint32_t claimed[NB];
+                uint32_t ncl = 0;
+#pragma unroll
+                for (int j = 0; j < NB; ++j) claimed[j] = NONE32;
+                for (uint32_t j = 0; j < nb && wc > 0; ++j) {
+                    const uint32_t l = sh.act[b0 + j];
+                    const uint32_t u = a.esrc[l];
+                    uint32_t* cj = cnt + j * S;
+                    const uint64_t* hw = a.have + (size_t)u * a.Wp;
+                    // earlier claims of this sweep that u also holds are no longer candidates
+                    if (lane == 0) {
+#pragma unroll
+                        for (int i = 0; i < NB; ++i) {
+                            if (i < (int)ncl) {
+                                const uint32_t c = claimed[i];
+                                if ((ldcg64(hw + (c >> 6)) >> (c & 63)) & 1ull) cj[c >> 12] -= 1;
+                            }
+                        }
+                    }
+                    __syncwarp();
+                    uint32_t n = 0;
+                    for (uint32_t s = lane; s < S; s += 32) n += cj[s];
+                    n = __reduce_add_sync(0xFFFFFFFFu, n);
+                    if (n == 0) {
+                        if (lane == 0) stcg32(a.empty_epoch + l, step + 1);
+                        continue;
+                    }
+                    const uint32_t r = philox_draw((uint32_t)t, (uint32_t)(t >> 32), l, 0u, a.k0, a.k1);
+                    uint32_t rem = __umulhi(r, n);   // k = (r * n) >> 32
+                    uint32_t seg = 0;
+                    for (uint32_t sb = 0; sb < S; sb += 32) {
+                        const uint32_t x = (sb + lane < S) ? cj[sb + lane] : 0u;
+                        const uint32_t incl = warp_incl_scan(x, lane);
+                        const uint32_t tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+                        if (rem < tot) {
+                            const uint32_t m = __ballot_sync(0xFFFFFFFFu, incl > rem);
+                            const int fl = __ffs(m) - 1;
+                            seg = sb + fl;
+                            rem -= __shfl_sync(0xFFFFFFFFu, incl - x, fl);
+                            break;
+                        }
+                        rem -= tot;
+                    }
+                    const uint32_t q = seg * SEG_U4 + lane;
+                    uint4 m4 = make_uint4(0, 0, 0, 0);
+                    if (q < Q) m4 = and128(ldcg128(reinterpret_cast<const uint4*>(hw) + q), ldcg128(wrow + q));
+#pragma unroll
+                    for (int i = 0; i < NB; ++i) {
+                        if (i < (int)ncl && (claimed[i] >> 7) == q) {
+                            const uint32_t b = claimed[i] & 127u;
+                            const uint32_t msk = ~(1u << (b & 31));
+                            if (b < 32) m4.x &= msk; else if (b < 64) m4.y &= msk; else if (b < 96) m4.z &= msk; else m4.w &= msk;
+                        }
+                    }
+                    const uint32_t pc = popc128(m4);
+                    const uint32_t incl = warp_incl_scan(pc, lane);
+                    const uint32_t mm = __ballot_sync(0xFFFFFFFFu, incl > rem);
+                    const int fl = (__ffs(mm) - 1) & 31;
+                    const uint32_t rem2 = rem - __shfl_sync(0xFFFFFFFFu, incl - pc, fl);
+                    uint32_t c = NONE32;
+                    if ((int)lane == fl && mm != 0) c = q * 128u + kth_bit128(m4, rem2);
+                    c = __shfl_sync(0xFFFFFFFFu, c, fl);
+                    if (c == NONE32) {   // cannot happen; fail loudly instead of corrupting
+                        if (lane == 0) atomicOr(&a.ctrl->err, 4u);
+                        continue;
+                    }
+#pragma unroll
+                    for (int i = 0; i < NB; ++i) if (i == (int)ncl) claimed[i] = c;
+                    ++ncl;
+                    --wc;
+                    // a8: claim -> link busy until t + w
+                    if (lane == 0) {
+                        const uint64_t te = t + a.w[l];
+                        atomicAnd((unsigned long long*)&a.wants[(size_t)v * a.Wp + (c >> 6)], ~(1ull << (c & 63)));
+                        stcg32(a.inflight + l, c);
+                        stcg64(a.free_t + l, te);
+                        atomicOr((unsigned long long*)&a.matchbits[(size_t)(step & 1) * a.nLw + (l >> 6)], 1ull << (l & 63));
+                        mymin = min(mymin, te);
+                        mymax = max(mymax, te);
+                    }
+                }
+                if (lane == 0) sh.wc = wc;
+                __threadfence();
+            }
+            __syncthreads();
+        }
+        __syncthreads();
+    }
+    if (warp == 0) {
+        for (int o = 16; o; o >>= 1) mymin = min(mymin, __shfl_xor_sync(0xFFFFFFFFu, mymin, o));
+        if (lane == 0) {
+            if (mymin != T_INF) atomicMin(&a.ctrl->tnext[(step + 1) % 3], (unsigned long long)mymin);
+            const uint32_t wc = sh.wc;
+            if (wc != wc_start) {
+                stcg32(a.wants_cnt + v, wc);
+                atomicAdd(&a.ctrl->total, (unsigned long long)(wc_start - wc));
+                atomicMax(&a.ctrl->tmax, (unsigned long long)mymax);
+            }
+        }
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(LOOP_THREADS) k_loop(const LoopArgs a) {
+    extern __shared__ uint32_t cnt[];   // [NB][S] candidate counts per segment
+    __shared__ CtaScratch sh;
+    cg::grid_group grid = cg::this_grid();
+    LoopStats st = {0, 0, 0};
+    uint32_t step = 0;
+    uint64_t t = 0;
+    uint64_t emit_base = 0;
+    for (;;) {
+        const uint64_t total_now = ldcg64((const uint64_t*)&a.ctrl->total);   // through event step-1
+        loop_phase_links(a, step, t, emit_base);
+        emit_base = total_now;
+        grid.sync();
+        for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x) match_destination(a, v, step, t, cnt, sh, st);
+        grid.sync();
+        t = ldcg64((const uint64_t*)&a.ctrl->tnext[(step + 1) % 3]);
+        ++step;
+        if (t == T_INF) break;
+    }
+    if (threadIdx.x == 0) {
+        if (st.rows) atomicAdd(&a.ctrl->rows_scanned, st.rows);
+        if (st.links) atomicAdd(&a.ctrl->links_scanned, st.links);
+        if (st.slow) atomicAdd(&a.ctrl->slow_picks, st.slow);
+        if (blockIdx.x == 0) a.ctrl->events = step;
+    }
+}
+
+// ==================================================================================================
+//  a9: emitter for reductions -- reverse in direction and time, then sort by (t_start, link).
+// ==================================================================================================
+// raw record of the transposed broadcast (c, psrc, pdst, l, ts, te)  ->  (c, psrc, pdst, l, T-te, T-ts);
+// the loop already reported the PHYSICAL endpoints, which are the reversed transfer's src -> dst.
+__global__ void k_reverse_keys(Rec* __restrict__ raw, uint64_t n, uint64_t T, uint32_t link_bits,
+                               uint64_t* __restrict__ keys, uint32_t* __restrict__ idx) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    Rec r = raw[i];
+    const uint64_t ts = T - r.t_end, te = T - r.t_start;
+    r.t_start = ts;
+    r.t_end = te;
+    raw[i] = r;
+    keys[i] = (ts << link_bits) | r.link;
+    idx[i] = (uint32_t)i;
+}
+
+__global__ void k_gather_shift(const Rec* __restrict__ raw, const uint32_t* __restrict__ idx, uint64_t n,
+                               uint64_t shift, Rec* __restrict__ out) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    Rec r = raw[idx[i]];
+    r.t_start += shift;
+    r.t_end += shift;
+    out[i] = r;
+}
+
+// ---- stable LSD radix sort, 8 bits per pass, (u64 key, u32 payload) -------------------------------
+constexpr int SORT_THREADS = 256;
+constexpr int SORT_ITEMS = 8;
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 2048 keys per block
+
+__global__ void __launch_bounds__(SORT_THREADS) k_sort_hist(const uint64_t* __restrict__ keys, uint64_t n,
+                                                            uint32_t shift, uint32_t* __restrict__ ghist,
+                                                            uint32_t nblocks) {
+    __shared__ uint32_t h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    const uint64_t base = (uint64_t)blockIdx.x * SORT_TILE;
+    for (int i = 0; i < SORT_ITEMS; ++i) {
+        const uint64_t p = base + (uint64_t)i * SORT_THREADS + threadIdx.x;
+        if (p < n) atomicAdd(&h[(keys[p] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    ghist[(size_t)threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
+}
+
+// exclusive scan of ghist (digit-major), single block
+__global__ void __launch_bounds__(1024) k_sort_scan(uint32_t* __restrict__ ghist, uint64_t len) {
+    __shared__ uint32_t wsum[32];
+    __shared__ uint32_t carry;
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (uint64_t b = 0; b < len; b += 1024) {
+        const uint64_t i = b + threadIdx.x;
+        const uint32_t x = (i < len) ? ghist[i] : 0u;
+        uint32_t incl = warp_incl_scan(x, lane);
+        if (lane == 31) wsum[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            const uint32_t y = wsum[lane];
+            const uint32_t yi = warp_incl_scan(y, lane);
+            wsum[lane] = yi - y;
+        }
+        __syncthreads();
+        const uint32_t c = carry;
+        const uint32_t excl = c + wsum[warp] + incl - x;
+        if (i < len) ghist[i] = excl;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry = excl + x;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(SORT_THREADS) k_sort_scatter(const uint64_t* __restrict__ kin,
+                                                               const uint32_t* __restrict__ vin,
+                                                               uint64_t* __restrict__ kout,
+                                                               uint32_t* __restrict__ vout, uint64_t n,
+                                                               uint32_t shift, const uint32_t* __restrict__ ghist,
+                                                               uint32_t nblocks) {
+    constexpr int NW = SORT_THREADS / 32;
+    __shared__ uint32_t wcount[NW][256];
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < NW * 256; i += SORT_THREADS) (&wcount[0][0])[i] = 0;
+    __syncthreads();
+    // warp w owns items [w*256, w*256+256) of the tile, visited in index order
+    const uint64_t wbase = (uint64_t)blockIdx.x * SORT_TILE + (uint64_t)warp * (32 * SORT_ITEMS);
+    uint64_t key[SORT_ITEMS];
+    uint32_t val[SORT_ITEMS], rank[SORT_ITEMS];
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        const uint64_t p = wbase + (uint64_t)r * 32 + lane;
+        const bool valid = p < n;
+        key[r] = valid ? kin[p] : 0;
+        val[r] = valid ? vin[p] : 0;
+        const uint32_t vm = __ballot_sync(0xFFFFFFFFu, valid);
+        rank[r] = 0;
+        if (valid) {
+            const uint32_t d = (uint32_t)(key[r] >> shift) & 255u;
+            const uint32_t peers = __match_any_sync(vm, d);
+            rank[r] = wcount[warp][d] + __popc(peers & ((1u << lane) - 1u));
+            __syncwarp(vm);
+            if ((int)lane == __ffs(peers) - 1) wcount[warp][d] += __popc(peers);
+            __syncwarp(vm);
+        }
+    }
+    __syncthreads();
+    {   // per digit: global base of this block, then exclusive prefix over the warps
+        const uint32_t d = threadIdx.x;
+        uint32_t run = ghist[(size_t)d * nblocks + blockIdx.x];
+#pragma unroll
+        for (int w = 0; w < NW; ++w) {
+            const uint32_t c = wcount[w][d];
+            wcount[w][d] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        const uint64_t p = wbase + (uint64_t)r * 32 + lane;
+        if (p < n) {
+            const uint32_t d = (uint32_t)(key[r] >> shift) & 255u;
+            const uint32_t pos = wcount[warp][d] + rank[r];
+            kout[pos] = key[r];
+            vout[pos] = val[r];
+        }
+    }
+}
+
+}  // namespace pccl

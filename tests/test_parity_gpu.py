@@ -1,0 +1,243 @@
+"""Parity of the CUDA path (through the C-ABI of include/pccl.h) against the CPU oracle.
+
+Bar: everything on this path is integer work, so every comparison is
+bit-exact -- identical records (chunk, src, dst, link, t_start_ps, t_end_ps) in identical
+canonical order, identical schedule time, identical event count.  On top of parity the
+independent checker (oracle/checker.py) validates the CUDA schedule against what the paper
+fixes (link exclusivity, causality, postconditions, relay-only non-members).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle  # noqa: E402
+import workloads as wl  # noqa: E402
+from oracle import checker  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def pk():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2606_07019_b200 as pk
+    pk.use_torch(0)
+    return pk
+
+
+def gpu_run(pk, p, flags=0):
+    return pk.synthesize(*p.args()) if flags == 0 else _problem_run(pk, p, flags)
+
+
+def _problem_run(pk, p, flags):
+    topo = pk.Topology(p.n_npus, p.links)
+    prob = pk.Problem(topo, p.group, p.n_chunks, p.pre, p.post, p.chunk_bytes)
+    return prob.synthesize(p.seed, flags)
+
+
+def assert_same(p, s, o):
+    tr = s.transfers
+    assert s.size == len(o.transfers), f"{p.name}: {s.size} transfers vs oracle {len(o.transfers)}"
+    assert s.time_ps == o.time_ps, f"{p.name}: T {s.time_ps} vs oracle {o.time_ps}"
+    for f in ("t_start_ps", "link", "chunk", "src", "dst", "t_end_ps"):
+        if not np.array_equal(tr[f], o.transfers[f]):
+            i = int(np.nonzero(tr[f] != o.transfers[f])[0][0])
+            raise AssertionError(f"{p.name}: field {f} differs first at record {i}: "
+                                 f"cuda {tr[i]} vs oracle {o.transfers[i]}")
+    st = s.stats
+    assert st["events"] == o.events
+    assert st["wants_total"] == o.wants_total
+    assert st["mode"] == o.mode
+    assert st["time_phase1_ps"] == o.time_phase1_ps
+
+
+# ------------------------------------------------------------------------------ single rows
+def test_a6_philox_device_matches_known_answers_and_oracle(pk, golden_dir):
+    import os
+    rows = []
+    with open(os.path.join(golden_dir, "philox_kat.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            rows.append([int(x, 16) for x in line.split()])
+    for v in rows:   # the published vectors, evaluated on the GPU
+        out = pk.device_philox([v[0:4]], v[4:6])
+        assert [int(x) for x in out[0]] == v[6:10]
+    rng = np.random.default_rng(7)
+    ctr = rng.integers(0, 2 ** 32, size=(1000, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, size=2, dtype=np.uint64).astype(np.uint32)
+    out = pk.device_philox(ctr, key)
+    for i in range(0, 1000, 37):
+        assert tuple(int(x) for x in out[i]) == oracle.philox4x32_10(ctr[i], key)
+
+
+def test_a0_link_costs(pk):
+    rng = np.random.default_rng(3)
+    links = np.zeros(500, dtype=wl.LINK_DT)
+    links["src"] = rng.integers(0, 40, 500)
+    links["dst"] = (links["src"] + 1 + rng.integers(0, 39, 500)) % 40
+    links["alpha_ps"] = rng.integers(0, 10 ** 6, 500)
+    links["bytes_per_ps"] = rng.integers(1, 1000, 500)
+    topo = pk.Topology(40, links)
+    for cb in (1, 63, 64, 1 << 20, (1 << 20) + 1, 10 ** 12 + 7):
+        got = topo.link_costs(cb)
+        want = [oracle.link_cost(int(l["alpha_ps"]), int(l["bytes_per_ps"]), cb) for l in links]
+        assert got.tolist() == want
+
+
+@pytest.mark.parametrize("maker", [wl.config1, wl.config2, wl.config3, wl.config5_small])
+def test_a1_distances(pk, maker):
+    p = maker(0)
+    topo = pk.Topology(p.n_npus, p.links)
+    tl = p.links.copy()
+    tl["src"], tl["dst"] = p.links["dst"], p.links["src"]
+    for s in (0, 1, p.n_npus // 2, p.n_npus - 1):
+        assert np.array_equal(topo.distances(p.chunk_bytes, s), oracle.distances(p.n_npus, p.links, p.chunk_bytes, s))
+        assert np.array_equal(topo.distances(p.chunk_bytes, s, transposed=True),
+                              oracle.distances(p.n_npus, tl, p.chunk_bytes, s))
+
+
+def test_a1_distances_unreachable_is_inf(pk):
+    links = np.array([(0, 1, 5, 1), (1, 2, 5, 1)], dtype=wl.LINK_DT)   # 3 unreachable, 0 not reachable from 2
+    topo = pk.Topology(4, links)
+    d = topo.distances(10, 0)
+    assert d.tolist() == [0, 15, 30, 2 ** 64 - 1]
+    assert np.array_equal(d, oracle.distances(4, links, 10, 0))
+
+
+def _copy_conditions(p):
+    """COPY-mode problem -> (cond_src, dest_off, dests) for oracle.wants."""
+    C = p.n_chunks
+    src = np.zeros(C, dtype=np.uint32)
+    src[p.pre["chunk"]] = p.pre["npu"]
+    order = np.lexsort((p.post["npu"], p.post["chunk"]))
+    pc, pn = p.post["chunk"][order], p.post["npu"][order]
+    keep = pn != src[pc]
+    pc, pn = pc[keep], pn[keep]
+    off = np.zeros(C + 1, dtype=np.uint64)
+    np.add.at(off, pc.astype(np.int64) + 1, 1)
+    return src, np.cumsum(off).astype(np.uint64), pn.astype(np.uint32)
+
+
+@pytest.mark.parametrize("maker", [wl.config1, wl.config4_small, wl.config5_small, wl.two_groups_mesh3x3])
+@pytest.mark.parametrize("seed", [0, 3])
+def test_a2_wants_bitmap(pk, maker, seed):
+    p = maker(seed)
+    src, off, dests = _copy_conditions(p)
+    want = oracle.wants(p.n_npus, p.links, p.n_chunks, src, off, dests, p.chunk_bytes, seed)
+    topo = pk.Topology(p.n_npus, p.links)
+    prob = pk.Problem(topo, p.group, p.n_chunks, p.pre, p.post, p.chunk_bytes)
+    got = prob.wants(0, seed)
+    assert len(got) == len(want)
+    assert np.array_equal(got["npu"], want["npu"]) and np.array_equal(got["chunk"], want["chunk"])
+
+
+# ------------------------------------------------------------------------------ whole path
+SMALL = [wl.config1, wl.config2, wl.config3, wl.config4_small, wl.config5_small, wl.two_groups_mesh3x3]
+
+
+@pytest.mark.parametrize("maker", SMALL, ids=lambda m: m.__name__)
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_schedule_bit_exact_small_configs(pk, maker, seed):
+    p = maker(seed)
+    o = oracle.synthesize(*p.args())
+    s = gpu_run(pk, p)
+    assert_same(p, s, o)
+    checker.check_schedule(p, s.transfers)
+
+
+@pytest.mark.parametrize("maker", [wl.config1, wl.config3, wl.config4_small], ids=lambda m: m.__name__)
+def test_idle_skip_does_not_change_the_schedule(pk, maker):
+    p = maker(1)
+    o = oracle.synthesize(*p.args())
+    a = gpu_run(pk, p, pk.PCCL_FLAG_NO_IDLE_SKIP)
+    b = gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE | pk.PCCL_FLAG_TIME_LOOP)
+    assert_same(p, a, o)
+    assert_same(p, b, o)
+    assert a.stats["rows_scanned"] >= b.stats["rows_scanned"]
+
+
+@pytest.mark.parametrize("n,bidir", [(2, False), (5, False), (8, True), (9, True)])
+def test_ring_all_gather_closed_form(pk, n, bidir, golden_dir):
+    p = wl.ring_all_gather(n, bidir, seed=1)
+    s = gpu_run(pk, p)
+    w = 520_972   # tests/golden/closed_forms.txt
+    steps = (n - 1) if not bidir else -(-(n - 1) // 2)
+    assert s.time_ps == steps * w
+    assert s.size == n * (n - 1)
+    assert_same(p, s, oracle.synthesize(*p.args()))
+
+
+def test_many_chunks_per_link_and_ragged_rows(pk):
+    """rows of 1, 2 and 130 words (ragged tail inside a 64-word segment and across segments),
+    several chunks per NPU so in-links of one destination overlap (the serial re-pick path)."""
+    for cpn, n in ((1, 6), (20, 7), (1040, 8)):
+        p = wl.ring_all_gather(n, True, seed=5, chunks_per_npu=cpn, chunk_bytes=4096)
+        o = oracle.synthesize(*p.args())
+        s = gpu_run(pk, p)
+        assert_same(p, s, o)
+
+
+def test_high_indegree_destination(pk):
+    """a full mesh of 40 nodes: 39 in-links per destination -> several sweeps of 8 in-links and
+    two 32-link windows are not needed, but 5 sweeps are; all-gather makes them overlap."""
+    p = wl.full_mesh_problem(40, "allgather", seed=2)
+    assert_same(p, gpu_run(pk, p), oracle.synthesize(*p.args()))
+    p = wl.full_mesh_problem(40, "alltoall", seed=2)
+    assert_same(p, gpu_run(pk, p), oracle.synthesize(*p.args()))
+
+
+def test_star_switch_with_70_inlinks(pk):
+    """one switch node with 70 in-links (three 32-link windows), all-to-all among the leaves."""
+    n = 70
+    links = [(i, n, 1000, 7) for i in range(n)] + [(n, i, 1000, 7) for i in range(n)]
+    links = np.array(links, dtype=wl.LINK_DT)
+    members = np.arange(n, dtype=np.uint32)
+    nc, pre, post = wl.all_to_all(members)
+    p = wl.Problem("star70_alltoall", n + 1, links, members, nc, pre, post, 1000, 11)
+    o = oracle.synthesize(*p.args())
+    s = gpu_run(pk, p)
+    assert_same(p, s, o)
+    checker.check_schedule(p, s.transfers)
+
+
+def test_empty_and_trivial(pk):
+    links = wl.ring_links(4, True)
+    members = np.arange(4, dtype=np.uint32)
+    # no chunks at all
+    p = wl.Problem("nochunks", 4, links, members, 0, np.zeros(0, wl.PAIR_DT), np.zeros(0, wl.PAIR_DT), 64, 0)
+    s = gpu_run(pk, p)
+    assert s.size == 0 and s.time_ps == 0 and len(s.transfers) == 0
+    # post == pre: nothing to move
+    pre = np.array([(0, 0), (1, 1)], dtype=wl.PAIR_DT)
+    p = wl.Problem("noop", 4, links, members, 2, pre, pre.copy(), 64, 0)
+    o = oracle.synthesize(*p.args())
+    s = gpu_run(pk, p)
+    assert s.size == 0 == len(o.transfers) and s.time_ps == 0
+    # no links, nothing to move
+    p = wl.Problem("nolinks", 2, np.zeros(0, wl.LINK_DT), members[:2], 1, pre[:1], pre[:1].copy(), 64, 0)
+    assert gpu_run(pk, p).size == 0
+
+
+def test_error_codes(pk):
+    links = np.array([(0, 1, 5, 1)], dtype=wl.LINK_DT)   # 1 cannot reach 0
+    members = np.array([0, 1], dtype=np.uint32)
+    pre = np.array([(1, 0)], dtype=wl.PAIR_DT)
+    post = np.array([(0, 0)], dtype=wl.PAIR_DT)
+    with pytest.raises(pk.PcclError) as e:
+        pk.synthesize(2, links, members, 1, pre, post, 64, 0)
+    assert e.value.code == pk.PCCL_ERR_UNREACHABLE
+    with pytest.raises(oracle.OracleError) as eo:
+        oracle.synthesize(2, links, members, 1, pre, post, 64, 0)
+    assert eo.value.code == oracle.ERR_UNREACHABLE
+
+
+@pytest.mark.slow
+def test_config4_full_size_bit_exact(pk):
+    """BASELINE.json configs[3] at full size (the bench workload): 512 NPUs, 261,632 chunks."""
+    p = wl.config4(0)
+    o = oracle.synthesize(*p.args())
+    s = gpu_run(pk, p)
+    assert s.size == 1_572_864 == o.wants_total     # sum of hop distances, closed form
+    assert_same(p, s, o)
+    checker.check_structure(p, s.transfers)
