@@ -168,7 +168,7 @@ class Topology:
         return out
 
     def close(self):
-        if getattr(self, "handle", None):
+        if getattr(self, "handle", None) and lib is not None:
             lib.pccl_topology_destroy(self.handle)
             self.handle = None
 
@@ -208,7 +208,7 @@ class Schedule:
         return {k: getattr(s, k) for k, _ in pccl_stats_t._fields_}
 
     def close(self):
-        if getattr(self, "handle", None):
+        if getattr(self, "handle", None) and lib is not None:
             lib.pccl_schedule_destroy(self.handle)
             self.handle = None
 
@@ -257,7 +257,7 @@ class Problem:
         return out
 
     def close(self):
-        if getattr(self, "handle", None):
+        if getattr(self, "handle", None) and lib is not None:
             lib.pccl_problem_destroy(self.handle)
             self.handle = None
 
