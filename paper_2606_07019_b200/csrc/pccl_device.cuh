@@ -26,7 +26,7 @@ namespace pccl {
 
 constexpr uint64_t T_INF = 0xFFFFFFFFFFFFFFFFull;
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
-constexpr int LOOP_THREADS = 512;  // threads per CTA of the event-loop kernel
+constexpr int LOOP_THREADS = 256;  // threads per CTA of the event-loop kernel (= NB warps)
 constexpr int NB = 8;              // in-links of one destination counted in one sweep
 constexpr int SEG_U4 = 32;         // uint4 per segment (one warp-wide load) = 64 words = 4096 chunks
 
@@ -358,21 +358,82 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
 
 // ---- P2: match one destination (a4..a8) -----------------------------------------------------------------
 struct CtaScratch {
-    uint32_t act[32];   // active in-links of the current window, ascending link id
+    uint32_t act[32];     // active in-links of the current window, ascending link id
     uint32_t nact;
-    uint32_t wc;        // chunks this destination still wants
+    uint32_t wc;          // chunks this destination still wants
+    uint32_t spec[NB];    // speculative pick of each in-link of the sweep (NONE32: no candidate)
+    uint32_t claimed[NB]; // chunks claimed so far in this sweep (warp 0 only)
 };
 
 struct LoopStats {
     unsigned long long rows, links, slow;
 };
 
+// The k-th candidate (0-based, ascending chunk id) of link-row `hrow` AND wants-row `wrow`, given the
+// per-segment candidate counts cj[0..S).  `excl[0..nex)` are chunks to treat as no longer wanted (claims
+// made earlier in the same sweep); cj must already be net of them.  Whole warp; returns the chunk id.
+__device__ __forceinline__ uint32_t kth_candidate(const uint32_t* cj, uint32_t S, uint32_t Q, const uint4* hrow,
+                                                  const uint4* wrow, uint32_t rem, const uint32_t* excl,
+                                                  uint32_t nex, uint32_t lane) {
+    uint32_t seg = 0;
+    for (uint32_t sb = 0; sb < S; sb += 32) {
+        const uint32_t x = (sb + lane < S) ? cj[sb + lane] : 0u;
+        const uint32_t incl = warp_incl_scan(x, lane);
+        const uint32_t tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        if (rem < tot) {
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, incl > rem);
+            const int fl = __ffs(m) - 1;
+            seg = sb + fl;
+            rem -= __shfl_sync(0xFFFFFFFFu, incl - x, fl);
+            break;
+        }
+        rem -= tot;
+    }
+    const uint32_t q = seg * SEG_U4 + lane;
+    uint4 m4 = make_uint4(0, 0, 0, 0);
+    if (q < Q) m4 = and128(ldcg128(hrow + q), ldcg128(wrow + q));
+    for (uint32_t i = 0; i < nex; ++i) {
+        const uint32_t c = excl[i];
+        if ((c >> 7) == q) {
+            const uint32_t b = c & 127u;
+            const uint32_t msk = ~(1u << (b & 31));
+            if (b < 32) m4.x &= msk; else if (b < 64) m4.y &= msk; else if (b < 96) m4.z &= msk; else m4.w &= msk;
+        }
+    }
+    const uint32_t pc = popc128(m4);
+    const uint32_t incl = warp_incl_scan(pc, lane);
+    const uint32_t mm = __ballot_sync(0xFFFFFFFFu, incl > rem);
+    const int fl = (__ffs(mm) - 1) & 31;
+    const uint32_t rem2 = rem - __shfl_sync(0xFFFFFFFFu, incl - pc, fl);
+    uint32_t c = NONE32;
+    if ((int)lane == fl && mm != 0) c = q * 128u + kth_bit128(m4, rem2);
+    return __shfl_sync(0xFFFFFFFFu, c, fl);
+}
+
+__device__ __forceinline__ uint32_t warp_sum_counts(const uint32_t* cj, uint32_t S, uint32_t lane) {
+    uint32_t n = 0;
+    for (uint32_t s = lane; s < S; s += 32) n += cj[s];
+    return __reduce_add_sync(0xFFFFFFFFu, n);
+}
+
+// a8: link l carries chunk c over [t, t + w_l); destination v no longer wants c
+__device__ __forceinline__ uint64_t commit_claim(const LoopArgs& a, uint32_t v, uint32_t l, uint32_t c, uint32_t step,
+                                                 uint64_t t) {
+    const uint64_t te = t + a.w[l];
+    atomicAnd((unsigned long long*)&a.wants[(size_t)v * a.Wp + (c >> 6)], ~(1ull << (c & 63)));
+    stcg32(a.inflight + l, c);
+    stcg64(a.free_t + l, te);
+    atomicOr((unsigned long long*)&a.matchbits[(size_t)(step & 1) * a.nLw + (l >> 6)], 1ull << (l & 63));
+    return te;
+}
+
 __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v, uint32_t step, uint64_t t,
                                                   uint32_t* cnt, CtaScratch& sh, LoopStats& st) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t Q = a.Wp >> 1;  // uint4 per row
     const uint32_t S = a.S;
-    const uint4* wrow = reinterpret_cast<const uint4*>(a.wants + (size_t)v * a.Wp);
+    const uint4* have4 = reinterpret_cast<const uint4*>(a.have);
+    const uint4* wrow = reinterpret_cast<const uint4*>(a.wants) + (size_t)v * Q;
     const uint32_t e0 = a.in_off[v], e1 = a.in_off[v + 1];
     if (tid == 0) sh.wc = ldcg32(a.wants_cnt + v);
     __syncthreads();
@@ -407,118 +468,120 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
         __syncthreads();
         const uint32_t nact = sh.nact;
         for (uint32_t b0 = 0; b0 < nact; b0 += NB) {
-            if (sh.wc == 0) break;   // CTA-uniform: sh.wc only changes between the two barriers below
+            if (sh.wc == 0) break;   // CTA-uniform: sh.wc only changes between the barriers below
             const uint32_t nb = min((uint32_t)NB, nact - b0);
             // a5: candidate counts per 64-word segment for nb in-links in one sweep of wants[v]
-            const uint4* hrow[NB];
+            {
+                size_t hoff[NB];
 #pragma unroll
-            for (int j = 0; j < NB; ++j)
-                hrow[j] = reinterpret_cast<const uint4*>(a.have + (size_t)a.esrc[sh.act[b0 + (j < (int)nb ? j : 0)]] * a.Wp);
-            for (uint32_t qb = warp * 32; qb < Q; qb += blockDim.x) {
-                const uint32_t q = qb + lane;
-                const bool ok = q < Q;
-                uint4 wv = make_uint4(0, 0, 0, 0);
-                uint4 h[NB];
-                if (ok) wv = ldcg128(wrow + q);
+                for (int j = 0; j < NB; ++j) hoff[j] = (size_t)a.esrc[sh.act[b0 + (j < (int)nb ? j : 0)]] * Q;
+                for (uint32_t qb = warp * 32; qb < Q; qb += blockDim.x) {
+                    const uint32_t q = qb + lane;
+                    const bool ok = q < Q;
+                    uint4 wv = make_uint4(0, 0, 0, 0);
+                    uint4 h[NB];
+                    if (ok) wv = ldcg128(wrow + q);
 #pragma unroll
-                for (int j = 0; j < NB; ++j) {
-                    h[j] = make_uint4(0, 0, 0, 0);
-                    if (j < (int)nb && ok) h[j] = ldcg128(hrow[j] + q);
-                }
+                    for (int j = 0; j < NB; ++j) {
+                        h[j] = make_uint4(0, 0, 0, 0);
+                        if (j < (int)nb && ok) h[j] = ldcg128(have4 + hoff[j] + q);
+                    }
 #pragma unroll
-                for (int j = 0; j < NB; ++j) {
-                    if (j < (int)nb) {
-                        const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)popc128(and128(h[j], wv)));
-                        if (lane == 0) cnt[j * S + (qb >> 5)] = tot;
+                    for (int j = 0; j < NB; ++j) {
+                        if (j < (int)nb) {
+                            const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)popc128(and128(h[j], wv)));
+                            if (lane == 0) cnt[j * S + (qb >> 5)] = tot;
+                        }
                     }
                 }
             }
             __syncthreads();
-            // a6 + a7: serial picks in ascending link id, each seeing the earlier claims
+            // a6: every in-link of the sweep picks from the wants row as it stood at the start of the
+            // sweep -- exact unless an earlier in-link's claim is also held by a later in-link's source
+            if (warp < nb) {
+                const uint32_t l = sh.act[b0 + warp];
+                const uint32_t* cj = cnt + warp * S;
+                const uint32_t n = warp_sum_counts(cj, S, lane);
+                uint32_t c = NONE32;
+                if (n != 0) {
+                    const uint32_t r = philox_draw((uint32_t)t, (uint32_t)(t >> 32), l, 0u, a.k0, a.k1);
+                    c = kth_candidate(cj, S, Q, have4 + (size_t)a.esrc[l] * Q, wrow, __umulhi(r, n), nullptr, 0, lane);
+                    if (c == NONE32 && lane == 0) atomicOr(&a.ctrl->err, 4u);   // cannot happen
+                }
+                if (lane == 0) sh.spec[warp] = c;
+            }
+            __syncthreads();
+            // a7: conflict resolve.  In-links are served in ascending link id, each seeing the earlier
+            // claims.  Link j's speculative pick stands iff no earlier claim is a candidate of j.
             if (warp == 0) {
                 st.rows += nb + 1;
                 st.links += nb;
+                uint32_t bad = 0;
+                for (uint32_t p = lane; p < nb * nb; p += 32) {
+                    const uint32_t i = p / nb, j = p % nb;
+                    if (i < j) {
+                        const uint32_t ci = sh.spec[i];
+                        if (ci != NONE32 && cnt[j * S + (ci >> 12)] != 0) {
+                            const uint32_t u = a.esrc[sh.act[b0 + j]];
+                            if ((ldcg64(a.have + (size_t)u * a.Wp + (ci >> 6)) >> (ci & 63)) & 1ull) bad |= 1u << j;
+                        }
+                    }
+                }
+                bad = __reduce_or_sync(0xFFFFFFFFu, bad);
+                const uint32_t first_bad = bad ? (uint32_t)(__ffs(bad) - 1) : nb;
+                // commit the picks that stand (one lane per link)
                 uint32_t wc = sh.wc;
-                uint32_t claimed[NB];
-                uint32_t ncl = 0;
-#pragma unroll
-                for (int j = 0; j < NB; ++j) claimed[j] = NONE32;
-                for (uint32_t j = 0; j < nb && wc > 0; ++j) {
+                {
+                    uint32_t c = NONE32, l = 0;
+                    if (lane < first_bad) { c = sh.spec[lane]; l = sh.act[b0 + lane]; }
+                    const uint32_t cm = __ballot_sync(0xFFFFFFFFu, c != NONE32);
+                    if (lane < first_bad) {
+                        if (c != NONE32) {
+                            const uint64_t te = commit_claim(a, v, l, c, step, t);
+                            mymin = min(mymin, te);
+                            mymax = max(mymax, te);
+                            sh.claimed[__popc(cm & ((1u << lane) - 1u))] = c;
+                        } else {
+                            stcg32(a.empty_epoch + l, step + 1);
+                        }
+                    }
+                    wc -= __popc(cm);
+                }
+                uint32_t ncl = __popc(__ballot_sync(0xFFFFFFFFu, lane < first_bad && sh.spec[lane] != NONE32));
+                __syncwarp();
+                // the rest, one by one, against the wants row net of the claims so far
+                for (uint32_t j = first_bad; j < nb && wc > 0; ++j) {
+                    if (lane == 0) ++st.slow;
                     const uint32_t l = sh.act[b0 + j];
                     const uint32_t u = a.esrc[l];
                     uint32_t* cj = cnt + j * S;
-                    const uint64_t* hw = a.have + (size_t)u * a.Wp;
-                    // earlier claims of this sweep that u also holds are no longer candidates
                     if (lane == 0) {
-#pragma unroll
-                        for (int i = 0; i < NB; ++i) {
-                            if (i < (int)ncl) {
-                                const uint32_t c = claimed[i];
-                                if ((ldcg64(hw + (c >> 6)) >> (c & 63)) & 1ull) cj[c >> 12] -= 1;
-                            }
+                        for (uint32_t i = 0; i < ncl; ++i) {
+                            const uint32_t c = sh.claimed[i];
+                            if ((ldcg64(a.have + (size_t)u * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) cj[c >> 12] -= 1;
                         }
                     }
                     __syncwarp();
-                    uint32_t n = 0;
-                    for (uint32_t s = lane; s < S; s += 32) n += cj[s];
-                    n = __reduce_add_sync(0xFFFFFFFFu, n);
+                    const uint32_t n = warp_sum_counts(cj, S, lane);
                     if (n == 0) {
                         if (lane == 0) stcg32(a.empty_epoch + l, step + 1);
                         continue;
                     }
                     const uint32_t r = philox_draw((uint32_t)t, (uint32_t)(t >> 32), l, 0u, a.k0, a.k1);
-                    uint32_t rem = __umulhi(r, n);   // k = (r * n) >> 32
-                    uint32_t seg = 0;
-                    for (uint32_t sb = 0; sb < S; sb += 32) {
-                        const uint32_t x = (sb + lane < S) ? cj[sb + lane] : 0u;
-                        const uint32_t incl = warp_incl_scan(x, lane);
-                        const uint32_t tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
-                        if (rem < tot) {
-                            const uint32_t m = __ballot_sync(0xFFFFFFFFu, incl > rem);
-                            const int fl = __ffs(m) - 1;
-                            seg = sb + fl;
-                            rem -= __shfl_sync(0xFFFFFFFFu, incl - x, fl);
-                            break;
-                        }
-                        rem -= tot;
-                    }
-                    const uint32_t q = seg * SEG_U4 + lane;
-                    uint4 m4 = make_uint4(0, 0, 0, 0);
-                    if (q < Q) m4 = and128(ldcg128(reinterpret_cast<const uint4*>(hw) + q), ldcg128(wrow + q));
-#pragma unroll
-                    for (int i = 0; i < NB; ++i) {
-                        if (i < (int)ncl && (claimed[i] >> 7) == q) {
-                            const uint32_t b = claimed[i] & 127u;
-                            const uint32_t msk = ~(1u << (b & 31));
-                            if (b < 32) m4.x &= msk; else if (b < 64) m4.y &= msk; else if (b < 96) m4.z &= msk; else m4.w &= msk;
-                        }
-                    }
-                    const uint32_t pc = popc128(m4);
-                    const uint32_t incl = warp_incl_scan(pc, lane);
-                    const uint32_t mm = __ballot_sync(0xFFFFFFFFu, incl > rem);
-                    const int fl = (__ffs(mm) - 1) & 31;
-                    const uint32_t rem2 = rem - __shfl_sync(0xFFFFFFFFu, incl - pc, fl);
-                    uint32_t c = NONE32;
-                    if ((int)lane == fl && mm != 0) c = q * 128u + kth_bit128(m4, rem2);
-                    c = __shfl_sync(0xFFFFFFFFu, c, fl);
+                    const uint32_t c = kth_candidate(cj, S, Q, have4 + (size_t)u * Q, wrow, __umulhi(r, n), sh.claimed, ncl, lane);
                     if (c == NONE32) {   // cannot happen; fail loudly instead of corrupting
                         if (lane == 0) atomicOr(&a.ctrl->err, 4u);
                         continue;
                     }
-#pragma unroll
-                    for (int i = 0; i < NB; ++i) if (i == (int)ncl) claimed[i] = c;
-                    ++ncl;
-                    --wc;
-                    // a8: claim -> link busy until t + w
                     if (lane == 0) {
-                        const uint64_t te = t + a.w[l];
-                        atomicAnd((unsigned long long*)&a.wants[(size_t)v * a.Wp + (c >> 6)], ~(1ull << (c & 63)));
-                        stcg32(a.inflight + l, c);
-                        stcg64(a.free_t + l, te);
-                        atomicOr((unsigned long long*)&a.matchbits[(size_t)(step & 1) * a.nLw + (l >> 6)], 1ull << (l & 63));
+                        sh.claimed[ncl] = c;
+                        const uint64_t te = commit_claim(a, v, l, c, step, t);
                         mymin = min(mymin, te);
                         mymax = max(mymax, te);
                     }
+                    ++ncl;
+                    --wc;
+                    __syncwarp();
                 }
                 if (lane == 0) sh.wc = wc;
                 __threadfence();
@@ -528,7 +591,10 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
         __syncthreads();
     }
     if (warp == 0) {
-        for (int o = 16; o; o >>= 1) mymin = min(mymin, __shfl_xor_sync(0xFFFFFFFFu, mymin, o));
+        for (int o = 16; o; o >>= 1) {
+            mymin = min(mymin, __shfl_xor_sync(0xFFFFFFFFu, mymin, o));
+            mymax = max(mymax, __shfl_xor_sync(0xFFFFFFFFu, mymax, o));
+        }
         if (lane == 0) {
             if (mymin != T_INF) atomicMin(&a.ctrl->tnext[(step + 1) % 3], (unsigned long long)mymin);
             const uint32_t wc = sh.wc;
@@ -542,7 +608,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
     __syncthreads();
 }
 
-__global__ void __launch_bounds__(LOOP_THREADS) k_loop(const LoopArgs a) {
+__global__ void __launch_bounds__(LOOP_THREADS, 4) k_loop(const LoopArgs a) {
     extern __shared__ uint32_t cnt[];   // [NB][S] candidate counts per segment
     __shared__ CtaScratch sh;
     cg::grid_group grid = cg::this_grid();
@@ -561,7 +627,7 @@ __global__ void __launch_bounds__(LOOP_THREADS) k_loop(const LoopArgs a) {
         ++step;
         if (t == T_INF) break;
     }
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0) {   // warp 0 lane 0 holds this CTA's counters
         if (st.rows) atomicAdd(&a.ctrl->rows_scanned, st.rows);
         if (st.links) atomicAdd(&a.ctrl->links_scanned, st.links);
         if (st.slow) atomicAdd(&a.ctrl->slow_picks, st.slow);
