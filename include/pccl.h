@@ -164,6 +164,7 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
 #define PCCL_FLAG_KEEP_ON_DEVICE 1u /* do not download the transfers until they are asked for */
 #define PCCL_FLAG_NO_IDLE_SKIP 2u   /* rescan idle links every event (debug / measurement) */
 #define PCCL_FLAG_TIME_LOOP 4u      /* record CUDA events around the event loop (stats) */
+#define PCCL_FLAG_TRACE 8u          /* record per-event phase timestamps (pccl_schedule_trace) */
 
 /* Steps A..F on the GPU for one seed.  Errors: UNREACHABLE, CUDA, NOMEM, INTERNAL. */
 int pccl_problem_synthesize(pccl_problem_t* problem, uint64_t seed, uint32_t flags,
@@ -197,6 +198,14 @@ typedef struct pccl_stats {
     uint32_t grid_blocks;    /* CTAs of the persistent event-loop kernel */
 } pccl_stats_t;
 int pccl_schedule_stats(const pccl_schedule_t* s, pccl_stats_t* out);
+
+/* Diagnostic trace (PCCL_FLAG_TRACE): for each event time of the last phase, PCCL_TRACE_SLOTS
+ * %globaltimer stamps (ns) taken by CTA 0 of the event-loop kernel: loop top, end of the
+ * links phase (emit + arrivals), end of grid barrier 1, in-link list built, candidates
+ * counted, picks made, destination done, end of grid barrier 2.  Returns the number of u64
+ * values available (events * PCCL_TRACE_SLOTS) and writes up to cap of them to out (host). */
+#define PCCL_TRACE_SLOTS 8
+int64_t pccl_schedule_trace(const pccl_schedule_t* s, uint64_t* out, uint64_t cap);
 
 /* ---------------------------------------------------------------------------------------
  * Single rows of the path, exposed for parity tests against the oracle.  Each runs the

@@ -27,7 +27,8 @@ TRANSFER_DT = np.dtype([("chunk", "<u4"), ("src", "<u4"), ("dst", "<u4"), ("link
 
 PCCL_OK, PCCL_ERR_INVALID, PCCL_ERR_UNSUPPORTED, PCCL_ERR_UNREACHABLE = 0, -1, -2, -3
 PCCL_ERR_CUDA, PCCL_ERR_NOMEM, PCCL_ERR_INTERNAL = -4, -5, -6
-PCCL_FLAG_KEEP_ON_DEVICE, PCCL_FLAG_NO_IDLE_SKIP, PCCL_FLAG_TIME_LOOP = 1, 2, 4
+PCCL_FLAG_KEEP_ON_DEVICE, PCCL_FLAG_NO_IDLE_SKIP, PCCL_FLAG_TIME_LOOP, PCCL_FLAG_TRACE = 1, 2, 4, 8
+PCCL_TRACE_SLOTS = 8
 
 
 class pccl_condition_t(C.Structure):
@@ -71,6 +72,7 @@ SIGNATURES = {
     "pccl_schedule_transfers_device": (_vp, [_vp]),
     "pccl_schedule_destroy": (None, [_vp]),
     "pccl_schedule_stats": (_int, [_vp, C.POINTER(pccl_stats_t)]),
+    "pccl_schedule_trace": (_i64, [_vp, _vp, _u64]),
     "pccl_device_philox": (_int, [_vp, _u64, _vp, _vp]),
     "pccl_device_link_costs": (_int, [_vp, _u64, _vp]),
     "pccl_device_distances": (_int, [_vp, _u64, _u32, _int, _vp]),
@@ -206,6 +208,15 @@ class Schedule:
         s = pccl_stats_t()
         _check(lib.pccl_schedule_stats(self.handle, C.byref(s)))
         return {k: getattr(s, k) for k, _ in pccl_stats_t._fields_}
+
+    @property
+    def trace(self) -> np.ndarray:
+        """[events, PCCL_TRACE_SLOTS] ns stamps (needs PCCL_FLAG_TRACE), else an empty array."""
+        n = int(lib.pccl_schedule_trace(self.handle, None, 0))
+        out = np.zeros(max(n, 0), dtype=np.uint64)
+        if n > 0:
+            lib.pccl_schedule_trace(self.handle, _ptr(out), n)
+        return out.reshape(-1, PCCL_TRACE_SLOTS)
 
     def close(self):
         if getattr(self, "handle", None) and lib is not None:

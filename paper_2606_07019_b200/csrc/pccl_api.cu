@@ -171,6 +171,7 @@ struct pccl_schedule {
     size_t h_bytes = 0;
     bool downloaded = false;
     pccl_stats_t stats;
+    std::vector<uint64_t> trace;   // PCCL_FLAG_TRACE: [events][TRACE_SLOTS] ns stamps of the last phase
 };
 
 // -----------------------------------------------------------------------------------------
@@ -574,7 +575,7 @@ struct LoopResult {
 
 // steps D..E: the event loop; records go to `out` (capacity M) in canonical order
 int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint32_t flags, Rec* out,
-               uint64_t t_offset, LoopResult* res) {
+               uint64_t t_offset, LoopResult* res, std::vector<uint64_t>* trace = nullptr) {
     const pccl_topology* t = P.topo;
     const PhaseView pv = view_of(t, ph.transposed);
     LoopArgs a;
@@ -585,6 +586,17 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     a.wants_cnt = W.wants_cnt; a.free_t = W.free_t; a.inflight = W.inflight; a.have_epoch = W.have_epoch;
     a.empty_epoch = W.empty_epoch; a.matchbits = W.matchbits; a.ctrl = W.ctrl; a.out = out; a.t_offset = t_offset;
     cudaStream_t st = G.stream;
+    a.trace = nullptr; a.trace_cap = 0;
+    void* trace_dev = nullptr;
+    if ((flags & PCCL_FLAG_TRACE) && trace) {
+        a.trace_cap = 1u << 14;
+        const size_t tb = (size_t)a.trace_cap * TRACE_SLOTS * 8;
+        int rc = dev_alloc(tb, &trace_dev);
+        if (rc) return rc;
+        if (cudaMemsetAsync(trace_dev, 0, tb, st) != cudaSuccess) { (void)cudaGetLastError(); dev_free(trace_dev); return PCCL_ERR_CUDA; }
+        a.trace = (uint64_t*)trace_dev;
+    }
+    struct TraceGuard { void* p; ~TraceGuard() { dev_free(p); } } trace_guard{trace_dev};
     const uint32_t n_init = std::max(std::max(a.L, a.N), std::max(2 * a.nLw, 1u));
     k_loop_init<<<(n_init + 255) / 256, 256, 0, st>>>(a);
     const size_t smem = (size_t)NB * W.S * 4;
@@ -604,6 +616,12 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     res->total = mb->total; res->tmax = mb->tmax; res->events = mb->events;
     res->rows = mb->rows_scanned; res->links = mb->links_scanned; res->slow = mb->slow_picks;
     res->grid = grid;
+    if (a.trace) {
+        const size_t n = (size_t)std::min<uint64_t>(res->events, a.trace_cap) * TRACE_SLOTS;
+        trace->assign(n, 0);
+        CU(cudaMemcpyAsync(trace->data(), a.trace, n * 8, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
     return PCCL_OK;
 }
 
@@ -701,7 +719,7 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
             rc = dev_alloc(M * sizeof(Rec), (void**)&raw);
             if (rc) return fail(rc);
             t_loop.start();
-            rc = phase_loop(*P, ph, W, seed, flags, raw, 0, &lr);
+            rc = phase_loop(*P, ph, W, seed, flags, raw, 0, &lr, &S->trace);
             if (rc) return fail(rc);
             t_loop.stop();
             if (lr.total != M) return fail(PCCL_ERR_INTERNAL);
@@ -730,7 +748,7 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
                 }
             }
             t_loop.start();
-            rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, toff, &lr);
+            rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, toff, &lr, &S->trace);
             if (rc) return fail(rc);
             t_loop.stop();
             if (lr.total != M) return fail(PCCL_ERR_INTERNAL);
@@ -799,6 +817,12 @@ extern "C" void pccl_schedule_destroy(pccl_schedule_t* s) {
     dev_free(s->d_recs);
     pinned_put(s->h_recs, s->h_bytes);
     delete s;
+}
+extern "C" int64_t pccl_schedule_trace(const pccl_schedule_t* s, uint64_t* out, uint64_t cap) {
+    if (!s || (cap && !out)) return PCCL_ERR_INVALID;
+    const uint64_t n = s->trace.size();
+    if (n && cap) memcpy(out, s->trace.data(), (size_t)std::min(n, cap) * 8);
+    return (int64_t)n;
 }
 extern "C" int pccl_schedule_stats(const pccl_schedule_t* s, pccl_stats_t* out) {
     if (!s || !out) return PCCL_ERR_INVALID;

@@ -261,7 +261,18 @@ struct LoopArgs {
     LoopCtrl* ctrl;
     Rec* out;
     uint64_t t_offset;      // added to the emitted times (phase 2 of all-reduce)
+    uint64_t* trace;        // optional [events][TRACE_SLOTS] globaltimer stamps of CTA 0 (diagnostic), or null
+    uint32_t trace_cap;     // events the trace buffer holds
 };
+
+constexpr int TRACE_SLOTS = 8;   // loop top, links phase, barrier 1, in-link list, count, pick, commit, barrier 2
+__device__ __forceinline__ void trace_stamp(const LoopArgs& a, uint32_t step, int slot) {
+    if (a.trace != nullptr && blockIdx.x == 0 && threadIdx.x == 0 && step < a.trace_cap) {
+        unsigned long long ns;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns));
+        a.trace[(size_t)step * TRACE_SLOTS + slot] = ns;
+    }
+}
 
 __global__ void k_loop_init(LoopArgs a) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -466,6 +477,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
             if (lane == 0) sh.nact = __popc(m);
         }
         __syncthreads();
+        trace_stamp(a, step, 3);
         const uint32_t nact = sh.nact;
         for (uint32_t b0 = 0; b0 < nact; b0 += NB) {
             if (sh.wc == 0) break;   // CTA-uniform: sh.wc only changes between the barriers below
@@ -496,6 +508,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 }
             }
             __syncthreads();
+            trace_stamp(a, step, 4);
             // a6: every in-link of the sweep picks from the wants row as it stood at the start of the
             // sweep -- exact unless an earlier in-link's claim is also held by a later in-link's source
             if (warp < nb) {
@@ -511,6 +524,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 if (lane == 0) sh.spec[warp] = c;
             }
             __syncthreads();
+            trace_stamp(a, step, 5);
             // a7: conflict resolve.  In-links are served in ascending link id, each seeing the earlier
             // claims.  Link j's speculative pick stands iff no earlier claim is a candidate of j.
             if (warp == 0) {
@@ -617,12 +631,17 @@ __global__ void __launch_bounds__(LOOP_THREADS, 4) k_loop(const LoopArgs a) {
     uint64_t t = 0;
     uint64_t emit_base = 0;
     for (;;) {
+        trace_stamp(a, step, 0);
         const uint64_t total_now = ldcg64((const uint64_t*)&a.ctrl->total);   // through event step-1
         loop_phase_links(a, step, t, emit_base);
         emit_base = total_now;
+        trace_stamp(a, step, 1);
         grid.sync();
+        trace_stamp(a, step, 2);
         for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x) match_destination(a, v, step, t, cnt, sh, st);
+        trace_stamp(a, step, 6);
         grid.sync();
+        trace_stamp(a, step, 7);
         t = ldcg64((const uint64_t*)&a.ctrl->tnext[(step + 1) % 3]);
         ++step;
         if (t == T_INF) break;
