@@ -252,13 +252,12 @@ def run_ours(args):
     alg_bytes = stats["rows_scanned"] * stats["row_bytes"]     # bitmap rows the kernel requested x padded row bytes
     achieved = alg_bytes / (loop_avg_ms * 1e-3) / 1e9
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "k_loop_traffic.json")   # from the committed ncu --set full capture
+    tpath = os.path.join(ROOT, "profiles", "k_loop_traffic.txt")   # from the committed ncu --set full capture
     if os.path.exists(tpath):
-        try:
-            with open(tpath) as f:
-                traffic = json.load(f).get(f"config{args.config}")
-        except Exception:
-            traffic = None
+        for ln in open(tpath):
+            f = ln.split()
+            if len(f) == 2 and f[0] == f"config{args.config}":
+                traffic = int(f[1])
     roofline = {"bound": "hbm", "kernel": "k_loop", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": loop_avg_ms,
