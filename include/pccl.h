@@ -164,6 +164,8 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
 #define PCCL_FLAG_KEEP_ON_DEVICE 1u /* do not download the transfers until they are asked for */
 #define PCCL_FLAG_NO_IDLE_SKIP 2u   /* rescan idle links every event (debug / measurement) */
 #define PCCL_FLAG_TIME_LOOP 4u      /* record CUDA events around the event loop (stats) */
+#define PCCL_FLAG_DENSE_SWEEP 16u   /* count candidates by sweeping whole rows, never the sector work list
+                                       (the plain bitmap scan; measurement of the memory-bound form) */
 #define PCCL_FLAG_TRACE 8u          /* record per-event phase timestamps (pccl_schedule_trace) */
 
 /* Steps A..F on the GPU for one seed.  Errors: UNREACHABLE, CUDA, NOMEM, INTERNAL. */
@@ -186,7 +188,11 @@ void pccl_schedule_destroy(pccl_schedule_t* s);
 typedef struct pccl_stats {
     uint64_t events;         /* event times processed (both phases of an all-reduce summed) */
     uint64_t wants_total;    /* popcount(wants) after step C == number of transfers */
-    uint64_t rows_scanned;   /* bitmap rows the match kernel requested (have + wants rows) */
+    uint64_t rows_scanned;   /* bitmap rows the match kernel swept (have + wants rows): the dense,
+                                algorithmic count -- rows_scanned * row_bytes = bytes a sweep without the
+                                sector summaries would request */
+    uint64_t bytes_requested;/* bytes the match kernel actually requested: bitmap sectors whose summary
+                                bits were set in both rows, the summary rows, the segments re-read by picks */
     uint64_t row_bytes;      /* bytes of one (padded) bitmap row */
     uint64_t links_scanned;  /* active in-links whose candidates were counted */
     uint64_t slow_picks;     /* picks that took the serial re-pick path */
@@ -204,7 +210,7 @@ int pccl_schedule_stats(const pccl_schedule_t* s, pccl_stats_t* out);
  * links phase (emit + arrivals), end of grid barrier 1, in-link list built, candidates
  * counted, picks made, destination done, end of grid barrier 2.  Returns the number of u64
  * values available (events * PCCL_TRACE_SLOTS) and writes up to cap of them to out (host). */
-#define PCCL_TRACE_SLOTS 8
+#define PCCL_TRACE_SLOTS 12
 int64_t pccl_schedule_trace(const pccl_schedule_t* s, uint64_t* out, uint64_t cap);
 
 /* ---------------------------------------------------------------------------------------

@@ -28,7 +28,8 @@ TRANSFER_DT = np.dtype([("chunk", "<u4"), ("src", "<u4"), ("dst", "<u4"), ("link
 PCCL_OK, PCCL_ERR_INVALID, PCCL_ERR_UNSUPPORTED, PCCL_ERR_UNREACHABLE = 0, -1, -2, -3
 PCCL_ERR_CUDA, PCCL_ERR_NOMEM, PCCL_ERR_INTERNAL = -4, -5, -6
 PCCL_FLAG_KEEP_ON_DEVICE, PCCL_FLAG_NO_IDLE_SKIP, PCCL_FLAG_TIME_LOOP, PCCL_FLAG_TRACE = 1, 2, 4, 8
-PCCL_TRACE_SLOTS = 8
+PCCL_FLAG_DENSE_SWEEP = 16
+PCCL_TRACE_SLOTS = 12
 
 
 class pccl_condition_t(C.Structure):
@@ -37,7 +38,7 @@ class pccl_condition_t(C.Structure):
 
 class pccl_stats_t(C.Structure):
     _fields_ = [("events", C.c_uint64), ("wants_total", C.c_uint64), ("rows_scanned", C.c_uint64),
-                ("row_bytes", C.c_uint64), ("links_scanned", C.c_uint64), ("slow_picks", C.c_uint64),
+                ("bytes_requested", C.c_uint64), ("row_bytes", C.c_uint64), ("links_scanned", C.c_uint64), ("slow_picks", C.c_uint64),
                 ("time_phase1_ps", C.c_uint64), ("loop_ms", C.c_float), ("setup_ms", C.c_float),
                 ("emit_ms", C.c_float), ("mode", C.c_uint32), ("grid_blocks", C.c_uint32)]
 

@@ -497,9 +497,15 @@ struct Work {   // device workspace of one phase
     uint64_t *w = nullptr, *D = nullptr, *have = nullptr, *wants = nullptr, *free_t = nullptr, *matchbits = nullptr;
     uint32_t *wants_cnt = nullptr, *inflight = nullptr, *have_epoch = nullptr, *empty_epoch = nullptr;
     LoopCtrl* ctrl = nullptr;
-    uint32_t Wp = 0, S = 0, nLw = 0;
+    uint64_t *hsum = nullptr, *wsum = nullptr;
+    uint32_t Wp = 0, S = 0, nLw = 0, SWp = 0;
     size_t zero_off = 0, zero_bytes = 0;   // have + wants + wants_cnt + ctrl are cleared per run
 };
+
+size_t loop_smem_bytes(uint32_t S, uint32_t SWp) {
+    (void)SWp;
+    return (size_t)((NB * S + 3u) & ~3u) * 4 + (size_t)LIST_CAP * 4;
+}
 
 int work_alloc(const pccl_problem& P, Work& W) {
     const size_t N = P.topo->N, L = P.topo->L, C = P.C;
@@ -509,12 +515,14 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.Wp = (uint32_t)std::max<size_t>(16, align_up(words, 16));   // rows are multiples of 128 bytes
     W.S = (W.Wp / 2 + SEG_U4 - 1) / SEG_U4;
     W.nLw = (uint32_t)((L + 63) / 64);
-    if ((size_t)NB * W.S * 4 > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+    W.SWp = (uint32_t)align_up((W.Wp / 4 + 63) / 64, 2);          // one summary bit per 4-word sector
+    if (loop_smem_bytes(W.S, W.SWp) > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
     Carver c;
     const size_t o_w = c.take(L * 8), o_D = c.take(max_sources * N * 8), o_free = c.take(L * 8),
                  o_mb = c.take((size_t)2 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4);
     W.zero_off = c.cur;
-    const size_t o_have = c.take(N * W.Wp * 8), o_wants = c.take(N * W.Wp * 8), o_wc = c.take(N * 4), o_ctrl = c.take(sizeof(LoopCtrl));
+    const size_t o_have = c.take(N * W.Wp * 8), o_wants = c.take(N * W.Wp * 8), o_hs = c.take(N * W.SWp * 8),
+                 o_ws = c.take(N * W.SWp * 8), o_wc = c.take(N * 4), o_ctrl = c.take(sizeof(LoopCtrl));
     W.zero_bytes = c.cur - W.zero_off;
     int rc = dev_alloc(c.cur, &W.blob);
     if (rc) return rc;
@@ -522,6 +530,7 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.w = (uint64_t*)(b + o_w); W.D = (uint64_t*)(b + o_D); W.free_t = (uint64_t*)(b + o_free);
     W.matchbits = (uint64_t*)(b + o_mb); W.inflight = (uint32_t*)(b + o_inf); W.have_epoch = (uint32_t*)(b + o_he);
     W.empty_epoch = (uint32_t*)(b + o_ee); W.have = (uint64_t*)(b + o_have); W.wants = (uint64_t*)(b + o_wants);
+    W.hsum = (uint64_t*)(b + o_hs); W.wsum = (uint64_t*)(b + o_ws);
     W.wants_cnt = (uint32_t*)(b + o_wc); W.ctrl = (LoopCtrl*)(b + o_ctrl);
     return PCCL_OK;
 }
@@ -550,12 +559,12 @@ int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t 
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_distances<<<NS, 256, smem, st>>>(pv.esrc, pv.edst, W.w, N, L, ph.d_sources, W.D);
     }
-    if (C) k_have<<<(C + 255) / 256, 256, 0, st>>>(ph.d_cond_src, C, W.Wp, W.have);
+    if (C) k_have<<<(C + 255) / 256, 256, 0, st>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
     const uint64_t ND = ph.dests.size();
     if (ND) {
         k_wants<<<(unsigned)((ND + 127) / 128), 128, 0, st>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, ND, pv.esrc, pv.in_off,
-                                                          pv.in_link, W.w, ph.d_sidx, W.D, N, W.Wp, k0, k1, W.wants,
-                                                          W.wants_cnt, &W.ctrl->err);
+                                                          pv.in_link, W.w, ph.d_sidx, W.D, N, W.Wp, W.SWp, k0, k1, W.wants,
+                                                          W.wsum, W.wants_cnt, &W.ctrl->err);
     }
     k_sum_u32<<<1, 1024, 0, st>>>(W.wants_cnt, N, &W.ctrl->wants_total);
     CU(cudaGetLastError());
@@ -569,7 +578,7 @@ int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t 
 }
 
 struct LoopResult {
-    uint64_t total, tmax, events, rows, links, slow;
+    uint64_t total, tmax, events, rows, links, slow, bytes;
     uint32_t grid;
 };
 
@@ -579,10 +588,11 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     const pccl_topology* t = P.topo;
     const PhaseView pv = view_of(t, ph.transposed);
     LoopArgs a;
-    a.N = t->N; a.L = t->L; a.Wp = W.Wp; a.S = W.S; a.nLw = W.nLw; a.flags = flags;
+    a.N = t->N; a.L = t->L; a.Wp = W.Wp; a.S = W.S; a.nLw = W.nLw; a.SWp = W.SWp; a.flags = flags;
     a.k0 = (uint32_t)(seed & 0xFFFFFFFFull); a.k1 = (uint32_t)(seed >> 32);
     a.esrc = pv.esrc; a.edst = pv.edst; a.psrc = t->d_src; a.pdst = t->d_dst;
     a.in_off = pv.in_off; a.in_link = pv.in_link; a.w = W.w; a.have = W.have; a.wants = W.wants;
+    a.hsum = W.hsum; a.wsum = W.wsum;
     a.wants_cnt = W.wants_cnt; a.free_t = W.free_t; a.inflight = W.inflight; a.have_epoch = W.have_epoch;
     a.empty_epoch = W.empty_epoch; a.matchbits = W.matchbits; a.ctrl = W.ctrl; a.out = out; a.t_offset = t_offset;
     cudaStream_t st = G.stream;
@@ -599,7 +609,7 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     struct TraceGuard { void* p; ~TraceGuard() { dev_free(p); } } trace_guard{trace_dev};
     const uint32_t n_init = std::max(std::max(a.L, a.N), std::max(2 * a.nLw, 1u));
     k_loop_init<<<(n_init + 255) / 256, 256, 0, st>>>(a);
-    const size_t smem = (size_t)NB * W.S * 4;
+    const size_t smem = loop_smem_bytes(W.S, W.SWp);
     if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_loop, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_loop, LOOP_THREADS, smem));
@@ -615,6 +625,7 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     if (mb->err) return PCCL_ERR_INTERNAL;
     res->total = mb->total; res->tmax = mb->tmax; res->events = mb->events;
     res->rows = mb->rows_scanned; res->links = mb->links_scanned; res->slow = mb->slow_picks;
+    res->bytes = mb->bytes_requested;
     res->grid = grid;
     if (a.trace) {
         const size_t n = (size_t)std::min<uint64_t>(res->events, a.trace_cap) * TRACE_SLOTS;
@@ -759,6 +770,7 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
         S->stats.rows_scanned += lr.rows;
         S->stats.links_scanned += lr.links;
         S->stats.slow_picks += lr.slow;
+        S->stats.bytes_requested += lr.bytes;
         S->stats.grid_blocks = lr.grid;
         S->stats.row_bytes = (uint64_t)W.Wp * 8;
     }

@@ -28,6 +28,7 @@ constexpr uint64_t T_INF = 0xFFFFFFFFFFFFFFFFull;
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
 constexpr int LOOP_THREADS = 256;  // threads per CTA of the event-loop kernel (= NB warps)
 constexpr int NB = 8;              // in-links of one destination counted in one sweep
+constexpr int LIST_CAP = 2048;     // candidate-sector work list entries per sweep (8 KB of shared memory)
 constexpr int SEG_U4 = 32;         // uint4 per segment (one warp-wide load) = 64 words = 4096 chunks
 
 struct Rec {  // == pccl_transfer_t
@@ -122,11 +123,16 @@ __global__ void k_distances(const uint32_t* __restrict__ esrc, const uint32_t* _
 }
 
 // ---- a2: holdings ------------------------------------------------------------------------------
-__global__ void k_have(const uint32_t* __restrict__ cond_src, uint32_t C, uint32_t Wp,
-                       uint64_t* __restrict__ have) {
+// hsum / wsum: one bit per 32-byte sector (4 words, 256 chunks) of a have / wants row, set while the
+// sector may hold a set bit.  They are a filter only: a sector whose bit is 0 in either row cannot hold a
+// candidate, so the count sweep never requests it.
+__global__ void k_have(const uint32_t* __restrict__ cond_src, uint32_t C, uint32_t Wp, uint32_t SWp,
+                       uint64_t* __restrict__ have, uint64_t* __restrict__ hsum) {
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= C) return;
-    atomicOr((unsigned long long*)&have[(size_t)cond_src[c] * Wp + (c >> 6)], 1ull << (c & 63));
+    const uint32_t s = cond_src[c];
+    atomicOr((unsigned long long*)&have[(size_t)s * Wp + (c >> 6)], 1ull << (c & 63));
+    atomicOr((unsigned long long*)&hsum[(size_t)s * SWp + (c >> 14)], 1ull << ((c >> 8) & 63));
 }
 
 // ---- a2: wants = thin relay tree, one thread per (chunk, dest) pair ----------------------------
@@ -139,8 +145,8 @@ __global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* _
                         const uint32_t* __restrict__ esrc, const uint32_t* __restrict__ in_off,
                         const uint32_t* __restrict__ in_link, const uint64_t* __restrict__ w,
                         const uint32_t* __restrict__ sidx, const uint64_t* __restrict__ D, uint32_t N,
-                        uint32_t Wp, uint32_t k0, uint32_t k1, uint64_t* __restrict__ wants,
-                        uint32_t* __restrict__ wants_cnt, uint32_t* __restrict__ err) {
+                        uint32_t Wp, uint32_t SWp, uint32_t k0, uint32_t k1, uint64_t* __restrict__ wants,
+                        uint64_t* __restrict__ wsum, uint32_t* __restrict__ wants_cnt, uint32_t* __restrict__ err) {
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n_pairs) return;
     const uint32_t c = dchunk[p];
@@ -152,6 +158,7 @@ __global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* _
     while (cur != s) {
         const unsigned long long old = atomicOr((unsigned long long*)&wants[(size_t)cur * Wp + (c >> 6)], bit);
         if (old & bit) break;
+        atomicOr((unsigned long long*)&wsum[(size_t)cur * SWp + (c >> 14)], 1ull << ((c >> 8) & 63));
         atomicAdd(&wants_cnt[cur], 1u);
         const uint64_t dcur = Ds[cur];
         const uint32_t e0 = in_off[cur], e1 = in_off[cur + 1];
@@ -233,6 +240,7 @@ struct LoopCtrl {                 // device-resident control block (zeroed / ini
     unsigned long long rows_scanned;
     unsigned long long links_scanned;
     unsigned long long slow_picks;
+    unsigned long long bytes_requested;
     unsigned long long wants_total;
     uint32_t err;
     uint32_t pad;
@@ -241,6 +249,7 @@ struct LoopCtrl {                 // device-resident control block (zeroed / ini
 struct LoopArgs {
     uint32_t N, L, Wp, S;   // nodes, links, words per padded row, segments per row
     uint32_t nLw;           // words of the per-event matched-link bitmap
+    uint32_t SWp;           // words per row of the sector summaries
     uint32_t flags;
     uint32_t k0, k1;        // Philox key
     const uint32_t* esrc;   // link endpoints in the synthesized direction
@@ -252,6 +261,8 @@ struct LoopArgs {
     const uint64_t* w;
     uint64_t* have;
     uint64_t* wants;
+    uint64_t* hsum;         // [N][SWp] sector summaries of have / wants
+    uint64_t* wsum;
     uint32_t* wants_cnt;
     uint64_t* free_t;
     uint32_t* inflight;
@@ -265,7 +276,8 @@ struct LoopArgs {
     uint32_t trace_cap;     // events the trace buffer holds
 };
 
-constexpr int TRACE_SLOTS = 8;   // loop top, links phase, barrier 1, in-link list, count, pick, commit, barrier 2
+constexpr int TRACE_SLOTS = 12;  // 0 loop top, 1 links phase, 2 barrier 1, 3 in-link list, 4 count, 5 pick, 6 commit,
+                                 // 7 barrier 2, 8 summary scan, 9 work list, 10 unused, 11 unused
 __device__ __forceinline__ void trace_stamp(const LoopArgs& a, uint32_t step, int slot) {
     if (a.trace != nullptr && blockIdx.x == 0 && threadIdx.x == 0 && step < a.trace_cap) {
         unsigned long long ns;
@@ -293,6 +305,7 @@ __global__ void k_loop_init(LoopArgs a) {
         a.ctrl->rows_scanned = 0;
         a.ctrl->links_scanned = 0;
         a.ctrl->slow_picks = 0;
+        a.ctrl->bytes_requested = 0;
     }
 }
 
@@ -357,6 +370,7 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
         if (ok && c != NONE32 && f == t) {   // arrival: forwardable from t on
             const uint32_t d = a.edst[l];
             atomicOr((unsigned long long*)&a.have[(size_t)d * a.Wp + (c >> 6)], 1ull << (c & 63));
+            atomicOr((unsigned long long*)&a.hsum[(size_t)d * a.SWp + (c >> 14)], 1ull << ((c >> 8) & 63));
             stcg32(a.inflight + l, NONE32);
             stcg32(a.have_epoch + d, step + 1);
         }
@@ -370,14 +384,18 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
 // ---- P2: match one destination (a4..a8) -----------------------------------------------------------------
 struct CtaScratch {
     uint32_t act[32];     // active in-links of the current window, ascending link id
+    uint32_t src[32];     // their sources
+    uint64_t actw[32];    // their costs
+    uint32_t sempty[NB];  // speculative pick j empties its wants sector
     uint32_t nact;
     uint32_t wc;          // chunks this destination still wants
+    uint32_t wtot[LOOP_THREADS / 32];   // block scan scratch
     uint32_t spec[NB];    // speculative pick of each in-link of the sweep (NONE32: no candidate)
     uint32_t claimed[NB]; // chunks claimed so far in this sweep (warp 0 only)
 };
 
 struct LoopStats {
-    unsigned long long rows, links, slow;
+    unsigned long long rows, links, slow, bytes;
 };
 
 // The k-th candidate (0-based, ascending chunk id) of link-row `hrow` AND wants-row `wrow`, given the
@@ -385,7 +403,7 @@ struct LoopStats {
 // made earlier in the same sweep); cj must already be net of them.  Whole warp; returns the chunk id.
 __device__ __forceinline__ uint32_t kth_candidate(const uint32_t* cj, uint32_t S, uint32_t Q, const uint4* hrow,
                                                   const uint4* wrow, uint32_t rem, const uint32_t* excl,
-                                                  uint32_t nex, uint32_t lane) {
+                                                  uint32_t nex, uint32_t lane, bool& sector_empty) {
     uint32_t seg = 0;
     for (uint32_t sb = 0; sb < S; sb += 32) {
         const uint32_t x = (sb + lane < S) ? cj[sb + lane] : 0u;
@@ -401,14 +419,15 @@ __device__ __forceinline__ uint32_t kth_candidate(const uint32_t* cj, uint32_t S
         rem -= tot;
     }
     const uint32_t q = seg * SEG_U4 + lane;
-    uint4 m4 = make_uint4(0, 0, 0, 0);
-    if (q < Q) m4 = and128(ldcg128(hrow + q), ldcg128(wrow + q));
+    uint4 m4 = make_uint4(0, 0, 0, 0), wv = m4;
+    if (q < Q) { wv = ldcg128(wrow + q); m4 = and128(ldcg128(hrow + q), wv); }
     for (uint32_t i = 0; i < nex; ++i) {
         const uint32_t c = excl[i];
         if ((c >> 7) == q) {
             const uint32_t b = c & 127u;
             const uint32_t msk = ~(1u << (b & 31));
-            if (b < 32) m4.x &= msk; else if (b < 64) m4.y &= msk; else if (b < 96) m4.z &= msk; else m4.w &= msk;
+            if (b < 32) { m4.x &= msk; wv.x &= msk; } else if (b < 64) { m4.y &= msk; wv.y &= msk; }
+            else if (b < 96) { m4.z &= msk; wv.z &= msk; } else { m4.w &= msk; wv.w &= msk; }
         }
     }
     const uint32_t pc = popc128(m4);
@@ -417,7 +436,15 @@ __device__ __forceinline__ uint32_t kth_candidate(const uint32_t* cj, uint32_t S
     const int fl = (__ffs(mm) - 1) & 31;
     const uint32_t rem2 = rem - __shfl_sync(0xFFFFFFFFu, incl - pc, fl);
     uint32_t c = NONE32;
-    if ((int)lane == fl && mm != 0) c = q * 128u + kth_bit128(m4, rem2);
+    if ((int)lane == fl && mm != 0) {
+        const uint32_t b = kth_bit128(m4, rem2);
+        c = q * 128u + b;
+        const uint32_t msk = ~(1u << (b & 31));
+        if (b < 32) wv.x &= msk; else if (b < 64) wv.y &= msk; else if (b < 96) wv.z &= msk; else wv.w &= msk;
+    }
+    // the sector (this lane's 16 bytes and its pair lane's) holds no other wanted chunk
+    const uint32_t z = (wv.x | wv.y | wv.z | wv.w) == 0u;
+    sector_empty = (__shfl_sync(0xFFFFFFFFu, z, fl) & __shfl_sync(0xFFFFFFFFu, z, fl ^ 1)) != 0u;
     return __shfl_sync(0xFFFFFFFFu, c, fl);
 }
 
@@ -428,27 +455,45 @@ __device__ __forceinline__ uint32_t warp_sum_counts(const uint32_t* cj, uint32_t
 }
 
 // a8: link l carries chunk c over [t, t + w_l); destination v no longer wants c
-__device__ __forceinline__ uint64_t commit_claim(const LoopArgs& a, uint32_t v, uint32_t l, uint32_t c, uint32_t step,
-                                                 uint64_t t) {
-    const uint64_t te = t + a.w[l];
+__device__ __forceinline__ uint64_t commit_claim(const LoopArgs& a, uint32_t v, uint32_t l, uint64_t wl, uint32_t c,
+                                                 bool sector_empty, uint32_t step, uint64_t t) {
+    const uint64_t te = t + wl;
     atomicAnd((unsigned long long*)&a.wants[(size_t)v * a.Wp + (c >> 6)], ~(1ull << (c & 63)));
+    // the pick saw no other wanted chunk in c's 32-byte sector: drop it from the wants summary.  (Two claims
+    // of one sweep in one sector each see the other's bit and leave the summary bit set: a wasted load later,
+    // never a wrong result -- the summaries are a filter only.)
+    if (sector_empty) atomicAnd((unsigned long long*)&a.wsum[(size_t)v * a.SWp + (c >> 14)], ~(1ull << ((c >> 8) & 63)));
     stcg32(a.inflight + l, c);
     stcg64(a.free_t + l, te);
     atomicOr((unsigned long long*)&a.matchbits[(size_t)(step & 1) * a.nLw + (l >> 6)], 1ull << (l & 63));
     return te;
 }
 
+// static per-destination tables kept in shared memory for the destinations a CTA serves first
+constexpr int DEST_CACHE = 2;
+struct DestCache {
+    uint32_t n_in;        // NONE32: not cached (more than 32 in-links)
+    uint32_t link[32];
+    uint32_t src[32];
+    uint64_t w[32];
+};
+
 __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v, uint32_t step, uint64_t t,
-                                                  uint32_t* cnt, CtaScratch& sh, LoopStats& st) {
+                                                  uint32_t* cnt, uint32_t* list, CtaScratch& sh, LoopStats& st,
+                                                  const DestCache* dc) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t Q = a.Wp >> 1;  // uint4 per row
+    const uint32_t SWp = a.SWp;
     const uint32_t S = a.S;
     const uint4* have4 = reinterpret_cast<const uint4*>(a.have);
     const uint4* wrow = reinterpret_cast<const uint4*>(a.wants) + (size_t)v * Q;
-    const uint32_t e0 = a.in_off[v], e1 = a.in_off[v + 1];
-    if (tid == 0) sh.wc = ldcg32(a.wants_cnt + v);
-    __syncthreads();
-    const uint32_t wc_start = sh.wc;
+    uint32_t e0 = 0, e1 = 0;
+    if (dc != nullptr) e1 = dc->n_in; else { e0 = a.in_off[v]; e1 = a.in_off[v + 1]; }
+    uint32_t wc_start = 0;               // warp 0 only
+    if (warp == 0) {
+        wc_start = ldcg32(a.wants_cnt + v);
+        if (lane == 0) sh.wc = wc_start;   // the other warps read it after the barrier below
+    }
     uint64_t mymin = T_INF, mymax = 0;   // meaningful in warp 0 only
     const bool idle_skip = !(a.flags & 2u);
 
@@ -456,24 +501,29 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
         // a4: active in-links of this window, ascending link id
         if (warp == 0) {
             const uint32_t e = eb + lane;
-            const uint32_t wc = sh.wc;
+            const uint32_t wc = (eb == e0) ? wc_start : sh.wc;
             bool active = false;
-            uint32_t l = 0;
+            uint32_t l = 0, u = 0;
             if (e < e1) {
-                l = a.in_link[e];
+                if (dc != nullptr) { l = dc->link[e]; u = dc->src[e]; } else { l = a.in_link[e]; u = a.esrc[l]; }
+                // one round trip: the three loads are independent
                 const uint64_t f = ldcg64(a.free_t + l);
+                const uint32_t ee = ldcg32(a.empty_epoch + l);
+                const uint32_t he = ldcg32(a.have_epoch + u);
                 if (f > t) {
                     mymin = min(mymin, f);
                 } else if (wc > 0) {
-                    active = true;
-                    if (idle_skip) {   // nothing arrived at the source since this link last found no candidate
-                        const uint32_t ee = ldcg32(a.empty_epoch + l);
-                        if (ee != 0 && ee >= ldcg32(a.have_epoch + a.esrc[l])) active = false;
-                    }
+                    // idle filter: nothing arrived at the source since this link last found no candidate
+                    active = !(idle_skip && ee != 0 && ee >= he);
                 }
             }
             const uint32_t m = __ballot_sync(0xFFFFFFFFu, active);
-            if (active) sh.act[__popc(m & ((1u << lane) - 1u))] = l;
+            if (active) {
+                const uint32_t k = __popc(m & ((1u << lane) - 1u));
+                sh.act[k] = l;
+                sh.src[k] = u;
+                sh.actw[k] = (dc != nullptr) ? dc->w[e] : a.w[l];
+            }
             if (lane == 0) sh.nact = __popc(m);
         }
         __syncthreads();
@@ -482,29 +532,100 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
         for (uint32_t b0 = 0; b0 < nact; b0 += NB) {
             if (sh.wc == 0) break;   // CTA-uniform: sh.wc only changes between the barriers below
             const uint32_t nb = min((uint32_t)NB, nact - b0);
-            // a5: candidate counts per 64-word segment for nb in-links in one sweep of wants[v]
+            // a5: candidate counts per 64-word segment.  Only sectors whose summary bit is set in BOTH the
+            // wants row and the source row can hold a candidate.  (1) AND the summary rows; (2) expand the set
+            // bits into a work list of (in-link, sector) items in shared memory (block-wide scan); (3) all
+            // threads stride the list: two 128-bit loads of the source sector, two of the wants sector, AND,
+            // popcount, shared-memory atomicAdd into the segment's counter.  Rows too dense for the list
+            // (more than LIST_CAP candidate sectors) take the plain dense sweep instead.
             {
-                size_t hoff[NB];
-#pragma unroll
-                for (int j = 0; j < NB; ++j) hoff[j] = (size_t)a.esrc[sh.act[b0 + (j < (int)nb ? j : 0)]] * Q;
-                for (uint32_t qb = warp * 32; qb < Q; qb += blockDim.x) {
-                    const uint32_t q = qb + lane;
-                    const bool ok = q < Q;
-                    uint4 wv = make_uint4(0, 0, 0, 0);
-                    uint4 h[NB];
-                    if (ok) wv = ldcg128(wrow + q);
-#pragma unroll
-                    for (int j = 0; j < NB; ++j) {
-                        h[j] = make_uint4(0, 0, 0, 0);
-                        if (j < (int)nb && ok) h[j] = ldcg128(have4 + hoff[j] + q);
+                const uint64_t* ws = a.wsum + (size_t)v * SWp;
+                const uint32_t nitems = nb * SWp;
+                uint32_t total = 0;
+                for (uint32_t base = 0; base < nitems; base += LOOP_THREADS) {
+                    const uint32_t it = base + tid;
+                    unsigned long long m = 0;
+                    uint32_t j = 0, i = 0;
+                    if (it < nitems) {
+                        j = it / SWp;
+                        i = it - j * SWp;
+                        m = ldcg64(ws + i) & ldcg64(a.hsum + (size_t)sh.src[b0 + j] * SWp + i);
                     }
+                    const uint32_t pc = __popcll(m);
+                    const uint32_t incl = warp_incl_scan(pc, lane);
+                    if (lane == 31) sh.wtot[warp] = incl;
+                    __syncthreads();
+                    uint32_t pre = 0, blk = 0;
 #pragma unroll
-                    for (int j = 0; j < NB; ++j) {
-                        if (j < (int)nb) {
-                            const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)popc128(and128(h[j], wv)));
-                            if (lane == 0) cnt[j * S + (qb >> 5)] = tot;
+                    for (int w2 = 0; w2 < LOOP_THREADS / 32; ++w2) {
+                        const uint32_t x = sh.wtot[w2];
+                        pre += (w2 < (int)warp) ? x : 0u;
+                        blk += x;
+                    }
+                    uint32_t off = total + pre + incl - pc;
+                    while (m) {
+                        const uint32_t b = __ffsll((long long)m) - 1;
+                        m &= m - 1;
+                        if (off < LIST_CAP) list[off] = (j << 28) | (i * 64u + b);
+                        ++off;
+                    }
+                    total += blk;
+                    trace_stamp(a, step, 8);
+                    __syncthreads();
+                }
+                for (uint32_t x = tid; x < nb * S; x += LOOP_THREADS) cnt[x] = 0;
+                __syncthreads();
+                trace_stamp(a, step, 9);
+                if (!(a.flags & 16u) && total <= LIST_CAP && total * 2u <= (nb + 1) * (Q >> 1)) {   // fewer sectors than the dense sweep
+                    // a lane pair per item: even lane the first 16 bytes of the sector, odd lane the second, so
+                    // that one warp-wide load touches 16 whole sectors; four items in flight per lane
+                    const uint32_t half = tid & 1u;
+                    constexpr uint32_t PAIRS = LOOP_THREADS / 2, UNR = 4;
+                    for (uint32_t idx = tid >> 1; idx < total; idx += UNR * PAIRS) {
+                        uint32_t jj[UNR], ss[UNR];
+                        uint4 hv[UNR], wv[UNR];
+#pragma unroll
+                        for (uint32_t k = 0; k < UNR; ++k) {
+                            const uint32_t ix = idx + k * PAIRS;
+                            hv[k] = make_uint4(0, 0, 0, 0);
+                            wv[k] = hv[k];
+                            jj[k] = 0; ss[k] = 0;
+                            if (ix < total) {
+                                const uint32_t e = list[ix];
+                                jj[k] = e >> 28;
+                                ss[k] = e & 0x0FFFFFFFu;
+                                hv[k] = ldcg128(have4 + (size_t)sh.src[b0 + jj[k]] * Q + 2u * ss[k] + half);
+                                wv[k] = ldcg128(wrow + 2u * ss[k] + half);
+                            }
+                        }
+#pragma unroll
+                        for (uint32_t k = 0; k < UNR; ++k) {
+                            const uint32_t pcs = popc128(and128(hv[k], wv[k]));
+                            if (pcs) atomicAdd(&cnt[jj[k] * S + (ss[k] >> 4)], pcs);
                         }
                     }
+                    if (tid == 0) st.bytes += (unsigned long long)total * 64u + (unsigned long long)nitems * 16u;
+                } else {
+                    // dense sweep: every lane one uint4 of the wants row and of each source row
+                    size_t hoff[NB];
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) hoff[j] = (size_t)sh.src[b0 + (j < (int)nb ? j : 0)] * Q;
+                    for (uint32_t qb = warp * 32; qb < Q; qb += blockDim.x) {
+                        const uint32_t q = qb + lane;
+                        const bool ok = q < Q;
+                        uint4 wv = make_uint4(0, 0, 0, 0);
+                        if (ok) wv = ldcg128(wrow + q);
+#pragma unroll
+                        for (int j = 0; j < NB; ++j) {
+                            if (j < (int)nb) {
+                                uint4 h = make_uint4(0, 0, 0, 0);
+                                if (ok) h = ldcg128(have4 + hoff[j] + q);
+                                const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)popc128(and128(h, wv)));
+                                if (lane == 0) cnt[j * S + (qb >> 5)] = tot;
+                            }
+                        }
+                    }
+                    if (tid == 0) st.bytes += (unsigned long long)(nb + 1) * a.Wp * 8u + (unsigned long long)nitems * 16u;
                 }
             }
             __syncthreads();
@@ -516,12 +637,17 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 const uint32_t* cj = cnt + warp * S;
                 const uint32_t n = warp_sum_counts(cj, S, lane);
                 uint32_t c = NONE32;
+                bool sem = false;
                 if (n != 0) {
                     const uint32_t r = philox_draw((uint32_t)t, (uint32_t)(t >> 32), l, 0u, a.k0, a.k1);
-                    c = kth_candidate(cj, S, Q, have4 + (size_t)a.esrc[l] * Q, wrow, __umulhi(r, n), nullptr, 0, lane);
+                    c = kth_candidate(cj, S, Q, have4 + (size_t)sh.src[b0 + warp] * Q, wrow, __umulhi(r, n), nullptr, 0, lane, sem);
                     if (c == NONE32 && lane == 0) atomicOr(&a.ctrl->err, 4u);   // cannot happen
                 }
-                if (lane == 0) sh.spec[warp] = c;
+                if (lane == 0) {
+                    sh.spec[warp] = c;
+                    sh.sempty[warp] = sem;
+                    if (n != 0) st.bytes += 2u * SEG_U4 * 16u;   // one segment of the source row and of the wants row
+                }
             }
             __syncthreads();
             trace_stamp(a, step, 5);
@@ -536,7 +662,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     if (i < j) {
                         const uint32_t ci = sh.spec[i];
                         if (ci != NONE32 && cnt[j * S + (ci >> 12)] != 0) {
-                            const uint32_t u = a.esrc[sh.act[b0 + j]];
+                            const uint32_t u = sh.src[b0 + j];
                             if ((ldcg64(a.have + (size_t)u * a.Wp + (ci >> 6)) >> (ci & 63)) & 1ull) bad |= 1u << j;
                         }
                     }
@@ -551,7 +677,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     const uint32_t cm = __ballot_sync(0xFFFFFFFFu, c != NONE32);
                     if (lane < first_bad) {
                         if (c != NONE32) {
-                            const uint64_t te = commit_claim(a, v, l, c, step, t);
+                            const uint64_t te = commit_claim(a, v, l, sh.actw[b0 + lane], c, sh.sempty[lane] != 0u, step, t);
                             mymin = min(mymin, te);
                             mymax = max(mymax, te);
                             sh.claimed[__popc(cm & ((1u << lane) - 1u))] = c;
@@ -567,7 +693,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 for (uint32_t j = first_bad; j < nb && wc > 0; ++j) {
                     if (lane == 0) ++st.slow;
                     const uint32_t l = sh.act[b0 + j];
-                    const uint32_t u = a.esrc[l];
+                    const uint32_t u = sh.src[b0 + j];
                     uint32_t* cj = cnt + j * S;
                     if (lane == 0) {
                         for (uint32_t i = 0; i < ncl; ++i) {
@@ -582,14 +708,15 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                         continue;
                     }
                     const uint32_t r = philox_draw((uint32_t)t, (uint32_t)(t >> 32), l, 0u, a.k0, a.k1);
-                    const uint32_t c = kth_candidate(cj, S, Q, have4 + (size_t)u * Q, wrow, __umulhi(r, n), sh.claimed, ncl, lane);
+                    bool sem = false;
+                    const uint32_t c = kth_candidate(cj, S, Q, have4 + (size_t)u * Q, wrow, __umulhi(r, n), sh.claimed, ncl, lane, sem);
                     if (c == NONE32) {   // cannot happen; fail loudly instead of corrupting
                         if (lane == 0) atomicOr(&a.ctrl->err, 4u);
                         continue;
                     }
                     if (lane == 0) {
                         sh.claimed[ncl] = c;
-                        const uint64_t te = commit_claim(a, v, l, c, step, t);
+                        const uint64_t te = commit_claim(a, v, l, sh.actw[b0 + j], c, sem, step, t);
                         mymin = min(mymin, te);
                         mymax = max(mymax, te);
                     }
@@ -598,7 +725,8 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     __syncwarp();
                 }
                 if (lane == 0) sh.wc = wc;
-                __threadfence();
+                // another sweep of this destination follows: its loads must see the wants bits just cleared
+                if (b0 + NB < nact || eb + 32 < e1) __threadfence();
             }
             __syncthreads();
         }
@@ -623,10 +751,26 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
 }
 
 __global__ void __launch_bounds__(LOOP_THREADS, 4) k_loop(const LoopArgs a) {
-    extern __shared__ uint32_t cnt[];   // [NB][S] candidate counts per segment
+    extern __shared__ __align__(16) uint32_t cnt[];   // [NB][S] candidate counts per segment, then the work list
+    uint32_t* list = cnt + ((NB * a.S + 3u) & ~3u);   // [LIST_CAP] (in-link << 28 | sector)
     __shared__ CtaScratch sh;
+    __shared__ DestCache dcache[DEST_CACHE];
     cg::grid_group grid = cg::this_grid();
-    LoopStats st = {0, 0, 0};
+    for (uint32_t k = threadIdx.x >> 5; k < DEST_CACHE; k += LOOP_THREADS / 32) {   // warp k fills slot k
+        const uint32_t v = blockIdx.x + k * gridDim.x, lane = threadIdx.x & 31;
+        if (v < a.N) {
+            const uint32_t e0 = a.in_off[v], n = a.in_off[v + 1] - e0;
+            if (lane == 0) dcache[k].n_in = (n <= 32) ? n : NONE32;
+            if (n <= 32 && lane < n) {
+                const uint32_t l = a.in_link[e0 + lane];
+                dcache[k].link[lane] = l;
+                dcache[k].src[lane] = a.esrc[l];
+                dcache[k].w[lane] = a.w[l];
+            }
+        }
+    }
+    __syncthreads();
+    LoopStats st = {0, 0, 0, 0};
     uint32_t step = 0;
     uint64_t t = 0;
     uint64_t emit_base = 0;
@@ -638,13 +782,23 @@ __global__ void __launch_bounds__(LOOP_THREADS, 4) k_loop(const LoopArgs a) {
         trace_stamp(a, step, 1);
         grid.sync();
         trace_stamp(a, step, 2);
-        for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x) match_destination(a, v, step, t, cnt, sh, st);
+        {
+            uint32_t k = 0;
+            for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x, ++k)
+                match_destination(a, v, step, t, cnt, list, sh, st,
+                                  (k < DEST_CACHE && dcache[k].n_in != NONE32) ? &dcache[k] : nullptr);
+        }
         trace_stamp(a, step, 6);
         grid.sync();
         trace_stamp(a, step, 7);
         t = ldcg64((const uint64_t*)&a.ctrl->tnext[(step + 1) % 3]);
         ++step;
         if (t == T_INF) break;
+    }
+    {   // bytes requested: every lane counted its own sectors
+        unsigned long long b = st.bytes;
+        for (int o = 16; o; o >>= 1) b += __shfl_xor_sync(0xFFFFFFFFu, b, o);
+        if ((threadIdx.x & 31) == 0 && b) atomicAdd(&a.ctrl->bytes_requested, b);
     }
     if (threadIdx.x == 0) {   // warp 0 lane 0 holds this CTA's counters
         if (st.rows) atomicAdd(&a.ctrl->rows_scanned, st.rows);

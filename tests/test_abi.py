@@ -46,7 +46,7 @@ def test_binding_is_marshalling_only():
 
 def test_struct_layouts(pk):
     assert pk.LINK_DT.itemsize == 24 and pk.PAIR_DT.itemsize == 8 and pk.TRANSFER_DT.itemsize == 32
-    assert C.sizeof(pk.pccl_stats_t) == 7 * 8 + 3 * 4 + 2 * 4 + 4   # tail padding to 8
+    assert C.sizeof(pk.pccl_stats_t) == 8 * 8 + 3 * 4 + 2 * 4 + 4   # tail padding to 8
 
 
 def test_topology_validation(pk):

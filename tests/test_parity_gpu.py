@@ -241,3 +241,28 @@ def test_config4_full_size_bit_exact(pk):
     assert s.size == 1_572_864 == o.wants_total     # sum of hop distances, closed form
     assert_same(p, s, o)
     checker.check_structure(p, s.transfers)
+
+
+@pytest.mark.parametrize("maker", [wl.config2, wl.config4_small, wl.config5_small], ids=lambda m: m.__name__)
+def test_dense_sweep_and_sector_list_agree(pk, maker):
+    """the sector work list (default) and the plain dense row sweep are two ways to the same counts."""
+    p = maker(2)
+    o = oracle.synthesize(*p.args())
+    d = gpu_run(pk, p, pk.PCCL_FLAG_DENSE_SWEEP)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE)
+    assert_same(p, d, o)
+    assert_same(p, s, o)
+    assert d.stats["rows_scanned"] == s.stats["rows_scanned"]
+    assert d.stats["bytes_requested"] >= s.stats["bytes_requested"]
+
+
+@pytest.mark.slow
+def test_config5_full_size_bit_exact(pk):
+    """BASELINE.json configs[4] at full size: 32x32 torus, 512-member group, Zipf All-to-Allv
+    (483,889 chunks, 7.76 M transfers).  The oracle needs a few minutes on one core."""
+    p = wl.config5(0)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE)
+    assert s.size == 7_761_800
+    o = oracle.synthesize(*p.args())
+    assert_same(p, s, o)
+    checker.check_structure(p, s.transfers)
