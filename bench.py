@@ -258,13 +258,66 @@ def run_ours(args):
             f = ln.split()
             if len(f) == 2 and f[0] == f"config{args.config}":
                 traffic = int(f[1])
+    req_bytes = stats["bytes_requested"]
     roofline = {"bound": "hbm", "kernel": "k_loop", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": loop_avg_ms,
                 "kernel_share_of_step": loop_avg_ms / (tot_ms / args.steps),
                 "frac_of_8TBps_nominal": achieved / 8000.0,
-                "note": "bytes = rows_scanned x row_bytes counted by the kernel itself; at config 4 both bitmaps "
-                        "(2 x 16.8 MB) fit in the 126 MB L2, so DRAM traffic is far below the algorithmic bytes"}
+                "requested_bytes_per_launch": req_bytes,
+                "requested_gbs": req_bytes / (loop_avg_ms * 1e-3) / 1e9,
+                "note": "algorithmic bytes = SURVEY 8(d): padded row bytes x (destinations + in-links swept), counted "
+                        "by the kernel (rows_scanned x row_bytes). The default kernel requests fewer: sector "
+                        "summaries rule out 32-byte sectors that cannot hold a candidate (requested_bytes). At "
+                        "config 4 both bitmaps (2 x 16.8 MB) sit in the 126 MB L2, so DRAM traffic is far below "
+                        "either figure; dense_sweep below is the same kernel forced to sweep whole rows"}
+    # the plain bitmap scan (PCCL_FLAG_DENSE_SWEEP): same kernel, whole rows, timed the same way
+    dense_ms = []
+    for i in range(2 + min(args.steps, 5)):
+        flush.zero_()
+        sd = prob.synthesize(seed, flags | pk.PCCL_FLAG_DENSE_SWEEP)
+        std = sd.stats
+        sd.close()
+        if i >= 2:
+            dense_ms.append(std["loop_ms"])
+    dms = sum(dense_ms) / len(dense_ms)
+    roofline["dense_sweep"] = {"kernel_ms": dms, "requested_bytes_per_launch": std["bytes_requested"],
+                               "achieved": std["bytes_requested"] / (dms * 1e-3) / 1e9, "unit": "GB/s",
+                               "frac": std["bytes_requested"] / (dms * 1e-3) / 1e9 / peak}
+
+    # ---- the other BASELINE.json configs, same path, resident inputs (context; parity is in tests/) ---
+    per_config = {}
+    if not args.no_other_configs:
+        for cfg in (1, 2, 3, 5):
+            if cfg == args.config:
+                continue
+            pc = workload(cfg, 0)
+            tc = pk.Topology(pc.n_npus, pc.links)
+            prc = pk.Problem(tc, pc.group, pc.n_chunks, pc.pre, pc.post, pc.chunk_bytes)
+            prc.upload()
+            ms_l, stc, sc = [], None, None
+            for i in range(4):
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                sc = prc.synthesize(0, flags)
+                e1.record()
+                e1.synchronize()
+                if i >= 1:
+                    ms_l.append(e0.elapsed_time(e1))
+                stc, mc, tcps = sc.stats, sc.size, sc.time_ps
+                sc.close()
+            ms_c = sorted(ms_l)[len(ms_l) // 2]
+            algb = stc["rows_scanned"] * stc["row_bytes"]
+            per_config[f"config{cfg}"] = {
+                "workload": pc.name, "synthesis_ms": ms_c, "loop_ms": stc["loop_ms"], "transfers": mc,
+                "matches_per_s": mc / (ms_c * 1e-3), "events": stc["events"], "schedule_time_ps": tcps,
+                "algorithmic_gbs": algb / (stc["loop_ms"] * 1e-3) / 1e9 if stc["loop_ms"] else None,
+                "frac_of_measured_hbm": (algb / (stc["loop_ms"] * 1e-3) / 1e9 / peak) if stc["loop_ms"] else None,
+                "requested_bytes": stc["bytes_requested"],
+                "roofline_note": "rows of 128 B: launch/sync-bound, roofline n/a" if stc["row_bytes"] <= 256 else "bitmap scan"}
+            prc.close()
+            tc.close()
 
     # ---- cpu baseline: the oracle on this box's host cores ----------------------------------------
     cpu = None
@@ -294,7 +347,7 @@ def run_ours(args):
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": 1e3 * e2e_tot / args.steps},
             "gpu_launches": KERNELS_PER_STEP_COPY * args.steps,
-            "roofline": roofline, "cpu_baseline": cpu, "clocks": clk.summary(),
+            "roofline": roofline, "cpu_baseline": cpu, "clocks": clk.summary(), "per_config": per_config,
             "paper_context": "PCCL reports 11.68 min for 512-NPU All-to-All synthesis, hardware not stated "
                              "(PAPER.md:9, :388); a different procedure, context only",
             "wall_s_timed_region": wall}
@@ -312,6 +365,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -164,8 +164,10 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
 #define PCCL_FLAG_KEEP_ON_DEVICE 1u /* do not download the transfers until they are asked for */
 #define PCCL_FLAG_NO_IDLE_SKIP 2u   /* rescan idle links every event (debug / measurement) */
 #define PCCL_FLAG_TIME_LOOP 4u      /* record CUDA events around the event loop (stats) */
-#define PCCL_FLAG_DENSE_SWEEP 16u   /* count candidates by sweeping whole rows, never the sector work list
-                                       (the plain bitmap scan; measurement of the memory-bound form) */
+#define PCCL_FLAG_RESCAN 32u        /* recount every free link's candidates at every event from the bitmaps
+                                       (sector work list), instead of keeping the counts current */
+#define PCCL_FLAG_DENSE_SWEEP 16u   /* implies RESCAN, and recounts by sweeping whole rows, never the sector
+                                       work list (the plain bitmap scan: the memory-bound form) */
 #define PCCL_FLAG_TRACE 8u          /* record per-event phase timestamps (pccl_schedule_trace) */
 
 /* Steps A..F on the GPU for one seed.  Errors: UNREACHABLE, CUDA, NOMEM, INTERNAL. */

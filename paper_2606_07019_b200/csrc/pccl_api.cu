@@ -135,6 +135,9 @@ struct pccl_topology {
     void* blob = nullptr;
     uint32_t *d_src = nullptr, *d_dst = nullptr, *d_in_off = nullptr, *d_in_link = nullptr,
              *d_out_off = nullptr, *d_out_link = nullptr;
+    // per entry of the out / in tables: the far end; per link: where the tables of its far node start
+    uint32_t *d_out_far = nullptr, *d_in_far = nullptr, *d_lo_off_n = nullptr, *d_lo_deg_n = nullptr,
+             *d_lo_off_t = nullptr, *d_lo_deg_t = nullptr;
     uint64_t *d_alpha = nullptr, *d_bpp = nullptr;
 };
 
@@ -254,7 +257,9 @@ int topo_upload(pccl_topology* t) {
     const size_t N = t->N, L = t->L;
     Carver c;
     const size_t o_src = c.take(L * 4), o_dst = c.take(L * 4), o_alpha = c.take(L * 8), o_bpp = c.take(L * 8),
-                 o_ino = c.take((N + 1) * 4), o_inl = c.take(L * 4), o_outo = c.take((N + 1) * 4), o_outl = c.take(L * 4);
+                 o_ino = c.take((N + 1) * 4), o_inl = c.take(L * 4), o_outo = c.take((N + 1) * 4), o_outl = c.take(L * 4),
+                 o_of = c.take(L * 4), o_if = c.take(L * 4), o_lon = c.take(L * 4), o_ldn = c.take(L * 4),
+                 o_lot = c.take(L * 4), o_ldt = c.take(L * 4);
     std::vector<unsigned char> h(c.cur ? c.cur : 256, 0);
     for (size_t l = 0; l < L; ++l) {
         ((uint32_t*)(h.data() + o_src))[l] = t->links[l].src;
@@ -268,6 +273,17 @@ int topo_upload(pccl_topology* t) {
         memcpy(h.data() + o_inl, t->in_link.data(), L * 4);
         memcpy(h.data() + o_outl, t->out_link.data(), L * 4);
     }
+    for (size_t e = 0; e < L; ++e) {
+        ((uint32_t*)(h.data() + o_of))[e] = t->links[t->out_link[e]].dst;
+        ((uint32_t*)(h.data() + o_if))[e] = t->links[t->in_link[e]].src;
+    }
+    for (size_t l = 0; l < L; ++l) {
+        const uint32_t d = t->links[l].dst, sN = t->links[l].src;
+        ((uint32_t*)(h.data() + o_lon))[l] = t->out_off[d];
+        ((uint32_t*)(h.data() + o_ldn))[l] = t->out_off[d + 1] - t->out_off[d];
+        ((uint32_t*)(h.data() + o_lot))[l] = t->in_off[sN];          // transposed view: far node = src, its "out" = in
+        ((uint32_t*)(h.data() + o_ldt))[l] = t->in_off[sN + 1] - t->in_off[sN];
+    }
     void* blob = nullptr;
     rc = dev_alloc(h.size(), &blob);
     if (rc) return rc;
@@ -279,6 +295,9 @@ int topo_upload(pccl_topology* t) {
     }
     unsigned char* b = (unsigned char*)blob;
     t->blob = blob;
+    t->d_out_far = (uint32_t*)(b + o_of); t->d_in_far = (uint32_t*)(b + o_if);
+    t->d_lo_off_n = (uint32_t*)(b + o_lon); t->d_lo_deg_n = (uint32_t*)(b + o_ldn);
+    t->d_lo_off_t = (uint32_t*)(b + o_lot); t->d_lo_deg_t = (uint32_t*)(b + o_ldt);
     t->d_src = (uint32_t*)(b + o_src); t->d_dst = (uint32_t*)(b + o_dst);
     t->d_alpha = (uint64_t*)(b + o_alpha); t->d_bpp = (uint64_t*)(b + o_bpp);
     t->d_in_off = (uint32_t*)(b + o_ino); t->d_in_link = (uint32_t*)(b + o_inl);
@@ -498,6 +517,7 @@ struct Work {   // device workspace of one phase
     uint32_t *wants_cnt = nullptr, *inflight = nullptr, *have_epoch = nullptr, *empty_epoch = nullptr;
     LoopCtrl* ctrl = nullptr;
     uint64_t *hsum = nullptr, *wsum = nullptr;
+    uint32_t *gcnt = nullptr, *gtot = nullptr;
     uint32_t Wp = 0, S = 0, nLw = 0, SWp = 0;
     size_t zero_off = 0, zero_bytes = 0;   // have + wants + wants_cnt + ctrl are cleared per run
 };
@@ -519,7 +539,8 @@ int work_alloc(const pccl_problem& P, Work& W) {
     if (loop_smem_bytes(W.S, W.SWp) > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
     Carver c;
     const size_t o_w = c.take(L * 8), o_D = c.take(max_sources * N * 8), o_free = c.take(L * 8),
-                 o_mb = c.take((size_t)2 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4);
+                 o_mb = c.take((size_t)2 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4),
+                 o_gc = c.take(L * W.S * 4), o_gt = c.take(L * 4);
     W.zero_off = c.cur;
     const size_t o_have = c.take(N * W.Wp * 8), o_wants = c.take(N * W.Wp * 8), o_hs = c.take(N * W.SWp * 8),
                  o_ws = c.take(N * W.SWp * 8), o_wc = c.take(N * 4), o_ctrl = c.take(sizeof(LoopCtrl));
@@ -531,16 +552,18 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.matchbits = (uint64_t*)(b + o_mb); W.inflight = (uint32_t*)(b + o_inf); W.have_epoch = (uint32_t*)(b + o_he);
     W.empty_epoch = (uint32_t*)(b + o_ee); W.have = (uint64_t*)(b + o_have); W.wants = (uint64_t*)(b + o_wants);
     W.hsum = (uint64_t*)(b + o_hs); W.wsum = (uint64_t*)(b + o_ws);
+    W.gcnt = (uint32_t*)(b + o_gc); W.gtot = (uint32_t*)(b + o_gt);
     W.wants_cnt = (uint32_t*)(b + o_wc); W.ctrl = (LoopCtrl*)(b + o_ctrl);
     return PCCL_OK;
 }
 
 struct PhaseView {   // link tables in the synthesized direction
-    const uint32_t *esrc, *edst, *in_off, *in_link;
+    const uint32_t *esrc, *edst, *in_off, *in_link, *out_link, *out_far, *lo_off, *lo_deg;
 };
 PhaseView view_of(const pccl_topology* t, bool transposed) {
-    if (!transposed) return {t->d_src, t->d_dst, t->d_in_off, t->d_in_link};
-    return {t->d_dst, t->d_src, t->d_out_off, t->d_out_link};
+    if (!transposed)
+        return {t->d_src, t->d_dst, t->d_in_off, t->d_in_link, t->d_out_link, t->d_out_far, t->d_lo_off_n, t->d_lo_deg_n};
+    return {t->d_dst, t->d_src, t->d_out_off, t->d_out_link, t->d_in_link, t->d_in_far, t->d_lo_off_t, t->d_lo_deg_t};
 }
 
 // steps A..C; on return the wants total is in *M (synchronises the stream)
@@ -593,6 +616,9 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     a.esrc = pv.esrc; a.edst = pv.edst; a.psrc = t->d_src; a.pdst = t->d_dst;
     a.in_off = pv.in_off; a.in_link = pv.in_link; a.w = W.w; a.have = W.have; a.wants = W.wants;
     a.hsum = W.hsum; a.wsum = W.wsum;
+    const bool rescan = (flags & (PCCL_FLAG_RESCAN | PCCL_FLAG_DENSE_SWEEP)) != 0;
+    a.gcnt = rescan ? nullptr : W.gcnt; a.gtot = rescan ? nullptr : W.gtot;
+    a.out_link = pv.out_link; a.out_far = pv.out_far; a.lo_off = pv.lo_off; a.lo_deg = pv.lo_deg;
     a.wants_cnt = W.wants_cnt; a.free_t = W.free_t; a.inflight = W.inflight; a.have_epoch = W.have_epoch;
     a.empty_epoch = W.empty_epoch; a.matchbits = W.matchbits; a.ctrl = W.ctrl; a.out = out; a.t_offset = t_offset;
     cudaStream_t st = G.stream;
@@ -609,6 +635,7 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     struct TraceGuard { void* p; ~TraceGuard() { dev_free(p); } } trace_guard{trace_dev};
     const uint32_t n_init = std::max(std::max(a.L, a.N), std::max(2 * a.nLw, 1u));
     k_loop_init<<<(n_init + 255) / 256, 256, 0, st>>>(a);
+    if (a.gcnt != nullptr && a.L) k_count_init<<<a.L, 256, 0, st>>>(a);
     const size_t smem = loop_smem_bytes(W.S, W.SWp);
     if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_loop, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;

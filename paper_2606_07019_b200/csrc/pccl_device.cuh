@@ -263,6 +263,12 @@ struct LoopArgs {
     uint64_t* wants;
     uint64_t* hsum;         // [N][SWp] sector summaries of have / wants
     uint64_t* wsum;
+    uint32_t* gcnt;         // [L][S] candidates of every link per 64-word segment, kept current (null: rescan mode)
+    uint32_t* gtot;         // [L] their sum
+    const uint32_t* out_link;  // per-node out-link table in the synthesized direction (entries)
+    const uint32_t* out_far;   // far end of each entry: edst[out_link[e]]
+    const uint32_t* lo_off;    // per link l: first entry / number of entries of the out-links of edst[l]
+    const uint32_t* lo_deg;
     uint32_t* wants_cnt;
     uint64_t* free_t;
     uint32_t* inflight;
@@ -283,6 +289,31 @@ __device__ __forceinline__ void trace_stamp(const LoopArgs& a, uint32_t step, in
         unsigned long long ns;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns));
         a.trace[(size_t)step * TRACE_SLOTS + slot] = ns;
+    }
+}
+
+// a5 (initial): cnt[l][s] = | have[src_l] & wants[dst_l] | restricted to segment s, for every link; one CTA per
+// link streams both rows once (128-bit coalesced loads).  The event loop then keeps the counts current.
+__global__ void __launch_bounds__(256) k_count_init(LoopArgs a) {
+    const uint32_t l = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t Q = a.Wp >> 1;
+    const uint4* hrow = reinterpret_cast<const uint4*>(a.have) + (size_t)a.esrc[l] * Q;
+    const uint4* wrow = reinterpret_cast<const uint4*>(a.wants) + (size_t)a.edst[l] * Q;
+    __shared__ uint32_t wsumc[8];
+    uint32_t mine = 0;
+    for (uint32_t qb = warp * 32; qb < Q; qb += blockDim.x) {
+        const uint32_t q = qb + lane;
+        uint32_t pc = 0;
+        if (q < Q) pc = popc128(and128(__ldg(hrow + q), __ldg(wrow + q)));
+        const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, pc);
+        if (lane == 0) { a.gcnt[(size_t)l * a.S + (qb >> 5)] = tot; mine += tot; }
+    }
+    if (lane == 0) wsumc[warp] = mine;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t t = 0;
+        for (int w = 0; w < 8; ++w) t += wsumc[w];
+        a.gtot[l] = t;
     }
 }
 
@@ -371,8 +402,29 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
             const uint32_t d = a.edst[l];
             atomicOr((unsigned long long*)&a.have[(size_t)d * a.Wp + (c >> 6)], 1ull << (c & 63));
             atomicOr((unsigned long long*)&a.hsum[(size_t)d * a.SWp + (c >> 14)], 1ull << ((c >> 8) & 63));
-            stcg32(a.inflight + l, NONE32);
-            stcg32(a.have_epoch + d, step + 1);
+            stcg32(a.have_epoch + d, step + 1);   // (inflight keeps the chunk: free_t == t holds at this event only)
+        }
+    }
+    // a5 (kept counts): the receiving node d now holds c, so c is a new candidate of every out-link of d whose
+    // far end wants it.  One thread per (arriving link, k-th out-link of d), taken from the END of the grid so
+    // that they run beside the warps above; three dependent round trips (link state, table entry, wants word).
+    if (a.gcnt != nullptr) {
+        constexpr uint32_t K = 8;
+        const uint32_t nthreads = gridDim.x * blockDim.x;
+        const uint32_t rid = nthreads - 1u - (blockIdx.x * blockDim.x + threadIdx.x);
+        for (uint64_t it = rid; it < (uint64_t)a.L * K; it += nthreads) {
+            const uint32_t l = (uint32_t)(it / K), k0 = (uint32_t)(it % K);
+            const uint32_t c = ldcg32(a.inflight + l);
+            const uint64_t f = ldcg64(a.free_t + l);
+            const uint32_t off = a.lo_off[l], deg = a.lo_deg[l];
+            if (c == NONE32 || f != t) continue;
+            for (uint32_t k = k0; k < deg; k += K) {
+                const uint32_t o = a.out_link[off + k], v2 = a.out_far[off + k];
+                if ((ldcg64(a.wants + (size_t)v2 * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) {
+                    atomicAdd(&a.gcnt[(size_t)o * a.S + (c >> 12)], 1u);
+                    atomicAdd(&a.gtot[o], 1u);
+                }
+            }
         }
     }
     // clear the bitmap the coming match phase writes; re-arm the ring slot after next
@@ -387,6 +439,8 @@ struct CtaScratch {
     uint32_t src[32];     // their sources
     uint64_t actw[32];    // their costs
     uint32_t sempty[NB];  // speculative pick j empties its wants sector
+    uint32_t acte[32];    // position of each active in-link in the destination's in-link list
+    uint32_t pbits[NB];   // per speculative pick: mask over the in-links whose source holds the picked chunk
     uint32_t nact;
     uint32_t wc;          // chunks this destination still wants
     uint32_t wtot[LOOP_THREADS / 32];   // block scan scratch
@@ -510,11 +564,12 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 const uint64_t f = ldcg64(a.free_t + l);
                 const uint32_t ee = ldcg32(a.empty_epoch + l);
                 const uint32_t he = ldcg32(a.have_epoch + u);
+                const uint32_t nc = (a.gtot != nullptr) ? ldcg32(a.gtot + l) : 1u;
                 if (f > t) {
                     mymin = min(mymin, f);
                 } else if (wc > 0) {
                     // idle filter: nothing arrived at the source since this link last found no candidate
-                    active = !(idle_skip && ee != 0 && ee >= he);
+                    active = !(idle_skip && ee != 0 && ee >= he) && nc != 0u;
                 }
             }
             const uint32_t m = __ballot_sync(0xFFFFFFFFu, active);
@@ -523,6 +578,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 sh.act[k] = l;
                 sh.src[k] = u;
                 sh.actw[k] = (dc != nullptr) ? dc->w[e] : a.w[l];
+                sh.acte[k] = e - e0;
             }
             if (lane == 0) sh.nact = __popc(m);
         }
@@ -538,11 +594,19 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
             // threads stride the list: two 128-bit loads of the source sector, two of the wants sector, AND,
             // popcount, shared-memory atomicAdd into the segment's counter.  Rows too dense for the list
             // (more than LIST_CAP candidate sectors) take the plain dense sweep instead.
-            {
+            if (a.gcnt != nullptr) {
+                // counts are kept current by arrivals (+) and claims (-): warp j copies the row of in-link j
+                if (warp < nb) {
+                    const uint32_t* g = a.gcnt + (size_t)sh.act[b0 + warp] * S;
+                    for (uint32_t x = lane; x < S; x += 32) cnt[warp * S + x] = ldcg32(g + x);
+                    if (lane == 0) st.bytes += (unsigned long long)S * 4u;
+                }
+            } else {
                 const uint64_t* ws = a.wsum + (size_t)v * SWp;
                 const uint32_t nitems = nb * SWp;
-                uint32_t total = 0;
-                for (uint32_t base = 0; base < nitems; base += LOOP_THREADS) {
+                const bool force_dense = (a.flags & 16u) != 0u;
+                uint32_t total = force_dense ? (uint32_t)LIST_CAP + 1u : 0u;
+                for (uint32_t base = 0; base < nitems && !force_dense; base += LOOP_THREADS) {
                     const uint32_t it = base + tid;
                     unsigned long long m = 0;
                     uint32_t j = 0, i = 0;
@@ -576,7 +640,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 for (uint32_t x = tid; x < nb * S; x += LOOP_THREADS) cnt[x] = 0;
                 __syncthreads();
                 trace_stamp(a, step, 9);
-                if (!(a.flags & 16u) && total <= LIST_CAP && total * 2u <= (nb + 1) * (Q >> 1)) {   // fewer sectors than the dense sweep
+                if (total <= LIST_CAP && total * 2u <= (nb + 1) * (Q >> 1)) {   // fewer sectors than the dense sweep
                     // a lane pair per item: even lane the first 16 bytes of the sector, odd lane the second, so
                     // that one warp-wide load touches 16 whole sectors; four items in flight per lane
                     const uint32_t half = tid & 1u;
@@ -614,18 +678,22 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                         const uint32_t q = qb + lane;
                         const bool ok = q < Q;
                         uint4 wv = make_uint4(0, 0, 0, 0);
+                        uint4 h[NB];
                         if (ok) wv = ldcg128(wrow + q);
+#pragma unroll
+                        for (int j = 0; j < NB; ++j) {   // all loads of the slice in flight before the first use
+                            h[j] = make_uint4(0, 0, 0, 0);
+                            if (j < (int)nb && ok) h[j] = ldcg128(have4 + hoff[j] + q);
+                        }
 #pragma unroll
                         for (int j = 0; j < NB; ++j) {
                             if (j < (int)nb) {
-                                uint4 h = make_uint4(0, 0, 0, 0);
-                                if (ok) h = ldcg128(have4 + hoff[j] + q);
-                                const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)popc128(and128(h, wv)));
+                                const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)popc128(and128(h[j], wv)));
                                 if (lane == 0) cnt[j * S + (qb >> 5)] = tot;
                             }
                         }
                     }
-                    if (tid == 0) st.bytes += (unsigned long long)(nb + 1) * a.Wp * 8u + (unsigned long long)nitems * 16u;
+                    if (tid == 0) st.bytes += (unsigned long long)(nb + 1) * a.Wp * 8u + (force_dense ? 0ull : (unsigned long long)nitems * 16u);
                 }
             }
             __syncthreads();
@@ -657,13 +725,37 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 st.rows += nb + 1;
                 st.links += nb;
                 uint32_t bad = 0;
-                for (uint32_t p = lane; p < nb * nb; p += 32) {
-                    const uint32_t i = p / nb, j = p % nb;
-                    if (i < j) {
-                        const uint32_t ci = sh.spec[i];
-                        if (ci != NONE32 && cnt[j * S + (ci >> 12)] != 0) {
-                            const uint32_t u = sh.src[b0 + j];
-                            if ((ldcg64(a.have + (size_t)u * a.Wp + (ci >> 6)) >> (ci & 63)) & 1ull) bad |= 1u << j;
+                const bool fastpairs = dc != nullptr;   // <= 32 in-links, tables in shared memory
+                if (fastpairs) {
+                    // one load per (speculative pick i, in-link e of v): does e's source hold pick i?  The answers
+                    // serve the conflict test (active later in-links) and the count upkeep (all in-links).
+                    uint32_t hit[NB];
+#pragma unroll
+                    for (int i = 0; i < NB; ++i) {
+                        hit[i] = 0;
+                        if (i < (int)nb) {
+                            const uint32_t ci = sh.spec[i];
+                            if (ci != NONE32 && lane < e1)
+                                hit[i] = (uint32_t)(ldcg64(a.have + (size_t)dc->src[lane] * a.Wp + (ci >> 6)) >> (ci & 63)) & 1u;
+                        }
+                    }
+#pragma unroll
+                    for (int i = 0; i < NB; ++i) {
+                        const uint32_t m = __ballot_sync(0xFFFFFFFFu, hit[i] != 0u);
+                        if (lane == 0) sh.pbits[i] = m;
+                        // lane j: is an earlier pick i held by my in-link's source?
+                        if (lane < nb && (int)lane > i && ((m >> sh.acte[b0 + lane]) & 1u)) bad |= 1u << lane;
+                    }
+                    if (lane == 0) st.bytes += (unsigned long long)nb * e1 * 32u;
+                } else {
+                    for (uint32_t p = lane; p < nb * nb; p += 32) {
+                        const uint32_t i = p / nb, j = p % nb;
+                        if (i < j) {
+                            const uint32_t ci = sh.spec[i];
+                            if (ci != NONE32 && cnt[j * S + (ci >> 12)] != 0) {
+                                const uint32_t u = sh.src[b0 + j];
+                                if ((ldcg64(a.have + (size_t)u * a.Wp + (ci >> 6)) >> (ci & 63)) & 1ull) bad |= 1u << j;
+                            }
                         }
                     }
                 }
@@ -689,6 +781,20 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 }
                 uint32_t ncl = __popc(__ballot_sync(0xFFFFFFFFu, lane < first_bad && sh.spec[lane] != NONE32));
                 __syncwarp();
+                const uint32_t ncl_spec = ncl;
+                if (fastpairs && a.gcnt != nullptr && lane < e1) {
+                    // count upkeep for the committed picks: lane e owns in-link e of v
+                    const uint32_t l2 = dc->link[lane];
+                    uint32_t dec = 0;
+                    for (uint32_t i = 0; i < first_bad; ++i) {
+                        const uint32_t ci = sh.spec[i];
+                        if (ci != NONE32 && ((sh.pbits[i] >> lane) & 1u)) {
+                            atomicSub(&a.gcnt[(size_t)l2 * S + (ci >> 12)], 1u);
+                            ++dec;
+                        }
+                    }
+                    if (dec) atomicSub(&a.gtot[l2], dec);
+                }
                 // the rest, one by one, against the wants row net of the claims so far
                 for (uint32_t j = first_bad; j < nb && wc > 0; ++j) {
                     if (lane == 0) ++st.slow;
@@ -723,6 +829,24 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     ++ncl;
                     --wc;
                     __syncwarp();
+                }
+                const uint32_t dec0 = fastpairs ? ncl_spec : 0u;   // claims before dec0 were handled above
+                if (a.gcnt != nullptr && ncl > dec0) {
+                    // v no longer wants the claimed chunks: every in-link of v (free or busy) whose source
+                    // holds one loses that candidate
+                    __syncwarp();
+                    const uint32_t n_in = e1 - e0;
+                    for (uint32_t p2 = lane; p2 < (ncl - dec0) * n_in; p2 += 32) {
+                        const uint32_t i = dec0 + p2 / n_in, e = e0 + (p2 % n_in);
+                        uint32_t l2, u2;
+                        if (dc != nullptr) { l2 = dc->link[e]; u2 = dc->src[e]; } else { l2 = a.in_link[e]; u2 = a.esrc[l2]; }
+                        const uint32_t c = sh.claimed[i];
+                        if ((ldcg64(a.have + (size_t)u2 * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) {
+                            atomicSub(&a.gcnt[(size_t)l2 * S + (c >> 12)], 1u);
+                            atomicSub(&a.gtot[l2], 1u);
+                        }
+                    }
+                    if (lane == 0) st.bytes += (unsigned long long)(ncl - dec0) * n_in * 32u;
                 }
                 if (lane == 0) sh.wc = wc;
                 // another sweep of this destination follows: its loads must see the wants bits just cleared

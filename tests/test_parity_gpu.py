@@ -243,17 +243,27 @@ def test_config4_full_size_bit_exact(pk):
     checker.check_structure(p, s.transfers)
 
 
-@pytest.mark.parametrize("maker", [wl.config2, wl.config4_small, wl.config5_small], ids=lambda m: m.__name__)
-def test_dense_sweep_and_sector_list_agree(pk, maker):
-    """the sector work list (default) and the plain dense row sweep are two ways to the same counts."""
+@pytest.mark.parametrize("maker", [wl.config1, wl.config2, wl.config3, wl.config4_small, wl.config5_small,
+                                   wl.two_groups_mesh3x3], ids=lambda m: m.__name__)
+def test_three_ways_to_the_candidate_counts_agree(pk, maker):
+    """kept-current counts (default), per-event recount through the sector work list (RESCAN) and the
+    plain dense row sweep (DENSE_SWEEP) must give the same schedule."""
     p = maker(2)
     o = oracle.synthesize(*p.args())
+    k = gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE)
+    r = gpu_run(pk, p, pk.PCCL_FLAG_RESCAN)
     d = gpu_run(pk, p, pk.PCCL_FLAG_DENSE_SWEEP)
-    s = gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE)
-    assert_same(p, d, o)
-    assert_same(p, s, o)
-    assert d.stats["rows_scanned"] == s.stats["rows_scanned"]
-    assert d.stats["bytes_requested"] >= s.stats["bytes_requested"]
+    for s in (k, r, d):
+        assert_same(p, s, o)
+    assert d.stats["bytes_requested"] >= r.stats["bytes_requested"]
+
+
+def test_rescan_modes_on_high_indegree_and_ragged_rows(pk):
+    for flags in (pk.PCCL_FLAG_RESCAN, pk.PCCL_FLAG_DENSE_SWEEP):
+        p = wl.full_mesh_problem(40, "allgather", seed=2)
+        assert_same(p, gpu_run(pk, p, flags), oracle.synthesize(*p.args()))
+        p = wl.ring_all_gather(8, True, seed=5, chunks_per_npu=1040, chunk_bytes=4096)
+        assert_same(p, gpu_run(pk, p, flags), oracle.synthesize(*p.args()))
 
 
 @pytest.mark.slow
@@ -263,6 +273,8 @@ def test_config5_full_size_bit_exact(pk):
     p = wl.config5(0)
     s = gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE)
     assert s.size == 7_761_800
+    r = gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE | pk.PCCL_FLAG_RESCAN)
     o = oracle.synthesize(*p.args())
     assert_same(p, s, o)
+    assert_same(p, r, o)
     checker.check_structure(p, s.transfers)
