@@ -131,6 +131,7 @@ struct pccl_topology {
     uint32_t N = 0, L = 0;
     std::vector<pccl_link_t> links;
     std::vector<uint32_t> in_off, in_link, out_off, out_link;   // ascending link id per node
+    uint32_t max_in = 0, max_out = 0;                           // largest in- / out-degree
     // device copy (one blob)
     void* blob = nullptr;
     uint32_t *d_src = nullptr, *d_dst = nullptr, *d_in_off = nullptr, *d_in_link = nullptr,
@@ -218,7 +219,12 @@ extern "C" int pccl_topology_create(uint32_t n_npus, const pccl_link_t* links, u
         t->in_off.assign((size_t)n_npus + 1, 0);
         t->out_off.assign((size_t)n_npus + 1, 0);
         for (uint32_t l = 0; l < n_links; ++l) { ++t->in_off[links[l].dst + 1]; ++t->out_off[links[l].src + 1]; }
-        for (uint32_t v = 0; v < n_npus; ++v) { t->in_off[v + 1] += t->in_off[v]; t->out_off[v + 1] += t->out_off[v]; }
+        for (uint32_t v = 0; v < n_npus; ++v) {
+            t->max_in = std::max(t->max_in, t->in_off[v + 1]);
+            t->max_out = std::max(t->max_out, t->out_off[v + 1]);
+            t->in_off[v + 1] += t->in_off[v];
+            t->out_off[v + 1] += t->out_off[v];
+        }
         t->in_link.resize(n_links);
         t->out_link.resize(n_links);
         std::vector<uint32_t> ci(t->in_off.begin(), t->in_off.end() - 1), co(t->out_off.begin(), t->out_off.end() - 1);
@@ -522,9 +528,8 @@ struct Work {   // device workspace of one phase
     size_t zero_off = 0, zero_bytes = 0;   // have + wants + wants_cnt + ctrl are cleared per run
 };
 
-size_t loop_smem_bytes(uint32_t S, uint32_t SWp) {
-    (void)SWp;
-    return (size_t)((NB * S + 3u) & ~3u) * 4 + (size_t)LIST_CAP * 4;
+size_t loop_smem_bytes(uint32_t S, uint32_t nbt = NB) {
+    return (size_t)((nbt * S + 3u) & ~3u) * 4 + (size_t)LIST_CAP * 4;
 }
 
 int work_alloc(const pccl_problem& P, Work& W) {
@@ -536,7 +541,7 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.S = (W.Wp / 2 + SEG_U4 - 1) / SEG_U4;
     W.nLw = (uint32_t)((L + 63) / 64);
     W.SWp = (uint32_t)align_up((W.Wp / 4 + 63) / 64, 2);          // one summary bit per 4-word sector
-    if (loop_smem_bytes(W.S, W.SWp) > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+    if (loop_smem_bytes(W.S) > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
     Carver c;
     const size_t o_w = c.take(L * 8), o_D = c.take(max_sources * N * 8), o_free = c.take(L * 8),
                  o_mb = c.take((size_t)2 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4),
@@ -636,16 +641,22 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     const uint32_t n_init = std::max(std::max(a.L, a.N), std::max(2 * a.nLw, 1u));
     k_loop_init<<<(n_init + 255) / 256, 256, 0, st>>>(a);
     if (a.gcnt != nullptr && a.L) k_count_init<<<a.L, 256, 0, st>>>(a);
-    const size_t smem = loop_smem_bytes(W.S, W.SWp);
-    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_loop, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    // one warp per in-link of a sweep: destinations with at most 4 in-links run in 128-thread CTAs (8 per SM),
+    // so that twice as many destinations are resident at once
+    const uint32_t max_deg = ph.transposed ? t->max_out : t->max_in;
+    const bool small = max_deg <= 4;
+    const void* kern = small ? (const void*)k_loop<4> : (const void*)k_loop<8>;
+    const int threads = small ? 128 : 256;
+    const size_t smem = loop_smem_bytes(W.S, small ? 4 : 8);
+    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_loop, LOOP_THREADS, smem));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
     if (occ < 1) return PCCL_ERR_CUDA;
     const uint32_t max_grid = (uint32_t)occ * (uint32_t)G.sm_count;
-    const uint32_t want = std::max(std::max(a.N, (a.L + LOOP_THREADS - 1) / LOOP_THREADS), 1u);
+    const uint32_t want = std::max(std::max(a.N, (a.L + threads - 1) / threads), 1u);
     const uint32_t grid = std::min(max_grid, want);
     void* args[] = {(void*)&a};
-    CU(cudaLaunchCooperativeKernel((const void*)k_loop, dim3(grid), dim3(LOOP_THREADS), args, smem, st));
+    CU(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(threads), args, smem, st));
     LoopCtrl* mb = (LoopCtrl*)G.mailbox;
     CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));

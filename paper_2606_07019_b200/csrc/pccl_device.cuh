@@ -26,8 +26,8 @@ namespace pccl {
 
 constexpr uint64_t T_INF = 0xFFFFFFFFFFFFFFFFull;
 constexpr uint32_t NONE32 = 0xFFFFFFFFu;
-constexpr int LOOP_THREADS = 256;  // threads per CTA of the event-loop kernel (= NB warps)
-constexpr int NB = 8;              // in-links of one destination counted in one sweep
+constexpr int NB = 8;              // most in-links of one destination served in one sweep (one warp each);
+                                   // k_loop<NBT> runs NBT * 32 threads per CTA, NBT = 8 or 4
 constexpr int LIST_CAP = 2048;     // candidate-sector work list entries per sweep (8 KB of shared memory)
 constexpr int SEG_U4 = 32;         // uint4 per segment (one warp-wide load) = 64 words = 4096 chunks
 
@@ -443,7 +443,7 @@ struct CtaScratch {
     uint32_t pbits[NB];   // per speculative pick: mask over the in-links whose source holds the picked chunk
     uint32_t nact;
     uint32_t wc;          // chunks this destination still wants
-    uint32_t wtot[LOOP_THREADS / 32];   // block scan scratch
+    uint32_t wtot[NB];   // block scan scratch (one per warp)
     uint32_t spec[NB];    // speculative pick of each in-link of the sweep (NONE32: no candidate)
     uint32_t claimed[NB]; // chunks claimed so far in this sweep (warp 0 only)
 };
@@ -532,9 +532,11 @@ struct DestCache {
     uint64_t w[32];
 };
 
+template <int NBT>
 __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v, uint32_t step, uint64_t t,
                                                   uint32_t* cnt, uint32_t* list, CtaScratch& sh, LoopStats& st,
                                                   const DestCache* dc) {
+    constexpr int THREADS = NBT * 32;   // one warp per in-link of a sweep
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t Q = a.Wp >> 1;  // uint4 per row
     const uint32_t SWp = a.SWp;
@@ -585,9 +587,9 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
         __syncthreads();
         trace_stamp(a, step, 3);
         const uint32_t nact = sh.nact;
-        for (uint32_t b0 = 0; b0 < nact; b0 += NB) {
+        for (uint32_t b0 = 0; b0 < nact; b0 += NBT) {
             if (sh.wc == 0) break;   // CTA-uniform: sh.wc only changes between the barriers below
-            const uint32_t nb = min((uint32_t)NB, nact - b0);
+            const uint32_t nb = min((uint32_t)NBT, nact - b0);
             // a5: candidate counts per 64-word segment.  Only sectors whose summary bit is set in BOTH the
             // wants row and the source row can hold a candidate.  (1) AND the summary rows; (2) expand the set
             // bits into a work list of (in-link, sector) items in shared memory (block-wide scan); (3) all
@@ -606,7 +608,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 const uint32_t nitems = nb * SWp;
                 const bool force_dense = (a.flags & 16u) != 0u;
                 uint32_t total = force_dense ? (uint32_t)LIST_CAP + 1u : 0u;
-                for (uint32_t base = 0; base < nitems && !force_dense; base += LOOP_THREADS) {
+                for (uint32_t base = 0; base < nitems && !force_dense; base += THREADS) {
                     const uint32_t it = base + tid;
                     unsigned long long m = 0;
                     uint32_t j = 0, i = 0;
@@ -621,7 +623,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     __syncthreads();
                     uint32_t pre = 0, blk = 0;
 #pragma unroll
-                    for (int w2 = 0; w2 < LOOP_THREADS / 32; ++w2) {
+                    for (int w2 = 0; w2 < THREADS / 32; ++w2) {
                         const uint32_t x = sh.wtot[w2];
                         pre += (w2 < (int)warp) ? x : 0u;
                         blk += x;
@@ -637,14 +639,14 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     trace_stamp(a, step, 8);
                     __syncthreads();
                 }
-                for (uint32_t x = tid; x < nb * S; x += LOOP_THREADS) cnt[x] = 0;
+                for (uint32_t x = tid; x < nb * S; x += THREADS) cnt[x] = 0;
                 __syncthreads();
                 trace_stamp(a, step, 9);
                 if (total <= LIST_CAP && total * 2u <= (nb + 1) * (Q >> 1)) {   // fewer sectors than the dense sweep
                     // a lane pair per item: even lane the first 16 bytes of the sector, odd lane the second, so
                     // that one warp-wide load touches 16 whole sectors; four items in flight per lane
                     const uint32_t half = tid & 1u;
-                    constexpr uint32_t PAIRS = LOOP_THREADS / 2, UNR = 4;
+                    constexpr uint32_t PAIRS = THREADS / 2, UNR = 4;
                     for (uint32_t idx = tid >> 1; idx < total; idx += UNR * PAIRS) {
                         uint32_t jj[UNR], ss[UNR];
                         uint4 hv[UNR], wv[UNR];
@@ -671,22 +673,22 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     if (tid == 0) st.bytes += (unsigned long long)total * 64u + (unsigned long long)nitems * 16u;
                 } else {
                     // dense sweep: every lane one uint4 of the wants row and of each source row
-                    size_t hoff[NB];
+                    size_t hoff[NBT];
 #pragma unroll
-                    for (int j = 0; j < NB; ++j) hoff[j] = (size_t)sh.src[b0 + (j < (int)nb ? j : 0)] * Q;
+                    for (int j = 0; j < NBT; ++j) hoff[j] = (size_t)sh.src[b0 + (j < (int)nb ? j : 0)] * Q;
                     for (uint32_t qb = warp * 32; qb < Q; qb += blockDim.x) {
                         const uint32_t q = qb + lane;
                         const bool ok = q < Q;
                         uint4 wv = make_uint4(0, 0, 0, 0);
-                        uint4 h[NB];
+                        uint4 h[NBT];
                         if (ok) wv = ldcg128(wrow + q);
 #pragma unroll
-                        for (int j = 0; j < NB; ++j) {   // all loads of the slice in flight before the first use
+                        for (int j = 0; j < NBT; ++j) {   // all loads of the slice in flight before the first use
                             h[j] = make_uint4(0, 0, 0, 0);
                             if (j < (int)nb && ok) h[j] = ldcg128(have4 + hoff[j] + q);
                         }
 #pragma unroll
-                        for (int j = 0; j < NB; ++j) {
+                        for (int j = 0; j < NBT; ++j) {
                             if (j < (int)nb) {
                                 const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)popc128(and128(h[j], wv)));
                                 if (lane == 0) cnt[j * S + (qb >> 5)] = tot;
@@ -729,22 +731,25 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 if (fastpairs) {
                     // one load per (speculative pick i, in-link e of v): does e's source hold pick i?  The answers
                     // serve the conflict test (active later in-links) and the count upkeep (all in-links).
-                    uint32_t hit[NB];
-#pragma unroll
-                    for (int i = 0; i < NB; ++i) {
-                        hit[i] = 0;
-                        if (i < (int)nb) {
-                            const uint32_t ci = sh.spec[i];
-                            if (ci != NONE32 && lane < e1)
-                                hit[i] = (uint32_t)(ldcg64(a.have + (size_t)dc->src[lane] * a.Wp + (ci >> 6)) >> (ci & 63)) & 1u;
-                        }
+                    if (lane < NBT) sh.pbits[lane] = 0;
+                    __syncwarp();
+                    const uint32_t npairs = nb * e1;
+                    for (uint32_t p0 = 0; p0 < npairs; p0 += 64) {   // two pairs per lane and round, loads first
+                        const uint32_t pa = p0 + lane, pb = p0 + 32 + lane;
+                        uint32_t ia = 0, ea = 0, ib = 0, eb2 = 0, ca = NONE32, cb = NONE32;
+                        unsigned long long wa = 0, wb = 0;
+                        if (pa < npairs) { ia = pa / e1; ea = pa - ia * e1; ca = sh.spec[ia]; }
+                        if (pb < npairs) { ib = pb / e1; eb2 = pb - ib * e1; cb = sh.spec[ib]; }
+                        if (ca != NONE32) wa = ldcg64(a.have + (size_t)dc->src[ea] * a.Wp + (ca >> 6));
+                        if (cb != NONE32) wb = ldcg64(a.have + (size_t)dc->src[eb2] * a.Wp + (cb >> 6));
+                        if (ca != NONE32 && ((wa >> (ca & 63)) & 1ull)) atomicOr(&sh.pbits[ia], 1u << ea);
+                        if (cb != NONE32 && ((wb >> (cb & 63)) & 1ull)) atomicOr(&sh.pbits[ib], 1u << eb2);
                     }
-#pragma unroll
-                    for (int i = 0; i < NB; ++i) {
-                        const uint32_t m = __ballot_sync(0xFFFFFFFFu, hit[i] != 0u);
-                        if (lane == 0) sh.pbits[i] = m;
-                        // lane j: is an earlier pick i held by my in-link's source?
-                        if (lane < nb && (int)lane > i && ((m >> sh.acte[b0 + lane]) & 1u)) bad |= 1u << lane;
+                    __syncwarp();
+                    if (lane < nb) {   // lane j: is an earlier pick held by my in-link's source?
+                        const uint32_t ej = sh.acte[b0 + lane];
+                        for (uint32_t i = 0; i < lane; ++i)
+                            if ((sh.pbits[i] >> ej) & 1u) bad |= 1u << lane;
                     }
                     if (lane == 0) st.bytes += (unsigned long long)nb * e1 * 32u;
                 } else {
@@ -760,6 +765,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     }
                 }
                 bad = __reduce_or_sync(0xFFFFFFFFu, bad);
+                trace_stamp(a, step, 8);
                 const uint32_t first_bad = bad ? (uint32_t)(__ffs(bad) - 1) : nb;
                 // commit the picks that stand (one lane per link)
                 uint32_t wc = sh.wc;
@@ -782,6 +788,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 uint32_t ncl = __popc(__ballot_sync(0xFFFFFFFFu, lane < first_bad && sh.spec[lane] != NONE32));
                 __syncwarp();
                 const uint32_t ncl_spec = ncl;
+                trace_stamp(a, step, 9);
                 if (fastpairs && a.gcnt != nullptr && lane < e1) {
                     // count upkeep for the committed picks: lane e owns in-link e of v
                     const uint32_t l2 = dc->link[lane];
@@ -830,6 +837,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     --wc;
                     __syncwarp();
                 }
+                trace_stamp(a, step, 10);
                 const uint32_t dec0 = fastpairs ? ncl_spec : 0u;   // claims before dec0 were handled above
                 if (a.gcnt != nullptr && ncl > dec0) {
                     // v no longer wants the claimed chunks: every in-link of v (free or busy) whose source
@@ -850,7 +858,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                 }
                 if (lane == 0) sh.wc = wc;
                 // another sweep of this destination follows: its loads must see the wants bits just cleared
-                if (b0 + NB < nact || eb + 32 < e1) __threadfence();
+                if (b0 + NBT < nact || eb + 32 < e1) __threadfence();
             }
             __syncthreads();
         }
@@ -874,13 +882,15 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
     __syncthreads();
 }
 
-__global__ void __launch_bounds__(LOOP_THREADS, 4) k_loop(const LoopArgs a) {
-    extern __shared__ __align__(16) uint32_t cnt[];   // [NB][S] candidate counts per segment, then the work list
-    uint32_t* list = cnt + ((NB * a.S + 3u) & ~3u);   // [LIST_CAP] (in-link << 28 | sector)
+template <int NBT>
+__global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop(const LoopArgs a) {
+    constexpr int THREADS = NBT * 32;
+    extern __shared__ __align__(16) uint32_t cnt[];   // [NBT][S] candidate counts per segment, then the work list
+    uint32_t* list = cnt + ((NBT * a.S + 3u) & ~3u);   // [LIST_CAP] (in-link << 28 | sector)
     __shared__ CtaScratch sh;
     __shared__ DestCache dcache[DEST_CACHE];
     cg::grid_group grid = cg::this_grid();
-    for (uint32_t k = threadIdx.x >> 5; k < DEST_CACHE; k += LOOP_THREADS / 32) {   // warp k fills slot k
+    for (uint32_t k = threadIdx.x >> 5; k < DEST_CACHE; k += THREADS / 32) {   // warp k fills slot k
         const uint32_t v = blockIdx.x + k * gridDim.x, lane = threadIdx.x & 31;
         if (v < a.N) {
             const uint32_t e0 = a.in_off[v], n = a.in_off[v + 1] - e0;
@@ -898,9 +908,10 @@ __global__ void __launch_bounds__(LOOP_THREADS, 4) k_loop(const LoopArgs a) {
     uint32_t step = 0;
     uint64_t t = 0;
     uint64_t emit_base = 0;
+    uint64_t total_now = 0;                 // transfers through event step-1
+    __shared__ unsigned long long s_next[2];   // one thread per CTA reads the two hot words after a barrier
     for (;;) {
         trace_stamp(a, step, 0);
-        const uint64_t total_now = ldcg64((const uint64_t*)&a.ctrl->total);   // through event step-1
         loop_phase_links(a, step, t, emit_base);
         emit_base = total_now;
         trace_stamp(a, step, 1);
@@ -909,13 +920,20 @@ __global__ void __launch_bounds__(LOOP_THREADS, 4) k_loop(const LoopArgs a) {
         {
             uint32_t k = 0;
             for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x, ++k)
-                match_destination(a, v, step, t, cnt, list, sh, st,
+                match_destination<NBT>(a, v, step, t, cnt, list, sh, st,
                                   (k < DEST_CACHE && dcache[k].n_in != NONE32) ? &dcache[k] : nullptr);
         }
         trace_stamp(a, step, 6);
         grid.sync();
         trace_stamp(a, step, 7);
-        t = ldcg64((const uint64_t*)&a.ctrl->tnext[(step + 1) % 3]);
+        if (threadIdx.x == 0) {
+            s_next[0] = ldcg64((const uint64_t*)&a.ctrl->tnext[(step + 1) % 3]);
+            s_next[1] = ldcg64((const uint64_t*)&a.ctrl->total);
+        }
+        __syncthreads();
+        t = s_next[0];
+        total_now = s_next[1];
+        __syncthreads();
         ++step;
         if (t == T_INF) break;
     }
