@@ -319,27 +319,46 @@ int topo_upload(pccl_topology* t) {
 int group_pairs(const pccl_condition_t* cnd, uint32_t C, uint32_t N, const std::vector<char>& member,
                 std::vector<uint64_t>& off, std::vector<uint32_t>& npus) {
     off.assign((size_t)C + 1, 0);
+    npus.resize(cnd->n_pairs);
+    bool ordered = true;   // chunk ids non-decreasing in the caller's array: the pairs are already grouped
+    uint32_t prev = 0;
+    const char* mem = member.data();
     for (uint64_t i = 0; i < cnd->n_pairs; ++i) {
-        const pccl_pair_t& p = cnd->pairs[i];
-        if (p.chunk >= C || p.npu >= N || !member[p.npu]) return PCCL_ERR_INVALID;
+        const pccl_pair_t p = cnd->pairs[i];
+        if (p.chunk >= C || p.npu >= N || !mem[p.npu]) return PCCL_ERR_INVALID;
         ++off[p.chunk + 1];
+        ordered &= p.chunk >= prev;
+        prev = p.chunk;
+        npus[i] = p.npu;
     }
-    for (uint32_t c = 0; c < C; ++c) off[c + 1] += off[c];
-    std::vector<uint32_t> tmp(cnd->n_pairs);
-    std::vector<uint64_t> cur(off.begin(), off.end() - 1);
-    for (uint64_t i = 0; i < cnd->n_pairs; ++i) tmp[cur[cnd->pairs[i].chunk]++] = cnd->pairs[i].npu;
-    // sort + unique each list, compacting in place
-    npus.clear();
-    npus.reserve(cnd->n_pairs);
-    std::vector<uint64_t> noff((size_t)C + 1, 0);
+    uint64_t longest = 0;
+    for (uint32_t c = 0; c < C; ++c) { longest = std::max(longest, off[c + 1]); off[c + 1] += off[c]; }
+    if (!ordered) {
+        std::vector<uint64_t> cur(off.begin(), off.end() - 1);
+        for (uint64_t i = 0; i < cnd->n_pairs; ++i) npus[cur[cnd->pairs[i].chunk]++] = cnd->pairs[i].npu;
+    }
+    if (longest <= 1) return PCCL_OK;   // every list has at most one holder: already sorted and duplicate-free
+    // sort each list; compact only if a duplicate shows up
+    bool dup = false;
     for (uint32_t c = 0; c < C; ++c) {
-        uint32_t* b = tmp.data() + off[c];
-        uint32_t* e = tmp.data() + off[c + 1];
-        if (e - b > 1) { std::sort(b, e); e = std::unique(b, e); }
-        npus.insert(npus.end(), b, e);
-        noff[c + 1] = npus.size();
+        uint32_t* b = npus.data() + off[c];
+        uint32_t* e = npus.data() + off[c + 1];
+        if (e - b > 1) {
+            std::sort(b, e);
+            dup |= std::adjacent_find(b, e) != e;
+        }
     }
-    off.swap(noff);
+    if (!dup) return PCCL_OK;
+    uint64_t w = 0, rd = 0;
+    for (uint32_t c = 0; c < C; ++c) {
+        const uint64_t end = off[c + 1];
+        off[c] = w;
+        for (uint64_t i = rd; i < end; ++i)
+            if (i == rd || npus[i] != npus[i - 1]) npus[w++] = npus[i];
+        rd = end;
+    }
+    off[C] = w;
+    npus.resize(w);
     return PCCL_OK;
 }
 
@@ -398,6 +417,7 @@ int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_membe
         Phase& ph = P.phases[0];
         ph.cond_src.resize(C);
         ph.dest_off.assign((size_t)C + 1, 0);
+        ph.dests.reserve(post_n.size());
         for (uint32_t c = 0; c < C; ++c)
             fill(ph, c, pre_n[pre_off[c]], post_n.data() + post_off[c], post_n.data() + post_off[c + 1]);
     } else if (all_multi_one) {   // REDUCE: broadcast root -> holders on the transposed links
