@@ -61,6 +61,9 @@ def lib():
         L.oracle_synthesize.argtypes = [u32, vp, u32, vp, u32, u32, vp, u64, vp, u64, u64, u64,
                                         C.POINTER(vp)]
         L.oracle_synthesize.restype = C.c_int
+        L.oracle_synthesize_relay.argtypes = [u32, vp, u32, vp, u32, u32, vp, u64, vp, u64, u64, u64, C.c_int,
+                                              C.POINTER(vp)]
+        L.oracle_synthesize_relay.restype = C.c_int
         L.oracle_wants.argtypes = [u32, vp, u32, u32, vp, vp, vp, u64, u64, vp, u64]
         L.oracle_wants.restype = i64
         for name in ("oracle_size", "oracle_time", "oracle_events", "oracle_wants_total",
@@ -115,17 +118,21 @@ class OracleSchedule:
         self.seconds = seconds                # wall time of the C++ call (steady clock)
 
 
-def synthesize(n_npus, links, group, n_chunks, pre, post, chunk_bytes, seed) -> OracleSchedule:
-    """Same problem statement as the product boundary (include/pccl.h), host arrays only."""
+RELAY_THIN, RELAY_DYNAMIC = 0, 1
+
+
+def synthesize(n_npus, links, group, n_chunks, pre, post, chunk_bytes, seed, relay: int = RELAY_THIN) -> OracleSchedule:
+    """Same problem statement as the product boundary (include/pccl.h), host arrays only.
+    relay: RELAY_THIN (static thin relay tree, the default) or RELAY_DYNAMIC (Q18)."""
     links = np.ascontiguousarray(links, dtype=LINK_DT)
     group = np.ascontiguousarray(group, dtype=np.uint32)
     pre = np.ascontiguousarray(pre, dtype=PAIR_DT)
     post = np.ascontiguousarray(post, dtype=PAIR_DT)
     h = C.c_void_p()
     t0 = time.perf_counter()
-    rc = lib().oracle_synthesize(n_npus, _ptr(links), len(links), _ptr(group), len(group),
-                                 n_chunks, _ptr(pre), len(pre), _ptr(post), len(post),
-                                 chunk_bytes, seed, C.byref(h))
+    rc = lib().oracle_synthesize_relay(n_npus, _ptr(links), len(links), _ptr(group), len(group),
+                                       n_chunks, _ptr(pre), len(pre), _ptr(post), len(post),
+                                       chunk_bytes, seed, int(relay), C.byref(h))
     dt = time.perf_counter() - t0
     if rc:
         raise OracleError(rc)

@@ -266,15 +266,142 @@ int synth_copy(uint32_t n, const std::vector<Link>& links, const std::vector<Con
 }
 
 // -------------------------------------------------------------------------------------
+// synth_copy_dynamic: the same loop with the DYNAMIC relay rule (reading Q18, the
+// forward-only analogue of the paper's "search the whole network, keep the useful paths",
+// PAPER.md:294-300).  Instead of fixing one relay tree per chunk up front:
+//   best[c][d]  = the smallest distance to dest d over the source and every node that has
+//                 CLAIMED chunk c so far (0 once d itself has claimed it),
+//   v wants c  <=>  for some dest d of c:  dist(v -> d) < best[c][d]      (strictly closer),
+// and best / wants are updated at the END of each event from that event's claims, so that
+// destinations stay independent within an event.  dist(v -> d) is the alpha-beta shortest
+// path cost (reading Q3).  Everything else (arrivals, candidates, pick, conflict order,
+// free-time advance) is step E of synth_copy unchanged.  A node claims a chunk at most once
+// (after its claim it is no longer strictly closer than the best holder), several nodes
+// may claim the same chunk, and some deliveries end up unused ("dead ends").
+// -------------------------------------------------------------------------------------
+int synth_copy_dynamic(uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& conds,
+                       uint64_t chunk_bytes, uint64_t seed, CopyResult& res,
+                       std::vector<std::vector<uint32_t>>* wants_out = nullptr) {
+    const uint32_t L = (uint32_t)links.size();
+    const uint32_t C = (uint32_t)conds.size();
+    std::vector<uint64_t> w(L);
+    for (uint32_t l = 0; l < L; ++l) w[l] = link_cost(links[l], chunk_bytes);
+    std::vector<std::vector<uint32_t>> inl(n);
+    for (uint32_t l = 0; l < L; ++l) inl[links[l].dst].push_back(l);
+
+    // distances TO every distinct dest: Dijkstra from d on the reversed links
+    std::vector<Link> rev(links);
+    for (Link& l : rev) std::swap(l.src, l.dst);
+    std::vector<std::vector<uint64_t>> Dto(n);
+    for (uint32_t c = 0; c < C; ++c) {
+        if (!conds[c].present) continue;
+        for (uint32_t d : conds[c].dests) {
+            if (Dto[d].empty()) Dto[d] = dijkstra(n, rev, w, d);
+            if (Dto[d][conds[c].src] == INF) return OR_ERR_UNREACHABLE;
+        }
+    }
+    // best[c][i] for the i-th dest of c, and the wants relation it implies
+    std::vector<std::vector<uint64_t>> best(C);
+    std::vector<std::vector<uint32_t>> have(n), wants(n);
+    auto wanted_by = [&](uint32_t c, uint32_t v) {
+        for (size_t i = 0; i < conds[c].dests.size(); ++i)
+            if (Dto[conds[c].dests[i]][v] < best[c][i]) return true;
+        return false;
+    };
+    for (uint32_t c = 0; c < C; ++c) {
+        if (!conds[c].present) continue;
+        insert_sorted(have[conds[c].src], c);
+        for (uint32_t d : conds[c].dests) best[c].push_back(Dto[d][conds[c].src]);
+        for (uint32_t v = 0; v < n; ++v)
+            if (wanted_by(c, v)) wants[v].push_back(c);   // c ascending: the lists stay sorted
+    }
+    res.wants_total = 0;
+    for (uint32_t v = 0; v < n; ++v) res.wants_total += wants[v].size();
+    if (wants_out) *wants_out = wants;
+
+    std::vector<uint64_t> free_t(L, 0);
+    std::vector<uint32_t> inflight(L, NONE);
+    uint64_t t = 0;
+    res.recs.clear();
+    res.events = 0;
+    std::vector<uint32_t> cand;
+    for (;;) {
+        ++res.events;
+        for (uint32_t l = 0; l < L; ++l) {   // E1 arrivals
+            if (inflight[l] != NONE && free_t[l] == t) {
+                insert_sorted(have[links[l].dst], inflight[l]);
+                inflight[l] = NONE;
+            }
+        }
+        const size_t first_new = res.recs.size();
+        for (uint32_t v = 0; v < n; ++v) {   // E2 match (identical to synth_copy)
+            for (uint32_t l : inl[v]) {
+                if (free_t[l] > t) continue;
+                if (wants[v].empty()) continue;
+                const std::vector<uint32_t>& hs = have[links[l].src];
+                cand.clear();
+                std::set_intersection(hs.begin(), hs.end(), wants[v].begin(), wants[v].end(),
+                                      std::back_inserter(cand));
+                if (cand.empty()) continue;
+                const uint32_t r = draw(seed, (uint32_t)(t & 0xFFFFFFFFull), (uint32_t)(t >> 32), l, 0);
+                const uint32_t c = cand[scale(r, cand.size())];
+                erase_sorted(wants[v], c);
+                inflight[l] = c;
+                free_t[l] = t + w[l];
+                res.recs.push_back(Rec{c, links[l].src, v, l, t, t + w[l]});
+            }
+        }
+        // E2' end of the event: the claims tighten best, and every node that is no longer
+        // strictly closer to some dest than the best holder stops wanting the chunk
+        std::set<uint32_t> touched;
+        for (size_t i = first_new; i < res.recs.size(); ++i) {
+            const Rec& r = res.recs[i];
+            for (size_t k = 0; k < conds[r.chunk].dests.size(); ++k)
+                best[r.chunk][k] = std::min(best[r.chunk][k], Dto[conds[r.chunk].dests[k]][r.dst]);
+            touched.insert(r.chunk);
+        }
+        for (uint32_t c : touched)
+            for (uint32_t v = 0; v < n; ++v)
+                if (contains(wants[v], c) && !wanted_by(c, v)) erase_sorted(wants[v], c);
+        uint64_t tn = INF;   // E3
+        for (uint32_t l = 0; l < L; ++l)
+            if (free_t[l] > t && free_t[l] < tn) tn = free_t[l];
+        if (tn == INF) break;
+        t = tn;
+    }
+    for (uint32_t v = 0; v < n; ++v)
+        if (!wants[v].empty()) return OR_ERR_INTERNAL;
+    for (uint32_t c = 0; c < C; ++c) {
+        if (!conds[c].present) continue;
+        for (uint32_t d : conds[c].dests)
+            if (!contains(have[d], c)) return OR_ERR_INTERNAL;
+    }
+    std::sort(res.recs.begin(), res.recs.end(), [](const Rec& a, const Rec& b) {
+        if (a.t_start_ps != b.t_start_ps) return a.t_start_ps < b.t_start_ps;
+        return a.link < b.link;
+    });
+    res.T = 0;
+    for (const Rec& r : res.recs) res.T = std::max(res.T, r.t_end_ps);
+    return OR_OK;
+}
+
+// relay rule used by the dispatchers below: 0 = thin relay tree (step C), 1 = dynamic
+int synth_copy_mode(int relay, uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& conds,
+                    uint64_t chunk_bytes, uint64_t seed, CopyResult& res) {
+    return relay == 1 ? synth_copy_dynamic(n, links, conds, chunk_bytes, seed, res)
+                      : synth_copy(n, links, conds, chunk_bytes, seed, res);
+}
+
+// -------------------------------------------------------------------------------------
 // REDUCE mode (reading Q10): synthesize the broadcast root -> holders on
 // the TRANSPOSED topology, then reverse every transfer in direction and in time.
 // -------------------------------------------------------------------------------------
 int synth_reduce(uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& bcast,
-                 uint64_t chunk_bytes, uint64_t seed, CopyResult& res) {
+                 uint64_t chunk_bytes, uint64_t seed, CopyResult& res, int relay = 0) {
     std::vector<Link> tr(links);
     for (Link& l : tr) std::swap(l.src, l.dst);
     CopyResult b;
-    const int rc = synth_copy(n, tr, bcast, chunk_bytes, seed, b);
+    const int rc = synth_copy_mode(relay, n, tr, bcast, chunk_bytes, seed, b);
     if (rc != OR_OK) return rc;
     res.recs.clear();
     for (const Rec& r : b.recs)   // (c, a, b, l, ts, te) -> (c, src=b, dst=a, l, T-te, T-ts)
@@ -305,7 +432,7 @@ struct Result {
 int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uint32_t* group,
                uint32_t n_members, uint32_t n_chunks, const Pair* pre_p, uint64_t n_pre,
                const Pair* post_p, uint64_t n_post, uint64_t chunk_bytes, uint64_t seed,
-               Result& out) {
+               Result& out, int relay = 0) {
     if (n_links && !links_p) return OR_ERR_INVALID;
     if (n_members && !group) return OR_ERR_INVALID;
     if ((n_pre && !pre_p) || (n_post && !post_p)) return OR_ERR_INVALID;
@@ -349,7 +476,7 @@ int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uin
             for (uint32_t d : post[c]) if (d != conds[c].src) conds[c].dests.push_back(d);
         }
         CopyResult r;
-        const int rc = synth_copy(n_npus, links, conds, chunk_bytes, seed, r);
+        const int rc = synth_copy_mode(relay, n_npus, links, conds, chunk_bytes, seed, r);
         if (rc != OR_OK) return rc;
         out.recs = std::move(r.recs); out.T = r.T; out.events = r.events;
         out.wants_total = r.wants_total; out.mode = 0;
@@ -363,7 +490,7 @@ int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uin
             for (uint32_t d : pre[c]) if (d != bc[c].src) bc[c].dests.push_back(d);
         }
         CopyResult r;
-        const int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r);
+        const int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r, relay);
         if (rc != OR_OK) return rc;
         out.recs = std::move(r.recs); out.T = r.T; out.events = r.events;
         out.wants_total = r.wants_total; out.mode = 1; out.T_phase1 = r.T;
@@ -382,9 +509,9 @@ int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uin
             for (uint32_t d : post[c]) if (d != root) cp[c].dests.push_back(d);
         }
         CopyResult r1, r2;
-        int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r1);
+        int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r1, relay);
         if (rc != OR_OK) return rc;
-        rc = synth_copy(n_npus, links, cp, chunk_bytes, seed, r2);
+        rc = synth_copy_mode(relay, n_npus, links, cp, chunk_bytes, seed, r2);
         if (rc != OR_OK) return rc;
         out.recs = std::move(r1.recs);
         for (const Rec& r : r2.recs)
@@ -445,6 +572,20 @@ int oracle_synthesize(uint32_t n_npus, const oracle_link* links, uint32_t n_link
     const int rc = synthesize(n_npus, (const Link*)links, n_links, group, n_members, n_chunks,
                               (const Pair*)pre, n_pre, (const Pair*)post, n_post, chunk_bytes,
                               seed, *r);
+    if (rc != OR_OK) { delete r; return rc; }
+    *handle = r;
+    return OR_OK;
+}
+
+int oracle_synthesize_relay(uint32_t n_npus, const oracle_link* links, uint32_t n_links,
+                            const uint32_t* group, uint32_t n_members, uint32_t n_chunks,
+                            const oracle_pair* pre, uint64_t n_pre, const oracle_pair* post,
+                            uint64_t n_post, uint64_t chunk_bytes, uint64_t seed, int relay, void** handle) {
+    if (!handle || relay < 0 || relay > 1) return OR_ERR_INVALID;
+    Result* r = new Result();
+    const int rc = synthesize(n_npus, (const Link*)links, n_links, group, n_members, n_chunks,
+                              (const Pair*)pre, n_pre, (const Pair*)post, n_post, chunk_bytes,
+                              seed, *r, relay);
     if (rc != OR_OK) { delete r; return rc; }
     *handle = r;
     return OR_OK;
