@@ -30,6 +30,7 @@ PCCL_ERR_CUDA, PCCL_ERR_NOMEM, PCCL_ERR_INTERNAL = -4, -5, -6
 PCCL_FLAG_KEEP_ON_DEVICE, PCCL_FLAG_NO_IDLE_SKIP, PCCL_FLAG_TIME_LOOP, PCCL_FLAG_TRACE = 1, 2, 4, 8
 PCCL_FLAG_DENSE_SWEEP = 16
 PCCL_FLAG_RESCAN = 32
+PCCL_FLAG_DYNAMIC_RELAY = 64
 PCCL_TRACE_SLOTS = 12
 
 

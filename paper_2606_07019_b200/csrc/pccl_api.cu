@@ -152,9 +152,12 @@ struct Phase {
     std::vector<uint32_t> dchunk;     // [n_dests] chunk of each (chunk, dest) pair
     std::vector<uint32_t> sources;    // distinct sources, ascending
     std::vector<uint32_t> sidx;       // [N] node -> row of D, NONE32 if not a source
+    std::vector<uint32_t> dsts;       // distinct dests, ascending (dynamic relay: rows of the to-dest distances)
+    std::vector<uint32_t> didx;       // [N] node -> row, NONE32 if not a dest
     void* blob = nullptr;
     uint32_t *d_cond_src = nullptr, *d_dests = nullptr, *d_dchunk = nullptr, *d_sources = nullptr,
-             *d_sidx = nullptr;
+             *d_sidx = nullptr, *d_dsts = nullptr, *d_didx = nullptr;
+    uint64_t* d_dest_off = nullptr;
 };
 
 }  // namespace
@@ -373,6 +376,11 @@ void finish_phase(Phase& ph, uint32_t N) {
     ph.sidx.assign(N, NONE32);
     for (uint32_t v = 0; v < N; ++v)
         if (is_src[v]) { ph.sidx[v] = (uint32_t)ph.sources.size(); ph.sources.push_back(v); }
+    std::vector<char> is_dst(N, 0);
+    for (uint32_t d : ph.dests) is_dst[d] = 1;
+    ph.didx.assign(N, NONE32);
+    for (uint32_t v = 0; v < N; ++v)
+        if (is_dst[v]) { ph.didx[v] = (uint32_t)ph.dsts.size(); ph.dsts.push_back(v); }
 }
 
 int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_members,
@@ -459,7 +467,12 @@ int phase_upload(Phase& ph, uint32_t N) {
     const size_t C = ph.cond_src.size(), ND = ph.dests.size(), NS = ph.sources.size();
     Carver c;
     const size_t o_cs = c.take(C * 4), o_d = c.take(ND * 4), o_dc = c.take(ND * 4), o_s = c.take(NS * 4), o_si = c.take((size_t)N * 4);
+    const size_t NDS = ph.dsts.size();
+    const size_t o_do = c.take((C + 1) * 8), o_ds = c.take(NDS * 4), o_di = c.take((size_t)N * 4);
     std::vector<unsigned char> h(c.cur ? c.cur : 256, 0);
+    memcpy(h.data() + o_do, ph.dest_off.data(), (C + 1) * 8);
+    if (NDS) memcpy(h.data() + o_ds, ph.dsts.data(), NDS * 4);
+    if (N) memcpy(h.data() + o_di, ph.didx.data(), (size_t)N * 4);
     if (C) memcpy(h.data() + o_cs, ph.cond_src.data(), C * 4);
     if (ND) { memcpy(h.data() + o_d, ph.dests.data(), ND * 4); memcpy(h.data() + o_dc, ph.dchunk.data(), ND * 4); }
     if (NS) memcpy(h.data() + o_s, ph.sources.data(), NS * 4);
@@ -477,6 +490,7 @@ int phase_upload(Phase& ph, uint32_t N) {
     ph.blob = blob;
     ph.d_cond_src = (uint32_t*)(b + o_cs); ph.d_dests = (uint32_t*)(b + o_d); ph.d_dchunk = (uint32_t*)(b + o_dc);
     ph.d_sources = (uint32_t*)(b + o_s); ph.d_sidx = (uint32_t*)(b + o_si);
+    ph.d_dest_off = (uint64_t*)(b + o_do); ph.d_dsts = (uint32_t*)(b + o_ds); ph.d_didx = (uint32_t*)(b + o_di);
     return PCCL_OK;
 }
 
@@ -544,6 +558,7 @@ struct Work {   // device workspace of one phase
     LoopCtrl* ctrl = nullptr;
     uint64_t *hsum = nullptr, *wsum = nullptr;
     uint32_t *gcnt = nullptr, *gtot = nullptr;
+    uint64_t* best = nullptr;
     uint32_t Wp = 0, S = 0, nLw = 0, SWp = 0;
     size_t zero_off = 0, zero_bytes = 0;   // have + wants + wants_cnt + ctrl are cleared per run
 };
@@ -555,7 +570,11 @@ size_t loop_smem_bytes(uint32_t S, uint32_t nbt = NB) {
 int work_alloc(const pccl_problem& P, Work& W) {
     const size_t N = P.topo->N, L = P.topo->L, C = P.C;
     size_t max_sources = 0;   // one workspace serves every phase
-    for (const Phase& ph : P.phases) max_sources = std::max(max_sources, ph.sources.size());
+    size_t max_pairs = 0;
+    for (const Phase& ph : P.phases) {
+        max_sources = std::max(max_sources, std::max(ph.sources.size(), ph.dsts.size()));   // D also holds the to-dest rows
+        max_pairs = std::max(max_pairs, ph.dests.size());
+    }
     const size_t words = (C + 63) / 64;
     W.Wp = (uint32_t)std::max<size_t>(16, align_up(words, 16));   // rows are multiples of 128 bytes
     W.S = (W.Wp / 2 + SEG_U4 - 1) / SEG_U4;
@@ -563,6 +582,7 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.SWp = (uint32_t)align_up((W.Wp / 4 + 63) / 64, 2);          // one summary bit per 4-word sector
     if (loop_smem_bytes(W.S) > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
     Carver c;
+    const size_t o_best = c.take(max_pairs * 8);
     const size_t o_w = c.take(L * 8), o_D = c.take(max_sources * N * 8), o_free = c.take(L * 8),
                  o_mb = c.take((size_t)2 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4),
                  o_gc = c.take(L * W.S * 4), o_gt = c.take(L * 4);
@@ -578,6 +598,7 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.empty_epoch = (uint32_t*)(b + o_ee); W.have = (uint64_t*)(b + o_have); W.wants = (uint64_t*)(b + o_wants);
     W.hsum = (uint64_t*)(b + o_hs); W.wsum = (uint64_t*)(b + o_ws);
     W.gcnt = (uint32_t*)(b + o_gc); W.gtot = (uint32_t*)(b + o_gt);
+    W.best = (uint64_t*)(b + o_best);
     W.wants_cnt = (uint32_t*)(b + o_wc); W.ctrl = (LoopCtrl*)(b + o_ctrl);
     return PCCL_OK;
 }
@@ -592,7 +613,7 @@ PhaseView view_of(const pccl_topology* t, bool transposed) {
 }
 
 // steps A..C; on return the wants total is in *M (synchronises the stream)
-int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint64_t* M) {
+int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint64_t* M, bool dynamic = false) {
     const pccl_topology* t = P.topo;
     const uint32_t N = t->N, L = t->L, C = P.C;
     const PhaseView pv = view_of(t, ph.transposed);
@@ -600,6 +621,31 @@ int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t 
     cudaStream_t st = G.stream;
     CU(cudaMemsetAsync((unsigned char*)W.blob + W.zero_off, 0, W.zero_bytes, st));
     if (L) k_link_cost<<<(L + 255) / 256, 256, 0, st>>>(t->d_alpha, t->d_bpp, L, P.chunk_bytes, W.w);
+    if (dynamic) {
+        // reading Q18: distances TO every distinct dest (Bellman-Ford on the reversed links), best = dist(src -> dest),
+        // wants = every node strictly closer to some dest than the source
+        const uint32_t NDS = (uint32_t)ph.dsts.size();
+        const uint64_t NP = ph.dests.size();
+        const size_t smem = (size_t)N * 8;
+        if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+        if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (NDS) k_distances<<<NDS, 256, smem, st>>>(pv.edst, pv.esrc, W.w, N, L, ph.d_dsts, W.D);
+        if (NP) k_best_init<<<(unsigned)((NP + 255) / 256), 256, 0, st>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, NP, ph.d_didx,
+                                                                         W.D, N, W.best, &W.ctrl->err);
+        if (C) k_have<<<(C + 255) / 256, 256, 0, st>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
+        const uint64_t nth = (uint64_t)N * ((C + 63) / 64);
+        if (nth) k_wants_dyn_init<<<(unsigned)((nth + 127) / 128), 128, 0, st>>>(ph.d_dest_off, ph.d_dests, ph.d_didx, W.D, W.best, N,
+                                                                                C, W.Wp, W.SWp, W.wants, W.wsum, W.wants_cnt);
+        k_sum_u32<<<1, 1024, 0, st>>>(W.wants_cnt, N, &W.ctrl->wants_total);
+        CU(cudaGetLastError());
+        LoopCtrl* mbx = (LoopCtrl*)G.mailbox;
+        CU(cudaMemcpyAsync(mbx, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        if (mbx->err & 1u) return PCCL_ERR_UNREACHABLE;
+        if (mbx->err) return PCCL_ERR_INTERNAL;
+        *M = mbx->wants_total;
+        return PCCL_OK;
+    }
     const uint32_t NS = (uint32_t)ph.sources.size();
     if (NS) {
         const size_t smem = (size_t)N * 8;
@@ -632,7 +678,9 @@ struct LoopResult {
 
 // steps D..E: the event loop; records go to `out` (capacity M) in canonical order
 int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint32_t flags, Rec* out,
-               uint64_t t_offset, LoopResult* res, std::vector<uint64_t>* trace = nullptr) {
+               uint64_t out_cap, uint64_t t_offset, LoopResult* res, std::vector<uint64_t>* trace = nullptr) {
+    const bool dynamic = (flags & PCCL_FLAG_DYNAMIC_RELAY) != 0;
+    if (dynamic) flags |= PCCL_FLAG_DENSE_SWEEP;   // wants rows are dense and shrink by rule: recount by whole rows
     const pccl_topology* t = P.topo;
     const PhaseView pv = view_of(t, ph.transposed);
     LoopArgs a;
@@ -646,6 +694,8 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     a.out_link = pv.out_link; a.out_far = pv.out_far; a.lo_off = pv.lo_off; a.lo_deg = pv.lo_deg;
     a.wants_cnt = W.wants_cnt; a.free_t = W.free_t; a.inflight = W.inflight; a.have_epoch = W.have_epoch;
     a.empty_epoch = W.empty_epoch; a.matchbits = W.matchbits; a.ctrl = W.ctrl; a.out = out; a.t_offset = t_offset;
+    a.out_cap = out_cap;
+    a.best = dynamic ? W.best : nullptr; a.Dto = W.D; a.didx = ph.d_didx; a.dest_off = ph.d_dest_off; a.dests = ph.d_dests;
     cudaStream_t st = G.stream;
     a.trace = nullptr; a.trace_cap = 0;
     void* trace_dev = nullptr;
@@ -680,6 +730,7 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     LoopCtrl* mb = (LoopCtrl*)G.mailbox;
     CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    if (mb->err & 32u) return PCCL_ERR_NOMEM;   // more transfers than the record buffer holds
     if (mb->err) return PCCL_ERR_INTERNAL;
     res->total = mb->total; res->tmax = mb->tmax; res->events = mb->events;
     res->rows = mb->rows_scanned; res->links = mb->links_scanned; res->slow = mb->slow_picks;
@@ -779,19 +830,24 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
         if (!W.blob) { rc = work_alloc(*P, W); if (rc) return fail(rc); }
         uint64_t M = 0;
         t_setup.start();
-        rc = phase_setup(*P, ph, W, seed, &M);
+        const bool dynamic = (flags & PCCL_FLAG_DYNAMIC_RELAY) != 0;
+        rc = phase_setup(*P, ph, W, seed, &M, dynamic);
         if (rc) return fail(rc);
         t_setup.stop();
         S->stats.wants_total += M;
+        // thin relay tree: exactly M transfers.  dynamic rule: at most M (a (node, chunk) pair is claimed at
+        // most once); the record buffer is sized for that bound, capped at 2^28 records
+        const uint64_t cap = dynamic ? std::min<uint64_t>(M, 1ull << 28) : M;
         LoopResult lr;
         if (ph.transposed) {
-            rc = dev_alloc(M * sizeof(Rec), (void**)&raw);
+            rc = dev_alloc(cap * sizeof(Rec), (void**)&raw);
             if (rc) return fail(rc);
             t_loop.start();
-            rc = phase_loop(*P, ph, W, seed, flags, raw, 0, &lr, &S->trace);
+            rc = phase_loop(*P, ph, W, seed, flags, raw, cap, 0, &lr, &S->trace);
             if (rc) return fail(rc);
             t_loop.stop();
-            if (lr.total != M) return fail(PCCL_ERR_INTERNAL);
+            if (dynamic ? lr.total > M : lr.total != M) return fail(PCCL_ERR_INTERNAL);
+            M = lr.total;
             Rec* dst = nullptr;
             rc = dev_alloc(M * sizeof(Rec), (void**)&dst);
             if (rc) return fail(rc);
@@ -808,7 +864,7 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
         } else {
             const uint64_t base = (pi == 0) ? 0 : M1;
             const uint64_t toff = (pi == 0) ? 0 : T1;
-            rc = dev_alloc((base + M) * sizeof(Rec), (void**)&out_recs);
+            rc = dev_alloc((base + cap) * sizeof(Rec), (void**)&out_recs);
             if (rc) return fail(rc);
             if (base) {
                 if (cudaMemcpyAsync(out_recs, stage1, base * sizeof(Rec), cudaMemcpyDeviceToDevice, G.stream) != cudaSuccess) {
@@ -817,10 +873,11 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
                 }
             }
             t_loop.start();
-            rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, toff, &lr, &S->trace);
+            rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, cap, toff, &lr, &S->trace);
             if (rc) return fail(rc);
             t_loop.stop();
-            if (lr.total != M) return fail(PCCL_ERR_INTERNAL);
+            if (dynamic ? lr.total > M : lr.total != M) return fail(PCCL_ERR_INTERNAL);
+            M = lr.total;
             S->M = base + M;
             S->T = toff + lr.tmax;
         }

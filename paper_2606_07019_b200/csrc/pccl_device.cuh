@@ -184,6 +184,45 @@ __global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* _
     }
 }
 
+// ---- a2 (dynamic relay, Q18): best[p] for every (chunk, dest) pair p starts at dist(source -> dest);
+// Dto[row(d)][v] = alpha-beta shortest cost v -> d (k_distances on the reversed links)
+__global__ void k_best_init(const uint32_t* __restrict__ cond_src, const uint32_t* __restrict__ dests,
+                            const uint32_t* __restrict__ dchunk, uint64_t n_pairs,
+                            const uint32_t* __restrict__ didx, const uint64_t* __restrict__ Dto, uint32_t N,
+                            uint64_t* __restrict__ best, uint32_t* __restrict__ err) {
+    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_pairs) return;
+    const uint64_t d0 = Dto[(size_t)didx[dests[p]] * N + cond_src[dchunk[p]]];
+    if (d0 == T_INF) atomicOr(err, 1u);
+    best[p] = d0;
+}
+
+// wants[u][c] = 1 iff some dest d of c has dist(u -> d) < best[c, d]; one thread per (node, 64-chunk word)
+__global__ void k_wants_dyn_init(const uint64_t* __restrict__ dest_off, const uint32_t* __restrict__ dests,
+                                 const uint32_t* __restrict__ didx, const uint64_t* __restrict__ Dto,
+                                 const uint64_t* __restrict__ best, uint32_t N, uint32_t C, uint32_t Wp,
+                                 uint32_t SWp, uint64_t* __restrict__ wants, uint64_t* __restrict__ wsum,
+                                 uint32_t* __restrict__ wants_cnt) {
+    const uint32_t words = (C + 63) >> 6;
+    const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (uint64_t)N * words) return;
+    const uint32_t u = (uint32_t)(gid / words), wi = (uint32_t)(gid % words);
+    unsigned long long word = 0;
+    for (uint32_t b = 0; b < 64; ++b) {
+        const uint32_t c = wi * 64 + b;
+        if (c >= C) break;
+        const uint64_t p1 = dest_off[c + 1];
+        for (uint64_t p = dest_off[c]; p < p1; ++p) {
+            if (Dto[(size_t)didx[dests[p]] * N + u] < best[p]) { word |= 1ull << b; break; }
+        }
+    }
+    if (word) {
+        wants[(size_t)u * Wp + wi] = word;
+        atomicOr((unsigned long long*)&wsum[(size_t)u * SWp + (wi >> 8)], 1ull << ((wi >> 2) & 63));
+        atomicAdd(&wants_cnt[u], (uint32_t)__popcll(word));
+    }
+}
+
 // sum of wants_cnt -> ctrl (one block)
 __global__ void k_sum_u32(const uint32_t* __restrict__ x, uint32_t n, unsigned long long* out) {
     __shared__ unsigned long long s[32];
@@ -278,6 +317,13 @@ struct LoopArgs {
     LoopCtrl* ctrl;
     Rec* out;
     uint64_t t_offset;      // added to the emitted times (phase 2 of all-reduce)
+    // dynamic relay rule (null best: static thin relay tree)
+    uint64_t* best;             // [pairs] smallest dist to the pair's dest over the source and all claimants
+    const uint64_t* Dto;        // [distinct dests][N]
+    const uint32_t* didx;       // [N] node -> row of Dto
+    const uint64_t* dest_off;   // [C+1] pairs of each chunk
+    const uint32_t* dests;      // [pairs]
+    uint64_t out_cap;           // records the output buffer holds
     uint64_t* trace;        // optional [events][TRACE_SLOTS] globaltimer stamps of CTA 0 (diagnostic), or null
     uint32_t trace_cap;     // events the trace buffer holds
 };
@@ -391,6 +437,7 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
                 if ((mine >> lane) & 1u) {
                     const uint64_t rank = pre + __popc(mine & ((1u << lane) - 1u));
                     const uint64_t wl = a.w[l];
+                    if (emit_base + rank >= a.out_cap) { atomicOr(&a.ctrl->err, 32u); continue; }
                     uint4* o = reinterpret_cast<uint4*>(a.out + emit_base + rank);
                     const uint64_t ts = f - wl + a.t_offset, te = f + a.t_offset;
                     o[0] = make_uint4(c, a.psrc[l], a.pdst[l], l);
@@ -431,6 +478,39 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
     uint64_t* mbcur = a.matchbits + (size_t)(step & 1) * a.nLw;
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < a.nLw; i += gridDim.x * blockDim.x) stcg64(mbcur + i, 0);
     if (blockIdx.x == 0 && threadIdx.x == 0) stcg64((uint64_t*)&a.ctrl->tnext[(step + 2) % 3], T_INF);
+}
+
+// ---- dynamic relay rule, end of an event (Q18).  U: every claim (c, v) of the event tightens
+// best[p] = min(best[p], dist(v -> d_p)) for the pairs p of c.  (grid barrier.)  W: for every claimed chunk,
+// each node that is no longer strictly closer to some dest than the best holder stops wanting it.
+__device__ __forceinline__ void dyn_update_best(const LoopArgs& a, uint32_t step) {
+    const uint64_t* mb = a.matchbits + (size_t)(step & 1) * a.nLw;
+    for (uint32_t l = blockIdx.x * blockDim.x + threadIdx.x; l < a.L; l += gridDim.x * blockDim.x) {
+        if (!((ldcg64(mb + (l >> 6)) >> (l & 63)) & 1ull)) continue;
+        const uint32_t c = ldcg32(a.inflight + l), v = a.edst[l];
+        const uint64_t p1 = a.dest_off[c + 1];
+        for (uint64_t p = a.dest_off[c]; p < p1; ++p)
+            atomicMin((unsigned long long*)&a.best[p], (unsigned long long)a.Dto[(size_t)a.didx[a.dests[p]] * a.N + v]);
+    }
+}
+__device__ __forceinline__ void dyn_shrink_wants(const LoopArgs& a, uint32_t step) {
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nW = (gridDim.x * blockDim.x) >> 5;
+    const uint64_t* mb = a.matchbits + (size_t)(step & 1) * a.nLw;
+    for (uint32_t l = gw; l < a.L; l += nW) {   // a warp per link matched at this event
+        if (!((ldcg64(mb + (l >> 6)) >> (l & 63)) & 1ull)) continue;
+        const uint32_t c = ldcg32(a.inflight + l);
+        const uint64_t p0 = a.dest_off[c], p1 = a.dest_off[c + 1];
+        const unsigned long long bit = 1ull << (c & 63);
+        for (uint32_t u = lane; u < a.N; u += 32) {
+            unsigned long long* wp = (unsigned long long*)&a.wants[(size_t)u * a.Wp + (c >> 6)];
+            if (!(ldcg64((const uint64_t*)wp) & bit)) continue;
+            bool keep = false;
+            for (uint64_t p = p0; p < p1 && !keep; ++p)
+                keep = a.Dto[(size_t)a.didx[a.dests[p]] * a.N + u] < ldcg64(a.best + p);
+            if (!keep && (atomicAnd(wp, ~bit) & bit)) atomicSub(&a.wants_cnt[u], 1u);   // once per (u, c)
+        }
+    }
 }
 
 // ---- P2: match one destination (a4..a8) -----------------------------------------------------------------
@@ -934,6 +1014,11 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop(const Loop
         t = s_next[0];
         total_now = s_next[1];
         __syncthreads();
+        if (a.best != nullptr && t != T_INF) {   // (the last event never has claims)
+            dyn_update_best(a, step);
+            grid.sync();
+            dyn_shrink_wants(a, step);   // runs beside the next links phase: both end at its barrier
+        }
         ++step;
         if (t == T_INF) break;
     }

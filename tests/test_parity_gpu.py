@@ -278,3 +278,41 @@ def test_config5_full_size_bit_exact(pk):
     assert_same(p, s, o)
     assert_same(p, r, o)
     checker.check_structure(p, s.transfers)
+
+
+# ------------------------------------------------------------------------------ dynamic relay rule (NEXT-1)
+@pytest.mark.parametrize("maker", SMALL, ids=lambda m: m.__name__)
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_dynamic_relay_bit_exact_small_configs(pk, maker, seed):
+    p = maker(seed)
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_DYNAMIC)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY)
+    assert_same(p, s, o)
+    checker.check_schedule(p, s.transfers)
+
+
+def test_dynamic_relay_rings_mesh_star_and_ragged_rows(pk):
+    cases = [wl.ring_all_gather(5, False, 1), wl.ring_all_gather(9, True, 2),
+             wl.ring_all_gather(8, True, 5, chunks_per_npu=1040, chunk_bytes=4096),
+             wl.full_mesh_problem(40, "allgather", seed=2), wl.full_mesh_problem(12, "alltoall", seed=4),
+             wl.path_point_to_point(6, 0)]
+    n = 70
+    links = np.array([(i, n, 1000, 7) for i in range(n)] + [(n, i, 1000, 7) for i in range(n)], dtype=wl.LINK_DT)
+    members = np.arange(n, dtype=np.uint32)
+    nc, pre, post = wl.all_to_all(members)
+    cases.append(wl.Problem("star70_alltoall", n + 1, links, members, nc, pre, post, 1000, 11))
+    for p in cases:
+        o = oracle.synthesize(*p.args(), relay=oracle.RELAY_DYNAMIC)
+        assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY), o)
+
+
+def test_dynamic_relay_unreachable(pk):
+    links = np.array([(0, 1, 5, 1)], dtype=wl.LINK_DT)
+    members = np.array([0, 1], dtype=np.uint32)
+    pre = np.array([(1, 0)], dtype=wl.PAIR_DT)
+    post = np.array([(0, 0)], dtype=wl.PAIR_DT)
+    topo = pk.Topology(2, links)
+    prob = pk.Problem(topo, members, 1, pre, post, 64)
+    with pytest.raises(pk.PcclError) as e:
+        prob.synthesize(0, pk.PCCL_FLAG_DYNAMIC_RELAY)
+    assert e.value.code == pk.PCCL_ERR_UNREACHABLE
