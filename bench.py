@@ -291,6 +291,26 @@ def run_ours(args):
                          "requested_gbs": stv["bytes_requested"] / (mv * 1e-3) / 1e9,
                          "algorithmic_bytes_per_launch": algv, "achieved": algv / (mv * 1e-3) / 1e9, "unit": "GB/s",
                          "frac": algv / (mv * 1e-3) / 1e9 / peak}
+    # ---- the dynamic relay rule (Q18) on the same problem: schedule quality vs cost ----
+    dynamic = None
+    if not args.no_other_configs:
+        ms_d, sd = [], None
+        for i in range(3):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            sd = prob.synthesize(seed, flags | pk.PCCL_FLAG_DYNAMIC_RELAY)
+            e1.record()
+            e1.synchronize()
+            if i >= 1:
+                ms_d.append(e0.elapsed_time(e1))
+            dM, dT, dst = sd.size, sd.time_ps, sd.stats
+            sd.close()
+        dynamic = {"synthesis_ms": sum(ms_d) / len(ms_d), "loop_ms": dst["loop_ms"], "transfers": dM,
+                   "events": dst["events"], "schedule_time_ps": dT,
+                   "schedule_time_vs_thin_tree": dT / T if T else None,
+                   "initial_wants": dst["wants_total"]}
+
     # ---- the other BASELINE.json configs, same path, resident inputs (context; parity is in tests/) ---
     per_config = {}
     if not args.no_other_configs:
@@ -322,6 +342,17 @@ def run_ours(args):
                 "frac_of_measured_hbm": (algb / (stc["loop_ms"] * 1e-3) / 1e9 / peak) if stc["loop_ms"] else None,
                 "requested_bytes": stc["bytes_requested"],
                 "roofline_note": "rows of 128 B: launch/sync-bound, roofline n/a" if stc["row_bytes"] <= 256 else "bitmap scan"}
+            if stc["row_bytes"] > 256:   # a real bitmap scan: the two recount modes beside the default
+                for key, fl in (("rescan_sector_list", pk.PCCL_FLAG_RESCAN), ("dense_sweep", pk.PCCL_FLAG_DENSE_SWEEP)):
+                    flush.zero_()
+                    sv = prc.synthesize(0, flags | fl)
+                    stv = sv.stats
+                    sv.close()
+                    algv = stv["rows_scanned"] * stv["row_bytes"]
+                    per_config[f"config{cfg}"][key] = {
+                        "loop_ms": stv["loop_ms"], "requested_bytes": stv["bytes_requested"],
+                        "algorithmic_gbs": algv / (stv["loop_ms"] * 1e-3) / 1e9,
+                        "frac_of_measured_hbm": algv / (stv["loop_ms"] * 1e-3) / 1e9 / peak}
             prc.close()
             tc.close()
 
@@ -353,7 +384,7 @@ def run_ours(args):
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": 1e3 * e2e_tot / args.steps},
             "gpu_launches": KERNELS_PER_STEP_COPY * args.steps,
-            "roofline": roofline, "cpu_baseline": cpu, "clocks": clk.summary(), "per_config": per_config,
+            "roofline": roofline, "cpu_baseline": cpu, "clocks": clk.summary(), "per_config": per_config, "dynamic_relay": dynamic,
             "paper_context": "PCCL reports 11.68 min for 512-NPU All-to-All synthesis, hardware not stated "
                              "(PAPER.md:9, :388); a different procedure, context only",
             "wall_s_timed_region": wall}

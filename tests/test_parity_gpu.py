@@ -316,3 +316,13 @@ def test_dynamic_relay_unreachable(pk):
     with pytest.raises(pk.PcclError) as e:
         prob.synthesize(0, pk.PCCL_FLAG_DYNAMIC_RELAY)
     assert e.value.code == pk.PCCL_ERR_UNREACHABLE
+
+
+@pytest.mark.slow
+def test_dynamic_relay_6x6x6_torus_all_to_all(pk):
+    """216 NPUs, 46,440 chunks (rows of 726 words: 12 segments with a ragged tail), 212 k transfers."""
+    p = wl.config4(0, dims=(6, 6, 6))
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_DYNAMIC)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY)
+    assert_same(p, s, o)
+    checker.check_structure(p, s.transfers)
