@@ -167,7 +167,8 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
 #define PCCL_FLAG_DYNAMIC_RELAY 64u /* relay rule of DESIGN.md Q18 instead of the static thin relay tree: a node
                                        takes a chunk iff it is strictly closer to some destination than the
                                        source and every node that claimed the chunk at an earlier event
-                                       (implies DENSE_SWEEP; fewer link-times, a few unused deliveries) */
+                                       (fewer link-times, a few unused deliveries; recounts by dense sweep unless KEPT_COUNTS or RESCAN) */
+#define PCCL_FLAG_KEPT_COUNTS 128u  /* with DYNAMIC_RELAY: keep the counts current instead of its default dense recount */
 #define PCCL_FLAG_RESCAN 32u        /* recount every free link's candidates at every event from the bitmaps
                                        (sector work list), instead of keeping the counts current */
 #define PCCL_FLAG_DENSE_SWEEP 16u   /* implies RESCAN, and recounts by sweeping whole rows, never the sector

@@ -31,6 +31,7 @@ PCCL_FLAG_KEEP_ON_DEVICE, PCCL_FLAG_NO_IDLE_SKIP, PCCL_FLAG_TIME_LOOP, PCCL_FLAG
 PCCL_FLAG_DENSE_SWEEP = 16
 PCCL_FLAG_RESCAN = 32
 PCCL_FLAG_DYNAMIC_RELAY = 64
+PCCL_FLAG_KEPT_COUNTS = 128
 PCCL_TRACE_SLOTS = 12
 
 

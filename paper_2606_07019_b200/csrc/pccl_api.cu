@@ -680,7 +680,9 @@ struct LoopResult {
 int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint32_t flags, Rec* out,
                uint64_t out_cap, uint64_t t_offset, LoopResult* res, std::vector<uint64_t>* trace = nullptr) {
     const bool dynamic = (flags & PCCL_FLAG_DYNAMIC_RELAY) != 0;
-    if (dynamic) flags |= PCCL_FLAG_DENSE_SWEEP;   // wants rows are dense and shrink by rule: recount by whole rows
+    // the dynamic rule's wants rows are dense and shrink by the thousand per event: keeping the counts current
+    // costs more than recounting by whole rows, so that is its default (KEPT_COUNTS overrides)
+    if (dynamic && !(flags & (PCCL_FLAG_RESCAN | PCCL_FLAG_KEPT_COUNTS))) flags |= PCCL_FLAG_DENSE_SWEEP;
     const pccl_topology* t = P.topo;
     const PhaseView pv = view_of(t, ph.transposed);
     LoopArgs a;

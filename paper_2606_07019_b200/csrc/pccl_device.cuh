@@ -480,19 +480,27 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
     if (blockIdx.x == 0 && threadIdx.x == 0) stcg64((uint64_t*)&a.ctrl->tnext[(step + 2) % 3], T_INF);
 }
 
-// ---- dynamic relay rule, end of an event (Q18).  U: every claim (c, v) of the event tightens
-// best[p] = min(best[p], dist(v -> d_p)) for the pairs p of c.  (grid barrier.)  W: for every claimed chunk,
-// each node that is no longer strictly closer to some dest than the best holder stops wanting it.
-__device__ __forceinline__ void dyn_update_best(const LoopArgs& a, uint32_t step) {
-    const uint64_t* mb = a.matchbits + (size_t)(step & 1) * a.nLw;
-    for (uint32_t l = blockIdx.x * blockDim.x + threadIdx.x; l < a.L; l += gridDim.x * blockDim.x) {
-        if (!((ldcg64(mb + (l >> 6)) >> (l & 63)) & 1ull)) continue;
-        const uint32_t c = ldcg32(a.inflight + l), v = a.edst[l];
-        const uint64_t p1 = a.dest_off[c + 1];
-        for (uint64_t p = a.dest_off[c]; p < p1; ++p)
-            atomicMin((unsigned long long*)&a.best[p], (unsigned long long)a.Dto[(size_t)a.didx[a.dests[p]] * a.N + v]);
+// ---- dynamic relay rule, end of an event (Q18).  Every claim (c, v) of the event has tightened
+// best[p] = min(best[p], dist(v -> d_p)) for the pairs p of c at commit; after the event's barrier, for every
+// claimed chunk, each node that is no longer strictly closer to some dest than the best holder stops wanting it
+// (and, with kept counts, its in-links lose the candidate).  A barrier follows: arrivals read wants.
+// v stops wanting c (dynamic rule): clear the bit once, and with kept counts take the candidate away from every
+// in-link of u whose source holds c
+__device__ __forceinline__ void dyn_drop(const LoopArgs& a, uint32_t u, uint32_t c) {
+    const unsigned long long bit = 1ull << (c & 63);
+    if (!(atomicAnd((unsigned long long*)&a.wants[(size_t)u * a.Wp + (c >> 6)], ~bit) & bit)) return;   // once per (u, c)
+    atomicSub(&a.wants_cnt[u], 1u);
+    if (a.gcnt == nullptr) return;
+    const uint32_t e1 = a.in_off[u + 1];
+    for (uint32_t e = a.in_off[u]; e < e1; ++e) {
+        const uint32_t l2 = a.in_link[e];
+        if ((ldcg64(a.have + (size_t)a.esrc[l2] * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) {
+            atomicSub(&a.gcnt[(size_t)l2 * a.S + (c >> 12)], 1u);
+            atomicSub(&a.gtot[l2], 1u);
+        }
     }
 }
+
 __device__ __forceinline__ void dyn_shrink_wants(const LoopArgs& a, uint32_t step) {
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nW = (gridDim.x * blockDim.x) >> 5;
@@ -502,13 +510,40 @@ __device__ __forceinline__ void dyn_shrink_wants(const LoopArgs& a, uint32_t ste
         const uint32_t c = ldcg32(a.inflight + l);
         const uint64_t p0 = a.dest_off[c], p1 = a.dest_off[c + 1];
         const unsigned long long bit = 1ull << (c & 63);
-        for (uint32_t u = lane; u < a.N; u += 32) {
-            unsigned long long* wp = (unsigned long long*)&a.wants[(size_t)u * a.Wp + (c >> 6)];
-            if (!(ldcg64((const uint64_t*)wp) & bit)) continue;
-            bool keep = false;
-            for (uint64_t p = p0; p < p1 && !keep; ++p)
-                keep = a.Dto[(size_t)a.didx[a.dests[p]] * a.N + u] < ldcg64(a.best + p);
-            if (!keep && (atomicAnd(wp, ~bit) & bit)) atomicSub(&a.wants_cnt[u], 1u);   // once per (u, c)
+        if (p1 - p0 <= 32) {
+            // lane q holds pair q (row of its dest in Dto, current best); four nodes per lane and round, their
+            // wants words loaded together, then one coalesced Dto load per pair and node
+            const uint32_t np = (uint32_t)(p1 - p0);
+            uint32_t row = 0;
+            unsigned long long bst = 0;
+            if (lane < np) { row = a.didx[a.dests[p0 + lane]]; bst = ldcg64(a.best + p0 + lane); }
+            for (uint32_t ub = 0; ub < a.N; ub += 128) {
+                bool need[4], keep[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint32_t u = ub + 32 * k + lane;
+                    need[k] = u < a.N && (ldcg64(a.wants + (size_t)u * a.Wp + (c >> 6)) & bit) != 0ull;
+                    keep[k] = false;
+                }
+                for (uint32_t q = 0; q < np; ++q) {
+                    const uint32_t r = __shfl_sync(0xFFFFFFFFu, row, q);
+                    const unsigned long long b = __shfl_sync(0xFFFFFFFFu, bst, q);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k)
+                        if (need[k] && !keep[k]) keep[k] = a.Dto[(size_t)r * a.N + ub + 32 * k + lane] < b;
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (need[k] && !keep[k]) dyn_drop(a, ub + 32 * k + lane, c);
+            }
+        } else {
+            for (uint32_t u = lane; u < a.N; u += 32) {
+                if (!(ldcg64(a.wants + (size_t)u * a.Wp + (c >> 6)) & bit)) continue;
+                bool keep = false;
+                for (uint64_t p = p0; p < p1 && !keep; ++p)
+                    keep = a.Dto[(size_t)a.didx[a.dests[p]] * a.N + u] < ldcg64(a.best + p);
+                if (!keep) dyn_drop(a, u, c);
+            }
         }
     }
 }
@@ -600,6 +635,11 @@ __device__ __forceinline__ uint64_t commit_claim(const LoopArgs& a, uint32_t v, 
     stcg32(a.inflight + l, c);
     stcg64(a.free_t + l, te);
     atomicOr((unsigned long long*)&a.matchbits[(size_t)(step & 1) * a.nLw + (l >> 6)], 1ull << (l & 63));
+    if (a.best != nullptr) {   // dynamic relay rule: v is now a holder of c (read only after the event's barrier)
+        const uint64_t p1 = a.dest_off[c + 1];
+        for (uint64_t p = a.dest_off[c]; p < p1; ++p)
+            atomicMin((unsigned long long*)&a.best[p], (unsigned long long)a.Dto[(size_t)a.didx[a.dests[p]] * a.N + v]);
+    }
     return te;
 }
 
@@ -1015,9 +1055,10 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop(const Loop
         total_now = s_next[1];
         __syncthreads();
         if (a.best != nullptr && t != T_INF) {   // (the last event never has claims)
-            dyn_update_best(a, step);
+            dyn_shrink_wants(a, step);
+            trace_stamp(a, step, 10);
             grid.sync();
-            dyn_shrink_wants(a, step);   // runs beside the next links phase: both end at its barrier
+            trace_stamp(a, step, 11);
         }
         ++step;
         if (t == T_INF) break;

@@ -306,6 +306,14 @@ def test_dynamic_relay_rings_mesh_star_and_ragged_rows(pk):
         assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY), o)
 
 
+@pytest.mark.parametrize("maker", [wl.config2, wl.config3, wl.config4_small, wl.config5_small], ids=lambda m: m.__name__)
+def test_dynamic_relay_three_counting_modes(pk, maker):
+    p = maker(1)
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_DYNAMIC)
+    for fl in (0, pk.PCCL_FLAG_KEPT_COUNTS, pk.PCCL_FLAG_RESCAN, pk.PCCL_FLAG_DENSE_SWEEP):
+        assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY | fl), o)
+
+
 def test_dynamic_relay_unreachable(pk):
     links = np.array([(0, 1, 5, 1)], dtype=wl.LINK_DT)
     members = np.array([0, 1], dtype=np.uint32)
