@@ -334,3 +334,41 @@ def test_dynamic_relay_6x6x6_torus_all_to_all(pk):
     s = gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY)
     assert_same(p, s, o)
     checker.check_structure(p, s.transfers)
+
+
+# ------------------------------------------------------------------------------ scale / shape stress
+def _torus_all_gather(dims, cpn, seed):
+    n = int(np.prod(dims))
+    m = np.arange(n, dtype=np.uint32)
+    nc, pre, post = wl.all_gather(m, cpn)
+    return wl.Problem(f"torus{'x'.join(map(str, dims))}_allgather{cpn}", n, wl.grid_links(dims, wrap=True), m, nc,
+                      pre, post, 1 << 16, seed)
+
+
+def _ring3000_a2a(seed):
+    n = 3000
+    mem = np.array([0, 400, 777, 1200, 1500, 2100, 2500, 2999], dtype=np.uint32)
+    nc, pre, post = wl.all_to_all(mem, np.full((8, 8), 3))
+    return wl.Problem("ring3000_a2a8", n, wl.ring_links(n, True), mem, nc, pre, post, 1 << 12, seed)
+
+
+@pytest.mark.parametrize("relay", [0, 1])
+def test_multi_dest_trees_at_scale(pk, relay):
+    """144-NPU torus All-Gather, 288 chunks with 143 dests each: every sweep has overlapping in-links (the
+    serial re-pick path), multi-dest relay trees, 41 k transfers."""
+    p = _torus_all_gather((12, 12), 2, 7)
+    o = oracle.synthesize(*p.args(), relay=relay)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY if relay else 0)
+    assert_same(p, s, o)
+    checker.check_structure(p, s.transfers)
+
+
+@pytest.mark.parametrize("relay", [0, 1])
+def test_more_nodes_than_resident_ctas(pk, relay):
+    """3000-node ring, 8 members: every CTA serves several destinations (the third and later from the
+    uncached tables), 1,500 events, almost all nodes only relay."""
+    p = _ring3000_a2a(3)
+    o = oracle.synthesize(*p.args(), relay=relay)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY if relay else 0)
+    assert_same(p, s, o)
+    checker.check_structure(p, s.transfers)
