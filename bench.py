@@ -394,6 +394,43 @@ def run_ours(args):
     return 0
 
 
+def run_fig12(args):
+    """Context run shaped like the paper's Fig. 12: All-to-All on 64 NPUs (8x8 mesh and
+    4x4x4 torus), 128 KiB chunks, 1..64 chunks per (source, destination) pair, i.e. 8..512 MiB per NPU.  The
+    paper reports 1.83 min for the 512 MiB point on its (unstated) host with its BFS procedure."""
+    import numpy as np
+    import torch
+    import paper_2606_07019_b200 as pk
+    import workloads as wl
+    pk.use_torch(0)
+    rows = []
+    for name, dims, wrap in (("mesh8x8", (8, 8), False), ("torus4x4x4", (4, 4, 4), True)):
+        links = wl.grid_links(dims, wrap=wrap)
+        members = np.arange(64, dtype=np.uint32)
+        topo = pk.Topology(64, links)
+        for k in (1, 2, 4, 8, 16, 32, 64):
+            nc, pre, post = wl.all_to_all(members, np.full((64, 64), k))
+            prob = pk.Problem(topo, members, nc, pre, post, 128 << 10)
+            prob.upload()
+            ms = []
+            for i in range(4):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                s = prob.synthesize(0, pk.PCCL_FLAG_KEEP_ON_DEVICE)
+                e1.record()
+                e1.synchronize()
+                if i:
+                    ms.append(e0.elapsed_time(e1))
+                m, t, ev = s.size, s.time_ps, s.stats["events"]
+                s.close()
+            rows.append({"topology": name, "chunks_per_pair": k, "mib_per_npu": k * 64 * 128 // 1024, "chunks": nc,
+                         "transfers": m, "events": ev, "synthesis_ms": sorted(ms)[1], "schedule_time_ps": t})
+            prob.close()
+        topo.close()
+    print(json.dumps({"experiment": "fig12-shaped chunks-per-NPU sweep (context)", "rows": rows}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -403,7 +440,10 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true")
+    ap.add_argument("--fig12", action="store_true", help="chunks-per-NPU sweep shaped like the paper's Fig. 12")
     args = ap.parse_args()
+    if args.fig12:
+        return run_fig12(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)
