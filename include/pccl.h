@@ -168,6 +168,7 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
                                        takes a chunk iff it is strictly closer to some destination than the
                                        source and every node that claimed the chunk at an earlier event
                                        (fewer link-times, a few unused deliveries; recounts by dense sweep unless KEPT_COUNTS or RESCAN) */
+#define PCCL_FLAG_TWO_BARRIERS 256u /* run the two-barrier event loop even where the one-barrier loop applies */
 #define PCCL_FLAG_KEPT_COUNTS 128u  /* with DYNAMIC_RELAY: keep the counts current instead of its default dense recount */
 #define PCCL_FLAG_RESCAN 32u        /* recount every free link's candidates at every event from the bitmaps
                                        (sector work list), instead of keeping the counts current */

@@ -32,6 +32,7 @@ PCCL_FLAG_DENSE_SWEEP = 16
 PCCL_FLAG_RESCAN = 32
 PCCL_FLAG_DYNAMIC_RELAY = 64
 PCCL_FLAG_KEPT_COUNTS = 128
+PCCL_FLAG_TWO_BARRIERS = 256
 PCCL_TRACE_SLOTS = 12
 
 

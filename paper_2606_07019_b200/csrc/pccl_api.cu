@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "pccl_device.cuh"
+#include "pccl_loop1.cuh"
 
 using namespace pccl;
 
@@ -559,6 +560,8 @@ struct Work {   // device workspace of one phase
     uint64_t *hsum = nullptr, *wsum = nullptr;
     uint32_t *gcnt = nullptr, *gtot = nullptr;
     uint64_t* best = nullptr;
+    uint64_t* st_free = nullptr;
+    uint32_t* st_inf = nullptr;
     uint32_t Wp = 0, S = 0, nLw = 0, SWp = 0;
     size_t zero_off = 0, zero_bytes = 0;   // have + wants + wants_cnt + ctrl are cleared per run
 };
@@ -582,9 +585,9 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.SWp = (uint32_t)align_up((W.Wp / 4 + 63) / 64, 2);          // one summary bit per 4-word sector
     if (loop_smem_bytes(W.S) > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
     Carver c;
-    const size_t o_best = c.take(max_pairs * 8);
+    const size_t o_best = c.take(max_pairs * 8), o_sf = c.take(L * 2 * 8), o_si = c.take(L * 2 * 4);
     const size_t o_w = c.take(L * 8), o_D = c.take(max_sources * N * 8), o_free = c.take(L * 8),
-                 o_mb = c.take((size_t)2 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4),
+                 o_mb = c.take((size_t)3 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4),
                  o_gc = c.take(L * W.S * 4), o_gt = c.take(L * 4);
     W.zero_off = c.cur;
     const size_t o_have = c.take(N * W.Wp * 8), o_wants = c.take(N * W.Wp * 8), o_hs = c.take(N * W.SWp * 8),
@@ -599,6 +602,7 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.hsum = (uint64_t*)(b + o_hs); W.wsum = (uint64_t*)(b + o_ws);
     W.gcnt = (uint32_t*)(b + o_gc); W.gtot = (uint32_t*)(b + o_gt);
     W.best = (uint64_t*)(b + o_best);
+    W.st_free = (uint64_t*)(b + o_sf); W.st_inf = (uint32_t*)(b + o_si);
     W.wants_cnt = (uint32_t*)(b + o_wc); W.ctrl = (LoopCtrl*)(b + o_ctrl);
     return PCCL_OK;
 }
@@ -710,23 +714,35 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
         a.trace = (uint64_t*)trace_dev;
     }
     struct TraceGuard { void* p; ~TraceGuard() { dev_free(p); } } trace_guard{trace_dev};
-    const uint32_t n_init = std::max(std::max(a.L, a.N), std::max(2 * a.nLw, 1u));
-    k_loop_init<<<(n_init + 255) / 256, 256, 0, st>>>(a);
-    if (a.gcnt != nullptr && a.L) k_count_init<<<a.L, 256, 0, st>>>(a);
+    const uint32_t n_init = std::max(std::max(a.L, a.N), std::max(3 * a.nLw, 1u));
     // one warp per in-link of a sweep: destinations with at most 4 in-links run in 128-thread CTAs (8 per SM),
     // so that twice as many destinations are resident at once
     const uint32_t max_deg = ph.transposed ? t->max_out : t->max_in;
     const bool small = max_deg <= 4;
-    const void* kern = small ? (const void*)k_loop<4> : (const void*)k_loop<8>;
     const int threads = small ? 128 : 256;
     const size_t smem = loop_smem_bytes(W.S, small ? 4 : 8);
-    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int occ = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
-    if (occ < 1) return PCCL_ERR_CUDA;
-    const uint32_t max_grid = (uint32_t)occ * (uint32_t)G.sm_count;
-    const uint32_t want = std::max(std::max(a.N, (a.L + threads - 1) / threads), 1u);
-    const uint32_t grid = std::min(max_grid, want);
+    // the one-barrier loop (pccl_loop1.cuh): kept counts, <= 8 in-links per node, <= 128 segments per row,
+    // at most DEST_CACHE destinations per CTA; everything else runs the two-barrier loop
+    bool fast = !rescan && !dynamic && !(flags & (PCCL_FLAG_TRACE | PCCL_FLAG_TWO_BARRIERS)) && max_deg <= 8 && W.S <= 128;
+    const void* kern = nullptr;
+    uint32_t grid = 0;
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        kern = fast ? (small ? (const void*)k_loop1<4> : (const void*)k_loop1<8>)
+                    : (small ? (const void*)k_loop<4> : (const void*)k_loop<8>);
+        if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int occ = 0;
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
+        if (occ < 1) return PCCL_ERR_CUDA;
+        const uint32_t max_grid = (uint32_t)occ * (uint32_t)G.sm_count;
+        const uint32_t want = std::max(std::max(a.N, (a.L + threads - 1) / threads), 1u);
+        grid = std::min(max_grid, want);
+        if (fast && (uint64_t)a.N > (uint64_t)DEST_CACHE * grid) { fast = false; continue; }
+        break;
+    }
+    a.st_free = fast ? W.st_free : nullptr;
+    a.st_inf = fast ? W.st_inf : nullptr;
+    k_loop_init<<<(n_init + 255) / 256, 256, 0, st>>>(a);
+    if (a.gcnt != nullptr && a.L) k_count_init<<<a.L, 256, 0, st>>>(a);
     void* args[] = {(void*)&a};
     CU(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(threads), args, smem, st));
     LoopCtrl* mb = (LoopCtrl*)G.mailbox;

@@ -324,6 +324,8 @@ struct LoopArgs {
     const uint64_t* dest_off;   // [C+1] pairs of each chunk
     const uint32_t* dests;      // [pairs]
     uint64_t out_cap;           // records the output buffer holds
+    uint64_t* st_free;          // [2][L] link state double-buffered by event parity (k_loop1 only)
+    uint32_t* st_inf;
     uint64_t* trace;        // optional [events][TRACE_SLOTS] globaltimer stamps of CTA 0 (diagnostic), or null
     uint32_t trace_cap;     // events the trace buffer holds
 };
@@ -371,7 +373,11 @@ __global__ void k_loop_init(LoopArgs a) {
         a.empty_epoch[i] = 0;
     }
     if (i < a.N) a.have_epoch[i] = 0;
-    if (i < 2 * a.nLw) a.matchbits[i] = 0;
+    if (i < a.L && a.st_free != nullptr) {
+        a.st_free[i] = 0; a.st_free[a.L + i] = 0;
+        a.st_inf[i] = NONE32; a.st_inf[a.L + i] = NONE32;
+    }
+    if (i < 3 * a.nLw) a.matchbits[i] = 0;
     if (i == 0) {
         a.ctrl->tnext[0] = 0;
         a.ctrl->tnext[1] = T_INF;
@@ -567,12 +573,14 @@ struct LoopStats {
     unsigned long long rows, links, slow, bytes;
 };
 
+// (`extra[0..nextra)`: chunks to treat as held by the source although their have bit is not stored yet.)
 // The k-th candidate (0-based, ascending chunk id) of link-row `hrow` AND wants-row `wrow`, given the
 // per-segment candidate counts cj[0..S).  `excl[0..nex)` are chunks to treat as no longer wanted (claims
 // made earlier in the same sweep); cj must already be net of them.  Whole warp; returns the chunk id.
 __device__ __forceinline__ uint32_t kth_candidate(const uint32_t* cj, uint32_t S, uint32_t Q, const uint4* hrow,
                                                   const uint4* wrow, uint32_t rem, const uint32_t* excl,
-                                                  uint32_t nex, uint32_t lane, bool& sector_empty) {
+                                                  uint32_t nex, uint32_t lane, bool& sector_empty,
+                                                  const uint32_t* extra = nullptr, uint32_t nextra = 0) {
     uint32_t seg = 0;
     for (uint32_t sb = 0; sb < S; sb += 32) {
         const uint32_t x = (sb + lane < S) ? cj[sb + lane] : 0u;
@@ -589,7 +597,18 @@ __device__ __forceinline__ uint32_t kth_candidate(const uint32_t* cj, uint32_t S
     }
     const uint32_t q = seg * SEG_U4 + lane;
     uint4 m4 = make_uint4(0, 0, 0, 0), wv = m4;
-    if (q < Q) { wv = ldcg128(wrow + q); m4 = and128(ldcg128(hrow + q), wv); }
+    if (q < Q) {
+        wv = ldcg128(wrow + q);
+        uint4 hv = ldcg128(hrow + q);
+        for (uint32_t i = 0; i < nextra; ++i) {   // chunks the source holds as of now but whose bit is not stored yet
+            const uint32_t c = extra[i];
+            if (c != NONE32 && (c >> 7) == q) {
+                const uint32_t b = c & 127u, bitm = 1u << (b & 31);
+                if (b < 32) hv.x |= bitm; else if (b < 64) hv.y |= bitm; else if (b < 96) hv.z |= bitm; else hv.w |= bitm;
+            }
+        }
+        m4 = and128(hv, wv);
+    }
     for (uint32_t i = 0; i < nex; ++i) {
         const uint32_t c = excl[i];
         if ((c >> 7) == q) {

@@ -372,3 +372,16 @@ def test_more_nodes_than_resident_ctas(pk, relay):
     s = gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY if relay else 0)
     assert_same(p, s, o)
     checker.check_structure(p, s.transfers)
+
+
+# ------------------------------------------------------------------------------ the two event loops
+@pytest.mark.parametrize("maker", SMALL + [lambda s: wl.ring_all_gather(8, True, s, chunks_per_npu=1040, chunk_bytes=4096),
+                                           lambda s: _torus_all_gather((12, 12), 2, s)],
+                         ids=lambda m: getattr(m, "__name__", "case"))
+def test_one_barrier_and_two_barrier_loops_agree(pk, maker):
+    """the default picks the one-barrier loop where it applies (<= 8 in-links per node); TWO_BARRIERS forces
+    the other one.  Both must equal the oracle."""
+    p = maker(3)
+    o = oracle.synthesize(*p.args())
+    assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE), o)
+    assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_TWO_BARRIERS), o)
