@@ -39,7 +39,7 @@ if ROOT not in sys.path:
 
 METRIC = "link-chunk matches/s, 512-NPU All-to-All synthesis"
 UNIT = "matches/s"
-KERNELS_PER_STEP_COPY = 8   # k_link_cost, k_distances, k_have, k_wants, k_sum_u32, k_loop_init, k_count_init, k_loop
+KERNELS_PER_STEP_COPY = 8   # k_link_cost, k_distances, k_have, k_wants, k_sum_u32, k_loop_init, k_count_init, k_loop1
 
 
 def workload(cfg: int, seed: int):
@@ -259,7 +259,7 @@ def run_ours(args):
             if len(f) == 2 and f[0] == f"config{args.config}":
                 traffic = int(f[1])
     req_bytes = stats["bytes_requested"]
-    roofline = {"bound": "hbm", "kernel": "k_loop", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": "k_loop1 (one-barrier event loop, kept counts)", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": loop_avg_ms,
                 "kernel_share_of_step": loop_avg_ms / (tot_ms / args.steps),
@@ -271,12 +271,13 @@ def run_ours(args):
                         "read. The default kernel keeps the per-segment candidate counts current instead (arrivals "
                         "add, claims subtract) and requests only requested_bytes, so achieved can exceed the HBM "
                         "peak and the loop is bound by grid barriers and dependent L2 round trips, not bandwidth. "
-                        "rescan_sector_list and dense_sweep below are the same kernel recounting at every event "
-                        "(PCCL_FLAG_RESCAN / PCCL_FLAG_DENSE_SWEEP); dense_sweep is the plain memory-bound bitmap "
-                        "scan. At config 4 both bitmaps (2 x 16.8 MB) sit in the 126 MB L2, so DRAM traffic is far "
+                        "two_barrier_kept_counts, rescan_sector_list and dense_sweep below are the two-barrier loop "
+                        "k_loop with kept counts and recounting at every event (PCCL_FLAG_TWO_BARRIERS / _RESCAN / "
+                        "_DENSE_SWEEP); dense_sweep is the plain memory-bound bitmap scan. At config 4 both bitmaps (2 x 16.8 MB) sit in the 126 MB L2, so DRAM traffic is far "
                         "below all of these figures"}
-    # the same kernel recounting candidates at every event, timed the same way
-    for key, fl in (("rescan_sector_list", pk.PCCL_FLAG_RESCAN), ("dense_sweep", pk.PCCL_FLAG_DENSE_SWEEP)):
+    # the two-barrier loop (k_loop) with kept counts, and recounting candidates at every event, timed the same way
+    for key, fl in (("two_barrier_kept_counts", pk.PCCL_FLAG_TWO_BARRIERS), ("rescan_sector_list", pk.PCCL_FLAG_RESCAN),
+                    ("dense_sweep", pk.PCCL_FLAG_DENSE_SWEEP)):
         ms_v, stv = [], None
         for i in range(2 + min(args.steps, 5)):
             flush.zero_()
