@@ -59,9 +59,38 @@ __device__ __forceinline__ bool holds_now(const LoopArgs& a, const FastCache& fc
     return ((ldcg64(a.have + (size_t)fc.src[e] * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) != 0ull;
 }
 
+// emit the records of event `ev` (claims are in the state buffer written at that event) in canonical order.
+// 32-link tasks; the calling warp is worker `wk` of `nwk` in its CTA.
+__device__ __forceinline__ void emit_event(const LoopArgs& a, uint32_t ev, uint64_t emit_base, uint32_t wk, uint32_t nwk) {
+    const uint32_t lane = threadIdx.x & 31;
+    const uint64_t* mb = a.matchbits + (size_t)(ev % 3) * a.nLw;
+    const uint32_t wr = ((ev & 1u) ^ 1u) * a.L;
+    for (uint32_t lb = (wk * gridDim.x + blockIdx.x) * 32; lb < a.L; lb += nwk * gridDim.x * 32) {
+        const uint32_t l = lb + lane, wq = lb >> 6;
+        const uint64_t word = ldcg64(mb + wq);
+        const uint32_t mine = (uint32_t)(word >> (lb & 32));
+        if (mine == 0) continue;   // warp-uniform
+        uint32_t pre = 0;
+        for (uint32_t i = lane; i < wq; i += 32) pre += __popcll(ldcg64(mb + i));
+        pre = __reduce_add_sync(0xFFFFFFFFu, pre);
+        if (lb & 32) pre += __popc((uint32_t)word);
+        if ((mine >> lane) & 1u) {
+            const uint64_t rank = pre + __popc(mine & ((1u << lane) - 1u));
+            if (emit_base + rank >= a.out_cap) { atomicOr(&a.ctrl->err, 32u); continue; }
+            const uint32_t c = ldcg32(a.st_inf + wr + l);
+            const uint64_t f = ldcg64(a.st_free + wr + l);
+            const uint64_t ts = f - a.w[l] + a.t_offset, te = f + a.t_offset;
+            uint4* o = reinterpret_cast<uint4*>(a.out + emit_base + rank);
+            o[0] = make_uint4(c, a.psrc[l], a.pdst[l], l);
+            o[1] = make_uint4((uint32_t)ts, (uint32_t)(ts >> 32), (uint32_t)te, (uint32_t)(te >> 32));
+        }
+    }
+}
+
 template <int NBT>
 __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32_t step, uint64_t t, uint32_t* cnt,
-                                           FastScratch& sh, const FastCache& fc, LoopStats& st) {
+                                           FastScratch& sh, const FastCache& fc, LoopStats& st, bool do_emit,
+                                           uint64_t emit_base) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t Q = a.Wp >> 1, S = a.S, L = a.L;
     const uint32_t rd = (step & 1u) * L, wr = ((step & 1u) ^ 1u) * L;
@@ -266,36 +295,12 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
                 atomicMax(&a.ctrl->tmax, (unsigned long long)mymax);
             }
         }
+    } else if (do_emit) {
+        // the other warps are idle now: they emit the previous event's records (a8), which only needs that
+        // event's finished bitmap and state buffer
+        emit_event(a, step - 1, emit_base, warp - 1, NBT - 1);
     }
     __syncthreads();
-}
-
-// emit the records of event `ev` (claims are in the state buffer written at that event) in canonical order
-__device__ __forceinline__ void emit_event(const LoopArgs& a, uint32_t ev, uint64_t emit_base) {
-    const uint32_t lane = threadIdx.x & 31;
-    const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nW = (gridDim.x * blockDim.x) >> 5;
-    const uint64_t* mb = a.matchbits + (size_t)(ev % 3) * a.nLw;
-    const uint32_t wr = ((ev & 1u) ^ 1u) * a.L;
-    for (uint32_t lb = gw * 32; lb < a.L; lb += nW * 32) {
-        const uint32_t l = lb + lane, wq = lb >> 6;
-        const uint64_t word = ldcg64(mb + wq);
-        const uint32_t mine = (uint32_t)(word >> (lb & 32));
-        if (mine == 0) continue;   // warp-uniform
-        uint32_t pre = 0;
-        for (uint32_t i = lane; i < wq; i += 32) pre += __popcll(ldcg64(mb + i));
-        pre = __reduce_add_sync(0xFFFFFFFFu, pre);
-        if (lb & 32) pre += __popc((uint32_t)word);
-        if ((mine >> lane) & 1u) {
-            const uint64_t rank = pre + __popc(mine & ((1u << lane) - 1u));
-            if (emit_base + rank >= a.out_cap) { atomicOr(&a.ctrl->err, 32u); continue; }
-            const uint32_t c = ldcg32(a.st_inf + wr + l);
-            const uint64_t f = ldcg64(a.st_free + wr + l);
-            const uint64_t ts = f - a.w[l] + a.t_offset, te = f + a.t_offset;
-            uint4* o = reinterpret_cast<uint4*>(a.out + emit_base + rank);
-            o[0] = make_uint4(c, a.psrc[l], a.pdst[l], l);
-            o[1] = make_uint4((uint32_t)ts, (uint32_t)(ts >> 32), (uint32_t)te, (uint32_t)(te >> 32));
-        }
-    }
 }
 
 template <int NBT>
@@ -331,9 +336,10 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop1(const Loo
         {
             uint32_t k = 0;
             for (uint32_t v = blockIdx.x; v < a.N && k < DEST_CACHE; v += gridDim.x, ++k)
-                fast_match<NBT>(a, v, step, t, cnt, sh, fc[k], st);
+                fast_match<NBT>(a, v, step, t, cnt, sh, fc[k], st, k == 0 && step > 0, tot_prev);
+            // (a CTA without a destination still takes its share of the emit)
+            if (k == 0 && step > 0 && (threadIdx.x >> 5) != 0) emit_event(a, step - 1, tot_prev, (threadIdx.x >> 5) - 1, NBT - 1);
         }
-        if (step > 0) emit_event(a, step - 1, tot_prev);
         {   // clear the bitmap the next event writes; re-arm the ring slot after next
             uint64_t* mbn = a.matchbits + (size_t)((step + 1) % 3) * a.nLw;
             for (uint32_t i = blockIdx.x * THREADS + threadIdx.x; i < a.nLw; i += gridDim.x * THREADS) stcg64(mbn + i, 0);
