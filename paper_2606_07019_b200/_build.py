@@ -13,7 +13,7 @@ DEPS = ["pccl_api.cu", "pccl_device.cuh", "pccl_loop1.cuh", os.path.join("..", "
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v",
+    "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "-shared", "-Xptxas", "-v",
 ]
 
 

@@ -9,6 +9,8 @@
 #include <algorithm>
 #include <cstdlib>
 #include <cstring>
+#include <future>
+#include <system_error>
 #include <mutex>
 #include <new>
 #include <vector>
@@ -398,10 +400,24 @@ int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_membe
     }
     std::vector<uint64_t> pre_off, post_off;
     std::vector<uint32_t> pre_n, post_n;
-    int rc = group_pairs(pre, C, N, member, pre_off, pre_n);
+    // the two conditions are grouped independently: the postcondition on a second host thread when it is large
+    int rc, rc2;
+    if (post->n_pairs >= 65536) {
+        std::future<int> fut;
+        bool threaded = true;
+        try {
+            fut = std::async(std::launch::async, [&] { return group_pairs(post, C, N, member, post_off, post_n); });
+        } catch (const std::system_error&) {
+            threaded = false;
+        }
+        rc = group_pairs(pre, C, N, member, pre_off, pre_n);
+        rc2 = threaded ? fut.get() : group_pairs(post, C, N, member, post_off, post_n);
+    } else {
+        rc = group_pairs(pre, C, N, member, pre_off, pre_n);
+        rc2 = group_pairs(post, C, N, member, post_off, post_n);
+    }
     if (rc) return rc;
-    rc = group_pairs(post, C, N, member, post_off, post_n);
-    if (rc) return rc;
+    if (rc2) return rc2;
     bool all_single = true, all_multi_one = true, all_multi_many = true;
     for (uint32_t c = 0; c < C; ++c) {
         const uint64_t np = pre_off[c + 1] - pre_off[c], nq = post_off[c + 1] - post_off[c];
