@@ -739,7 +739,7 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     const size_t smem = loop_smem_bytes(W.S, small ? 4 : 8);
     // the one-barrier loop (pccl_loop1.cuh): kept counts, <= 8 in-links per node, <= 128 segments per row,
     // at most DEST_CACHE destinations per CTA; everything else runs the two-barrier loop
-    bool fast = !rescan && !dynamic && !(flags & (PCCL_FLAG_TRACE | PCCL_FLAG_TWO_BARRIERS)) && max_deg <= 8 && W.S <= 128;
+    bool fast = !rescan && !dynamic && !(flags & PCCL_FLAG_TWO_BARRIERS) && max_deg <= 8 && W.S <= 128;
     const void* kern = nullptr;
     uint32_t grid = 0;
     for (int attempt = 0; attempt < 2; ++attempt) {

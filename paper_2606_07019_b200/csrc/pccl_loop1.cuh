@@ -119,6 +119,9 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
         for (int x = 0; x < 4; ++x)
             if (lane + 32u * x < S) rowv[x] = ldcg32(g + lane + 32u * x);
     }
+    // the pick's random draw depends only on (t, link): computed while the loads are in flight
+    uint32_t r_pre = 0;
+    if (warp < n_in) r_pre = philox_draw((uint32_t)t, (uint32_t)(t >> 32), fc.link[warp], 0u, a.k0, a.k1);
     // ---- consume -----------------------------------------------------------------------------------
     if (is_own) {
         const bool arrived = c_own != NONE32 && f_own == t;   // a3: the chunk is at v from now on
@@ -144,6 +147,7 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
     }
     if (tid == 0) sh.wc = wc0;
     __syncthreads();
+    trace_stamp(a, step, 1);
 
     // ---- per in-link: count upkeep for the pending chunks, then the pick (a5, a6) ---------------------
     if (warp < n_in) {
@@ -163,8 +167,7 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
         uint32_t c = NONE32;
         bool sem = false;
         if (sh.free_[j] <= t && n != 0u && wc0 != 0u) {
-            const uint32_t r = philox_draw((uint32_t)t, (uint32_t)(t >> 32), l, 0u, a.k0, a.k1);
-            c = kth_candidate(cj, S, Q, have4 + (size_t)fc.src[j] * Q, wrow, __umulhi(r, n), nullptr, 0, lane, sem,
+            c = kth_candidate(cj, S, Q, have4 + (size_t)fc.src[j] * Q, wrow, __umulhi(r_pre, n), nullptr, 0, lane, sem,
                               sh.pend_c + h0, h1 - h0);
             if (c == NONE32 && lane == 0) atomicOr(&a.ctrl->err, 4u);   // cannot happen
             if (lane == 0) {
@@ -173,25 +176,21 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
                 st.rows += 1;
             }
         }
-        if (lane == 0) { sh.spec[j] = c; sh.sempty[j] = sem; sh.newc[j] = NONE32; }
+        // which in-links' sources hold the pick (stored or arriving now)?  lane e answers for in-link e; the mask
+        // serves the conflict test and the count upkeep
+        uint32_t hit = 0;
+        if (c != NONE32 && lane < n_in) hit = holds_now(a, fc, sh, lane, c);
+        const uint32_t hm = __ballot_sync(0xFFFFFFFFu, hit != 0u);
+        if (lane == 0) { sh.spec[j] = c; sh.sempty[j] = sem; sh.newc[j] = NONE32; sh.pbits[j] = hm; }
     }
     __syncthreads();
+    trace_stamp(a, step, 2);
 
     // ---- conflict resolve, commit, count upkeep, next state (a7, a8): warp 0 ---------------------------
     if (warp == 0) {
         uint64_t mymin = T_INF, mymax = 0;
-        if (lane < NB) sh.pbits[lane] = 0;
-        __syncwarp();
         uint32_t anyspec = 0;
-        for (uint32_t p0 = 0; p0 < n_in * n_in; p0 += 32) {   // pair (pick i, in-link e): does e's source hold pick i?
-            const uint32_t p = p0 + lane;
-            if (p < n_in * n_in) {
-                const uint32_t i = p / n_in, e = p - i * n_in;
-                const uint32_t ci = sh.spec[i];
-                if (ci != NONE32 && holds_now(a, fc, sh, e, ci)) atomicOr(&sh.pbits[i], 1u << e);
-            }
-        }
-        __syncwarp();
+        trace_stamp(a, step, 6);
         uint32_t bad = 0;
         if (lane < n_in) {
             anyspec = sh.spec[lane] != NONE32;
@@ -221,6 +220,7 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
         }
         uint32_t ncl = __popc(__ballot_sync(0xFFFFFFFFu, lane < first_bad && sh.spec[lane] != NONE32));
         __syncwarp();
+        trace_stamp(a, step, 7);
         if (lane < n_in) {   // count upkeep for the committed picks: lane e owns in-link e
             const uint32_t l2 = fc.link[lane];
             uint32_t dec = 0;
@@ -273,6 +273,7 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
             __syncwarp();
         }
         __syncwarp();
+        trace_stamp(a, step, 8);
         // next state of every own in-link (the buffer the next event reads)
         if (lane < n_in) {
             const uint32_t l = fc.link[lane];
@@ -295,6 +296,7 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
                 atomicMax(&a.ctrl->tmax, (unsigned long long)mymax);
             }
         }
+        trace_stamp(a, step, 9);
     } else if (do_emit) {
         // the other warps are idle now: they emit the previous event's records (a8), which only needs that
         // event's finished bitmap and state buffer
@@ -333,6 +335,7 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop1(const Loo
     uint32_t step = 0;
     uint64_t t = 0, tot_prev = 0, tot_cur = 0;
     for (;;) {
+        trace_stamp(a, step, 0);
         {
             uint32_t k = 0;
             for (uint32_t v = blockIdx.x; v < a.N && k < DEST_CACHE; v += gridDim.x, ++k)
@@ -340,12 +343,15 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop1(const Loo
             // (a CTA without a destination still takes its share of the emit)
             if (k == 0 && step > 0 && (threadIdx.x >> 5) != 0) emit_event(a, step - 1, tot_prev, (threadIdx.x >> 5) - 1, NBT - 1);
         }
+        trace_stamp(a, step, 3);
         {   // clear the bitmap the next event writes; re-arm the ring slot after next
             uint64_t* mbn = a.matchbits + (size_t)((step + 1) % 3) * a.nLw;
             for (uint32_t i = blockIdx.x * THREADS + threadIdx.x; i < a.nLw; i += gridDim.x * THREADS) stcg64(mbn + i, 0);
             if (blockIdx.x == 0 && threadIdx.x == 0) stcg64((uint64_t*)&a.ctrl->tnext[(step + 2) % 3], T_INF);
         }
+        trace_stamp(a, step, 4);
         grid.sync();
+        trace_stamp(a, step, 5);
         if (threadIdx.x == 0) {
             s_next[0] = ldcg64((const uint64_t*)&a.ctrl->tnext[(step + 1) % 3]);
             s_next[1] = ldcg64((const uint64_t*)&a.ctrl->total);
