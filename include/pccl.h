@@ -192,6 +192,19 @@ const pccl_transfer_t* pccl_schedule_transfers(pccl_schedule_t* s);
 const pccl_transfer_t* pccl_schedule_transfers_device(const pccl_schedule_t* s);
 void pccl_schedule_destroy(pccl_schedule_t* s);
 
+/* Translation (section 4.8): the schedule as one program per node.  Every transfer gives
+ * two operations: kind 0 = its destination RECEIVES `chunk` from `peer` over `link`, complete at time_ps =
+ * t_end; kind 1 = its source SENDS `chunk` to `peer` over `link`, starting at time_ps = t_start.  A node's
+ * program lists its operations by (time_ps, kind, link) -- a receive precedes a send at the same instant
+ * (store-and-forward).  offsets: host, n_npus + 1 entries; the program of node v is
+ * ops[offsets[v] .. offsets[v+1]).  ops: host, 2 * pccl_schedule_size(s) entries.  Built on the GPU (two
+ * stable radix sorts) from the device copy of the transfers.  Errors: INVALID, UNSUPPORTED, CUDA, NOMEM. */
+typedef struct pccl_op {
+    uint32_t kind, peer, chunk, link;
+    uint64_t time_ps;
+} pccl_op_t;
+int pccl_schedule_programs(pccl_schedule_t* s, uint64_t* offsets, pccl_op_t* ops);
+
 /* Counters of the run that produced the schedule. */
 typedef struct pccl_stats {
     uint64_t events;         /* event times processed (both phases of an all-reduce summed) */

@@ -175,3 +175,24 @@ def schedule_hash(transfers: np.ndarray) -> str:
         for f in ("chunk", "src", "dst", "link", "t_start_ps", "t_end_ps"):
             h = ((h ^ int(r[f])) * 0x100000001B3) & mask
     return f"{h:016x}"
+
+
+OP_DT = np.dtype([("kind", "<u4"), ("peer", "<u4"), ("chunk", "<u4"), ("link", "<u4"), ("time_ps", "<u8")])
+
+
+def programs(transfers: np.ndarray, n_npus: int):
+    """Translation step (section 4.8) written out: every transfer is a RECEIVE (kind 0) at its
+    destination, complete at t_end, and a SEND (kind 1) at its source, starting at t_start; a node's program is
+    its operations ordered by (time, kind, link).  Returns (offsets[n_npus + 1], ops)."""
+    m = len(transfers)
+    node = np.concatenate([transfers["dst"], transfers["src"]]).astype(np.int64)
+    ops = np.zeros(2 * m, dtype=OP_DT)
+    ops["kind"] = np.concatenate([np.zeros(m, np.uint32), np.ones(m, np.uint32)])
+    ops["peer"] = np.concatenate([transfers["src"], transfers["dst"]])
+    ops["chunk"] = np.concatenate([transfers["chunk"], transfers["chunk"]])
+    ops["link"] = np.concatenate([transfers["link"], transfers["link"]])
+    ops["time_ps"] = np.concatenate([transfers["t_end_ps"], transfers["t_start_ps"]])
+    order = np.lexsort((ops["link"], ops["kind"], ops["time_ps"], node))   # last key is the primary one
+    offsets = np.zeros(n_npus + 1, dtype=np.uint64)
+    offsets[1:] = np.cumsum(np.bincount(node, minlength=n_npus))
+    return offsets, ops[order]

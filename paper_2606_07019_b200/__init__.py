@@ -22,6 +22,7 @@ from . import _build
 
 LINK_DT = np.dtype([("src", "<u4"), ("dst", "<u4"), ("alpha_ps", "<u8"), ("bytes_per_ps", "<u8")])
 PAIR_DT = np.dtype([("npu", "<u4"), ("chunk", "<u4")])
+OP_DT = np.dtype([("kind", "<u4"), ("peer", "<u4"), ("chunk", "<u4"), ("link", "<u4"), ("time_ps", "<u8")])
 TRANSFER_DT = np.dtype([("chunk", "<u4"), ("src", "<u4"), ("dst", "<u4"), ("link", "<u4"),
                         ("t_start_ps", "<u8"), ("t_end_ps", "<u8")])
 
@@ -78,6 +79,7 @@ SIGNATURES = {
     "pccl_schedule_destroy": (None, [_vp]),
     "pccl_schedule_stats": (_int, [_vp, C.POINTER(pccl_stats_t)]),
     "pccl_schedule_trace": (_i64, [_vp, _vp, _u64]),
+    "pccl_schedule_programs": (_int, [_vp, _vp, _vp]),
     "pccl_device_philox": (_int, [_vp, _u64, _vp, _vp]),
     "pccl_device_link_costs": (_int, [_vp, _u64, _vp]),
     "pccl_device_distances": (_int, [_vp, _u64, _u32, _int, _vp]),
@@ -213,6 +215,13 @@ class Schedule:
         s = pccl_stats_t()
         _check(lib.pccl_schedule_stats(self.handle, C.byref(s)))
         return {k: getattr(s, k) for k, _ in pccl_stats_t._fields_}
+
+    def programs(self, n_npus: int):
+        """(offsets, ops): the program of node v is ops[offsets[v]:offsets[v+1]] (OP_DT records)."""
+        offsets = np.zeros(n_npus + 1, dtype=np.uint64)
+        ops = np.zeros(2 * self.size, dtype=OP_DT)
+        _check(lib.pccl_schedule_programs(self.handle, _ptr(offsets), _ptr(ops)))
+        return offsets, ops
 
     @property
     def trace(self) -> np.ndarray:

@@ -176,6 +176,7 @@ struct pccl_problem {
 
 struct pccl_schedule {
     uint64_t M = 0, T = 0;
+    uint32_t n_links = 0, n_npus = 0;
     Rec* d_recs = nullptr;
     void* h_recs = nullptr;
     size_t h_bytes = 0;
@@ -779,6 +780,19 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     return PCCL_OK;
 }
 
+// stable LSD radix sort of (key, value) pairs on the low `bits` bits; returns which of the two buffers holds the result
+int radix_sort_pairs(uint64_t* keys[2], uint32_t* vals[2], uint64_t n, uint32_t bits, uint32_t* ghist, uint32_t nblocks,
+                     int cur) {
+    cudaStream_t st = G.stream;
+    for (uint32_t shift = 0; shift < bits; shift += 8) {
+        k_sort_hist<<<nblocks, SORT_THREADS, 0, st>>>(keys[cur], n, shift, ghist, nblocks);
+        k_sort_scan<<<1, 1024, 0, st>>>(ghist, (uint64_t)256 * nblocks);
+        k_sort_scatter<<<nblocks, SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n, shift, ghist, nblocks);
+        cur ^= 1;
+    }
+    return cur;
+}
+
 // a9 for reductions: raw (transposed-broadcast) records -> reversed, sorted by (t_start, link), into out
 int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out) {
     if (M == 0) return PCCL_OK;
@@ -801,13 +815,7 @@ int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out) {
     uint32_t* ghist = (uint32_t*)(b + o_h);
     const unsigned g256 = (unsigned)((M + 255) / 256);
     k_reverse_keys<<<g256, 256, 0, st>>>(raw, M, T, link_bits, keys[0], vals[0]);
-    int cur = 0;
-    for (uint32_t shift = 0; shift < t_bits + link_bits; shift += 8) {
-        k_sort_hist<<<nblocks, SORT_THREADS, 0, st>>>(keys[cur], M, shift, ghist, nblocks);
-        k_sort_scan<<<1, 1024, 0, st>>>(ghist, (uint64_t)256 * nblocks);
-        k_sort_scatter<<<nblocks, SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], M, shift, ghist, nblocks);
-        cur ^= 1;
-    }
+    const int cur = radix_sort_pairs(keys, vals, M, t_bits + link_bits, ghist, nblocks, 0);
     k_gather_shift<<<g256, 256, 0, st>>>(raw, vals[cur], M, 0, out);
     cudaError_t e = cudaGetLastError();
     dev_free(blob);   // stream-ordered: freed after the kernels above
@@ -926,6 +934,8 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
     dev_free(W.blob); W.blob = nullptr;
     dev_free(stage1); stage1 = nullptr;
     S->d_recs = out_recs;
+    S->n_links = P->topo->L;
+    S->n_npus = P->topo->N;
     S->stats.loop_ms = t_loop.acc; S->stats.setup_ms = t_setup.acc; S->stats.emit_ms = t_emit.acc;
     if (!(flags & PCCL_FLAG_KEEP_ON_DEVICE)) {
         if (S->M && !pccl_schedule_transfers(S)) { pccl_schedule_destroy(S); return PCCL_ERR_CUDA; }
@@ -979,6 +989,53 @@ extern "C" void pccl_schedule_destroy(pccl_schedule_t* s) {
     pinned_put(s->h_recs, s->h_bytes);
     delete s;
 }
+static_assert(sizeof(pccl_op_t) == sizeof(Op), "op layout");
+
+extern "C" int pccl_schedule_programs(pccl_schedule_t* s, uint64_t* offsets, pccl_op_t* ops) {
+    if (!s || !offsets || (s->M && !ops)) return PCCL_ERR_INVALID;
+    const uint32_t N = s->n_npus;
+    const uint64_t M = s->M, n = 2 * M;
+    if (M == 0) {
+        for (uint32_t v = 0; v <= N; ++v) offsets[v] = 0;
+        return PCCL_OK;
+    }
+    if (!s->d_recs) return PCCL_ERR_INVALID;
+    uint32_t link_bits = 1;
+    while ((1ull << link_bits) < (uint64_t)s->n_links) ++link_bits;
+    uint32_t t_bits = 1;
+    while (t_bits < 64 && (s->T >> t_bits)) ++t_bits;
+    uint32_t node_bits = 1;
+    while ((1ull << node_bits) < (uint64_t)N) ++node_bits;
+    if (t_bits + 1 + link_bits > 64 || n > 0xFFFFFFFFull) return PCCL_ERR_UNSUPPORTED;
+    cudaStream_t st = G.stream;
+    const uint32_t nblocks = (uint32_t)((n + SORT_TILE - 1) / SORT_TILE);
+    Carver c;
+    const size_t o_k0 = c.take(n * 8), o_k1 = c.take(n * 8), o_v0 = c.take(n * 4), o_v1 = c.take(n * 4),
+                 o_h = c.take((size_t)256 * nblocks * 4), o_ops = c.take(n * sizeof(Op)), o_off = c.take(((size_t)N + 1) * 8);
+    void* blob = nullptr;
+    int rc = dev_alloc(c.cur, &blob);
+    if (rc) return rc;
+    unsigned char* b = (unsigned char*)blob;
+    uint64_t* keys[2] = {(uint64_t*)(b + o_k0), (uint64_t*)(b + o_k1)};
+    uint32_t* vals[2] = {(uint32_t*)(b + o_v0), (uint32_t*)(b + o_v1)};
+    uint32_t* ghist = (uint32_t*)(b + o_h);
+    const unsigned g256 = (unsigned)((n + 255) / 256);
+    // stable LSD order: first by (time, kind, link), then by node
+    k_ops_keys<<<g256, 256, 0, st>>>(s->d_recs, M, link_bits, keys[0], vals[0]);
+    int cur = radix_sort_pairs(keys, vals, n, t_bits + 1 + link_bits, ghist, nblocks, 0);
+    k_ops_nodes<<<g256, 256, 0, st>>>(s->d_recs, M, vals[cur], keys[cur]);
+    cur = radix_sort_pairs(keys, vals, n, node_bits, ghist, nblocks, cur);
+    k_ops_gather<<<g256, 256, 0, st>>>(s->d_recs, M, vals[cur], (Op*)(b + o_ops));
+    k_ops_offsets<<<(N + 1 + 255) / 256, 256, 0, st>>>(keys[cur], n, N, (uint64_t*)(b + o_off));
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ops, b + o_ops, n * sizeof(Op), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(offsets, b + o_off, ((size_t)N + 1) * 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    dev_free(blob);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return PCCL_ERR_CUDA; }
+    return PCCL_OK;
+}
+
 extern "C" int64_t pccl_schedule_trace(const pccl_schedule_t* s, uint64_t* out, uint64_t cap) {
     if (!s || (cap && !out)) return PCCL_ERR_INVALID;
     const uint64_t n = s->trace.size();

@@ -1227,4 +1227,64 @@ __global__ void __launch_bounds__(SORT_THREADS) k_sort_scatter(const uint64_t* _
     }
 }
 
+// ==================================================================================================
+//  Translation (section 4.8): the schedule as one program per node.  Every transfer gives
+//  two operations: its destination RECEIVES the chunk (completes at t_end) and its source SENDS it (starts
+//  at t_start).  A node's program lists its operations by (time, kind: receive before send, link).
+// ==================================================================================================
+struct Op {   // == pccl_op_t
+    uint32_t kind, peer, chunk, link;
+    uint64_t time;
+};
+static_assert(sizeof(Op) == 24, "layout");
+
+// operation i < M: the receive of record i; operation M + i: its send.  keyA orders within a node.
+__global__ void k_ops_keys(const Rec* __restrict__ recs, uint64_t M, uint32_t link_bits, uint64_t* __restrict__ keyA,
+                           uint32_t* __restrict__ idx) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * M) return;
+    const bool send = i >= M;
+    const Rec r = recs[send ? i - M : i];
+    const uint64_t time = send ? r.t_start : r.t_end;
+    keyA[i] = (time << (1 + link_bits)) | ((uint64_t)(send ? 1u : 0u) << link_bits) | r.link;
+    idx[i] = (uint32_t)i;
+}
+// second (stable) pass: the node of every operation, in the order of the first pass
+__global__ void k_ops_nodes(const Rec* __restrict__ recs, uint64_t M, const uint32_t* __restrict__ idx,
+                            uint64_t* __restrict__ keyB) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * M) return;
+    const uint32_t o = idx[i];
+    const bool send = o >= M;
+    const Rec r = recs[send ? o - M : o];
+    keyB[i] = send ? r.src : r.dst;
+}
+__global__ void k_ops_gather(const Rec* __restrict__ recs, uint64_t M, const uint32_t* __restrict__ idx,
+                             Op* __restrict__ ops) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * M) return;
+    const uint32_t o = idx[i];
+    const bool send = o >= M;
+    const Rec r = recs[send ? o - M : o];
+    Op op;
+    op.kind = send ? 1u : 0u;
+    op.peer = send ? r.dst : r.src;
+    op.chunk = r.chunk;
+    op.link = r.link;
+    op.time = send ? r.t_start : r.t_end;
+    ops[i] = op;
+}
+// offsets[v] = first operation of node v in the node-sorted key array (lower bound), offsets[n] = 2M
+__global__ void k_ops_offsets(const uint64_t* __restrict__ keyB, uint64_t n_ops, uint32_t n_nodes,
+                              uint64_t* __restrict__ offsets) {
+    const uint32_t v = blockIdx.x * blockDim.x + threadIdx.x;
+    if (v > n_nodes) return;
+    uint64_t lo = 0, hi = n_ops;
+    while (lo < hi) {
+        const uint64_t mid = (lo + hi) >> 1;
+        if (keyB[mid] < v) lo = mid + 1; else hi = mid;
+    }
+    offsets[v] = lo;
+}
+
 }  // namespace pccl
