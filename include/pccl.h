@@ -160,21 +160,24 @@ uint32_t pccl_problem_n_chunks(const pccl_problem_t* problem);
 int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, uint32_t chunk,
                                uint32_t* src, uint32_t* dests, uint64_t cap);
 
-/* flags for pccl_problem_synthesize */
-#define PCCL_FLAG_KEEP_ON_DEVICE 1u /* do not download the transfers until they are asked for */
-#define PCCL_FLAG_NO_IDLE_SKIP 2u   /* rescan idle links every event (debug / measurement) */
-#define PCCL_FLAG_TIME_LOOP 4u      /* record CUDA events around the event loop (stats) */
-#define PCCL_FLAG_DYNAMIC_RELAY 64u /* relay rule of DESIGN.md Q18 instead of the static thin relay tree: a node
-                                       takes a chunk iff it is strictly closer to some destination than the
-                                       source and every node that claimed the chunk at an earlier event
-                                       (fewer link-times, a few unused deliveries; recounts by dense sweep unless KEPT_COUNTS or RESCAN) */
-#define PCCL_FLAG_TWO_BARRIERS 256u /* run the two-barrier event loop even where the one-barrier loop applies */
-#define PCCL_FLAG_KEPT_COUNTS 128u  /* with DYNAMIC_RELAY: keep the counts current instead of its default dense recount */
-#define PCCL_FLAG_RESCAN 32u        /* recount every free link's candidates at every event from the bitmaps
-                                       (sector work list), instead of keeping the counts current */
-#define PCCL_FLAG_DENSE_SWEEP 16u   /* implies RESCAN, and recounts by sweeping whole rows, never the sector
-                                       work list (the plain bitmap scan: the memory-bound form) */
-#define PCCL_FLAG_TRACE 8u          /* record per-event phase timestamps (pccl_schedule_trace) */
+/* flags for pccl_problem_synthesize.  None of them changes the result except DYNAMIC_RELAY (a different relay
+ * rule); the others select how the same schedule is computed, for measurement and cross-checks. */
+#define PCCL_FLAG_KEEP_ON_DEVICE 1u  /* do not download the transfers until they are asked for */
+#define PCCL_FLAG_NO_IDLE_SKIP 2u    /* recount modes: rescan idle links every event */
+#define PCCL_FLAG_TIME_LOOP 4u       /* record CUDA events around setup / event loop / emitter (stats) */
+#define PCCL_FLAG_TRACE 8u           /* record per-event phase timestamps (pccl_schedule_trace) */
+#define PCCL_FLAG_DENSE_SWEEP 16u    /* recount every free link's candidates at every event by sweeping whole
+                                        bitmap rows: the plain memory-bound scan (two-barrier loop) */
+#define PCCL_FLAG_RESCAN 32u         /* recount at every event, but only the 32-byte sectors whose summary bits
+                                        are set in both rows (sector work list; two-barrier loop) */
+#define PCCL_FLAG_DYNAMIC_RELAY 64u  /* relay rule of DESIGN.md Q18 instead of the static thin relay tree: a node
+                                        takes a chunk iff it is strictly closer to some destination than the
+                                        source and every node that claimed the chunk at an earlier event (fewer
+                                        link-times, a few unused deliveries; dense recount unless KEPT_COUNTS
+                                        or RESCAN is given) */
+#define PCCL_FLAG_KEPT_COUNTS 128u   /* with DYNAMIC_RELAY: keep the candidate counts current (the default of
+                                        the thin-tree rule) instead of its dense recount */
+#define PCCL_FLAG_TWO_BARRIERS 256u  /* run the two-barrier event loop even where the one-barrier loop applies */
 
 /* Steps A..F on the GPU for one seed.  Errors: UNREACHABLE, CUDA, NOMEM, INTERNAL. */
 int pccl_problem_synthesize(pccl_problem_t* problem, uint64_t seed, uint32_t flags,
