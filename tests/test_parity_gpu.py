@@ -385,3 +385,72 @@ def test_one_barrier_and_two_barrier_loops_agree(pk, maker):
     o = oracle.synthesize(*p.args())
     assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE), o)
     assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_TWO_BARRIERS), o)
+
+
+# ------------------------------------------------------------------------------ randomized problems
+def _random_problem(i):
+    """seeded random directed multigraph with heterogeneous links, a random process group and a random
+    collective (copy with multi-dest chunks, reduce, or all-reduce); may be unreachable on purpose"""
+    rng = np.random.default_rng(1000 + i)
+    n = int(rng.integers(3, 40))
+    base = [(a, (a + 1) % n) for a in range(n)] if rng.random() < 0.8 else []          # a ring keeps most cases connected
+    extra = int(rng.integers(n, 6 * n))
+    src = rng.integers(0, n, extra)
+    dst = (src + 1 + rng.integers(0, n - 1, extra)) % n
+    pairs = base + list(zip(src.tolist(), dst.tolist()))
+    if rng.random() < 0.5:
+        pairs += [(b, a) for a, b in pairs]                                            # symmetric half of the time
+    links = np.zeros(len(pairs), dtype=wl.LINK_DT)
+    links["src"], links["dst"] = zip(*pairs)
+    if rng.random() < 0.5:
+        links["alpha_ps"], links["bytes_per_ps"] = 500, 10
+    else:
+        links["alpha_ps"] = rng.integers(0, 2000, len(pairs))
+        links["bytes_per_ps"] = rng.integers(1, 50, len(pairs))
+    g = int(rng.integers(2, n + 1))
+    members = np.sort(rng.choice(n, size=g, replace=False)).astype(np.uint32)
+    kind = int(rng.integers(0, 3))
+    nc = int(rng.integers(1, 200))
+    pre, post = [], []
+    for c in range(nc):
+        if kind == 0:      # copy: one holder, 1..g dests
+            s = int(rng.choice(members))
+            pre.append((s, c))
+            for d in rng.choice(members, size=int(rng.integers(1, g + 1)), replace=False):
+                post.append((int(d), c))
+        elif kind == 1:    # reduce: several holders, one root
+            hs = rng.choice(members, size=int(rng.integers(2, g + 1)), replace=False) if g >= 2 else members
+            pre += [(int(h), c) for h in hs]
+            post.append((int(rng.choice(members)), c))
+        else:              # all-reduce
+            hs = rng.choice(members, size=int(rng.integers(2, g + 1)), replace=False)
+            ds = rng.choice(members, size=int(rng.integers(2, g + 1)), replace=False)
+            pre += [(int(h), c) for h in hs]
+            post += [(int(d), c) for d in ds]
+    pre = np.array(pre, dtype=wl.PAIR_DT)
+    post = np.array(post, dtype=wl.PAIR_DT)
+    return wl.Problem(f"random{i}", n, links, members, nc, pre, post, int(rng.integers(1, 5000)), int(rng.integers(0, 2 ** 63)))
+
+
+@pytest.mark.parametrize("block", range(6))
+def test_randomized_problems_all_modes(pk, block):
+    """120 random problems: each must give the oracle's schedule (or the oracle's error) under both relay rules;
+    every sixth also under the recount modes and the two-barrier loop."""
+    for i in range(block * 20, block * 20 + 20):
+        p = _random_problem(i)
+        for relay, rflag in ((0, 0), (1, pk.PCCL_FLAG_DYNAMIC_RELAY)):
+            try:
+                o = oracle.synthesize(*p.args(), relay=relay)
+            except oracle.OracleError as e:
+                with pytest.raises(pk.PcclError) as g:
+                    gpu_run(pk, p, rflag | pk.PCCL_FLAG_KEEP_ON_DEVICE)
+                assert g.value.code == {oracle.ERR_UNREACHABLE: pk.PCCL_ERR_UNREACHABLE,
+                                        oracle.ERR_UNSUPPORTED: pk.PCCL_ERR_UNSUPPORTED,
+                                        oracle.ERR_INVALID: pk.PCCL_ERR_INVALID}[e.code], p.name
+                continue
+            assert_same(p, gpu_run(pk, p, rflag | pk.PCCL_FLAG_KEEP_ON_DEVICE), o)
+            if i % 6 == 0:
+                for fl in (pk.PCCL_FLAG_TWO_BARRIERS, pk.PCCL_FLAG_RESCAN, pk.PCCL_FLAG_DENSE_SWEEP):
+                    assert_same(p, gpu_run(pk, p, rflag | fl), o)
+            if relay == 0:
+                checker.check_schedule(p, o.transfers)
