@@ -66,7 +66,28 @@ class ClockSampler:
     def __init__(self, index: int):
         self.index, self.rows, self.stop, self.th = index, [], threading.Event(), None
 
+    def _run_nvml(self):
+        import pynvml
+        pynvml.nvmlInit()
+        h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+        mx = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
+        get_reasons = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
+            pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+        bits = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40}
+        while not self.stop.is_set():
+            sm = pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)
+            r = int(get_reasons(h))
+            row = [str(sm), str(mx), "0"] + [("Active" if r & bits[n] else "Not Active")
+                                            for n in ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")]
+            self.rows.append(row)
+            self.stop.wait(0.002)
+
     def _run(self):
+        try:
+            self._run_nvml()          # NVML: a sample every ~2 ms (the timed region is ~50 ms long)
+            return
+        except Exception:
+            pass
         while not self.stop.is_set():
             try:
                 out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
