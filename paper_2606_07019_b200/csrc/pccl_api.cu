@@ -736,24 +736,28 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     // so that twice as many destinations are resident at once
     const uint32_t max_deg = ph.transposed ? t->max_out : t->max_in;
     const bool small = max_deg <= 4;
-    const int threads = small ? 128 : 256;
-    const size_t smem = loop_smem_bytes(W.S, small ? 4 : 8);
+    int threads = small ? 128 : 256;
+    size_t smem = loop_smem_bytes(W.S, small ? 4 : 8);
     // the one-barrier loop (pccl_loop1.cuh): kept counts, <= 8 in-links per node, <= 128 segments per row,
     // at most DEST_CACHE destinations per CTA; everything else runs the two-barrier loop
     bool fast = !rescan && !dynamic && !(flags & PCCL_FLAG_TWO_BARRIERS) && max_deg <= 8 && W.S <= 128;
     const void* kern = nullptr;
     uint32_t grid = 0;
     for (int attempt = 0; attempt < 2; ++attempt) {
-        kern = fast ? (small ? (const void*)k_loop1<4> : (const void*)k_loop1<8>)
+        // one-barrier loop: teams of 4 warps are paired in 256-thread CTAs (half as many CTAs at the barrier)
+        kern = fast ? (small ? (const void*)k_loop1<4, 2> : (const void*)k_loop1<8, 1>)
                     : (small ? (const void*)k_loop<4> : (const void*)k_loop<8>);
+        const int teams = (fast && small) ? 2 : 1;
+        threads = (small ? 128 : 256) * teams;
+        smem = loop_smem_bytes(W.S, small ? 4 : 8) * teams;
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int occ = 0;
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
         if (occ < 1) return PCCL_ERR_CUDA;
         const uint32_t max_grid = (uint32_t)occ * (uint32_t)G.sm_count;
-        const uint32_t want = std::max(std::max(a.N, (a.L + threads - 1) / threads), 1u);
+        const uint32_t want = std::max(std::max((a.N + teams - 1) / teams, (a.L + threads - 1) / threads), 1u);
         grid = std::min(max_grid, want);
-        if (fast && (uint64_t)a.N > (uint64_t)DEST_CACHE * grid) { fast = false; continue; }
+        if (fast && (uint64_t)a.N > (uint64_t)DEST_CACHE * grid * teams) { fast = false; continue; }
         break;
     }
     a.st_free = fast ? W.st_free : nullptr;

@@ -87,11 +87,23 @@ __device__ __forceinline__ void emit_event(const LoopArgs& a, uint32_t ev, uint6
     }
 }
 
-template <int NBT>
+// barrier among the NBT warps of one team (named barrier team + 1; barrier 0 is __syncthreads)
+template <int NBT, int TEAMS>
+__device__ __forceinline__ void team_sync(uint32_t team) {
+    static_assert(TEAMS <= 4, "one literal barrier id per team");
+    if (TEAMS == 1) { __syncthreads(); return; }
+    if (team == 0) asm volatile("bar.sync 1, %0;" ::"r"(NBT * 32) : "memory");
+    else if (team == 1) asm volatile("bar.sync 2, %0;" ::"r"(NBT * 32) : "memory");
+    else if (team == 2) asm volatile("bar.sync 3, %0;" ::"r"(NBT * 32) : "memory");
+    else asm volatile("bar.sync 4, %0;" ::"r"(NBT * 32) : "memory");
+}
+
+template <int NBT, int TEAMS>
 __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32_t step, uint64_t t, uint32_t* cnt,
                                            FastScratch& sh, const FastCache& fc, LoopStats& st, bool do_emit,
                                            uint64_t emit_base) {
-    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t team = threadIdx.x / (NBT * 32);
+    const uint32_t tid = threadIdx.x % (NBT * 32), lane = tid & 31, warp = tid >> 5;
     const uint32_t Q = a.Wp >> 1, S = a.S, L = a.L;
     const uint32_t rd = (step & 1u) * L, wr = ((step & 1u) ^ 1u) * L;
     const uint32_t n_in = fc.n_in, nhop = fc.nhop;
@@ -146,7 +158,7 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
             if (lane + 32u * x < S) cnt[warp * S + lane + 32u * x] = rowv[x];
     }
     if (tid == 0) sh.wc = wc0;
-    __syncthreads();
+    team_sync<NBT, TEAMS>(team);
     trace_stamp(a, step, 1);
 
     // ---- per in-link: count upkeep for the pending chunks, then the pick (a5, a6) ---------------------
@@ -183,7 +195,7 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
         const uint32_t hm = __ballot_sync(0xFFFFFFFFu, hit != 0u);
         if (lane == 0) { sh.spec[j] = c; sh.sempty[j] = sem; sh.newc[j] = NONE32; sh.pbits[j] = hm; }
     }
-    __syncthreads();
+    team_sync<NBT, TEAMS>(team);
     trace_stamp(a, step, 2);
 
     // ---- conflict resolve, commit, count upkeep, next state (a7, a8): warp 0 ---------------------------
@@ -300,21 +312,26 @@ __device__ __forceinline__ void fast_match(const LoopArgs& a, uint32_t v, uint32
     } else if (do_emit) {
         // the other warps are idle now: they emit the previous event's records (a8), which only needs that
         // event's finished bitmap and state buffer
-        emit_event(a, step - 1, emit_base, warp - 1, NBT - 1);
+        emit_event(a, step - 1, emit_base, team * (NBT - 1) + warp - 1, TEAMS * (NBT - 1));
     }
-    __syncthreads();
+    team_sync<NBT, TEAMS>(team);
 }
 
-template <int NBT>
-__global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop1(const LoopArgs a) {
-    constexpr int THREADS = NBT * 32;
-    extern __shared__ __align__(16) uint32_t cnt[];   // [NBT][S]
-    __shared__ FastScratch sh;
-    __shared__ FastCache fc[DEST_CACHE];
+template <int NBT, int TEAMS>
+__global__ void __launch_bounds__(NBT * 32 * TEAMS, 1024 / (NBT * 32 * TEAMS)) k_loop1(const LoopArgs a) {
+    constexpr int THREADS = NBT * 32 * TEAMS;   // TEAMS teams of NBT warps, each serving its own destinations
+    extern __shared__ __align__(16) uint32_t cnt_all[];   // [TEAMS][NBT][S]
+    __shared__ FastScratch sh_all[TEAMS];
+    __shared__ FastCache fc_all[TEAMS][DEST_CACHE];
+    const uint32_t team = threadIdx.x / (NBT * 32), ttid = threadIdx.x % (NBT * 32);
+    const uint32_t nslots = gridDim.x * TEAMS, slot = team * gridDim.x + blockIdx.x;   // team-major: CTAs stay balanced
+    uint32_t* cnt = cnt_all + team * ((NBT * a.S + 3u) & ~3u);
+    FastScratch& sh = sh_all[team];
+    FastCache* fc = fc_all[team];
     __shared__ unsigned long long s_next[2];
     cg::grid_group grid = cg::this_grid();
-    if (threadIdx.x < DEST_CACHE) {   // one thread builds the tables of one destination (once)
-        const uint32_t k = threadIdx.x, v = blockIdx.x + k * gridDim.x;
+    if (ttid < DEST_CACHE) {   // one thread builds the tables of one destination (once)
+        const uint32_t k = ttid, v = slot + k * nslots;
         FastCache& c = fc[k];
         c.n_in = 0; c.nhop = 0; c.hop_off[0] = 0;
         if (v < a.N) {
@@ -338,10 +355,11 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop1(const Loo
         trace_stamp(a, step, 0);
         {
             uint32_t k = 0;
-            for (uint32_t v = blockIdx.x; v < a.N && k < DEST_CACHE; v += gridDim.x, ++k)
-                fast_match<NBT>(a, v, step, t, cnt, sh, fc[k], st, k == 0 && step > 0, tot_prev);
-            // (a CTA without a destination still takes its share of the emit)
-            if (k == 0 && step > 0 && (threadIdx.x >> 5) != 0) emit_event(a, step - 1, tot_prev, (threadIdx.x >> 5) - 1, NBT - 1);
+            for (uint32_t v = slot; v < a.N && k < DEST_CACHE; v += nslots, ++k)
+                fast_match<NBT, TEAMS>(a, v, step, t, cnt, sh, fc[k], st, k == 0 && step > 0, tot_prev);
+            // (a team without a destination still takes its share of the emit)
+            if (k == 0 && step > 0 && (ttid >> 5) != 0)
+                emit_event(a, step - 1, tot_prev, team * (NBT - 1) + (ttid >> 5) - 1, TEAMS * (NBT - 1));
         }
         trace_stamp(a, step, 3);
         {   // clear the bitmap the next event writes; re-arm the ring slot after next
