@@ -123,6 +123,44 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def lower_bound_ps(p):
+    """Bandwidth lower bound of the collective time for COPY problems on homogeneous links (DESIGN.md
+    "Lower bound"; harness arithmetic, not part of the method): max of the ingress bound
+    max_v ceil(chunks v must receive / indeg v), the egress bound likewise, and the work bound
+    ceil(sum over (chunk, dest) of hop distance / L) for single-dest chunks, times the link cost."""
+    import numpy as np
+    from scipy.sparse import csr_matrix
+    from scipy.sparse.csgraph import shortest_path
+    links = p.links
+    if len(np.unique(links["alpha_ps"])) != 1 or len(np.unique(links["bytes_per_ps"])) != 1:
+        return None
+    w = int(links["alpha_ps"][0]) + -(-int(p.chunk_bytes) // int(links["bytes_per_ps"][0]))
+    n = p.n_npus
+    src_of = np.full(p.n_chunks, -1, dtype=np.int64)
+    cnt = np.bincount(p.pre["chunk"], minlength=p.n_chunks)
+    if cnt.max() != 1:
+        return None                                    # reductions: not bounded here
+    src_of[p.pre["chunk"]] = p.pre["npu"]
+    need = p.post[src_of[p.post["chunk"]] != p.post["npu"]]          # (dest, chunk) that must be delivered
+    indeg = np.bincount(links["dst"], minlength=n)
+    outdeg = np.bincount(links["src"], minlength=n)
+    need_in = np.bincount(need["npu"], minlength=n)
+    has_dest = np.zeros(p.n_chunks, dtype=bool)
+    has_dest[need["chunk"]] = True
+    need_out = np.bincount(src_of[has_dest], minlength=n)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        ingress = int(np.nanmax(np.where(need_in > 0, np.ceil(need_in / np.maximum(indeg, 1)), 0)))
+        egress = int(np.nanmax(np.where(need_out > 0, np.ceil(need_out / np.maximum(outdeg, 1)), 0)))
+    bound = max(ingress, egress)
+    per_chunk = np.bincount(need["chunk"], minlength=p.n_chunks)
+    if per_chunk.max() == 1:                            # single-dest chunks: every hop of a shortest path is a transfer
+        g = csr_matrix((np.ones(len(links)), (links["src"], links["dst"])), shape=(n, n))
+        hops = shortest_path(g, method="D", unweighted=True)
+        total = int(hops[src_of[need["chunk"]], need["npu"]].sum())
+        bound = max(bound, -(-total // len(links)))
+    return bound * w
+
+
 def time_oracle(p, budget_s: float, max_runs: int):
     """Oracle wall times (its own steady-clock seconds) for up to max_runs runs within budget_s."""
     import oracle
@@ -363,6 +401,7 @@ def run_ours(args):
                 "algorithmic_gbs": algb / (stc["loop_ms"] * 1e-3) / 1e9 if stc["loop_ms"] else None,
                 "frac_of_measured_hbm": (algb / (stc["loop_ms"] * 1e-3) / 1e9 / peak) if stc["loop_ms"] else None,
                 "requested_bytes": stc["bytes_requested"],
+                "schedule_time_over_lower_bound": (tcps / lower_bound_ps(pc)) if lower_bound_ps(pc) else None,
                 "roofline_note": "rows of 128 B: launch/sync-bound, roofline n/a" if stc["row_bytes"] <= 256 else "bitmap scan"}
             if stc["row_bytes"] > 256:   # a real bitmap scan: the two recount modes beside the default
                 for key, fl in (("rescan_sector_list", pk.PCCL_FLAG_RESCAN), ("dense_sweep", pk.PCCL_FLAG_DENSE_SWEEP)):
@@ -387,14 +426,7 @@ def run_ours(args):
                "sample": f"the whole config{args.config} problem once ({secs[0]:.2f} s, single thread)",
                "host_cores": os.cpu_count(), "seconds": secs[0]}
 
-    lb = None
-    try:
-        import workloads as wl  # noqa: F401
-        if args.config == 4:
-            w = 500_000 + -(-p.chunk_bytes // 50)
-            lb = 512 * w           # work bound: sum of hop distances / links
-    except Exception:
-        pass
+    lb = lower_bound_ps(p)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": tot_ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
