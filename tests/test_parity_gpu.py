@@ -374,6 +374,21 @@ def test_more_nodes_than_resident_ctas(pk, relay):
     checker.check_structure(p, s.transfers)
 
 
+@pytest.mark.parametrize("relay", [0, 1])
+def test_ten_thousand_nodes(pk, relay):
+    """10,000-node ring, 4 members: the distance kernel's per-source table is 80 KB of shared memory (the
+    opt-in size), there are more destinations than the one-barrier loop caches (it falls back to the
+    two-barrier loop), 5,000 events."""
+    n = 10000
+    mem = np.array([0, 2500, 5000, 7500], dtype=np.uint32)
+    nc, pre, post = wl.all_to_all(mem, np.full((4, 4), 2))
+    p = wl.Problem("ring10000_a2a4", n, wl.ring_links(n, True), mem, nc, pre, post, 1 << 12, 5)
+    o = oracle.synthesize(*p.args(), relay=relay)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY if relay else 0)
+    assert_same(p, s, o)
+    checker.check_structure(p, s.transfers)
+
+
 # ------------------------------------------------------------------------------ the two event loops
 @pytest.mark.parametrize("maker", SMALL + [lambda s: wl.ring_all_gather(8, True, s, chunks_per_npu=1040, chunk_bytes=4096),
                                            lambda s: _torus_all_gather((12, 12), 2, s)],
