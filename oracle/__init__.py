@@ -118,12 +118,13 @@ class OracleSchedule:
         self.seconds = seconds                # wall time of the C++ call (steady clock)
 
 
-RELAY_THIN, RELAY_DYNAMIC = 0, 1
+RELAY_THIN, RELAY_DYNAMIC, RELAY_BFS = 0, 1, 2
 
 
 def synthesize(n_npus, links, group, n_chunks, pre, post, chunk_bytes, seed, relay: int = RELAY_THIN) -> OracleSchedule:
     """Same problem statement as the product boundary (include/pccl.h), host arrays only.
-    relay: RELAY_THIN (static thin relay tree, the default) or RELAY_DYNAMIC (Q18)."""
+    relay: RELAY_THIN (static thin relay tree, the default), RELAY_DYNAMIC (Q18) or RELAY_BFS (the paper's
+    own per-condition search, Alg. 1-3, Q19-Q22; `events` then counts conditions routed)."""
     links = np.ascontiguousarray(links, dtype=LINK_DT)
     group = np.ascontiguousarray(group, dtype=np.uint32)
     pre = np.ascontiguousarray(pre, dtype=PAIR_DT)

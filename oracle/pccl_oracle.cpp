@@ -33,6 +33,7 @@
 #include <cstring>
 #include <functional>
 #include <limits>
+#include <map>
 #include <queue>
 #include <set>
 #include <utility>
@@ -385,9 +386,143 @@ int synth_copy_dynamic(uint32_t n, const std::vector<Link>& links, const std::ve
     return OR_OK;
 }
 
-// relay rule used by the dispatchers below: 0 = thin relay tree (step C), 1 = dynamic
+// -------------------------------------------------------------------------------------
+// synth_copy_bfs: the PAPER'S OWN synthesizer, Algorithms 1-3 with the heterogeneous rules of
+// section 4.6, condition by condition (readings Q19-Q22).
+//
+//   Alg. 3 lines 1-7  c.dist = max over dests of ShortestPath(c.src, dest) on the idle network
+//                     (alpha-beta cost, reading Q3); conditions in DESCENDING c.dist.  Ties
+//                     (paper silent, Q19): ascending Philox(seed; chunk, tag 2) draw, then chunk id.
+//   Alg. 3 line 10    BFS(TEN, c): earliest-arrival search from c.src over the WHOLE network
+//                     (PAPER.md:300).  Section 4.6 "Chunk Arrival Time": visited carries the time
+//                     the chunk reaches each device, a device forwards only after that time.
+//                     A link l = (u -> v) of cost w(l) may start at the earliest s >= arrival(u)
+//                     such that [s, s + w(l)) overlaps no interval already taken on l
+//                     (NextAvailableTime of Alg. 1 applied per link + Fig. 10);
+//                     the chunk then reaches v at s + w(l).  arrival(v) is the minimum over v's
+//                     in-links; devices are visited in order of arrival (the BFS of Alg. 2 visits
+//                     them timestep by timestep).  Which of several links reaching v at the same
+//                     earliest time is kept is not fixed by Alg. 2 (iteration order of a set):
+//                     reading Q20 keeps the LOWEST LINK ID.
+//   PAPER.md:298      filter: keep only the transfers on the recorded paths src -> dest.
+//   Alg. 3 line 13    "Remove p from TEN": every kept transfer's interval [s, s + w) becomes busy
+//                     on its link for all later conditions.
+// A later condition may use a gap in front of an earlier one's interval if its transfer fits.
+// -------------------------------------------------------------------------------------
+struct BusyLink {                                         // disjoint intervals, ascending
+    std::vector<std::pair<uint64_t, uint64_t>> iv;        // [start, end)
+};
+
+// earliest s >= a with [s, s + w) free on the link
+uint64_t earliest_start(const BusyLink& b, uint64_t a, uint64_t w) {
+    uint64_t s = a;
+    // intervals are disjoint and ascending, so their ends ascend too: skip those ending at or before s
+    auto it = std::upper_bound(b.iv.begin(), b.iv.end(), s,
+                               [](uint64_t x, const std::pair<uint64_t, uint64_t>& p) { return x < p.second; });
+    for (; it != b.iv.end(); ++it) {
+        if (s + w <= it->first) break;   // fits in front of this interval (and of all later ones)
+        s = it->second;                  // overlaps it: next try right behind it
+    }
+    return s;
+}
+
+void occupy(BusyLink& b, uint64_t s, uint64_t e) {
+    auto it = std::lower_bound(b.iv.begin(), b.iv.end(), std::make_pair(s, e));
+    b.iv.insert(it, std::make_pair(s, e));
+}
+
+int synth_copy_bfs(uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& conds,
+                   uint64_t chunk_bytes, uint64_t seed, CopyResult& res) {
+    const uint32_t L = (uint32_t)links.size();
+    const uint32_t C = (uint32_t)conds.size();
+    std::vector<uint64_t> w(L);
+    for (uint32_t l = 0; l < L; ++l) w[l] = link_cost(links[l], chunk_bytes);
+    std::vector<std::vector<uint32_t>> out(n);
+    for (uint32_t l = 0; l < L; ++l) out[links[l].src].push_back(l);
+
+    // Alg. 3 lines 1-7
+    struct Key { uint64_t dist; uint32_t draw, chunk; };
+    std::vector<Key> order;
+    std::map<uint32_t, std::vector<uint64_t>> dist_from;
+    for (uint32_t c = 0; c < C; ++c) {
+        if (!conds[c].present || conds[c].dests.empty()) continue;
+        auto f = dist_from.find(conds[c].src);
+        if (f == dist_from.end()) f = dist_from.emplace(conds[c].src, dijkstra(n, links, w, conds[c].src)).first;
+        uint64_t dmax = 0;
+        for (uint32_t d : conds[c].dests) {
+            if (f->second[d] == INF) return OR_ERR_UNREACHABLE;
+            dmax = std::max(dmax, f->second[d]);
+        }
+        order.push_back(Key{dmax, draw(seed, c, 0, 0, 2), c});
+    }
+    std::sort(order.begin(), order.end(), [](const Key& a, const Key& b) {
+        if (a.dist != b.dist) return a.dist > b.dist;
+        if (a.draw != b.draw) return a.draw < b.draw;
+        return a.chunk < b.chunk;
+    });
+
+    std::vector<BusyLink> busy(L);
+    res = CopyResult{};
+    std::vector<uint64_t> arr(n);
+    std::vector<uint32_t> pred(n);
+    std::vector<char> done(n), keep(n);
+    for (const Key& k : order) {                              // Alg. 3 line 9
+        const Cond& c = conds[k.chunk];
+        // Alg. 2 + section 4.6: visit devices in order of arrival
+        std::fill(arr.begin(), arr.end(), INF);
+        std::fill(pred.begin(), pred.end(), NONE);
+        std::fill(done.begin(), done.end(), 0);
+        using QE = std::pair<uint64_t, uint32_t>;
+        std::priority_queue<QE, std::vector<QE>, std::greater<QE>> pq;
+        arr[c.src] = 0;
+        pq.push({0, c.src});
+        size_t left = c.dests.size();
+        uint64_t last = 0;                                    // arrival at the last dest reached
+        while (!pq.empty()) {
+            auto [a, u] = pq.top();
+            pq.pop();
+            if (done[u] || a != arr[u]) continue;
+            if (left == 0 && a > last) break;                 // Alg. 2 line 4: all dests visited
+            done[u] = 1;
+            if (left && std::binary_search(c.dests.begin(), c.dests.end(), u)) { --left; last = a; }
+            for (uint32_t l : out[u]) {                       // NextDevices(TEN, u, .)
+                const uint32_t v = links[l].dst;
+                if (done[v]) continue;                        // Alg. 2 line 7
+                const uint64_t t = earliest_start(busy[l], a, w[l]) + w[l];
+                if (t < arr[v] || (t == arr[v] && l < pred[v])) {   // Q20
+                    arr[v] = t;
+                    pred[v] = l;
+                    pq.push({t, v});
+                }
+            }
+        }
+        if (left) return OR_ERR_UNREACHABLE;
+        // keep the paths to the dests only
+        std::fill(keep.begin(), keep.end(), 0);
+        for (uint32_t d : c.dests)
+            for (uint32_t v = d; v != c.src && !keep[v]; v = links[pred[v]].src) keep[v] = 1;
+        for (uint32_t v = 0; v < n; ++v) {
+            if (!keep[v]) continue;
+            const uint32_t l = pred[v];
+            res.recs.push_back(Rec{k.chunk, links[l].src, v, l, arr[v] - w[l], arr[v]});
+            occupy(busy[l], arr[v] - w[l], arr[v]);           // Alg. 3 line 13
+            res.T = std::max(res.T, arr[v]);
+        }
+        ++res.events;                                         // here: conditions routed
+    }
+    std::sort(res.recs.begin(), res.recs.end(), [](const Rec& a, const Rec& b) {
+        if (a.t_start_ps != b.t_start_ps) return a.t_start_ps < b.t_start_ps;
+        return a.link < b.link;
+    });
+    res.wants_total = res.recs.size();
+    return OR_OK;
+}
+
+// relay rule used by the dispatchers below: 0 = thin relay tree (step C), 1 = dynamic,
+// 2 = the paper's per-condition BFS (no matching loop at all)
 int synth_copy_mode(int relay, uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& conds,
                     uint64_t chunk_bytes, uint64_t seed, CopyResult& res) {
+    if (relay == 2) return synth_copy_bfs(n, links, conds, chunk_bytes, seed, res);
     return relay == 1 ? synth_copy_dynamic(n, links, conds, chunk_bytes, seed, res)
                       : synth_copy(n, links, conds, chunk_bytes, seed, res);
 }
@@ -581,7 +716,7 @@ int oracle_synthesize_relay(uint32_t n_npus, const oracle_link* links, uint32_t 
                             const uint32_t* group, uint32_t n_members, uint32_t n_chunks,
                             const oracle_pair* pre, uint64_t n_pre, const oracle_pair* post,
                             uint64_t n_post, uint64_t chunk_bytes, uint64_t seed, int relay, void** handle) {
-    if (!handle || relay < 0 || relay > 1) return OR_ERR_INVALID;
+    if (!handle || relay < 0 || relay > 2) return OR_ERR_INVALID;
     Result* r = new Result();
     const int rc = synthesize(n_npus, (const Link*)links, n_links, group, n_members, n_chunks,
                               (const Pair*)pre, n_pre, (const Pair*)post, n_post, chunk_bytes,

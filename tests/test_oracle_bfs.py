@@ -1,0 +1,259 @@
+"""Pins of the oracle's BFS mode -- the paper's own synthesizer, Algorithms 1-3 with the
+heterogeneous rules of section 4.6 (Q19-Q22).  No GPU.
+
+The oracle keeps per-link busy INTERVALS and finds departures by first fit; the pin below is
+the paper's literal data structure instead: a boolean TEN[t][link] over integer timesteps,
+searched timestep by timestep (Alg. 2), with every overlapping entry removed after a path is
+taken (Fig. 10).  The two share nothing but the problem statement.  A dropped tie rule, an
+off-by-one in the overlap test, a missed gap in front of a taken interval, a wrong sort
+direction in Alg. 3 or a missing path filter all make the record lists differ.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+from oracle import checker
+
+BFS = oracle.RELAY_BFS
+
+
+def run(p):
+    return oracle.synthesize(*p.args(), relay=BFS)
+
+
+def _links(triples):
+    """(src, dst, cost) with integer cost >= 1: alpha = cost - 1, one byte per ps, 1-byte chunks."""
+    a = np.zeros(len(triples), dtype=wl.LINK_DT)
+    for i, (s, d, c) in enumerate(triples):
+        a[i] = (s, d, c - 1, 1)
+    return a
+
+
+def _pairs(items):
+    a = np.zeros(len(items), dtype=wl.PAIR_DT)
+    for i, (v, c) in enumerate(items):
+        a[i] = (v, c)
+    return a
+
+
+def _problem(name, n, triples, conds, seed=0, group=None):
+    """conds: list of (src, [dests]); chunk id = index"""
+    pre = _pairs([(s, c) for c, (s, _) in enumerate(conds)])
+    post = _pairs([(d, c) for c, (_, ds) in enumerate(conds) for d in ds])
+    if group is None:
+        group = sorted({s for s, _ in conds} | {d for _, ds in conds for d in ds})
+    return wl.Problem(name, n, _links(triples), np.array(group, dtype=np.uint32), len(conds), pre, post, 1, seed)
+
+
+# ------------------------------------------------------------------ the literal TEN (brute force)
+def _hop_costs(n, links, w, src):
+    """Bellman-Ford on the idle network (ShortestPath of Alg. 3)"""
+    D = [None] * n
+    D[src] = 0
+    for _ in range(n):
+        for l, k in enumerate(links):
+            u, v = int(k["src"]), int(k["dst"])
+            if D[u] is not None and (D[v] is None or D[u] + w[l] < D[v]):
+                D[v] = D[u] + w[l]
+    return D
+
+
+def literal_ten(n, links, conds, seed):
+    """Alg. 3 over Alg. 2 on a boolean TEN[t][link] (stored as the set of removed entries)."""
+    w = [int(k["alpha_ps"]) + 1 for k in links]
+    removed = set()                                   # (t, link): TEN entry taken
+    keyed = []
+    for c, (src, dests) in enumerate(conds):
+        if not dests:
+            continue
+        D = _hop_costs(n, links, w, src)
+        keyed.append((-max(D[d] for d in dests), int(wl.philox_first_word(c, 0, 0, 2, seed)), c))
+    out = []
+    for _, _, c in sorted(keyed):                     # Alg. 3 line 7 (+ reading Q19 for ties)
+        src, dests = conds[c]
+        arr, pred = {src: 0}, {}
+        t = 0
+        while not all(d in arr and arr[d] <= t for d in dests):   # Alg. 2 line 4
+            for l, k in enumerate(links):             # every TEN link that starts at timestep t
+                u, v = int(k["src"]), int(k["dst"])
+                if u not in arr or arr[u] > t:        # 4.6: the chunk must have arrived at `current`
+                    continue
+                if any((t + i, l) in removed for i in range(w[l])):
+                    continue                          # overlaps a taken entry (Fig. 10)
+                a = t + w[l]
+                if v == src:
+                    continue
+                if v not in arr or a < arr[v] or (a == arr[v] and l < pred[v][0]):
+                    arr[v], pred[v] = a, (l, t)
+            t += 1
+            assert t < 10_000
+        keep = set()
+        for d in dests:                               # keep the useful paths
+            v = d
+            while v != src and v not in keep:
+                keep.add(v)
+                v = int(links[pred[v][0]]["src"])
+        for v in sorted(keep):
+            l, ts = pred[v]
+            out.append((ts, l, c, int(links[l]["src"]), v, ts + w[l]))
+            for i in range(w[l]):                     # Alg. 3 line 13
+                assert (ts + i, l) not in removed
+                removed.add((ts + i, l))
+    out.sort()
+    return out
+
+
+def _as_tuples(tr):
+    return [(int(r["t_start_ps"]), int(r["link"]), int(r["chunk"]), int(r["src"]), int(r["dst"]), int(r["t_end_ps"]))
+            for r in tr]
+
+
+def _random_case(i):
+    rng = np.random.default_rng(7000 + i)
+    n = int(rng.integers(4, 10))
+    triples = []
+    perm = rng.permutation(n)
+    for a in range(n):                                # a ring through all nodes keeps it strongly connected
+        triples.append((int(perm[a]), int(perm[(a + 1) % n]), int(rng.integers(1, 5))))
+    for _ in range(int(rng.integers(n, 3 * n))):
+        u, v = rng.choice(n, 2, replace=False)
+        triples.append((int(u), int(v), int(rng.integers(1, 5))))   # parallel links allowed
+    members = sorted(rng.choice(n, int(rng.integers(2, n + 1)), replace=False).tolist())
+    conds = []
+    kind = i % 3
+    for s in members:
+        others = [m for m in members if m != s]
+        if kind == 0:                                 # All-Gather like, several chunks per member
+            conds += [(s, others)] * int(rng.integers(1, 4))
+        elif kind == 1:                               # All-to-All like
+            conds += [(s, [d]) for d in others for _ in range(int(rng.integers(0, 3)))]
+        else:                                         # random dest subsets
+            for _ in range(int(rng.integers(1, 4))):
+                k = int(rng.integers(1, len(others) + 1))
+                conds.append((s, sorted(rng.choice(others, k, replace=False).tolist())))
+    if not conds:
+        conds = [(members[0], [members[1]])]
+    return n, triples, conds, members
+
+
+@pytest.mark.parametrize("i", range(30))
+def test_equals_the_literal_boolean_ten(i):
+    n, triples, conds, members = _random_case(i)
+    p = _problem(f"rand{i}", n, triples, conds, seed=i, group=members)
+    s = run(p)
+    assert _as_tuples(s.transfers) == literal_ten(n, p.links, conds, i)
+    checker.check_schedule(p, s.transfers)
+
+
+def test_reduction_is_the_reversed_search_on_the_transposed_links():
+    """Reduce-Scatter = reversed All-Gather.  Literal TEN on the transposed links, every
+    transfer reversed in direction and in time."""
+    n, triples, _, _ = _random_case(3)
+    members = list(range(n))
+    # chunk c is reduced from all members into root c % n
+    conds_b = [(c % n, [m for m in members if m != c % n]) for c in range(n + 2)]
+    pre = _pairs([(m, c) for c in range(len(conds_b)) for m in members])
+    post = _pairs([(c % n, c) for c in range(len(conds_b))])
+    p = wl.Problem("rs", n, _links(triples), np.array(members, dtype=np.uint32), len(conds_b), pre, post, 1, 5)
+    s = run(p)
+    tl = p.links.copy()
+    tl["src"], tl["dst"] = p.links["dst"], p.links["src"]
+    b = literal_ten(n, tl, conds_b, 5)
+    T = max(r[5] for r in b)
+    want = sorted((T - te, l, c, v, u, T - ts) for ts, l, c, u, v, te in b)
+    assert _as_tuples(s.transfers) == want
+    assert s.time_ps == T
+
+
+# ------------------------------------------------------------------ worked examples and closed forms
+def test_worked_example_gap_in_front_of_a_taken_interval():
+    """links: l0 = 0->1 cost 10, l1 = 1->2 cost 4, l2 = 3->1 cost 1.  Conditions (chunk: src -> dest):
+    c0: 0->2 (dist 14), c1..c3: 3->2 (dist 5).  Alg. 3 routes c0 first: l0 [0,10), l1 [10,14).
+    The three short ones follow in the order of their tie draws, whichever it is; the k-th of them leaves
+    node 3 at k-1 (l2 is busy one step per chunk) and needs 4 free steps on l1:
+      1st: l2 [0,1), l1 [1,5)      2nd: l2 [1,2), l1 [5,9)   (fits in front of [10,14))
+      3rd: l2 [2,3), l1 [14,18)    ([9,13) would overlap [10,14))."""
+    p = _problem("gap", 4, [(0, 1, 10), (1, 2, 4), (3, 1, 1)], [(0, [2]), (3, [2]), (3, [2]), (3, [2])], seed=11)
+    s = run(p)
+    got = sorted((int(r["link"]), int(r["t_start_ps"]), int(r["t_end_ps"])) for r in s.transfers)
+    assert got == [(0, 0, 10), (1, 1, 5), (1, 5, 9), (1, 10, 14), (1, 14, 18), (2, 0, 1), (2, 1, 2), (2, 2, 3)]
+    on_l1 = {int(r["t_start_ps"]): int(r["chunk"]) for r in s.transfers if r["link"] == 1}
+    assert on_l1[10] == 0
+    assert s.time_ps == 18
+
+
+@pytest.mark.parametrize("k,m,cost", [(1, 5, 3), (4, 1, 7), (5, 6, 2)])
+def test_pipeline_on_a_line(k, m, cost):
+    """m chunks over a line of k equal links: the j-th routed leaves at j*cost on every hop's first free
+    slot, so T = (k + m - 1) * cost and every link carries back-to-back transfers."""
+    triples = [(i, i + 1, cost) for i in range(k)]
+    p = _problem("line", k + 1, triples, [(0, [k])] * m)
+    s = run(p)
+    assert s.time_ps == (k + m - 1) * cost
+    assert len(s.transfers) == k * m
+    for l in range(k):
+        starts = sorted(int(r["t_start_ps"]) for r in s.transfers if r["link"] == l)
+        assert starts == [(l + j) * cost for j in range(m)]
+
+
+def test_longest_condition_goes_first_and_gets_its_shortest_path():
+    """Alg. 3 line 7: the condition with the largest c.dist is routed on the idle network, so it arrives
+    after exactly c.dist even though a shorter condition competes for its first link."""
+    #  0 -> 1 -> 2 -> 3   and a short condition 0 -> 1
+    p = _problem("order", 4, [(0, 1, 2), (1, 2, 2), (2, 3, 2)], [(0, [1]), (0, [3])])
+    s = run(p)
+    long_ = s.transfers[s.transfers["chunk"] == 1]
+    assert sorted(int(t) for t in long_["t_end_ps"]) == [2, 4, 6]
+    short = s.transfers[s.transfers["chunk"] == 0]
+    assert (int(short["t_start_ps"][0]), int(short["t_end_ps"][0])) == (2, 4)
+
+
+def test_lowest_link_id_wins_equal_arrivals():
+    """reading Q20: two parallel links and a two-hop detour all reach node 1 at time 4"""
+    p = _problem("tie", 3, [(0, 2, 2), (0, 1, 4), (2, 1, 2), (0, 1, 4)], [(0, [1])])
+    s = run(p)
+    assert [(int(r["link"]), int(r["t_start_ps"])) for r in s.transfers] == [(1, 0)]
+
+
+def test_broadcast_keeps_only_useful_paths():
+    """a star with 5 leaves, dests = 2 of them: exactly 2 transfers"""
+    p = _problem("filter", 6, [(0, i, 1) for i in range(1, 6)], [(0, [2, 4])])
+    s = run(p)
+    assert sorted(int(d) for d in s.transfers["dst"]) == [2, 4]
+
+
+def test_non_members_relay(tmp_path):
+    """links outside the process group are used"""
+    p = wl.two_groups_mesh3x3(0)
+    s = run(p)
+    checker.check_schedule(p, s.transfers)
+    touched = set(s.transfers["src"].tolist()) | set(s.transfers["dst"].tolist())
+    assert touched - set(p.group.tolist())
+
+
+def test_unreachable():
+    p = _problem("unreach", 3, [(0, 1, 1)], [(0, [2])])
+    with pytest.raises(oracle.OracleError) as e:
+        run(p)
+    assert e.value.code == oracle.ERR_UNREACHABLE
+
+
+# ------------------------------------------------------------------ the paper's workload shapes
+@pytest.mark.parametrize("maker", [wl.config1, wl.config2, wl.config3, wl.config4_small, wl.config5_small])
+def test_valid_on_the_configs(maker):
+    p = maker(0)
+    s = run(p)
+    checker.check_schedule(p, s.transfers)
+    assert s.events > 0
+
+
+def test_first_routed_condition_takes_c_dist():
+    """on config 1 (16 equal conditions on an idle 4x4 torus) T can not be below the eccentricity, and the
+    first routed chunk reaches its farthest dest after exactly 4 hops"""
+    p = wl.config1(0)
+    s = run(p)
+    w = int(checker.link_costs(p.links, p.chunk_bytes)[0])
+    assert s.time_ps >= 4 * w
+    first = int(np.lexsort((np.arange(16), wl.philox_first_word(np.arange(16), 0, 0, 2, p.seed)))[0])
+    assert int(s.transfers[s.transfers["chunk"] == first]["t_end_ps"].max()) == 4 * w
