@@ -178,6 +178,17 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
 #define PCCL_FLAG_KEPT_COUNTS 128u   /* with DYNAMIC_RELAY: keep the candidate counts current (the default of
                                         the thin-tree rule) instead of its dense recount */
 #define PCCL_FLAG_TWO_BARRIERS 256u  /* run the two-barrier event loop even where the one-barrier loop applies */
+#define PCCL_FLAG_BFS 512u           /* the paper's own synthesizer instead of the matching loop (Alg. 1-3,
+                                        :332-344 section 4.6; Q19-Q22): conditions in descending c.dist
+                                        (ties: Philox(seed; chunk, tag 2), then chunk id), each routed by an
+                                        earliest-arrival search over the whole network against the busy intervals of
+                                        the conditions before it (lowest link id on equal arrivals), only the paths to
+                                        its dests kept, their intervals then busy.  The other mode flags are ignored.
+                                        Statistics: events = conditions routed, wants_total = transfers,
+                                        rows_scanned = searches run (a condition is searched again when a condition
+                                        ahead of it took an interval it used), links_scanned = link relaxations,
+                                        slow_picks = commit rounds.  UNSUPPORTED if a time does not fit in
+                                        64 - ceil(log2(n_links)) bits or n_npus > 12,800. */
 
 /* Steps A..F on the GPU for one seed.  Errors: UNREACHABLE, CUDA, NOMEM, INTERNAL. */
 int pccl_problem_synthesize(pccl_problem_t* problem, uint64_t seed, uint32_t flags,

@@ -34,6 +34,7 @@ PCCL_FLAG_RESCAN = 32
 PCCL_FLAG_DYNAMIC_RELAY = 64
 PCCL_FLAG_KEPT_COUNTS = 128
 PCCL_FLAG_TWO_BARRIERS = 256
+PCCL_FLAG_BFS = 512
 PCCL_TRACE_SLOTS = 12
 
 

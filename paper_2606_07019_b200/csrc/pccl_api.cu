@@ -17,6 +17,7 @@
 
 #include "pccl_device.cuh"
 #include "pccl_loop1.cuh"
+#include "pccl_bfs.cuh"
 
 using namespace pccl;
 
@@ -798,7 +799,8 @@ int radix_sort_pairs(uint64_t* keys[2], uint32_t* vals[2], uint64_t n, uint32_t 
 }
 
 // a9 for reductions: raw (transposed-broadcast) records -> reversed, sorted by (t_start, link), into out
-int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out) {
+// (reverse = false: only sorted, times shifted by `shift`; T then only bounds the key width)
+int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out, bool reverse = true, uint64_t shift = 0) {
     if (M == 0) return PCCL_OK;
     cudaStream_t st = G.stream;
     uint32_t link_bits = 1;
@@ -818,9 +820,9 @@ int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out) {
     uint32_t* vals[2] = {(uint32_t*)(b + o_v0), (uint32_t*)(b + o_v1)};
     uint32_t* ghist = (uint32_t*)(b + o_h);
     const unsigned g256 = (unsigned)((M + 255) / 256);
-    k_reverse_keys<<<g256, 256, 0, st>>>(raw, M, T, link_bits, keys[0], vals[0]);
+    k_reverse_keys<<<g256, 256, 0, st>>>(raw, M, T, link_bits, keys[0], vals[0], reverse);
     const int cur = radix_sort_pairs(keys, vals, M, t_bits + link_bits, ghist, nblocks, 0);
-    k_gather_shift<<<g256, 256, 0, st>>>(raw, vals[cur], M, 0, out);
+    k_gather_shift<<<g256, 256, 0, st>>>(raw, vals[cur], M, shift, out);
     cudaError_t e = cudaGetLastError();
     dev_free(blob);   // stream-ordered: freed after the kernels above
     return e == cudaSuccess ? PCCL_OK : PCCL_ERR_CUDA;
@@ -843,6 +845,149 @@ struct Timer {
     }
     ~Timer() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
 };
+
+// ---------------------------------------------------------------------------------------
+// PCCL_FLAG_BFS: one phase of the paper's own synthesizer (pccl_bfs.cuh).  On return *out_recs
+// holds the M records in canonical order (reversed in direction and time for a transposed
+// phase, shifted by t_shift otherwise); the caller owns it.
+// ---------------------------------------------------------------------------------------
+struct BfsResult {
+    uint64_t M, tmax, conditions, searches, relax, rounds;
+    uint32_t grid;
+};
+
+int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_shift, Rec** out_recs, BfsResult* res,
+              Timer& t_setup, Timer& t_loop, Timer& t_emit) {
+    const pccl_topology* t = P.topo;
+    const uint32_t N = t->N, L = t->L, C = P.C;
+    const PhaseView pv = view_of(t, ph.transposed);
+    cudaStream_t st = G.stream;
+    *out_recs = nullptr;
+    memset(res, 0, sizeof(*res));
+    if (C == 0 || ph.dests.empty()) return PCCL_OK;
+    if (L == 0) return PCCL_ERR_UNREACHABLE;
+    uint32_t link_bits = 1;
+    while ((1ull << link_bits) < (uint64_t)L) ++link_bits;
+    const size_t smem = (size_t)N * 16;
+    if (smem > 200 * 1024 || (size_t)N * 8 > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+
+    // ---- order (Alg. 3 lines 1-7) ----
+    t_setup.start();
+    const uint32_t NS = (uint32_t)ph.sources.size();
+    const uint32_t sort_blocks = (uint32_t)((C + SORT_TILE - 1) / SORT_TILE);
+    Carver c;
+    const size_t o_w = c.take((size_t)L * 8), o_D = c.take((size_t)NS * N * 8), o_cd = c.take((size_t)C * 8),
+                 o_k0 = c.take((size_t)C * 8), o_k1 = c.take((size_t)C * 8), o_v0 = c.take((size_t)C * 4),
+                 o_v1 = c.take((size_t)C * 4), o_h = c.take((size_t)256 * sort_blocks * 4), o_ctrl = c.take(sizeof(BfsCtrl));
+    void* blob = nullptr;
+    int rc = dev_alloc(c.cur, &blob);
+    if (rc) return rc;
+    struct Guard { void* p[4] = {nullptr, nullptr, nullptr, nullptr}; ~Guard() { for (void* q : p) dev_free(q); } } guard;
+    guard.p[0] = blob;
+    unsigned char* b = (unsigned char*)blob;
+    uint64_t* d_w = (uint64_t*)(b + o_w);
+    uint64_t* d_D = (uint64_t*)(b + o_D);
+    uint64_t* d_cdist = (uint64_t*)(b + o_cd);
+    uint64_t* keys[2] = {(uint64_t*)(b + o_k0), (uint64_t*)(b + o_k1)};
+    uint32_t* vals[2] = {(uint32_t*)(b + o_v0), (uint32_t*)(b + o_v1)};
+    uint32_t* ghist = (uint32_t*)(b + o_h);
+    BfsCtrl* ctrl = (BfsCtrl*)(b + o_ctrl);
+    CU(cudaMemsetAsync(ctrl, 0, sizeof(BfsCtrl), st));
+    k_link_cost<<<(L + 255) / 256, 256, 0, st>>>(t->d_alpha, t->d_bpp, L, P.chunk_bytes, d_w);
+    if (NS) {
+        const size_t ds = (size_t)N * 8;
+        if (ds > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ds));
+        k_distances<<<NS, 256, ds, st>>>(pv.esrc, pv.edst, d_w, N, L, ph.d_sources, d_D);
+    }
+    const uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
+    const unsigned gC = (C + 255) / 256;
+    k_bfs_keys<<<gC, 256, 0, st>>>(ph.d_cond_src, ph.d_dest_off, ph.d_dests, C, ph.d_sidx, d_D, N, k0, k1, d_cdist, keys[0],
+                                   vals[0], ctrl);
+    int cur = radix_sort_pairs(keys, vals, C, 64, ghist, sort_blocks, 0);          // by (draw, chunk)
+    k_bfs_keys2<<<gC, 256, 0, st>>>(d_cdist, vals[cur], C, keys[cur ^ 1], vals[cur ^ 1]);
+    cur = radix_sort_pairs(keys, vals, C, 64, ghist, sort_blocks, cur ^ 1);         // stable, by descending c.dist
+    const uint32_t* d_order = vals[cur];
+    CU(cudaGetLastError());
+    BfsCtrl* mb = (BfsCtrl*)G.mailbox;
+    CU(cudaMemcpyAsync(mb, ctrl, sizeof(BfsCtrl), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (mb->err & 1u) return PCCL_ERR_UNREACHABLE;
+    if (mb->err) return PCCL_ERR_INTERNAL;
+    const uint32_t nact = mb->nact;
+    t_setup.stop();
+    if (nact == 0) return PCCL_OK;
+
+    // ---- window size = co-resident CTAs ----
+    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_bfs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bfs, (int)BFS_THREADS, smem));
+    if (occ < 1) return PCCL_ERR_CUDA;
+    const uint32_t B = std::max(1u, std::min(std::min((uint32_t)occ, 4u) * (uint32_t)G.sm_count, nact));
+
+    // ---- record capacity: a tree has at most N - 1 transfers; retried with the exact count if short ----
+    uint64_t cap = 0;
+    for (uint32_t ci = 0; ci < C; ++ci) {
+        const uint64_t nd = ph.dest_off[ci + 1] - ph.dest_off[ci];
+        cap += std::min<uint64_t>((uint64_t)N - 1, nd * 16);
+    }
+    uint32_t R = 64;
+    for (int attempt = 0; attempt < 8; ++attempt) {
+        Carver w2;
+        const size_t o_runs = w2.take((size_t)L * R * 16), o_rn = w2.take((size_t)L * 4), o_rs = w2.take((size_t)L * B * 8),
+                     o_rp = w2.take((size_t)L * B * 4), o_tl = w2.take((size_t)B * N * 4), o_ts = w2.take((size_t)B * N * 8);
+        void* ws = nullptr;
+        rc = dev_alloc(w2.cur, &ws);
+        if (rc) return rc;
+        guard.p[1] = ws;
+        Rec* raw = nullptr;
+        rc = dev_alloc(std::max<uint64_t>(cap, 1) * sizeof(Rec), (void**)&raw);
+        if (rc) return rc;
+        guard.p[2] = raw;
+        unsigned char* q = (unsigned char*)ws;
+        BfsArgs a;
+        a.N = N; a.L = L; a.R = R; a.B = B; a.link_bits = link_bits; a.nact = nact;
+        a.esrc = pv.esrc; a.edst = pv.edst; a.psrc = t->d_src; a.pdst = t->d_dst; a.w = d_w;
+        a.cond_src = ph.d_cond_src; a.dest_off = ph.d_dest_off; a.dests = ph.d_dests; a.order = d_order;
+        a.runs = (ulonglong2*)(q + o_runs); a.rl_n = (uint32_t*)(q + o_rn); a.rl_start = (uint64_t*)(q + o_rs);
+        a.rl_pos = (uint32_t*)(q + o_rp); a.tr_link = (uint32_t*)(q + o_tl); a.tr_start = (uint64_t*)(q + o_ts);
+        a.out = raw; a.out_cap = cap; a.t_offset = 0; a.ctrl = ctrl;
+        t_loop.start();
+        k_bfs_init<<<(std::max(L, 1u) + 255) / 256, 256, 0, st>>>(a);
+        void* args[] = {(void*)&a};
+        CU(cudaLaunchCooperativeKernel((const void*)k_bfs, dim3(B), dim3(BFS_THREADS), args, smem, st));
+        CU(cudaMemcpyAsync(mb, ctrl, sizeof(BfsCtrl), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        t_loop.stop();
+        const uint32_t err = mb->err;
+        if (err & 1u) return PCCL_ERR_UNREACHABLE;
+        if (err & 2u) return PCCL_ERR_UNSUPPORTED;          // times do not fit beside the link id in 64 bits
+        if (err & 16u) return PCCL_ERR_INTERNAL;
+        if (err & (4u | 8u)) {                              // a busy-run row or the record buffer was too small
+            if (err & 4u) R *= 4;
+            if (err & 8u) cap = mb->nrec;
+            dev_free(ws); dev_free(raw);
+            guard.p[1] = guard.p[2] = nullptr;
+            CU(cudaMemsetAsync(&ctrl->err, 0, 4, st));
+            continue;
+        }
+        const uint64_t M = mb->nrec;
+        res->M = M; res->tmax = mb->tmax; res->conditions = nact; res->searches = mb->searches; res->relax = mb->relax;
+        res->rounds = mb->rounds; res->grid = B;
+        dev_free(ws);
+        guard.p[1] = nullptr;
+        if (M == 0) return PCCL_OK;
+        Rec* sorted = nullptr;
+        rc = dev_alloc(M * sizeof(Rec), (void**)&sorted);
+        if (rc) return rc;
+        t_emit.start();
+        rc = reverse_sorted(raw, M, mb->tmax, L, sorted, ph.transposed, ph.transposed ? 0 : t_shift);
+        if (rc) { dev_free(sorted); return rc; }
+        t_emit.stop();
+        *out_recs = sorted;
+        return PCCL_OK;
+    }
+    return PCCL_ERR_NOMEM;
+}
 
 }  // namespace
 
@@ -873,6 +1018,43 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
     for (size_t pi = 0; pi < P->phases.size(); ++pi) {
         const Phase& ph = P->phases[pi];
         const bool last = pi + 1 == P->phases.size();
+        if (flags & PCCL_FLAG_BFS) {   // the paper's per-condition search instead of the matching loop
+            BfsResult br;
+            Rec* recs = nullptr;
+            const uint64_t toff = (pi == 0) ? 0 : T1;
+            rc = bfs_phase(*P, ph, seed, toff, &recs, &br, t_setup, t_loop, t_emit);
+            if (rc) return fail(rc);
+            S->stats.wants_total += br.M;
+            S->stats.events += br.conditions;
+            S->stats.rows_scanned += br.searches;
+            S->stats.links_scanned += br.relax;
+            S->stats.slow_picks += br.rounds;
+            S->stats.grid_blocks = br.grid;
+            if (ph.transposed) {
+                if (last) { out_recs = recs; S->M = br.M; S->T = br.tmax; } else stage1 = recs;
+                M1 = br.M; T1 = br.tmax;
+                S->stats.time_phase1_ps = br.tmax;
+            } else {
+                const uint64_t base = (pi == 0) ? 0 : M1;
+                if (base) {
+                    rc = dev_alloc((base + br.M) * sizeof(Rec), (void**)&out_recs);
+                    if (rc) { dev_free(recs); return fail(rc); }
+                    if (cudaMemcpyAsync(out_recs, stage1, base * sizeof(Rec), cudaMemcpyDeviceToDevice, G.stream) != cudaSuccess ||
+                        (br.M && cudaMemcpyAsync(out_recs + base, recs, br.M * sizeof(Rec), cudaMemcpyDeviceToDevice, G.stream) !=
+                                     cudaSuccess)) {
+                        (void)cudaGetLastError();
+                        dev_free(recs);
+                        return fail(PCCL_ERR_CUDA);
+                    }
+                    dev_free(recs);
+                } else {
+                    out_recs = recs;
+                }
+                S->M = base + br.M;
+                S->T = toff + br.tmax;
+            }
+            continue;
+        }
         if (!W.blob) { rc = work_alloc(*P, W); if (rc) return fail(rc); }
         uint64_t M = 0;
         t_setup.start();

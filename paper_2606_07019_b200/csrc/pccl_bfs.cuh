@@ -1,0 +1,342 @@
+// =====================================================================================
+//  pccl_bfs.cuh -- the paper's own synthesizer on the GPU: Algorithms 1-3 with the timing
+//  rules of section 4.6, condition by condition
+//  (readings Q19-Q22).  PCCL_FLAG_BFS selects it.
+//
+//  What is computed (the same result as routing the conditions strictly one after another):
+//    order      Alg. 3 lines 1-7: conditions by descending c.dist; ties by a Philox draw keyed
+//               on the chunk (tag 2), then chunk id.
+//    search     Alg. 2 + 4.6: earliest arrival of the chunk at every device, where link l may
+//               start at the first s >= arrival(src(l)) with [s, s + w(l)) free on l; of
+//               several links reaching a device at its earliest time the lowest link id is
+//               recorded.
+//    filter     PAPER.md:298: only the recorded paths src -> dests are kept.
+//    remove     Alg. 3 line 13 / Fig. 10: their intervals become busy for later conditions.
+//
+//  How: conditions depend on each other only through busy intervals, so a WINDOW of B
+//  consecutive conditions (one per CTA) is searched at once against the same snapshot of the
+//  busy intervals, optimistically.  A result stays exact as long as none of its kept transfers
+//  overlaps an interval taken by a condition earlier in the order (arrivals can only grow when
+//  intervals are added, and a path whose own intervals are untouched still reaches its nodes
+//  at the snapshot's earliest times, through the same lowest-id links).  Each round:
+//    S  search (only CTAs whose result was invalidated or whose slot moved on) and post every
+//       kept transfer on its link's round list
+//    C  every condition looks for an overlap with a lower-positioned one on those lists;
+//       first_bad = the lowest position that has one
+//    M  conditions below first_bad commit: records are emitted, their intervals are merged into
+//       the links' busy runs (one thread per link, no locks); later results that overlap a
+//       committed interval are invalidated; the window slides to first_bad
+//  with a grid barrier after each.  The position at the window base never has a conflict, so
+//  every round commits at least one condition.
+//
+//  Busy runs of a link: sorted, disjoint [start, end) pairs in a row of R 16-byte entries
+//  (entry 0 holds the count).  Every transfer on link l lasts w(l), so a gap shorter than w(l)
+//  can never be used: such gaps are closed when runs are merged, which keeps rows short.
+// =====================================================================================
+#pragma once
+
+namespace pccl {
+
+struct BfsCtrl {
+    unsigned long long first_bad[2];   // per round parity: lowest conflicting position
+    unsigned long long nrec;           // records emitted (counted past the capacity too)
+    unsigned long long tmax;           // max t_end (without the phase offset)
+    unsigned long long searches, relax, rounds;
+    uint32_t nact;                     // conditions with at least one dest
+    uint32_t err;                      // 1 unreachable, 2 time bits, 4 run row full, 8 record buffer full, 16 internal
+};
+
+struct BfsArgs {
+    uint32_t N, L, R, B, link_bits, nact;
+    const uint32_t *esrc, *edst, *psrc, *pdst;
+    const uint64_t* w;
+    const uint32_t* cond_src;
+    const uint64_t* dest_off;
+    const uint32_t* dests;
+    const uint32_t* order;             // [nact] chunk ids in routing order
+    ulonglong2* runs;                  // [L][R]
+    uint32_t* rl_n;                    // [L]    round list length
+    uint64_t* rl_start;                // [L][B]
+    uint32_t* rl_pos;                  // [L][B]
+    uint32_t* tr_link;                 // [B][N] kept transfers of each slot
+    uint64_t* tr_start;                // [B][N]
+    Rec* out;
+    uint64_t out_cap, t_offset;
+    BfsCtrl* ctrl;
+};
+
+constexpr uint32_t BFS_THREADS = 256;
+constexpr unsigned long long BFS_INF = ~0ull;
+
+// ---- Alg. 3 lines 1-7: c.dist and the two sort keys ----------------------------------------
+__global__ void k_bfs_keys(const uint32_t* __restrict__ cond_src, const uint64_t* __restrict__ dest_off,
+                           const uint32_t* __restrict__ dests, uint32_t C, const uint32_t* __restrict__ sidx,
+                           const uint64_t* __restrict__ D, uint32_t N, uint32_t k0, uint32_t k1,
+                           uint64_t* __restrict__ cdist, uint64_t* __restrict__ key, uint32_t* __restrict__ val,
+                           BfsCtrl* ctrl) {
+    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= C) return;
+    const uint64_t d0 = dest_off[c], d1 = dest_off[c + 1];
+    uint64_t dmax = 0;
+    if (d1 > d0) {
+        const uint64_t* row = D + (size_t)sidx[cond_src[c]] * N;
+        for (uint64_t i = d0; i < d1; ++i) dmax = max(dmax, (uint64_t)row[dests[i]]);
+        if (dmax == T_INF) atomicOr(&ctrl->err, 1u);
+        atomicAdd(&ctrl->nact, 1u);
+    }
+    cdist[c] = dmax;                                   // 0 = nothing to route: sorts last
+    key[c] = ((uint64_t)philox_draw(c, 0, 0, 2, k0, k1) << 32) | c;
+    val[c] = c;
+}
+
+// second (stable) pass: descending c.dist
+__global__ void k_bfs_keys2(const uint64_t* __restrict__ cdist, const uint32_t* __restrict__ val_in, uint32_t C,
+                            uint64_t* __restrict__ key, uint32_t* __restrict__ val) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= C) return;
+    const uint32_t c = val_in[i];
+    key[i] = ~cdist[c];
+    val[i] = c;
+}
+
+__global__ void k_bfs_init(BfsArgs a) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < a.L) {
+        a.runs[(size_t)i * a.R] = make_ulonglong2(0ull, 0ull);
+        a.rl_n[i] = 0;
+    }
+    if (i == 0) {
+        a.ctrl->first_bad[0] = BFS_INF; a.ctrl->first_bad[1] = BFS_INF;
+        a.ctrl->nrec = 0; a.ctrl->tmax = 0; a.ctrl->searches = 0; a.ctrl->relax = 0; a.ctrl->rounds = 0;
+    }
+}
+
+// ---- NextAvailableTime for one link (Alg. 1 + Fig. 10): first s >= a with [s, s + w) free ---
+__device__ __forceinline__ uint64_t bfs_depart(const ulonglong2* __restrict__ row, uint64_t a, uint64_t w) {
+    const ulonglong2 h = __ldcg(row), r1 = __ldcg(row + 1), r2 = __ldcg(row + 2), r3 = __ldcg(row + 3);
+    const uint32_t n = (uint32_t)h.x;
+    uint64_t s = a;
+    uint32_t i = 1;
+    if (n > 3) {                                       // first run ending after s (ends ascend)
+        uint32_t lo = 1, hi = n + 1;
+        while (lo < hi) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (__ldcg(row + mid).y <= s) lo = mid + 1; else hi = mid;
+        }
+        i = lo;
+    }
+    for (; i <= n; ++i) {
+        const ulonglong2 r = (i == 1) ? r1 : (i == 2) ? r2 : (i == 3) ? r3 : __ldcg(row + i);
+        if (r.y <= s) continue;
+        if (s + w <= r.x) break;
+        s = r.y;
+    }
+    return s;
+}
+
+// ---- Alg. 3 line 13: take [s, s + w) on a link (single writer per link) ----------------------
+__device__ __forceinline__ bool bfs_occupy(ulonglong2* row, uint32_t R, uint64_t s, uint64_t w) {
+    uint32_t n = (uint32_t)row[0].x;
+    const uint64_t e = s + w;
+    uint32_t i = 1;                                    // first run starting after s
+    while (i <= n && row[i].x <= s) ++i;
+    const bool mp = i > 1 && s - row[i - 1].y < w;     // gap to the run in front is unusable (or none)
+    const bool mn = i <= n && row[i].x - e < w;
+    if (mp && mn) {
+        row[i - 1].y = row[i].y;
+        for (uint32_t j = i; j < n; ++j) row[j] = row[j + 1];
+        --n;
+    } else if (mp) {
+        row[i - 1].y = e;
+    } else if (mn) {
+        row[i].x = s;
+    } else {
+        if (n + 2 > R) return false;
+        for (uint32_t j = n + 1; j > i; --j) row[j] = row[j - 1];
+        row[i] = make_ulonglong2(s, e);
+        ++n;
+    }
+    row[0].x = n;
+    return true;
+}
+
+// ---- Alg. 2 + 4.6 for one condition, by one CTA ---------------------------------------------
+// key[v] = (arrival(v) << link_bits) | recorded link, so that one 64-bit min keeps the earliest
+// arrival and, among equal arrivals, the lowest link id (reading Q20).  Label-correcting sweeps
+// over the links whose source improved in the previous sweep; sources that arrive after every
+// dest has been reached (`bound`) are not expanded: they can not lie on a kept path.
+struct BfsShared {
+    unsigned long long bound;
+    uint32_t cnt, minconf, fb_lo, fb_hi, base_idx_lo, base_idx_hi;
+    unsigned long long tmax;
+};
+
+__device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long* key, uint32_t* stamp, uint32_t* keep,
+                           BfsShared& sh, uint32_t slot, uint32_t& ntr, uint64_t& relax) {
+    const uint32_t tid = threadIdx.x, lb = a.link_bits;
+    const uint64_t lmask = (1ull << lb) - 1;
+    const uint32_t src = a.cond_src[chunk];
+    const uint64_t d0 = a.dest_off[chunk];
+    const uint32_t nd = (uint32_t)(a.dest_off[chunk + 1] - d0);
+    for (uint32_t v = tid; v < a.N; v += BFS_THREADS) { key[v] = BFS_INF; stamp[v] = NONE32; keep[v] = 0; }
+    __syncthreads();
+    if (tid == 0) { key[src] = 0; stamp[src] = 0; }
+    __syncthreads();
+    for (uint32_t it = 0;; ++it) {
+        if (tid == 0) sh.bound = 0;
+        __syncthreads();
+        unsigned long long bl = 0;
+        for (uint32_t k = tid; k < nd; k += BFS_THREADS) bl = max(bl, key[a.dests[d0 + k]] >> lb);
+        if (bl) atomicMax(&sh.bound, bl);
+        __syncthreads();
+        const unsigned long long bound = sh.bound;
+        int any = 0;
+        for (uint32_t l = tid; l < a.L; l += BFS_THREADS) {
+            const uint32_t u = a.esrc[l];
+            if (((volatile uint32_t*)stamp)[u] != it) continue;
+            const unsigned long long au = ((volatile unsigned long long*)key)[u] >> lb;
+            if (au > bound) continue;
+            const uint32_t v = a.edst[l];
+            if (v == src) continue;
+            const uint64_t wl = a.w[l];
+            const uint64_t cand = bfs_depart(a.runs + (size_t)l * a.R, au, wl) + wl;
+            ++relax;
+            if (cand >> (64 - lb)) { atomicOr(&a.ctrl->err, 2u); continue; }
+            const unsigned long long kc = (cand << lb) | l;
+            const unsigned long long old = atomicMin(&key[v], kc);
+            if (kc < old && cand < (old >> lb)) { ((volatile uint32_t*)stamp)[v] = it + 1; any = 1; }
+        }
+        if (!__syncthreads_or(any)) break;
+        if (it > a.N + 1) { if (tid == 0) atomicOr(&a.ctrl->err, 16u); break; }
+    }
+    // walk back from every dest; stop at a node that is already kept
+    for (uint32_t k = tid; k < nd; k += BFS_THREADS) {
+        uint32_t v = a.dests[d0 + k];
+        if (key[v] == BFS_INF) { atomicOr(&a.ctrl->err, 1u); continue; }
+        uint32_t guard = 0;
+        while (v != src && atomicExch(&keep[v], 1u) == 0u) {
+            v = a.esrc[(uint32_t)(key[v] & lmask)];
+            if (++guard > a.N) { atomicOr(&a.ctrl->err, 16u); break; }
+        }
+    }
+    if (tid == 0) sh.cnt = 0;
+    __syncthreads();
+    uint32_t* tl = a.tr_link + (size_t)slot * a.N;
+    uint64_t* ts = a.tr_start + (size_t)slot * a.N;
+    for (uint32_t v = tid; v < a.N; v += BFS_THREADS) {
+        if (!keep[v]) continue;
+        const uint32_t i = atomicAdd(&sh.cnt, 1u);
+        const uint32_t l = (uint32_t)(key[v] & lmask);
+        tl[i] = l;
+        ts[i] = (key[v] >> lb) - a.w[l];
+    }
+    __syncthreads();
+    ntr = sh.cnt;
+}
+
+__global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
+    cg::grid_group grid = cg::this_grid();
+    extern __shared__ unsigned long long bfs_smem[];
+    unsigned long long* key = bfs_smem;                         // [N]
+    uint32_t* stamp = (uint32_t*)(key + a.N);                   // [N]
+    uint32_t* keep = stamp + a.N;                               // [N]
+    __shared__ BfsShared sh;
+    const uint32_t tid = threadIdx.x, slot = blockIdx.x, B = a.B;
+    const uint32_t gtid = blockIdx.x * BFS_THREADS + tid, gthreads = gridDim.x * BFS_THREADS;
+    uint32_t* tl = a.tr_link + (size_t)slot * a.N;
+    uint64_t* ts = a.tr_start + (size_t)slot * a.N;
+    uint64_t base = 0, relax = 0, searches = 0;
+    uint32_t pos = NONE32, ntr = 0;   // the result this CTA holds (CTA-uniform)
+    bool valid = false;
+    for (uint32_t round = 0; base < a.nact; ++round) {
+        // ---- S: search + post ---------------------------------------------------------------
+        const uint64_t p64 = base + ((slot + B - (uint32_t)(base % B)) % B);
+        const bool active = p64 < a.nact;
+        const uint32_t p = (uint32_t)p64;
+        if (active) {
+            if (!(valid && pos == p)) {
+                bfs_search(a, a.order[p], key, stamp, keep, sh, slot, ntr, relax);
+                pos = p; valid = true; ++searches;
+            }
+            for (uint32_t i = tid; i < ntr; i += BFS_THREADS) {
+                const uint32_t l = tl[i];
+                const uint32_t j = atomicAdd(&a.rl_n[l], 1u);
+                if (j < B) { a.rl_start[(size_t)l * B + j] = ts[i]; a.rl_pos[(size_t)l * B + j] = p; }
+                else atomicOr(&a.ctrl->err, 16u);
+            }
+        }
+        grid.sync();
+        // ---- C: lowest earlier position whose transfer overlaps one of mine --------------------
+        if (tid == 0) { sh.minconf = NONE32; sh.tmax = 0; }
+        __syncthreads();
+        if (active) {
+            uint32_t mc = NONE32;
+            for (uint32_t i = tid; i < ntr; i += BFS_THREADS) {
+                const uint32_t l = tl[i];
+                const uint64_t s = ts[i], wl = a.w[l];
+                const uint32_t n = min(ldcg32(a.rl_n + l), B);
+                for (uint32_t j = 0; j < n; ++j) {
+                    const uint32_t q = ldcg32(a.rl_pos + (size_t)l * B + j);
+                    if (q >= p) continue;
+                    const uint64_t sq = ldcg64(a.rl_start + (size_t)l * B + j);
+                    if (s < sq + wl && sq < s + wl) mc = min(mc, q);
+                }
+            }
+            if (mc != NONE32) atomicMin(&sh.minconf, mc);
+        }
+        __syncthreads();
+        if (active && tid == 0 && sh.minconf != NONE32) atomicMin(&a.ctrl->first_bad[round & 1], (unsigned long long)p);
+        grid.sync();
+        // ---- M: commit below first_bad ----------------------------------------------------------
+        if (tid == 0) {
+            const unsigned long long fbv = ldcg64((const uint64_t*)&a.ctrl->first_bad[round & 1]);
+            const uint64_t lim = min((uint64_t)a.nact, base + B);
+            const uint64_t fb = fbv < lim ? fbv : lim;
+            sh.fb_lo = (uint32_t)fb; sh.fb_hi = (uint32_t)(fb >> 32);
+            if (active && p < fb) {
+                const unsigned long long bi = atomicAdd(&a.ctrl->nrec, (unsigned long long)ntr);
+                sh.base_idx_lo = (uint32_t)bi; sh.base_idx_hi = (uint32_t)(bi >> 32);
+            }
+        }
+        __syncthreads();
+        const uint64_t fb = ((uint64_t)sh.fb_hi << 32) | sh.fb_lo;
+        if (active && p < fb) {
+            const uint64_t bi = ((uint64_t)sh.base_idx_hi << 32) | sh.base_idx_lo;
+            const uint32_t chunk = a.order[p];
+            unsigned long long tm = 0;
+            for (uint32_t i = tid; i < ntr; i += BFS_THREADS) {
+                const uint32_t l = tl[i];
+                const uint64_t s = ts[i], e = s + a.w[l];
+                tm = max(tm, (unsigned long long)e);
+                if (bi + i < a.out_cap) a.out[bi + i] = Rec{chunk, a.psrc[l], a.pdst[l], l, s + a.t_offset, e + a.t_offset};
+                else atomicOr(&a.ctrl->err, 8u);
+            }
+            if (tm) atomicMax(&sh.tmax, tm);
+            __syncthreads();
+            if (tid == 0 && sh.tmax) atomicMax(&a.ctrl->tmax, sh.tmax);
+            valid = false;
+        } else if (active) {
+            valid = sh.minconf == NONE32 || sh.minconf >= fb;
+        }
+        for (uint32_t l = gtid; l < a.L; l += gthreads) {
+            const uint32_t n = min(ldcg32(a.rl_n + l), B);
+            if (!n) continue;
+            ulonglong2* row = a.runs + (size_t)l * a.R;
+            const uint64_t wl = a.w[l];
+            for (uint32_t j = 0; j < n; ++j) {
+                if (ldcg32(a.rl_pos + (size_t)l * B + j) >= fb) continue;
+                if (!bfs_occupy(row, a.R, ldcg64(a.rl_start + (size_t)l * B + j), wl)) atomicOr(&a.ctrl->err, 4u);
+            }
+            a.rl_n[l] = 0;
+        }
+        if (gtid == 0) { a.ctrl->first_bad[(round + 1) & 1] = BFS_INF; a.ctrl->rounds = round + 1; }
+        base = fb;
+        grid.sync();
+    }
+    // statistics
+    for (int o = 16; o; o >>= 1) relax += __shfl_down_sync(0xFFFFFFFFu, relax, o);
+    if ((tid & 31) == 0 && relax) atomicAdd(&a.ctrl->relax, (unsigned long long)relax);
+    if (tid == 0 && searches) atomicAdd(&a.ctrl->searches, (unsigned long long)searches);
+}
+
+}  // namespace pccl

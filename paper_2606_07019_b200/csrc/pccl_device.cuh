@@ -1101,14 +1101,17 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop(const Loop
 // raw record of the transposed broadcast (c, psrc, pdst, l, ts, te)  ->  (c, psrc, pdst, l, T-te, T-ts);
 // the loop already reported the PHYSICAL endpoints, which are the reversed transfer's src -> dst.
 __global__ void k_reverse_keys(Rec* __restrict__ raw, uint64_t n, uint64_t T, uint32_t link_bits,
-                               uint64_t* __restrict__ keys, uint32_t* __restrict__ idx) {
+                               uint64_t* __restrict__ keys, uint32_t* __restrict__ idx, bool reverse = true) {
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     Rec r = raw[i];
-    const uint64_t ts = T - r.t_end, te = T - r.t_start;
-    r.t_start = ts;
-    r.t_end = te;
-    raw[i] = r;
+    uint64_t ts = r.t_start;
+    if (reverse) {
+        ts = T - r.t_end;
+        r.t_end = T - r.t_start;
+        r.t_start = ts;
+        raw[i] = r;
+    }
     keys[i] = (ts << link_bits) | r.link;
     idx[i] = (uint32_t)i;
 }

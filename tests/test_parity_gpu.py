@@ -402,6 +402,43 @@ def test_one_barrier_and_two_barrier_loops_agree(pk, maker):
     assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_TWO_BARRIERS), o)
 
 
+# ------------------------------------------------------------------------------ the paper's own synthesizer (BFS)
+BFS_CASES = [wl.config1, wl.config2, wl.config3, wl.config4_small, wl.config5_small, wl.two_groups_mesh3x3,
+             lambda s: wl.ring_all_gather(8, False, s), lambda s: wl.ring_all_gather(9, True, s, chunks_per_npu=3),
+             lambda s: wl.path_point_to_point(6, s), lambda s: _torus_all_gather((12, 12), 2, s)]
+
+
+@pytest.mark.parametrize("maker", BFS_CASES, ids=lambda m: getattr(m, "__name__", "case"))
+@pytest.mark.parametrize("seed", [0, 1])
+def test_bfs_mode_equals_oracle(pk, maker, seed):
+    """PCCL_FLAG_BFS (Alg. 1-3 + section 4.6, windowed optimistic search) against the strictly sequential oracle:
+    identical records, T, condition count, transfer count."""
+    p = maker(seed)
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_BFS)
+    assert_same(p, s, o)
+    checker.check_structure(p, s.transfers)
+    st = s.stats
+    assert st["rows_scanned"] >= st["events"] and st["slow_picks"] >= 1
+
+
+def test_bfs_mode_many_conditions_per_link(pk):
+    """8-node ring, 1040 chunks per node: 8,320 conditions over 16 links -- long busy-run rows, most windows
+    conflict at once (almost every round commits few conditions)"""
+    p = wl.ring_all_gather(8, True, 2, chunks_per_npu=130, chunk_bytes=4096)
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_BFS)
+    assert_same(p, s, o)
+
+
+def test_bfs_mode_ring3000(pk):
+    p = _ring3000_a2a(3)
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_BFS)
+    assert_same(p, s, o)
+    checker.check_structure(p, s.transfers)
+
+
 # ------------------------------------------------------------------------------ randomized problems
 def _random_problem(i):
     """seeded random directed multigraph with heterogeneous links, a random process group and a random
