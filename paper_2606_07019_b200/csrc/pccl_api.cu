@@ -7,6 +7,7 @@
 #include "../../include/pccl.h"
 
 #include <algorithm>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <future>
@@ -868,8 +869,8 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     if (L == 0) return PCCL_ERR_UNREACHABLE;
     uint32_t link_bits = 1;
     while ((1ull << link_bits) < (uint64_t)L) ++link_bits;
-    const size_t smem = (size_t)N * 16;
-    if (smem > 200 * 1024 || (size_t)N * 8 > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+    const size_t smem = (size_t)N * 20;
+    if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
 
     // ---- order (Alg. 3 lines 1-7) ----
     t_setup.start();
@@ -918,7 +919,7 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     if (nact == 0) return PCCL_OK;
 
     // ---- window size = co-resident CTAs ----
-    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_bfs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (smem > 40 * 1024) CU(cudaFuncSetAttribute(k_bfs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bfs, (int)BFS_THREADS, smem));
     if (occ < 1) return PCCL_ERR_CUDA;
@@ -946,6 +947,8 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         unsigned char* q = (unsigned char*)ws;
         BfsArgs a;
         a.N = N; a.L = L; a.R = R; a.B = B; a.link_bits = link_bits; a.nact = nact;
+        a.max_deg = std::max(1u, ph.transposed ? t->max_in : t->max_out);
+        a.out_off = ph.transposed ? t->d_in_off : t->d_out_off; a.out_link = pv.out_link;
         a.esrc = pv.esrc; a.edst = pv.edst; a.psrc = t->d_src; a.pdst = t->d_dst; a.w = d_w;
         a.cond_src = ph.d_cond_src; a.dest_off = ph.d_dest_off; a.dests = ph.d_dests; a.order = d_order;
         a.runs = (ulonglong2*)(q + o_runs); a.rl_n = (uint32_t*)(q + o_rn); a.rl_start = (uint64_t*)(q + o_rs);
@@ -970,6 +973,9 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
             CU(cudaMemsetAsync(&ctrl->err, 0, 4, st));
             continue;
         }
+        if (getenv("PCCL_BFS_DEBUG"))
+            fprintf(stderr, "[pccl bfs] rounds %llu searches %llu iters %llu relax %llu  search %.2f ms check %.2f ms commit %.2f ms  R %u B %u\n",
+                    mb->rounds, mb->searches, mb->iters, mb->relax, mb->ns_search * 1e-6, mb->ns_check * 1e-6, mb->ns_commit * 1e-6, R, B);
         const uint64_t M = mb->nrec;
         res->M = M; res->tmax = mb->tmax; res->conditions = nact; res->searches = mb->searches; res->relax = mb->relax;
         res->rounds = mb->rounds; res->grid = B;

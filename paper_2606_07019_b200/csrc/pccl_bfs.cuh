@@ -42,12 +42,14 @@ struct BfsCtrl {
     unsigned long long nrec;           // records emitted (counted past the capacity too)
     unsigned long long tmax;           // max t_end (without the phase offset)
     unsigned long long searches, relax, rounds;
+    unsigned long long ns_search, ns_check, ns_commit, iters;   // phase times seen by CTA 0 (barrier waits included)
     uint32_t nact;                     // conditions with at least one dest
     uint32_t err;                      // 1 unreachable, 2 time bits, 4 run row full, 8 record buffer full, 16 internal
 };
 
 struct BfsArgs {
-    uint32_t N, L, R, B, link_bits, nact;
+    uint32_t N, L, R, B, link_bits, nact, max_deg;
+    const uint32_t *out_off, *out_link;   // out-links per device in the direction being synthesized
     const uint32_t *esrc, *edst, *psrc, *pdst;
     const uint64_t* w;
     const uint32_t* cond_src;
@@ -67,6 +69,12 @@ struct BfsArgs {
 
 constexpr uint32_t BFS_THREADS = 256;
 constexpr unsigned long long BFS_INF = ~0ull;
+
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 
 // ---- Alg. 3 lines 1-7: c.dist and the two sort keys ----------------------------------------
 __global__ void k_bfs_keys(const uint32_t* __restrict__ cond_src, const uint64_t* __restrict__ dest_off,
@@ -108,30 +116,58 @@ __global__ void k_bfs_init(BfsArgs a) {
     if (i == 0) {
         a.ctrl->first_bad[0] = BFS_INF; a.ctrl->first_bad[1] = BFS_INF;
         a.ctrl->nrec = 0; a.ctrl->tmax = 0; a.ctrl->searches = 0; a.ctrl->relax = 0; a.ctrl->rounds = 0;
+        a.ctrl->ns_search = 0; a.ctrl->ns_check = 0; a.ctrl->ns_commit = 0; a.ctrl->iters = 0;
     }
 }
 
 // ---- NextAvailableTime for one link (Alg. 1 + Fig. 10): first s >= a with [s, s + w) free ---
+// bfs_occupy keeps every gap between consecutive runs >= w, so the first fit is either `a` itself (it fits
+// in front of the first run that ends after a) or the end of that run.  Finding that run takes at most two
+// rounds of independent loads for rows of up to 64 runs (8 samples, then the 8 entries between two samples).
 __device__ __forceinline__ uint64_t bfs_depart(const ulonglong2* __restrict__ row, uint64_t a, uint64_t w) {
     const ulonglong2 h = __ldcg(row), r1 = __ldcg(row + 1), r2 = __ldcg(row + 2), r3 = __ldcg(row + 3);
     const uint32_t n = (uint32_t)h.x;
-    uint64_t s = a;
-    uint32_t i = 1;
-    if (n > 3) {                                       // first run ending after s (ends ascend)
-        uint32_t lo = 1, hi = n + 1;
-        while (lo < hi) {
-            const uint32_t mid = (lo + hi) >> 1;
-            if (__ldcg(row + mid).y <= s) lo = mid + 1; else hi = mid;
+    if (n == 0) return a;
+    ulonglong2 r;
+    if (r1.y > a) r = r1;
+    else if (n >= 2 && r2.y > a) r = r2;
+    else if (n >= 3 && r3.y > a) r = r3;
+    else if (n <= 3) return a;
+    else {
+        uint32_t lo = 4, hi = n + 1;                   // the answer is in [lo, hi]; hi = n + 1: no such run
+        const uint32_t stride = (n - 3 + 7) / 8;
+        if (stride <= 8) {
+            ulonglong2 smp[7];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) {
+                const uint32_t j = 3 + (k + 1) * stride;
+                smp[k] = j <= n ? __ldcg(row + j) : make_ulonglong2(0ull, BFS_INF);
+            }
+#pragma unroll
+            for (int k = 6; k >= 0; --k) {
+                const uint32_t j = 3 + (k + 1) * stride;
+                if (j <= n) { if (smp[k].y > a) hi = j; else lo = max(lo, j + 1); }
+            }
+            // hi = first sampled index whose run ends after a (or n + 1); lo = one past the last sampled one that does not
+            ulonglong2 blk[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) blk[k] = (lo + k < hi && lo + k <= n) ? __ldcg(row + lo + k) : make_ulonglong2(0ull, BFS_INF);
+            uint32_t i = hi;
+#pragma unroll
+            for (int k = 7; k >= 0; --k)
+                if (lo + k < hi && lo + k <= n && blk[k].y > a) i = lo + k;
+            if (i > n) return a;
+            r = __ldcg(row + i);
+        } else {
+            while (lo < hi) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (__ldcg(row + mid).y <= a) lo = mid + 1; else hi = mid;
+            }
+            if (lo > n) return a;
+            r = __ldcg(row + lo);
         }
-        i = lo;
     }
-    for (; i <= n; ++i) {
-        const ulonglong2 r = (i == 1) ? r1 : (i == 2) ? r2 : (i == 3) ? r3 : __ldcg(row + i);
-        if (r.y <= s) continue;
-        if (s + w <= r.x) break;
-        s = r.y;
-    }
-    return s;
+    return (a + w <= r.x) ? a : r.y;
 }
 
 // ---- Alg. 3 line 13: take [s, s + w) on a link (single writer per link) ----------------------
@@ -162,53 +198,78 @@ __device__ __forceinline__ bool bfs_occupy(ulonglong2* row, uint32_t R, uint64_t
 
 // ---- Alg. 2 + 4.6 for one condition, by one CTA ---------------------------------------------
 // key[v] = (arrival(v) << link_bits) | recorded link, so that one 64-bit min keeps the earliest
-// arrival and, among equal arrivals, the lowest link id (reading Q20).  Label-correcting sweeps
-// over the links whose source improved in the previous sweep; sources that arrive after every
-// dest has been reached (`bound`) are not expanded: they can not lie on a kept path.
+// arrival and, among equal arrivals, the lowest link id (reading Q20).  Label-correcting sweeps:
+// the devices whose arrival improved in one sweep are the frontier of the next, one thread per
+// (frontier device, out-link).  A device that arrives after every dest has been reached
+// (`bound`) is not expanded: it can not lie on a kept path.  One block barrier per sweep.
 struct BfsShared {
     unsigned long long bound;
+    uint32_t nf[3];                 // frontier sizes, ring: sweep `it` reads [it % 3], fills [(it + 1) % 3]
     uint32_t cnt, minconf, fb_lo, fb_hi, base_idx_lo, base_idx_hi;
     unsigned long long tmax;
 };
 
-__device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long* key, uint32_t* stamp, uint32_t* keep,
+__device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long* key, uint32_t* stamp, uint32_t* fr0, uint32_t* fr1,
                            BfsShared& sh, uint32_t slot, uint32_t& ntr, uint64_t& relax) {
     const uint32_t tid = threadIdx.x, lb = a.link_bits;
     const uint64_t lmask = (1ull << lb) - 1;
     const uint32_t src = a.cond_src[chunk];
     const uint64_t d0 = a.dest_off[chunk];
     const uint32_t nd = (uint32_t)(a.dest_off[chunk + 1] - d0);
-    for (uint32_t v = tid; v < a.N; v += BFS_THREADS) { key[v] = BFS_INF; stamp[v] = NONE32; keep[v] = 0; }
+    const uint32_t MD = a.max_deg;
+    for (uint32_t v = tid; v < a.N; v += BFS_THREADS) { key[v] = BFS_INF; stamp[v] = NONE32; }
+    if (tid == 0) { sh.nf[0] = 1; sh.nf[1] = 0; sh.nf[2] = 0; fr0[0] = src; }
     __syncthreads();
-    if (tid == 0) { key[src] = 0; stamp[src] = 0; }
+    if (tid == 0) key[src] = 0;
     __syncthreads();
+    uint32_t dloc[8];                                   // up to 8 dests are followed by every thread itself
+#pragma unroll
+    for (int k = 0; k < 8; ++k) dloc[k] = (uint32_t)k < nd ? a.dests[d0 + k] : src;
     for (uint32_t it = 0;; ++it) {
-        if (tid == 0) sh.bound = 0;
-        __syncthreads();
-        unsigned long long bl = 0;
-        for (uint32_t k = tid; k < nd; k += BFS_THREADS) bl = max(bl, key[a.dests[d0 + k]] >> lb);
-        if (bl) atomicMax(&sh.bound, bl);
-        __syncthreads();
-        const unsigned long long bound = sh.bound;
-        int any = 0;
-        for (uint32_t l = tid; l < a.L; l += BFS_THREADS) {
-            const uint32_t u = a.esrc[l];
-            if (((volatile uint32_t*)stamp)[u] != it) continue;
-            const unsigned long long au = ((volatile unsigned long long*)key)[u] >> lb;
-            if (au > bound) continue;
+        const uint32_t nf = sh.nf[it % 3];
+        if (nf == 0) { if (tid == 0) atomicAdd(&a.ctrl->iters, (unsigned long long)it); break; }
+        if (it > a.N + 1) { if (tid == 0) atomicOr(&a.ctrl->err, 16u); break; }
+        unsigned long long bound = 0;
+        if (nd <= 8) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) bound = max(bound, ((volatile unsigned long long*)key)[dloc[k]] >> lb);
+        } else {
+            if (tid == 0) sh.bound = 0;
+            __syncthreads();
+            unsigned long long bl = 0;
+            for (uint32_t k = tid; k < nd; k += BFS_THREADS) bl = max(bl, key[a.dests[d0 + k]] >> lb);
+            if (bl) atomicMax(&sh.bound, bl);
+            __syncthreads();
+            bound = sh.bound;
+        }
+        if (tid == 0) sh.nf[(it + 2) % 3] = 0;
+        const uint32_t* cur = (it & 1) ? fr1 : fr0;
+        uint32_t* nxt = (it & 1) ? fr0 : fr1;
+        uint32_t* nfn = &sh.nf[(it + 1) % 3];
+        for (uint32_t i = tid; i < nf * MD; i += BFS_THREADS) {
+            const uint32_t u = cur[i / MD], k = i % MD;
+            const uint32_t o0 = a.out_off[u];
+            if (k >= a.out_off[u + 1] - o0) continue;
+            const uint32_t l = a.out_link[o0 + k];
             const uint32_t v = a.edst[l];
             if (v == src) continue;
+            const unsigned long long au = ((volatile unsigned long long*)key)[u] >> lb;
+            if (au > bound) continue;
             const uint64_t wl = a.w[l];
             const uint64_t cand = bfs_depart(a.runs + (size_t)l * a.R, au, wl) + wl;
             ++relax;
             if (cand >> (64 - lb)) { atomicOr(&a.ctrl->err, 2u); continue; }
             const unsigned long long kc = (cand << lb) | l;
             const unsigned long long old = atomicMin(&key[v], kc);
-            if (kc < old && cand < (old >> lb)) { ((volatile uint32_t*)stamp)[v] = it + 1; any = 1; }
+            if (kc < old && cand < (old >> lb)) {       // arrival improved: v is in the next frontier (once)
+                if (atomicExch(&stamp[v], it) != it) nxt[atomicAdd(nfn, 1u)] = v;
+            }
         }
-        if (!__syncthreads_or(any)) break;
-        if (it > a.N + 1) { if (tid == 0) atomicOr(&a.ctrl->err, 16u); break; }
+        __syncthreads();
     }
+    uint32_t* keep = fr0;                               // the frontier lists are dead now
+    for (uint32_t v = tid; v < a.N; v += BFS_THREADS) keep[v] = 0;
+    __syncthreads();
     // walk back from every dest; stop at a node that is already kept
     for (uint32_t k = tid; k < nd; k += BFS_THREADS) {
         uint32_t v = a.dests[d0 + k];
@@ -239,7 +300,8 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
     extern __shared__ unsigned long long bfs_smem[];
     unsigned long long* key = bfs_smem;                         // [N]
     uint32_t* stamp = (uint32_t*)(key + a.N);                   // [N]
-    uint32_t* keep = stamp + a.N;                               // [N]
+    uint32_t* fr0 = stamp + a.N;                                // [N] frontier lists; fr0 doubles as the keep marks
+    uint32_t* fr1 = fr0 + a.N;                                  // [N]
     __shared__ BfsShared sh;
     const uint32_t tid = threadIdx.x, slot = blockIdx.x, B = a.B;
     const uint32_t gtid = blockIdx.x * BFS_THREADS + tid, gthreads = gridDim.x * BFS_THREADS;
@@ -250,12 +312,14 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
     bool valid = false;
     for (uint32_t round = 0; base < a.nact; ++round) {
         // ---- S: search + post ---------------------------------------------------------------
+        unsigned long long tq0 = 0;
+        if (gtid == 0) tq0 = globaltimer_ns();
         const uint64_t p64 = base + ((slot + B - (uint32_t)(base % B)) % B);
         const bool active = p64 < a.nact;
         const uint32_t p = (uint32_t)p64;
         if (active) {
             if (!(valid && pos == p)) {
-                bfs_search(a, a.order[p], key, stamp, keep, sh, slot, ntr, relax);
+                bfs_search(a, a.order[p], key, stamp, fr0, fr1, sh, slot, ntr, relax);
                 pos = p; valid = true; ++searches;
             }
             for (uint32_t i = tid; i < ntr; i += BFS_THREADS) {
@@ -266,6 +330,8 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
             }
         }
         grid.sync();
+        unsigned long long tq1 = 0;
+        if (gtid == 0) tq1 = globaltimer_ns();
         // ---- C: lowest earlier position whose transfer overlaps one of mine --------------------
         if (tid == 0) { sh.minconf = NONE32; sh.tmax = 0; }
         __syncthreads();
@@ -287,6 +353,8 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
         __syncthreads();
         if (active && tid == 0 && sh.minconf != NONE32) atomicMin(&a.ctrl->first_bad[round & 1], (unsigned long long)p);
         grid.sync();
+        unsigned long long tq2 = 0;
+        if (gtid == 0) tq2 = globaltimer_ns();
         // ---- M: commit below first_bad ----------------------------------------------------------
         if (tid == 0) {
             const unsigned long long fbv = ldcg64((const uint64_t*)&a.ctrl->first_bad[round & 1]);
@@ -332,6 +400,10 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
         if (gtid == 0) { a.ctrl->first_bad[(round + 1) & 1] = BFS_INF; a.ctrl->rounds = round + 1; }
         base = fb;
         grid.sync();
+        if (gtid == 0) {
+            const unsigned long long tq3 = globaltimer_ns();
+            a.ctrl->ns_search += tq1 - tq0; a.ctrl->ns_check += tq2 - tq1; a.ctrl->ns_commit += tq3 - tq2;
+        }
     }
     // statistics
     for (int o = 16; o; o >>= 1) relax += __shfl_down_sync(0xFFFFFFFFu, relax, o);
