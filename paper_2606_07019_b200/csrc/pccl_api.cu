@@ -869,7 +869,7 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     if (L == 0) return PCCL_ERR_UNREACHABLE;
     uint32_t link_bits = 1;
     while ((1ull << link_bits) < (uint64_t)L) ++link_bits;
-    const size_t smem = (size_t)N * 20;
+    const size_t smem = (size_t)N * 20 + ((size_t)N + 1) * 4;
     if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
 
     // ---- order (Alg. 3 lines 1-7) ----
@@ -879,7 +879,8 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     Carver c;
     const size_t o_w = c.take((size_t)L * 8), o_D = c.take((size_t)NS * N * 8), o_cd = c.take((size_t)C * 8),
                  o_k0 = c.take((size_t)C * 8), o_k1 = c.take((size_t)C * 8), o_v0 = c.take((size_t)C * 4),
-                 o_v1 = c.take((size_t)C * 4), o_h = c.take((size_t)256 * sort_blocks * 4), o_ctrl = c.take(sizeof(BfsCtrl));
+                 o_v1 = c.take((size_t)C * 4), o_h = c.take((size_t)256 * sort_blocks * 4), o_ctrl = c.take(sizeof(BfsCtrl)),
+                 o_os = c.take((size_t)L * 16);
     void* blob = nullptr;
     int rc = dev_alloc(c.cur, &blob);
     if (rc) return rc;
@@ -895,6 +896,8 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     BfsCtrl* ctrl = (BfsCtrl*)(b + o_ctrl);
     CU(cudaMemsetAsync(ctrl, 0, sizeof(BfsCtrl), st));
     k_link_cost<<<(L + 255) / 256, 256, 0, st>>>(t->d_alpha, t->d_bpp, L, P.chunk_bytes, d_w);
+    uint4* d_oslot = (uint4*)(b + o_os);
+    k_bfs_pack<<<(L + 255) / 256, 256, 0, st>>>(pv.out_link, pv.edst, d_w, L, d_oslot);
     if (NS) {
         const size_t ds = (size_t)N * 8;
         if (ds > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ds));
@@ -923,7 +926,9 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bfs, (int)BFS_THREADS, smem));
     if (occ < 1) return PCCL_ERR_CUDA;
-    const uint32_t B = std::max(1u, std::min(std::min((uint32_t)occ, 4u) * (uint32_t)G.sm_count, nact));
+    uint32_t Bwant = (uint32_t)G.sm_count;   // one 1024-thread CTA per SM
+    if (const char* e = getenv("PCCL_BFS_WINDOW")) Bwant = std::min<uint32_t>((uint32_t)occ * (uint32_t)G.sm_count, std::max(1, atoi(e)));
+    const uint32_t B = std::max(1u, std::min(Bwant, nact));
 
     // ---- record capacity: a tree has at most N - 1 transfers; retried with the exact count if short ----
     uint64_t cap = 0;
@@ -948,7 +953,7 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         BfsArgs a;
         a.N = N; a.L = L; a.R = R; a.B = B; a.link_bits = link_bits; a.nact = nact;
         a.max_deg = std::max(1u, ph.transposed ? t->max_in : t->max_out);
-        a.out_off = ph.transposed ? t->d_in_off : t->d_out_off; a.out_link = pv.out_link;
+        a.out_off = ph.transposed ? t->d_in_off : t->d_out_off; a.oslot = d_oslot;
         a.esrc = pv.esrc; a.edst = pv.edst; a.psrc = t->d_src; a.pdst = t->d_dst; a.w = d_w;
         a.cond_src = ph.d_cond_src; a.dest_off = ph.d_dest_off; a.dests = ph.d_dests; a.order = d_order;
         a.runs = (ulonglong2*)(q + o_runs); a.rl_n = (uint32_t*)(q + o_rn); a.rl_start = (uint64_t*)(q + o_rs);
@@ -974,8 +979,10 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
             continue;
         }
         if (getenv("PCCL_BFS_DEBUG"))
-            fprintf(stderr, "[pccl bfs] rounds %llu searches %llu iters %llu relax %llu  search %.2f ms check %.2f ms commit %.2f ms  R %u B %u\n",
-                    mb->rounds, mb->searches, mb->iters, mb->relax, mb->ns_search * 1e-6, mb->ns_check * 1e-6, mb->ns_commit * 1e-6, R, B);
+            fprintf(stderr, "[pccl bfs] rounds %llu searches %llu sweeps %llu relax %llu | CTA 0: search %.2f ms check %.2f ms commit %.2f ms | "
+                            "per search: sweeps %.2f us filter %.2f us | R %u B %u\n",
+                    mb->rounds, mb->searches, mb->iters, mb->relax, mb->ns_search * 1e-6, mb->ns_check * 1e-6, mb->ns_commit * 1e-6,
+                    mb->searches ? mb->ns_sweeps * 1e-3 / mb->searches : 0.0, mb->searches ? mb->ns_filter * 1e-3 / mb->searches : 0.0, R, B);
         const uint64_t M = mb->nrec;
         res->M = M; res->tmax = mb->tmax; res->conditions = nact; res->searches = mb->searches; res->relax = mb->relax;
         res->rounds = mb->rounds; res->grid = B;

@@ -43,13 +43,15 @@ struct BfsCtrl {
     unsigned long long tmax;           // max t_end (without the phase offset)
     unsigned long long searches, relax, rounds;
     unsigned long long ns_search, ns_check, ns_commit, iters;   // phase times seen by CTA 0 (barrier waits included)
+    unsigned long long ns_sweeps, ns_filter;                    // summed over all searches: the sweeps, the path filter
     uint32_t nact;                     // conditions with at least one dest
     uint32_t err;                      // 1 unreachable, 2 time bits, 4 run row full, 8 record buffer full, 16 internal
 };
 
 struct BfsArgs {
     uint32_t N, L, R, B, link_bits, nact, max_deg;
-    const uint32_t *out_off, *out_link;   // out-links per device in the direction being synthesized
+    const uint32_t* out_off;              // [N + 1] out-links per device in the direction being synthesized
+    const uint4* oslot;                   // [L] per out-link entry: {link, far end, w lo, w hi}
     const uint32_t *esrc, *edst, *psrc, *pdst;
     const uint64_t* w;
     const uint32_t* cond_src;
@@ -67,7 +69,7 @@ struct BfsArgs {
     BfsCtrl* ctrl;
 };
 
-constexpr uint32_t BFS_THREADS = 256;
+constexpr uint32_t BFS_THREADS = 1024;
 constexpr unsigned long long BFS_INF = ~0ull;
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
@@ -107,6 +109,15 @@ __global__ void k_bfs_keys2(const uint64_t* __restrict__ cdist, const uint32_t* 
     val[i] = c;
 }
 
+__global__ void k_bfs_pack(const uint32_t* __restrict__ out_link, const uint32_t* __restrict__ edst,
+                           const uint64_t* __restrict__ w, uint32_t L, uint4* __restrict__ oslot) {
+    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= L) return;
+    const uint32_t l = out_link[e];
+    const uint64_t wl = w[l];
+    oslot[e] = make_uint4(l, edst[l], (uint32_t)wl, (uint32_t)(wl >> 32));
+}
+
 __global__ void k_bfs_init(BfsArgs a) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < a.L) {
@@ -116,7 +127,7 @@ __global__ void k_bfs_init(BfsArgs a) {
     if (i == 0) {
         a.ctrl->first_bad[0] = BFS_INF; a.ctrl->first_bad[1] = BFS_INF;
         a.ctrl->nrec = 0; a.ctrl->tmax = 0; a.ctrl->searches = 0; a.ctrl->relax = 0; a.ctrl->rounds = 0;
-        a.ctrl->ns_search = 0; a.ctrl->ns_check = 0; a.ctrl->ns_commit = 0; a.ctrl->iters = 0;
+        a.ctrl->ns_search = 0; a.ctrl->ns_check = 0; a.ctrl->ns_commit = 0; a.ctrl->iters = 0; a.ctrl->ns_sweeps = 0; a.ctrl->ns_filter = 0;
     }
 }
 
@@ -137,7 +148,7 @@ __device__ __forceinline__ uint64_t bfs_depart(const ulonglong2* __restrict__ ro
         uint32_t lo = 4, hi = n + 1;                   // the answer is in [lo, hi]; hi = n + 1: no such run
         const uint32_t stride = (n - 3 + 7) / 8;
         if (stride <= 8) {
-            ulonglong2 smp[7];
+            ulonglong2 smp[7], rhi = make_ulonglong2(0ull, 0ull);
 #pragma unroll
             for (int k = 0; k < 7; ++k) {
                 const uint32_t j = 3 + (k + 1) * stride;
@@ -146,18 +157,18 @@ __device__ __forceinline__ uint64_t bfs_depart(const ulonglong2* __restrict__ ro
 #pragma unroll
             for (int k = 6; k >= 0; --k) {
                 const uint32_t j = 3 + (k + 1) * stride;
-                if (j <= n) { if (smp[k].y > a) hi = j; else lo = max(lo, j + 1); }
+                if (j <= n) { if (smp[k].y > a) { hi = j; rhi = smp[k]; } else lo = max(lo, j + 1); }
             }
             // hi = first sampled index whose run ends after a (or n + 1); lo = one past the last sampled one that does not
             ulonglong2 blk[8];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) blk[k] = (lo + k < hi && lo + k <= n) ? __ldcg(row + lo + k) : make_ulonglong2(0ull, BFS_INF);
-            uint32_t i = hi;
+            for (int k = 0; k < 8; ++k) blk[k] = (lo + k < hi && lo + k <= n) ? __ldcg(row + lo + k) : make_ulonglong2(0ull, 0ull);
+            bool found = hi <= n;
+            r = rhi;
 #pragma unroll
             for (int k = 7; k >= 0; --k)
-                if (lo + k < hi && lo + k <= n && blk[k].y > a) i = lo + k;
-            if (i > n) return a;
-            r = __ldcg(row + i);
+                if (blk[k].y > a) { r = blk[k]; found = true; }
+            if (!found) return a;
         } else {
             while (lo < hi) {
                 const uint32_t mid = (lo + hi) >> 1;
@@ -210,6 +221,7 @@ struct BfsShared {
 };
 
 __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long* key, uint32_t* stamp, uint32_t* fr0, uint32_t* fr1,
+                           const uint32_t* s_off,
                            BfsShared& sh, uint32_t slot, uint32_t& ntr, uint64_t& relax) {
     const uint32_t tid = threadIdx.x, lb = a.link_bits;
     const uint64_t lmask = (1ull << lb) - 1;
@@ -217,6 +229,8 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
     const uint64_t d0 = a.dest_off[chunk];
     const uint32_t nd = (uint32_t)(a.dest_off[chunk + 1] - d0);
     const uint32_t MD = a.max_deg;
+    unsigned long long dbg0 = 0, dbg1 = 0;
+    if (tid == 0) dbg0 = globaltimer_ns();
     for (uint32_t v = tid; v < a.N; v += BFS_THREADS) { key[v] = BFS_INF; stamp[v] = NONE32; }
     if (tid == 0) { sh.nf[0] = 1; sh.nf[1] = 0; sh.nf[2] = 0; fr0[0] = src; }
     __syncthreads();
@@ -248,14 +262,14 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
         uint32_t* nfn = &sh.nf[(it + 1) % 3];
         for (uint32_t i = tid; i < nf * MD; i += BFS_THREADS) {
             const uint32_t u = cur[i / MD], k = i % MD;
-            const uint32_t o0 = a.out_off[u];
-            if (k >= a.out_off[u + 1] - o0) continue;
-            const uint32_t l = a.out_link[o0 + k];
-            const uint32_t v = a.edst[l];
-            if (v == src) continue;
+            const uint32_t o0 = s_off[u];
+            if (k >= s_off[u + 1] - o0) continue;
             const unsigned long long au = ((volatile unsigned long long*)key)[u] >> lb;
             if (au > bound) continue;
-            const uint64_t wl = a.w[l];
+            const uint4 os = a.oslot[o0 + k];
+            const uint32_t l = os.x, v = os.y;
+            if (v == src) continue;
+            const uint64_t wl = ((uint64_t)os.w << 32) | os.z;
             const uint64_t cand = bfs_depart(a.runs + (size_t)l * a.R, au, wl) + wl;
             ++relax;
             if (cand >> (64 - lb)) { atomicOr(&a.ctrl->err, 2u); continue; }
@@ -267,6 +281,7 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
         }
         __syncthreads();
     }
+    if (tid == 0) dbg1 = globaltimer_ns();
     uint32_t* keep = fr0;                               // the frontier lists are dead now
     for (uint32_t v = tid; v < a.N; v += BFS_THREADS) keep[v] = 0;
     __syncthreads();
@@ -293,6 +308,7 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
     }
     __syncthreads();
     ntr = sh.cnt;
+    if (tid == 0) { const unsigned long long dbg2 = globaltimer_ns(); atomicAdd(&a.ctrl->ns_sweeps, dbg1 - dbg0); atomicAdd(&a.ctrl->ns_filter, dbg2 - dbg1); }
 }
 
 __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
@@ -302,6 +318,7 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
     uint32_t* stamp = (uint32_t*)(key + a.N);                   // [N]
     uint32_t* fr0 = stamp + a.N;                                // [N] frontier lists; fr0 doubles as the keep marks
     uint32_t* fr1 = fr0 + a.N;                                  // [N]
+    uint32_t* s_off = fr1 + a.N;                                // [N + 1] copy of out_off
     __shared__ BfsShared sh;
     const uint32_t tid = threadIdx.x, slot = blockIdx.x, B = a.B;
     const uint32_t gtid = blockIdx.x * BFS_THREADS + tid, gthreads = gridDim.x * BFS_THREADS;
@@ -309,6 +326,8 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
     uint64_t* ts = a.tr_start + (size_t)slot * a.N;
     uint64_t base = 0, relax = 0, searches = 0;
     uint32_t pos = NONE32, ntr = 0;   // the result this CTA holds (CTA-uniform)
+    for (uint32_t v = tid; v <= a.N; v += BFS_THREADS) s_off[v] = a.out_off[v];
+    __syncthreads();
     bool valid = false;
     for (uint32_t round = 0; base < a.nact; ++round) {
         // ---- S: search + post ---------------------------------------------------------------
@@ -319,7 +338,7 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
         const uint32_t p = (uint32_t)p64;
         if (active) {
             if (!(valid && pos == p)) {
-                bfs_search(a, a.order[p], key, stamp, fr0, fr1, sh, slot, ntr, relax);
+                bfs_search(a, a.order[p], key, stamp, fr0, fr1, s_off, sh, slot, ntr, relax);
                 pos = p; valid = true; ++searches;
             }
             for (uint32_t i = tid; i < ntr; i += BFS_THREADS) {

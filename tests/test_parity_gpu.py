@@ -439,6 +439,18 @@ def test_bfs_mode_ring3000(pk):
     checker.check_structure(p, s.transfers)
 
 
+@pytest.mark.slow
+def test_bfs_mode_config4_full_size(pk):
+    """BASELINE.json configs[3] at full size through the paper's synthesizer: 261,632 conditions, 1.66 M
+    transfers (more than the 1,572,864 of minimal routing: detours through idle links)."""
+    p = wl.config4(0)
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_BFS)
+    assert_same(p, s, o)
+    assert s.size >= 1_572_864
+    checker.check_structure(p, s.transfers)
+
+
 # ------------------------------------------------------------------------------ randomized problems
 def _random_problem(i):
     """seeded random directed multigraph with heterogeneous links, a random process group and a random
@@ -486,11 +498,11 @@ def _random_problem(i):
 
 @pytest.mark.parametrize("block", range(6))
 def test_randomized_problems_all_modes(pk, block):
-    """120 random problems: each must give the oracle's schedule (or the oracle's error) under both relay rules;
-    every sixth also under the recount modes and the two-barrier loop."""
+    """120 random problems: each must give the oracle's schedule (or the oracle's error) under both relay rules
+    and under the paper's BFS synthesizer; every sixth also under the recount modes and the two-barrier loop."""
     for i in range(block * 20, block * 20 + 20):
         p = _random_problem(i)
-        for relay, rflag in ((0, 0), (1, pk.PCCL_FLAG_DYNAMIC_RELAY)):
+        for relay, rflag in ((0, 0), (1, pk.PCCL_FLAG_DYNAMIC_RELAY), (2, pk.PCCL_FLAG_BFS)):
             try:
                 o = oracle.synthesize(*p.args(), relay=relay)
             except oracle.OracleError as e:
@@ -501,7 +513,7 @@ def test_randomized_problems_all_modes(pk, block):
                                         oracle.ERR_INVALID: pk.PCCL_ERR_INVALID}[e.code], p.name
                 continue
             assert_same(p, gpu_run(pk, p, rflag | pk.PCCL_FLAG_KEEP_ON_DEVICE), o)
-            if i % 6 == 0:
+            if i % 6 == 0 and relay != 2:
                 for fl in (pk.PCCL_FLAG_TWO_BARRIERS, pk.PCCL_FLAG_RESCAN, pk.PCCL_FLAG_DENSE_SWEEP):
                     assert_same(p, gpu_run(pk, p, rflag | fl), o)
             if relay == 0:
