@@ -371,6 +371,29 @@ def run_ours(args):
                    "schedule_time_vs_thin_tree": dT / T if T else None,
                    "initial_wants": dst["wants_total"]}
 
+    # ---- the paper's own per-condition synthesizer (PCCL_FLAG_BFS; Q19-Q22) on the same problem
+    bfs = None
+    if not args.no_other_configs:
+        ms_b = []
+        for i in range(3):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            sb = prob.synthesize(seed, flags | pk.PCCL_FLAG_BFS)
+            e1.record()
+            e1.synchronize()
+            if i >= 1:
+                ms_b.append(e0.elapsed_time(e1))
+            bM, bT, bst = sb.size, sb.time_ps, sb.stats
+            sb.close()
+        bms = sum(ms_b) / len(ms_b)
+        bfs = {"synthesis_ms": bms, "loop_ms": bst["loop_ms"], "conditions": bst["events"], "transfers": bM,
+               "conditions_per_s": bst["events"] / (bms * 1e-3), "searches": bst["rows_scanned"],
+               "link_relaxations": bst["links_scanned"], "commit_rounds": bst["slow_picks"], "window": bst["grid_blocks"],
+               "schedule_time_ps": bT, "schedule_time_vs_matching": bT / T if T else None,
+               "schedule_time_over_lower_bound": (bT / lower_bound_ps(p)) if lower_bound_ps(p) else None,
+               "bound": "latency: ~10 dependent sweeps per search, one L2 round trip or more each; see DESIGN.md"}
+
     # ---- the other BASELINE.json configs, same path, resident inputs (context; parity is in tests/) ---
     per_config = {}
     if not args.no_other_configs:
@@ -438,7 +461,7 @@ def run_ours(args):
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": 1e3 * e2e_tot / args.steps},
             "gpu_launches": KERNELS_PER_STEP_COPY * args.steps,
-            "roofline": roofline, "cpu_baseline": cpu, "clocks": clk.summary(), "per_config": per_config, "dynamic_relay": dynamic,
+            "roofline": roofline, "cpu_baseline": cpu, "clocks": clk.summary(), "per_config": per_config, "dynamic_relay": dynamic, "paper_bfs": bfs,
             "paper_context": "PCCL reports 11.68 min for 512-NPU All-to-All synthesis, hardware not stated "
                              "(PAPER.md:9, :388); a different procedure, context only",
             "wall_s_timed_region": wall}

@@ -936,7 +936,7 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         const uint64_t nd = ph.dest_off[ci + 1] - ph.dest_off[ci];
         cap += std::min<uint64_t>((uint64_t)N - 1, nd * 16);
     }
-    uint32_t R = 64;
+    uint32_t R = 256;   // 4 KB per link
     for (int attempt = 0; attempt < 8; ++attempt) {
         Carver w2;
         const size_t o_runs = w2.take((size_t)L * R * 16), o_rn = w2.take((size_t)L * 4), o_rs = w2.take((size_t)L * B * 8),
@@ -952,7 +952,11 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         unsigned char* q = (unsigned char*)ws;
         BfsArgs a;
         a.N = N; a.L = L; a.R = R; a.B = B; a.link_bits = link_bits; a.nact = nact;
-        a.max_deg = std::max(1u, ph.transposed ? t->max_in : t->max_out);
+        {
+            const uint32_t md = std::max(1u, ph.transposed ? t->max_in : t->max_out);
+            a.deg_shift = 0;
+            while ((1u << a.deg_shift) < md && a.deg_shift < 5) ++a.deg_shift;
+        }
         a.out_off = ph.transposed ? t->d_in_off : t->d_out_off; a.oslot = d_oslot;
         a.esrc = pv.esrc; a.edst = pv.edst; a.psrc = t->d_src; a.pdst = t->d_dst; a.w = d_w;
         a.cond_src = ph.d_cond_src; a.dest_off = ph.d_dest_off; a.dests = ph.d_dests; a.order = d_order;
