@@ -142,8 +142,13 @@ def use_torch(device: int | None = None) -> None:
         except Exception:
             return None
 
+    _delete = torch.cuda.caching_allocator_delete
+
     def _free(ptr, _user):
-        torch.cuda.caching_allocator_delete(int(ptr))
+        try:
+            _delete(int(ptr))
+        except Exception:   # interpreter shutdown: torch is already torn down, the context goes with the process
+            pass
 
     _hooks = (pccl_alloc_fn(_alloc), pccl_free_fn(_free))
     lib.pccl_set_allocator(_hooks[0], _hooks[1], None)

@@ -869,8 +869,10 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     if (L == 0) return PCCL_ERR_UNREACHABLE;
     uint32_t link_bits = 1;
     while ((1ull << link_bits) < (uint64_t)L) ++link_bits;
-    const size_t smem = (size_t)N * 20 + ((size_t)N + 1) * 4;
-    if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+    const size_t smem_base = align_up((size_t)N * 20 + ((size_t)N + 1) * 4, 16);
+    if (smem_base > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+    const bool os_in_smem = (size_t)L * 16 <= 64 * 1024 && smem_base + (size_t)L * 16 <= 200 * 1024;
+    const size_t smem = smem_base + (os_in_smem ? (size_t)L * 16 : 0);
 
     // ---- order (Alg. 3 lines 1-7) ----
     t_setup.start();
@@ -934,9 +936,10 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     uint64_t cap = 0;
     for (uint32_t ci = 0; ci < C; ++ci) {
         const uint64_t nd = ph.dest_off[ci + 1] - ph.dest_off[ci];
-        cap += std::min<uint64_t>((uint64_t)N - 1, nd * 16);
+        cap += std::min<uint64_t>((uint64_t)N - 1, nd * 32);
     }
-    uint32_t R = 256;   // 4 KB per link
+    uint32_t R = 256;   // busy runs per link row (4 KB); a full row makes the kernel stop and the phase is rerun with 4 R
+    if (const char* e = getenv("PCCL_BFS_ROWS")) R = (uint32_t)std::max(8, atoi(e));   // (tests: force the rerun)
     for (int attempt = 0; attempt < 8; ++attempt) {
         Carver w2;
         const size_t o_runs = w2.take((size_t)L * R * 16), o_rn = w2.take((size_t)L * 4), o_rs = w2.take((size_t)L * B * 8),
@@ -952,6 +955,7 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         unsigned char* q = (unsigned char*)ws;
         BfsArgs a;
         a.N = N; a.L = L; a.R = R; a.B = B; a.link_bits = link_bits; a.nact = nact;
+        a.os_in_smem = os_in_smem ? 1u : 0u; a.os_smem_off8 = (uint32_t)(smem_base / 8);
         {
             const uint32_t md = std::max(1u, ph.transposed ? t->max_in : t->max_out);
             a.deg_shift = 0;

@@ -49,6 +49,7 @@ struct BfsCtrl {
 };
 
 struct BfsArgs {
+    uint32_t os_in_smem, os_smem_off8;   // oslot copied to shared memory at this offset (in 8-byte words)
     uint32_t N, L, R, B, link_bits, nact, deg_shift;   // deg_shift: log2 of the lanes per frontier device
     const uint32_t* out_off;              // [N + 1] out-links per device in the direction being synthesized
     const uint4* oslot;                   // [L] per out-link entry: {link, far end, w lo, w hi}
@@ -208,7 +209,7 @@ struct BfsShared {
 };
 
 __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long* key, uint32_t* stamp, uint32_t* fr0, uint32_t* fr1,
-                           const uint32_t* s_off,
+                           const uint32_t* s_off, const uint4* s_os,
                            BfsShared& sh, uint32_t slot, uint32_t& ntr, uint64_t& relax) {
     const uint32_t tid = threadIdx.x, lb = a.link_bits;
     const uint64_t lmask = (1ull << lb) - 1;
@@ -254,7 +255,7 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
             const unsigned long long au = ((volatile unsigned long long*)key)[u] >> lb;
             if (au > bound) continue;
             for (uint32_t k = tid & ((1u << mds) - 1); k < deg; k += 1u << mds) {
-                const uint4 os = a.oslot[o0 + k];
+                const uint4 os = s_os ? s_os[o0 + k] : a.oslot[o0 + k];
                 const uint32_t l = os.x, v = os.y;
                 if (v == src) continue;
                 const uint64_t wl = ((uint64_t)os.w << 32) | os.z;
@@ -262,6 +263,7 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
                 ++relax;
                 if (cand >> (64 - lb)) { atomicOr(&a.ctrl->err, 2u); continue; }
                 const unsigned long long kc = (cand << lb) | l;
+                if (kc >= ((volatile unsigned long long*)key)[v]) continue;
                 const unsigned long long old = atomicMin(&key[v], kc);
                 if (kc < old && cand < (old >> lb)) {   // arrival improved: v is in the next frontier (once)
                     if (atomicExch(&stamp[v], it) != it) nxt[atomicAdd(nfn, 1u)] = v;
@@ -308,6 +310,7 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
     uint32_t* fr0 = stamp + a.N;                                // [N] frontier lists; fr0 doubles as the keep marks
     uint32_t* fr1 = fr0 + a.N;                                  // [N]
     uint32_t* s_off = fr1 + a.N;                                // [N + 1] copy of out_off
+    uint4* s_os = a.os_in_smem ? (uint4*)(bfs_smem + a.os_smem_off8) : nullptr;   // [L] copy of oslot when it fits
     __shared__ BfsShared sh;
     const uint32_t tid = threadIdx.x, slot = blockIdx.x, B = a.B;
     const uint32_t gtid = blockIdx.x * BFS_THREADS + tid, gthreads = gridDim.x * BFS_THREADS;
@@ -316,6 +319,7 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
     uint64_t base = 0, relax = 0, searches = 0;
     uint32_t pos = NONE32, ntr = 0;   // the result this CTA holds (CTA-uniform)
     for (uint32_t v = tid; v <= a.N; v += BFS_THREADS) s_off[v] = a.out_off[v];
+    if (s_os) for (uint32_t e = tid; e < a.L; e += BFS_THREADS) s_os[e] = a.oslot[e];
     __syncthreads();
     bool valid = false;
     for (uint32_t round = 0; base < a.nact; ++round) {
@@ -327,7 +331,7 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
         const uint32_t p = (uint32_t)p64;
         if (active) {
             if (!(valid && pos == p)) {
-                bfs_search(a, a.order[p], key, stamp, fr0, fr1, s_off, sh, slot, ntr, relax);
+                bfs_search(a, a.order[p], key, stamp, fr0, fr1, s_off, s_os, sh, slot, ntr, relax);
                 pos = p; valid = true; ++searches;
             }
             for (uint32_t i = tid; i < ntr; i += BFS_THREADS) {
@@ -341,8 +345,10 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
         unsigned long long tq1 = 0;
         if (gtid == 0) tq1 = globaltimer_ns();
         // ---- C: lowest earlier position whose transfer overlaps one of mine --------------------
-        if (tid == 0) { sh.minconf = NONE32; sh.tmax = 0; }
+        // (err is only written before the barrier above or after the next one: every CTA reads the same value)
+        if (tid == 0) { sh.minconf = NONE32; sh.tmax = 0; sh.cnt = ldcg32(&a.ctrl->err) & (2u | 4u | 16u); }
         __syncthreads();
+        if (sh.cnt) break;   // a run row overflowed or an invariant broke: the host retries or reports
         if (active) {
             uint32_t mc = NONE32;
             for (uint32_t i = tid; i < ntr; i += BFS_THREADS) {

@@ -431,6 +431,16 @@ def test_bfs_mode_many_conditions_per_link(pk):
     assert_same(p, s, o)
 
 
+def test_bfs_mode_reruns_when_a_busy_run_row_fills(pk, monkeypatch):
+    """rows of 8 entries overflow at once on the 8-node ring with 130 chunks per node (gaps open and close on
+    every link): the kernel stops at the next round, the phase is rerun with longer rows, same schedule"""
+    p = wl.config5_small(1)
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS)
+    monkeypatch.setenv("PCCL_BFS_ROWS", "8")
+    s = gpu_run(pk, p, pk.PCCL_FLAG_BFS)
+    assert_same(p, s, o)
+
+
 def test_bfs_mode_ring3000(pk):
     p = _ring3000_a2a(3)
     o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS)
