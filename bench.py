@@ -500,8 +500,19 @@ def run_fig12(args):
                     ms.append(e0.elapsed_time(e1))
                 m, t, ev = s.size, s.time_ps, s.stats["events"]
                 s.close()
+            msb = []
+            for i in range(2):   # the paper's own procedure (PCCL_FLAG_BFS) on the same problem
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                sb = prob.synthesize(0, pk.PCCL_FLAG_KEEP_ON_DEVICE | pk.PCCL_FLAG_BFS)
+                e1.record()
+                e1.synchronize()
+                msb.append(e0.elapsed_time(e1))
+                mb, tb, rb = sb.size, sb.time_ps, sb.stats["slow_picks"]
+                sb.close()
             rows.append({"topology": name, "chunks_per_pair": k, "mib_per_npu": k * 64 * 128 // 1024, "chunks": nc,
-                         "transfers": m, "events": ev, "synthesis_ms": sorted(ms)[1], "schedule_time_ps": t})
+                         "transfers": m, "events": ev, "synthesis_ms": sorted(ms)[1], "schedule_time_ps": t,
+                         "bfs_synthesis_ms": min(msb), "bfs_transfers": mb, "bfs_rounds": rb, "bfs_schedule_time_ps": tb})
             prob.close()
         topo.close()
     print(json.dumps({"experiment": "fig12-shaped chunks-per-NPU sweep (context)", "rows": rows}), flush=True)

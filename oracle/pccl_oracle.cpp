@@ -27,6 +27,12 @@
 //  it is pinned only by the Philox known-answer vectors, by brute-force enumeration of
 //  the k-th candidate in tests, and by the closed forms / invariants that any valid pick
 //  must satisfy.
+//
+//  synth_copy_bfs (relay mode 2) is the paper's OWN synthesizer (Alg. 1-3 + section 4.6), kept
+//  beside the matching procedure: readings Q19-Q22; the paper prints no values for its worked
+//  example (Fig. 6/7 are images), so it is "parity unpinned" by the paper and pinned by a
+//  literal boolean-TEN brute force, a hand-worked example and closed forms in
+//  tests/test_oracle_bfs.py.
 // =====================================================================================
 #include <algorithm>
 #include <cstdint>

@@ -938,7 +938,10 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         const uint64_t nd = ph.dest_off[ci + 1] - ph.dest_off[ci];
         cap += std::min<uint64_t>((uint64_t)N - 1, nd * 32);
     }
-    uint32_t R = 256;   // busy runs per link row (4 KB); a full row makes the kernel stop and the phase is rerun with 4 R
+    // busy runs per link row: 256 (4 KB), more when many conditions share few links (<= 4096 and <= 1 GB in all);
+    // a full row makes the kernel stop and the phase is rerun with 4 R
+    uint32_t R = 256;
+    while (R < 4096 && R < nact / std::max(L, 1u) && (size_t)L * (R * 2) * 16 <= ((size_t)1 << 30)) R *= 2;
     if (const char* e = getenv("PCCL_BFS_ROWS")) R = (uint32_t)std::max(8, atoi(e));   // (tests: force the rerun)
     for (int attempt = 0; attempt < 8; ++attempt) {
         Carver w2;
