@@ -871,8 +871,9 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     while ((1ull << link_bits) < (uint64_t)L) ++link_bits;
     const size_t smem_base = align_up((size_t)N * 20 + ((size_t)N + 1) * 4, 16);
     if (smem_base > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
-    const bool os_in_smem = (size_t)L * 16 <= 64 * 1024 && smem_base + (size_t)L * 16 <= 200 * 1024;
-    const size_t smem = smem_base + (os_in_smem ? (size_t)L * 16 : 0);
+    // the out-link table and entry 0 of every busy-run row live in shared memory when they fit (32 bytes per link)
+    const bool os_in_smem = smem_base + (size_t)L * 32 <= 200 * 1024;
+    const size_t smem = smem_base + (os_in_smem ? (size_t)L * 32 : 0);
 
     // ---- order (Alg. 3 lines 1-7) ----
     t_setup.start();

@@ -139,32 +139,24 @@ __global__ void k_bfs_init(BfsArgs a) {
 // decided by entry 0 alone, 21 % by the first three runs, the rest have 4.5 runs on average.  A lookup is a
 // scattered 16-byte load per lane and round, so it is written to need as few rounds as possible: entry 0, then
 // runs 1-3 together, then runs 4-7 together, then a binary search.
-__device__ __forceinline__ uint64_t bfs_depart(const ulonglong2* __restrict__ row, uint64_t a, uint64_t w) {
-    const ulonglong2 h = __ldcg(row);                  // x = count, y = end of the last run
-    if (a >= h.y) return a;                            // (covers the empty row: y = 0)
+__device__ __forceinline__ uint64_t bfs_depart(const ulonglong2* __restrict__ row, ulonglong2 h, uint64_t a, uint64_t w) {
+    if (a >= h.y) return a;                            // h = entry 0: x = count, y = end of the last run (0: empty row)
     const uint32_t n = (uint32_t)h.x;
-    ulonglong2 e[4];
+    ulonglong2 e[8];
 #pragma unroll
-    for (int k = 1; k <= 3; ++k) e[k] = __ldcg(row + k);
+    for (int k = 1; k <= 7; ++k) e[k] = __ldcg(row + k);   // the rest of the row's first 128-byte line, one round
     ulonglong2 r = make_ulonglong2(0ull, 0ull);
     bool found = false;
 #pragma unroll
-    for (int k = 3; k >= 1; --k)
+    for (int k = 7; k >= 1; --k)
         if ((uint32_t)k <= n && e[k].y > a) { r = e[k]; found = true; }
-    if (!found) {                                      // a < end of the last run, so some run in [4, n] ends after a
-#pragma unroll
-        for (int k = 0; k < 4; ++k) e[k] = __ldcg(row + 4 + k);
-#pragma unroll
-        for (int k = 3; k >= 0; --k)
-            if ((uint32_t)(4 + k) <= n && e[k].y > a) { r = e[k]; found = true; }
-        if (!found) {
-            uint32_t lo = 8, hi = n;
-            while (lo < hi) {
-                const uint32_t mid = (lo + hi) >> 1;
-                if (__ldcg(row + mid).y <= a) lo = mid + 1; else hi = mid;
-            }
-            r = __ldcg(row + lo);
+    if (!found) {                                      // a < end of the last run, so some run in [8, n] ends after a
+        uint32_t lo = 8, hi = n;
+        while (lo < hi) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (__ldcg(row + mid).y <= a) lo = mid + 1; else hi = mid;
         }
+        r = __ldcg(row + lo);
     }
     return (a + w <= r.x) ? a : r.y;
 }
@@ -209,7 +201,7 @@ struct BfsShared {
 };
 
 __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long* key, uint32_t* stamp, uint32_t* fr0, uint32_t* fr1,
-                           const uint32_t* s_off, const uint4* s_os,
+                           const uint32_t* s_off, const uint4* s_os, ulonglong2* s_hdr,
                            BfsShared& sh, uint32_t slot, uint32_t& ntr, uint64_t& relax) {
     const uint32_t tid = threadIdx.x, lb = a.link_bits;
     const uint64_t lmask = (1ull << lb) - 1;
@@ -220,35 +212,41 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
     unsigned long long dbg0 = 0, dbg1 = 0;
     if (tid == 0) dbg0 = globaltimer_ns();
     for (uint32_t v = tid; v < a.N; v += BFS_THREADS) { key[v] = BFS_INF; stamp[v] = NONE32; }
+    if (s_hdr) for (uint32_t l = tid; l < a.L; l += BFS_THREADS) s_hdr[l] = __ldcg(a.runs + (size_t)l * a.R);
     if (tid == 0) { sh.nf[0] = 1; sh.nf[1] = 0; sh.nf[2] = 0; fr0[0] = src; }
     __syncthreads();
     if (tid == 0) key[src] = 0;
     __syncthreads();
-    uint32_t dloc[8];                                   // up to 8 dests are followed by every thread itself
-#pragma unroll
-    for (int k = 0; k < 8; ++k) dloc[k] = (uint32_t)k < nd ? a.dests[d0 + k] : src;
+    // 32 warps run every sweep, most of them without a frontier device: what they execute between two block
+    // barriers is kept to a handful of instructions (the sweep is issue-bound otherwise)
+    const uint32_t d_first = a.dests[d0];
+    uint32_t r0 = 0, r1 = 1, r2 = 2;                    // ring positions of this, the next and the sweep after
     for (uint32_t it = 0;; ++it) {
-        const uint32_t nf = sh.nf[it % 3];
-        if (nf == 0) { if (tid == 0) atomicAdd(&a.ctrl->iters, (unsigned long long)it); break; }
-        if (it > a.N + 1) { if (tid == 0) atomicOr(&a.ctrl->err, 16u); break; }
-        unsigned long long bound = 0;
-        if (nd <= 8) {
-#pragma unroll
-            for (int k = 0; k < 8; ++k)
-                if ((uint32_t)k < nd) bound = max(bound, ((volatile unsigned long long*)key)[dloc[k]] >> lb);
-        } else {
+        const uint32_t nf = sh.nf[r0];
+        if (nf == 0 || it > a.N + 1) {
+            if (tid == 0) { atomicAdd(&a.ctrl->iters, (unsigned long long)it); if (nf) atomicOr(&a.ctrl->err, 16u); }
+            break;
+        }
+        if (nd > 8) {                                   // many dests: max of their arrivals, by the whole CTA
             if (tid == 0) sh.bound = 0;
             __syncthreads();
             unsigned long long bl = 0;
             for (uint32_t k = tid; k < nd; k += BFS_THREADS) bl = max(bl, key[a.dests[d0 + k]] >> lb);
             if (bl) atomicMax(&sh.bound, bl);
             __syncthreads();
-            bound = sh.bound;
         }
-        if (tid == 0) sh.nf[(it + 2) % 3] = 0;
+        if (tid == 0) sh.nf[r2] = 0;
         const uint32_t* cur = (it & 1) ? fr1 : fr0;
         uint32_t* nxt = (it & 1) ? fr0 : fr1;
-        uint32_t* nfn = &sh.nf[(it + 1) % 3];
+        uint32_t* nfn = &sh.nf[r1];
+        { const uint32_t t = r0; r0 = r1; r1 = r2; r2 = t; }
+        if (((tid & ~31u) >> mds) >= nf) { __syncthreads(); continue; }   // no frontier device for this whole warp
+        unsigned long long bound;
+        if (nd > 8) bound = sh.bound;
+        else {
+            bound = ((volatile unsigned long long*)key)[d_first] >> lb;
+            for (uint32_t k = 1; k < nd; ++k) bound = max(bound, ((volatile unsigned long long*)key)[a.dests[d0 + k]] >> lb);
+        }
         for (uint32_t j = tid >> mds; j < nf; j += BFS_THREADS >> mds) {     // 2^mds lanes per frontier device
             const uint32_t u = cur[j];
             const uint32_t o0 = s_off[u], deg = s_off[u + 1] - o0;
@@ -259,14 +257,20 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
                 const uint32_t l = os.x, v = os.y;
                 if (v == src) continue;
                 const uint64_t wl = ((uint64_t)os.w << 32) | os.z;
-                const uint64_t cand = bfs_depart(a.runs + (size_t)l * a.R, au, wl) + wl;
+                const ulonglong2* row = a.runs + (size_t)l * a.R;
+                const uint64_t cand = bfs_depart(row, s_hdr ? s_hdr[l] : __ldcg(row), au, wl) + wl;
                 ++relax;
                 if (cand >> (64 - lb)) { atomicOr(&a.ctrl->err, 2u); continue; }
                 const unsigned long long kc = (cand << lb) | l;
                 if (kc >= ((volatile unsigned long long*)key)[v]) continue;
                 const unsigned long long old = atomicMin(&key[v], kc);
                 if (kc < old && cand < (old >> lb)) {   // arrival improved: v is in the next frontier (once)
-                    if (atomicExch(&stamp[v], it) != it) nxt[atomicAdd(nfn, 1u)] = v;
+                    if (atomicExch(&stamp[v], it) != it) {
+                        cg::coalesced_group g = cg::coalesced_threads();         // one counter update per warp
+                        uint32_t b0 = 0;
+                        if (g.thread_rank() == 0) b0 = atomicAdd(nfn, g.size());
+                        nxt[g.shfl(b0, 0) + g.thread_rank()] = v;
+                    }
                 }
             }
         }
@@ -311,6 +315,7 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
     uint32_t* fr1 = fr0 + a.N;                                  // [N]
     uint32_t* s_off = fr1 + a.N;                                // [N + 1] copy of out_off
     uint4* s_os = a.os_in_smem ? (uint4*)(bfs_smem + a.os_smem_off8) : nullptr;   // [L] copy of oslot when it fits
+    ulonglong2* s_hdr = a.os_in_smem ? (ulonglong2*)(s_os + a.L) : nullptr;        // [L] entry 0 of every row, reloaded per search
     __shared__ BfsShared sh;
     const uint32_t tid = threadIdx.x, slot = blockIdx.x, B = a.B;
     const uint32_t gtid = blockIdx.x * BFS_THREADS + tid, gthreads = gridDim.x * BFS_THREADS;
@@ -331,7 +336,7 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
         const uint32_t p = (uint32_t)p64;
         if (active) {
             if (!(valid && pos == p)) {
-                bfs_search(a, a.order[p], key, stamp, fr0, fr1, s_off, s_os, sh, slot, ntr, relax);
+                bfs_search(a, a.order[p], key, stamp, fr0, fr1, s_off, s_os, s_hdr, sh, slot, ntr, relax);
                 pos = p; valid = true; ++searches;
             }
             for (uint32_t i = tid; i < ntr; i += BFS_THREADS) {
