@@ -188,7 +188,7 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
                                         rows_scanned = searches run (a condition is searched again when a condition
                                         ahead of it took an interval it used), links_scanned = link relaxations,
                                         slow_picks = commit rounds.  UNSUPPORTED if a time does not fit in
-                                        64 - ceil(log2(n_links)) bits or n_npus > 10,240. */
+                                        64 - ceil(log2(n_links)) bits or n_npus > 8,500. */
 
 /* Steps A..F on the GPU for one seed.  Errors: UNREACHABLE, CUDA, NOMEM, INTERNAL. */
 int pccl_problem_synthesize(pccl_problem_t* problem, uint64_t seed, uint32_t flags,

@@ -137,8 +137,9 @@ __global__ void k_bfs_init(BfsArgs a) {
 // in front of the first run that ends after a) or the end of that run.  Entry 0 of the row holds the run count
 // and the end of the last run.  Measured on config 4: 67 % of the lookups come after the last run and are
 // decided by entry 0 alone, 21 % by the first three runs, the rest have 4.5 runs on average.  A lookup is a
-// scattered 16-byte load per lane and round, so it is written to need as few rounds as possible: entry 0, then
-// runs 1-3 together, then runs 4-7 together, then a binary search.
+// scattered 16-byte load per lane and round, so it is written to need as few rounds as possible: entry 0 (the
+// caller passes it, from shared memory when the headers fit there), then runs 1-7 together (the rest of the
+// row's first 128-byte line), then a binary search.
 __device__ __forceinline__ uint64_t bfs_depart(const ulonglong2* __restrict__ row, ulonglong2 h, uint64_t a, uint64_t w) {
     if (a >= h.y) return a;                            // h = entry 0: x = count, y = end of the last run (0: empty row)
     const uint32_t n = (uint32_t)h.x;
