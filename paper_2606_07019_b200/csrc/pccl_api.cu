@@ -42,6 +42,10 @@ struct Globals {
     std::vector<Pinned> pinned_free;
     int sm_count = 0;
     int dev = -1;
+    // streaming the records out while the event loop runs: a copy stream of our own and the event the
+    // polling host thread watches
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t loop_done = nullptr;
 } G;
 
 #define CU(call)                                   \
@@ -88,6 +92,8 @@ int ensure_device() {
     void* mb = nullptr;
     CU(cudaHostAlloc(&mb, 4096, cudaHostAllocDefault));
     G.mailbox = mb;
+    CU(cudaStreamCreateWithFlags(&G.copy_stream, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&G.loop_done, cudaEventDisableTiming));
     G.sm_count = sms;
     G.dev = dev;
     return PCCL_OK;
@@ -127,6 +133,65 @@ void pinned_put(void* p, size_t bytes) {
     G.pinned_free.push_back({p, bytes});
 }
 
+// Host arrays of the normaliser: blocks of 64 KB and more come from a small process-wide cache (power-of-two
+// size classes) instead of a fresh mmap per call -- at config 4 the ~17 MB of per-call vectors cost more in page
+// faults than the grouping itself.  Smaller blocks go to malloc.
+struct HostPool {
+    static constexpr int MIN_LOG = 16, MAX_LOG = 34;
+    static constexpr size_t CACHE_CAP = (size_t)512 << 20;
+    std::mutex mu;
+    std::vector<void*> free_[MAX_LOG + 1];
+    size_t cached = 0;
+    static int size_class(size_t bytes) {
+        int k = MIN_LOG;
+        while (k < MAX_LOG && ((size_t)1 << k) < bytes) ++k;
+        return k;
+    }
+    void* get(size_t bytes) {
+        if (bytes < ((size_t)1 << MIN_LOG) || bytes > ((size_t)1 << MAX_LOG)) return malloc(bytes ? bytes : 1);
+        const int k = size_class(bytes);
+        {
+            std::lock_guard<std::mutex> lk(mu);
+            if (!free_[k].empty()) {
+                void* p = free_[k].back();
+                free_[k].pop_back();
+                cached -= (size_t)1 << k;
+                return p;
+            }
+        }
+        return malloc((size_t)1 << k);
+    }
+    void put(void* p, size_t bytes) {
+        if (!p) return;
+        if (bytes >= ((size_t)1 << MIN_LOG) && bytes <= ((size_t)1 << MAX_LOG)) {
+            const int k = size_class(bytes);
+            std::lock_guard<std::mutex> lk(mu);
+            if (cached + ((size_t)1 << k) <= CACHE_CAP) {
+                free_[k].push_back(p);
+                cached += (size_t)1 << k;
+                return;
+            }
+        }
+        free(p);
+    }
+} HP;
+
+template <class T>
+struct PoolAlloc {
+    using value_type = T;
+    PoolAlloc() = default;
+    template <class U> PoolAlloc(const PoolAlloc<U>&) {}
+    T* allocate(size_t n) {
+        void* p = HP.get(n * sizeof(T));
+        if (!p) throw std::bad_alloc();
+        return (T*)p;
+    }
+    void deallocate(T* p, size_t n) { HP.put(p, n * sizeof(T)); }
+    template <class U> bool operator==(const PoolAlloc<U>&) const { return true; }
+    template <class U> bool operator!=(const PoolAlloc<U>&) const { return false; }
+};
+template <class T> using hvec = std::vector<T, PoolAlloc<T>>;
+
 }  // namespace
 
 // -----------------------------------------------------------------------------------------
@@ -151,14 +216,14 @@ namespace {
 
 struct Phase {
     bool transposed = false;          // run on the reversed links (reductions, Q10)
-    std::vector<uint32_t> cond_src;   // [C] source (copy) or root (reduce) of each chunk
-    std::vector<uint64_t> dest_off;   // [C+1]
-    std::vector<uint32_t> dests;      // ascending per chunk
-    std::vector<uint32_t> dchunk;     // [n_dests] chunk of each (chunk, dest) pair
-    std::vector<uint32_t> sources;    // distinct sources, ascending
-    std::vector<uint32_t> sidx;       // [N] node -> row of D, NONE32 if not a source
-    std::vector<uint32_t> dsts;       // distinct dests, ascending (dynamic relay: rows of the to-dest distances)
-    std::vector<uint32_t> didx;       // [N] node -> row, NONE32 if not a dest
+    hvec<uint32_t> cond_src;   // [C] source (copy) or root (reduce) of each chunk
+    hvec<uint64_t> dest_off;   // [C+1]
+    hvec<uint32_t> dests;      // ascending per chunk
+    hvec<uint32_t> dchunk;     // [n_dests] chunk of each (chunk, dest) pair
+    hvec<uint32_t> sources;    // distinct sources, ascending
+    hvec<uint32_t> sidx;       // [N] node -> row of D, NONE32 if not a source
+    hvec<uint32_t> dsts;       // distinct dests, ascending (dynamic relay: rows of the to-dest distances)
+    hvec<uint32_t> didx;       // [N] node -> row, NONE32 if not a dest
     void* blob = nullptr;
     uint32_t *d_cond_src = nullptr, *d_dests = nullptr, *d_dchunk = nullptr, *d_sources = nullptr,
              *d_sidx = nullptr, *d_dsts = nullptr, *d_didx = nullptr;
@@ -326,7 +391,7 @@ int topo_upload(pccl_topology* t) {
 // ---------------------------------------------------------------------------------------
 // per-chunk ascending, duplicate-free NPU lists
 int group_pairs(const pccl_condition_t* cnd, uint32_t C, uint32_t N, const std::vector<char>& member,
-                std::vector<uint64_t>& off, std::vector<uint32_t>& npus) {
+                hvec<uint64_t>& off, hvec<uint32_t>& npus) {
     off.assign((size_t)C + 1, 0);
     npus.resize(cnd->n_pairs);
     bool ordered = true;   // chunk ids non-decreasing in the caller's array: the pairs are already grouped
@@ -343,7 +408,7 @@ int group_pairs(const pccl_condition_t* cnd, uint32_t C, uint32_t N, const std::
     uint64_t longest = 0;
     for (uint32_t c = 0; c < C; ++c) { longest = std::max(longest, off[c + 1]); off[c + 1] += off[c]; }
     if (!ordered) {
-        std::vector<uint64_t> cur(off.begin(), off.end() - 1);
+        hvec<uint64_t> cur(off.begin(), off.end() - 1);
         for (uint64_t i = 0; i < cnd->n_pairs; ++i) npus[cur[cnd->pairs[i].chunk]++] = cnd->pairs[i].npu;
     }
     if (longest <= 1) return PCCL_OK;   // every list has at most one holder: already sorted and duplicate-free
@@ -371,22 +436,26 @@ int group_pairs(const pccl_condition_t* cnd, uint32_t C, uint32_t N, const std::
     return PCCL_OK;
 }
 
+// distinct sources / dests (ascending) and their row indices, from per-node flags
+void index_phase(Phase& ph, uint32_t N, const std::vector<char>& is_src, const std::vector<char>& is_dst) {
+    ph.sidx.assign(N, NONE32);
+    for (uint32_t v = 0; v < N; ++v)
+        if (is_src[v]) { ph.sidx[v] = (uint32_t)ph.sources.size(); ph.sources.push_back(v); }
+    ph.didx.assign(N, NONE32);
+    for (uint32_t v = 0; v < N; ++v)
+        if (is_dst[v]) { ph.didx[v] = (uint32_t)ph.dsts.size(); ph.dsts.push_back(v); }
+}
+
 void finish_phase(Phase& ph, uint32_t N) {
     const uint32_t C = (uint32_t)ph.cond_src.size();
     ph.dchunk.resize(ph.dests.size());
-    std::vector<char> is_src(N, 0);
+    std::vector<char> is_src(N, 0), is_dst(N, 0);
     for (uint32_t c = 0; c < C; ++c) {
         for (uint64_t i = ph.dest_off[c]; i < ph.dest_off[c + 1]; ++i) ph.dchunk[i] = c;
         if (ph.dest_off[c + 1] > ph.dest_off[c]) is_src[ph.cond_src[c]] = 1;
     }
-    ph.sidx.assign(N, NONE32);
-    for (uint32_t v = 0; v < N; ++v)
-        if (is_src[v]) { ph.sidx[v] = (uint32_t)ph.sources.size(); ph.sources.push_back(v); }
-    std::vector<char> is_dst(N, 0);
     for (uint32_t d : ph.dests) is_dst[d] = 1;
-    ph.didx.assign(N, NONE32);
-    for (uint32_t v = 0; v < N; ++v)
-        if (is_dst[v]) { ph.didx[v] = (uint32_t)ph.dsts.size(); ph.dsts.push_back(v); }
+    index_phase(ph, N, is_src, is_dst);
 }
 
 int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_members,
@@ -401,8 +470,8 @@ int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_membe
         if (group[i] >= N || member[group[i]]) return PCCL_ERR_INVALID;
         member[group[i]] = 1;
     }
-    std::vector<uint64_t> pre_off, post_off;
-    std::vector<uint32_t> pre_n, post_n;
+    hvec<uint64_t> pre_off, post_off;
+    hvec<uint32_t> pre_n, post_n;
     // the two conditions are grouped independently: the postcondition on a second host thread when it is large
     int rc, rc2;
     if (post->n_pairs >= 65536) {
@@ -421,7 +490,17 @@ int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_membe
     }
     if (rc) return rc;
     if (rc2) return rc2;
+    // one pass classifies the call (Q12) and, as long as every chunk so far has a single pre-holder, already writes
+    // the COPY conditions -- the common large case (All-to-All(v), All-Gather) needs no second sweep
     bool all_single = true, all_multi_one = true, all_multi_many = true;
+    Phase cp;
+    cp.cond_src.resize(C);
+    cp.dest_off.resize((size_t)C + 1);
+    cp.dests.resize(post_n.size());
+    cp.dchunk.resize(post_n.size());
+    cp.dest_off[0] = 0;
+    std::vector<char> cp_src(N, 0), cp_dst(N, 0);
+    uint64_t nd = 0;
     for (uint32_t c = 0; c < C; ++c) {
         const uint64_t np = pre_off[c + 1] - pre_off[c], nq = post_off[c + 1] - post_off[c];
         if (np == 0 || nq == 0) return PCCL_ERR_INVALID;
@@ -429,6 +508,21 @@ int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_membe
         all_single &= single;
         all_multi_one &= (!single && nq == 1);
         all_multi_many &= (!single && nq > 1);
+        if (all_single) {
+            const uint32_t src = pre_n[pre_off[c]];
+            const uint64_t first = nd;
+            cp.cond_src[c] = src;
+            for (uint64_t i = post_off[c]; i < post_off[c + 1]; ++i) {
+                const uint32_t d = post_n[i];
+                if (d == src) continue;
+                cp.dests[nd] = d;
+                cp.dchunk[nd] = c;
+                cp_dst[d] = 1;
+                ++nd;
+            }
+            cp.dest_off[c + 1] = nd;
+            if (nd > first) cp_src[src] = 1;
+        }
     }
     P.topo = topo;
     P.C = C;
@@ -441,13 +535,11 @@ int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_membe
     };
     if (all_single) {   // COPY: the one pre-holder is the source
         P.mode = 0;
-        P.phases.resize(1);
-        Phase& ph = P.phases[0];
-        ph.cond_src.resize(C);
-        ph.dest_off.assign((size_t)C + 1, 0);
-        ph.dests.reserve(post_n.size());
-        for (uint32_t c = 0; c < C; ++c)
-            fill(ph, c, pre_n[pre_off[c]], post_n.data() + post_off[c], post_n.data() + post_off[c + 1]);
+        cp.dests.resize(nd);
+        cp.dchunk.resize(nd);
+        index_phase(cp, N, cp_src, cp_dst);
+        P.phases.push_back(std::move(cp));
+        return PCCL_OK;
     } else if (all_multi_one) {   // REDUCE: broadcast root -> holders on the transposed links
         P.mode = 1;
         P.phases.resize(1);
@@ -489,7 +581,15 @@ int phase_upload(Phase& ph, uint32_t N) {
     const size_t o_cs = c.take(C * 4), o_d = c.take(ND * 4), o_dc = c.take(ND * 4), o_s = c.take(NS * 4), o_si = c.take((size_t)N * 4);
     const size_t NDS = ph.dsts.size();
     const size_t o_do = c.take((C + 1) * 8), o_ds = c.take(NDS * 4), o_di = c.take((size_t)N * 4);
-    std::vector<unsigned char> h(c.cur ? c.cur : 256, 0);
+    // staged in pinned memory from the library's cache: the copy runs at full PCIe rate and no fresh pages are touched
+    struct Stage {
+        unsigned char* p; size_t bytes;
+        unsigned char* data() const { return p; }
+        size_t size() const { return bytes; }
+        ~Stage() { pinned_put(p, bytes); }
+    } h{nullptr, c.cur ? c.cur : 256};
+    h.p = (unsigned char*)pinned_get(h.bytes);
+    if (!h.p) return PCCL_ERR_NOMEM;
     memcpy(h.data() + o_do, ph.dest_off.data(), (C + 1) * 8);
     if (NDS) memcpy(h.data() + o_ds, ph.dsts.data(), NDS * 4);
     if (N) memcpy(h.data() + o_di, ph.didx.data(), (size_t)N * 4);
@@ -700,8 +800,11 @@ struct LoopResult {
 };
 
 // steps D..E: the event loop; records go to `out` (capacity M) in canonical order
+// host_out (optional, pinned, out_cap records): with the one-barrier loop the records are copied there while the
+// loop runs (the kernel publishes how many are final, this thread issues the copies); *streamed says whether
 int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint32_t flags, Rec* out,
-               uint64_t out_cap, uint64_t t_offset, LoopResult* res, std::vector<uint64_t>* trace = nullptr) {
+               uint64_t out_cap, uint64_t t_offset, LoopResult* res, std::vector<uint64_t>* trace = nullptr,
+               Rec* host_out = nullptr, bool* streamed = nullptr) {
     const bool dynamic = (flags & PCCL_FLAG_DYNAMIC_RELAY) != 0;
     // the dynamic rule's wants rows are dense and shrink by the thousand per event: keeping the counts current
     // costs more than recounting by whole rows, so that is its default (KEPT_COUNTS overrides)
@@ -764,13 +867,52 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     }
     a.st_free = fast ? W.st_free : nullptr;
     a.st_inf = fast ? W.st_inf : nullptr;
+    // the progress word lives in the second half of the pinned mailbox (mapped: the kernel stores to it directly)
+    static_assert(sizeof(LoopCtrl) <= 2048, "mailbox halves");
+    volatile unsigned long long* progress = (volatile unsigned long long*)((unsigned char*)G.mailbox + 2048);
+    const bool stream_out = fast && host_out != nullptr && out_cap > 0;
+    a.progress = nullptr;
+    if (stream_out) {
+        *progress = 0;
+        void* dp = nullptr;
+        CU(cudaHostGetDevicePointer(&dp, (void*)progress, 0));
+        a.progress = (unsigned long long*)dp;
+    }
     k_loop_init<<<(n_init + 255) / 256, 256, 0, st>>>(a);
     if (a.gcnt != nullptr && a.L) k_count_init<<<a.L, 256, 0, st>>>(a);
     void* args[] = {(void*)&a};
     CU(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(threads), args, smem, st));
     LoopCtrl* mb = (LoopCtrl*)G.mailbox;
     CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
+    if (stream_out) {
+        // copy finished records in pieces of >= 2 MB on the copy stream while the loop is still running; the tail
+        // follows once the loop is done.  The copy stream is drained before anything can fail or return.
+        constexpr uint64_t PIECE = 1u << 16;
+        uint64_t copied = 0;
+        cudaError_t e = cudaEventRecord(G.loop_done, st), q = cudaErrorNotReady;
+        while (e == cudaSuccess && (q = cudaEventQuery(G.loop_done)) == cudaErrorNotReady) {
+            const uint64_t p = std::min<uint64_t>(*progress, out_cap);
+            if (p >= copied + PIECE) {
+                e = cudaMemcpyAsync(host_out + copied, out + copied, (p - copied) * sizeof(Rec), cudaMemcpyDeviceToHost,
+                                    G.copy_stream);
+                copied = p;
+            }
+        }
+        if (e == cudaSuccess && q != cudaSuccess) e = q;
+        if (e == cudaSuccess && mb->err == 0 && mb->total <= out_cap && mb->total > copied)
+            e = cudaMemcpyAsync(host_out + copied, out + copied, (mb->total - copied) * sizeof(Rec), cudaMemcpyDeviceToHost,
+                                G.copy_stream);
+        const cudaError_t e2 = cudaStreamSynchronize(G.copy_stream);
+        if (e != cudaSuccess || e2 != cudaSuccess) {
+            (void)cudaGetLastError();
+            (void)cudaStreamSynchronize(st);
+            (void)cudaGetLastError();
+            return PCCL_ERR_CUDA;
+        }
+        if (streamed) *streamed = true;
+    } else {
+        CU(cudaStreamSynchronize(st));
+    }
     if (mb->err & 32u) return PCCL_ERR_NOMEM;   // more transfers than the record buffer holds
     if (mb->err) return PCCL_ERR_INTERNAL;
     res->total = mb->total; res->tmax = mb->tmax; res->events = mb->events;
@@ -1036,6 +1178,7 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
     auto fail = [&](int code) {
         dev_free(W.blob); dev_free(out_recs); dev_free(raw); dev_free(stage1);
         if (cudaStreamSynchronize(G.stream) != cudaSuccess) (void)cudaGetLastError();
+        pinned_put(S->h_recs, S->h_bytes);
         delete S;
         return code;
     };
@@ -1125,14 +1268,21 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
                     return fail(PCCL_ERR_CUDA);
                 }
             }
+            // a schedule that goes to the host anyway is streamed out while the loop runs (single copy phase)
+            bool streamed = false;
+            if (base == 0 && last && !dynamic && cap && !(flags & PCCL_FLAG_KEEP_ON_DEVICE)) {
+                S->h_bytes = cap * sizeof(Rec);
+                S->h_recs = pinned_get(S->h_bytes);   // null: no streaming, the download reports the failure
+            }
             t_loop.start();
-            rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, cap, toff, &lr, &S->trace);
+            rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, cap, toff, &lr, &S->trace, (Rec*)S->h_recs, &streamed);
             if (rc) return fail(rc);
             t_loop.stop();
             if (dynamic ? lr.total > M : lr.total != M) return fail(PCCL_ERR_INTERNAL);
             M = lr.total;
             S->M = base + M;
             S->T = toff + lr.tmax;
+            S->downloaded = streamed;
         }
         S->stats.events += lr.events;
         S->stats.rows_scanned += lr.rows;

@@ -328,6 +328,8 @@ struct LoopArgs {
     uint32_t* st_inf;
     uint64_t* trace;        // optional [events][TRACE_SLOTS] globaltimer stamps of CTA 0 (diagnostic), or null
     uint32_t trace_cap;     // events the trace buffer holds
+    unsigned long long* progress;   // optional word in mapped pinned HOST memory: records [0, *progress) of `out` are
+                                    // final (k_loop1 only; the host streams them out while the loop runs), or null
 };
 
 constexpr int TRACE_SLOTS = 12;  // 0 loop top, 1 links phase, 2 barrier 1, 3 in-link list, 4 count, 5 pick, 6 commit,
