@@ -173,10 +173,10 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
 #define PCCL_FLAG_DYNAMIC_RELAY 64u  /* relay rule of DESIGN.md Q18 instead of the static thin relay tree: a node
                                         takes a chunk iff it is strictly closer to some destination than the
                                         source and every node that claimed the chunk at an earlier event (fewer
-                                        link-times, a few unused deliveries; dense recount unless KEPT_COUNTS
-                                        or RESCAN is given) */
-#define PCCL_FLAG_KEPT_COUNTS 128u   /* with DYNAMIC_RELAY: keep the candidate counts current (the default of
-                                        the thin-tree rule) instead of its dense recount */
+                                        link-times, a few unused deliveries; kept counts with per-chunk holder
+                                        lists unless DENSE_SWEEP or RESCAN is given) */
+#define PCCL_FLAG_KEPT_COUNTS 128u   /* with DYNAMIC_RELAY: keep the candidate counts current (its default; the
+                                        flag is accepted for compatibility) */
 #define PCCL_FLAG_TWO_BARRIERS 256u  /* run the two-barrier event loop even where the one-barrier loop applies */
 #define PCCL_FLAG_BFS 512u           /* the paper's own synthesizer instead of the matching loop (Alg. 1-3,
                                         :332-344 section 4.6; Q19-Q22): conditions in descending c.dist

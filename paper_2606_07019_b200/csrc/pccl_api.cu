@@ -679,6 +679,7 @@ struct Work {   // device workspace of one phase
     uint64_t *hsum = nullptr, *wsum = nullptr;
     uint32_t *gcnt = nullptr, *gtot = nullptr;
     uint64_t* best = nullptr;
+    uint32_t *hold_cnt = nullptr, *hold = nullptr;   // dynamic rule with kept counts: holders of each chunk
     uint64_t* st_free = nullptr;
     uint32_t* st_inf = nullptr;
     uint32_t Wp = 0, S = 0, nLw = 0, SWp = 0;
@@ -707,10 +708,10 @@ int work_alloc(const pccl_problem& P, Work& W) {
     const size_t o_best = c.take(max_pairs * 8), o_sf = c.take(L * 2 * 8), o_si = c.take(L * 2 * 4);
     const size_t o_w = c.take(L * 8), o_D = c.take(max_sources * N * 8), o_free = c.take(L * 8),
                  o_mb = c.take((size_t)3 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4),
-                 o_gc = c.take(L * W.S * 4), o_gt = c.take(L * 4);
+                 o_gc = c.take(L * W.S * 4), o_gt = c.take(L * 4), o_hold = c.take(C * HOLD_ROW * 4);
     W.zero_off = c.cur;
     const size_t o_have = c.take(N * W.Wp * 8), o_wants = c.take(N * W.Wp * 8), o_hs = c.take(N * W.SWp * 8),
-                 o_ws = c.take(N * W.SWp * 8), o_wc = c.take(N * 4), o_ctrl = c.take(sizeof(LoopCtrl));
+                 o_ws = c.take(N * W.SWp * 8), o_wc = c.take(N * 4), o_hc = c.take(C * 4), o_ctrl = c.take(sizeof(LoopCtrl));
     W.zero_bytes = c.cur - W.zero_off;
     int rc = dev_alloc(c.cur, &W.blob);
     if (rc) return rc;
@@ -721,18 +722,21 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.hsum = (uint64_t*)(b + o_hs); W.wsum = (uint64_t*)(b + o_ws);
     W.gcnt = (uint32_t*)(b + o_gc); W.gtot = (uint32_t*)(b + o_gt);
     W.best = (uint64_t*)(b + o_best);
+    W.hold = (uint32_t*)(b + o_hold); W.hold_cnt = (uint32_t*)(b + o_hc);
     W.st_free = (uint64_t*)(b + o_sf); W.st_inf = (uint32_t*)(b + o_si);
     W.wants_cnt = (uint32_t*)(b + o_wc); W.ctrl = (LoopCtrl*)(b + o_ctrl);
     return PCCL_OK;
 }
 
 struct PhaseView {   // link tables in the synthesized direction
-    const uint32_t *esrc, *edst, *in_off, *in_link, *out_link, *out_far, *lo_off, *lo_deg;
+    const uint32_t *esrc, *edst, *in_off, *in_link, *out_link, *out_far, *lo_off, *lo_deg, *out_off;
 };
 PhaseView view_of(const pccl_topology* t, bool transposed) {
     if (!transposed)
-        return {t->d_src, t->d_dst, t->d_in_off, t->d_in_link, t->d_out_link, t->d_out_far, t->d_lo_off_n, t->d_lo_deg_n};
-    return {t->d_dst, t->d_src, t->d_out_off, t->d_out_link, t->d_in_link, t->d_in_far, t->d_lo_off_t, t->d_lo_deg_t};
+        return {t->d_src, t->d_dst, t->d_in_off, t->d_in_link, t->d_out_link, t->d_out_far, t->d_lo_off_n, t->d_lo_deg_n,
+                t->d_out_off};
+    return {t->d_dst, t->d_src, t->d_out_off, t->d_out_link, t->d_in_link, t->d_in_far, t->d_lo_off_t, t->d_lo_deg_t,
+            t->d_in_off};
 }
 
 // steps A..C; on return the wants total is in *M (synchronises the stream)
@@ -806,9 +810,8 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
                uint64_t out_cap, uint64_t t_offset, LoopResult* res, std::vector<uint64_t>* trace = nullptr,
                Rec* host_out = nullptr, bool* streamed = nullptr) {
     const bool dynamic = (flags & PCCL_FLAG_DYNAMIC_RELAY) != 0;
-    // the dynamic rule's wants rows are dense and shrink by the thousand per event: keeping the counts current
-    // costs more than recounting by whole rows, so that is its default (KEPT_COUNTS overrides)
-    if (dynamic && !(flags & (PCCL_FLAG_RESCAN | PCCL_FLAG_KEPT_COUNTS))) flags |= PCCL_FLAG_DENSE_SWEEP;
+    // the dynamic rule keeps the counts current too: wants bits are only dropped where a neighbour holds the chunk
+    // (holder lists, dyn_shrink_wants); DENSE_SWEEP / RESCAN recount instead and drop every bit at once
     const pccl_topology* t = P.topo;
     const PhaseView pv = view_of(t, ph.transposed);
     LoopArgs a;
@@ -823,6 +826,10 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     a.wants_cnt = W.wants_cnt; a.free_t = W.free_t; a.inflight = W.inflight; a.have_epoch = W.have_epoch;
     a.empty_epoch = W.empty_epoch; a.matchbits = W.matchbits; a.ctrl = W.ctrl; a.out = out; a.t_offset = t_offset;
     a.out_cap = out_cap;
+    // dynamic rule with kept counts: a tightened best revisits only the out-neighbours of the chunk's holders
+    const bool lazy = dynamic && !(flags & (PCCL_FLAG_RESCAN | PCCL_FLAG_DENSE_SWEEP));
+    a.csrc = ph.d_cond_src; a.out_off = pv.out_off;
+    a.hold = lazy ? W.hold : nullptr; a.hold_cnt = lazy ? W.hold_cnt : nullptr;
     a.best = dynamic ? W.best : nullptr; a.Dto = W.D; a.didx = ph.d_didx; a.dest_off = ph.d_dest_off; a.dests = ph.d_dests;
     cudaStream_t st = G.stream;
     a.trace = nullptr; a.trace_cap = 0;

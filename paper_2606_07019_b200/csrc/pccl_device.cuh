@@ -328,10 +328,17 @@ struct LoopArgs {
     uint32_t* st_inf;
     uint64_t* trace;        // optional [events][TRACE_SLOTS] globaltimer stamps of CTA 0 (diagnostic), or null
     uint32_t trace_cap;     // events the trace buffer holds
+    // dynamic rule with kept counts: the holders of each chunk (nodes whose have bit is stored), so that a tightened
+    // best only revisits the out-neighbours of holders (null: every node is revisited)
+    const uint32_t* csrc;       // [C] source of each chunk
+    const uint32_t* out_off;    // [N+1] per-node offsets into out_link / out_far
+    uint32_t* hold_cnt;         // [C] arrivals of the chunk so far
+    uint32_t* hold;             // [C][HOLD_ROW] slots 1..HOLD_CAP: the first HOLD_CAP arrival nodes
     unsigned long long* progress;   // optional word in mapped pinned HOST memory: records [0, *progress) of `out` are
                                     // final (k_loop1 only; the host streams them out while the loop runs), or null
 };
 
+constexpr uint32_t HOLD_ROW = 32, HOLD_CAP = 31;
 constexpr int TRACE_SLOTS = 12;  // 0 loop top, 1 links phase, 2 barrier 1, 3 in-link list, 4 count, 5 pick, 6 commit,
                                  // 7 barrier 2, 8 summary scan, 9 work list, 10 unused, 11 unused
 __device__ __forceinline__ void trace_stamp(const LoopArgs& a, uint32_t step, int slot) {
@@ -417,6 +424,15 @@ __device__ __forceinline__ uint32_t kth_bit128(uint4 m, uint32_t k) {
     return 0xFFFFFFFFu;
 }
 
+// dynamic rule (Q18): node u still wants chunk c iff it is strictly closer to some dest of c than the
+// best holder so far
+__device__ __forceinline__ bool dyn_still_wants(const LoopArgs& a, uint32_t u, uint32_t c) {
+    const uint64_t p1 = a.dest_off[c + 1];
+    for (uint64_t p = a.dest_off[c]; p < p1; ++p)
+        if (a.Dto[(size_t)a.didx[a.dests[p]] * a.N + u] < ldcg64(a.best + p)) return true;
+    return false;
+}
+
 // ---- P1: ordered emit of the previous event's matches (a8) + arrivals at time t (a3) ---------------
 __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t step, uint64_t t,
                                                  uint64_t emit_base) {
@@ -458,6 +474,10 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
             atomicOr((unsigned long long*)&a.have[(size_t)d * a.Wp + (c >> 6)], 1ull << (c & 63));
             atomicOr((unsigned long long*)&a.hsum[(size_t)d * a.SWp + (c >> 14)], 1ull << ((c >> 8) & 63));
             stcg32(a.have_epoch + d, step + 1);   // (inflight keeps the chunk: free_t == t holds at this event only)
+            if (a.hold != nullptr) {
+                const uint32_t k = atomicAdd(a.hold_cnt + c, 1u) + 1u;
+                if (k <= HOLD_CAP) stcg32(a.hold + (size_t)c * HOLD_ROW + k, d);
+            }
         }
     }
     // a5 (kept counts): the receiving node d now holds c, so c is a new candidate of every out-link of d whose
@@ -476,8 +496,16 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
             for (uint32_t k = k0; k < deg; k += K) {
                 const uint32_t o = a.out_link[off + k], v2 = a.out_far[off + k];
                 if ((ldcg64(a.wants + (size_t)v2 * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) {
-                    atomicAdd(&a.gcnt[(size_t)o * a.S + (c >> 12)], 1u);
-                    atomicAdd(&a.gtot[o], 1u);
+                    if (a.hold != nullptr && !dyn_still_wants(a, v2, c)) {
+                        // lazy dynamic rule: v2 stopped wanting c while no neighbour held it; the bit goes now, and no
+                        // count can include it (a neighbour that held c would have had it cleared at the tightening)
+                        const unsigned long long bit = 1ull << (c & 63);
+                        if (atomicAnd((unsigned long long*)&a.wants[(size_t)v2 * a.Wp + (c >> 6)], ~bit) & bit)
+                            atomicSub(&a.wants_cnt[v2], 1u);
+                    } else {
+                        atomicAdd(&a.gcnt[(size_t)o * a.S + (c >> 12)], 1u);
+                        atomicAdd(&a.gtot[o], 1u);
+                    }
                 }
             }
         }
@@ -500,15 +528,65 @@ __device__ __forceinline__ void dyn_drop(const LoopArgs& a, uint32_t u, uint32_t
     atomicSub(&a.wants_cnt[u], 1u);
     if (a.gcnt == nullptr) return;
     const uint32_t e1 = a.in_off[u + 1];
-    for (uint32_t e = a.in_off[u]; e < e1; ++e) {
-        const uint32_t l2 = a.in_link[e];
-        if ((ldcg64(a.have + (size_t)a.esrc[l2] * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) {
-            atomicSub(&a.gcnt[(size_t)l2 * a.S + (c >> 12)], 1u);
-            atomicSub(&a.gtot[l2], 1u);
+    for (uint32_t eb = a.in_off[u]; eb < e1; eb += 4) {   // four in-links per round: table, source, have word
+        uint32_t l2[4];
+        unsigned long long hw[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) l2[k] = (eb + k < e1) ? a.in_link[eb + k] : NONE32;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) hw[k] = (l2[k] != NONE32) ? ldcg64(a.have + (size_t)a.esrc[l2[k]] * a.Wp + (c >> 6)) : 0ull;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if ((hw[k] >> (c & 63)) & 1ull) {
+                atomicSub(&a.gcnt[(size_t)l2[k] * a.S + (c >> 12)], 1u);
+                atomicSub(&a.gtot[l2[k]], 1u);
+            }
+    }
+}
+
+// every node that no longer wants claimed chunk c loses the bit (whole warp; scans all nodes)
+__device__ __forceinline__ void dyn_shrink_chunk(const LoopArgs& a, uint32_t c, uint32_t lane) {
+    const uint64_t p0 = a.dest_off[c], p1 = a.dest_off[c + 1];
+    const unsigned long long bit = 1ull << (c & 63);
+    if (p1 - p0 <= 32) {
+        // lane q holds pair q (row of its dest in Dto, current best); four nodes per lane and round, their
+        // wants words loaded together, then one coalesced Dto load per pair and node
+        const uint32_t np = (uint32_t)(p1 - p0);
+        uint32_t row = 0;
+        unsigned long long bst = 0;
+        if (lane < np) { row = a.didx[a.dests[p0 + lane]]; bst = ldcg64(a.best + p0 + lane); }
+        for (uint32_t ub = 0; ub < a.N; ub += 128) {
+            bool need[4], keep[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t u = ub + 32 * k + lane;
+                need[k] = u < a.N && (ldcg64(a.wants + (size_t)u * a.Wp + (c >> 6)) & bit) != 0ull;
+                keep[k] = false;
+            }
+            for (uint32_t q = 0; q < np; ++q) {
+                const uint32_t r = __shfl_sync(0xFFFFFFFFu, row, q);
+                const unsigned long long b = __shfl_sync(0xFFFFFFFFu, bst, q);
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (need[k] && !keep[k]) keep[k] = a.Dto[(size_t)r * a.N + ub + 32 * k + lane] < b;
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (need[k] && !keep[k]) dyn_drop(a, ub + 32 * k + lane, c);
+        }
+    } else {
+        for (uint32_t u = lane; u < a.N; u += 32) {
+            if (!(ldcg64(a.wants + (size_t)u * a.Wp + (c >> 6)) & bit)) continue;
+            if (!dyn_still_wants(a, u, c)) dyn_drop(a, u, c);
         }
     }
 }
 
+// With holder lists (kept counts) only the out-neighbours of the chunk's holders are revisited: a wants bit can
+// only be read through an in-link whose source holds the chunk (candidates are have[src] & wants[dst]), so the
+// bits of all other nodes may stay stale until a neighbour receives the chunk -- the arrival then applies the rule
+// (loop_phase_links).  A chunk with more than HOLD_CAP arrivals falls back to the scan over all nodes, which is
+// exact whatever was skipped before.
 __device__ __forceinline__ void dyn_shrink_wants(const LoopArgs& a, uint32_t step) {
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nW = (gridDim.x * blockDim.x) >> 5;
@@ -516,42 +594,41 @@ __device__ __forceinline__ void dyn_shrink_wants(const LoopArgs& a, uint32_t ste
     for (uint32_t l = gw; l < a.L; l += nW) {   // a warp per link matched at this event
         if (!((ldcg64(mb + (l >> 6)) >> (l & 63)) & 1ull)) continue;
         const uint32_t c = ldcg32(a.inflight + l);
+        if (a.hold == nullptr) { dyn_shrink_chunk(a, c, lane); continue; }
+        // everything keyed on c in one round trip: the arrival count, the pairs, the holder slots (slots past the
+        // count hold garbage and are masked below).  Lane 0: the source, lanes 1..nh: the arrival nodes
+        const uint32_t nh = ldcg32(a.hold_cnt + c);
         const uint64_t p0 = a.dest_off[c], p1 = a.dest_off[c + 1];
+        uint32_t u = (lane == 0) ? a.csrc[c] : ldcg32(a.hold + (size_t)c * HOLD_ROW + lane);
+        if (nh > HOLD_CAP || p1 - p0 > 32) { dyn_shrink_chunk(a, c, lane); continue; }
+        if (lane > nh) u = NONE32;
+        const uint32_t np = (uint32_t)(p1 - p0);
+        uint32_t row = 0;               // lane q: pair q of c (row of its dest in Dto, current best)
+        unsigned long long bst = 0;
+        if (lane < np) { row = a.didx[a.dests[p0 + lane]]; bst = ldcg64(a.best + p0 + lane); }
+        uint32_t off = 0, deg = 0;      // the holders' out-links, flattened over the warp
+        if (u != NONE32) { off = a.out_off[u]; deg = a.out_off[u + 1] - off; }
+        const uint32_t incl = warp_incl_scan(deg, lane);
+        const uint32_t T = __shfl_sync(0xFFFFFFFFu, incl, 31);
         const unsigned long long bit = 1ull << (c & 63);
-        if (p1 - p0 <= 32) {
-            // lane q holds pair q (row of its dest in Dto, current best); four nodes per lane and round, their
-            // wants words loaded together, then one coalesced Dto load per pair and node
-            const uint32_t np = (uint32_t)(p1 - p0);
-            uint32_t row = 0;
-            unsigned long long bst = 0;
-            if (lane < np) { row = a.didx[a.dests[p0 + lane]]; bst = ldcg64(a.best + p0 + lane); }
-            for (uint32_t ub = 0; ub < a.N; ub += 128) {
-                bool need[4], keep[4];
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const uint32_t u = ub + 32 * k + lane;
-                    need[k] = u < a.N && (ldcg64(a.wants + (size_t)u * a.Wp + (c >> 6)) & bit) != 0ull;
-                    keep[k] = false;
-                }
-                for (uint32_t q = 0; q < np; ++q) {
-                    const uint32_t r = __shfl_sync(0xFFFFFFFFu, row, q);
-                    const unsigned long long b = __shfl_sync(0xFFFFFFFFu, bst, q);
-#pragma unroll
-                    for (int k = 0; k < 4; ++k)
-                        if (need[k] && !keep[k]) keep[k] = a.Dto[(size_t)r * a.N + ub + 32 * k + lane] < b;
-                }
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    if (need[k] && !keep[k]) dyn_drop(a, ub + 32 * k + lane, c);
+        for (uint32_t x0 = 0; x0 < T; x0 += 32) {
+            const uint32_t x = x0 + lane;
+            uint32_t j = 0;   // holder of item x: the number of holders whose items all come before x
+            for (uint32_t jj = 0; jj <= nh; ++jj) j += (__shfl_sync(0xFFFFFFFFu, incl, jj) <= x) ? 1u : 0u;
+            const uint32_t js = min(j, 31u);
+            const uint32_t first = __shfl_sync(0xFFFFFFFFu, incl - deg, js), offj = __shfl_sync(0xFFFFFFFFu, off, js);
+            uint32_t v2 = 0;
+            bool need = false, keep = false;
+            if (x < T) {
+                v2 = a.out_far[offj + (x - first)];
+                need = (ldcg64(a.wants + (size_t)v2 * a.Wp + (c >> 6)) & bit) != 0ull;
             }
-        } else {
-            for (uint32_t u = lane; u < a.N; u += 32) {
-                if (!(ldcg64(a.wants + (size_t)u * a.Wp + (c >> 6)) & bit)) continue;
-                bool keep = false;
-                for (uint64_t p = p0; p < p1 && !keep; ++p)
-                    keep = a.Dto[(size_t)a.didx[a.dests[p]] * a.N + u] < ldcg64(a.best + p);
-                if (!keep) dyn_drop(a, u, c);
+            for (uint32_t q = 0; q < np; ++q) {
+                const uint32_t r = __shfl_sync(0xFFFFFFFFu, row, q);
+                const unsigned long long b = __shfl_sync(0xFFFFFFFFu, bst, q);
+                if (need && !keep) keep = a.Dto[(size_t)r * a.N + v2] < b;
             }
+            if (need && !keep) dyn_drop(a, v2, c);
         }
     }
 }
@@ -645,8 +722,16 @@ __device__ __forceinline__ uint32_t warp_sum_counts(const uint32_t* cj, uint32_t
 }
 
 // a8: link l carries chunk c over [t, t + w_l); destination v no longer wants c
+// dynamic relay rule: v becomes a holder of c, best[p] of c's pairs tightens (read only after the event's barrier)
+__device__ __forceinline__ void commit_best(const LoopArgs& a, uint32_t v, uint32_t c) {
+    if (a.best == nullptr) return;
+    const uint64_t p1 = a.dest_off[c + 1];
+    for (uint64_t p = a.dest_off[c]; p < p1; ++p)
+        atomicMin((unsigned long long*)&a.best[p], (unsigned long long)a.Dto[(size_t)a.didx[a.dests[p]] * a.N + v]);
+}
+
 __device__ __forceinline__ uint64_t commit_claim(const LoopArgs& a, uint32_t v, uint32_t l, uint64_t wl, uint32_t c,
-                                                 bool sector_empty, uint32_t step, uint64_t t) {
+                                                 bool sector_empty, uint32_t step, uint64_t t, bool tighten = true) {
     const uint64_t te = t + wl;
     atomicAnd((unsigned long long*)&a.wants[(size_t)v * a.Wp + (c >> 6)], ~(1ull << (c & 63)));
     // the pick saw no other wanted chunk in c's 32-byte sector: drop it from the wants summary.  (Two claims
@@ -656,11 +741,7 @@ __device__ __forceinline__ uint64_t commit_claim(const LoopArgs& a, uint32_t v, 
     stcg32(a.inflight + l, c);
     stcg64(a.free_t + l, te);
     atomicOr((unsigned long long*)&a.matchbits[(size_t)(step & 1) * a.nLw + (l >> 6)], 1ull << (l & 63));
-    if (a.best != nullptr) {   // dynamic relay rule: v is now a holder of c (read only after the event's barrier)
-        const uint64_t p1 = a.dest_off[c + 1];
-        for (uint64_t p = a.dest_off[c]; p < p1; ++p)
-            atomicMin((unsigned long long*)&a.best[p], (unsigned long long)a.Dto[(size_t)a.didx[a.dests[p]] * a.N + v]);
-    }
+    if (tighten) commit_best(a, v, c);
     return te;
 }
 
@@ -949,11 +1030,9 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     const uint32_t l = sh.act[b0 + j];
                     const uint32_t u = sh.src[b0 + j];
                     uint32_t* cj = cnt + j * S;
-                    if (lane == 0) {
-                        for (uint32_t i = 0; i < ncl; ++i) {
-                            const uint32_t c = sh.claimed[i];
-                            if ((ldcg64(a.have + (size_t)u * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) cj[c >> 12] -= 1;
-                        }
+                    if (lane < ncl) {   // (at most NBT claims: one lane each, one round trip)
+                        const uint32_t c = sh.claimed[lane];
+                        if ((ldcg64(a.have + (size_t)u * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) atomicSub(&cj[c >> 12], 1u);
                     }
                     __syncwarp();
                     const uint32_t n = warp_sum_counts(cj, S, lane);
@@ -970,7 +1049,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     }
                     if (lane == 0) {
                         sh.claimed[ncl] = c;
-                        const uint64_t te = commit_claim(a, v, l, sh.actw[b0 + j], c, sem, step, t);
+                        const uint64_t te = commit_claim(a, v, l, sh.actw[b0 + j], c, sem, step, t, false);
                         mymin = min(mymin, te);
                         mymax = max(mymax, te);
                     }
@@ -978,6 +1057,8 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     --wc;
                     __syncwarp();
                 }
+                // (their best[] updates are off the serial chain: one lane per re-picked claim)
+                if (lane >= ncl_spec && lane < ncl) commit_best(a, v, sh.claimed[lane]);
                 trace_stamp(a, step, 10);
                 const uint32_t dec0 = fastpairs ? ncl_spec : 0u;   // claims before dec0 were handled above
                 if (a.gcnt != nullptr && ncl > dec0) {
