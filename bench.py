@@ -13,7 +13,8 @@ synthesized schedule / synthesis time; synthesis seconds are reported beside it.
   value   inputs (topology + normalised conditions) resident in HBM, schedule left in HBM;
           timed per step with CUDA events on the launching stream, L2 flushed between steps.
   e2e     the same through pccl_synthesize with HOST buffers: normalise, host->device copies,
-          all kernels, device->host copy of the schedule, all inside the timed region.
+          all kernels, device->host copy of the schedule (streamed out in pieces on a copy
+          stream while the event loop is still running), all inside the timed region.
   roofline  the event-loop kernel k_loop: bitmap bytes it requested / its CUDA-event time,
           against MEASURED_PEAKS.json's HBM copy bandwidth.
   cpu_baseline  the oracle, as it stands, one thread, on this box's host cores.
@@ -369,7 +370,13 @@ def run_ours(args):
         dynamic = {"synthesis_ms": sum(ms_d) / len(ms_d), "loop_ms": dst["loop_ms"], "transfers": dM,
                    "events": dst["events"], "schedule_time_ps": dT,
                    "schedule_time_vs_thin_tree": dT / T if T else None,
-                   "initial_wants": dst["wants_total"]}
+                   "initial_wants": dst["wants_total"],
+                   "counting": "kept counts + per-chunk holder lists (the rule's default)"}
+        # the same rule recounting by the dense sweep and dropping every stale wants bit at once (cross-check mode)
+        sd = prob.synthesize(seed, flags | pk.PCCL_FLAG_DYNAMIC_RELAY | pk.PCCL_FLAG_DENSE_SWEEP)
+        assert (sd.size, sd.time_ps) == (dM, dT)
+        dynamic["dense_sweep_loop_ms"] = sd.stats["loop_ms"]
+        sd.close()
 
     # ---- the paper's own per-condition synthesizer (PCCL_FLAG_BFS; Q19-Q22) on the same problem
     bfs = None
