@@ -27,8 +27,10 @@
  *   - Device work is enqueued on the stream set with pccl_set_stream (default: the legacy
  *     default stream) of the CUDA device that is current when the handle is created, and is
  *     synchronised before a function returns host-visible results.
- *   - Calls on distinct handles are independent; a single handle must not be used from two
- *     threads at once.  The process-wide settings (stream, allocator) are not thread-safe.
+ *   - Calls on distinct handles may come from different threads: the entry points that touch the
+ *     device serialise themselves (one runs at a time; they share a control mailbox, a copy
+ *     stream and the stream below).  A single handle must not be used from two threads at once.
+ *     The process-wide settings (stream, allocator) are set once, before any other thread calls.
  *   - There is NO CPU fallback: without a CUDA device every compute entry point returns
  *     PCCL_ERR_CUDA.
  * ========================================================================================= */

@@ -36,6 +36,9 @@ struct Globals {
     pccl_free_fn release = nullptr;
     void* user = nullptr;
     std::mutex mu;
+    // device entry points share the mailbox, the copy stream and G.stream: one call at a time (re-entrant: an
+    // entry point may call another)
+    std::recursive_mutex call_mu;
     // pinned host memory: a small mailbox for control blocks and a free-list of result buffers
     void* mailbox = nullptr;
     struct Pinned { void* p; size_t bytes; };
@@ -47,6 +50,8 @@ struct Globals {
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t loop_done = nullptr;
 } G;
+
+#define SERIALISE std::lock_guard<std::recursive_mutex> call_lock__(G.call_mu)
 
 #define CU(call)                                   \
     do {                                           \
@@ -315,6 +320,7 @@ extern "C" int pccl_topology_create(uint32_t n_npus, const pccl_link_t* links, u
 }
 
 extern "C" void pccl_topology_destroy(pccl_topology_t* t) {
+    SERIALISE;
     if (!t) return;
     dev_free(t->blob);
     delete t;
@@ -635,12 +641,14 @@ extern "C" int pccl_problem_create(const pccl_topology_t* topo, const uint32_t* 
 }
 
 extern "C" void pccl_problem_destroy(pccl_problem_t* P) {
+    SERIALISE;
     if (!P) return;
     for (Phase& ph : P->phases) dev_free(ph.blob);
     delete P;
 }
 
 extern "C" int pccl_problem_upload(pccl_problem_t* P) {
+    SERIALISE;
     if (!P) return PCCL_ERR_INVALID;
     if (P->uploaded) return PCCL_OK;
     int rc = topo_upload(const_cast<pccl_topology*>(P->topo));
@@ -1166,6 +1174,7 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
 }  // namespace
 
 extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_t flags, pccl_schedule_t** out) {
+    SERIALISE;
     if (!P || !out) return PCCL_ERR_INVALID;
     int rc = pccl_problem_upload(P);
     if (rc) return rc;
@@ -1333,6 +1342,7 @@ extern "C" int pccl_synthesize(const pccl_topology_t* topo, const uint32_t* grou
 extern "C" uint64_t pccl_schedule_time(const pccl_schedule_t* s) { return s ? s->T : 0; }
 extern "C" uint64_t pccl_schedule_size(const pccl_schedule_t* s) { return s ? s->M : 0; }
 extern "C" const pccl_transfer_t* pccl_schedule_transfers(pccl_schedule_t* s) {
+    SERIALISE;
     if (!s || s->M == 0) return nullptr;
     if (!s->downloaded) {
         if (!s->d_recs) return nullptr;
@@ -1352,6 +1362,7 @@ extern "C" const pccl_transfer_t* pccl_schedule_transfers_device(const pccl_sche
     return s ? (const pccl_transfer_t*)s->d_recs : nullptr;
 }
 extern "C" void pccl_schedule_destroy(pccl_schedule_t* s) {
+    SERIALISE;
     if (!s) return;
     dev_free(s->d_recs);
     pinned_put(s->h_recs, s->h_bytes);
@@ -1360,6 +1371,7 @@ extern "C" void pccl_schedule_destroy(pccl_schedule_t* s) {
 static_assert(sizeof(pccl_op_t) == sizeof(Op), "op layout");
 
 extern "C" int pccl_schedule_programs(pccl_schedule_t* s, uint64_t* offsets, pccl_op_t* ops) {
+    SERIALISE;
     if (!s || !offsets || (s->M && !ops)) return PCCL_ERR_INVALID;
     const uint32_t N = s->n_npus;
     const uint64_t M = s->M, n = 2 * M;
@@ -1420,6 +1432,7 @@ extern "C" int pccl_schedule_stats(const pccl_schedule_t* s, pccl_stats_t* out) 
 // single rows for parity tests
 // -----------------------------------------------------------------------------------------
 extern "C" int pccl_device_philox(const uint32_t* ctr, uint64_t n, const uint32_t key[2], uint32_t* out) {
+    SERIALISE;
     if ((n && (!ctr || !out)) || !key) return PCCL_ERR_INVALID;
     if (n == 0) return PCCL_OK;
     int rc = ensure_device();
@@ -1442,6 +1455,7 @@ extern "C" int pccl_device_philox(const uint32_t* ctr, uint64_t n, const uint32_
 }
 
 extern "C" int pccl_device_link_costs(pccl_topology_t* t, uint64_t chunk_bytes, uint64_t* out) {
+    SERIALISE;
     if (!t || !out || chunk_bytes == 0) return PCCL_ERR_INVALID;
     int rc = topo_upload(t);
     if (rc) return rc;
@@ -1460,6 +1474,7 @@ extern "C" int pccl_device_link_costs(pccl_topology_t* t, uint64_t chunk_bytes, 
 
 extern "C" int pccl_device_distances(pccl_topology_t* t, uint64_t chunk_bytes, uint32_t src, int transposed,
                                      uint64_t* out) {
+    SERIALISE;
     if (!t || !out || chunk_bytes == 0 || src >= t->N) return PCCL_ERR_INVALID;
     int rc = topo_upload(t);
     if (rc) return rc;
@@ -1488,6 +1503,7 @@ extern "C" int pccl_device_distances(pccl_topology_t* t, uint64_t chunk_bytes, u
 }
 
 extern "C" int64_t pccl_device_wants(pccl_problem_t* P, uint32_t phase, uint64_t seed, pccl_pair_t* out, uint64_t cap) {
+    SERIALISE;
     if (!P || phase >= P->phases.size() || (cap && !out)) return PCCL_ERR_INVALID;
     int rc = pccl_problem_upload(P);
     if (rc) return rc;

@@ -201,6 +201,31 @@ def test_star_switch_with_70_inlinks(pk):
     checker.check_schedule(p, s.transfers)
 
 
+def test_concurrent_calls_from_two_threads(pk):
+    """include/pccl.h: calls on distinct handles may come from different threads (the device entry points
+    serialise themselves).  Two threads synthesize different problems back to back; every result must be the
+    oracle's."""
+    import threading
+    probs = [wl.config4_small(0), wl.config2(1), wl.config5_small(2), wl.config3(0)]
+    expect = [oracle.synthesize(*p.args()) for p in probs]
+    errors = []
+
+    def work(order):
+        try:
+            for _ in range(3):
+                for i in order:
+                    assert_same(probs[i], gpu_run(pk, probs[i]), expect[i])
+        except BaseException as e:   # noqa: BLE001 - reported by the main thread
+            errors.append(e)
+
+    threads = [threading.Thread(target=work, args=(o,)) for o in ([0, 1, 2, 3], [3, 2, 1, 0])]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors[0]
+
+
 def test_empty_and_trivial(pk):
     links = wl.ring_links(4, True)
     members = np.arange(4, dtype=np.uint32)
@@ -312,6 +337,37 @@ def test_dynamic_relay_three_counting_modes(pk, maker):
     o = oracle.synthesize(*p.args(), relay=oracle.RELAY_DYNAMIC)
     for fl in (0, pk.PCCL_FLAG_KEPT_COUNTS, pk.PCCL_FLAG_RESCAN, pk.PCCL_FLAG_DENSE_SWEEP):
         assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY | fl), o)
+
+
+def test_dynamic_relay_holder_rows_overflow(pk):
+    """The holder row of a chunk has 31 slots: past that a claim falls back to the scan over all
+    nodes.  A 40-node path (one chunk, 39 arrivals: the switch happens mid-run, with stale bits around), rings with
+    32 dests and 32+ arrivals per chunk, a mesh where every chunk has more than 32 dests."""
+    mesh = wl.grid_links((7, 6), wrap=False)
+    m42 = np.arange(42, dtype=np.uint32)
+    nc, pre, post = wl.all_gather(m42, 2)
+    cases = [wl.path_point_to_point(40, 0), wl.ring_all_gather(33, False, 3), wl.ring_all_gather(36, True, 1),
+             wl.ring_all_gather(33, True, 2, chunks_per_npu=3, chunk_bytes=4096),
+             wl.Problem("mesh7x6_allgather2", 42, mesh, m42, nc, pre, post, 1 << 16, 5)]
+    for p in cases:
+        o = oracle.synthesize(*p.args(), relay=oracle.RELAY_DYNAMIC)
+        for fl in (0, pk.PCCL_FLAG_DENSE_SWEEP):
+            assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY | fl), o)
+
+
+def test_dynamic_relay_config4_full_size_two_forms_agree(pk):
+    """Full size (58 M initial wants, 1.58 M transfers; the oracle needs 15 minutes here): the holder-list form and
+    the all-nodes scan must emit the same records, and the result must be a valid schedule."""
+    p = wl.config4(0)
+    topo = pk.Topology(p.n_npus, p.links)
+    prob = pk.Problem(topo, p.group, p.n_chunks, p.pre, p.post, p.chunk_bytes)
+    a = prob.synthesize(0, pk.PCCL_FLAG_DYNAMIC_RELAY)
+    b = prob.synthesize(0, pk.PCCL_FLAG_DYNAMIC_RELAY | pk.PCCL_FLAG_DENSE_SWEEP)
+    ta, tb = a.transfers, b.transfers
+    assert a.size == b.size == 1_579_300 and a.time_ps == b.time_ps == 273_214_495   # = the oracle's M and T (DESIGN.md)
+    for f in ta.dtype.names:
+        assert np.array_equal(ta[f], tb[f]), f
+    checker.check_structure(p, ta)
 
 
 def test_dynamic_relay_unreachable(pk):
