@@ -192,6 +192,9 @@ struct PoolAlloc {
         return (T*)p;
     }
     void deallocate(T* p, size_t n) { HP.put(p, n * sizeof(T)); }
+    // resize(n) leaves new elements uninitialised (every user writes all of them); resize(n, v) / assign still fill
+    template <class U> void construct(U* p) noexcept { ::new ((void*)p) U; }
+    template <class U, class... A> void construct(U* p, A&&... a) { ::new ((void*)p) U(std::forward<A>(a)...); }
     template <class U> bool operator==(const PoolAlloc<U>&) const { return true; }
     template <class U> bool operator!=(const PoolAlloc<U>&) const { return false; }
 };
@@ -464,6 +467,58 @@ void finish_phase(Phase& ph, uint32_t N) {
     index_phase(ph, N, is_src, is_dst);
 }
 
+// The common large case in one streaming pass over the caller's arrays: both pair lists already ordered by chunk,
+// exactly one pre-holder per chunk (COPY mode), post-holders of a chunk strictly ascending.  Returns false on ANY
+// deviation (including invalid input) without touching P: the general path below then decides, errors included.
+bool normalise_ordered_copy(const pccl_condition_t* pre, const pccl_condition_t* post, uint32_t C, uint32_t N,
+                            const std::vector<char>& member, Phase& cp) {
+    if (pre->n_pairs != C || post->n_pairs < C) return false;
+    const pccl_pair_t* __restrict__ pp = pre->pairs;
+    const pccl_pair_t* __restrict__ qp = post->pairs;
+    const uint64_t nq = post->n_pairs;
+    const char* mem = member.data();
+    cp.cond_src.resize(C);
+    cp.dest_off.resize((size_t)C + 1);
+    cp.dests.resize(nq);
+    cp.dchunk.resize(nq);
+    uint32_t* __restrict__ o_src = cp.cond_src.data();
+    uint64_t* __restrict__ o_off = cp.dest_off.data();
+    uint32_t* __restrict__ o_dst = cp.dests.data();
+    uint32_t* __restrict__ o_chk = cp.dchunk.data();
+    std::vector<uint32_t> f_src(N, 0), f_dst(N, 0);
+    o_off[0] = 0;
+    uint64_t k = 0, nd = 0;
+    for (uint32_t c = 0; c < C; ++c) {
+        const pccl_pair_t a = pp[c];
+        if (a.chunk != c || a.npu >= N || !mem[a.npu]) return false;
+        const uint32_t src = a.npu;
+        if (k >= nq || qp[k].chunk != c) return false;   // no post-holder, or not ordered
+        const uint64_t first = nd;
+        uint32_t prev = 0;
+        bool have_prev = false;
+        while (k < nq && qp[k].chunk == c) {
+            const uint32_t d = qp[k].npu;
+            if (d >= N || !mem[d] || (have_prev && d <= prev)) return false;
+            prev = d;
+            have_prev = true;
+            ++k;
+            if (d == src) continue;
+            o_dst[nd] = d;
+            o_chk[nd] = c;
+            f_dst[d] = 1;
+            ++nd;
+        }
+        o_src[c] = src;
+        o_off[c + 1] = nd;
+        if (nd > first) f_src[src] = 1;
+    }
+    if (k != nq) return false;   // pairs of a chunk id >= C, or out of order
+    cp.dests.resize(nd);
+    cp.dchunk.resize(nd);
+    index_phase(cp, N, std::vector<char>(f_src.begin(), f_src.end()), std::vector<char>(f_dst.begin(), f_dst.end()));
+    return true;
+}
+
 int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_members,
               const pccl_condition_t* pre, const pccl_condition_t* post, uint64_t chunk_bytes,
               pccl_problem& P) {
@@ -475,6 +530,18 @@ int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_membe
     for (uint32_t i = 0; i < n_members; ++i) {
         if (group[i] >= N || member[group[i]]) return PCCL_ERR_INVALID;
         member[group[i]] = 1;
+    }
+    if (C > 0) {
+        Phase cp;
+        if (normalise_ordered_copy(pre, post, C, N, member, cp)) {
+            P.topo = topo;
+            P.C = C;
+            P.chunk_bytes = chunk_bytes;
+            P.mode = 0;
+            P.phases.clear();
+            P.phases.push_back(std::move(cp));
+            return PCCL_OK;
+        }
     }
     hvec<uint64_t> pre_off, post_off;
     hvec<uint32_t> pre_n, post_n;
@@ -505,31 +572,46 @@ int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_membe
     cp.dests.resize(post_n.size());
     cp.dchunk.resize(post_n.size());
     cp.dest_off[0] = 0;
-    std::vector<char> cp_src(N, 0), cp_dst(N, 0);
+    std::vector<uint32_t> cp_src32(N, 0), cp_dst32(N, 0);
     uint64_t nd = 0;
-    for (uint32_t c = 0; c < C; ++c) {
-        const uint64_t np = pre_off[c + 1] - pre_off[c], nq = post_off[c + 1] - post_off[c];
-        if (np == 0 || nq == 0) return PCCL_ERR_INVALID;
-        const bool single = np == 1;
-        all_single &= single;
-        all_multi_one &= (!single && nq == 1);
-        all_multi_many &= (!single && nq > 1);
-        if (all_single) {
-            const uint32_t src = pre_n[pre_off[c]];
-            const uint64_t first = nd;
-            cp.cond_src[c] = src;
-            for (uint64_t i = post_off[c]; i < post_off[c + 1]; ++i) {
-                const uint32_t d = post_n[i];
-                if (d == src) continue;
-                cp.dests[nd] = d;
-                cp.dchunk[nd] = c;
-                cp_dst[d] = 1;
-                ++nd;
+    {
+        // raw restrict pointers: the arrays are distinct, and without this every flag store forces the compiler to
+        // reload all the others
+        const uint64_t* __restrict__ po = pre_off.data();
+        const uint64_t* __restrict__ qo = post_off.data();
+        const uint32_t* __restrict__ pn = pre_n.data();
+        const uint32_t* __restrict__ qn = post_n.data();
+        uint32_t* __restrict__ o_src = cp.cond_src.data();
+        uint64_t* __restrict__ o_off = cp.dest_off.data();
+        uint32_t* __restrict__ o_dst = cp.dests.data();
+        uint32_t* __restrict__ o_chk = cp.dchunk.data();
+        uint32_t* __restrict__ f_src = cp_src32.data();
+        uint32_t* __restrict__ f_dst = cp_dst32.data();
+        for (uint32_t c = 0; c < C; ++c) {
+            const uint64_t pb = po[c], np = po[c + 1] - pb, qb = qo[c], qe = qo[c + 1], nq = qe - qb;
+            if (np == 0 || nq == 0) return PCCL_ERR_INVALID;
+            const bool single = np == 1;
+            all_single &= single;
+            all_multi_one &= (!single && nq == 1);
+            all_multi_many &= (!single && nq > 1);
+            if (all_single) {
+                const uint32_t src = pn[pb];
+                const uint64_t first = nd;
+                o_src[c] = src;
+                for (uint64_t i = qb; i < qe; ++i) {
+                    const uint32_t d = qn[i];
+                    if (d == src) continue;
+                    o_dst[nd] = d;
+                    o_chk[nd] = c;
+                    f_dst[d] = 1;
+                    ++nd;
+                }
+                o_off[c + 1] = nd;
+                if (nd > first) f_src[src] = 1;
             }
-            cp.dest_off[c + 1] = nd;
-            if (nd > first) cp_src[src] = 1;
         }
     }
+    std::vector<char> cp_src(cp_src32.begin(), cp_src32.end()), cp_dst(cp_dst32.begin(), cp_dst32.end());
     P.topo = topo;
     P.C = C;
     P.chunk_bytes = chunk_bytes;

@@ -83,6 +83,39 @@ def test_step_R_copy_mode(pk):
         pr.condition(0, 16)
 
 
+def _conditions(pk, p, pre, post):
+    pr = pk.Problem(pk.Topology(p.n_npus, p.links), p.group, p.n_chunks, pre, post, p.chunk_bytes)
+    out = []
+    for c in range(p.n_chunks):
+        src, d = pr.condition(0, c)
+        out.append((src, tuple(d.tolist())))
+    return pr.mode, out
+
+
+@pytest.mark.parametrize("maker", [wl.config1, wl.config4_small, wl.config5_small,
+                                   lambda s=0: wl.full_mesh_problem(9, "alltoall", seed=s),
+                                   lambda s=0: wl.ring_all_gather(7, True, s, chunks_per_npu=3)])
+def test_step_R_one_pass_and_general_normaliser_agree(pk, maker):
+    """Chunk-ordered COPY input takes the one-pass normaliser; any other arrangement of the same pairs (shuffled,
+    dests descending, duplicated pairs) takes the general grouping path.  Both must give the same conditions --
+    and those are the definition: source = the one pre-holder, dests = post(c) minus the source, ascending."""
+    p = maker(0)
+    rng = np.random.default_rng(7)
+    mode, ref = _conditions(pk, p, p.pre, p.post)
+    assert mode == 0
+    pre_of = {int(c): int(n) for n, c in zip(p.pre["npu"], p.pre["chunk"])}
+    post_of = {}
+    for n, c in zip(p.post["npu"], p.post["chunk"]):
+        post_of.setdefault(int(c), set()).add(int(n))
+    assert ref == [(pre_of[c], tuple(sorted(post_of[c] - {pre_of[c]}))) for c in range(p.n_chunks)]
+    variants = [(rng.permutation(p.pre), rng.permutation(p.post)),
+                (p.pre, p.post[::-1].copy()),
+                (np.concatenate([p.pre, p.pre[:3]]), np.concatenate([p.post, p.post[-5:]])),
+                (p.pre[::-1].copy(), p.post)]
+    for pre, post in variants:
+        assert _conditions(pk, p, pre, post) == (0, ref)
+
+
 def test_step_R_reduce_mode_and_duplicates(pk):
     p = wl.config3()
     pr = _problem(pk, p)
