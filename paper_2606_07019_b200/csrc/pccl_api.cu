@@ -14,6 +14,8 @@
 #include <system_error>
 #include <mutex>
 #include <new>
+#include <atomic>
+#include <unordered_set>
 #include <vector>
 
 #include "pccl_device.cuh"
@@ -143,10 +145,35 @@ void pinned_put(void* p, size_t bytes) {
 // faults than the grouping itself.  Smaller blocks go to malloc.
 struct HostPool {
     static constexpr int MIN_LOG = 16, MAX_LOG = 34;
-    static constexpr size_t CACHE_CAP = (size_t)512 << 20;
+    static constexpr size_t CACHE_CAP = (size_t)256 << 20;
     std::mutex mu;
     std::vector<void*> free_[MAX_LOG + 1];
     size_t cached = 0;
+    // pooled blocks are page-locked when a CUDA device is there (the condition arrays are uploaded straight from
+    // them); without one -- the no-GPU tests -- they are plain malloc blocks
+    std::unordered_set<void*> pinned;
+    std::atomic<bool> try_pinned{true};
+    void* fresh(size_t bytes) {
+        if (try_pinned && bytes <= ((size_t)256 << 20)) {
+            void* p = nullptr;
+            if (cudaHostAlloc(&p, bytes, cudaHostAllocDefault) == cudaSuccess) {
+                std::lock_guard<std::mutex> lk(mu);
+                pinned.insert(p);
+                return p;
+            }
+            (void)cudaGetLastError();
+            try_pinned = false;
+        }
+        return malloc(bytes);
+    }
+    void release(void* p) {
+        bool was_pinned;
+        {
+            std::lock_guard<std::mutex> lk(mu);
+            was_pinned = pinned.erase(p) != 0;
+        }
+        if (was_pinned) (void)cudaFreeHost(p); else free(p);
+    }
     static int size_class(size_t bytes) {
         int k = MIN_LOG;
         while (k < MAX_LOG && ((size_t)1 << k) < bytes) ++k;
@@ -164,18 +191,22 @@ struct HostPool {
                 return p;
             }
         }
-        return malloc((size_t)1 << k);
+        return fresh((size_t)1 << k);
     }
     void put(void* p, size_t bytes) {
         if (!p) return;
         if (bytes >= ((size_t)1 << MIN_LOG) && bytes <= ((size_t)1 << MAX_LOG)) {
             const int k = size_class(bytes);
-            std::lock_guard<std::mutex> lk(mu);
-            if (cached + ((size_t)1 << k) <= CACHE_CAP) {
-                free_[k].push_back(p);
-                cached += (size_t)1 << k;
-                return;
+            {
+                std::lock_guard<std::mutex> lk(mu);
+                if (cached + ((size_t)1 << k) <= CACHE_CAP) {
+                    free_[k].push_back(p);
+                    cached += (size_t)1 << k;
+                    return;
+                }
             }
+            release(p);
+            return;
         }
         free(p);
     }
@@ -669,27 +700,27 @@ int phase_upload(Phase& ph, uint32_t N) {
     const size_t o_cs = c.take(C * 4), o_d = c.take(ND * 4), o_dc = c.take(ND * 4), o_s = c.take(NS * 4), o_si = c.take((size_t)N * 4);
     const size_t NDS = ph.dsts.size();
     const size_t o_do = c.take((C + 1) * 8), o_ds = c.take(NDS * 4), o_di = c.take((size_t)N * 4);
-    // staged in pinned memory from the library's cache: the copy runs at full PCIe rate and no fresh pages are touched
-    struct Stage {
-        unsigned char* p; size_t bytes;
-        unsigned char* data() const { return p; }
-        size_t size() const { return bytes; }
-        ~Stage() { pinned_put(p, bytes); }
-    } h{nullptr, c.cur ? c.cur : 256};
-    h.p = (unsigned char*)pinned_get(h.bytes);
-    if (!h.p) return PCCL_ERR_NOMEM;
-    memcpy(h.data() + o_do, ph.dest_off.data(), (C + 1) * 8);
-    if (NDS) memcpy(h.data() + o_ds, ph.dsts.data(), NDS * 4);
-    if (N) memcpy(h.data() + o_di, ph.didx.data(), (size_t)N * 4);
-    if (C) memcpy(h.data() + o_cs, ph.cond_src.data(), C * 4);
-    if (ND) { memcpy(h.data() + o_d, ph.dests.data(), ND * 4); memcpy(h.data() + o_dc, ph.dchunk.data(), ND * 4); }
-    if (NS) memcpy(h.data() + o_s, ph.sources.data(), NS * 4);
-    if (N) memcpy(h.data() + o_si, ph.sidx.data(), (size_t)N * 4);
+    // copied straight from the normaliser's arrays (pooled, page-locked when a device is there): no staging pass
     void* blob = nullptr;
-    int rc = dev_alloc(h.size(), &blob);
+    int rc = dev_alloc(c.cur ? c.cur : 256, &blob);
     if (rc) return rc;
-    if (cudaMemcpyAsync(blob, h.data(), h.size(), cudaMemcpyHostToDevice, G.stream) != cudaSuccess ||
-        cudaStreamSynchronize(G.stream) != cudaSuccess) {
+    unsigned char* d = (unsigned char*)blob;
+    cudaError_t e = cudaSuccess;
+    auto up = [&](size_t off, const void* src, size_t bytes) {
+        if (bytes && e == cudaSuccess) e = cudaMemcpyAsync(d + off, src, bytes, cudaMemcpyHostToDevice, G.stream);
+    };
+    up(o_do, ph.dest_off.data(), (C + 1) * 8);
+    up(o_ds, ph.dsts.data(), NDS * 4);
+    up(o_di, ph.didx.data(), (size_t)N * 4);
+    up(o_cs, ph.cond_src.data(), C * 4);
+    up(o_d, ph.dests.data(), ND * 4);
+    up(o_dc, ph.dchunk.data(), ND * 4);
+    up(o_s, ph.sources.data(), NS * 4);
+    up(o_si, ph.sidx.data(), (size_t)N * 4);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(G.stream);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        (void)cudaStreamSynchronize(G.stream);
         (void)cudaGetLastError();
         dev_free(blob);
         return PCCL_ERR_CUDA;
