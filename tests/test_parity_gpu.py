@@ -562,6 +562,50 @@ def _random_problem(i):
     return wl.Problem(f"random{i}", n, links, members, nc, pre, post, int(rng.integers(1, 5000)), int(rng.integers(0, 2 ** 63)))
 
 
+def _random_multi_dest_problem(i):
+    """40..150 nodes, a ring plus random (often symmetric) extra links, 20..100 chunks with up to |group| dests each:
+    chunks with a handful of holders and chunks with more arrivals than a holder row has slots in one problem"""
+    rng = np.random.default_rng(50000 + i)
+    n = int(rng.integers(40, 150))
+    extra = int(rng.integers(n // 2, 3 * n))
+    src = rng.integers(0, n, extra)
+    dst = (src + 1 + rng.integers(0, n - 1, extra)) % n
+    pairs = [(a, (a + 1) % n) for a in range(n)] + list(zip(src.tolist(), dst.tolist()))
+    if rng.random() < 0.6:
+        pairs += [(b, a) for a, b in pairs]
+    links = np.zeros(len(pairs), dtype=wl.LINK_DT)
+    links["src"], links["dst"] = zip(*pairs)
+    if rng.random() < 0.5:
+        links["alpha_ps"], links["bytes_per_ps"] = 500, 10
+    else:
+        links["alpha_ps"] = rng.integers(0, 2000, len(pairs))
+        links["bytes_per_ps"] = rng.integers(1, 50, len(pairs))
+    g = int(rng.integers(n // 2, n + 1))
+    members = np.sort(rng.choice(n, size=g, replace=False)).astype(np.uint32)
+    nc = int(rng.integers(20, 100))
+    pre, post = [], []
+    for c in range(nc):
+        pre.append((int(rng.choice(members)), c))
+        k = int(rng.integers(1, g + 1)) if rng.random() < 0.5 else int(rng.integers(1, 34))
+        for d in rng.choice(members, size=min(k, g), replace=False):
+            post.append((int(d), c))
+    return wl.Problem(f"multidest{i}", n, links, members, nc, np.array(pre, dtype=wl.PAIR_DT),
+                      np.array(post, dtype=wl.PAIR_DT), int(rng.integers(1, 5000)), int(rng.integers(0, 2 ** 63)))
+
+
+def test_dynamic_relay_random_multi_dest_problems(pk):
+    """The holder-list form of the dynamic rule (lazy wants bits, fall-back to the all-nodes scan per chunk) and the
+    all-nodes form against the oracle on 24 medium-sized random problems."""
+    for i in range(24):
+        p = _random_multi_dest_problem(i)
+        try:
+            o = oracle.synthesize(*p.args(), relay=oracle.RELAY_DYNAMIC)
+        except oracle.OracleError:
+            continue
+        for fl in (0, pk.PCCL_FLAG_DENSE_SWEEP):
+            assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY | fl), o)
+
+
 @pytest.mark.parametrize("block", range(6))
 def test_randomized_problems_all_modes(pk, block):
     """120 random problems: each must give the oracle's schedule (or the oracle's error) under both relay rules
