@@ -881,8 +881,9 @@ int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t 
         if (NP) k_best_init<<<(unsigned)((NP + 255) / 256), 256, 0, st>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, NP, ph.d_didx,
                                                                          W.D, N, W.best, &W.ctrl->err);
         if (C) k_have<<<(C + 255) / 256, 256, 0, st>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
-        const uint64_t nth = (uint64_t)N * ((C + 63) / 64);
-        if (nth) k_wants_dyn_init<<<(unsigned)((nth + 127) / 128), 128, 0, st>>>(ph.d_dest_off, ph.d_dests, ph.d_didx, W.D, W.best, N,
+        const uint64_t nth = (uint64_t)N * ((C + 63) / 64);   // warps: one per (node, 64-chunk word)
+        if (nth > (0x7FFFFFFFull << 2)) return PCCL_ERR_UNSUPPORTED;
+        if (nth) k_wants_dyn_init<<<(unsigned)((nth * 32 + 127) / 128), 128, 0, st>>>(ph.d_dest_off, ph.d_dests, ph.d_didx, W.D, W.best, N,
                                                                                 C, W.Wp, W.SWp, W.wants, W.wsum, W.wants_cnt);
         k_sum_u32<<<1, 1024, 0, st>>>(W.wants_cnt, N, &W.ctrl->wants_total);
         CU(cudaGetLastError());

@@ -197,26 +197,31 @@ __global__ void k_best_init(const uint32_t* __restrict__ cond_src, const uint32_
     best[p] = d0;
 }
 
-// wants[u][c] = 1 iff some dest d of c has dist(u -> d) < best[c, d]; one thread per (node, 64-chunk word)
+// wants[u][c] = 1 iff some dest d of c has dist(u -> d) < best[c, d]; one warp per (node, 64-chunk word)
 __global__ void k_wants_dyn_init(const uint64_t* __restrict__ dest_off, const uint32_t* __restrict__ dests,
                                  const uint32_t* __restrict__ didx, const uint64_t* __restrict__ Dto,
                                  const uint64_t* __restrict__ best, uint32_t N, uint32_t C, uint32_t Wp,
                                  uint32_t SWp, uint64_t* __restrict__ wants, uint64_t* __restrict__ wsum,
                                  uint32_t* __restrict__ wants_cnt) {
+    // a warp per (node, 64-chunk word): lane b evaluates chunks b and 32 + b of the word, so the per-chunk tables
+    // (dest_off, dests, best) are read coalesced; the two ballots are the word
     const uint32_t words = (C + 63) >> 6;
-    const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gid >= (uint64_t)N * words) return;
-    const uint32_t u = (uint32_t)(gid / words), wi = (uint32_t)(gid % words);
+    const uint64_t wid = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const uint32_t lane = threadIdx.x & 31;
+    if (wid >= (uint64_t)N * words) return;   // warp-uniform
+    const uint32_t u = (uint32_t)(wid / words), wi = (uint32_t)(wid % words);
     unsigned long long word = 0;
-    for (uint32_t b = 0; b < 64; ++b) {
-        const uint32_t c = wi * 64 + b;
-        if (c >= C) break;
-        const uint64_t p1 = dest_off[c + 1];
-        for (uint64_t p = dest_off[c]; p < p1; ++p) {
-            if (Dto[(size_t)didx[dests[p]] * N + u] < best[p]) { word |= 1ull << b; break; }
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+        const uint32_t c = wi * 64 + half * 32 + lane;
+        bool w = false;
+        if (c < C) {
+            const uint64_t p1 = dest_off[c + 1];
+            for (uint64_t p = dest_off[c]; p < p1 && !w; ++p) w = Dto[(size_t)didx[dests[p]] * N + u] < best[p];
         }
+        word |= (unsigned long long)__ballot_sync(0xFFFFFFFFu, w) << (32 * half);
     }
-    if (word) {
+    if (lane == 0 && word) {
         wants[(size_t)u * Wp + wi] = word;
         atomicOr((unsigned long long*)&wsum[(size_t)u * SWp + (wi >> 8)], 1ull << ((wi >> 2) & 63));
         atomicAdd(&wants_cnt[u], (uint32_t)__popcll(word));
