@@ -156,28 +156,42 @@ __global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* _
     if (Ds[cur] == T_INF) { atomicOr(err, 1u); return; }
     const unsigned long long bit = 1ull << (c & 63);
     while (cur != s) {
+        // the node's tables are loaded before the mark's round trip is waited for
+        const uint64_t dcur = Ds[cur];
+        const uint32_t e0 = in_off[cur], e1 = in_off[cur + 1];
         const unsigned long long old = atomicOr((unsigned long long*)&wants[(size_t)cur * Wp + (c >> 6)], bit);
         if (old & bit) break;
         atomicOr((unsigned long long*)&wsum[(size_t)cur * SWp + (c >> 14)], 1ull << ((c >> 8) & 63));
         atomicAdd(&wants_cnt[cur], 1u);
-        const uint64_t dcur = Ds[cur];
-        const uint32_t e0 = in_off[cur], e1 = in_off[cur + 1];
-        uint32_t ntight = 0;
-        for (uint32_t e = e0; e < e1; ++e) {
-            const uint32_t l = in_link[e];
-            const uint64_t du = Ds[esrc[l]];
-            ntight += (du != T_INF && du + w[l] == dcur);
-        }
-        if (ntight == 0) { atomicOr(err, 2u); return; }
-        uint32_t j = __umulhi(philox_draw(c, cur, 0u, 1u, k0, k1), ntight);
         uint32_t nxt = cur;
-        for (uint32_t e = e0; e < e1; ++e) {
-            const uint32_t l = in_link[e];
-            const uint32_t u = esrc[l];
-            const uint64_t du = Ds[u];
-            if (du != T_INF && du + w[l] == dcur) {
-                if (j == 0) { nxt = u; break; }
-                --j;
+        if (e1 - e0 <= 32) {
+            // one pass: tight in-links as a bit mask (ascending link id = ascending bit), then the j-th set bit
+            uint32_t mask = 0;
+            for (uint32_t e = e0; e < e1; ++e) {
+                const uint32_t l = in_link[e];
+                const uint64_t du = Ds[esrc[l]];
+                if (du != T_INF && du + w[l] == dcur) mask |= 1u << (e - e0);
+            }
+            if (mask == 0) { atomicOr(err, 2u); return; }
+            const uint32_t j = __umulhi(philox_draw(c, cur, 0u, 1u, k0, k1), (uint32_t)__popc(mask));
+            nxt = esrc[in_link[e0 + __fns(mask, 0, (int)j + 1)]];
+        } else {
+            uint32_t ntight = 0;
+            for (uint32_t e = e0; e < e1; ++e) {
+                const uint32_t l = in_link[e];
+                const uint64_t du = Ds[esrc[l]];
+                ntight += (du != T_INF && du + w[l] == dcur);
+            }
+            if (ntight == 0) { atomicOr(err, 2u); return; }
+            uint32_t j = __umulhi(philox_draw(c, cur, 0u, 1u, k0, k1), ntight);
+            for (uint32_t e = e0; e < e1; ++e) {
+                const uint32_t l = in_link[e];
+                const uint32_t u = esrc[l];
+                const uint64_t du = Ds[u];
+                if (du != T_INF && du + w[l] == dcur) {
+                    if (j == 0) { nxt = u; break; }
+                    --j;
+                }
             }
         }
         cur = nxt;
