@@ -800,6 +800,7 @@ struct Work {   // device workspace of one phase
     uint32_t *gcnt = nullptr, *gtot = nullptr;
     uint64_t* best = nullptr;
     uint32_t *hold_cnt = nullptr, *hold = nullptr;   // dynamic rule with kept counts: holders of each chunk
+    uint32_t* drow = nullptr;                        // dynamic rule: Dto row of each (chunk, dest) pair
     uint64_t* st_free = nullptr;
     uint32_t* st_inf = nullptr;
     uint32_t Wp = 0, S = 0, nLw = 0, SWp = 0;
@@ -825,6 +826,7 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.SWp = (uint32_t)align_up((W.Wp / 4 + 63) / 64, 2);          // one summary bit per 4-word sector
     if (loop_smem_bytes(W.S) > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
     Carver c;
+    const size_t o_drow = c.take(max_pairs * 4);
     const size_t o_best = c.take(max_pairs * 8), o_sf = c.take(L * 2 * 8), o_si = c.take(L * 2 * 4);
     const size_t o_w = c.take(L * 8), o_D = c.take(max_sources * N * 8), o_free = c.take(L * 8),
                  o_mb = c.take((size_t)3 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4),
@@ -841,7 +843,7 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.empty_epoch = (uint32_t*)(b + o_ee); W.have = (uint64_t*)(b + o_have); W.wants = (uint64_t*)(b + o_wants);
     W.hsum = (uint64_t*)(b + o_hs); W.wsum = (uint64_t*)(b + o_ws);
     W.gcnt = (uint32_t*)(b + o_gc); W.gtot = (uint32_t*)(b + o_gt);
-    W.best = (uint64_t*)(b + o_best);
+    W.best = (uint64_t*)(b + o_best); W.drow = (uint32_t*)(b + o_drow);
     W.hold = (uint32_t*)(b + o_hold); W.hold_cnt = (uint32_t*)(b + o_hc);
     W.st_free = (uint64_t*)(b + o_sf); W.st_inf = (uint32_t*)(b + o_si);
     W.wants_cnt = (uint32_t*)(b + o_wc); W.ctrl = (LoopCtrl*)(b + o_ctrl);
@@ -849,14 +851,14 @@ int work_alloc(const pccl_problem& P, Work& W) {
 }
 
 struct PhaseView {   // link tables in the synthesized direction
-    const uint32_t *esrc, *edst, *in_off, *in_link, *out_link, *out_far, *lo_off, *lo_deg, *out_off;
+    const uint32_t *esrc, *edst, *in_off, *in_link, *out_link, *out_far, *lo_off, *lo_deg, *out_off, *in_far;
 };
 PhaseView view_of(const pccl_topology* t, bool transposed) {
     if (!transposed)
         return {t->d_src, t->d_dst, t->d_in_off, t->d_in_link, t->d_out_link, t->d_out_far, t->d_lo_off_n, t->d_lo_deg_n,
-                t->d_out_off};
+                t->d_out_off, t->d_in_far};
     return {t->d_dst, t->d_src, t->d_out_off, t->d_out_link, t->d_in_link, t->d_in_far, t->d_lo_off_t, t->d_lo_deg_t,
-            t->d_in_off};
+            t->d_in_off, t->d_out_far};
 }
 
 // steps A..C; on return the wants total is in *M (synchronises the stream)
@@ -878,7 +880,7 @@ int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t 
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         if (NDS) k_distances<<<NDS, 256, smem, st>>>(pv.edst, pv.esrc, W.w, N, L, ph.d_dsts, W.D);
         if (NP) k_best_init<<<(unsigned)((NP + 255) / 256), 256, 0, st>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, NP, ph.d_didx,
-                                                                         W.D, N, W.best, &W.ctrl->err);
+                                                                         W.D, N, W.best, W.drow, &W.ctrl->err);
         if (C) k_have<<<(C + 255) / 256, 256, 0, st>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
         const uint64_t nth = (uint64_t)N * ((C + 63) / 64);   // warps: one per (node, 64-chunk word)
         if (nth > (0x7FFFFFFFull << 2)) return PCCL_ERR_UNSUPPORTED;
@@ -949,7 +951,7 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     a.out_cap = out_cap;
     // dynamic rule with kept counts: a tightened best revisits only the out-neighbours of the chunk's holders
     const bool lazy = dynamic && !(flags & (PCCL_FLAG_RESCAN | PCCL_FLAG_DENSE_SWEEP));
-    a.csrc = ph.d_cond_src; a.out_off = pv.out_off;
+    a.csrc = ph.d_cond_src; a.out_off = pv.out_off; a.drow = W.drow; a.in_far = pv.in_far;
     a.hold = lazy ? W.hold : nullptr; a.hold_cnt = lazy ? W.hold_cnt : nullptr;
     a.best = dynamic ? W.best : nullptr; a.Dto = W.D; a.didx = ph.d_didx; a.dest_off = ph.d_dest_off; a.dests = ph.d_dests;
     cudaStream_t st = G.stream;

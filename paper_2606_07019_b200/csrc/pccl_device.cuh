@@ -203,10 +203,12 @@ __global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* _
 __global__ void k_best_init(const uint32_t* __restrict__ cond_src, const uint32_t* __restrict__ dests,
                             const uint32_t* __restrict__ dchunk, uint64_t n_pairs,
                             const uint32_t* __restrict__ didx, const uint64_t* __restrict__ Dto, uint32_t N,
-                            uint64_t* __restrict__ best, uint32_t* __restrict__ err) {
+                            uint64_t* __restrict__ best, uint32_t* __restrict__ drow, uint32_t* __restrict__ err) {
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n_pairs) return;
-    const uint64_t d0 = Dto[(size_t)didx[dests[p]] * N + cond_src[dchunk[p]]];
+    const uint32_t row = didx[dests[p]];
+    drow[p] = row;
+    const uint64_t d0 = Dto[(size_t)row * N + cond_src[dchunk[p]]];
     if (d0 == T_INF) atomicOr(err, 1u);
     best[p] = d0;
 }
@@ -349,6 +351,8 @@ struct LoopArgs {
     uint32_t trace_cap;     // events the trace buffer holds
     // dynamic rule with kept counts: the holders of each chunk (nodes whose have bit is stored), so that a tightened
     // best only revisits the out-neighbours of holders (null: every node is revisited)
+    const uint32_t* drow;       // [pairs] didx[dests[p]]: the pair's row of Dto
+    const uint32_t* in_far;     // per in-link table entry: the link's source (esrc[in_link[e]])
     const uint32_t* csrc;       // [C] source of each chunk
     const uint32_t* out_off;    // [N+1] per-node offsets into out_link / out_far
     uint32_t* hold_cnt;         // [C] arrivals of the chunk so far
@@ -448,7 +452,7 @@ __device__ __forceinline__ uint32_t kth_bit128(uint4 m, uint32_t k) {
 __device__ __forceinline__ bool dyn_still_wants(const LoopArgs& a, uint32_t u, uint32_t c) {
     const uint64_t p1 = a.dest_off[c + 1];
     for (uint64_t p = a.dest_off[c]; p < p1; ++p)
-        if (a.Dto[(size_t)a.didx[a.dests[p]] * a.N + u] < ldcg64(a.best + p)) return true;
+        if (a.Dto[(size_t)a.drow[p] * a.N + u] < ldcg64(a.best + p)) return true;
     return false;
 }
 
@@ -548,12 +552,16 @@ __device__ __forceinline__ void dyn_drop(const LoopArgs& a, uint32_t u, uint32_t
     if (a.gcnt == nullptr) return;
     const uint32_t e1 = a.in_off[u + 1];
     for (uint32_t eb = a.in_off[u]; eb < e1; eb += 4) {   // four in-links per round: table, source, have word
-        uint32_t l2[4];
+        uint32_t l2[4], u2[4];
         unsigned long long hw[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) l2[k] = (eb + k < e1) ? a.in_link[eb + k] : NONE32;
+        for (int k = 0; k < 4; ++k) {
+            const bool in = eb + k < e1;
+            l2[k] = in ? a.in_link[eb + k] : NONE32;
+            u2[k] = in ? a.in_far[eb + k] : 0u;
+        }
 #pragma unroll
-        for (int k = 0; k < 4; ++k) hw[k] = (l2[k] != NONE32) ? ldcg64(a.have + (size_t)a.esrc[l2[k]] * a.Wp + (c >> 6)) : 0ull;
+        for (int k = 0; k < 4; ++k) hw[k] = (l2[k] != NONE32) ? ldcg64(a.have + (size_t)u2[k] * a.Wp + (c >> 6)) : 0ull;
 #pragma unroll
         for (int k = 0; k < 4; ++k)
             if ((hw[k] >> (c & 63)) & 1ull) {
@@ -573,7 +581,7 @@ __device__ __forceinline__ void dyn_shrink_chunk(const LoopArgs& a, uint32_t c, 
         const uint32_t np = (uint32_t)(p1 - p0);
         uint32_t row = 0;
         unsigned long long bst = 0;
-        if (lane < np) { row = a.didx[a.dests[p0 + lane]]; bst = ldcg64(a.best + p0 + lane); }
+        if (lane < np) { row = a.drow[p0 + lane]; bst = ldcg64(a.best + p0 + lane); }
         for (uint32_t ub = 0; ub < a.N; ub += 128) {
             bool need[4], keep[4];
 #pragma unroll
@@ -624,7 +632,7 @@ __device__ __forceinline__ void dyn_shrink_wants(const LoopArgs& a, uint32_t ste
         const uint32_t np = (uint32_t)(p1 - p0);
         uint32_t row = 0;               // lane q: pair q of c (row of its dest in Dto, current best)
         unsigned long long bst = 0;
-        if (lane < np) { row = a.didx[a.dests[p0 + lane]]; bst = ldcg64(a.best + p0 + lane); }
+        if (lane < np) { row = a.drow[p0 + lane]; bst = ldcg64(a.best + p0 + lane); }
         uint32_t off = 0, deg = 0;      // the holders' out-links, flattened over the warp
         if (u != NONE32) { off = a.out_off[u]; deg = a.out_off[u + 1] - off; }
         const uint32_t incl = warp_incl_scan(deg, lane);
@@ -746,7 +754,7 @@ __device__ __forceinline__ void commit_best(const LoopArgs& a, uint32_t v, uint3
     if (a.best == nullptr) return;
     const uint64_t p1 = a.dest_off[c + 1];
     for (uint64_t p = a.dest_off[c]; p < p1; ++p)
-        atomicMin((unsigned long long*)&a.best[p], (unsigned long long)a.Dto[(size_t)a.didx[a.dests[p]] * a.N + v]);
+        atomicMin((unsigned long long*)&a.best[p], (unsigned long long)a.Dto[(size_t)a.drow[p] * a.N + v]);
 }
 
 __device__ __forceinline__ uint64_t commit_claim(const LoopArgs& a, uint32_t v, uint32_t l, uint64_t wl, uint32_t c,
