@@ -972,7 +972,134 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
             trace_stamp(a, step, 5);
             // a7: conflict resolve.  In-links are served in ascending link id, each seeing the earlier
             // claims.  Link j's speculative pick stands iff no earlier claim is a candidate of j.
-            if (warp == 0) {
+            if (warp == 0 && dc != nullptr && a.gcnt != nullptr) {
+                // <= 32 in-links, tables in shared memory, kept counts.  The picks are settled prefix by prefix: the
+                // longest run of picks that no earlier final pick invalidates is committed at once; the first
+                // invalidated link re-picks exactly (it is the first unsettled one), its new pick replaces its
+                // speculative one in the test, and the links after it keep their speculative picks unless THAT
+                // invalidates them.  Same result as serving the links one by one.
+                st.rows += nb + 1;
+                st.links += nb;
+                // H[i] (sh.pbits[i]): mask over the in-links of v whose source holds pick i -- one load per (pick,
+                // in-link); serves the test and the count upkeep
+                if (lane < NBT) sh.pbits[lane] = 0;
+                __syncwarp();
+                const uint32_t npairs = nb * e1;
+                for (uint32_t p0 = 0; p0 < npairs; p0 += 64) {   // two pairs per lane and round, loads first
+                    const uint32_t pa = p0 + lane, pb = p0 + 32 + lane;
+                    uint32_t ia = 0, ea = 0, ib = 0, eb2 = 0, ca = NONE32, cb = NONE32;
+                    unsigned long long wa = 0, wb = 0;
+                    if (pa < npairs) { ia = pa / e1; ea = pa - ia * e1; ca = sh.spec[ia]; }
+                    if (pb < npairs) { ib = pb / e1; eb2 = pb - ib * e1; cb = sh.spec[ib]; }
+                    if (ca != NONE32) wa = ldcg64(a.have + (size_t)dc->src[ea] * a.Wp + (ca >> 6));
+                    if (cb != NONE32) wb = ldcg64(a.have + (size_t)dc->src[eb2] * a.Wp + (cb >> 6));
+                    if (ca != NONE32 && ((wa >> (ca & 63)) & 1ull)) atomicOr(&sh.pbits[ia], 1u << ea);
+                    if (cb != NONE32 && ((wb >> (cb & 63)) & 1ull)) atomicOr(&sh.pbits[ib], 1u << eb2);
+                }
+                __syncwarp();
+                if (lane == 0) st.bytes += (unsigned long long)nb * e1 * 32u;
+                trace_stamp(a, step, 8);
+                const uint32_t ej = (lane < nb) ? sh.acte[b0 + lane] : 0u;
+                uint32_t wc = sh.wc, ncl = 0, done = 0, repicked = 0;
+                while (done < nb) {
+                    // the first unsettled link whose source holds an earlier pick (sh.spec holds the final pick of every
+                    // settled link and the speculative one of the others)
+                    bool isbad = false;
+                    if (lane >= done && lane < nb)
+                        for (uint32_t i = 0; i < lane; ++i)
+                            if (sh.spec[i] != NONE32 && ((sh.pbits[i] >> ej) & 1u)) isbad = true;
+                    const uint32_t bm = __ballot_sync(0xFFFFFFFFu, isbad);
+                    const uint32_t fb = bm ? (uint32_t)(__ffs(bm) - 1) : nb;
+                    // commit [done, fb): one lane per link
+                    {
+                        const bool mine = lane >= done && lane < fb;
+                        uint32_t c = NONE32, l = 0;
+                        if (mine) { c = sh.spec[lane]; l = sh.act[b0 + lane]; }
+                        const uint32_t cm = __ballot_sync(0xFFFFFFFFu, c != NONE32);
+                        if (mine) {
+                            if (c != NONE32) {
+                                const uint64_t te = commit_claim(a, v, l, sh.actw[b0 + lane], c, sh.sempty[lane] != 0u, step, t);
+                                mymin = min(mymin, te);
+                                mymax = max(mymax, te);
+                                sh.claimed[ncl + __popc(cm & ((1u << lane) - 1u))] = c;
+                            } else {
+                                stcg32(a.empty_epoch + l, step + 1);
+                            }
+                        }
+                        ncl += __popc(cm);
+                        wc -= __popc(cm);
+                        __syncwarp();
+                        if (lane < e1) {   // count upkeep for these picks: lane e owns in-link e of v
+                            const uint32_t l2 = dc->link[lane];
+                            uint32_t dec = 0;
+                            for (uint32_t i = done; i < fb; ++i) {
+                                const uint32_t ci = sh.spec[i];
+                                if (ci != NONE32 && ((sh.pbits[i] >> lane) & 1u)) {
+                                    atomicSub(&a.gcnt[(size_t)l2 * S + (ci >> 12)], 1u);
+                                    ++dec;
+                                }
+                            }
+                            if (dec) atomicSub(&a.gtot[l2], dec);
+                        }
+                    }
+                    if (fb >= nb) break;
+                    if (wc == 0) break;   // v wants nothing more: no later link can have a candidate
+                    // link fb re-picks against the wants row net of the claims so far
+                    if (lane == 0) ++st.slow;
+                    const uint32_t j = fb;
+                    const uint32_t l = sh.act[b0 + j], u = sh.src[b0 + j], ejj = sh.acte[b0 + j];
+                    uint32_t* cj = cnt + j * S;
+                    if (lane < j) {   // earlier final picks held by u leave its counts (H says which: no load)
+                        const uint32_t ci = sh.spec[lane];
+                        if (ci != NONE32 && ((sh.pbits[lane] >> ejj) & 1u)) atomicSub(&cj[ci >> 12], 1u);
+                    }
+                    __syncwarp();
+                    const uint32_t n = warp_sum_counts(cj, S, lane);
+                    uint32_t cnew = NONE32;
+                    if (n == 0) {
+                        if (lane == 0) stcg32(a.empty_epoch + l, step + 1);
+                    } else {
+                        const uint32_t r = philox_draw((uint32_t)t, (uint32_t)(t >> 32), l, 0u, a.k0, a.k1);
+                        bool sem = false;
+                        cnew = kth_candidate(cj, S, Q, have4 + (size_t)u * Q, wrow, __umulhi(r, n), sh.claimed, ncl, lane, sem);
+                        if (cnew == NONE32) {   // cannot happen; fail loudly instead of corrupting
+                            if (lane == 0) atomicOr(&a.ctrl->err, 4u);
+                        } else {
+                            if (lane == 0) {
+                                sh.claimed[ncl] = cnew;
+                                const uint64_t te = commit_claim(a, v, l, sh.actw[b0 + j], cnew, sem, step, t, false);
+                                mymin = min(mymin, te);
+                                mymax = max(mymax, te);
+                            }
+                            repicked |= 1u << ncl;
+                            ++ncl;
+                            --wc;
+                        }
+                    }
+                    // the new pick's holders among the in-links of v: the next test and its count upkeep
+                    bool holds = false;
+                    if (cnew != NONE32 && lane < e1)
+                        holds = ((ldcg64(a.have + (size_t)dc->src[lane] * a.Wp + (cnew >> 6)) >> (cnew & 63)) & 1ull) != 0ull;
+                    const uint32_t hm = __ballot_sync(0xFFFFFFFFu, holds);
+                    if (holds) {
+                        atomicSub(&a.gcnt[(size_t)dc->link[lane] * S + (cnew >> 12)], 1u);
+                        atomicSub(&a.gtot[dc->link[lane]], 1u);
+                    }
+                    if (lane == 0) {
+                        sh.spec[j] = cnew;
+                        sh.pbits[j] = hm;
+                        if (cnew != NONE32) st.bytes += (unsigned long long)e1 * 32u;
+                    }
+                    __syncwarp();
+                    done = j + 1;
+                }
+                // the best[] updates of re-picked claims are off the serial chain: one lane per claim
+                if (lane < ncl && ((repicked >> lane) & 1u)) commit_best(a, v, sh.claimed[lane]);
+                trace_stamp(a, step, 10);
+                if (lane == 0) sh.wc = wc;
+                // another sweep of this destination follows: its loads must see the wants bits just cleared
+                if (b0 + NBT < nact || eb + 32 < e1) __threadfence();
+            } else if (warp == 0) {
                 st.rows += nb + 1;
                 st.links += nb;
                 uint32_t bad = 0;
