@@ -981,7 +981,8 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     for (int attempt = 0; attempt < 2; ++attempt) {
         // one-barrier loop: teams of 4 warps are paired in 256-thread CTAs (half as many CTAs at the barrier)
         kern = fast ? (small ? (const void*)k_loop1<4, 2> : (const void*)k_loop1<8, 1>)
-                    : (small ? (const void*)k_loop<4> : (const void*)k_loop<8>);
+                    : (dynamic ? (small ? (const void*)k_loop<4, true> : (const void*)k_loop<8, true>)
+                               : (small ? (const void*)k_loop<4, false> : (const void*)k_loop<8, false>));
         const int teams = (fast && small) ? 2 : 1;
         threads = (small ? 128 : 256) * teams;
         smem = loop_smem_bytes(W.S, small ? 4 : 8) * teams;

@@ -457,6 +457,7 @@ __device__ __forceinline__ bool dyn_still_wants(const LoopArgs& a, uint32_t u, u
 }
 
 // ---- P1: ordered emit of the previous event's matches (a8) + arrivals at time t (a3) ---------------
+template <bool DYN>
 __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t step, uint64_t t,
                                                  uint64_t emit_base) {
     const uint32_t lane = threadIdx.x & 31;
@@ -497,7 +498,7 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
             atomicOr((unsigned long long*)&a.have[(size_t)d * a.Wp + (c >> 6)], 1ull << (c & 63));
             atomicOr((unsigned long long*)&a.hsum[(size_t)d * a.SWp + (c >> 14)], 1ull << ((c >> 8) & 63));
             stcg32(a.have_epoch + d, step + 1);   // (inflight keeps the chunk: free_t == t holds at this event only)
-            if (a.hold != nullptr) {
+            if (DYN && a.hold != nullptr) {
                 const uint32_t k = atomicAdd(a.hold_cnt + c, 1u) + 1u;
                 if (k <= HOLD_CAP) stcg32(a.hold + (size_t)c * HOLD_ROW + k, d);
             }
@@ -519,7 +520,7 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
             for (uint32_t k = k0; k < deg; k += K) {
                 const uint32_t o = a.out_link[off + k], v2 = a.out_far[off + k];
                 if ((ldcg64(a.wants + (size_t)v2 * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) {
-                    if (a.hold != nullptr && !dyn_still_wants(a, v2, c)) {
+                    if (DYN && a.hold != nullptr && !dyn_still_wants(a, v2, c)) {
                         // lazy dynamic rule: v2 stopped wanting c while no neighbour held it; the bit goes now, and no
                         // count can include it (a neighbour that held c would have had it cleared at the tightening)
                         const unsigned long long bit = 1ull << (c & 63);
@@ -750,13 +751,15 @@ __device__ __forceinline__ uint32_t warp_sum_counts(const uint32_t* cj, uint32_t
 
 // a8: link l carries chunk c over [t, t + w_l); destination v no longer wants c
 // dynamic relay rule: v becomes a holder of c, best[p] of c's pairs tightens (read only after the event's barrier)
+template <bool DYN>
 __device__ __forceinline__ void commit_best(const LoopArgs& a, uint32_t v, uint32_t c) {
-    if (a.best == nullptr) return;
+    if (!DYN || a.best == nullptr) return;
     const uint64_t p1 = a.dest_off[c + 1];
     for (uint64_t p = a.dest_off[c]; p < p1; ++p)
         atomicMin((unsigned long long*)&a.best[p], (unsigned long long)a.Dto[(size_t)a.drow[p] * a.N + v]);
 }
 
+template <bool DYN>
 __device__ __forceinline__ uint64_t commit_claim(const LoopArgs& a, uint32_t v, uint32_t l, uint64_t wl, uint32_t c,
                                                  bool sector_empty, uint32_t step, uint64_t t, bool tighten = true) {
     const uint64_t te = t + wl;
@@ -768,7 +771,7 @@ __device__ __forceinline__ uint64_t commit_claim(const LoopArgs& a, uint32_t v, 
     stcg32(a.inflight + l, c);
     stcg64(a.free_t + l, te);
     atomicOr((unsigned long long*)&a.matchbits[(size_t)(step & 1) * a.nLw + (l >> 6)], 1ull << (l & 63));
-    if (tighten) commit_best(a, v, c);
+    if (tighten) commit_best<DYN>(a, v, c);
     return te;
 }
 
@@ -781,7 +784,7 @@ struct DestCache {
     uint64_t w[32];
 };
 
-template <int NBT>
+template <int NBT, bool DYN>
 __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v, uint32_t step, uint64_t t,
                                                   uint32_t* cnt, uint32_t* list, CtaScratch& sh, LoopStats& st,
                                                   const DestCache* dc) {
@@ -1018,7 +1021,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                         const uint32_t cm = __ballot_sync(0xFFFFFFFFu, c != NONE32);
                         if (mine) {
                             if (c != NONE32) {
-                                const uint64_t te = commit_claim(a, v, l, sh.actw[b0 + lane], c, sh.sempty[lane] != 0u, step, t);
+                                const uint64_t te = commit_claim<DYN>(a, v, l, sh.actw[b0 + lane], c, sh.sempty[lane] != 0u, step, t);
                                 mymin = min(mymin, te);
                                 mymax = max(mymax, te);
                                 sh.claimed[ncl + __popc(cm & ((1u << lane) - 1u))] = c;
@@ -1067,7 +1070,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                         } else {
                             if (lane == 0) {
                                 sh.claimed[ncl] = cnew;
-                                const uint64_t te = commit_claim(a, v, l, sh.actw[b0 + j], cnew, sem, step, t, false);
+                                const uint64_t te = commit_claim<DYN>(a, v, l, sh.actw[b0 + j], cnew, sem, step, t, false);
                                 mymin = min(mymin, te);
                                 mymax = max(mymax, te);
                             }
@@ -1094,7 +1097,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     done = j + 1;
                 }
                 // the best[] updates of re-picked claims are off the serial chain: one lane per claim
-                if (lane < ncl && ((repicked >> lane) & 1u)) commit_best(a, v, sh.claimed[lane]);
+                if (lane < ncl && ((repicked >> lane) & 1u)) commit_best<DYN>(a, v, sh.claimed[lane]);
                 trace_stamp(a, step, 10);
                 if (lane == 0) sh.wc = wc;
                 // another sweep of this destination follows: its loads must see the wants bits just cleared
@@ -1151,7 +1154,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     const uint32_t cm = __ballot_sync(0xFFFFFFFFu, c != NONE32);
                     if (lane < first_bad) {
                         if (c != NONE32) {
-                            const uint64_t te = commit_claim(a, v, l, sh.actw[b0 + lane], c, sh.sempty[lane] != 0u, step, t);
+                            const uint64_t te = commit_claim<DYN>(a, v, l, sh.actw[b0 + lane], c, sh.sempty[lane] != 0u, step, t);
                             mymin = min(mymin, te);
                             mymax = max(mymax, te);
                             sh.claimed[__popc(cm & ((1u << lane) - 1u))] = c;
@@ -1203,7 +1206,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     }
                     if (lane == 0) {
                         sh.claimed[ncl] = c;
-                        const uint64_t te = commit_claim(a, v, l, sh.actw[b0 + j], c, sem, step, t, false);
+                        const uint64_t te = commit_claim<DYN>(a, v, l, sh.actw[b0 + j], c, sem, step, t, false);
                         mymin = min(mymin, te);
                         mymax = max(mymax, te);
                     }
@@ -1212,7 +1215,7 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
                     __syncwarp();
                 }
                 // (their best[] updates are off the serial chain: one lane per re-picked claim)
-                if (lane >= ncl_spec && lane < ncl) commit_best(a, v, sh.claimed[lane]);
+                if (lane >= ncl_spec && lane < ncl) commit_best<DYN>(a, v, sh.claimed[lane]);
                 trace_stamp(a, step, 10);
                 const uint32_t dec0 = fastpairs ? ncl_spec : 0u;   // claims before dec0 were handled above
                 if (a.gcnt != nullptr && ncl > dec0) {
@@ -1258,7 +1261,9 @@ __device__ __forceinline__ void match_destination(const LoopArgs& a, uint32_t v,
     __syncthreads();
 }
 
-template <int NBT>
+// DYN: the dynamic relay rule's code (best[], holder lists, the wants-shrink phase) is compiled in; the thin-tree
+// instantiation stays lean
+template <int NBT, bool DYN>
 __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop(const LoopArgs a) {
     constexpr int THREADS = NBT * 32;
     extern __shared__ __align__(16) uint32_t cnt[];   // [NBT][S] candidate counts per segment, then the work list
@@ -1288,7 +1293,7 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop(const Loop
     __shared__ unsigned long long s_next[2];   // one thread per CTA reads the two hot words after a barrier
     for (;;) {
         trace_stamp(a, step, 0);
-        loop_phase_links(a, step, t, emit_base);
+        loop_phase_links<DYN>(a, step, t, emit_base);
         emit_base = total_now;
         trace_stamp(a, step, 1);
         grid.sync();
@@ -1296,7 +1301,7 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop(const Loop
         {
             uint32_t k = 0;
             for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x, ++k)
-                match_destination<NBT>(a, v, step, t, cnt, list, sh, st,
+                match_destination<NBT, DYN>(a, v, step, t, cnt, list, sh, st,
                                   (k < DEST_CACHE && dcache[k].n_in != NONE32) ? &dcache[k] : nullptr);
         }
         trace_stamp(a, step, 6);
@@ -1310,7 +1315,7 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop(const Loop
         t = s_next[0];
         total_now = s_next[1];
         __syncthreads();
-        if (a.best != nullptr && t != T_INF) {   // (the last event never has claims)
+        if (DYN && a.best != nullptr && t != T_INF) {   // (the last event never has claims)
             dyn_shrink_wants(a, step);
             trace_stamp(a, step, 10);
             grid.sync();
