@@ -25,8 +25,9 @@
  *   - Several concurrent process groups go in ONE call: group_members is their union, chunk
  *     ids are globally unique.
  *   - Device work is enqueued on the stream set with pccl_set_stream (default: the legacy
- *     default stream) of the CUDA device that is current when the handle is created, and is
- *     synchronised before a function returns host-visible results.
+ *     default stream) and is synchronised before a function returns host-visible results.
+ *     The library binds to the CUDA device that is current at its first device call; a later
+ *     call made with another device current returns PCCL_ERR_INVALID.
  *   - Calls on distinct handles may come from different threads: the entry points that touch the
  *     device serialise themselves (one runs at a time; they share a control mailbox, a copy
  *     stream and the stream below).  A single handle must not be used from two threads at once.
@@ -108,6 +109,20 @@ void pccl_set_allocator(pccl_alloc_fn alloc, pccl_free_fn release, void* user);
 
 const char* pccl_strerror(int err);
 int pccl_version(void);
+
+/* Process-wide tuning options (everything is an argument of the C-ABI: the library reads no environment variables
+ * and no files).  value 0 restores the default.  Errors: INVALID (unknown option). */
+typedef enum pccl_option {
+    PCCL_OPT_BFS_WINDOW = 1,   /* PCCL_FLAG_BFS: conditions searched optimistically per round (default: one per SM) */
+    PCCL_OPT_BFS_ROWS = 2      /* PCCL_FLAG_BFS: initial capacity of a link's busy-run row, in runs (default: 256 or
+                                  more; a full row reruns the phase with 4x longer rows) */
+} pccl_option;
+int pccl_set_option(int option, uint64_t value);
+uint64_t pccl_get_option(int option);
+
+/* Number of CUDA kernels the library has launched in this process so far (every launch is counted where it is
+ * issued).  The difference across a region is the library's own count of its GPU work there. */
+uint64_t pccl_launch_count(void);
 
 /* ---------------------------------------------------------------------------------------
  * Topology store (DESIGN.md row a0 and the link/in-link tables).
@@ -192,6 +207,19 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
                                         slow_picks = commit rounds.  UNSUPPORTED if a time does not fit in
                                         64 - ceil(log2(n_links)) bits or n_npus > 8,500. */
 
+#define PCCL_FLAG_BARRIER_LOOP 1024u  /* run the barrier loops (one grid barrier per event where that loop applies, else
+                                        two) even where the barrier-free loop applies */
+#define PCCL_FLAG_ASYNC 2048u        /* run the barrier-free loop (one warp per destination, pairwise synchronisation
+                                        through per-node claim logs) even when the link costs differ
+                                        by more than 16x -- its lookahead is the cheapest in-link of a node, so idle
+                                        regions then advance in small time steps.  It is the default for the static
+                                        relay tree when every node has at most 8 in-links, at most 16 x SM-count nodes,
+                                        and link costs within 16x of each other */
+
+#define PCCL_FLAG_LSU_SWEEP 4096u    /* the streaming candidate sweep (row a5: seeds the kept counts of the barrier loops;
+                                        pccl_device_candidate_sweep) loads its rows with per-lane 128-bit loads instead of
+                                        staging them in shared memory by bulk asynchronous copies (TMA) */
+
 /* Steps A..F on the GPU for one seed.  Errors: UNREACHABLE, CUDA, NOMEM, INTERNAL. */
 int pccl_problem_synthesize(pccl_problem_t* problem, uint64_t seed, uint32_t flags,
                             pccl_schedule_t** out);
@@ -268,6 +296,18 @@ int pccl_device_distances(pccl_topology_t* topo, uint64_t chunk_bytes, uint32_t 
  * negative pccl_error.  out: host. */
 int64_t pccl_device_wants(pccl_problem_t* problem, uint32_t phase, uint64_t seed,
                           pccl_pair_t* out, uint64_t cap);
+
+/* a5: the candidate bitmap of every link, cand(l) = have[src_l] & wants[dst_l], at t = 0 (after steps A..C for `seed`),
+ * by the streaming sweep kernel alone: (N + L) bitmap rows per sweep, rows staged in shared memory by bulk asynchronous
+ * copies (PCCL_FLAG_LSU_SWEEP: per-lane 128-bit loads).  Runs `iters` sweeps between two CUDA events.
+ * ms_per_sweep, bytes_per_sweep (algorithmic bytes of one sweep: rows x padded row bytes) and totals (host, n_links u32:
+ * |cand(l)|) may each be NULL.  Errors: INVALID, UNREACHABLE, CUDA, NOMEM. */
+int pccl_device_candidate_sweep(pccl_problem_t* problem, uint32_t phase, uint64_t seed, uint32_t flags, uint32_t iters,
+                                float* ms_per_sweep, uint64_t* bytes_per_sweep, uint32_t* totals);
+/* Measurement aid: reads a device buffer of `bytes` bytes sequentially with the sweeps' access pattern (128-bit
+ * ld.global.cg, grid-stride) `iters` times and reports the milliseconds per pass: the measured ceiling of L2 when the
+ * buffer fits there, of HBM when it does not.  Errors: INVALID, CUDA, NOMEM. */
+int pccl_device_read_bandwidth(uint64_t bytes, uint32_t iters, float* ms_per_pass);
 
 #ifdef __cplusplus
 }

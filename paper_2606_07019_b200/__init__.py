@@ -35,7 +35,11 @@ PCCL_FLAG_DYNAMIC_RELAY = 64
 PCCL_FLAG_KEPT_COUNTS = 128
 PCCL_FLAG_TWO_BARRIERS = 256
 PCCL_FLAG_BFS = 512
+PCCL_FLAG_BARRIER_LOOP = 1024
+PCCL_FLAG_ASYNC = 2048
+PCCL_FLAG_LSU_SWEEP = 4096
 PCCL_TRACE_SLOTS = 12
+PCCL_OPT_BFS_WINDOW, PCCL_OPT_BFS_ROWS = 1, 2
 
 
 class pccl_condition_t(C.Structure):
@@ -59,6 +63,9 @@ SIGNATURES = {
     "pccl_set_allocator": (None, [pccl_alloc_fn, pccl_free_fn, _vp]),
     "pccl_strerror": (C.c_char_p, [_int]),
     "pccl_version": (_int, []),
+    "pccl_set_option": (_int, [_int, _u64]),
+    "pccl_get_option": (_u64, [_int]),
+    "pccl_launch_count": (_u64, []),
     "pccl_topology_create": (_int, [_u32, _vp, _u32, C.POINTER(_vp)]),
     "pccl_topology_destroy": (None, [_vp]),
     "pccl_topology_n_npus": (_u32, [_vp]),
@@ -85,6 +92,8 @@ SIGNATURES = {
     "pccl_device_link_costs": (_int, [_vp, _u64, _vp]),
     "pccl_device_distances": (_int, [_vp, _u64, _u32, _int, _vp]),
     "pccl_device_wants": (_i64, [_vp, _u32, _u64, _vp, _u64]),
+    "pccl_device_candidate_sweep": (_int, [_vp, _u32, _u64, _u32, _u32, C.POINTER(C.c_float), C.POINTER(_u64), _vp]),
+    "pccl_device_read_bandwidth": (_int, [_u64, _u32, C.POINTER(C.c_float)]),
 }
 
 
@@ -153,6 +162,15 @@ def use_torch(device: int | None = None) -> None:
     _hooks = (pccl_alloc_fn(_alloc), pccl_free_fn(_free))
     lib.pccl_set_allocator(_hooks[0], _hooks[1], None)
     lib.pccl_set_stream(C.c_void_p(torch.cuda.current_stream().cuda_stream))
+
+
+def set_option(option: int, value: int) -> None:
+    _check(lib.pccl_set_option(option, value))
+
+
+def launch_count() -> int:
+    """Kernels the library has launched so far in this process."""
+    return int(lib.pccl_launch_count())
 
 
 def sync_stream() -> None:
@@ -287,6 +305,13 @@ class Problem:
             raise PcclError(PCCL_ERR_INTERNAL if m >= 0 else int(m))
         return out
 
+    def candidate_sweep(self, phase: int, seed: int, flags: int = 0, iters: int = 1):
+        """(ms per sweep, algorithmic bytes per sweep, |cand(l)| of every link at t = 0)."""
+        ms, nbytes = C.c_float(), C.c_uint64()
+        tot = np.zeros(self.topo.n_links, dtype=np.uint32)
+        _check(lib.pccl_device_candidate_sweep(self.handle, phase, seed, flags, iters, C.byref(ms), C.byref(nbytes), _ptr(tot)))
+        return float(ms.value), int(nbytes.value), tot
+
     def close(self):
         if getattr(self, "handle", None) and lib is not None:
             lib.pccl_problem_destroy(self.handle)
@@ -309,6 +334,13 @@ def synthesize(n_npus, links, group, n_chunks, pre, post, chunk_bytes, seed) -> 
         return Schedule(h)
     finally:
         topo.close()
+
+
+def read_bandwidth_gbs(nbytes: int, iters: int = 20) -> float:
+    """GB/s of a sequential 128-bit read of an nbytes device buffer (L2-resident or not, by its size)."""
+    ms = C.c_float()
+    _check(lib.pccl_device_read_bandwidth(nbytes, iters, C.byref(ms)))
+    return nbytes / (ms.value * 1e-3) / 1e9
 
 
 def device_philox(ctr, key) -> np.ndarray:

@@ -9,11 +9,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpccl.so")
 SOURCES = ["pccl_api.cu"]
-DEPS = ["pccl_api.cu", "pccl_device.cuh", "pccl_loop1.cuh", "pccl_bfs.cuh", os.path.join("..", "..", "include", "pccl.h")]
+DEPS = ["pccl_api.cu", "pccl_device.cuh", "pccl_loop1.cuh", "pccl_loop2.cuh", "pccl_sweep.cuh", "pccl_bfs.cuh", os.path.join("..", "..", "include", "pccl.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "-shared", "-Xptxas", "-v",
+    "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "-shared", "-Xptxas", "-v", "-ldl",
 ]
 
 

@@ -18,8 +18,12 @@
 #include <unordered_set>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "pccl_device.cuh"
 #include "pccl_loop1.cuh"
+#include "pccl_loop2.cuh"
+#include "pccl_sweep.cuh"
 #include "pccl_bfs.cuh"
 
 using namespace pccl;
@@ -51,7 +55,14 @@ struct Globals {
     // polling host thread watches
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t loop_done = nullptr;
+    std::atomic<uint64_t> launches{0};   // kernels launched by the library (pccl_launch_count)
+    // process-wide options (pccl_set_option); 0 = default
+    std::atomic<uint64_t> opt_bfs_window{0}, opt_bfs_rows{0};
 } G;
+
+// every kernel launch of the library passes its stream through here: the count is the library's own evidence of what
+// ran on the device (bench.py reports it as gpu_launches)
+inline cudaStream_t counted(cudaStream_t s) { G.launches.fetch_add(1, std::memory_order_relaxed); return s; }
 
 #define SERIALISE std::lock_guard<std::recursive_mutex> call_lock__(G.call_mu)
 
@@ -87,20 +98,29 @@ void dev_free(void* p) {
     else if (cudaFreeAsync(p, G.stream) != cudaSuccess) (void)cudaGetLastError();
 }
 
+// The library binds to the CUDA device that is current at its first device call (mailbox, copy stream, SM count);
+// a later call with another current device is refused instead of mixing contexts.
 int ensure_device() {
-    if (G.dev >= 0) return PCCL_OK;
     int dev = 0;
     CU(cudaGetDevice(&dev));
-    int sms = 0;
+    if (G.dev >= 0) return dev == G.dev ? PCCL_OK : PCCL_ERR_INVALID;
+    int sms = 0, coop = 0;
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    int coop = 0;
     CU(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
     if (!coop) return PCCL_ERR_CUDA;
     void* mb = nullptr;
-    CU(cudaHostAlloc(&mb, 4096, cudaHostAllocDefault));
-    G.mailbox = mb;
-    CU(cudaStreamCreateWithFlags(&G.copy_stream, cudaStreamNonBlocking));
-    CU(cudaEventCreateWithFlags(&G.loop_done, cudaEventDisableTiming));
+    cudaStream_t cs = nullptr;
+    cudaEvent_t ev = nullptr;
+    if (cudaHostAlloc(&mb, 4096, cudaHostAllocDefault) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (ev) (void)cudaEventDestroy(ev);
+        if (cs) (void)cudaStreamDestroy(cs);
+        if (mb) (void)cudaFreeHost(mb);
+        return PCCL_ERR_CUDA;
+    }
+    G.mailbox = mb; G.copy_stream = cs; G.loop_done = ev;
     G.sm_count = sms;
     G.dev = dev;
     return PCCL_OK;
@@ -300,6 +320,21 @@ extern "C" void pccl_set_allocator(pccl_alloc_fn a, pccl_free_fn f, void* user) 
     else { G.alloc = nullptr; G.release = nullptr; G.user = nullptr; }
 }
 extern "C" int pccl_version(void) { return PCCL_VERSION; }
+extern "C" uint64_t pccl_launch_count(void) { return G.launches.load(std::memory_order_relaxed); }
+extern "C" int pccl_set_option(int option, uint64_t value) {
+    switch (option) {
+        case PCCL_OPT_BFS_WINDOW: G.opt_bfs_window = value; return PCCL_OK;
+        case PCCL_OPT_BFS_ROWS: G.opt_bfs_rows = value; return PCCL_OK;
+        default: return PCCL_ERR_INVALID;
+    }
+}
+extern "C" uint64_t pccl_get_option(int option) {
+    switch (option) {
+        case PCCL_OPT_BFS_WINDOW: return G.opt_bfs_window;
+        case PCCL_OPT_BFS_ROWS: return G.opt_bfs_rows;
+        default: return 0;
+    }
+}
 extern "C" const char* pccl_strerror(int err) {
     switch (err) {
         case PCCL_OK: return "ok";
@@ -380,7 +415,12 @@ int topo_upload(pccl_topology* t) {
                  o_ino = c.take((N + 1) * 4), o_inl = c.take(L * 4), o_outo = c.take((N + 1) * 4), o_outl = c.take(L * 4),
                  o_of = c.take(L * 4), o_if = c.take(L * 4), o_lon = c.take(L * 4), o_ldn = c.take(L * 4),
                  o_lot = c.take(L * 4), o_ldt = c.take(L * 4);
-    std::vector<unsigned char> h(c.cur ? c.cur : 256, 0);
+    std::vector<unsigned char> h;
+    try {
+        h.assign(c.cur ? c.cur : 256, 0);
+    } catch (const std::bad_alloc&) {
+        return PCCL_ERR_NOMEM;
+    }
     for (size_t l = 0; l < L; ++l) {
         ((uint32_t*)(h.data() + o_src))[l] = t->links[l].src;
         ((uint32_t*)(h.data() + o_dst))[l] = t->links[l].dst;
@@ -805,6 +845,13 @@ struct Work {   // device workspace of one phase
     uint32_t* st_inf = nullptr;
     uint32_t Wp = 0, S = 0, nLw = 0, SWp = 0;
     size_t zero_off = 0, zero_bytes = 0;   // have + wants + wants_cnt + ctrl are cleared per run
+    // barrier-free loop (pccl_loop2.cuh): plan arrays and its control block; the large arrays are allocated per phase
+    unsigned long long *nbase = nullptr, *poff = nullptr, *loff = nullptr;
+    uint32_t* soff = nullptr;
+    A2Ctrl* a2ctrl = nullptr;
+    bool a2_planned = false;               // phase_setup ran the plan kernel; a2 holds its results
+    A2Ctrl a2;                             // host copy
+    uint32_t a2_grid = 0, a2_wpc = 0;
 };
 
 size_t loop_smem_bytes(uint32_t S, uint32_t nbt = NB) {
@@ -831,9 +878,11 @@ int work_alloc(const pccl_problem& P, Work& W) {
     const size_t o_w = c.take(L * 8), o_D = c.take(max_sources * N * 8), o_free = c.take(L * 8),
                  o_mb = c.take((size_t)3 * W.nLw * 8), o_inf = c.take(L * 4), o_he = c.take(N * 4), o_ee = c.take(L * 4),
                  o_gc = c.take(L * W.S * 4), o_gt = c.take(L * 4), o_hold = c.take(C * HOLD_ROW * 4);
+    const size_t o_nb = c.take((N + 1) * 8), o_po = c.take((N + 1) * 8), o_lo = c.take((L + 1) * 8), o_so = c.take(N * 4);
     W.zero_off = c.cur;
     const size_t o_have = c.take(N * W.Wp * 8), o_wants = c.take(N * W.Wp * 8), o_hs = c.take(N * W.SWp * 8),
-                 o_ws = c.take(N * W.SWp * 8), o_wc = c.take(N * 4), o_hc = c.take(C * 4), o_ctrl = c.take(sizeof(LoopCtrl));
+                 o_ws = c.take(N * W.SWp * 8), o_wc = c.take(N * 4), o_hc = c.take(C * 4), o_ctrl = c.take(sizeof(LoopCtrl)),
+                 o_a2 = c.take(sizeof(A2Ctrl));
     W.zero_bytes = c.cur - W.zero_off;
     int rc = dev_alloc(c.cur, &W.blob);
     if (rc) return rc;
@@ -847,6 +896,8 @@ int work_alloc(const pccl_problem& P, Work& W) {
     W.hold = (uint32_t*)(b + o_hold); W.hold_cnt = (uint32_t*)(b + o_hc);
     W.st_free = (uint64_t*)(b + o_sf); W.st_inf = (uint32_t*)(b + o_si);
     W.wants_cnt = (uint32_t*)(b + o_wc); W.ctrl = (LoopCtrl*)(b + o_ctrl);
+    W.nbase = (unsigned long long*)(b + o_nb); W.poff = (unsigned long long*)(b + o_po);
+    W.loff = (unsigned long long*)(b + o_lo); W.soff = (uint32_t*)(b + o_so); W.a2ctrl = (A2Ctrl*)(b + o_a2);
     return PCCL_OK;
 }
 
@@ -862,14 +913,15 @@ PhaseView view_of(const pccl_topology* t, bool transposed) {
 }
 
 // steps A..C; on return the wants total is in *M (synchronises the stream)
-int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint64_t* M, bool dynamic = false) {
+int phase_setup(const pccl_problem& P, const Phase& ph, Work& W, uint64_t seed, uint64_t* M, bool dynamic = false,
+                bool plan_async = false) {
     const pccl_topology* t = P.topo;
     const uint32_t N = t->N, L = t->L, C = P.C;
     const PhaseView pv = view_of(t, ph.transposed);
     const uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
     cudaStream_t st = G.stream;
     CU(cudaMemsetAsync((unsigned char*)W.blob + W.zero_off, 0, W.zero_bytes, st));
-    if (L) k_link_cost<<<(L + 255) / 256, 256, 0, st>>>(t->d_alpha, t->d_bpp, L, P.chunk_bytes, W.w);
+    if (L) k_link_cost<<<(L + 255) / 256, 256, 0, counted(st)>>>(t->d_alpha, t->d_bpp, L, P.chunk_bytes, W.w);
     if (dynamic) {
         // reading Q18: distances TO every distinct dest (Bellman-Ford on the reversed links), best = dist(src -> dest),
         // wants = every node strictly closer to some dest than the source
@@ -878,15 +930,15 @@ int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t 
         const size_t smem = (size_t)N * 8;
         if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        if (NDS) k_distances<<<NDS, 256, smem, st>>>(pv.edst, pv.esrc, W.w, N, L, ph.d_dsts, W.D);
-        if (NP) k_best_init<<<(unsigned)((NP + 255) / 256), 256, 0, st>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, NP, ph.d_didx,
+        if (NDS) k_distances<<<NDS, 256, smem, counted(st)>>>(pv.edst, pv.esrc, W.w, N, L, ph.d_dsts, W.D);
+        if (NP) k_best_init<<<(unsigned)((NP + 255) / 256), 256, 0, counted(st)>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, NP, ph.d_didx,
                                                                          W.D, N, W.best, W.drow, &W.ctrl->err);
-        if (C) k_have<<<(C + 255) / 256, 256, 0, st>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
+        if (C) k_have<<<(C + 255) / 256, 256, 0, counted(st)>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
         const uint64_t nth = (uint64_t)N * ((C + 63) / 64);   // warps: one per (node, 64-chunk word)
         if (nth > (0x7FFFFFFFull << 2)) return PCCL_ERR_UNSUPPORTED;
-        if (nth) k_wants_dyn_init<<<(unsigned)((nth * 32 + 127) / 128), 128, 0, st>>>(ph.d_dest_off, ph.d_dests, ph.d_didx, W.D, W.best, N,
+        if (nth) k_wants_dyn_init<<<(unsigned)((nth * 32 + 127) / 128), 128, 0, counted(st)>>>(ph.d_dest_off, ph.d_dests, ph.d_didx, W.D, W.best, N,
                                                                                 C, W.Wp, W.SWp, W.wants, W.wsum, W.wants_cnt);
-        k_sum_u32<<<1, 1024, 0, st>>>(W.wants_cnt, N, &W.ctrl->wants_total);
+        k_sum_u32<<<1, 1024, 0, counted(st)>>>(W.wants_cnt, N, &W.ctrl->wants_total);
         CU(cudaGetLastError());
         LoopCtrl* mbx = (LoopCtrl*)G.mailbox;
         CU(cudaMemcpyAsync(mbx, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
@@ -901,23 +953,58 @@ int phase_setup(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t 
         const size_t smem = (size_t)N * 8;
         if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        k_distances<<<NS, 256, smem, st>>>(pv.esrc, pv.edst, W.w, N, L, ph.d_sources, W.D);
+        k_distances<<<NS, 256, smem, counted(st)>>>(pv.esrc, pv.edst, W.w, N, L, ph.d_sources, W.D);
     }
-    if (C) k_have<<<(C + 255) / 256, 256, 0, st>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
+    if (C) k_have<<<(C + 255) / 256, 256, 0, counted(st)>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
     const uint64_t ND = ph.dests.size();
     if (ND) {
-        k_wants<<<(unsigned)((ND + 127) / 128), 128, 0, st>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, ND, pv.esrc, pv.in_off,
+        k_wants<<<(unsigned)((ND + 127) / 128), 128, 0, counted(st)>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, ND, pv.esrc, pv.in_off,
                                                           pv.in_link, W.w, ph.d_sidx, W.D, N, W.Wp, W.SWp, k0, k1, W.wants,
                                                           W.wsum, W.wants_cnt, &W.ctrl->err);
     }
-    k_sum_u32<<<1, 1024, 0, st>>>(W.wants_cnt, N, &W.ctrl->wants_total);
+    k_sum_u32<<<1, 1024, 0, counted(st)>>>(W.wants_cnt, N, &W.ctrl->wants_total);
+    W.a2_planned = false;
+    if (plan_async) {
+        // barrier-free loop: one warp per destination, ceil(N / SMs) destinations per CTA, one CTA per SM
+        W.a2_wpc = std::max(1u, (N + (uint32_t)G.sm_count - 1) / (uint32_t)G.sm_count);
+        W.a2_grid = (N + W.a2_wpc - 1) / W.a2_wpc;
+        A2Args pa;
+        memset(&pa, 0, sizeof(pa));
+        pa.N = N; pa.L = L; pa.grid = W.a2_grid; pa.wpc = W.a2_wpc;
+        pa.esrc = pv.esrc; pa.in_off = pv.in_off; pa.w = W.w; pa.wants_cnt = W.wants_cnt;
+        pa.nbase = W.nbase; pa.poff = W.poff; pa.loff = W.loff; pa.soff = W.soff; pa.ctrl = W.a2ctrl;
+        k_a2_plan<<<1, 1024, 0, counted(st)>>>(pa);
+    }
     CU(cudaGetLastError());
     LoopCtrl* mb = (LoopCtrl*)G.mailbox;
+    A2Ctrl* mb2 = (A2Ctrl*)((unsigned char*)G.mailbox + 1024);
+    static_assert(sizeof(LoopCtrl) <= 1024 && sizeof(A2Ctrl) <= 1024, "mailbox quarters");
     CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
+    if (plan_async) CU(cudaMemcpyAsync(mb2, W.a2ctrl, sizeof(A2Ctrl), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     if (mb->err & 1u) return PCCL_ERR_UNREACHABLE;
     if (mb->err) return PCCL_ERR_INTERNAL;
     *M = mb->wants_total;
+    if (plan_async) { W.a2 = *mb2; W.a2_planned = true; }
+    return PCCL_OK;
+}
+
+// row a5 as a streaming kernel (pccl_sweep.cuh): candidate counts of every link; seeds the kept counts of the barrier
+// loops.  Rows staged by bulk asynchronous copies unless PCCL_FLAG_LSU_SWEEP asks for the per-lane 128-bit loads.
+int launch_count_sweep(const LoopArgs& a, uint32_t flags) {
+    if (a.N == 0 || a.L == 0) return PCCL_OK;
+    cudaStream_t st = G.stream;
+    const bool tma = !(flags & PCCL_FLAG_LSU_SWEEP);
+    const void* kern = tma ? (const void*)k_count_sweep<true> : (const void*)k_count_sweep<false>;
+    const size_t smem = tma ? (size_t)SW_STAGES * SW_ROWS * SW_SLICE_U4 * 16 : 0;
+    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, SW_THREADS, smem));
+    if (occ < 1) return PCCL_ERR_CUDA;
+    const uint32_t grid = std::min<uint32_t>(a.N, (uint32_t)occ * (uint32_t)G.sm_count);
+    if (tma) k_count_sweep<true><<<grid, SW_THREADS, smem, counted(st)>>>(a);
+    else k_count_sweep<false><<<grid, SW_THREADS, smem, counted(st)>>>(a);
+    CU(cudaGetLastError());
     return PCCL_OK;
 }
 
@@ -926,6 +1013,111 @@ struct LoopResult {
     uint32_t grid;
 };
 
+// stable LSD radix sort / reduce emitter, defined below
+int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out, bool reverse, uint64_t shift);
+
+// steps D..E without a grid barrier (pccl_loop2.cuh): setup of the per-destination entry lists and translation
+// tables, the loop, and the ranking of the logged claims into canonical order.  `raw_only`: leave the records in log
+// order (a transposed phase sorts them after the reversal anyway).
+int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint32_t flags, Rec* out,
+                     uint64_t out_cap, uint64_t t_offset, bool raw_only, LoopResult* res) {
+    const pccl_topology* t = P.topo;
+    const PhaseView pv = view_of(t, ph.transposed);
+    const uint32_t N = t->N, L = t->L;
+    const uint64_t M = out_cap;
+    cudaStream_t st = G.stream;
+    A2Args a;
+    memset(&a, 0, sizeof(a));
+    a.N = N; a.L = L; a.Wp = W.Wp; a.nLw = W.nLw;
+    a.k0 = (uint32_t)(seed & 0xFFFFFFFFull); a.k1 = (uint32_t)(seed >> 32);
+    a.grid = W.a2_grid; a.wpc = W.a2_wpc;
+    a.esrc = pv.esrc; a.edst = pv.edst; a.psrc = t->d_src; a.pdst = t->d_dst; a.in_off = pv.in_off; a.in_link = pv.in_link;
+    a.w = W.w; a.wants = W.wants; a.wants_cnt = W.wants_cnt; a.csrc = ph.d_cond_src;
+    a.nbase = W.nbase; a.poff = W.poff; a.loff = W.loff; a.soff = W.soff; a.ctrl = W.a2ctrl; a.abort_flag = &W.ctrl->err;
+    a.tcap = 1u << 16;
+    a.ecap = (uint32_t)std::min<uint64_t>(16384, std::max<uint64_t>(64, ((uint64_t)64 << 20) / ((uint64_t)std::max(W.nLw, 1u) * 12)));
+    a.out = out; a.out_cap = out_cap; a.t_offset = t_offset;
+    Carver c;
+    const size_t o_ids = c.take(M * 4), o_rp = c.take((size_t)N * W.Wp * 4), o_xm = c.take(W.a2.xmap_total * 4),
+                 o_pr = c.take(W.a2.priv_total * 4), o_hdr = c.take((size_t)N * 16), o_es = c.take(M * 4),
+                 o_us = c.take((size_t)a.ecap * 4), o_cs = c.take((size_t)a.ecap * 4), o_eb = c.take((size_t)a.ecap * 8),
+                 o_wb = c.take((size_t)a.ecap * W.nLw * 4), o_tr = c.take((size_t)a.tcap * 4);
+    const size_t o_ff = c.cur;                                   // filled with 0xFF: the log and the time keys
+    const size_t o_log = c.take(M * 16), o_tk = c.take((size_t)a.tcap * 8);
+    const size_t o_zero = c.cur;                                 // cleared
+    const size_t o_tc = c.take((size_t)a.tcap * 4), o_tf = c.take((size_t)a.tcap * 4), o_bm = c.take((size_t)a.ecap * W.nLw * 8);
+    void* blob = nullptr;
+    int rc = dev_alloc(c.cur, &blob);
+    if (rc) return rc;
+    struct Guard { void* p; ~Guard() { dev_free(p); } } guard{blob};
+    unsigned char* b = (unsigned char*)blob;
+    a.ids = (uint32_t*)(b + o_ids); a.rowpre = (uint32_t*)(b + o_rp); a.xmap = (uint32_t*)(b + o_xm);
+    a.priv = (uint32_t*)(b + o_pr); a.hdr = (U128*)(b + o_hdr); a.eslot = (uint32_t*)(b + o_es);
+    a.used = (uint32_t*)(b + o_us); a.cnt_sorted = (uint32_t*)(b + o_cs); a.ebase = (unsigned long long*)(b + o_eb);
+    a.wbase = (uint32_t*)(b + o_wb); a.trank = (uint32_t*)(b + o_tr); a.log = (U128*)(b + o_log);
+    a.tkey = (unsigned long long*)(b + o_tk); a.tcnt = (uint32_t*)(b + o_tc); a.tflag = (uint32_t*)(b + o_tf);
+    a.bm = (unsigned long long*)(b + o_bm);
+    CU(cudaMemsetAsync(b + o_ff, 0xFF, o_zero - o_ff, st));
+    CU(cudaMemsetAsync(b + o_zero, 0, c.cur - o_zero, st));
+    // entries, translation tables, private images (once per phase)
+    k_a2_entries<<<N, 256, 0, counted(st)>>>(a);
+    if (L) k_a2_xmap<<<L, 128, 0, counted(st)>>>(a);
+    k_a2_priv<<<N, 128, 0, counted(st)>>>(a);
+    const size_t smem = (size_t)W.a2.smem_need;
+    const int threads = (int)W.a2_wpc * 32;
+    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_loop2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_loop2, threads, smem));
+    if (occ < 1 || (uint64_t)occ * (uint64_t)G.sm_count < W.a2_grid) return PCCL_ERR_INTERNAL;   // (checked by the caller's plan)
+    void* args[] = {(void*)&a};
+    CU(cudaLaunchCooperativeKernel((const void*)k_loop2, dim3(W.a2_grid), dim3(threads), args, smem, counted(st)));
+    // emit
+    k_emit_times<<<N, 256, 0, counted(st)>>>(a);
+    if (!raw_only) {
+        k_emit_rank<<<(a.ecap + 255) / 256, 256, 0, counted(st)>>>(a);
+        k_emit_base<<<1, 1024, 0, counted(st)>>>(a);
+        k_emit_bits<<<N, 256, 0, counted(st)>>>(a);
+        k_emit_wbase<<<(a.ecap + 7) / 8, 256, 0, counted(st)>>>(a);
+        k_emit_write<<<N, 256, 0, counted(st)>>>(a);
+    } else {
+        k_emit_raw<<<N, 256, 0, counted(st)>>>(a);
+    }
+    CU(cudaGetLastError());
+    LoopCtrl* mb = (LoopCtrl*)G.mailbox;
+    A2Ctrl* mb2 = (A2Ctrl*)((unsigned char*)G.mailbox + 1024);
+    CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(mb2, W.a2ctrl, sizeof(A2Ctrl), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+#ifdef PCCL_A2_PROFILE
+    fprintf(stderr, "[a2 profile] actions %llu polls %llu | cycles per action: philox %.0f poll %.0f apply %.0f pick %.0f commit %.0f next %.0f | per poll: load wait %.0f evaluate %.0f\n",
+            mb2->actions, mb2->polls, (double)mb2->prof[0] / mb2->actions, (double)mb2->prof[1] / mb2->actions,
+            (double)mb2->prof[2] / mb2->actions, (double)mb2->prof[3] / mb2->actions, (double)mb2->prof[4] / mb2->actions,
+            (double)mb2->prof[5] / mb2->actions, (double)mb2->prof[6] / mb2->polls, (double)mb2->prof[7] / mb2->polls);
+#endif
+    if (mb->err) return PCCL_ERR_INTERNAL;
+    if (mb2->err & 2u) return PCCL_ERR_NOMEM;
+    if (!raw_only && (mb2->err & 1u)) {
+        // more distinct event times than the time table or the per-event bitmaps hold: records in log order, then the
+        // general sort by (t_start, link)
+        Rec* tmp = nullptr;
+        rc = dev_alloc(std::max<uint64_t>(M, 1) * sizeof(Rec), (void**)&tmp);
+        if (rc) return rc;
+        A2Args a2 = a;
+        a2.out = tmp; a2.t_offset = 0;
+        k_emit_raw<<<N, 256, 0, counted(st)>>>(a2);
+        rc = reverse_sorted(tmp, mb2->total, mb2->tmax, L, out, false, t_offset);
+        cudaError_t e = cudaStreamSynchronize(st);
+        dev_free(tmp);
+        if (rc) return rc;
+        if (e != cudaSuccess) { (void)cudaGetLastError(); return PCCL_ERR_CUDA; }
+    }
+    res->total = mb2->total; res->tmax = mb2->tmax;
+    res->events = (uint64_t)mb2->n_end + 1;   // event times = {0} and every distinct t_end (each free time is visited)
+    res->rows = mb2->actions; res->links = mb2->picks; res->slow = mb2->slow; res->bytes = mb2->bytes;
+    res->grid = W.a2_grid;
+    return PCCL_OK;
+}
+
 // steps D..E: the event loop; records go to `out` (capacity M) in canonical order
 // host_out (optional, pinned, out_cap records): with the one-barrier loop the records are copied there while the
 // loop runs (the kernel publishes how many are final, this thread issues the copies); *streamed says whether
@@ -933,6 +1125,9 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
                uint64_t out_cap, uint64_t t_offset, LoopResult* res, std::vector<uint64_t>* trace = nullptr,
                Rec* host_out = nullptr, bool* streamed = nullptr) {
     const bool dynamic = (flags & PCCL_FLAG_DYNAMIC_RELAY) != 0;
+    if (W.a2_planned && out_cap > 0 && out_cap <= 0xFFFFFFFFull && W.a2.smem_need <= 220 * 1024 &&
+        ((flags & PCCL_FLAG_ASYNC) || W.a2.w_max / 16 <= W.a2.w_min))
+        return phase_loop_async(P, ph, W, seed, flags, out, out_cap, t_offset, ph.transposed, res);
     // the dynamic rule keeps the counts current too: wants bits are only dropped where a neighbour holds the chunk
     // (holder lists, dyn_shrink_wants); DENSE_SWEEP / RESCAN recount instead and drop every bit at once
     const pccl_topology* t = P.topo;
@@ -1009,10 +1204,10 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
         CU(cudaHostGetDevicePointer(&dp, (void*)progress, 0));
         a.progress = (unsigned long long*)dp;
     }
-    k_loop_init<<<(n_init + 255) / 256, 256, 0, st>>>(a);
-    if (a.gcnt != nullptr && a.L) k_count_init<<<a.L, 256, 0, st>>>(a);
+    k_loop_init<<<(n_init + 255) / 256, 256, 0, counted(st)>>>(a);
+    if (a.gcnt != nullptr && a.L) { const int rcs = launch_count_sweep(a, flags); if (rcs) return rcs; }
     void* args[] = {(void*)&a};
-    CU(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(threads), args, smem, st));
+    CU(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(threads), args, smem, counted(st)));
     LoopCtrl* mb = (LoopCtrl*)G.mailbox;
     CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
     if (stream_out) {
@@ -1044,7 +1239,7 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     } else {
         CU(cudaStreamSynchronize(st));
     }
-    if (mb->err & 32u) return PCCL_ERR_NOMEM;   // more transfers than the record buffer holds
+    if (mb->err & 32u) { res->total = mb->total; return PCCL_ERR_NOMEM; }   // more transfers than the record buffer holds
     if (mb->err) return PCCL_ERR_INTERNAL;
     res->total = mb->total; res->tmax = mb->tmax; res->events = mb->events;
     res->rows = mb->rows_scanned; res->links = mb->links_scanned; res->slow = mb->slow_picks;
@@ -1052,7 +1247,11 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     res->grid = grid;
     if (a.trace) {
         const size_t n = (size_t)std::min<uint64_t>(res->events, a.trace_cap) * TRACE_SLOTS;
-        trace->assign(n, 0);
+        try {
+            trace->assign(n, 0);
+        } catch (const std::bad_alloc&) {
+            return PCCL_ERR_NOMEM;
+        }
         CU(cudaMemcpyAsync(trace->data(), a.trace, n * 8, cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
     }
@@ -1064,9 +1263,9 @@ int radix_sort_pairs(uint64_t* keys[2], uint32_t* vals[2], uint64_t n, uint32_t 
                      int cur) {
     cudaStream_t st = G.stream;
     for (uint32_t shift = 0; shift < bits; shift += 8) {
-        k_sort_hist<<<nblocks, SORT_THREADS, 0, st>>>(keys[cur], n, shift, ghist, nblocks);
-        k_sort_scan<<<1, 1024, 0, st>>>(ghist, (uint64_t)256 * nblocks);
-        k_sort_scatter<<<nblocks, SORT_THREADS, 0, st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n, shift, ghist, nblocks);
+        k_sort_hist<<<nblocks, SORT_THREADS, 0, counted(st)>>>(keys[cur], n, shift, ghist, nblocks);
+        k_sort_scan<<<1, 1024, 0, counted(st)>>>(ghist, (uint64_t)256 * nblocks);
+        k_sort_scatter<<<nblocks, SORT_THREADS, 0, counted(st)>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n, shift, ghist, nblocks);
         cur ^= 1;
     }
     return cur;
@@ -1074,7 +1273,7 @@ int radix_sort_pairs(uint64_t* keys[2], uint32_t* vals[2], uint64_t n, uint32_t 
 
 // a9 for reductions: raw (transposed-broadcast) records -> reversed, sorted by (t_start, link), into out
 // (reverse = false: only sorted, times shifted by `shift`; T then only bounds the key width)
-int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out, bool reverse = true, uint64_t shift = 0) {
+int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out, bool reverse, uint64_t shift) {
     if (M == 0) return PCCL_OK;
     cudaStream_t st = G.stream;
     uint32_t link_bits = 1;
@@ -1094,30 +1293,42 @@ int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out, bool 
     uint32_t* vals[2] = {(uint32_t*)(b + o_v0), (uint32_t*)(b + o_v1)};
     uint32_t* ghist = (uint32_t*)(b + o_h);
     const unsigned g256 = (unsigned)((M + 255) / 256);
-    k_reverse_keys<<<g256, 256, 0, st>>>(raw, M, T, link_bits, keys[0], vals[0], reverse);
+    k_reverse_keys<<<g256, 256, 0, counted(st)>>>(raw, M, T, link_bits, keys[0], vals[0], reverse);
     const int cur = radix_sort_pairs(keys, vals, M, t_bits + link_bits, ghist, nblocks, 0);
-    k_gather_shift<<<g256, 256, 0, st>>>(raw, vals[cur], M, shift, out);
+    k_gather_shift<<<g256, 256, 0, counted(st)>>>(raw, vals[cur], M, shift, out);
     cudaError_t e = cudaGetLastError();
     dev_free(blob);   // stream-ordered: freed after the kernels above
     return e == cudaSuccess ? PCCL_OK : PCCL_ERR_CUDA;
 }
 
+// A phase of the call: an NVTX range (setup / loop / emit, visible in Nsight Systems and ncu --nvtx) and, with
+// PCCL_FLAG_TIME_LOOP, CUDA events around it.
 struct Timer {
+    const char* name;
     cudaEvent_t a = nullptr, b = nullptr;
-    bool on = false;
+    bool on = false, open = false;
     float acc = 0.f;
+    explicit Timer(const char* n) : name(n) {}
     void init(bool enable) {
         on = enable && cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess;
     }
-    void start() { if (on) cudaEventRecord(a, G.stream); }
+    void start() {
+        if (!open) { nvtxRangePushA(name); open = true; }
+        if (on) cudaEventRecord(a, G.stream);
+    }
     void stop() {   // call after the stream was synchronised or right before a sync
+        if (open) { nvtxRangePop(); open = false; }
         if (!on) return;
         cudaEventRecord(b, G.stream);
         cudaEventSynchronize(b);
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) acc += ms;
     }
-    ~Timer() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+    ~Timer() {
+        if (open) nvtxRangePop();
+        if (a) cudaEventDestroy(a);
+        if (b) cudaEventDestroy(b);
+    }
 };
 
 // ---------------------------------------------------------------------------------------
@@ -1171,20 +1382,20 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     uint32_t* ghist = (uint32_t*)(b + o_h);
     BfsCtrl* ctrl = (BfsCtrl*)(b + o_ctrl);
     CU(cudaMemsetAsync(ctrl, 0, sizeof(BfsCtrl), st));
-    k_link_cost<<<(L + 255) / 256, 256, 0, st>>>(t->d_alpha, t->d_bpp, L, P.chunk_bytes, d_w);
+    k_link_cost<<<(L + 255) / 256, 256, 0, counted(st)>>>(t->d_alpha, t->d_bpp, L, P.chunk_bytes, d_w);
     uint4* d_oslot = (uint4*)(b + o_os);
-    k_bfs_pack<<<(L + 255) / 256, 256, 0, st>>>(pv.out_link, pv.edst, d_w, L, d_oslot);
+    k_bfs_pack<<<(L + 255) / 256, 256, 0, counted(st)>>>(pv.out_link, pv.edst, d_w, L, d_oslot);
     if (NS) {
         const size_t ds = (size_t)N * 8;
         if (ds > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ds));
-        k_distances<<<NS, 256, ds, st>>>(pv.esrc, pv.edst, d_w, N, L, ph.d_sources, d_D);
+        k_distances<<<NS, 256, ds, counted(st)>>>(pv.esrc, pv.edst, d_w, N, L, ph.d_sources, d_D);
     }
     const uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
     const unsigned gC = (C + 255) / 256;
-    k_bfs_keys<<<gC, 256, 0, st>>>(ph.d_cond_src, ph.d_dest_off, ph.d_dests, C, ph.d_sidx, d_D, N, k0, k1, d_cdist, keys[0],
+    k_bfs_keys<<<gC, 256, 0, counted(st)>>>(ph.d_cond_src, ph.d_dest_off, ph.d_dests, C, ph.d_sidx, d_D, N, k0, k1, d_cdist, keys[0],
                                    vals[0], ctrl);
     int cur = radix_sort_pairs(keys, vals, C, 64, ghist, sort_blocks, 0);          // by (draw, chunk)
-    k_bfs_keys2<<<gC, 256, 0, st>>>(d_cdist, vals[cur], C, keys[cur ^ 1], vals[cur ^ 1]);
+    k_bfs_keys2<<<gC, 256, 0, counted(st)>>>(d_cdist, vals[cur], C, keys[cur ^ 1], vals[cur ^ 1]);
     cur = radix_sort_pairs(keys, vals, C, 64, ghist, sort_blocks, cur ^ 1);         // stable, by descending c.dist
     const uint32_t* d_order = vals[cur];
     CU(cudaGetLastError());
@@ -1203,7 +1414,7 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bfs, (int)BFS_THREADS, smem));
     if (occ < 1) return PCCL_ERR_CUDA;
     uint32_t Bwant = (uint32_t)G.sm_count;   // one 1024-thread CTA per SM
-    if (const char* e = getenv("PCCL_BFS_WINDOW")) Bwant = std::min<uint32_t>((uint32_t)occ * (uint32_t)G.sm_count, std::max(1, atoi(e)));
+    if (const uint64_t o = G.opt_bfs_window) Bwant = (uint32_t)std::min<uint64_t>((uint64_t)occ * (uint64_t)G.sm_count, o);
     const uint32_t B = std::max(1u, std::min(Bwant, nact));
 
     // ---- record capacity: a tree has at most N - 1 transfers; retried with the exact count if short ----
@@ -1216,7 +1427,7 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     // a full row makes the kernel stop and the phase is rerun with 4 R
     uint32_t R = 256;
     while (R < 4096 && R < nact / std::max(L, 1u) && (size_t)L * (R * 2) * 16 <= ((size_t)1 << 30)) R *= 2;
-    if (const char* e = getenv("PCCL_BFS_ROWS")) R = (uint32_t)std::max(8, atoi(e));   // (tests: force the rerun)
+    if (const uint64_t o = G.opt_bfs_rows) R = (uint32_t)std::min<uint64_t>(std::max<uint64_t>(8, o), 1u << 20);   // (tests: force the rerun)
     for (int attempt = 0; attempt < 8; ++attempt) {
         Carver w2;
         const size_t o_runs = w2.take((size_t)L * R * 16), o_rn = w2.take((size_t)L * 4), o_rs = w2.take((size_t)L * B * 8),
@@ -1245,9 +1456,9 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         a.rl_pos = (uint32_t*)(q + o_rp); a.tr_link = (uint32_t*)(q + o_tl); a.tr_start = (uint64_t*)(q + o_ts);
         a.out = raw; a.out_cap = cap; a.t_offset = 0; a.ctrl = ctrl;
         t_loop.start();
-        k_bfs_init<<<(std::max(L, 1u) + 255) / 256, 256, 0, st>>>(a);
+        k_bfs_init<<<(std::max(L, 1u) + 255) / 256, 256, 0, counted(st)>>>(a);
         void* args[] = {(void*)&a};
-        CU(cudaLaunchCooperativeKernel((const void*)k_bfs, dim3(B), dim3(BFS_THREADS), args, smem, st));
+        CU(cudaLaunchCooperativeKernel((const void*)k_bfs, dim3(B), dim3(BFS_THREADS), args, smem, counted(st)));
         CU(cudaMemcpyAsync(mb, ctrl, sizeof(BfsCtrl), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
         t_loop.stop();
@@ -1263,11 +1474,12 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
             CU(cudaMemsetAsync(&ctrl->err, 0, 4, st));
             continue;
         }
-        if (getenv("PCCL_BFS_DEBUG"))
-            fprintf(stderr, "[pccl bfs] rounds %llu searches %llu sweeps %llu relax %llu | CTA 0: search %.2f ms check %.2f ms commit %.2f ms | "
-                            "per search: sweeps %.2f us filter %.2f us | R %u B %u\n",
-                    mb->rounds, mb->searches, mb->iters, mb->relax, mb->ns_search * 1e-6, mb->ns_check * 1e-6, mb->ns_commit * 1e-6,
-                    mb->searches ? mb->ns_sweeps * 1e-3 / mb->searches : 0.0, mb->searches ? mb->ns_filter * 1e-3 / mb->searches : 0.0, R, B);
+#ifdef PCCL_BFS_PROFILE
+        fprintf(stderr, "[pccl bfs] rounds %llu searches %llu sweeps %llu relax %llu | CTA 0: search %.2f ms check %.2f ms commit %.2f ms | "
+                        "per search: sweeps %.2f us filter %.2f us | R %u B %u\n",
+                mb->rounds, mb->searches, mb->iters, mb->relax, mb->ns_search * 1e-6, mb->ns_check * 1e-6, mb->ns_commit * 1e-6,
+                mb->searches ? mb->ns_sweeps * 1e-3 / mb->searches : 0.0, mb->searches ? mb->ns_filter * 1e-3 / mb->searches : 0.0, R, B);
+#endif
         const uint64_t M = mb->nrec;
         res->M = M; res->tmax = mb->tmax; res->conditions = nact; res->searches = mb->searches; res->relax = mb->relax;
         res->rounds = mb->rounds; res->grid = B;
@@ -1298,7 +1510,7 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
     if (!S) return PCCL_ERR_NOMEM;
     memset(&S->stats, 0, sizeof(S->stats));
     S->stats.mode = (uint32_t)P->mode;
-    Timer t_setup, t_loop, t_emit;
+    Timer t_setup("pccl:setup"), t_loop("pccl:loop"), t_emit("pccl:emit");
     const bool timed = (flags & PCCL_FLAG_TIME_LOOP) != 0;
     t_setup.init(timed); t_loop.init(timed); t_emit.init(timed);
 
@@ -1359,62 +1571,91 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
         uint64_t M = 0;
         t_setup.start();
         const bool dynamic = (flags & PCCL_FLAG_DYNAMIC_RELAY) != 0;
-        rc = phase_setup(*P, ph, W, seed, &M, dynamic);
+        // the barrier-free loop applies to the static thin relay tree with kept counts, at most 8 in-links per node and
+        // one warp per destination resident (pccl_loop2.cuh); everything else runs the barrier loops
+        const uint32_t deg_view = ph.transposed ? P->topo->max_out : P->topo->max_in;
+        const bool plan_async = !dynamic && !(flags & (PCCL_FLAG_RESCAN | PCCL_FLAG_DENSE_SWEEP | PCCL_FLAG_TWO_BARRIERS |
+                                                      PCCL_FLAG_BARRIER_LOOP | PCCL_FLAG_TRACE)) &&
+                                deg_view <= A2_MAX_IN && P->topo->N <= (uint32_t)G.sm_count * A2_MAX_WARPS;
+        rc = phase_setup(*P, ph, W, seed, &M, dynamic, plan_async);
         if (rc) return fail(rc);
         t_setup.stop();
         S->stats.wants_total += M;
-        // thin relay tree: exactly M transfers.  dynamic rule: at most M (a (node, chunk) pair is claimed at
-        // most once); the record buffer is sized for that bound, capped at 2^28 records
-        const uint64_t cap = dynamic ? std::min<uint64_t>(M, 1ull << 28) : M;
+        // thin relay tree: exactly M transfers.  dynamic rule: at most M (a (node, chunk) pair is claimed at most once),
+        // usually far fewer (config 4: 58 M initial wants, 1.58 M transfers): the record buffer starts at a few records
+        // per (chunk, dest) pair and, if that is short, the phase is rerun with the exact count the first run reports
+        uint64_t cap = dynamic ? std::min<uint64_t>(M, std::max<uint64_t>(4 * (uint64_t)ph.dests.size() + P->topo->N, 1u << 16)) : M;
         LoopResult lr;
-        if (ph.transposed) {
-            rc = dev_alloc(cap * sizeof(Rec), (void**)&raw);
-            if (rc) return fail(rc);
-            t_loop.start();
-            rc = phase_loop(*P, ph, W, seed, flags, raw, cap, 0, &lr, &S->trace);
-            if (rc) return fail(rc);
-            t_loop.stop();
-            if (dynamic ? lr.total > M : lr.total != M) return fail(PCCL_ERR_INTERNAL);
-            M = lr.total;
-            Rec* dst = nullptr;
-            rc = dev_alloc(M * sizeof(Rec), (void**)&dst);
-            if (rc) return fail(rc);
-            if (last) out_recs = dst; else stage1 = dst;
-            t_emit.start();
-            rc = reverse_sorted(raw, M, lr.tmax, L, dst);
-            if (rc) return fail(rc);
-            t_emit.stop();
-            dev_free(raw);
-            raw = nullptr;
-            M1 = M; T1 = lr.tmax;
-            if (last) { S->M = M; S->T = lr.tmax; }
-            S->stats.time_phase1_ps = lr.tmax;
-        } else {
-            const uint64_t base = (pi == 0) ? 0 : M1;
-            const uint64_t toff = (pi == 0) ? 0 : T1;
-            rc = dev_alloc((base + cap) * sizeof(Rec), (void**)&out_recs);
-            if (rc) return fail(rc);
-            if (base) {
-                if (cudaMemcpyAsync(out_recs, stage1, base * sizeof(Rec), cudaMemcpyDeviceToDevice, G.stream) != cudaSuccess) {
-                    (void)cudaGetLastError();
-                    return fail(PCCL_ERR_CUDA);
+        memset(&lr, 0, sizeof(lr));
+        for (int attempt = 0;; ++attempt) {
+            if (attempt > 0) {   // rerun: steps A..C again (the loop consumed the wants), exact capacity
+                if (cap > (1ull << 31)) return fail(PCCL_ERR_NOMEM);
+                uint64_t M2 = 0;
+                rc = phase_setup(*P, ph, W, seed, &M2, dynamic, false);
+                if (rc) return fail(rc);
+            }
+            if (ph.transposed) {
+                rc = dev_alloc(cap * sizeof(Rec), (void**)&raw);
+                if (rc) return fail(rc);
+                t_loop.start();
+                rc = phase_loop(*P, ph, W, seed, flags, raw, cap, 0, &lr, &S->trace);
+                if (rc == PCCL_ERR_NOMEM && dynamic && attempt == 0 && lr.total > cap && lr.total <= M) {
+                    t_loop.stop();
+                    dev_free(raw); raw = nullptr;
+                    cap = lr.total;
+                    continue;
                 }
+                if (rc) return fail(rc);
+                t_loop.stop();
+                if (dynamic ? lr.total > M : lr.total != M) return fail(PCCL_ERR_INTERNAL);
+                M = lr.total;
+                Rec* dst = nullptr;
+                rc = dev_alloc(M * sizeof(Rec), (void**)&dst);
+                if (rc) return fail(rc);
+                if (last) out_recs = dst; else stage1 = dst;
+                t_emit.start();
+                rc = reverse_sorted(raw, M, lr.tmax, L, dst, true, 0);
+                if (rc) return fail(rc);
+                t_emit.stop();
+                dev_free(raw);
+                raw = nullptr;
+                M1 = M; T1 = lr.tmax;
+                if (last) { S->M = M; S->T = lr.tmax; }
+                S->stats.time_phase1_ps = lr.tmax;
+            } else {
+                const uint64_t base = (pi == 0) ? 0 : M1;
+                const uint64_t toff = (pi == 0) ? 0 : T1;
+                rc = dev_alloc((base + cap) * sizeof(Rec), (void**)&out_recs);
+                if (rc) return fail(rc);
+                if (base) {
+                    if (cudaMemcpyAsync(out_recs, stage1, base * sizeof(Rec), cudaMemcpyDeviceToDevice, G.stream) != cudaSuccess) {
+                        (void)cudaGetLastError();
+                        return fail(PCCL_ERR_CUDA);
+                    }
+                }
+                // a schedule that goes to the host anyway is streamed out while the loop runs (single copy phase)
+                bool streamed = false;
+                if (base == 0 && last && !dynamic && cap && !(flags & PCCL_FLAG_KEEP_ON_DEVICE)) {
+                    S->h_bytes = cap * sizeof(Rec);
+                    S->h_recs = pinned_get(S->h_bytes);   // null: no streaming, the download reports the failure
+                }
+                t_loop.start();
+                rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, cap, toff, &lr, &S->trace, (Rec*)S->h_recs, &streamed);
+                if (rc == PCCL_ERR_NOMEM && dynamic && attempt == 0 && lr.total > cap && lr.total <= M) {
+                    t_loop.stop();
+                    dev_free(out_recs); out_recs = nullptr;
+                    cap = lr.total;
+                    continue;
+                }
+                if (rc) return fail(rc);
+                t_loop.stop();
+                if (dynamic ? lr.total > M : lr.total != M) return fail(PCCL_ERR_INTERNAL);
+                M = lr.total;
+                S->M = base + M;
+                S->T = toff + lr.tmax;
+                S->downloaded = streamed;
             }
-            // a schedule that goes to the host anyway is streamed out while the loop runs (single copy phase)
-            bool streamed = false;
-            if (base == 0 && last && !dynamic && cap && !(flags & PCCL_FLAG_KEEP_ON_DEVICE)) {
-                S->h_bytes = cap * sizeof(Rec);
-                S->h_recs = pinned_get(S->h_bytes);   // null: no streaming, the download reports the failure
-            }
-            t_loop.start();
-            rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, cap, toff, &lr, &S->trace, (Rec*)S->h_recs, &streamed);
-            if (rc) return fail(rc);
-            t_loop.stop();
-            if (dynamic ? lr.total > M : lr.total != M) return fail(PCCL_ERR_INTERNAL);
-            M = lr.total;
-            S->M = base + M;
-            S->T = toff + lr.tmax;
-            S->downloaded = streamed;
+            break;
         }
         S->stats.events += lr.events;
         S->stats.rows_scanned += lr.rows;
@@ -1517,12 +1758,12 @@ extern "C" int pccl_schedule_programs(pccl_schedule_t* s, uint64_t* offsets, pcc
     uint32_t* ghist = (uint32_t*)(b + o_h);
     const unsigned g256 = (unsigned)((n + 255) / 256);
     // stable LSD order: first by (time, kind, link), then by node
-    k_ops_keys<<<g256, 256, 0, st>>>(s->d_recs, M, link_bits, keys[0], vals[0]);
+    k_ops_keys<<<g256, 256, 0, counted(st)>>>(s->d_recs, M, link_bits, keys[0], vals[0]);
     int cur = radix_sort_pairs(keys, vals, n, t_bits + 1 + link_bits, ghist, nblocks, 0);
-    k_ops_nodes<<<g256, 256, 0, st>>>(s->d_recs, M, vals[cur], keys[cur]);
+    k_ops_nodes<<<g256, 256, 0, counted(st)>>>(s->d_recs, M, vals[cur], keys[cur]);
     cur = radix_sort_pairs(keys, vals, n, node_bits, ghist, nblocks, cur);
-    k_ops_gather<<<g256, 256, 0, st>>>(s->d_recs, M, vals[cur], (Op*)(b + o_ops));
-    k_ops_offsets<<<(N + 1 + 255) / 256, 256, 0, st>>>(keys[cur], n, N, (uint64_t*)(b + o_off));
+    k_ops_gather<<<g256, 256, 0, counted(st)>>>(s->d_recs, M, vals[cur], (Op*)(b + o_ops));
+    k_ops_offsets<<<(N + 1 + 255) / 256, 256, 0, counted(st)>>>(keys[cur], n, N, (uint64_t*)(b + o_off));
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(ops, b + o_ops, n * sizeof(Op), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(offsets, b + o_off, ((size_t)N + 1) * 8, cudaMemcpyDeviceToHost, st);
@@ -1561,7 +1802,7 @@ extern "C" int pccl_device_philox(const uint32_t* ctr, uint64_t n, const uint32_
     cudaStream_t st = G.stream;
     cudaError_t e = cudaMemcpyAsync(dc, ctr, n * 16, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) {
-        k_philox<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(dc, n, key[0], key[1], dout);
+        k_philox<<<(unsigned)((n + 255) / 256), 256, 0, counted(st)>>>(dc, n, key[0], key[1], dout);
         e = cudaMemcpyAsync(out, dout, n * 16, cudaMemcpyDeviceToHost, st);
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -1580,7 +1821,7 @@ extern "C" int pccl_device_link_costs(pccl_topology_t* t, uint64_t chunk_bytes, 
     rc = dev_alloc((size_t)t->L * 8, &d);
     if (rc) return rc;
     cudaStream_t st = G.stream;
-    k_link_cost<<<(t->L + 255) / 256, 256, 0, st>>>(t->d_alpha, t->d_bpp, t->L, chunk_bytes, (uint64_t*)d);
+    k_link_cost<<<(t->L + 255) / 256, 256, 0, counted(st)>>>(t->d_alpha, t->d_bpp, t->L, chunk_bytes, (uint64_t*)d);
     cudaError_t e = cudaMemcpyAsync(out, d, (size_t)t->L * 8, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     dev_free(d);
@@ -1608,8 +1849,8 @@ extern "C" int pccl_device_distances(pccl_topology_t* t, uint64_t chunk_bytes, u
     if (e == cudaSuccess && N * 8 > 48 * 1024)
         e = cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(N * 8));
     if (e == cudaSuccess) {
-        if (L) k_link_cost<<<(unsigned)((L + 255) / 256), 256, 0, st>>>(t->d_alpha, t->d_bpp, (uint32_t)L, chunk_bytes, (uint64_t*)(b + o_w));
-        k_distances<<<1, 256, N * 8, st>>>(pv.esrc, pv.edst, (uint64_t*)(b + o_w), (uint32_t)N, (uint32_t)L, (uint32_t*)(b + o_s), (uint64_t*)(b + o_D));
+        if (L) k_link_cost<<<(unsigned)((L + 255) / 256), 256, 0, counted(st)>>>(t->d_alpha, t->d_bpp, (uint32_t)L, chunk_bytes, (uint64_t*)(b + o_w));
+        k_distances<<<1, 256, N * 8, counted(st)>>>(pv.esrc, pv.edst, (uint64_t*)(b + o_w), (uint32_t)N, (uint32_t)L, (uint32_t*)(b + o_s), (uint64_t*)(b + o_D));
         e = cudaMemcpyAsync(out, b + o_D, N * 8, cudaMemcpyDeviceToHost, st);
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -1632,8 +1873,15 @@ extern "C" int64_t pccl_device_wants(pccl_problem_t* P, uint32_t phase, uint64_t
     if (rc) { dev_free(W.blob); return rc; }
     const uint32_t N = P->topo->N;
     // node bases from wants_cnt (host exclusive scan; accessor only)
-    std::vector<uint32_t> wc(N);
-    std::vector<uint64_t> base((size_t)N + 1, 0);
+    std::vector<uint32_t> wc;
+    std::vector<uint64_t> base;
+    try {
+        wc.assign(N, 0);
+        base.assign((size_t)N + 1, 0);
+    } catch (const std::bad_alloc&) {
+        dev_free(W.blob);
+        return PCCL_ERR_NOMEM;
+    }
     cudaStream_t st = G.stream;
     cudaError_t e = cudaMemcpyAsync(wc.data(), W.wants_cnt, (size_t)N * 4, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -1648,7 +1896,7 @@ extern "C" int64_t pccl_device_wants(pccl_problem_t* P, uint32_t phase, uint64_t
     unsigned char* b = (unsigned char*)d;
     e = cudaMemcpyAsync(b + o_b, base.data(), ((size_t)N + 1) * 8, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess && N) {
-        k_wants_pairs<<<(N + 3) / 4, 128, 0, st>>>(W.wants, N, W.Wp, (const uint64_t*)(b + o_b), (uint32_t*)(b + o_p), n_out);
+        k_wants_pairs<<<(N + 3) / 4, 128, 0, counted(st)>>>(W.wants, N, W.Wp, (const uint64_t*)(b + o_b), (uint32_t*)(b + o_p), n_out);
         if (n_out) e = cudaMemcpyAsync(out, b + o_p, n_out * 8, cudaMemcpyDeviceToHost, st);
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -1656,4 +1904,95 @@ extern "C" int64_t pccl_device_wants(pccl_problem_t* P, uint32_t phase, uint64_t
     dev_free(W.blob);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return PCCL_ERR_CUDA; }
     return (int64_t)M;
+}
+
+// a5: candidate counts |have[src_l] & wants[dst_l]| of every link at t = 0 by the streaming sweep kernel, timed alone
+extern "C" int pccl_device_candidate_sweep(pccl_problem_t* P, uint32_t phase, uint64_t seed, uint32_t flags, uint32_t iters,
+                                           float* ms_per_sweep, uint64_t* bytes_per_sweep, uint32_t* totals) {
+    SERIALISE;
+    if (!P || phase >= P->phases.size() || iters == 0) return PCCL_ERR_INVALID;
+    int rc = pccl_problem_upload(P);
+    if (rc) return rc;
+    const Phase& ph = P->phases[phase];
+    Work W;
+    rc = work_alloc(*P, W);
+    if (rc) return rc;
+    struct Guard { void* p; ~Guard() { dev_free(p); } } guard{W.blob};
+    uint64_t M = 0;
+    rc = phase_setup(*P, ph, W, seed, &M);
+    if (rc) return rc;
+    const pccl_topology* t = P->topo;
+    const PhaseView pv = view_of(t, ph.transposed);
+    LoopArgs a;
+    memset(&a, 0, sizeof(a));
+    a.N = t->N; a.L = t->L; a.Wp = W.Wp; a.S = W.S;
+    a.esrc = pv.esrc; a.edst = pv.edst; a.in_off = pv.in_off; a.in_link = pv.in_link;
+    a.have = W.have; a.wants = W.wants; a.gcnt = W.gcnt; a.gtot = W.gtot;
+    cudaStream_t st = G.stream;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (e0) cudaEventDestroy(e0);
+        return PCCL_ERR_CUDA;
+    }
+    struct EvGuard { cudaEvent_t a, b; ~EvGuard() { cudaEventDestroy(a); cudaEventDestroy(b); } } evg{e0, e1};
+    rc = launch_count_sweep(a, flags);                       // warm-up (and the result)
+    if (rc) return rc;
+    CU(cudaEventRecord(e0, st));
+    for (uint32_t i = 0; i < iters; ++i) { rc = launch_count_sweep(a, flags); if (rc) return rc; }
+    CU(cudaEventRecord(e1, st));
+    CU(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, e0, e1));
+    if (ms_per_sweep) *ms_per_sweep = ms / (float)iters;
+    // algorithmic bytes of one sweep: one wants row per node with in-links and one have row per link
+    if (bytes_per_sweep) {
+        uint64_t rows = t->L;
+        for (uint32_t v = 0; v < t->N; ++v) {
+            const uint32_t deg = ph.transposed ? t->out_off[v + 1] - t->out_off[v] : t->in_off[v + 1] - t->in_off[v];
+            rows += (deg + NB - 1) / NB;
+        }
+        *bytes_per_sweep = rows * (uint64_t)W.Wp * 8;
+    }
+    if (totals && t->L) {
+        CU(cudaMemcpyAsync(totals, W.gtot, (size_t)t->L * 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
+    return PCCL_OK;
+}
+
+// sequential 128-bit read of a `bytes`-sized device buffer, `iters` times: ms per pass (the measured ceiling of L2 when the
+// buffer fits there, of HBM when it does not, for the access pattern of the bitmap sweeps)
+extern "C" int pccl_device_read_bandwidth(uint64_t bytes, uint32_t iters, float* ms_per_pass) {
+    SERIALISE;
+    if (bytes < 16 || iters == 0 || !ms_per_pass) return PCCL_ERR_INVALID;
+    int rc = ensure_device();
+    if (rc) return rc;
+    void* d = nullptr;
+    rc = dev_alloc(bytes + 256, &d);
+    if (rc) return rc;
+    struct Guard { void* p; ~Guard() { dev_free(p); } } guard{d};
+    cudaStream_t st = G.stream;
+    CU(cudaMemsetAsync(d, 0x5A, bytes, st));
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_read_sweep, SW_THREADS, 0));
+    const uint32_t grid = (uint32_t)std::max(1, occ) * (uint32_t)G.sm_count;
+    uint32_t* sink = (uint32_t*)((unsigned char*)d + (bytes & ~(uint64_t)15));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (e0) cudaEventDestroy(e0);
+        return PCCL_ERR_CUDA;
+    }
+    struct EvGuard { cudaEvent_t a, b; ~EvGuard() { cudaEventDestroy(a); cudaEventDestroy(b); } } evg{e0, e1};
+    for (int i = 0; i < 2; ++i) k_read_sweep<<<grid, SW_THREADS, 0, counted(st)>>>((const uint4*)d, bytes / 16, sink);
+    CU(cudaEventRecord(e0, st));
+    for (uint32_t i = 0; i < iters; ++i) k_read_sweep<<<grid, SW_THREADS, 0, counted(st)>>>((const uint4*)d, bytes / 16, sink);
+    CU(cudaEventRecord(e1, st));
+    CU(cudaEventSynchronize(e1));
+    CU(cudaGetLastError());
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, e0, e1));
+    *ms_per_pass = ms / (float)iters;
+    return PCCL_OK;
 }

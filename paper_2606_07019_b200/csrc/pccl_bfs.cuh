@@ -210,8 +210,10 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
     const uint64_t d0 = a.dest_off[chunk];
     const uint32_t nd = (uint32_t)(a.dest_off[chunk + 1] - d0);
     const uint32_t mds = a.deg_shift;
+#ifdef PCCL_BFS_PROFILE
     unsigned long long dbg0 = 0, dbg1 = 0;
     if (tid == 0) dbg0 = globaltimer_ns();
+#endif
     for (uint32_t v = tid; v < a.N; v += BFS_THREADS) { key[v] = BFS_INF; stamp[v] = NONE32; }
     if (s_hdr) for (uint32_t l = tid; l < a.L; l += BFS_THREADS) s_hdr[l] = __ldcg(a.runs + (size_t)l * a.R);
     if (tid == 0) { sh.nf[0] = 1; sh.nf[1] = 0; sh.nf[2] = 0; fr0[0] = src; }
@@ -225,7 +227,10 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
     for (uint32_t it = 0;; ++it) {
         const uint32_t nf = sh.nf[r0];
         if (nf == 0 || it > a.N + 1) {
-            if (tid == 0) { atomicAdd(&a.ctrl->iters, (unsigned long long)it); if (nf) atomicOr(&a.ctrl->err, 16u); }
+#ifdef PCCL_BFS_PROFILE
+            if (tid == 0) atomicAdd(&a.ctrl->iters, (unsigned long long)it);
+#endif
+            if (tid == 0 && nf) atomicOr(&a.ctrl->err, 16u);
             break;
         }
         if (nd > 8) {                                   // many dests: max of their arrivals, by the whole CTA
@@ -277,7 +282,9 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
         }
         __syncthreads();
     }
+#ifdef PCCL_BFS_PROFILE
     if (tid == 0) dbg1 = globaltimer_ns();
+#endif
     uint32_t* keep = fr0;                               // the frontier lists are dead now
     for (uint32_t v = tid; v < a.N; v += BFS_THREADS) keep[v] = 0;
     __syncthreads();
@@ -304,7 +311,9 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
     }
     __syncthreads();
     ntr = sh.cnt;
+#ifdef PCCL_BFS_PROFILE
     if (tid == 0) { const unsigned long long dbg2 = globaltimer_ns(); atomicAdd(&a.ctrl->ns_sweeps, dbg1 - dbg0); atomicAdd(&a.ctrl->ns_filter, dbg2 - dbg1); }
+#endif
 }
 
 __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
@@ -330,8 +339,10 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
     bool valid = false;
     for (uint32_t round = 0; base < a.nact; ++round) {
         // ---- S: search + post ---------------------------------------------------------------
+#ifdef PCCL_BFS_PROFILE
         unsigned long long tq0 = 0;
         if (gtid == 0) tq0 = globaltimer_ns();
+#endif
         const uint64_t p64 = base + ((slot + B - (uint32_t)(base % B)) % B);
         const bool active = p64 < a.nact;
         const uint32_t p = (uint32_t)p64;
@@ -348,8 +359,10 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
             }
         }
         grid.sync();
+#ifdef PCCL_BFS_PROFILE
         unsigned long long tq1 = 0;
         if (gtid == 0) tq1 = globaltimer_ns();
+#endif
         // ---- C: lowest earlier position whose transfer overlaps one of mine --------------------
         // (err is only written before the barrier above or after the next one: every CTA reads the same value)
         if (tid == 0) { sh.minconf = NONE32; sh.tmax = 0; sh.cnt = ldcg32(&a.ctrl->err) & (2u | 4u | 16u); }
@@ -373,8 +386,10 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
         __syncthreads();
         if (active && tid == 0 && sh.minconf != NONE32) atomicMin(&a.ctrl->first_bad[round & 1], (unsigned long long)p);
         grid.sync();
+#ifdef PCCL_BFS_PROFILE
         unsigned long long tq2 = 0;
         if (gtid == 0) tq2 = globaltimer_ns();
+#endif
         // ---- M: commit below first_bad ----------------------------------------------------------
         if (tid == 0) {
             const unsigned long long fbv = ldcg64((const uint64_t*)&a.ctrl->first_bad[round & 1]);
@@ -420,10 +435,12 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
         if (gtid == 0) { a.ctrl->first_bad[(round + 1) & 1] = BFS_INF; a.ctrl->rounds = round + 1; }
         base = fb;
         grid.sync();
+#ifdef PCCL_BFS_PROFILE
         if (gtid == 0) {
             const unsigned long long tq3 = globaltimer_ns();
             a.ctrl->ns_search += tq1 - tq0; a.ctrl->ns_check += tq2 - tq1; a.ctrl->ns_commit += tq3 - tq2;
         }
+#endif
     }
     // statistics
     for (int o = 16; o; o >>= 1) relax += __shfl_down_sync(0xFFFFFFFFu, relax, o);

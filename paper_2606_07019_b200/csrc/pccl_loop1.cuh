@@ -379,7 +379,11 @@ __global__ void __launch_bounds__(NBT * 32 * TEAMS, 1024 / (NBT * 32 * TEAMS)) k
         tot_prev = tot_cur;
         tot_cur = s_next[1];
         // the records of event step-1 were emitted before the barrier above: [0, tot_prev) is final, tell the host
-        if (a.progress != nullptr && blockIdx.x == 0 && threadIdx.x == 0) *(volatile unsigned long long*)a.progress = tot_prev;
+        // (the host DMA-reads other CTAs' records on this signal: order them at system scope first)
+        if (a.progress != nullptr && blockIdx.x == 0 && threadIdx.x == 0) {
+            __threadfence_system();
+            *(volatile unsigned long long*)a.progress = tot_prev;
+        }
         __syncthreads();
         ++step;
         if (t == T_INF) break;

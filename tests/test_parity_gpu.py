@@ -266,6 +266,7 @@ def test_config4_full_size_bit_exact(pk):
     assert s.size == 1_572_864 == o.wants_total     # sum of hop distances, closed form
     assert_same(p, s, o)
     checker.check_structure(p, s.transfers)
+    assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_BARRIER_LOOP), o)
 
 
 @pytest.mark.parametrize("maker", [wl.config1, wl.config2, wl.config3, wl.config4_small, wl.config5_small,
@@ -299,9 +300,11 @@ def test_config5_full_size_bit_exact(pk):
     s = gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE)
     assert s.size == 7_761_800
     r = gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE | pk.PCCL_FLAG_RESCAN)
+    b = gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE | pk.PCCL_FLAG_BARRIER_LOOP)
     o = oracle.synthesize(*p.args())
     assert_same(p, s, o)
     assert_same(p, r, o)
+    assert_same(p, b, o)
     checker.check_structure(p, s.transfers)
 
 
@@ -449,12 +452,15 @@ def test_ten_thousand_nodes(pk, relay):
 @pytest.mark.parametrize("maker", SMALL + [lambda s: wl.ring_all_gather(8, True, s, chunks_per_npu=1040, chunk_bytes=4096),
                                            lambda s: _torus_all_gather((12, 12), 2, s)],
                          ids=lambda m: getattr(m, "__name__", "case"))
-def test_one_barrier_and_two_barrier_loops_agree(pk, maker):
-    """the default picks the one-barrier loop where it applies (<= 8 in-links per node); TWO_BARRIERS forces
-    the other one.  Both must equal the oracle."""
+def test_the_three_event_loops_agree(pk, maker):
+    """the default is the barrier-free loop where it applies (<= 8 in-links per node, link costs within 16x; ASYNC
+    forces it for any link costs); BARRIER_LOOP selects the one-barrier loop (or the two-barrier one where that
+    does not apply), TWO_BARRIERS the two-barrier loop.  All must equal the oracle."""
     p = maker(3)
     o = oracle.synthesize(*p.args())
     assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_KEEP_ON_DEVICE), o)
+    assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_ASYNC), o)
+    assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_BARRIER_LOOP), o)
     assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_TWO_BARRIERS), o)
 
 
@@ -487,14 +493,24 @@ def test_bfs_mode_many_conditions_per_link(pk):
     assert_same(p, s, o)
 
 
-def test_bfs_mode_reruns_when_a_busy_run_row_fills(pk, monkeypatch):
+def test_bfs_mode_reruns_when_a_busy_run_row_fills(pk):
     """rows of 8 entries overflow at once on the 8-node ring with 130 chunks per node (gaps open and close on
     every link): the kernel stops at the next round, the phase is rerun with longer rows, same schedule"""
     p = wl.config5_small(1)
     o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS)
-    monkeypatch.setenv("PCCL_BFS_ROWS", "8")
-    s = gpu_run(pk, p, pk.PCCL_FLAG_BFS)
+    pk.set_option(pk.PCCL_OPT_BFS_ROWS, 8)
+    try:
+        s = gpu_run(pk, p, pk.PCCL_FLAG_BFS)
+    finally:
+        pk.set_option(pk.PCCL_OPT_BFS_ROWS, 0)
     assert_same(p, s, o)
+    pk.set_option(pk.PCCL_OPT_BFS_WINDOW, 3)      # a 3-wide window: more rounds, same schedule
+    try:
+        s = gpu_run(pk, p, pk.PCCL_FLAG_BFS)
+    finally:
+        pk.set_option(pk.PCCL_OPT_BFS_WINDOW, 0)
+    assert_same(p, s, o)
+    assert s.stats["grid_blocks"] == 3
 
 
 def test_bfs_mode_ring3000(pk):
@@ -626,5 +642,8 @@ def test_randomized_problems_all_modes(pk, block):
             if i % 6 == 0 and relay != 2:
                 for fl in (pk.PCCL_FLAG_TWO_BARRIERS, pk.PCCL_FLAG_RESCAN, pk.PCCL_FLAG_DENSE_SWEEP):
                     assert_same(p, gpu_run(pk, p, rflag | fl), o)
+            if relay == 0:   # the barrier-free loop with heterogeneous link costs, and the one-barrier loop
+                assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_ASYNC), o)
+                assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_BARRIER_LOOP), o)
             if relay == 0:
                 checker.check_schedule(p, o.transfers)
