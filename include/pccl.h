@@ -114,8 +114,11 @@ int pccl_version(void);
  * and no files).  value 0 restores the default.  Errors: INVALID (unknown option). */
 typedef enum pccl_option {
     PCCL_OPT_BFS_WINDOW = 1,   /* PCCL_FLAG_BFS: conditions searched optimistically per round (default: one per SM) */
-    PCCL_OPT_BFS_ROWS = 2      /* PCCL_FLAG_BFS: initial capacity of a link's busy-run row, in runs (default: 256 or
+    PCCL_OPT_BFS_ROWS = 2,     /* PCCL_FLAG_BFS: initial capacity of a link's busy-run row, in runs (default: 256 or
                                   more; a full row reruns the phase with 4x longer rows) */
+    PCCL_OPT_DYNAMIC_RECORDS = 3 /* PCCL_FLAG_DYNAMIC_RELAY: initial capacity of the record buffer (default: 1.25 x the
+                                  static relay tree's transfer count; a short buffer reruns the phase with the exact
+                                  count) */
 } pccl_option;
 int pccl_set_option(int option, uint64_t value);
 uint64_t pccl_get_option(int option);

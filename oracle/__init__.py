@@ -64,6 +64,9 @@ def lib():
         L.oracle_synthesize_relay.argtypes = [u32, vp, u32, vp, u32, u32, vp, u64, vp, u64, u64, u64, C.c_int,
                                               C.POINTER(vp)]
         L.oracle_synthesize_relay.restype = C.c_int
+        L.oracle_synthesize_switches.argtypes = [u32, vp, u32, vp, u32, u32, vp, u64, vp, u64, u64, u64, vp, vp,
+                                                 C.POINTER(vp)]
+        L.oracle_synthesize_switches.restype = C.c_int
         L.oracle_wants.argtypes = [u32, vp, u32, u32, vp, vp, vp, u64, u64, vp, u64]
         L.oracle_wants.restype = i64
         for name in ("oracle_size", "oracle_time", "oracle_events", "oracle_wants_total",
@@ -121,19 +124,34 @@ class OracleSchedule:
 RELAY_THIN, RELAY_DYNAMIC, RELAY_BFS = 0, 1, 2
 
 
-def synthesize(n_npus, links, group, n_chunks, pre, post, chunk_bytes, seed, relay: int = RELAY_THIN) -> OracleSchedule:
+NO_LIMIT = 0xFFFFFFFF
+
+
+def synthesize(n_npus, links, group, n_chunks, pre, post, chunk_bytes, seed, relay: int = RELAY_THIN,
+               buffer_limit=None, no_multicast=None) -> OracleSchedule:
     """Same problem statement as the product boundary (include/pccl.h), host arrays only.
     relay: RELAY_THIN (static thin relay tree, the default), RELAY_DYNAMIC (Q18) or RELAY_BFS (the paper's
-    own per-condition search, Alg. 1-3, Q19-Q22; `events` then counts conditions routed)."""
+    own per-condition search, Alg. 1-3, Q19-Q22; `events` then counts conditions routed).
+    buffer_limit / no_multicast (RELAY_BFS only): the switch model of PAPER.md:348, per node (Q23-Q25)."""
     links = np.ascontiguousarray(links, dtype=LINK_DT)
     group = np.ascontiguousarray(group, dtype=np.uint32)
     pre = np.ascontiguousarray(pre, dtype=PAIR_DT)
     post = np.ascontiguousarray(post, dtype=PAIR_DT)
     h = C.c_void_p()
     t0 = time.perf_counter()
-    rc = lib().oracle_synthesize_relay(n_npus, _ptr(links), len(links), _ptr(group), len(group),
-                                       n_chunks, _ptr(pre), len(pre), _ptr(post), len(post),
-                                       chunk_bytes, seed, int(relay), C.byref(h))
+    if buffer_limit is not None or no_multicast is not None:
+        if relay != RELAY_BFS:
+            raise ValueError("the switch model applies to RELAY_BFS only")
+        bl = None if buffer_limit is None else np.ascontiguousarray(buffer_limit, dtype=np.uint32)
+        nm = None if no_multicast is None else np.ascontiguousarray(no_multicast, dtype=np.uint8)
+        assert (bl is None or len(bl) == n_npus) and (nm is None or len(nm) == n_npus)
+        rc = lib().oracle_synthesize_switches(n_npus, _ptr(links), len(links), _ptr(group), len(group),
+                                              n_chunks, _ptr(pre), len(pre), _ptr(post), len(post), chunk_bytes, seed,
+                                              None if bl is None else _ptr(bl), None if nm is None else _ptr(nm), C.byref(h))
+    else:
+        rc = lib().oracle_synthesize_relay(n_npus, _ptr(links), len(links), _ptr(group), len(group),
+                                           n_chunks, _ptr(pre), len(pre), _ptr(post), len(post),
+                                           chunk_bytes, seed, int(relay), C.byref(h))
     dt = time.perf_counter() - t0
     if rc:
         raise OracleError(rc)

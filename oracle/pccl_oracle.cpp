@@ -437,8 +437,51 @@ void occupy(BusyLink& b, uint64_t s, uint64_t e) {
     b.iv.insert(it, std::make_pair(s, e));
 }
 
+// -------------------------------------------------------------------------------------
+// Section 4.7 "Modeling Switches", readings Q23-Q25 of DESIGN.md.  Optional per-node
+// parameters of the BFS mode:
+//   buffer limit   "We track the number of chunks buffered at each switch node, and the BFS pathfinding
+//                  algorithm skips visiting a TEN node at a given timestep if the switch node exceeds the
+//                  provided buffer size."  A chunk is buffered at a node it is forwarded from, from its
+//                  arrival there until the end of the last transfer that forwards it (store and forward,
+//                  PAPER.md:338) -- a half-open stay [arrival, release).  Visiting node v at time t (the
+//                  arrival of a transfer) is skipped while the stays of the conditions routed BEFORE hold
+//                  limit(v) chunks or more at t; the link then starts at the earliest later time whose
+//                  arrival finds a free buffer (and a free link interval).  The test is made at the visit
+//                  time only, as the paper states it.
+//   no multicast   "if the switch node does not support multicast, the BFS algorithm visits only one next
+//                  neighbor ... visits next nodes one by one": such a node forwards over its out-links one
+//                  after the other, in ascending link id, the next transfer starting no earlier than the end
+//                  of the one before -- whether or not the visit is kept by the path filter afterwards.
+// -------------------------------------------------------------------------------------
+struct SwitchBuf {                                        // stays of the conditions routed so far
+    std::vector<uint64_t> arr, rel;                       // sorted arrival / release times
+    uint64_t occ(uint64_t t) const {                      // chunks buffered at time t: arrived by t, not released by t
+        return (uint64_t)(std::upper_bound(arr.begin(), arr.end(), t) - arr.begin()) -
+               (uint64_t)(std::upper_bound(rel.begin(), rel.end(), t) - rel.begin());
+    }
+    uint64_t next_free(uint64_t t, uint64_t limit) const { // earliest time >= t with fewer than `limit` chunks buffered
+        while (occ(t) >= limit) t = *std::upper_bound(rel.begin(), rel.end(), t);   // occ > 0: a release after t exists
+        return t;
+    }
+    void add(uint64_t a, uint64_t r) {
+        arr.insert(std::upper_bound(arr.begin(), arr.end(), a), a);
+        rel.insert(std::upper_bound(rel.begin(), rel.end(), r), r);
+    }
+};
+
+// earliest s >= a with [s, s + w) free on the link AND a free buffer at the far node at the arrival s + w
+uint64_t earliest_start_buffered(const BusyLink& b, uint64_t a, uint64_t w, const SwitchBuf* sb, uint64_t limit) {
+    for (;;) {
+        const uint64_t s = earliest_start(b, a, w);
+        if (!sb || sb->occ(s + w) < limit) return s;
+        a = sb->next_free(s + w, limit) - w;              // (> s: the buffer frees after s + w)
+    }
+}
+
 int synth_copy_bfs(uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& conds,
-                   uint64_t chunk_bytes, uint64_t seed, CopyResult& res) {
+                   uint64_t chunk_bytes, uint64_t seed, CopyResult& res,
+                   const uint32_t* buf_limit = nullptr, const uint8_t* no_mcast = nullptr) {
     const uint32_t L = (uint32_t)links.size();
     const uint32_t C = (uint32_t)conds.size();
     std::vector<uint64_t> w(L);
@@ -468,6 +511,8 @@ int synth_copy_bfs(uint32_t n, const std::vector<Link>& links, const std::vector
     });
 
     std::vector<BusyLink> busy(L);
+    std::vector<SwitchBuf> sbuf(buf_limit ? n : 0);
+    auto limited = [&](uint32_t v) { return buf_limit && buf_limit[v] != NONE; };
     res = CopyResult{};
     std::vector<uint64_t> arr(n);
     std::vector<uint32_t> pred(n);
@@ -491,10 +536,16 @@ int synth_copy_bfs(uint32_t n, const std::vector<Link>& links, const std::vector
             if (left == 0 && a > last) break;                 // Alg. 2 line 4: all dests visited
             done[u] = 1;
             if (left && std::binary_search(c.dests.begin(), c.dests.end(), u)) { --left; last = a; }
-            for (uint32_t l : out[u]) {                       // NextDevices(TEN, u, .)
+            uint64_t from = a;                                // a node without multicast: one out-link after the other (4.7)
+            for (uint32_t l : out[u]) {                       // NextDevices(TEN, u, .), ascending link id
                 const uint32_t v = links[l].dst;
-                if (done[v]) continue;                        // Alg. 2 line 7
-                const uint64_t t = earliest_start(busy[l], a, w[l]) + w[l];
+                const bool serial = no_mcast && no_mcast[u];
+                if (done[v] && !serial) continue;             // Alg. 2 line 7
+                if (limited(v) && buf_limit[v] == 0) continue;   // a node that buffers nothing is never visited
+                const uint64_t t = earliest_start_buffered(busy[l], from, w[l], limited(v) ? &sbuf[v] : nullptr,
+                                                           limited(v) ? buf_limit[v] : 0) + w[l];
+                if (serial) from = t;
+                if (done[v]) continue;
                 if (t < arr[v] || (t == arr[v] && l < pred[v])) {   // Q20
                     arr[v] = t;
                     pred[v] = l;
@@ -507,13 +558,18 @@ int synth_copy_bfs(uint32_t n, const std::vector<Link>& links, const std::vector
         std::fill(keep.begin(), keep.end(), 0);
         for (uint32_t d : c.dests)
             for (uint32_t v = d; v != c.src && !keep[v]; v = links[pred[v]].src) keep[v] = 1;
+        std::vector<uint64_t> release(buf_limit ? n : 0, 0);  // end of the last kept transfer out of each node
         for (uint32_t v = 0; v < n; ++v) {
             if (!keep[v]) continue;
             const uint32_t l = pred[v];
             res.recs.push_back(Rec{k.chunk, links[l].src, v, l, arr[v] - w[l], arr[v]});
             occupy(busy[l], arr[v] - w[l], arr[v]);           // Alg. 3 line 13
             res.T = std::max(res.T, arr[v]);
+            if (buf_limit) release[links[l].src] = std::max(release[links[l].src], arr[v]);
         }
+        if (buf_limit)                                        // the chunk was buffered at every limited node that forwarded it
+            for (uint32_t v = 0; v < n; ++v)
+                if (limited(v) && keep[v] && release[v] > 0) sbuf[v].add(arr[v], release[v]);
         ++res.events;                                         // here: conditions routed
     }
     std::sort(res.recs.begin(), res.recs.end(), [](const Rec& a, const Rec& b) {
@@ -526,9 +582,11 @@ int synth_copy_bfs(uint32_t n, const std::vector<Link>& links, const std::vector
 
 // relay rule used by the dispatchers below: 0 = thin relay tree (step C), 1 = dynamic,
 // 2 = the paper's per-condition BFS (no matching loop at all)
+struct SwitchModel { const uint32_t* buf_limit = nullptr; const uint8_t* no_mcast = nullptr; };   // section 4.7, BFS mode only
+
 int synth_copy_mode(int relay, uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& conds,
-                    uint64_t chunk_bytes, uint64_t seed, CopyResult& res) {
-    if (relay == 2) return synth_copy_bfs(n, links, conds, chunk_bytes, seed, res);
+                    uint64_t chunk_bytes, uint64_t seed, CopyResult& res, SwitchModel sw = SwitchModel()) {
+    if (relay == 2) return synth_copy_bfs(n, links, conds, chunk_bytes, seed, res, sw.buf_limit, sw.no_mcast);
     return relay == 1 ? synth_copy_dynamic(n, links, conds, chunk_bytes, seed, res)
                       : synth_copy(n, links, conds, chunk_bytes, seed, res);
 }
@@ -538,11 +596,11 @@ int synth_copy_mode(int relay, uint32_t n, const std::vector<Link>& links, const
 // the TRANSPOSED topology, then reverse every transfer in direction and in time.
 // -------------------------------------------------------------------------------------
 int synth_reduce(uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& bcast,
-                 uint64_t chunk_bytes, uint64_t seed, CopyResult& res, int relay = 0) {
+                 uint64_t chunk_bytes, uint64_t seed, CopyResult& res, int relay = 0, SwitchModel sw = SwitchModel()) {
     std::vector<Link> tr(links);
     for (Link& l : tr) std::swap(l.src, l.dst);
     CopyResult b;
-    const int rc = synth_copy_mode(relay, n, tr, bcast, chunk_bytes, seed, b);
+    const int rc = synth_copy_mode(relay, n, tr, bcast, chunk_bytes, seed, b, sw);
     if (rc != OR_OK) return rc;
     res.recs.clear();
     for (const Rec& r : b.recs)   // (c, a, b, l, ts, te) -> (c, src=b, dst=a, l, T-te, T-ts)
@@ -573,7 +631,7 @@ struct Result {
 int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uint32_t* group,
                uint32_t n_members, uint32_t n_chunks, const Pair* pre_p, uint64_t n_pre,
                const Pair* post_p, uint64_t n_post, uint64_t chunk_bytes, uint64_t seed,
-               Result& out, int relay = 0) {
+               Result& out, int relay = 0, SwitchModel sw = SwitchModel()) {
     if (n_links && !links_p) return OR_ERR_INVALID;
     if (n_members && !group) return OR_ERR_INVALID;
     if ((n_pre && !pre_p) || (n_post && !post_p)) return OR_ERR_INVALID;
@@ -617,7 +675,7 @@ int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uin
             for (uint32_t d : post[c]) if (d != conds[c].src) conds[c].dests.push_back(d);
         }
         CopyResult r;
-        const int rc = synth_copy_mode(relay, n_npus, links, conds, chunk_bytes, seed, r);
+        const int rc = synth_copy_mode(relay, n_npus, links, conds, chunk_bytes, seed, r, sw);
         if (rc != OR_OK) return rc;
         out.recs = std::move(r.recs); out.T = r.T; out.events = r.events;
         out.wants_total = r.wants_total; out.mode = 0;
@@ -631,7 +689,7 @@ int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uin
             for (uint32_t d : pre[c]) if (d != bc[c].src) bc[c].dests.push_back(d);
         }
         CopyResult r;
-        const int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r, relay);
+        const int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r, relay, sw);
         if (rc != OR_OK) return rc;
         out.recs = std::move(r.recs); out.T = r.T; out.events = r.events;
         out.wants_total = r.wants_total; out.mode = 1; out.T_phase1 = r.T;
@@ -650,9 +708,9 @@ int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uin
             for (uint32_t d : post[c]) if (d != root) cp[c].dests.push_back(d);
         }
         CopyResult r1, r2;
-        int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r1, relay);
+        int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r1, relay, sw);
         if (rc != OR_OK) return rc;
-        rc = synth_copy_mode(relay, n_npus, links, cp, chunk_bytes, seed, r2);
+        rc = synth_copy_mode(relay, n_npus, links, cp, chunk_bytes, seed, r2, sw);
         if (rc != OR_OK) return rc;
         out.recs = std::move(r1.recs);
         for (const Rec& r : r2.recs)
@@ -727,6 +785,25 @@ int oracle_synthesize_relay(uint32_t n_npus, const oracle_link* links, uint32_t 
     const int rc = synthesize(n_npus, (const Link*)links, n_links, group, n_members, n_chunks,
                               (const Pair*)pre, n_pre, (const Pair*)post, n_post, chunk_bytes,
                               seed, *r, relay);
+    if (rc != OR_OK) { delete r; return rc; }
+    *handle = r;
+    return OR_OK;
+}
+
+// BFS mode with the switch model of section 4.7: buf_limit[n_npus] (0xFFFFFFFF = no limit) and no_mcast[n_npus]
+// (non-zero = the node forwards one transfer at a time); either may be NULL
+int oracle_synthesize_switches(uint32_t n_npus, const oracle_link* links, uint32_t n_links,
+                               const uint32_t* group, uint32_t n_members, uint32_t n_chunks,
+                               const oracle_pair* pre, uint64_t n_pre, const oracle_pair* post,
+                               uint64_t n_post, uint64_t chunk_bytes, uint64_t seed,
+                               const uint32_t* buf_limit, const uint8_t* no_mcast, void** handle) {
+    if (!handle) return OR_ERR_INVALID;
+    Result* r = new Result();
+    SwitchModel sw;
+    sw.buf_limit = buf_limit; sw.no_mcast = no_mcast;
+    const int rc = synthesize(n_npus, (const Link*)links, n_links, group, n_members, n_chunks,
+                              (const Pair*)pre, n_pre, (const Pair*)post, n_post, chunk_bytes,
+                              seed, *r, 2, sw);
     if (rc != OR_OK) { delete r; return rc; }
     *handle = r;
     return OR_OK;

@@ -57,7 +57,7 @@ struct Globals {
     cudaEvent_t loop_done = nullptr;
     std::atomic<uint64_t> launches{0};   // kernels launched by the library (pccl_launch_count)
     // process-wide options (pccl_set_option); 0 = default
-    std::atomic<uint64_t> opt_bfs_window{0}, opt_bfs_rows{0};
+    std::atomic<uint64_t> opt_bfs_window{0}, opt_bfs_rows{0}, opt_dyn_records{0};
 } G;
 
 // every kernel launch of the library passes its stream through here: the count is the library's own evidence of what
@@ -325,6 +325,7 @@ extern "C" int pccl_set_option(int option, uint64_t value) {
     switch (option) {
         case PCCL_OPT_BFS_WINDOW: G.opt_bfs_window = value; return PCCL_OK;
         case PCCL_OPT_BFS_ROWS: G.opt_bfs_rows = value; return PCCL_OK;
+        case PCCL_OPT_DYNAMIC_RECORDS: G.opt_dyn_records = value; return PCCL_OK;
         default: return PCCL_ERR_INVALID;
     }
 }
@@ -332,6 +333,7 @@ extern "C" uint64_t pccl_get_option(int option) {
     switch (option) {
         case PCCL_OPT_BFS_WINDOW: return G.opt_bfs_window;
         case PCCL_OPT_BFS_ROWS: return G.opt_bfs_rows;
+        case PCCL_OPT_DYNAMIC_RECORDS: return G.opt_dyn_records;
         default: return 0;
     }
 }
@@ -1001,9 +1003,16 @@ int launch_count_sweep(const LoopArgs& a, uint32_t flags) {
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, SW_THREADS, smem));
     if (occ < 1) return PCCL_ERR_CUDA;
-    const uint32_t grid = std::min<uint32_t>(a.N, (uint32_t)occ * (uint32_t)G.sm_count);
-    if (tma) k_count_sweep<true><<<grid, SW_THREADS, smem, counted(st)>>>(a);
-    else k_count_sweep<false><<<grid, SW_THREADS, smem, counted(st)>>>(a);
+    // (the kernel can cut a row into parts to balance the CTAs; measured on B200 the restart of the copy pipeline per part
+    // costs the TMA form more than the balance gains -- 70 -> 77 us on the 28x28 workload -- so rows stay whole)
+    const uint32_t resident = (uint32_t)occ * (uint32_t)G.sm_count;
+    const uint32_t parts = 1;
+    LoopArgs b = a;
+    b.flags = parts;                                           // (the sweep kernel reads its parts count here)
+    if (parts > 1) CU(cudaMemsetAsync(a.gtot, 0, (size_t)a.L * 4, st));
+    const uint32_t grid = (uint32_t)std::min<uint64_t>((uint64_t)a.N * parts, resident);
+    if (tma) k_count_sweep<true><<<grid, SW_THREADS, smem, counted(st)>>>(b);
+    else k_count_sweep<false><<<grid, SW_THREADS, smem, counted(st)>>>(b);
     CU(cudaGetLastError());
     return PCCL_OK;
 }
@@ -1013,6 +1022,60 @@ struct LoopResult {
     uint32_t grid;
 };
 
+// A phase of the call: an NVTX range (setup / loop / emit, visible in Nsight Systems and ncu --nvtx) and, with
+// PCCL_FLAG_TIME_LOOP, a pair of CUDA events around every segment of it (read once at the end of the call: recording
+// does not synchronise).
+struct Timer {
+    const char* name;
+    bool on = false, open = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> seg;
+    explicit Timer(const char* n) : name(n) {}
+    void init(bool enable) { on = enable; }
+    void start() {
+        if (open) return;
+        nvtxRangePushA(name);
+        open = true;
+        if (!on) return;
+        cudaEvent_t a = nullptr, b = nullptr;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) {
+            (void)cudaGetLastError();
+            if (a) cudaEventDestroy(a);
+            on = false;
+            return;
+        }
+        try {
+            seg.emplace_back(a, b);
+        } catch (const std::bad_alloc&) {
+            cudaEventDestroy(a); cudaEventDestroy(b);
+            on = false;
+            return;
+        }
+        cudaEventRecord(a, G.stream);
+    }
+    void stop() {
+        if (!open) return;
+        nvtxRangePop();
+        open = false;
+        if (on && !seg.empty()) cudaEventRecord(seg.back().second, G.stream);
+    }
+    float total() {   // milliseconds over all segments (waits for the last event of each)
+        float acc = 0.f;
+        for (auto& p : seg) {
+            float ms = 0.f;
+            if (cudaEventSynchronize(p.second) == cudaSuccess && cudaEventElapsedTime(&ms, p.first, p.second) == cudaSuccess) acc += ms;
+            else (void)cudaGetLastError();
+        }
+        return acc;
+    }
+    ~Timer() {
+        if (open) nvtxRangePop();
+        for (auto& p : seg) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
+    }
+};
+struct Timers {
+    Timer setup{"pccl:setup"}, loop{"pccl:loop"}, emit{"pccl:emit"};
+};
+
 // stable LSD radix sort / reduce emitter, defined below
 int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out, bool reverse, uint64_t shift);
 
@@ -1020,7 +1083,7 @@ int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out, bool 
 // tables, the loop, and the ranking of the logged claims into canonical order.  `raw_only`: leave the records in log
 // order (a transposed phase sorts them after the reversal anyway).
 int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint32_t flags, Rec* out,
-                     uint64_t out_cap, uint64_t t_offset, bool raw_only, LoopResult* res) {
+                     uint64_t out_cap, uint64_t t_offset, bool raw_only, LoopResult* res, Timers* tm) {
     const pccl_topology* t = P.topo;
     const PhaseView pv = view_of(t, ph.transposed);
     const uint32_t N = t->N, L = t->L;
@@ -1060,6 +1123,7 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     CU(cudaMemsetAsync(b + o_ff, 0xFF, o_zero - o_ff, st));
     CU(cudaMemsetAsync(b + o_zero, 0, c.cur - o_zero, st));
     // entries, translation tables, private images (once per phase)
+    if (tm) tm->setup.start();
     k_a2_entries<<<N, 256, 0, counted(st)>>>(a);
     if (L) k_a2_xmap<<<L, 128, 0, counted(st)>>>(a);
     k_a2_priv<<<N, 128, 0, counted(st)>>>(a);
@@ -1070,7 +1134,9 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_loop2, threads, smem));
     if (occ < 1 || (uint64_t)occ * (uint64_t)G.sm_count < W.a2_grid) return PCCL_ERR_INTERNAL;   // (checked by the caller's plan)
     void* args[] = {(void*)&a};
+    if (tm) { tm->setup.stop(); tm->loop.start(); }
     CU(cudaLaunchCooperativeKernel((const void*)k_loop2, dim3(W.a2_grid), dim3(threads), args, smem, counted(st)));
+    if (tm) { tm->loop.stop(); tm->emit.start(); }
     // emit
     k_emit_times<<<N, 256, 0, counted(st)>>>(a);
     if (!raw_only) {
@@ -1083,6 +1149,7 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
         k_emit_raw<<<N, 256, 0, counted(st)>>>(a);
     }
     CU(cudaGetLastError());
+    if (tm) tm->emit.stop();
     LoopCtrl* mb = (LoopCtrl*)G.mailbox;
     A2Ctrl* mb2 = (A2Ctrl*)((unsigned char*)G.mailbox + 1024);
     CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
@@ -1105,7 +1172,9 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
         A2Args a2 = a;
         a2.out = tmp; a2.t_offset = 0;
         k_emit_raw<<<N, 256, 0, counted(st)>>>(a2);
+        if (tm) tm->emit.start();
         rc = reverse_sorted(tmp, mb2->total, mb2->tmax, L, out, false, t_offset);
+        if (tm) tm->emit.stop();
         cudaError_t e = cudaStreamSynchronize(st);
         dev_free(tmp);
         if (rc) return rc;
@@ -1122,12 +1191,12 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
 // host_out (optional, pinned, out_cap records): with the one-barrier loop the records are copied there while the
 // loop runs (the kernel publishes how many are final, this thread issues the copies); *streamed says whether
 int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint32_t flags, Rec* out,
-               uint64_t out_cap, uint64_t t_offset, LoopResult* res, std::vector<uint64_t>* trace = nullptr,
+               uint64_t out_cap, uint64_t t_offset, LoopResult* res, Timers* tm, std::vector<uint64_t>* trace = nullptr,
                Rec* host_out = nullptr, bool* streamed = nullptr) {
     const bool dynamic = (flags & PCCL_FLAG_DYNAMIC_RELAY) != 0;
     if (W.a2_planned && out_cap > 0 && out_cap <= 0xFFFFFFFFull && W.a2.smem_need <= 220 * 1024 &&
         ((flags & PCCL_FLAG_ASYNC) || W.a2.w_max / 16 <= W.a2.w_min))
-        return phase_loop_async(P, ph, W, seed, flags, out, out_cap, t_offset, ph.transposed, res);
+        return phase_loop_async(P, ph, W, seed, flags, out, out_cap, t_offset, ph.transposed, res, tm);
     // the dynamic rule keeps the counts current too: wants bits are only dropped where a neighbour holds the chunk
     // (holder lists, dyn_shrink_wants); DENSE_SWEEP / RESCAN recount instead and drop every bit at once
     const pccl_topology* t = P.topo;
@@ -1204,10 +1273,13 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
         CU(cudaHostGetDevicePointer(&dp, (void*)progress, 0));
         a.progress = (unsigned long long*)dp;
     }
+    if (tm) tm->setup.start();
     k_loop_init<<<(n_init + 255) / 256, 256, 0, counted(st)>>>(a);
     if (a.gcnt != nullptr && a.L) { const int rcs = launch_count_sweep(a, flags); if (rcs) return rcs; }
     void* args[] = {(void*)&a};
+    if (tm) { tm->setup.stop(); tm->loop.start(); }
     CU(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(threads), args, smem, counted(st)));
+    if (tm) tm->loop.stop();
     LoopCtrl* mb = (LoopCtrl*)G.mailbox;
     CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
     if (stream_out) {
@@ -1300,36 +1372,6 @@ int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out, bool 
     dev_free(blob);   // stream-ordered: freed after the kernels above
     return e == cudaSuccess ? PCCL_OK : PCCL_ERR_CUDA;
 }
-
-// A phase of the call: an NVTX range (setup / loop / emit, visible in Nsight Systems and ncu --nvtx) and, with
-// PCCL_FLAG_TIME_LOOP, CUDA events around it.
-struct Timer {
-    const char* name;
-    cudaEvent_t a = nullptr, b = nullptr;
-    bool on = false, open = false;
-    float acc = 0.f;
-    explicit Timer(const char* n) : name(n) {}
-    void init(bool enable) {
-        on = enable && cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess;
-    }
-    void start() {
-        if (!open) { nvtxRangePushA(name); open = true; }
-        if (on) cudaEventRecord(a, G.stream);
-    }
-    void stop() {   // call after the stream was synchronised or right before a sync
-        if (open) { nvtxRangePop(); open = false; }
-        if (!on) return;
-        cudaEventRecord(b, G.stream);
-        cudaEventSynchronize(b);
-        float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) acc += ms;
-    }
-    ~Timer() {
-        if (open) nvtxRangePop();
-        if (a) cudaEventDestroy(a);
-        if (b) cudaEventDestroy(b);
-    }
-};
 
 // ---------------------------------------------------------------------------------------
 // PCCL_FLAG_BFS: one phase of the paper's own synthesizer (pccl_bfs.cuh).  On return *out_recs
@@ -1510,7 +1552,8 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
     if (!S) return PCCL_ERR_NOMEM;
     memset(&S->stats, 0, sizeof(S->stats));
     S->stats.mode = (uint32_t)P->mode;
-    Timer t_setup("pccl:setup"), t_loop("pccl:loop"), t_emit("pccl:emit");
+    Timers tm;
+    Timer &t_setup = tm.setup, &t_loop = tm.loop, &t_emit = tm.emit;
     const bool timed = (flags & PCCL_FLAG_TIME_LOOP) != 0;
     t_setup.init(timed); t_loop.init(timed); t_emit.init(timed);
 
@@ -1577,14 +1620,21 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
         const bool plan_async = !dynamic && !(flags & (PCCL_FLAG_RESCAN | PCCL_FLAG_DENSE_SWEEP | PCCL_FLAG_TWO_BARRIERS |
                                                       PCCL_FLAG_BARRIER_LOOP | PCCL_FLAG_TRACE)) &&
                                 deg_view <= A2_MAX_IN && P->topo->N <= (uint32_t)G.sm_count * A2_MAX_WARPS;
+        uint64_t M_thin = 0;
+        if (dynamic) {   // the thin relay tree's transfer count sizes the dynamic rule's record buffer (below)
+            rc = phase_setup(*P, ph, W, seed, &M_thin, false, false);
+            if (rc) return fail(rc);
+        }
         rc = phase_setup(*P, ph, W, seed, &M, dynamic, plan_async);
         if (rc) return fail(rc);
         t_setup.stop();
         S->stats.wants_total += M;
         // thin relay tree: exactly M transfers.  dynamic rule: at most M (a (node, chunk) pair is claimed at most once),
-        // usually far fewer (config 4: 58 M initial wants, 1.58 M transfers): the record buffer starts at a few records
-        // per (chunk, dest) pair and, if that is short, the phase is rerun with the exact count the first run reports
-        uint64_t cap = dynamic ? std::min<uint64_t>(M, std::max<uint64_t>(4 * (uint64_t)ph.dests.size() + P->topo->N, 1u << 16)) : M;
+        // in practice a little more than the thin tree's count (config 4: 58 M initial wants, 1.573 M thin-tree transfers,
+        // 1.579 M with the rule): the record buffer holds 1.25 x the thin tree's count and, if that is short, the phase
+        // is rerun with the exact count the first run reports
+        uint64_t cap = dynamic ? std::min<uint64_t>(M, M_thin + M_thin / 4 + P->topo->N + 1024) : M;
+        if (dynamic && G.opt_dyn_records) cap = std::min<uint64_t>(M, G.opt_dyn_records);   // (tests: force the rerun)
         LoopResult lr;
         memset(&lr, 0, sizeof(lr));
         for (int attempt = 0;; ++attempt) {
@@ -1597,16 +1647,13 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
             if (ph.transposed) {
                 rc = dev_alloc(cap * sizeof(Rec), (void**)&raw);
                 if (rc) return fail(rc);
-                t_loop.start();
-                rc = phase_loop(*P, ph, W, seed, flags, raw, cap, 0, &lr, &S->trace);
+                rc = phase_loop(*P, ph, W, seed, flags, raw, cap, 0, &lr, &tm, &S->trace);
                 if (rc == PCCL_ERR_NOMEM && dynamic && attempt == 0 && lr.total > cap && lr.total <= M) {
-                    t_loop.stop();
                     dev_free(raw); raw = nullptr;
                     cap = lr.total;
                     continue;
                 }
                 if (rc) return fail(rc);
-                t_loop.stop();
                 if (dynamic ? lr.total > M : lr.total != M) return fail(PCCL_ERR_INTERNAL);
                 M = lr.total;
                 Rec* dst = nullptr;
@@ -1639,16 +1686,13 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
                     S->h_bytes = cap * sizeof(Rec);
                     S->h_recs = pinned_get(S->h_bytes);   // null: no streaming, the download reports the failure
                 }
-                t_loop.start();
-                rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, cap, toff, &lr, &S->trace, (Rec*)S->h_recs, &streamed);
+                rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, cap, toff, &lr, &tm, &S->trace, (Rec*)S->h_recs, &streamed);
                 if (rc == PCCL_ERR_NOMEM && dynamic && attempt == 0 && lr.total > cap && lr.total <= M) {
-                    t_loop.stop();
                     dev_free(out_recs); out_recs = nullptr;
                     cap = lr.total;
                     continue;
                 }
                 if (rc) return fail(rc);
-                t_loop.stop();
                 if (dynamic ? lr.total > M : lr.total != M) return fail(PCCL_ERR_INTERNAL);
                 M = lr.total;
                 S->M = base + M;
@@ -1670,7 +1714,7 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
     S->d_recs = out_recs;
     S->n_links = P->topo->L;
     S->n_npus = P->topo->N;
-    S->stats.loop_ms = t_loop.acc; S->stats.setup_ms = t_setup.acc; S->stats.emit_ms = t_emit.acc;
+    S->stats.loop_ms = t_loop.total(); S->stats.setup_ms = t_setup.total(); S->stats.emit_ms = t_emit.total();
     if (!(flags & PCCL_FLAG_KEEP_ON_DEVICE)) {
         if (S->M && !pccl_schedule_transfers(S)) { pccl_schedule_destroy(S); return PCCL_ERR_CUDA; }
     }

@@ -485,11 +485,14 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
                 if ((mine >> lane) & 1u) {
                     const uint64_t rank = pre + __popc(mine & ((1u << lane) - 1u));
                     const uint64_t wl = a.w[l];
-                    if (emit_base + rank >= a.out_cap) { atomicOr(&a.ctrl->err, 32u); continue; }
-                    uint4* o = reinterpret_cast<uint4*>(a.out + emit_base + rank);
-                    const uint64_t ts = f - wl + a.t_offset, te = f + a.t_offset;
-                    o[0] = make_uint4(c, a.psrc[l], a.pdst[l], l);
-                    o[1] = make_uint4((uint32_t)ts, (uint32_t)(ts >> 32), (uint32_t)te, (uint32_t)(te >> 32));
+                    if (emit_base + rank >= a.out_cap) {
+                        atomicOr(&a.ctrl->err, 32u);   // the record is dropped, the run goes on: its total sizes the rerun
+                    } else {
+                        uint4* o = reinterpret_cast<uint4*>(a.out + emit_base + rank);
+                        const uint64_t ts = f - wl + a.t_offset, te = f + a.t_offset;
+                        o[0] = make_uint4(c, a.psrc[l], a.pdst[l], l);
+                        o[1] = make_uint4((uint32_t)ts, (uint32_t)(ts >> 32), (uint32_t)te, (uint32_t)(te >> 32));
+                    }
                 }
             }
         }

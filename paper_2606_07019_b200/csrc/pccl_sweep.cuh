@@ -65,7 +65,14 @@ __global__ void __launch_bounds__(SW_THREADS) k_count_sweep(LoopArgs a) {
         __syncthreads();
     }
     uint32_t phase_bits = 0;                                     // parity of each stage's barrier (bit s)
-    for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x) {
+    // work units: (destination v, sweep of NB in-links, part of the row) dealt round-robin to the CTAs -- `parts` row
+    // parts per destination keep the CTAs balanced when there are only a few destinations per CTA
+    const uint32_t parts = max(1u, a.flags);                      // (a.flags carries the number of parts here)
+    const uint32_t per_part = (nsl + parts - 1) / parts;
+    for (uint32_t unit = blockIdx.x; unit < a.N * parts; unit += gridDim.x) {
+        const uint32_t v = unit / parts, part = unit - v * parts;
+        const uint32_t k_lo = part * per_part, k_hi = min(nsl, k_lo + per_part);
+        if (k_lo >= k_hi) continue;                               // block-uniform
         const uint32_t e0 = a.in_off[v], e1 = a.in_off[v + 1];
         for (uint32_t eb = e0; eb < e1; eb += NB) {              // in-links in sweeps of NB
             const uint32_t nb = min((uint32_t)NB, e1 - eb);
@@ -76,8 +83,8 @@ __global__ void __launch_bounds__(SW_THREADS) k_count_sweep(LoopArgs a) {
 #pragma unroll
             for (int j = 0; j < NB; ++j) tot[j] = 0;
             if (TMA) {
-                auto issue = [&](uint32_t k) {                   // thread 0: slice k of all rows into stage k % STAGES
-                    const uint32_t st = k % SW_STAGES;
+                auto issue = [&](uint32_t k) {                   // thread 0: slice k of all rows into stage (k - k_lo) % STAGES
+                    const uint32_t st = (k - k_lo) % SW_STAGES;
                     const uint32_t q0 = k * SW_SLICE_U4, nq = min((uint32_t)SW_SLICE_U4, Q - q0);
                     unsigned char* base = sw_smem + (size_t)st * SW_ROWS * SW_SLICE_U4 * 16;
                     mbar_expect_tx(&full[st], (nb + 1) * nq * 16);
@@ -86,10 +93,10 @@ __global__ void __launch_bounds__(SW_THREADS) k_count_sweep(LoopArgs a) {
                         bulk_g2s(base + (size_t)(j + 1) * SW_SLICE_U4 * 16, have4 + (size_t)s_src[j] * Q + q0, nq * 16, &full[st]);
                 };
                 if (tid == 0)
-                    for (uint32_t k = 0; k < SW_STAGES - 1 && k < nsl; ++k) issue(k);
-                for (uint32_t k = 0; k < nsl; ++k) {
-                    if (tid == 0 && k + SW_STAGES - 1 < nsl) issue(k + SW_STAGES - 1);   // its stage was handed back at the end of slice k - 1
-                    const uint32_t st = k % SW_STAGES;
+                    for (uint32_t k = k_lo; k < k_lo + SW_STAGES - 1 && k < k_hi; ++k) issue(k);
+                for (uint32_t k = k_lo; k < k_hi; ++k) {
+                    if (tid == 0 && k + SW_STAGES - 1 < k_hi) issue(k + SW_STAGES - 1);   // its stage was handed back at the end of slice k - 1
+                    const uint32_t st = (k - k_lo) % SW_STAGES;
                     mbar_wait(&full[st], (phase_bits >> st) & 1u);
                     phase_bits ^= 1u << st;
                     const uint4* base = reinterpret_cast<const uint4*>(sw_smem + (size_t)st * SW_ROWS * SW_SLICE_U4 * 16);
@@ -108,7 +115,7 @@ __global__ void __launch_bounds__(SW_THREADS) k_count_sweep(LoopArgs a) {
                     __syncthreads();                              // every thread is done with the stage: it may be refilled
                 }
             } else {
-                for (uint32_t k = 0; k < nsl; ++k) {
+                for (uint32_t k = k_lo; k < k_hi; ++k) {
                     const uint32_t q = k * SW_SLICE_U4 + tid;
                     const bool ok = q < Q;
                     uint4 wv = make_uint4(0, 0, 0, 0), hv[NB];
@@ -134,7 +141,8 @@ __global__ void __launch_bounds__(SW_THREADS) k_count_sweep(LoopArgs a) {
             if (tid < nb) {
                 uint32_t t = 0;
                 for (int w = 0; w < SW_THREADS / 32; ++w) t += s_tot[tid][w];
-                a.gtot[s_link[tid]] = t;
+                if (parts == 1) a.gtot[s_link[tid]] = t;
+                else if (t) atomicAdd(&a.gtot[s_link[tid]], t);  // (zeroed by the launcher)
             }
         }
     }

@@ -257,3 +257,165 @@ def test_first_routed_condition_takes_c_dist():
     assert s.time_ps >= 4 * w
     first = int(np.lexsort((np.arange(16), wl.philox_first_word(np.arange(16), 0, 0, 2, p.seed)))[0])
     assert int(s.transfers[s.transfers["chunk"] == first]["t_end_ps"].max()) == 4 * w
+
+
+# ------------------------------------------------------------------ section 4.7: switches (Q23-Q25)
+def literal_ten_switches(n, links, conds, seed, limit, nomc):
+    """The literal TEN again, with the paper's two switch rules written timestep by timestep: a visit of node v at
+    timestep a is skipped while limit[v] chunks of EARLIER conditions are buffered there at a (a stay lasts from the
+    arrival to the end of the last kept transfer out); a node in `nomc` starts its out-links one at a time, in ascending
+    link id, the next no earlier than the end of the one before."""
+    w = [int(k["alpha_ps"]) + 1 for k in links]
+    out_links = [[l for l, k in enumerate(links) if int(k["src"]) == u] for u in range(n)]
+    removed = set()
+    stays = {v: [] for v in range(n)}
+    keyed = []
+    for c, (src, dests) in enumerate(conds):
+        if dests:
+            D = _hop_costs(n, links, w, src)
+            keyed.append((-max(D[d] for d in dests), int(wl.philox_first_word(c, 0, 0, 2, seed)), c))
+    out = []
+
+    def full(v, a):
+        return v in limit and sum(1 for (x, y) in stays[v] if x <= a < y) >= limit[v]
+
+    for _, _, c in sorted(keyed):
+        src, dests = conds[c]
+        arr, pred = {src: 0}, {}
+        ptr, busy_until = {}, {}                       # no-multicast nodes: next out-link to serve, end of the current send
+        t = 0
+        while not all(d in arr and arr[d] <= t for d in dests):
+            for u in range(n):
+                if u not in arr or arr[u] > t:
+                    continue
+                if u in nomc:
+                    ptr.setdefault(u, 0)
+                    if t < busy_until.get(u, 0) or ptr[u] >= len(out_links[u]):
+                        continue
+                    todo = [out_links[u][ptr[u]]]
+                else:
+                    todo = out_links[u]
+                for l in todo:
+                    v = int(links[l]["dst"])
+                    if limit.get(v, 1) == 0:           # never visitable: the turn passes without a send
+                        if u in nomc:
+                            ptr[u] += 1
+                        continue
+                    if any((t + i, l) in removed for i in range(w[l])) or full(v, t + w[l]):
+                        continue                       # (a serial node waits at this out-link)
+                    a = t + w[l]
+                    if u in nomc:
+                        ptr[u] += 1
+                        busy_until[u] = a
+                    if v == src:
+                        continue
+                    if v not in arr or a < arr[v] or (a == arr[v] and l < pred[v][0]):
+                        arr[v], pred[v] = a, (l, t)
+            t += 1
+            assert t < 10_000
+        keep = set()
+        for d in dests:
+            v = d
+            while v != src and v not in keep:
+                keep.add(v)
+                v = int(links[pred[v][0]]["src"])
+        last_out = {}
+        for v in sorted(keep):
+            l, ts = pred[v]
+            out.append((ts, l, c, int(links[l]["src"]), v, ts + w[l]))
+            for i in range(w[l]):
+                assert (ts + i, l) not in removed
+                removed.add((ts + i, l))
+            u = int(links[l]["src"])
+            last_out[u] = max(last_out.get(u, 0), ts + w[l])
+        for v in keep:
+            if v in limit and v in last_out:
+                stays[v].append((arr[v], last_out[v]))
+    out.sort()
+    return out
+
+
+def _switch_arrays(n, limit, nomc):
+    bl = np.full(n, oracle.NO_LIMIT, dtype=np.uint32)
+    for v, k in limit.items():
+        bl[v] = k
+    nm = np.zeros(n, dtype=np.uint8)
+    nm[list(nomc)] = 1
+    return bl, nm
+
+
+@pytest.mark.parametrize("i", range(40))
+def test_switch_rules_against_the_literal_ten(i):
+    n, triples, conds, members = _random_case(i)
+    rng = np.random.default_rng(8100 + i)
+    others = [v for v in range(n) if v not in members] or list(range(n))
+    limit = {int(v): int(rng.integers(1, 3)) for v in rng.choice(others, size=min(len(others), int(rng.integers(1, 4))), replace=False)} if i % 4 != 3 else {}
+    nomc = set(int(v) for v in rng.choice(n, size=int(rng.integers(1, 3)), replace=False)) if i % 2 else set()
+    p = _problem(f"sw{i}", n, triples, conds, seed=i, group=members)
+    bl, nm = _switch_arrays(n, limit, nomc)
+    s = oracle.synthesize(*p.args(), relay=BFS, buffer_limit=bl, no_multicast=nm)
+    assert _as_tuples(s.transfers) == literal_ten_switches(n, p.links, conds, i, limit, nomc)
+    checker.check_structure(p, s.transfers)
+
+
+def test_no_limits_is_the_plain_bfs_mode():
+    for i in range(6):
+        n, triples, conds, members = _random_case(i)
+        p = _problem(f"sw_none{i}", n, triples, conds, seed=i, group=members)
+        bl, nm = _switch_arrays(n, {}, set())
+        a = oracle.synthesize(*p.args(), relay=BFS, buffer_limit=bl, no_multicast=nm)
+        b = run(p)
+        assert _as_tuples(a.transfers) == _as_tuples(b.transfers)
+    for mk in (wl.config3, wl.config4_small):
+        p = mk(0)
+        bl, nm = _switch_arrays(p.n_npus, {}, set())
+        a = oracle.synthesize(*p.args(), relay=BFS, buffer_limit=bl, no_multicast=nm)
+        assert _as_tuples(a.transfers) == _as_tuples(run(p).transfers)
+
+
+def test_buffer_limit_hand_example():
+    """NPUs 0, 1 -> switch 2 -> NPUs 3, 4, unit links.  Two chunks (0 -> 3, 1 -> 4) cross the switch side by side in two
+    timesteps when it buffers two chunks; with a one-chunk buffer the second may only ARRIVE once the first has left:
+    it starts at 1 (arrival 2 = the first one's release), leaves over [2, 3): three timesteps."""
+    tri = [(0, 2, 1), (1, 2, 1), (2, 3, 1), (2, 4, 1)]
+    conds = [(0, [3]), (1, [4])]
+    p = _problem("two_through_one_switch", 5, tri, conds, seed=0, group=[0, 1, 3, 4])
+    assert run(p).time_ps == 2
+    bl, nm = _switch_arrays(5, {2: 1}, set())
+    s = oracle.synthesize(*p.args(), relay=BFS, buffer_limit=bl, no_multicast=nm)
+    assert s.time_ps == 3
+    t = _as_tuples(s.transfers)
+    into = sorted(r for r in t if r[4] == 2)
+    assert [r[0] for r in into] == [0, 1] and [r[5] for r in into] == [1, 2]      # arrivals at the switch: 1, then 2
+    bl2, _ = _switch_arrays(5, {2: 2}, set())
+    assert oracle.synthesize(*p.args(), relay=BFS, buffer_limit=bl2, no_multicast=nm).time_ps == 2
+    bl0, _ = _switch_arrays(5, {2: 0}, set())
+    with pytest.raises(oracle.OracleError) as e:                                    # a switch without buffers cannot relay
+        oracle.synthesize(*p.args(), relay=BFS, buffer_limit=bl0, no_multicast=nm)
+    assert e.value.code == oracle.ERR_UNREACHABLE
+
+
+def test_no_multicast_hand_example():
+    """0 -> switch 1 -> {2, 3, 4}: one chunk for all three.  With multicast the switch sends the three copies at once
+    (arrivals 2, 2, 2); without, one after the other in link order (arrivals 2, 3, 4)."""
+    tri = [(0, 1, 1), (1, 2, 1), (1, 3, 1), (1, 4, 1)]
+    p = _problem("fanout", 5, tri, [(0, [2, 3, 4])], seed=0, group=[0, 2, 3, 4])
+    assert sorted(r[5] for r in _as_tuples(run(p).transfers) if r[3] == 1) == [2, 2, 2]
+    bl, nm = _switch_arrays(5, {}, {1})
+    s = oracle.synthesize(*p.args(), relay=BFS, buffer_limit=bl, no_multicast=nm)
+    assert [(r[4], r[0], r[5]) for r in _as_tuples(s.transfers) if r[3] == 1] == [(2, 1, 2), (3, 2, 3), (4, 3, 4)]
+    assert s.time_ps == 4
+
+
+def test_switch_model_on_config3():
+    """config 3's pod switches with two-chunk buffers and no multicast: still a valid Reduce-Scatter, not faster than
+    with ideal switches, and every visit respected the buffers of the conditions routed before it."""
+    p = wl.config3(0)
+    base = run(p)
+    bl = np.full(p.n_npus, oracle.NO_LIMIT, dtype=np.uint32)
+    bl[64:] = 2
+    nm = np.zeros(p.n_npus, dtype=np.uint8)
+    nm[64:] = 1
+    s = oracle.synthesize(*p.args(), relay=BFS, buffer_limit=bl, no_multicast=nm)
+    checker.check_schedule(p, s.transfers)
+    assert s.time_ps >= base.time_ps and len(s.transfers) >= 1408

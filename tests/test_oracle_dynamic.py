@@ -6,7 +6,10 @@ PAPER.md:294-300); what the paper fixes still binds it and is checked here: vali
 The rule itself -- "a node takes a chunk only if it is strictly closer to some destination
 than the source and every node that claimed the chunk at an EARLIER event" -- is re-derived
 from the emitted schedule with scipy distances, so a wrong sign, a non-strict comparison or
-an update applied inside the event instead of at its end fails here.
+an update applied inside the event instead of at its end fails here.  The first test below is the necessary
+side (every claim satisfied the rule); test_the_rule_is_work_conserving is the sufficient side (at every event
+every free link whose candidate set under the rule is non-empty starts a transfer of one of exactly those
+candidates), which is what catches an update applied too early (claims would go missing) or a link left idle.
 """
 import numpy as np
 import pytest
@@ -71,6 +74,84 @@ def test_every_claim_was_strictly_closer_than_all_earlier_holders(maker, seed):
         holders[c].append((t, v))
     # and nothing useful was left undone: every dest holds its chunks (checker V4)
     checker.check_schedule(p, tr)
+
+
+def _torus3_a2a(seed):
+    m = np.arange(27, dtype=np.uint32)
+    nc, pre, post = wl.all_to_all(m)
+    return wl.Problem("torus3x3x3_alltoall", 27, wl.grid_links((3, 3, 3), wrap=True), m, nc, pre, post, 1 << 16, seed)
+
+
+def _mesh_multi_dest(seed):
+    """4x3 mesh, 10 chunks with 2..6 dests each, heterogeneous links: multi-dest chunks, several claimants per chunk"""
+    rng = np.random.default_rng(77 + seed)
+    links = wl.grid_links((4, 3), wrap=False).copy()
+    links["alpha_ps"] = rng.integers(100, 900, len(links))
+    links["bytes_per_ps"] = rng.integers(1, 9, len(links))
+    m = np.arange(12, dtype=np.uint32)
+    pre, post = [], []
+    for c in range(10):
+        s = int(rng.integers(0, 12))
+        pre.append((s, c))
+        for d in rng.choice(12, size=int(rng.integers(2, 7)), replace=False):
+            post.append((int(d), c))
+    return wl.Problem("mesh4x3_multidest", 12, links, m, 10, np.array(pre, dtype=wl.PAIR_DT), np.array(post, dtype=wl.PAIR_DT),
+                      2000, seed)
+
+
+@pytest.mark.parametrize("maker", [wl.config1, wl.two_groups_mesh3x3, _torus3_a2a, _mesh_multi_dest,
+                                   lambda s: wl.ring_all_gather(7, True, s, chunks_per_npu=3),
+                                   lambda s: wl.path_point_to_point(5, s)], ids=lambda m: getattr(m, "__name__", "case"))
+@pytest.mark.parametrize("seed", [0, 1])
+def test_the_rule_is_work_conserving(maker, seed):
+    """The sufficient side of reading Q18, event by event, from the emitted schedule alone (scipy distances):
+    at every event time t and for every node v, its in-links in ascending id that are free at t are served in turn;
+    candidates of link l = chunks its source holds by t (own, or delivered with t_end <= t) that v has not claimed
+    before t nor at t through an earlier in-link, and for which v is strictly closer to some dest than the source and
+    every claimant of an event BEFORE t.  A non-empty candidate set must start a transfer of one of its members at t;
+    an empty one must not start anything."""
+    p = maker(seed)
+    tr = run(p).transfers
+    D = _dist_to(p)
+    src, dests = _conditions(p)
+    n, L, C = p.n_npus, len(p.links), p.n_chunks
+    inl = [[] for _ in range(n)]
+    for l in range(L):
+        inl[int(p.links[l]["dst"])].append(l)
+    starts = {}                                   # (t_start, link) -> chunk
+    for r in tr:
+        starts[(int(r["t_start_ps"]), int(r["link"]))] = int(r["chunk"])
+    events = sorted({0} | {int(x) for x in tr["t_end_ps"]})
+    assert {int(x) for x in tr["t_start_ps"]} <= set(events)
+    for t in events:
+        done = tr[tr["t_end_ps"] <= t]
+        before = tr[tr["t_start_ps"] < t]
+        have = np.zeros((n, C), dtype=bool)
+        for c, s_ in src.items():
+            have[s_, c] = True
+        have[done["dst"], done["chunk"]] = True
+        claimed = np.zeros((n, C), dtype=bool)
+        claimed[before["dst"], before["chunk"]] = True
+        wants = np.zeros((n, C), dtype=bool)
+        for c, ds in dests.items():
+            holders = [src[c]] + [int(v) for v in before["dst"][before["chunk"] == c]]
+            for d in ds:
+                wants[:, c] |= D[d] < min(D[d][h] for h in holders)
+        wants &= ~claimed
+        busy = set(int(l) for l in before["link"][before["t_end_ps"] > t])
+        for v in range(n):
+            now = set()
+            for l in inl[v]:
+                if l in busy:
+                    assert (t, l) not in starts
+                    continue
+                cand = {int(c) for c in np.nonzero(have[int(p.links[l]["src"])] & wants[v])[0]} - now
+                got = starts.get((t, l))
+                if cand:
+                    assert got in cand, f"{p.name}: t={t} link {l}: candidates {sorted(cand)[:8]}.. but the link carries {got}"
+                    now.add(got)
+                else:
+                    assert got is None, f"{p.name}: t={t} link {l} carries {got} with no candidate under the rule"
 
 
 @pytest.mark.parametrize("maker", [wl.config1, wl.config2, wl.config3, wl.config4_small, wl.config5_small,

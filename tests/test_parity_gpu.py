@@ -132,6 +132,30 @@ def test_a2_wants_bitmap(pk, maker, seed):
     assert np.array_equal(got["npu"], want["npu"]) and np.array_equal(got["chunk"], want["chunk"])
 
 
+@pytest.mark.parametrize("maker", [wl.config1, wl.config4_small, wl.config5_small, wl.two_groups_mesh3x3,
+                                   lambda s: wl.ring_all_gather(8, True, s, chunks_per_npu=1040, chunk_bytes=4096),
+                                   lambda s: wl.full_mesh_problem(40, "allgather", seed=s)],
+                         ids=lambda m: getattr(m, "__name__", "case"))
+def test_a5_candidate_sweep(pk, maker):
+    """Row a5 alone: |have[src_l] & wants[dst_l]| of every link at t = 0 from the streaming sweep kernel (rows staged by
+    bulk asynchronous copies, and the per-lane-load form) against the oracle's wants relation intersected with the
+    initial holdings -- rows of 1, 2, 130 and 4088 words, 39 in-links per destination (five sweeps of 8)."""
+    p = maker(2)
+    src, off, dests = _copy_conditions(p)
+    want = oracle.wants(p.n_npus, p.links, p.n_chunks, src, off, dests, p.chunk_bytes, p.seed)
+    wanted = set(zip(want["npu"].tolist(), want["chunk"].tolist()))
+    by_src = {}
+    for c, s_ in enumerate(src.tolist()):
+        by_src.setdefault(s_, []).append(c)
+    expect = np.array([sum((int(l["dst"]), c) in wanted for c in by_src.get(int(l["src"]), [])) for l in p.links], dtype=np.uint32)
+    topo = pk.Topology(p.n_npus, p.links)
+    prob = pk.Problem(topo, p.group, p.n_chunks, p.pre, p.post, p.chunk_bytes)
+    for fl in (0, pk.PCCL_FLAG_LSU_SWEEP):
+        ms, nbytes, tot = prob.candidate_sweep(0, p.seed, fl, iters=2)
+        assert np.array_equal(tot, expect), fl
+        assert ms > 0 and nbytes >= (len(p.links) + 1) * 128
+
+
 # ------------------------------------------------------------------------------ whole path
 SMALL = [wl.config1, wl.config2, wl.config3, wl.config4_small, wl.config5_small, wl.two_groups_mesh3x3]
 
@@ -358,19 +382,64 @@ def test_dynamic_relay_holder_rows_overflow(pk):
             assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY | fl), o)
 
 
-def test_dynamic_relay_config4_full_size_two_forms_agree(pk):
-    """Full size (58 M initial wants, 1.58 M transfers; the oracle needs 15 minutes here): the holder-list form and
-    the all-nodes scan must emit the same records, and the result must be a valid schedule."""
-    p = wl.config4(0)
-    topo = pk.Topology(p.n_npus, p.links)
-    prob = pk.Problem(topo, p.group, p.n_chunks, p.pre, p.post, p.chunk_bytes)
-    a = prob.synthesize(0, pk.PCCL_FLAG_DYNAMIC_RELAY)
-    b = prob.synthesize(0, pk.PCCL_FLAG_DYNAMIC_RELAY | pk.PCCL_FLAG_DENSE_SWEEP)
-    ta, tb = a.transfers, b.transfers
-    assert a.size == b.size == 1_579_300 and a.time_ps == b.time_ps == 273_214_495   # = the oracle's M and T (DESIGN.md)
-    for f in ta.dtype.names:
-        assert np.array_equal(ta[f], tb[f]), f
-    checker.check_structure(p, ta)
+def _golden(case):
+    """line of tests/golden/oracle_schedules.txt (written by tests/golden/make_golden.py from oracle/ only)"""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_schedules.txt")
+    for ln in open(path):
+        f = ln.split()
+        if f and f[0] == case:
+            return {"seed": int(f[1]), "transfers": int(f[2]), "time_ps": int(f[3]), "events": int(f[4]),
+                    "wants_total": int(f[5]), "sha256": f[6]}
+    return None
+
+
+def _assert_digest(s, g, name):
+    import hashlib
+    assert s.size == g["transfers"], f"{name}: {s.size} transfers vs oracle {g['transfers']}"
+    assert s.time_ps == g["time_ps"], f"{name}: T {s.time_ps} vs oracle {g['time_ps']}"
+    st = s.stats
+    assert st["events"] == g["events"] and st["wants_total"] == g["wants_total"], name
+    assert hashlib.sha256(s.transfers.tobytes()).hexdigest() == g["sha256"], f"{name}: records differ from the oracle's"
+
+
+FULL_SIZE = [("cfg4:thin", 0), ("cfg4:thin", "BARRIER_LOOP"), ("cfg4:dynamic", "DYNAMIC_RELAY"),
+             ("cfg4:dynamic", "DYNAMIC_RELAY|DENSE_SWEEP"), ("cfg4:bfs", "BFS"), ("cfg5:thin", 0),
+             ("cfg5:thin", "DENSE_SWEEP"), ("cfg5:dynamic", "DYNAMIC_RELAY"), ("cfg5:bfs", "BFS")]
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("case,mode", FULL_SIZE, ids=lambda x: str(x))
+def test_full_size_schedule_equals_the_oracles_digest(pk, case, mode):
+    """BASELINE.json configs 4 and 5 at full size under every relay mode: the CUDA schedule's records, T, event count and
+    initial wants against the digest of the ORACLE's run (the oracle needs 15 minutes for cfg4:dynamic, hours for
+    cfg5:dynamic, so its results are stored: tests/golden/oracle_schedules.txt, written by make_golden.py from oracle/
+    only).  The dynamic rule is checked in both of its forms (holder lists / all-nodes scan)."""
+    g = _golden(case)
+    if g is None:
+        pytest.skip(f"no oracle digest for {case} in tests/golden/oracle_schedules.txt (run tests/golden/make_golden.py {case})")
+    flags = pk.PCCL_FLAG_KEEP_ON_DEVICE
+    for name in (mode.split("|") if mode else []):
+        flags |= getattr(pk, "PCCL_FLAG_" + name)
+    p = {"cfg4": wl.config4, "cfg5": wl.config5}[case.split(":")[0]](g["seed"])
+    s = gpu_run(pk, p, flags)
+    _assert_digest(s, g, f"{case} {mode}")
+    checker.check_structure(p, s.transfers)
+
+
+def test_dynamic_relay_record_buffer_rerun(pk):
+    """The dynamic rule's record buffer is sized from the static relay tree's transfer count; when it is short the run
+    still finishes (records past the end are dropped, the count goes on) and the phase is rerun with the exact count.
+    Forced here with a 100-record buffer on copy, reduce and all-reduce problems."""
+    cases = [wl.config4_small(1), wl.config3(0), wl.config2(2)]
+    pk.set_option(pk.PCCL_OPT_DYNAMIC_RECORDS, 100)
+    try:
+        for p in cases:
+            o = oracle.synthesize(*p.args(), relay=oracle.RELAY_DYNAMIC)
+            assert len(o.transfers) > 100
+            assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_DYNAMIC_RELAY), o)
+    finally:
+        pk.set_option(pk.PCCL_OPT_DYNAMIC_RECORDS, 0)
 
 
 def test_dynamic_relay_unreachable(pk):
