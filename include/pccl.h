@@ -135,6 +135,15 @@ uint64_t pccl_launch_count(void);
  * ------------------------------------------------------------------------------------- */
 int pccl_topology_create(uint32_t n_npus, const pccl_link_t* links, uint32_t n_links,
                          pccl_topology_t** out);
+/* Switch model of PAPER.md:348 (section 4.7), per node; used by PCCL_FLAG_BFS (the other modes return UNSUPPORTED
+ * while a model is set).  buffer_limit: host, n_npus u32, chunks the node may buffer at once (0xFFFFFFFF: no limit) --
+ * a chunk is buffered at a node it is forwarded from, from its arrival until the end of the last transfer that forwards
+ * it, and a visit of the node at time t is skipped while the conditions routed before hold that many chunks there at t
+ * (Q23, Q24).  no_multicast: host, n_npus bytes, non-zero: the node forwards over its out-links one transfer
+ * at a time, in ascending link id (Q25).  Either may be NULL; both NULL (or all unlimited / zero) removes the model.
+ * With a model the conditions are routed strictly one after another (a one-condition window).
+ * Errors: INVALID, NOMEM. */
+int pccl_topology_set_switch_model(pccl_topology_t* topo, const uint32_t* buffer_limit, const uint8_t* no_multicast);
 void pccl_topology_destroy(pccl_topology_t* topo);
 uint32_t pccl_topology_n_npus(const pccl_topology_t* topo);
 uint32_t pccl_topology_n_links(const pccl_topology_t* topo);

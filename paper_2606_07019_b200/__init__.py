@@ -67,6 +67,7 @@ SIGNATURES = {
     "pccl_get_option": (_u64, [_int]),
     "pccl_launch_count": (_u64, []),
     "pccl_topology_create": (_int, [_u32, _vp, _u32, C.POINTER(_vp)]),
+    "pccl_topology_set_switch_model": (_int, [_vp, _vp, _vp]),
     "pccl_topology_destroy": (None, [_vp]),
     "pccl_topology_n_npus": (_u32, [_vp]),
     "pccl_topology_n_links": (_u32, [_vp]),
@@ -189,6 +190,13 @@ class Topology:
         _check(lib.pccl_topology_create(n_npus, _ptr(self._links), len(self._links), C.byref(h)))
         self.handle = h
         self.n_npus, self.n_links = int(n_npus), len(self._links)
+
+    def set_switch_model(self, buffer_limit=None, no_multicast=None) -> None:
+        """per-node buffer limits (0xFFFFFFFF = none) and no-multicast flags for PCCL_FLAG_BFS."""
+        bl = None if buffer_limit is None else np.ascontiguousarray(buffer_limit, dtype=np.uint32)
+        nm = None if no_multicast is None else np.ascontiguousarray(no_multicast, dtype=np.uint8)
+        assert (bl is None or len(bl) == self.n_npus) and (nm is None or len(nm) == self.n_npus)
+        _check(lib.pccl_topology_set_switch_model(self.handle, None if bl is None else _ptr(bl), None if nm is None else _ptr(nm)))
 
     def link_costs(self, chunk_bytes: int) -> np.ndarray:
         out = np.zeros(self.n_links, dtype=np.uint64)

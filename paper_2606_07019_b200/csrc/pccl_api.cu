@@ -261,6 +261,9 @@ struct pccl_topology {
     std::vector<pccl_link_t> links;
     std::vector<uint32_t> in_off, in_link, out_off, out_link;   // ascending link id per node
     uint32_t max_in = 0, max_out = 0;                           // largest in- / out-degree
+    // switch model of PAPER.md:348 (pccl_topology_set_switch_model); empty: none
+    std::vector<uint32_t> buf_limit;
+    std::vector<unsigned char> no_mcast;
     // device copy (one blob)
     void* blob = nullptr;
     uint32_t *d_src = nullptr, *d_dst = nullptr, *d_in_off = nullptr, *d_in_link = nullptr,
@@ -387,6 +390,29 @@ extern "C" int pccl_topology_create(uint32_t n_npus, const pccl_link_t* links, u
         return PCCL_ERR_NOMEM;
     }
     *out = t;
+    return PCCL_OK;
+}
+
+extern "C" int pccl_topology_set_switch_model(pccl_topology_t* t, const uint32_t* buffer_limit, const uint8_t* no_multicast) {
+    SERIALISE;
+    if (!t) return PCCL_ERR_INVALID;
+    try {
+        std::vector<uint32_t> bl;
+        std::vector<unsigned char> nm;
+        bool any = false;
+        if (buffer_limit) for (uint32_t v = 0; v < t->N; ++v) any |= buffer_limit[v] != 0xFFFFFFFFu;
+        if (no_multicast) for (uint32_t v = 0; v < t->N; ++v) any |= no_multicast[v] != 0;
+        if (any) {
+            bl.assign(t->N, 0xFFFFFFFFu);
+            nm.assign(t->N, 0);
+            if (buffer_limit) bl.assign(buffer_limit, buffer_limit + t->N);
+            if (no_multicast) nm.assign(no_multicast, no_multicast + t->N);
+        }
+        t->buf_limit.swap(bl);
+        t->no_mcast.swap(nm);
+    } catch (const std::bad_alloc&) {
+        return PCCL_ERR_NOMEM;
+    }
     return PCCL_OK;
 }
 
@@ -1451,13 +1477,29 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     if (nact == 0) return PCCL_OK;
 
     // ---- window size = co-resident CTAs ----
-    if (smem > 40 * 1024) CU(cudaFuncSetAttribute(k_bfs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const void* kbfs = !t->buf_limit.empty() ? (const void*)k_bfs<true> : (const void*)k_bfs<false>;
+    if (smem > 40 * 1024) CU(cudaFuncSetAttribute(kbfs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bfs, (int)BFS_THREADS, smem));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kbfs, (int)BFS_THREADS, smem));
     if (occ < 1) return PCCL_ERR_CUDA;
+    // switch model: per limited node a sorted table of the stays committed so far; conditions are then
+    // routed strictly one after another (a one-condition window), so a search sees every earlier stay
+    const bool sw_model = !t->buf_limit.empty();
+    std::vector<uint32_t> h_swidx;
+    uint32_t n_lim = 0;
+    if (sw_model) {
+        try {
+            h_swidx.assign(N, NONE32);
+        } catch (const std::bad_alloc&) {
+            return PCCL_ERR_NOMEM;
+        }
+        for (uint32_t v = 0; v < N; ++v)
+            if (t->buf_limit[v] != 0xFFFFFFFFu) h_swidx[v] = n_lim++;
+        if ((uint64_t)std::max(n_lim, 1u) * nact * 16 > ((uint64_t)1 << 30)) return PCCL_ERR_UNSUPPORTED;
+    }
     uint32_t Bwant = (uint32_t)G.sm_count;   // one 1024-thread CTA per SM
     if (const uint64_t o = G.opt_bfs_window) Bwant = (uint32_t)std::min<uint64_t>((uint64_t)occ * (uint64_t)G.sm_count, o);
-    const uint32_t B = std::max(1u, std::min(Bwant, nact));
+    const uint32_t B = sw_model ? 1u : std::max(1u, std::min(Bwant, nact));
 
     // ---- record capacity: a tree has at most N - 1 transfers; retried with the exact count if short ----
     uint64_t cap = 0;
@@ -1474,6 +1516,11 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         Carver w2;
         const size_t o_runs = w2.take((size_t)L * R * 16), o_rn = w2.take((size_t)L * 4), o_rs = w2.take((size_t)L * B * 8),
                      o_rp = w2.take((size_t)L * B * 4), o_tl = w2.take((size_t)B * N * 4), o_ts = w2.take((size_t)B * N * 8);
+        const size_t nl1 = std::max(n_lim, 1u);
+        const size_t o_swi = w2.take(sw_model ? (size_t)N * 4 : 0), o_swl = w2.take(sw_model ? (size_t)N * 4 : 0),
+                     o_swm = w2.take(sw_model ? (size_t)N : 0), o_sba = w2.take(sw_model ? nl1 * nact * 8 : 0),
+                     o_sbr = w2.take(sw_model ? nl1 * nact * 8 : 0), o_sbn = w2.take(sw_model ? nl1 * 4 : 0),
+                     o_sta = w2.take(sw_model ? nl1 * B * 8 : 0), o_str = w2.take(sw_model ? nl1 * B * 8 : 0);
         void* ws = nullptr;
         rc = dev_alloc(w2.cur, &ws);
         if (rc) return rc;
@@ -1497,10 +1544,21 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         a.runs = (ulonglong2*)(q + o_runs); a.rl_n = (uint32_t*)(q + o_rn); a.rl_start = (uint64_t*)(q + o_rs);
         a.rl_pos = (uint32_t*)(q + o_rp); a.tr_link = (uint32_t*)(q + o_tl); a.tr_start = (uint64_t*)(q + o_ts);
         a.out = raw; a.out_cap = cap; a.t_offset = 0; a.ctrl = ctrl;
+        a.swidx = nullptr; a.buf_limit = nullptr; a.no_mcast = nullptr; a.n_lim = 0; a.sb_cap = 0;
+        a.sb_arr = a.sb_rel = a.st_arr = a.st_rel = nullptr; a.sb_n = nullptr;
+        if (sw_model) {
+            a.swidx = (uint32_t*)(q + o_swi); a.buf_limit = (uint32_t*)(q + o_swl); a.no_mcast = (unsigned char*)(q + o_swm);
+            a.n_lim = n_lim; a.sb_cap = nact;
+            a.sb_arr = (unsigned long long*)(q + o_sba); a.sb_rel = (unsigned long long*)(q + o_sbr); a.sb_n = (uint32_t*)(q + o_sbn);
+            a.st_arr = (unsigned long long*)(q + o_sta); a.st_rel = (unsigned long long*)(q + o_str);
+            CU(cudaMemcpyAsync(q + o_swi, h_swidx.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st));
+            CU(cudaMemcpyAsync(q + o_swl, t->buf_limit.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st));
+            CU(cudaMemcpyAsync(q + o_swm, t->no_mcast.data(), (size_t)N, cudaMemcpyHostToDevice, st));
+        }
         t_loop.start();
-        k_bfs_init<<<(std::max(L, 1u) + 255) / 256, 256, 0, counted(st)>>>(a);
+        k_bfs_init<<<(std::max(std::max(L, n_lim), 1u) + 255) / 256, 256, 0, counted(st)>>>(a);
         void* args[] = {(void*)&a};
-        CU(cudaLaunchCooperativeKernel((const void*)k_bfs, dim3(B), dim3(BFS_THREADS), args, smem, counted(st)));
+        CU(cudaLaunchCooperativeKernel(kbfs, dim3(B), dim3(BFS_THREADS), args, smem, counted(st)));
         CU(cudaMemcpyAsync(mb, ctrl, sizeof(BfsCtrl), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
         t_loop.stop();
@@ -1610,6 +1668,7 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
             }
             continue;
         }
+        if (!P->topo->buf_limit.empty()) return fail(PCCL_ERR_UNSUPPORTED);   // the switch model belongs to PCCL_FLAG_BFS
         if (!W.blob) { rc = work_alloc(*P, W); if (rc) return fail(rc); }
         uint64_t M = 0;
         t_setup.start();

@@ -68,6 +68,17 @@ struct BfsArgs {
     Rec* out;
     uint64_t out_cap, t_offset;
     BfsCtrl* ctrl;
+    // switch model of section 4.7 (Q23-Q25); swidx == nullptr: none.  With a switch model the
+    // window is one condition wide (B == 1): conditions are routed strictly one after another
+    const uint32_t* swidx;            // [N] row of a node with a buffer limit in the stay tables, NONE32 otherwise
+    const uint32_t* buf_limit;        // [N] chunks the node buffers at once (NONE32: no limit)
+    const unsigned char* no_mcast;    // [N] non-zero: the node forwards one transfer at a time
+    uint32_t n_lim, sb_cap;           // limited nodes; stays a row holds
+    unsigned long long* sb_arr;       // [n_lim][sb_cap] arrival times of the stays committed so far, ascending
+    unsigned long long* sb_rel;       // [n_lim][sb_cap] their release times, ascending
+    uint32_t* sb_n;                   // [n_lim]
+    unsigned long long* st_arr;       // [B][n_lim] stay of the slot's current result at each limited node ...
+    unsigned long long* st_rel;       // [B][n_lim] ... release 0: the node does not forward the chunk
 };
 
 constexpr uint32_t BFS_THREADS = 1024;
@@ -125,6 +136,7 @@ __global__ void k_bfs_init(BfsArgs a) {
         a.runs[(size_t)i * a.R] = make_ulonglong2(0ull, 0ull);
         a.rl_n[i] = 0;
     }
+    if (a.swidx != nullptr && i < a.n_lim) a.sb_n[i] = 0;
     if (i == 0) {
         a.ctrl->first_bad[0] = BFS_INF; a.ctrl->first_bad[1] = BFS_INF;
         a.ctrl->nrec = 0; a.ctrl->tmax = 0; a.ctrl->searches = 0; a.ctrl->relax = 0; a.ctrl->rounds = 0;
@@ -160,6 +172,33 @@ __device__ __forceinline__ uint64_t bfs_depart(const ulonglong2* __restrict__ ro
         r = __ldcg(row + lo);
     }
     return (a + w <= r.x) ? a : r.y;
+}
+
+// ---- section 4.7: chunks buffered at a limited node at time t = stays with arrival <= t < release -----------------
+__device__ __forceinline__ uint32_t sb_upper(const unsigned long long* a, uint32_t n, unsigned long long t) {
+    uint32_t lo = 0, hi = n;                            // first index with a[i] > t
+    while (lo < hi) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (__ldcg(a + mid) <= t) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+// earliest start s >= a of link `row` (cost w) whose arrival s + w finds fewer than `limit` chunks buffered at the far
+// node (stay tables arr / rel of n entries): first fit on the link, then wait for a release, and again
+__device__ __forceinline__ uint64_t bfs_depart_buffered(const ulonglong2* __restrict__ row, uint64_t a, uint64_t w,
+                                                        const unsigned long long* arr, const unsigned long long* rel, uint32_t n,
+                                                        uint32_t limit) {
+    for (;;) {
+        const uint64_t s = bfs_depart(row, __ldcg(row), a, w);
+        unsigned long long t = s + w;
+        if (sb_upper(arr, n, t) - sb_upper(rel, n, t) < limit) return s;
+        for (;;) {                                      // next time with a free buffer: walk the releases after t
+            const uint32_t r = sb_upper(rel, n, t);
+            t = __ldcg(rel + r);                        // (occupancy > 0: a release after t exists)
+            if (sb_upper(arr, n, t) - sb_upper(rel, n, t) < limit) break;
+        }
+        a = t - w;
+    }
 }
 
 // ---- Alg. 3 line 13: take [s, s + w) on a link (single writer per link) ----------------------
@@ -201,6 +240,7 @@ struct BfsShared {
     unsigned long long tmax;
 };
 
+template <bool SW>   // SW: the switch model of section 4.7 is compiled in
 __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long* key, uint32_t* stamp, uint32_t* fr0, uint32_t* fr1,
                            const uint32_t* s_off, const uint4* s_os, ulonglong2* s_hdr,
                            BfsShared& sh, uint32_t slot, uint32_t& ntr, uint64_t& relax) {
@@ -258,14 +298,31 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
             const uint32_t o0 = s_off[u], deg = s_off[u + 1] - o0;
             const unsigned long long au = ((volatile unsigned long long*)key)[u] >> lb;
             if (au > bound) continue;
-            for (uint32_t k = tid & ((1u << mds) - 1); k < deg; k += 1u << mds) {
+            // a node without multicast forwards over its out-links one after the other, in ascending link id (4.7): one
+            // lane walks them, each transfer starting no earlier than the end of the one before
+            const bool serial = SW && a.no_mcast[u] != 0;
+            const uint32_t kstep = serial ? 1u : (1u << mds);
+            uint64_t from = au;
+            if (serial && (tid & ((1u << mds) - 1)) != 0) continue;
+            for (uint32_t k = serial ? 0u : (tid & ((1u << mds) - 1)); k < deg; k += kstep) {
                 const uint4 os = s_os ? s_os[o0 + k] : a.oslot[o0 + k];
                 const uint32_t l = os.x, v = os.y;
-                if (v == src) continue;
+                if (v == src && !serial) continue;
                 const uint64_t wl = ((uint64_t)os.w << 32) | os.z;
                 const ulonglong2* row = a.runs + (size_t)l * a.R;
-                const uint64_t cand = bfs_depart(row, s_hdr ? s_hdr[l] : __ldcg(row), au, wl) + wl;
+                uint64_t cand;
+                const uint32_t sr = SW ? a.swidx[v] : NONE32;
+                if (sr != NONE32) {
+                    const uint32_t lim = a.buf_limit[v];
+                    if (lim == 0) continue;                        // a node that buffers nothing is never visited
+                    cand = bfs_depart_buffered(row, from, wl, a.sb_arr + (size_t)sr * a.sb_cap, a.sb_rel + (size_t)sr * a.sb_cap,
+                                               ldcg32(a.sb_n + sr), lim) + wl;
+                } else {
+                    cand = bfs_depart(row, s_hdr ? s_hdr[l] : __ldcg(row), from, wl) + wl;
+                }
+                if (serial) from = cand;
                 ++relax;
+                if (v == src) continue;
                 if (cand >> (64 - lb)) { atomicOr(&a.ctrl->err, 2u); continue; }
                 const unsigned long long kc = (cand << lb) | l;
                 if (kc >= ((volatile unsigned long long*)key)[v]) continue;
@@ -302,12 +359,23 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
     __syncthreads();
     uint32_t* tl = a.tr_link + (size_t)slot * a.N;
     uint64_t* ts = a.tr_start + (size_t)slot * a.N;
+    if (SW)                                             // (section 4.7) the stays of this result, per limited node
+        for (uint32_t r = tid; r < a.n_lim; r += BFS_THREADS) a.st_rel[(size_t)slot * a.n_lim + r] = 0ull;
+    __syncthreads();
     for (uint32_t v = tid; v < a.N; v += BFS_THREADS) {
         if (!keep[v]) continue;
         const uint32_t i = atomicAdd(&sh.cnt, 1u);
         const uint32_t l = (uint32_t)(key[v] & lmask);
         tl[i] = l;
         ts[i] = (key[v] >> lb) - a.w[l];
+        if (SW) {                                       // the chunk stays buffered at the sender until this transfer ends
+            const uint32_t u = a.esrc[l];
+            const uint32_t sr = u != src ? a.swidx[u] : NONE32;
+            if (sr != NONE32) {
+                a.st_arr[(size_t)slot * a.n_lim + sr] = key[u] >> lb;
+                atomicMax(&a.st_rel[(size_t)slot * a.n_lim + sr], key[v] >> lb);
+            }
+        }
     }
     __syncthreads();
     ntr = sh.cnt;
@@ -316,6 +384,7 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
 #endif
 }
 
+template <bool SW>
 __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
     cg::grid_group grid = cg::this_grid();
     extern __shared__ unsigned long long bfs_smem[];
@@ -348,7 +417,7 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
         const uint32_t p = (uint32_t)p64;
         if (active) {
             if (!(valid && pos == p)) {
-                bfs_search(a, a.order[p], key, stamp, fr0, fr1, s_off, s_os, s_hdr, sh, slot, ntr, relax);
+                bfs_search<SW>(a, a.order[p], key, stamp, fr0, fr1, s_off, s_os, s_hdr, sh, slot, ntr, relax);
                 pos = p; valid = true; ++searches;
             }
             for (uint32_t i = tid; i < ntr; i += BFS_THREADS) {
@@ -417,6 +486,26 @@ __global__ void __launch_bounds__(BFS_THREADS) k_bfs(BfsArgs a) {
             if (tm) atomicMax(&sh.tmax, tm);
             __syncthreads();
             if (tid == 0 && sh.tmax) atomicMax(&a.ctrl->tmax, sh.tmax);
+            if (SW) {
+                // (section 4.7; one condition commits per round) its stays join the limited nodes' sorted tables
+                __threadfence();
+                for (uint32_t r = tid; r < a.n_lim; r += BFS_THREADS) {
+                    const unsigned long long rel = __ldcg(a.st_rel + (size_t)slot * a.n_lim + r);
+                    if (rel == 0ull) continue;
+                    const unsigned long long arv = __ldcg(a.st_arr + (size_t)slot * a.n_lim + r);
+                    const uint32_t n = a.sb_n[r];
+                    if (n >= a.sb_cap) { atomicOr(&a.ctrl->err, 16u); continue; }
+                    unsigned long long* A = a.sb_arr + (size_t)r * a.sb_cap;
+                    unsigned long long* R = a.sb_rel + (size_t)r * a.sb_cap;
+                    uint32_t i = n;
+                    while (i > 0 && A[i - 1] > arv) { A[i] = A[i - 1]; --i; }
+                    A[i] = arv;
+                    i = n;
+                    while (i > 0 && R[i - 1] > rel) { R[i] = R[i - 1]; --i; }
+                    R[i] = rel;
+                    a.sb_n[r] = n + 1;
+                }
+            }
             valid = false;
         } else if (active) {
             valid = sh.minconf == NONE32 || sh.minconf >= fb;

@@ -716,3 +716,88 @@ def test_randomized_problems_all_modes(pk, block):
                 assert_same(p, gpu_run(pk, p, pk.PCCL_FLAG_BARRIER_LOOP), o)
             if relay == 0:
                 checker.check_schedule(p, o.transfers)
+
+
+# ------------------------------------------------------------------------------ switch model (NEXT-3)
+def _bfs_with_switches(pk, p, bl, nm):
+    topo = pk.Topology(p.n_npus, p.links)
+    topo.set_switch_model(bl, nm)
+    prob = pk.Problem(topo, p.group, p.n_chunks, p.pre, p.post, p.chunk_bytes)
+    return prob.synthesize(p.seed, pk.PCCL_FLAG_BFS)
+
+
+def _random_switch_problem(i):
+    """a random heterogeneous multigraph problem (copy / reduce / all-reduce) with buffer limits of 1..3 chunks on a few
+    nodes and some nodes without multicast"""
+    p = _random_problem(300 + i)
+    rng = np.random.default_rng(4200 + i)
+    n = p.n_npus
+    bl = np.full(n, oracle.NO_LIMIT, dtype=np.uint32)
+    nm = np.zeros(n, dtype=np.uint8)
+    members = set(int(x) for x in p.group)
+    others = [v for v in range(n) if v not in members] or list(range(n))
+    for v in rng.choice(others, size=min(len(others), int(rng.integers(1, 5))), replace=False):
+        bl[int(v)] = int(rng.integers(1, 4))
+    if i % 3:
+        for v in rng.choice(n, size=int(rng.integers(1, 4)), replace=False):
+            nm[int(v)] = 1
+    if i % 5 == 4:
+        bl[:] = oracle.NO_LIMIT            # no multicast only
+    return p, bl, nm
+
+
+@pytest.mark.parametrize("block", range(3))
+def test_switch_model_random_problems(pk, block):
+    """PCCL_FLAG_BFS with per-node buffer limits and no-multicast nodes against the oracle's switch model, 30 problems"""
+    for i in range(block * 10, block * 10 + 10):
+        p, bl, nm = _random_switch_problem(i)
+        try:
+            o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS, buffer_limit=bl, no_multicast=nm)
+        except oracle.OracleError as e:
+            with pytest.raises(pk.PcclError) as g:
+                _bfs_with_switches(pk, p, bl, nm)
+            assert g.value.code == {oracle.ERR_UNREACHABLE: pk.PCCL_ERR_UNREACHABLE, oracle.ERR_UNSUPPORTED: pk.PCCL_ERR_UNSUPPORTED,
+                                    oracle.ERR_INVALID: pk.PCCL_ERR_INVALID}[e.code], p.name
+            continue
+        assert_same(p, _bfs_with_switches(pk, p, bl, nm), o)
+
+
+@pytest.mark.parametrize("limit,unicast", [(2, True), (1, False), (oracle.NO_LIMIT, True)])
+def test_switch_model_config3(pk, limit, unicast):
+    """config 3's eight pod switches with finite buffers and / or without multicast (Reduce-Scatter, both directions of
+    the model through the transposed phase)"""
+    p = wl.config3(0)
+    bl = np.full(p.n_npus, oracle.NO_LIMIT, dtype=np.uint32)
+    bl[64:] = limit
+    nm = np.zeros(p.n_npus, dtype=np.uint8)
+    nm[64:] = 1 if unicast else 0
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS, buffer_limit=bl, no_multicast=nm)
+    s = _bfs_with_switches(pk, p, bl, nm)
+    assert_same(p, s, o)
+    checker.check_schedule(p, s.transfers)
+
+
+def test_switch_model_hand_examples_and_modes(pk):
+    links = np.array([(0, 2, 0, 1), (1, 2, 0, 1), (2, 3, 0, 1), (2, 4, 0, 1)], dtype=wl.LINK_DT)
+    pre = np.array([(0, 0), (1, 1)], dtype=wl.PAIR_DT)
+    post = np.array([(3, 0), (4, 1)], dtype=wl.PAIR_DT)
+    p = wl.Problem("two_through_one_switch", 5, links, np.array([0, 1, 3, 4], dtype=np.uint32), 2, pre, post, 1, 0)
+    bl = np.array([oracle.NO_LIMIT] * 5, dtype=np.uint32)
+    bl[2] = 1
+    s = _bfs_with_switches(pk, p, bl, None)
+    assert s.time_ps == 3                                        # tests/test_oracle_bfs.py: test_buffer_limit_hand_example
+    assert_same(p, s, oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS, buffer_limit=bl))
+    bl[2] = 0
+    with pytest.raises(pk.PcclError) as e:
+        _bfs_with_switches(pk, p, bl, None)
+    assert e.value.code == pk.PCCL_ERR_UNREACHABLE
+    # the matching loops do not model switches: refused while a model is set, fine again once it is removed
+    topo = pk.Topology(p.n_npus, p.links)
+    bl[2] = 1
+    topo.set_switch_model(bl, None)
+    prob = pk.Problem(topo, p.group, p.n_chunks, p.pre, p.post, p.chunk_bytes)
+    with pytest.raises(pk.PcclError) as e:
+        prob.synthesize(0, 0)
+    assert e.value.code == pk.PCCL_ERR_UNSUPPORTED
+    topo.set_switch_model(None, None)
+    assert prob.synthesize(0, 0).time_ps == 2
