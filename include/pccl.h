@@ -232,6 +232,13 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
                                         pccl_device_candidate_sweep) loads its rows with per-lane 128-bit loads instead of
                                         staging them in shared memory by bulk asynchronous copies (TMA) */
 
+#define PCCL_FLAG_PIPELINE 8192u     /* with PCCL_FLAG_BFS, on an All-Reduce problem: the copy phase of a chunk starts as soon
+                                        as its root holds the complete sum (the end of the last transfer of the chunk into
+                                        the root) instead of after the whole reduce phase; it is routed against the link
+                                        intervals the reduce phase took (Q26; PAPER.md:330 composes the phases).
+                                        Other collectives: no effect.  UNSUPPORTED without PCCL_FLAG_BFS or with a switch
+                                        model.  time_phase1_ps = end of the reduce phase, schedule time = the later end */
+
 /* Steps A..F on the GPU for one seed.  Errors: UNREACHABLE, CUDA, NOMEM, INTERNAL. */
 int pccl_problem_synthesize(pccl_problem_t* problem, uint64_t seed, uint32_t flags,
                             pccl_schedule_t** out);

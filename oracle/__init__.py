@@ -67,6 +67,8 @@ def lib():
         L.oracle_synthesize_switches.argtypes = [u32, vp, u32, vp, u32, u32, vp, u64, vp, u64, u64, u64, vp, vp,
                                                  C.POINTER(vp)]
         L.oracle_synthesize_switches.restype = C.c_int
+        L.oracle_synthesize_pipelined.argtypes = [u32, vp, u32, vp, u32, u32, vp, u64, vp, u64, u64, u64, C.POINTER(vp)]
+        L.oracle_synthesize_pipelined.restype = C.c_int
         L.oracle_wants.argtypes = [u32, vp, u32, u32, vp, vp, vp, u64, u64, vp, u64]
         L.oracle_wants.restype = i64
         for name in ("oracle_size", "oracle_time", "oracle_events", "oracle_wants_total",
@@ -128,18 +130,25 @@ NO_LIMIT = 0xFFFFFFFF
 
 
 def synthesize(n_npus, links, group, n_chunks, pre, post, chunk_bytes, seed, relay: int = RELAY_THIN,
-               buffer_limit=None, no_multicast=None) -> OracleSchedule:
+               buffer_limit=None, no_multicast=None, pipeline: bool = False) -> OracleSchedule:
     """Same problem statement as the product boundary (include/pccl.h), host arrays only.
     relay: RELAY_THIN (static thin relay tree, the default), RELAY_DYNAMIC (Q18) or RELAY_BFS (the paper's
     own per-condition search, Alg. 1-3, Q19-Q22; `events` then counts conditions routed).
-    buffer_limit / no_multicast (RELAY_BFS only): the switch model of PAPER.md:348, per node (Q23-Q25)."""
+    buffer_limit / no_multicast (RELAY_BFS only): the switch model of PAPER.md:348, per node (Q23-Q25).
+    pipeline (RELAY_BFS only): an All-Reduce's copy phase of a chunk starts when its root is complete (Q26)."""
     links = np.ascontiguousarray(links, dtype=LINK_DT)
     group = np.ascontiguousarray(group, dtype=np.uint32)
     pre = np.ascontiguousarray(pre, dtype=PAIR_DT)
     post = np.ascontiguousarray(post, dtype=PAIR_DT)
     h = C.c_void_p()
     t0 = time.perf_counter()
-    if buffer_limit is not None or no_multicast is not None:
+    if pipeline:
+        if relay != RELAY_BFS or buffer_limit is not None or no_multicast is not None:
+            raise ValueError("pipelined All-Reduce: RELAY_BFS without a switch model")
+        rc = lib().oracle_synthesize_pipelined(n_npus, _ptr(links), len(links), _ptr(group), len(group),
+                                               n_chunks, _ptr(pre), len(pre), _ptr(post), len(post), chunk_bytes, seed,
+                                               C.byref(h))
+    elif buffer_limit is not None or no_multicast is not None:
         if relay != RELAY_BFS:
             raise ValueError("the switch model applies to RELAY_BFS only")
         bl = None if buffer_limit is None else np.ascontiguousarray(buffer_limit, dtype=np.uint32)

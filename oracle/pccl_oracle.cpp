@@ -481,7 +481,10 @@ uint64_t earliest_start_buffered(const BusyLink& b, uint64_t a, uint64_t w, cons
 
 int synth_copy_bfs(uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& conds,
                    uint64_t chunk_bytes, uint64_t seed, CopyResult& res,
-                   const uint32_t* buf_limit = nullptr, const uint8_t* no_mcast = nullptr) {
+                   const uint32_t* buf_limit = nullptr, const uint8_t* no_mcast = nullptr,
+                   const std::vector<BusyLink>* busy0 = nullptr, const std::vector<uint64_t>* ready = nullptr) {
+    // busy0 / ready (pipelined All-Reduce, Q26): intervals already taken on every link when the first condition
+    // is routed, and the time from which each chunk is available at its source
     const uint32_t L = (uint32_t)links.size();
     const uint32_t C = (uint32_t)conds.size();
     std::vector<uint64_t> w(L);
@@ -511,6 +514,7 @@ int synth_copy_bfs(uint32_t n, const std::vector<Link>& links, const std::vector
     });
 
     std::vector<BusyLink> busy(L);
+    if (busy0) busy = *busy0;
     std::vector<SwitchBuf> sbuf(buf_limit ? n : 0);
     auto limited = [&](uint32_t v) { return buf_limit && buf_limit[v] != NONE; };
     res = CopyResult{};
@@ -525,8 +529,9 @@ int synth_copy_bfs(uint32_t n, const std::vector<Link>& links, const std::vector
         std::fill(done.begin(), done.end(), 0);
         using QE = std::pair<uint64_t, uint32_t>;
         std::priority_queue<QE, std::vector<QE>, std::greater<QE>> pq;
-        arr[c.src] = 0;
-        pq.push({0, c.src});
+        const uint64_t t0 = ready ? (*ready)[k.chunk] : 0;
+        arr[c.src] = t0;
+        pq.push({t0, c.src});
         size_t left = c.dests.size();
         uint64_t last = 0;                                    // arrival at the last dest reached
         while (!pq.empty()) {
@@ -631,7 +636,7 @@ struct Result {
 int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uint32_t* group,
                uint32_t n_members, uint32_t n_chunks, const Pair* pre_p, uint64_t n_pre,
                const Pair* post_p, uint64_t n_post, uint64_t chunk_bytes, uint64_t seed,
-               Result& out, int relay = 0, SwitchModel sw = SwitchModel()) {
+               Result& out, int relay = 0, SwitchModel sw = SwitchModel(), bool pipeline = false) {
     if (n_links && !links_p) return OR_ERR_INVALID;
     if (n_members && !group) return OR_ERR_INVALID;
     if ((n_pre && !pre_p) || (n_post && !post_p)) return OR_ERR_INVALID;
@@ -710,6 +715,33 @@ int synthesize(uint32_t n_npus, const Link* links_p, uint32_t n_links, const uin
         CopyResult r1, r2;
         int rc = synth_reduce(n_npus, links, bc, chunk_bytes, seed, r1, relay, sw);
         if (rc != OR_OK) return rc;
+        if (pipeline) {
+            // Pipelined All-Reduce (PAPER.md:330 composes the phases, reading Q26 lets them overlap): the
+            // copy phase of chunk c may start as soon as root(c) holds the complete sum -- the end of the last transfer of
+            // c into the root -- instead of at the end of the whole reduce phase.  Both phases share the links, so the
+            // copy phase is routed by the per-condition search (BFS mode only) against the intervals the reduce phase took.
+            if (relay != 2 || sw.buf_limit || sw.no_mcast) return OR_ERR_UNSUPPORTED;
+            std::vector<BusyLink> busy(links.size());
+            std::vector<uint64_t> ready(n_chunks, 0);
+            for (const Rec& r : r1.recs) {
+                occupy(busy[r.link], r.t_start_ps, r.t_end_ps);
+                if (r.dst == cp[r.chunk].src) ready[r.chunk] = std::max(ready[r.chunk], r.t_end_ps);
+            }
+            rc = synth_copy_bfs(n_npus, links, cp, chunk_bytes, seed, r2, nullptr, nullptr, &busy, &ready);
+            if (rc != OR_OK) return rc;
+            out.recs = std::move(r1.recs);
+            out.recs.insert(out.recs.end(), r2.recs.begin(), r2.recs.end());
+            std::sort(out.recs.begin(), out.recs.end(), [](const Rec& a, const Rec& b) {
+                if (a.t_start_ps != b.t_start_ps) return a.t_start_ps < b.t_start_ps;
+                return a.link < b.link;
+            });
+            out.T_phase1 = r1.T;
+            out.T = std::max(r1.T, r2.T);
+            out.events = r1.events + r2.events;
+            out.wants_total = r1.wants_total + r2.wants_total;
+            out.mode = 2;
+            return OR_OK;
+        }
         rc = synth_copy_mode(relay, n_npus, links, cp, chunk_bytes, seed, r2, sw);
         if (rc != OR_OK) return rc;
         out.recs = std::move(r1.recs);
@@ -804,6 +836,21 @@ int oracle_synthesize_switches(uint32_t n_npus, const oracle_link* links, uint32
     const int rc = synthesize(n_npus, (const Link*)links, n_links, group, n_members, n_chunks,
                               (const Pair*)pre, n_pre, (const Pair*)post, n_post, chunk_bytes,
                               seed, *r, 2, sw);
+    if (rc != OR_OK) { delete r; return rc; }
+    *handle = r;
+    return OR_OK;
+}
+
+// BFS mode, All-Reduce with overlapping phases (reading Q26); anything but an all-reduce problem is synthesized as usual
+int oracle_synthesize_pipelined(uint32_t n_npus, const oracle_link* links, uint32_t n_links,
+                                const uint32_t* group, uint32_t n_members, uint32_t n_chunks,
+                                const oracle_pair* pre, uint64_t n_pre, const oracle_pair* post,
+                                uint64_t n_post, uint64_t chunk_bytes, uint64_t seed, void** handle) {
+    if (!handle) return OR_ERR_INVALID;
+    Result* r = new Result();
+    const int rc = synthesize(n_npus, (const Link*)links, n_links, group, n_members, n_chunks,
+                              (const Pair*)pre, n_pre, (const Pair*)post, n_post, chunk_bytes,
+                              seed, *r, 2, SwitchModel(), true);
     if (rc != OR_OK) { delete r; return rc; }
     *handle = r;
     return OR_OK;

@@ -1409,8 +1409,10 @@ struct BfsResult {
     uint32_t grid;
 };
 
+// pre / n_pre / t_pre (pipelined All-Reduce, Q26): the reduce phase's records in forward time (device) and their
+// largest t_end -- they pre-occupy the links, and a chunk's search starts when its root has received the last of them
 int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_shift, Rec** out_recs, BfsResult* res,
-              Timer& t_setup, Timer& t_loop, Timer& t_emit) {
+              Timer& t_setup, Timer& t_loop, Timer& t_emit, const Rec* pre = nullptr, uint64_t n_pre = 0, uint64_t t_pre = 0) {
     const pccl_topology* t = P.topo;
     const uint32_t N = t->N, L = t->L, C = P.C;
     const PhaseView pv = view_of(t, ph.transposed);
@@ -1436,6 +1438,9 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
                  o_k0 = c.take((size_t)C * 8), o_k1 = c.take((size_t)C * 8), o_v0 = c.take((size_t)C * 4),
                  o_v1 = c.take((size_t)C * 4), o_h = c.take((size_t)256 * sort_blocks * 4), o_ctrl = c.take(sizeof(BfsCtrl)),
                  o_os = c.take((size_t)L * 16);
+    const uint32_t pre_blocks = (uint32_t)((n_pre + SORT_TILE - 1) / SORT_TILE);
+    const size_t o_rdy = c.take(pre ? (size_t)C * 8 : 0), o_pk0 = c.take(n_pre * 8), o_pk1 = c.take(n_pre * 8),
+                 o_pv0 = c.take(n_pre * 4), o_pv1 = c.take(n_pre * 4), o_ph = c.take((size_t)256 * pre_blocks * 4);
     void* blob = nullptr;
     int rc = dev_alloc(c.cur, &blob);
     if (rc) return rc;
@@ -1466,6 +1471,22 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
     k_bfs_keys2<<<gC, 256, 0, counted(st)>>>(d_cdist, vals[cur], C, keys[cur ^ 1], vals[cur ^ 1]);
     cur = radix_sort_pairs(keys, vals, C, 64, ghist, sort_blocks, cur ^ 1);         // stable, by descending c.dist
     const uint32_t* d_order = vals[cur];
+    // pipelined All-Reduce: ready times and the reduce phase's records sorted by (link, t_start)
+    unsigned long long* d_ready = nullptr;
+    const uint64_t* d_pkeys = nullptr;
+    const uint32_t* d_pidx = nullptr;
+    uint32_t pre_tbits = 1;
+    if (pre && n_pre) {
+        while (pre_tbits < 64 && (t_pre >> pre_tbits)) ++pre_tbits;
+        if (pre_tbits + link_bits > 64 || n_pre > 0xFFFFFFFFull) return PCCL_ERR_UNSUPPORTED;
+        d_ready = (unsigned long long*)(b + o_rdy);
+        CU(cudaMemsetAsync(d_ready, 0, (size_t)C * 8, st));
+        uint64_t* pk[2] = {(uint64_t*)(b + o_pk0), (uint64_t*)(b + o_pk1)};
+        uint32_t* pvv[2] = {(uint32_t*)(b + o_pv0), (uint32_t*)(b + o_pv1)};
+        k_bfs_ready<<<(unsigned)((n_pre + 255) / 256), 256, 0, counted(st)>>>(pre, n_pre, ph.d_cond_src, d_ready, pre_tbits, pk[0], pvv[0]);
+        const int pc = radix_sort_pairs(pk, pvv, n_pre, pre_tbits + link_bits, (uint32_t*)(b + o_ph), pre_blocks, 0);
+        d_pkeys = pk[pc]; d_pidx = pvv[pc];
+    }
     CU(cudaGetLastError());
     BfsCtrl* mb = (BfsCtrl*)G.mailbox;
     CU(cudaMemcpyAsync(mb, ctrl, sizeof(BfsCtrl), cudaMemcpyDeviceToHost, st));
@@ -1544,6 +1565,7 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         a.runs = (ulonglong2*)(q + o_runs); a.rl_n = (uint32_t*)(q + o_rn); a.rl_start = (uint64_t*)(q + o_rs);
         a.rl_pos = (uint32_t*)(q + o_rp); a.tr_link = (uint32_t*)(q + o_tl); a.tr_start = (uint64_t*)(q + o_ts);
         a.out = raw; a.out_cap = cap; a.t_offset = 0; a.ctrl = ctrl;
+        a.t_ready = d_ready;
         a.swidx = nullptr; a.buf_limit = nullptr; a.no_mcast = nullptr; a.n_lim = 0; a.sb_cap = 0;
         a.sb_arr = a.sb_rel = a.st_arr = a.st_rel = nullptr; a.sb_n = nullptr;
         if (sw_model) {
@@ -1557,6 +1579,7 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
         }
         t_loop.start();
         k_bfs_init<<<(std::max(std::max(L, n_lim), 1u) + 255) / 256, 256, 0, counted(st)>>>(a);
+        if (d_pkeys) k_bfs_preoccupy<<<(L + 127) / 128, 128, 0, counted(st)>>>(a, pre, n_pre, d_pkeys, d_pidx, pre_tbits);
         void* args[] = {(void*)&a};
         CU(cudaLaunchCooperativeKernel(kbfs, dim3(B), dim3(BFS_THREADS), args, smem, counted(st)));
         CU(cudaMemcpyAsync(mb, ctrl, sizeof(BfsCtrl), cudaMemcpyDeviceToHost, st));
@@ -1634,8 +1657,13 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
         if (flags & PCCL_FLAG_BFS) {   // the paper's per-condition search instead of the matching loop
             BfsResult br;
             Rec* recs = nullptr;
-            const uint64_t toff = (pi == 0) ? 0 : T1;
-            rc = bfs_phase(*P, ph, seed, toff, &recs, &br, t_setup, t_loop, t_emit);
+            // All-Reduce with PCCL_FLAG_PIPELINE: the copy phase is routed against the reduce phase's intervals, each chunk
+            // from the time its root is complete (Q26) -- no shift, the two record lists are merged afterwards
+            const bool pipelined = (flags & PCCL_FLAG_PIPELINE) && pi == 1 && stage1 != nullptr;
+            if ((flags & PCCL_FLAG_PIPELINE) && P->mode == 2 && !P->topo->buf_limit.empty()) return fail(PCCL_ERR_UNSUPPORTED);
+            const uint64_t toff = (pi == 0 || pipelined) ? 0 : T1;
+            rc = pipelined ? bfs_phase(*P, ph, seed, 0, &recs, &br, t_setup, t_loop, t_emit, stage1, M1, T1)
+                           : bfs_phase(*P, ph, seed, toff, &recs, &br, t_setup, t_loop, t_emit);
             if (rc) return fail(rc);
             S->stats.wants_total += br.M;
             S->stats.events += br.conditions;
@@ -1660,15 +1688,27 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
                         return fail(PCCL_ERR_CUDA);
                     }
                     dev_free(recs);
+                    if (pipelined && br.M) {   // the phases overlap in time: one sort of the concatenation by (t_start, link)
+                        Rec* merged = nullptr;
+                        rc = dev_alloc((base + br.M) * sizeof(Rec), (void**)&merged);
+                        if (rc) return fail(rc);
+                        t_emit.start();
+                        rc = reverse_sorted(out_recs, base + br.M, std::max(T1, br.tmax), L, merged, false, 0);
+                        t_emit.stop();
+                        if (rc) { dev_free(merged); return fail(rc); }
+                        dev_free(out_recs);
+                        out_recs = merged;
+                    }
                 } else {
                     out_recs = recs;
                 }
                 S->M = base + br.M;
-                S->T = toff + br.tmax;
+                S->T = pipelined ? std::max(T1, br.tmax) : toff + br.tmax;
             }
             continue;
         }
         if (!P->topo->buf_limit.empty()) return fail(PCCL_ERR_UNSUPPORTED);   // the switch model belongs to PCCL_FLAG_BFS
+        if ((flags & PCCL_FLAG_PIPELINE) && P->mode == 2) return fail(PCCL_ERR_UNSUPPORTED);   // and so does the pipelined All-Reduce
         if (!W.blob) { rc = work_alloc(*P, W); if (rc) return fail(rc); }
         uint64_t M = 0;
         t_setup.start();

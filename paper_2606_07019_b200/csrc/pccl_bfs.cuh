@@ -68,6 +68,7 @@ struct BfsArgs {
     Rec* out;
     uint64_t out_cap, t_offset;
     BfsCtrl* ctrl;
+    const unsigned long long* t_ready;   // [C] time from which each chunk is at its source (pipelined All-Reduce, Q26), or null
     // switch model of section 4.7 (Q23-Q25); swidx == nullptr: none.  With a switch model the
     // window is one condition wide (B == 1): conditions are routed strictly one after another
     const uint32_t* swidx;            // [N] row of a node with a buffer limit in the stay tables, NONE32 otherwise
@@ -227,6 +228,36 @@ __device__ __forceinline__ bool bfs_occupy(ulonglong2* row, uint32_t R, uint64_t
     return true;
 }
 
+// ---- pipelined All-Reduce (Q26): the reduce phase's records pre-occupy the links of the copy phase ----------
+// ready[c] = end of the last transfer of chunk c into its root (the copy phase's source)
+__global__ void k_bfs_ready(const Rec* __restrict__ pre, uint64_t n, const uint32_t* __restrict__ root,
+                            unsigned long long* __restrict__ ready, uint32_t tbits, uint64_t* __restrict__ keys,
+                            uint32_t* __restrict__ idx) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const Rec r = pre[i];
+    if (r.dst == root[r.chunk]) atomicMax(&ready[r.chunk], (unsigned long long)r.t_end);
+    keys[i] = ((uint64_t)r.link << tbits) | r.t_start;            // for the sort by (link, t_start)
+    idx[i] = (uint32_t)i;
+}
+// one thread per link: its reduce-phase intervals, in time order, become busy runs
+__global__ void k_bfs_preoccupy(BfsArgs a, const Rec* __restrict__ pre, uint64_t n, const uint64_t* __restrict__ keys,
+                                const uint32_t* __restrict__ idx, uint32_t tbits) {
+    const uint32_t l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= a.L) return;
+    uint64_t lo = 0, hi = n;
+    const uint64_t first = (uint64_t)l << tbits;
+    while (lo < hi) {
+        const uint64_t mid = (lo + hi) >> 1;
+        if (keys[mid] < first) lo = mid + 1; else hi = mid;
+    }
+    ulonglong2* row = a.runs + (size_t)l * a.R;
+    for (uint64_t i = lo; i < n && (keys[i] >> tbits) == l; ++i) {
+        const Rec r = pre[idx[i]];
+        if (!bfs_occupy(row, a.R, r.t_start, r.t_end - r.t_start)) { atomicOr(&a.ctrl->err, 4u); return; }
+    }
+}
+
 // ---- Alg. 2 + 4.6 for one condition, by one CTA ---------------------------------------------
 // key[v] = (arrival(v) << link_bits) | recorded link, so that one 64-bit min keeps the earliest
 // arrival and, among equal arrivals, the lowest link id (reading Q20).  Label-correcting sweeps:
@@ -258,7 +289,11 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
     if (s_hdr) for (uint32_t l = tid; l < a.L; l += BFS_THREADS) s_hdr[l] = __ldcg(a.runs + (size_t)l * a.R);
     if (tid == 0) { sh.nf[0] = 1; sh.nf[1] = 0; sh.nf[2] = 0; fr0[0] = src; }
     __syncthreads();
-    if (tid == 0) key[src] = 0;
+    if (tid == 0) {
+        const unsigned long long t0 = a.t_ready != nullptr ? a.t_ready[chunk] : 0ull;
+        if (t0 >> (64 - lb)) atomicOr(&a.ctrl->err, 2u);
+        key[src] = t0 << lb;
+    }
     __syncthreads();
     // 32 warps run every sweep, most of them without a frontier device: what they execute between two block
     // barriers is kept to a handful of instructions (the sweep is issue-bound otherwise)

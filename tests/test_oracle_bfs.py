@@ -59,10 +59,11 @@ def _hop_costs(n, links, w, src):
     return D
 
 
-def literal_ten(n, links, conds, seed):
-    """Alg. 3 over Alg. 2 on a boolean TEN[t][link] (stored as the set of removed entries)."""
+def literal_ten(n, links, conds, seed, removed0=None, ready=None):
+    """Alg. 3 over Alg. 2 on a boolean TEN[t][link] (stored as the set of removed entries).
+    removed0 / ready: entries already taken and the timestep from which each chunk is at its source (pipelined All-Reduce)."""
     w = [int(k["alpha_ps"]) + 1 for k in links]
-    removed = set()                                   # (t, link): TEN entry taken
+    removed = set(removed0 or ())                     # (t, link): TEN entry taken
     keyed = []
     for c, (src, dests) in enumerate(conds):
         if not dests:
@@ -72,7 +73,7 @@ def literal_ten(n, links, conds, seed):
     out = []
     for _, _, c in sorted(keyed):                     # Alg. 3 line 7 (+ reading Q19 for ties)
         src, dests = conds[c]
-        arr, pred = {src: 0}, {}
+        arr, pred = {src: ready[c] if ready else 0}, {}
         t = 0
         while not all(d in arr and arr[d] <= t for d in dests):   # Alg. 2 line 4
             for l, k in enumerate(links):             # every TEN link that starts at timestep t
@@ -419,3 +420,98 @@ def test_switch_model_on_config3():
     s = oracle.synthesize(*p.args(), relay=BFS, buffer_limit=bl, no_multicast=nm)
     checker.check_schedule(p, s.transfers)
     assert s.time_ps >= base.time_ps and len(s.transfers) >= 1408
+
+
+# ------------------------------------------------------------------ pipelined All-Reduce (Q26)
+def _allreduce_case(i):
+    rng = np.random.default_rng(9100 + i)
+    n = int(rng.integers(4, 9))
+    triples = []
+    perm = rng.permutation(n)
+    for a in range(n):
+        u, v = int(perm[a]), int(perm[(a + 1) % n])
+        c = int(rng.integers(1, 4))
+        triples += [(u, v, c), (v, u, c)]              # both directions: the reduce phase runs on the transposed links
+    for _ in range(int(rng.integers(0, n))):
+        u, v = rng.choice(n, 2, replace=False)
+        triples.append((int(u), int(v), int(rng.integers(1, 4))))
+    members = sorted(rng.choice(n, int(rng.integers(2, n + 1)), replace=False).tolist())
+    nc = int(rng.integers(1, 7))
+    return n, triples, members, nc
+
+
+def literal_pipelined_allreduce(n, links, members, nc, seed):
+    """Reduce phase = the literal TEN on the transposed links, reversed in time and direction; the copy
+    phase of chunk c starts at the end of the last transfer of c into its root, on a TEN from which the reduce phase's
+    entries are already removed."""
+    w = [int(k["alpha_ps"]) + 1 for k in links]
+    tl = links.copy()
+    tl["src"], tl["dst"] = links["dst"], links["src"]
+    root = [members[c % len(members)] for c in range(nc)]          # pre = post = members: I = members (DESIGN.md step R)
+    others = [[m for m in members if m != root[c]] for c in range(nc)]
+    b = literal_ten(n, tl, [(root[c], others[c]) for c in range(nc)], seed)
+    T1 = max(r[5] for r in b)
+    red = [(T1 - te, l, c, dst, src, T1 - ts) for (ts, l, c, src, dst, te) in b]
+    removed, ready = set(), [0] * nc
+    for ts, l, c, src, dst, te in red:
+        for t in range(ts, te):
+            removed.add((t, l))
+        if dst == root[c]:
+            ready[c] = max(ready[c], te)
+    cp = literal_ten(n, links, [(root[c], others[c]) for c in range(nc)], seed, removed, ready)
+    return sorted(red + cp), T1
+
+
+@pytest.mark.parametrize("i", range(25))
+def test_pipelined_allreduce_against_the_literal_ten(i):
+    n, triples, members, nc = _allreduce_case(i)
+    links = _links(triples)
+    pairs = _pairs([(m, c) for c in range(nc) for m in members])
+    p = wl.Problem(f"ar{i}", n, links, np.array(members, dtype=np.uint32), nc, pairs, pairs.copy(), 1, i)
+    s = oracle.synthesize(*p.args(), relay=BFS, pipeline=True)
+    want, T1 = literal_pipelined_allreduce(n, links, members, nc, i)
+    assert _as_tuples(s.transfers) == want
+    assert s.time_phase1_ps == T1 and s.time_ps == max(r[5] for r in want) and s.mode == 2
+    checker.check_schedule(p, s.transfers)             # one collective: link exclusivity and sums across both phases
+    seq = oracle.synthesize(*p.args(), relay=BFS)
+    assert seq.time_phase1_ps == T1                    # the reduce phase is the same; only the copy phase moves
+
+
+def test_pipelined_allreduce_hand_example():
+    """Path 0 - 1 - 2 (unit links both ways), one chunk, all three reduce, root = node 0 (chunk 0 mod 3).  Reduce: 2 -> 1
+    over [0, 1), 1 -> 0 over [1, 2): the root is complete at 2 either way, so the copy phase 0 -> 1 [2, 3), 1 -> 2 [3, 4)
+    cannot start earlier: pipelined = sequential = 4.  With a second chunk rooted at node 1 (chunk 1 mod 3) the reduce
+    of chunk 1 ends at ... the broadcast from 1 reaches 0 and 2 at timestep 1, reversed it ends at T1 = 2 as well; its copy
+    phase 1 -> 0, 1 -> 2 over [2, 3) shares no link with chunk 0's copy 0 -> 1 [2, 3), but chunk 0's second hop 1 -> 2 now
+    waits for chunk 1's copy on that link or takes it first: T = 4 in both compositions, and the pipelined records are a
+    valid all-reduce."""
+    tri = [(0, 1, 1), (1, 0, 1), (1, 2, 1), (2, 1, 1)]
+    links = _links(tri)
+    for nc in (1, 2):
+        pairs = _pairs([(m, c) for c in range(nc) for m in (0, 1, 2)])
+        p = wl.Problem("path3_ar", 3, links, np.array([0, 1, 2], dtype=np.uint32), nc, pairs, pairs.copy(), 1, 0)
+        a = oracle.synthesize(*p.args(), relay=BFS)
+        b = oracle.synthesize(*p.args(), relay=BFS, pipeline=True)
+        assert a.time_ps == 4 and b.time_ps == 4 and b.time_phase1_ps == 2
+        checker.check_schedule(p, b.transfers)
+
+
+def test_pipelining_a_staggered_reduce_helps():
+    """Two chunks rooted at the two ends of a 4-node path with a slow middle link: the reduce of the chunk whose root
+    sits next to the fast links completes well before the whole reduce phase does, and its copy phase starts then."""
+    tri = [(0, 1, 1), (1, 0, 1), (1, 2, 3), (2, 1, 3), (2, 3, 1), (3, 2, 1)]
+    links = _links(tri)
+    members = [0, 1]
+    pairs = _pairs([(m, c) for c in range(2) for m in members])
+    p = wl.Problem("path4_ar_stagger", 4, links, np.array(members, dtype=np.uint32), 2, pairs, pairs.copy(), 1, 0)
+    a = oracle.synthesize(*p.args(), relay=BFS)
+    b = oracle.synthesize(*p.args(), relay=BFS, pipeline=True)
+    assert b.time_ps <= a.time_ps
+    checker.check_schedule(p, b.transfers)
+
+
+def test_pipeline_flag_leaves_other_collectives_alone():
+    for mk in (wl.config1, wl.config3, wl.config4_small):
+        p = mk(1)
+        a, b = run(p), oracle.synthesize(*p.args(), relay=BFS, pipeline=True)
+        assert _as_tuples(a.transfers) == _as_tuples(b.transfers)

@@ -801,3 +801,40 @@ def test_switch_model_hand_examples_and_modes(pk):
     assert e.value.code == pk.PCCL_ERR_UNSUPPORTED
     topo.set_switch_model(None, None)
     assert prob.synthesize(0, 0).time_ps == 2
+
+
+# ------------------------------------------------------------------------------ pipelined All-Reduce (NEXT-4, Q26)
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_pipelined_allreduce_config2(pk, seed):
+    p = wl.config2(seed)
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS, pipeline=True)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_BFS | pk.PCCL_FLAG_PIPELINE)
+    assert_same(p, s, o)
+    checker.check_schedule(p, s.transfers)
+    seq = gpu_run(pk, p, pk.PCCL_FLAG_BFS)
+    assert s.stats["time_phase1_ps"] == seq.stats["time_phase1_ps"] and s.time_ps <= seq.time_ps
+
+
+def test_pipelined_allreduce_random_problems(pk):
+    """every all-reduce among 90 random problems (heterogeneous links, random groups), and the flag's no-effect on the
+    copy and reduce problems among them"""
+    seen = 0
+    for i in range(90):
+        p = _random_problem(i)
+        try:
+            o = oracle.synthesize(*p.args(), relay=oracle.RELAY_BFS, pipeline=True)
+        except oracle.OracleError:
+            continue
+        s = gpu_run(pk, p, pk.PCCL_FLAG_BFS | pk.PCCL_FLAG_PIPELINE | pk.PCCL_FLAG_KEEP_ON_DEVICE)
+        assert_same(p, s, o)
+        seen += o.mode == 2
+    assert seen >= 15
+
+
+def test_pipeline_flag_needs_the_bfs_mode(pk):
+    p = wl.config2(0)
+    with pytest.raises(pk.PcclError) as e:
+        gpu_run(pk, p, pk.PCCL_FLAG_PIPELINE)
+    assert e.value.code == pk.PCCL_ERR_UNSUPPORTED
+    q = wl.config1(0)                                  # not an all-reduce: the flag has no effect
+    assert_same(q, gpu_run(pk, q, pk.PCCL_FLAG_PIPELINE), oracle.synthesize(*q.args()))
