@@ -124,6 +124,7 @@ class OracleSchedule:
 
 
 RELAY_THIN, RELAY_DYNAMIC, RELAY_BFS = 0, 1, 2
+RELAY_THIN_DIST_PICK = 3      # the thin relay tree with the c.dist-priority pick (Q27)
 
 
 NO_LIMIT = 0xFFFFFFFF

@@ -155,9 +155,14 @@ void erase_sorted(std::vector<uint32_t>& v, uint32_t x) {
 // synth_copy: steps A..F for non-reduction conditions (one source per chunk).
 // conds[c] is the condition of chunk c; chunks with !present or no dests need nothing.
 // -------------------------------------------------------------------------------------
+// pick_dist (reading Q27): Alg. 3 routes the conditions with the largest c.dist first
+// ("assigning paths to chunks that must traverse the network for the longest duration first").  As a
+// pick policy of the matching loop: a link takes, among its candidates, one of those with the LARGEST c.dist =
+// max over dests of ShortestPath(c.src, dest) (Alg. 3 lines 1-6, alpha-beta cost, reading Q3); ties by the same seeded
+// draw as the default policy -- the k-th of the tied candidates in ascending chunk id, k = (Philox(t, link) * |tied|) >> 32.
 int synth_copy(uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& conds,
                uint64_t chunk_bytes, uint64_t seed, CopyResult& res,
-               std::vector<std::vector<uint32_t>>* wants_out = nullptr) {
+               std::vector<std::vector<uint32_t>>* wants_out = nullptr, bool pick_dist = false) {
     const uint32_t L = (uint32_t)links.size();
     const uint32_t C = (uint32_t)conds.size();
 
@@ -207,6 +212,11 @@ int synth_copy(uint32_t n, const std::vector<Link>& links, const std::vector<Con
     res.wants_total = 0;
     for (uint32_t v = 0; v < n; ++v) res.wants_total += wants[v].size();
     if (wants_out) *wants_out = wants;
+    std::vector<uint64_t> cdist(C, 0);                       // Alg. 3 lines 1-6
+    if (pick_dist)
+        for (uint32_t c = 0; c < C; ++c)
+            if (conds[c].present)
+                for (uint32_t d : conds[c].dests) cdist[c] = std::max(cdist[c], D[conds[c].src][d]);
 
     // D. init
     std::vector<uint64_t> free_t(L, 0);
@@ -237,6 +247,13 @@ int synth_copy(uint32_t n, const std::vector<Link>& links, const std::vector<Con
                 std::set_intersection(hs.begin(), hs.end(), wants[v].begin(), wants[v].end(),
                                       std::back_inserter(cand));
                 if (cand.empty()) continue;            // link stays free
+                if (pick_dist) {                       // keep the candidates with the largest c.dist (ascending chunk id)
+                    uint64_t far = 0;
+                    for (uint32_t c : cand) far = std::max(far, cdist[c]);
+                    std::vector<uint32_t> tied;
+                    for (uint32_t c : cand) if (cdist[c] == far) tied.push_back(c);
+                    cand.swap(tied);
+                }
                 const uint32_t r = draw(seed, (uint32_t)(t & 0xFFFFFFFFull),
                                         (uint32_t)(t >> 32), l, 0);
                 const uint32_t k = scale(r, cand.size());
@@ -592,6 +609,7 @@ struct SwitchModel { const uint32_t* buf_limit = nullptr; const uint8_t* no_mcas
 int synth_copy_mode(int relay, uint32_t n, const std::vector<Link>& links, const std::vector<Cond>& conds,
                     uint64_t chunk_bytes, uint64_t seed, CopyResult& res, SwitchModel sw = SwitchModel()) {
     if (relay == 2) return synth_copy_bfs(n, links, conds, chunk_bytes, seed, res, sw.buf_limit, sw.no_mcast);
+    if (relay == 3) return synth_copy(n, links, conds, chunk_bytes, seed, res, nullptr, true);   // thin tree, c.dist pick
     return relay == 1 ? synth_copy_dynamic(n, links, conds, chunk_bytes, seed, res)
                       : synth_copy(n, links, conds, chunk_bytes, seed, res);
 }
@@ -812,7 +830,7 @@ int oracle_synthesize_relay(uint32_t n_npus, const oracle_link* links, uint32_t 
                             const uint32_t* group, uint32_t n_members, uint32_t n_chunks,
                             const oracle_pair* pre, uint64_t n_pre, const oracle_pair* post,
                             uint64_t n_post, uint64_t chunk_bytes, uint64_t seed, int relay, void** handle) {
-    if (!handle || relay < 0 || relay > 2) return OR_ERR_INVALID;
+    if (!handle || relay < 0 || relay > 3) return OR_ERR_INVALID;
     Result* r = new Result();
     const int rc = synthesize(n_npus, (const Link*)links, n_links, group, n_members, n_chunks,
                               (const Pair*)pre, n_pre, (const Pair*)post, n_post, chunk_bytes,
