@@ -536,6 +536,33 @@ def run_ours(args):
                "schedule_time_over_lower_bound": (bT / lb) if lb else None,
                "bound": "latency: ~10 dependent sweeps per search, one L2 round trip or more each; see DESIGN.md"}
 
+    # ---- NEXT-4 variants: the c.dist-priority pick on the same problem; the pipelined All-Reduce on config 2 (BFS mode) ----
+    variants = None
+    if not args.no_other_configs:
+        ms_v = []
+        for i in range(3):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            sv = prob.synthesize(seed, flags | pk.PCCL_FLAG_DIST_PICK)
+            e1.record()
+            e1.synchronize()
+            if i >= 1:
+                ms_v.append(e0.elapsed_time(e1))
+            vT, vst = sv.time_ps, sv.stats
+            sv.close()
+        variants = {"dist_pick": {"synthesis_ms": sum(ms_v) / len(ms_v), "loop_kernel_ms": vst["loop_ms"], "schedule_time_ps": vT,
+                                  "schedule_time_vs_uniform_pick": vT / T if T else None,
+                                  "schedule_time_over_lower_bound": (vT / lb) if lb else None}}
+        p2 = workload(2, 0)
+        t2 = pk.Topology(p2.n_npus, p2.links)
+        pr2 = pk.Problem(t2, p2.group, p2.n_chunks, p2.pre, p2.post, p2.chunk_bytes)
+        sq = pr2.synthesize(0, flags | pk.PCCL_FLAG_BFS)
+        pl = pr2.synthesize(0, flags | pk.PCCL_FLAG_BFS | pk.PCCL_FLAG_PIPELINE)
+        variants["pipelined_allreduce_config2_bfs"] = {"sequential_T_ps": sq.time_ps, "pipelined_T_ps": pl.time_ps,
+                                                       "ratio": pl.time_ps / sq.time_ps, "reduce_phase_T_ps": pl.stats["time_phase1_ps"]}
+        sq.close(); pl.close(); pr2.close(); t2.close()
+
     # ---- the other BASELINE.json configs, same path, resident inputs (context; parity is in tests/) ---
     per_config = {}
     if not args.no_other_configs:
@@ -604,7 +631,7 @@ def run_ours(args):
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": 1e3 * e2e_tot / args.steps},
             "gpu_launches": launches_timed,
-            "roofline": roofline, "cpu_baseline": cpu, "clocks": clk.summary(), "per_config": per_config, "dynamic_relay": dynamic, "paper_bfs": bfs,
+            "roofline": roofline, "cpu_baseline": cpu, "clocks": clk.summary(), "per_config": per_config, "dynamic_relay": dynamic, "paper_bfs": bfs, "variants": variants,
             "paper_context": "PCCL reports 11.68 min for 512-NPU All-to-All synthesis, hardware not stated "
                              "(PAPER.md:9, :388); a different procedure, context only",
             "wall_s_timed_region": wall}

@@ -239,6 +239,13 @@ int64_t pccl_problem_condition(const pccl_problem_t* problem, uint32_t phase, ui
                                         Other collectives: no effect.  UNSUPPORTED without PCCL_FLAG_BFS or with a switch
                                         model.  time_phase1_ps = end of the reduce phase, schedule time = the later end */
 
+#define PCCL_FLAG_DIST_PICK 16384u   /* pick policy of the matching loop (Q27; Alg. 3's order, as a
+                                        priority): a link takes one of its candidates with the LARGEST c.dist = max over dests
+                                        of the alpha-beta shortest path from the chunk's source, ties by the seeded draw (the
+                                        k-th tied candidate in ascending chunk id).  Runs in the barrier-free loop on chunks
+                                        relabelled in (c.dist, id) order; UNSUPPORTED where that loop does not apply (a node
+                                        with more than 8 in-links) and with the other mode flags */
+
 /* Steps A..F on the GPU for one seed.  Errors: UNREACHABLE, CUDA, NOMEM, INTERNAL. */
 int pccl_problem_synthesize(pccl_problem_t* problem, uint64_t seed, uint32_t flags,
                             pccl_schedule_t** out);

@@ -39,6 +39,7 @@ PCCL_FLAG_BARRIER_LOOP = 1024
 PCCL_FLAG_ASYNC = 2048
 PCCL_FLAG_LSU_SWEEP = 4096
 PCCL_FLAG_PIPELINE = 8192
+PCCL_FLAG_DIST_PICK = 16384
 PCCL_TRACE_SLOTS = 12
 PCCL_OPT_BFS_WINDOW, PCCL_OPT_BFS_ROWS, PCCL_OPT_DYNAMIC_RECORDS = 1, 2, 3
 

@@ -286,6 +286,11 @@ struct Phase {
     hvec<uint32_t> sidx;       // [N] node -> row of D, NONE32 if not a source
     hvec<uint32_t> dsts;       // distinct dests, ascending (dynamic relay: rows of the to-dest distances)
     hvec<uint32_t> didx;       // [N] node -> row, NONE32 if not a dest
+    // c.dist-priority pick (PCCL_FLAG_DIST_PICK): this phase with its chunks RELABELLED in (descending c.dist, ascending
+    // chunk id) order -- orig[c'] = the caller's chunk id, cls[c'] = index of its c.dist class (0 = farthest)
+    hvec<uint32_t> orig, cls;
+    uint32_t ncls = 0;
+    uint32_t *d_orig = nullptr, *d_cls = nullptr;
     void* blob = nullptr;
     uint32_t *d_cond_src = nullptr, *d_dests = nullptr, *d_dchunk = nullptr, *d_sources = nullptr,
              *d_sidx = nullptr, *d_dsts = nullptr, *d_didx = nullptr;
@@ -300,6 +305,7 @@ struct pccl_problem {
     uint64_t chunk_bytes = 0;
     int mode = 0;
     std::vector<Phase> phases;
+    std::vector<Phase> prio_phases;   // the phases relabelled for PCCL_FLAG_DIST_PICK (built on first use)
     bool uploaded = false;
 };
 
@@ -767,6 +773,7 @@ int phase_upload(Phase& ph, uint32_t N) {
     const size_t o_cs = c.take(C * 4), o_d = c.take(ND * 4), o_dc = c.take(ND * 4), o_s = c.take(NS * 4), o_si = c.take((size_t)N * 4);
     const size_t NDS = ph.dsts.size();
     const size_t o_do = c.take((C + 1) * 8), o_ds = c.take(NDS * 4), o_di = c.take((size_t)N * 4);
+    const size_t o_or = c.take(ph.orig.size() * 4), o_cl = c.take(ph.cls.size() * 4);
     // copied straight from the normaliser's arrays (pooled, page-locked when a device is there): no staging pass
     void* blob = nullptr;
     int rc = dev_alloc(c.cur ? c.cur : 256, &blob);
@@ -784,6 +791,8 @@ int phase_upload(Phase& ph, uint32_t N) {
     up(o_dc, ph.dchunk.data(), ND * 4);
     up(o_s, ph.sources.data(), NS * 4);
     up(o_si, ph.sidx.data(), (size_t)N * 4);
+    up(o_or, ph.orig.data(), ph.orig.size() * 4);
+    up(o_cl, ph.cls.data(), ph.cls.size() * 4);
     if (e == cudaSuccess) e = cudaStreamSynchronize(G.stream);
     if (e != cudaSuccess) {
         (void)cudaGetLastError();
@@ -797,6 +806,8 @@ int phase_upload(Phase& ph, uint32_t N) {
     ph.d_cond_src = (uint32_t*)(b + o_cs); ph.d_dests = (uint32_t*)(b + o_d); ph.d_dchunk = (uint32_t*)(b + o_dc);
     ph.d_sources = (uint32_t*)(b + o_s); ph.d_sidx = (uint32_t*)(b + o_si);
     ph.d_dest_off = (uint64_t*)(b + o_do); ph.d_dsts = (uint32_t*)(b + o_ds); ph.d_didx = (uint32_t*)(b + o_di);
+    ph.d_orig = ph.orig.empty() ? nullptr : (uint32_t*)(b + o_or);
+    ph.d_cls = ph.cls.empty() ? nullptr : (uint32_t*)(b + o_cl);
     return PCCL_OK;
 }
 
@@ -824,6 +835,7 @@ extern "C" void pccl_problem_destroy(pccl_problem_t* P) {
     SERIALISE;
     if (!P) return;
     for (Phase& ph : P->phases) dev_free(ph.blob);
+    for (Phase& ph : P->prio_phases) dev_free(ph.blob);
     delete P;
 }
 
@@ -988,7 +1000,7 @@ int phase_setup(const pccl_problem& P, const Phase& ph, Work& W, uint64_t seed, 
     if (ND) {
         k_wants<<<(unsigned)((ND + 127) / 128), 128, 0, counted(st)>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, ND, pv.esrc, pv.in_off,
                                                           pv.in_link, W.w, ph.d_sidx, W.D, N, W.Wp, W.SWp, k0, k1, W.wants,
-                                                          W.wsum, W.wants_cnt, &W.ctrl->err);
+                                                          W.wsum, W.wants_cnt, &W.ctrl->err, ph.d_orig);
     }
     k_sum_u32<<<1, 1024, 0, counted(st)>>>(W.wants_cnt, N, &W.ctrl->wants_total);
     W.a2_planned = false;
@@ -998,7 +1010,7 @@ int phase_setup(const pccl_problem& P, const Phase& ph, Work& W, uint64_t seed, 
         W.a2_grid = (N + W.a2_wpc - 1) / W.a2_wpc;
         A2Args pa;
         memset(&pa, 0, sizeof(pa));
-        pa.N = N; pa.L = L; pa.grid = W.a2_grid; pa.wpc = W.a2_wpc;
+        pa.N = N; pa.L = L; pa.grid = W.a2_grid; pa.wpc = W.a2_wpc; pa.ncls = ph.ncls;
         pa.esrc = pv.esrc; pa.in_off = pv.in_off; pa.w = W.w; pa.wants_cnt = W.wants_cnt;
         pa.nbase = W.nbase; pa.poff = W.poff; pa.loff = W.loff; pa.soff = W.soff; pa.ctrl = W.a2ctrl;
         k_a2_plan<<<1, 1024, 0, counted(st)>>>(pa);
@@ -1120,6 +1132,7 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     a.N = N; a.L = L; a.Wp = W.Wp; a.nLw = W.nLw;
     a.k0 = (uint32_t)(seed & 0xFFFFFFFFull); a.k1 = (uint32_t)(seed >> 32);
     a.grid = W.a2_grid; a.wpc = W.a2_wpc;
+    a.ncls = ph.ncls; a.cls = ph.d_cls; a.orig = ph.d_orig;
     a.esrc = pv.esrc; a.edst = pv.edst; a.psrc = t->d_src; a.pdst = t->d_dst; a.in_off = pv.in_off; a.in_link = pv.in_link;
     a.w = W.w; a.wants = W.wants; a.wants_cnt = W.wants_cnt; a.csrc = ph.d_cond_src;
     a.nbase = W.nbase; a.poff = W.poff; a.loff = W.loff; a.soff = W.soff; a.ctrl = W.a2ctrl; a.abort_flag = &W.ctrl->err;
@@ -1155,13 +1168,14 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     k_a2_priv<<<N, 128, 0, counted(st)>>>(a);
     const size_t smem = (size_t)W.a2.smem_need;
     const int threads = (int)W.a2_wpc * 32;
-    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_loop2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const void* kloop2 = ph.ncls ? (const void*)k_loop2<true> : (const void*)k_loop2<false>;
+    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kloop2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_loop2, threads, smem));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kloop2, threads, smem));
     if (occ < 1 || (uint64_t)occ * (uint64_t)G.sm_count < W.a2_grid) return PCCL_ERR_INTERNAL;   // (checked by the caller's plan)
     void* args[] = {(void*)&a};
     if (tm) { tm->setup.stop(); tm->loop.start(); }
-    CU(cudaLaunchCooperativeKernel((const void*)k_loop2, dim3(W.a2_grid), dim3(threads), args, smem, counted(st)));
+    CU(cudaLaunchCooperativeKernel(kloop2, dim3(W.a2_grid), dim3(threads), args, smem, counted(st)));
     if (tm) { tm->loop.stop(); tm->emit.start(); }
     // emit
     k_emit_times<<<N, 256, 0, counted(st)>>>(a);
@@ -1221,8 +1235,9 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
                Rec* host_out = nullptr, bool* streamed = nullptr) {
     const bool dynamic = (flags & PCCL_FLAG_DYNAMIC_RELAY) != 0;
     if (W.a2_planned && out_cap > 0 && out_cap <= 0xFFFFFFFFull && W.a2.smem_need <= 220 * 1024 &&
-        ((flags & PCCL_FLAG_ASYNC) || W.a2.w_max / 16 <= W.a2.w_min))
+        ((flags & (PCCL_FLAG_ASYNC | PCCL_FLAG_DIST_PICK)) || W.a2.w_max / 16 <= W.a2.w_min))
         return phase_loop_async(P, ph, W, seed, flags, out, out_cap, t_offset, ph.transposed, res, tm);
+    if ((flags & PCCL_FLAG_DIST_PICK) && out_cap > 0) return PCCL_ERR_UNSUPPORTED;   // the c.dist pick lives in the barrier-free loop
     // the dynamic rule keeps the counts current too: wants bits are only dropped where a neighbour holds the chunk
     // (holder lists, dyn_shrink_wants); DENSE_SWEEP / RESCAN recount instead and drop every bit at once
     const pccl_topology* t = P.topo;
@@ -1404,6 +1419,80 @@ int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out, bool 
 // holds the M records in canonical order (reversed in direction and time for a transposed
 // phase, shifted by t_shift otherwise); the caller owns it.
 // ---------------------------------------------------------------------------------------
+// PCCL_FLAG_DIST_PICK: the phases of P with their chunks relabelled in (descending c.dist, ascending chunk id) order, so
+// that "the candidates with the largest c.dist" are the candidates of the lowest class of labels and ascending label =
+// ascending chunk id inside a class.  c.dist and the order are computed on the device (link costs, distances, k_cdist,
+// stable radix sort); the host only re-indexes the condition arrays with that order.  Cached in the problem.
+int prio_prepare(pccl_problem& P) {
+    if (!P.prio_phases.empty()) return PCCL_OK;
+    const pccl_topology* t = P.topo;
+    const uint32_t N = t->N, L = t->L, C = P.C;
+    cudaStream_t st = G.stream;
+    std::vector<Phase> out;
+    try {
+        for (const Phase& ph : P.phases) {
+            const PhaseView pv = view_of(t, ph.transposed);
+            const uint32_t NS = (uint32_t)ph.sources.size();
+            const uint32_t nblocks = (uint32_t)((C + SORT_TILE - 1) / SORT_TILE);
+            Carver c;
+            const size_t o_w = c.take((size_t)L * 8), o_D = c.take((size_t)NS * N * 8), o_cd = c.take((size_t)C * 8),
+                         o_k0 = c.take((size_t)C * 8), o_k1 = c.take((size_t)C * 8), o_v0 = c.take((size_t)C * 4),
+                         o_v1 = c.take((size_t)C * 4), o_h = c.take((size_t)256 * std::max(nblocks, 1u) * 4);
+            void* blob = nullptr;
+            int rc = dev_alloc(c.cur, &blob);
+            if (rc) return rc;
+            struct Guard { void* p; ~Guard() { dev_free(p); } } guard{blob};
+            unsigned char* b = (unsigned char*)blob;
+            uint64_t* keys[2] = {(uint64_t*)(b + o_k0), (uint64_t*)(b + o_k1)};
+            uint32_t* vals[2] = {(uint32_t*)(b + o_v0), (uint32_t*)(b + o_v1)};
+            std::vector<uint64_t> h_cd(C);
+            std::vector<uint32_t> h_order(C);
+            if (C) {
+                if (L) k_link_cost<<<(L + 255) / 256, 256, 0, counted(st)>>>(t->d_alpha, t->d_bpp, L, P.chunk_bytes, (uint64_t*)(b + o_w));
+                if (NS) {
+                    const size_t smem = (size_t)N * 8;
+                    if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
+                    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                    k_distances<<<NS, 256, smem, counted(st)>>>(pv.esrc, pv.edst, (uint64_t*)(b + o_w), N, L, ph.d_sources, (uint64_t*)(b + o_D));
+                }
+                k_cdist<<<(C + 255) / 256, 256, 0, counted(st)>>>(ph.d_cond_src, ph.d_dest_off, ph.d_dests, C, ph.d_sidx, (uint64_t*)(b + o_D), N,
+                                                                  (uint64_t*)(b + o_cd), keys[0], vals[0]);
+                const int cur = radix_sort_pairs(keys, vals, C, 64, (uint32_t*)(b + o_h), nblocks, 0);
+                CU(cudaGetLastError());
+                CU(cudaMemcpyAsync(h_cd.data(), b + o_cd, (size_t)C * 8, cudaMemcpyDeviceToHost, st));
+                CU(cudaMemcpyAsync(h_order.data(), vals[cur], (size_t)C * 4, cudaMemcpyDeviceToHost, st));
+                CU(cudaStreamSynchronize(st));
+            }
+            // re-index the conditions with the device's order (no arithmetic of the method here)
+            Phase pp;
+            pp.transposed = ph.transposed;
+            pp.sources = ph.sources; pp.sidx = ph.sidx; pp.dsts = ph.dsts; pp.didx = ph.didx;
+            pp.cond_src.resize(C); pp.dest_off.resize((size_t)C + 1); pp.dests.resize(ph.dests.size()); pp.dchunk.resize(ph.dests.size());
+            pp.orig.resize(C); pp.cls.resize(C);
+            uint64_t nd = 0;
+            uint32_t cls = 0;
+            pp.dest_off[0] = 0;
+            for (uint32_t i = 0; i < C; ++i) {
+                const uint32_t c0 = h_order[i];
+                if (i > 0 && h_cd[c0] != h_cd[h_order[i - 1]]) ++cls;
+                pp.orig[i] = c0; pp.cls[i] = cls;
+                pp.cond_src[i] = ph.cond_src[c0];
+                for (uint64_t k = ph.dest_off[c0]; k < ph.dest_off[c0 + 1]; ++k) { pp.dests[nd] = ph.dests[k]; pp.dchunk[nd] = i; ++nd; }
+                pp.dest_off[i + 1] = nd;
+            }
+            pp.ncls = C ? cls + 1 : 0;
+            int rc2 = phase_upload(pp, N);
+            if (rc2) return rc2;
+            out.push_back(std::move(pp));
+        }
+    } catch (const std::bad_alloc&) {
+        for (Phase& ph : out) dev_free(ph.blob);
+        return PCCL_ERR_NOMEM;
+    }
+    P.prio_phases = std::move(out);
+    return PCCL_OK;
+}
+
 struct BfsResult {
     uint64_t M, tmax, conditions, searches, relax, rounds;
     uint32_t grid;
@@ -1651,8 +1740,15 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
         return code;
     };
     const uint32_t L = P->topo->L;
+    const bool dist_pick = (flags & PCCL_FLAG_DIST_PICK) != 0;
+    if (dist_pick) {
+        if (flags & (PCCL_FLAG_BFS | PCCL_FLAG_DYNAMIC_RELAY | PCCL_FLAG_RESCAN | PCCL_FLAG_DENSE_SWEEP | PCCL_FLAG_TWO_BARRIERS |
+                     PCCL_FLAG_BARRIER_LOOP | PCCL_FLAG_TRACE)) return fail(PCCL_ERR_UNSUPPORTED);
+        rc = prio_prepare(*P);
+        if (rc) return fail(rc);
+    }
     for (size_t pi = 0; pi < P->phases.size(); ++pi) {
-        const Phase& ph = P->phases[pi];
+        const Phase& ph = dist_pick ? P->prio_phases[pi] : P->phases[pi];
         const bool last = pi + 1 == P->phases.size();
         if (flags & PCCL_FLAG_BFS) {   // the paper's per-condition search instead of the matching loop
             BfsResult br;

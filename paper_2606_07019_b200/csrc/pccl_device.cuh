@@ -146,10 +146,12 @@ __global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* _
                         const uint32_t* __restrict__ in_link, const uint64_t* __restrict__ w,
                         const uint32_t* __restrict__ sidx, const uint64_t* __restrict__ D, uint32_t N,
                         uint32_t Wp, uint32_t SWp, uint32_t k0, uint32_t k1, uint64_t* __restrict__ wants,
-                        uint64_t* __restrict__ wsum, uint32_t* __restrict__ wants_cnt, uint32_t* __restrict__ err) {
+                        uint64_t* __restrict__ wsum, uint32_t* __restrict__ wants_cnt, uint32_t* __restrict__ err,
+                        const uint32_t* __restrict__ orig = nullptr) {   // orig: the caller's id of a relabelled chunk (keys the draw)
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n_pairs) return;
     const uint32_t c = dchunk[p];
+    const uint32_t ck = orig != nullptr ? orig[c] : c;
     const uint32_t s = cond_src[c];
     const uint64_t* Ds = D + (size_t)sidx[s] * N;
     uint32_t cur = dests[p];
@@ -173,7 +175,7 @@ __global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* _
                 if (du != T_INF && du + w[l] == dcur) mask |= 1u << (e - e0);
             }
             if (mask == 0) { atomicOr(err, 2u); return; }
-            const uint32_t j = __umulhi(philox_draw(c, cur, 0u, 1u, k0, k1), (uint32_t)__popc(mask));
+            const uint32_t j = __umulhi(philox_draw(ck, cur, 0u, 1u, k0, k1), (uint32_t)__popc(mask));
             nxt = esrc[in_link[e0 + __fns(mask, 0, (int)j + 1)]];
         } else {
             uint32_t ntight = 0;
@@ -183,7 +185,7 @@ __global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* _
                 ntight += (du != T_INF && du + w[l] == dcur);
             }
             if (ntight == 0) { atomicOr(err, 2u); return; }
-            uint32_t j = __umulhi(philox_draw(c, cur, 0u, 1u, k0, k1), ntight);
+            uint32_t j = __umulhi(philox_draw(ck, cur, 0u, 1u, k0, k1), ntight);
             for (uint32_t e = e0; e < e1; ++e) {
                 const uint32_t l = in_link[e];
                 const uint32_t u = esrc[l];
@@ -242,6 +244,25 @@ __global__ void k_wants_dyn_init(const uint64_t* __restrict__ dest_off, const ui
         atomicOr((unsigned long long*)&wsum[(size_t)u * SWp + (wi >> 8)], 1ull << ((wi >> 2) & 63));
         atomicAdd(&wants_cnt[u], (uint32_t)__popcll(word));
     }
+}
+
+// Alg. 3 lines 1-6: c.dist = max over dests of ShortestPath(c.src, dest); key = ~c.dist so that an
+// ascending stable sort lists the farthest conditions first, equal ones in ascending chunk id
+__global__ void k_cdist(const uint32_t* __restrict__ cond_src, const uint64_t* __restrict__ dest_off,
+                        const uint32_t* __restrict__ dests, uint32_t C, const uint32_t* __restrict__ sidx,
+                        const uint64_t* __restrict__ D, uint32_t N, uint64_t* __restrict__ cdist, uint64_t* __restrict__ key,
+                        uint32_t* __restrict__ val) {
+    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= C) return;
+    const uint64_t d0 = dest_off[c], d1 = dest_off[c + 1];
+    uint64_t dmax = 0;
+    if (d1 > d0) {
+        const uint64_t* row = D + (size_t)sidx[cond_src[c]] * N;
+        for (uint64_t i = d0; i < d1; ++i) dmax = max(dmax, (uint64_t)row[dests[i]]);
+    }
+    cdist[c] = dmax;
+    key[c] = ~dmax;
+    val[c] = c;
 }
 
 // sum of wants_cnt -> ctrl (one block)

@@ -102,18 +102,23 @@ struct A2Fixed {
 };
 static_assert(sizeof(A2Fixed) % 16 == 0, "alignment of the arrays that follow");
 
-__host__ __device__ __forceinline__ uint32_t a2_priv_words(uint32_t W, uint32_t nin) {
+// ncls > 0 (PCCL_FLAG_DIST_PICK): the image ends with the destination's class boundaries in entry space,
+// [nb][bnd[0 .. ncls]]: bnd[i] = first entry of the i-th c.dist class present among the entries, bnd[nb] = W
+__host__ __device__ __forceinline__ uint32_t a2_priv_words(uint32_t W, uint32_t nin, uint32_t ncls) {
     const uint32_t Wd = (W + 31) >> 5, G = (Wd + 31) >> 5;
-    return Wd * (1 + nin) + nin * G;          // live[Wd], cb[nin][Wd], grp[nin][G]
+    return Wd * (1 + nin) + nin * G + (ncls ? ncls + 2 : 0);   // live[Wd], cb[nin][Wd], grp[nin][G], boundaries
 }
-__host__ __device__ __forceinline__ uint32_t a2_warp_bytes(uint32_t W, uint32_t nin) {
-    return (uint32_t)sizeof(A2Fixed) + ((a2_priv_words(W, nin) * 4u + 15u) & ~15u);
+__host__ __device__ __forceinline__ uint32_t a2_warp_bytes(uint32_t W, uint32_t nin, uint32_t ncls) {
+    return (uint32_t)sizeof(A2Fixed) + ((a2_priv_words(W, nin, ncls) * 4u + 15u) & ~15u);
 }
 
 struct A2Args {
     uint32_t N, L, Wp, nLw;
     uint32_t k0, k1;
     uint32_t grid, wpc;               // CTAs and warps per CTA of k_loop2 (destination v = cta + warp * grid)
+    uint32_t ncls;                    // c.dist classes of the relabelled chunks (PCCL_FLAG_DIST_PICK), 0: uniform pick
+    const uint32_t* cls;              // [C] class of each (relabelled) chunk
+    const uint32_t* orig;             // [C] the caller's chunk id of each relabelled chunk, or null
     const uint32_t *esrc, *edst, *psrc, *pdst, *in_off, *in_link;
     const uint64_t* w;
     const uint64_t* wants;            // [N][Wp], static
@@ -193,7 +198,7 @@ __global__ void __launch_bounds__(1024) k_a2_plan(A2Args a) {
     carry = 0;
     for (uint32_t b = 0; b < a.N; b += 1024) {                       // poff
         const uint32_t v = b + tid;
-        const unsigned long long x = v < a.N ? a2_priv_words(a.wants_cnt[v], a.in_off[v + 1] - a.in_off[v]) : 0ull;
+        const unsigned long long x = v < a.N ? a2_priv_words(a.wants_cnt[v], a.in_off[v + 1] - a.in_off[v], a.ncls) : 0ull;
         const unsigned long long ex = block_excl_scan_1024(x, &tot, sm);
         if (v < a.N) a.poff[v] = carry + ex;
         carry += tot;
@@ -219,7 +224,7 @@ __global__ void __launch_bounds__(1024) k_a2_plan(A2Args a) {
             const uint32_t v = cta + wi * a.grid;
             if (v >= a.N) break;
             a.soff[v] = off;
-            off += a2_warp_bytes(a.wants_cnt[v], a.in_off[v + 1] - a.in_off[v]);
+            off += a2_warp_bytes(a.wants_cnt[v], a.in_off[v + 1] - a.in_off[v], a.ncls);
         }
         mx = max(mx, (unsigned long long)off);
     }
@@ -316,6 +321,29 @@ __global__ void __launch_bounds__(128) k_a2_priv(A2Args a) {
         for (uint32_t wd = g * 32; wd < min(Wd, g * 32 + 32); ++wd) s += __popc(cb[(size_t)j * Wd + wd]);
         grp[i] = s;
     }
+    if (a.ncls) {
+        // entries ascend in (relabelled) chunk id, so their classes ascend too: the boundaries are the entries whose
+        // class differs from the entry before; bnd[i] is written at the rank of its class among the present ones
+        uint32_t* pb = grp + (size_t)nin * G;       // [nb][bnd ...]
+        __shared__ uint32_t s_nb;
+        if (threadIdx.x == 0) s_nb = 0;
+        __syncthreads();
+        for (uint32_t e = threadIdx.x; e < W; e += blockDim.x)
+            if (e == 0 || a.cls[ids[e]] != a.cls[ids[e - 1]]) pb[1 + atomicAdd(&s_nb, 1u)] = e;
+        __syncthreads();
+        if (threadIdx.x == 0) {                     // few boundaries: insertion sort, then the sentinel
+            const uint32_t nb = s_nb;
+            uint32_t* B = pb + 1;
+            for (uint32_t i = 1; i < nb; ++i) {
+                const uint32_t x = B[i];
+                uint32_t k = i;
+                while (k > 0 && B[k - 1] > x) { B[k] = B[k - 1]; --k; }
+                B[k] = x;
+            }
+            pb[0] = nb;
+            B[nb] = W;
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -400,6 +428,48 @@ __device__ __forceinline__ uint32_t a2_quad_select(const uint32_t* cbj, const ui
     return __shfl_sync(0xFFFFFFFFu, e, qbase + own);
 }
 
+// candidates of row cbj with an entry index below hi, by the quad (same layout as a2_quad_select)
+__device__ __forceinline__ uint32_t a2_quad_rank(const uint32_t* cbj, const uint32_t* grpj, uint32_t Wd, uint32_t hi, bool on,
+                                                 uint32_t q) {
+    uint32_t sum = 0;
+    const uint32_t gh = hi >> 10, wh = hi >> 5;
+    if (on) {
+        for (uint32_t g = q; g < gh; g += 4) sum += grpj[g];          // whole groups below hi
+        const uint32_t w0 = gh * 32 + q * 8;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const uint32_t wi = w0 + i;
+            if (wi < Wd && wi <= wh) {
+                const uint32_t word = cbj[wi];
+                sum += __popc(wi < wh ? word : (word & ((1u << (hi & 31)) - 1u)));
+            }
+        }
+    }
+    sum += __shfl_xor_sync(0xFFFFFFFFu, sum, 1);
+    sum += __shfl_xor_sync(0xFFFFFFFFu, sum, 2);
+    return sum;
+}
+
+// The pick of one in-link by its quad: the k-th candidate, k = (r * n) >> 32 -- over all n candidates, or (PRIO, reading
+// Q27) over the candidates of the first candidate's c.dist class: the entries are in (class, chunk id) order, so those are
+// the candidates below the class's end bnd[.] and the k-th of them is the k-th candidate overall.
+template <bool PRIO>
+__device__ __forceinline__ uint32_t a2_pick(const uint32_t* cbj, const uint32_t* grpj, uint32_t Wd, uint32_t G, uint32_t n,
+                                            uint32_t r, bool on, uint32_t q, uint32_t lane, const uint32_t* pb, uint32_t W) {
+    if (PRIO) {
+        const uint32_t e0 = a2_quad_select(cbj, grpj, Wd, G, 0u, on, q, lane);
+        uint32_t hi = W;
+        if (on) {
+            const uint32_t nb = pb[0];
+            for (uint32_t i = q; i <= nb; i += 4) { const uint32_t b = pb[1 + i]; if (b > e0) hi = min(hi, b); }
+        }
+        hi = min(hi, __shfl_xor_sync(0xFFFFFFFFu, hi, 1));
+        hi = min(hi, __shfl_xor_sync(0xFFFFFFFFu, hi, 2));
+        n = a2_quad_rank(cbj, grpj, Wd, hi, on, q);
+    }
+    return a2_quad_select(cbj, grpj, Wd, G, __umulhi(r, n), on, q, lane);
+}
+
 // The quads whose `doit` is set claim their entry e for in-link j4 = lane / 4 at time t: the entry leaves every
 // in-link's candidates (lane q of the quad serves rows q and q + 4), the link is busy until t + w,
 // the claim goes to the log at position rank.  Entries of different quads are distinct.
@@ -425,6 +495,7 @@ __device__ __forceinline__ void a2_commit(A2Fixed& f, uint32_t* live, uint32_t* 
     }
 }
 
+template <bool PRIO>
 __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) {
     extern __shared__ __align__(16) unsigned char a2_smem[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -438,6 +509,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
     const uint32_t Wd = (W + 31) >> 5, G = (Wd + 31) >> 5;
     uint32_t* cb = live + Wd;
     uint32_t* grp = cb + nin * Wd;
+    const uint32_t* pb = grp + nin * G;                              // class boundaries (PRIO)
     // ---- static tables (once) ----
     if (lane == 0) {
         f.nin = nin; f.W = W; f.Wd = Wd; f.G = G;
@@ -468,7 +540,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
     for (uint32_t h = lane; h < A2_MAX_IN * 8; h += 32) { f.pend_e[h] = NONE32; f.pend_te[h] = T_INF; }
     {
         const uint32_t* img = a.priv + a.poff[v];
-        const uint32_t words = a2_priv_words(W, nin);
+        const uint32_t words = a2_priv_words(W, nin, a.ncls);
         for (uint32_t i = lane; i < words; i += 32) live[i] = img[i];
     }
     __syncwarp();
@@ -666,8 +738,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
             const bool on = inl && nj != 0u && frj <= t;
             if (inl && q4 == 0 && frj > t) nt_o = min(nt_o, frj);                       // a busy in-link frees
             const uint32_t rj = __shfl_sync(0xFFFFFFFFu, r_mine, j4);
-            const uint32_t e_spec = a2_quad_select(cb + (inl ? j4 : 0u) * Wd, grp + (inl ? j4 : 0u) * G, Wd, G,
-                                                   __umulhi(rj, nj), on, q4, lane);
+            const uint32_t e_spec = a2_pick<PRIO>(cb + (inl ? j4 : 0u) * Wd, grp + (inl ? j4 : 0u) * G, Wd, G, nj, rj, on, q4, lane, pb, W);
             const uint32_t onmask = __ballot_sync(0xFFFFFFFFu, on && q4 == 0);          // bit 4j
             // is an earlier pick i < j a candidate of in-link j?
             bool bad = false;
@@ -708,7 +779,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
                     const uint32_t n2 = f.n[j];
                     if (n2 == 0u || f.free_te[j] > t) continue;
                     const uint32_t r2 = __shfl_sync(0xFFFFFFFFu, r_mine, j);
-                    const uint32_t e2 = a2_quad_select(cb + j * Wd, grp + j * G, Wd, G, __umulhi(r2, n2), j4 == j, q4, lane);
+                    const uint32_t e2 = a2_pick<PRIO>(cb + j * Wd, grp + j * G, Wd, G, n2, r2, j4 == j, q4, lane, pb, W);
                     const uint32_t e = __shfl_sync(0xFFFFFFFFu, e2, 4 * j);
                     if (e == NONE32) { if (lane == 0) atomicOr(a.abort_flag, 4u); return; }   // cannot happen
                     a2_commit(f, live, cb, grp, nin, Wd, G, j4 == j, e, j4, q4, t, mylog + cnt + claims);
@@ -875,7 +946,8 @@ __global__ void __launch_bounds__(256) k_emit_write(A2Args a) {
         if (pos >= a.out_cap) { atomicOr(&a.ctrl->err, 2u); continue; }
         const unsigned long long ts = en.lo + a.t_offset, te = en.lo + a.w[l] + a.t_offset;
         uint4* o = reinterpret_cast<uint4*>(a.out + pos);
-        o[0] = make_uint4(ids[(uint32_t)en.hi], a.psrc[l], a.pdst[l], l);
+        const uint32_t ch = ids[(uint32_t)en.hi];
+        o[0] = make_uint4(a.orig != nullptr ? a.orig[ch] : ch, a.psrc[l], a.pdst[l], l);
         o[1] = make_uint4((uint32_t)ts, (uint32_t)(ts >> 32), (uint32_t)te, (uint32_t)(te >> 32));
     }
 }
@@ -894,7 +966,8 @@ __global__ void __launch_bounds__(256) k_emit_raw(A2Args a) {
         if (base + i >= a.out_cap) { atomicOr(&a.ctrl->err, 2u); continue; }
         const unsigned long long ts = en.lo + a.t_offset, te = en.lo + a.w[l] + a.t_offset;
         uint4* o = reinterpret_cast<uint4*>(a.out + base + i);
-        o[0] = make_uint4(ids[(uint32_t)en.hi], a.psrc[l], a.pdst[l], l);
+        const uint32_t ch = ids[(uint32_t)en.hi];
+        o[0] = make_uint4(a.orig != nullptr ? a.orig[ch] : ch, a.psrc[l], a.pdst[l], l);
         o[1] = make_uint4((uint32_t)ts, (uint32_t)(ts >> 32), (uint32_t)te, (uint32_t)(te >> 32));
     }
 }

@@ -202,7 +202,7 @@ def test_compute_fails_loudly_without_a_device(pk):
 def test_flag_constants_match_the_header(pk):
     src = open(os.path.join(ROOT, "include", "pccl.h")).read()
     flags = dict(re.findall(r"#define (PCCL_FLAG_[A-Z_]+) (\d+)u", src))
-    assert len(flags) == 14
+    assert len(flags) == 15
     for name, val in flags.items():
         assert getattr(pk, name) == int(val), name
     assert int(re.search(r"#define PCCL_TRACE_SLOTS (\d+)", src).group(1)) == pk.PCCL_TRACE_SLOTS

@@ -838,3 +838,50 @@ def test_pipeline_flag_needs_the_bfs_mode(pk):
     assert e.value.code == pk.PCCL_ERR_UNSUPPORTED
     q = wl.config1(0)                                  # not an all-reduce: the flag has no effect
     assert_same(q, gpu_run(pk, q, pk.PCCL_FLAG_PIPELINE), oracle.synthesize(*q.args()))
+
+
+# ------------------------------------------------------------------------------ c.dist-priority pick (NEXT-4, Q27)
+@pytest.mark.parametrize("maker", [wl.config1, wl.config2, wl.config4_small, wl.config5_small, wl.two_groups_mesh3x3,
+                                   lambda s: wl.ring_all_gather(8, True, s, chunks_per_npu=1040, chunk_bytes=4096),
+                                   lambda s: _torus_all_gather((12, 12), 2, s)], ids=lambda m: getattr(m, "__name__", "case"))
+@pytest.mark.parametrize("seed", [0, 1])
+def test_dist_pick_equals_oracle(pk, maker, seed):
+    p = maker(seed)
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_THIN_DIST_PICK)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_DIST_PICK)
+    assert_same(p, s, o)
+    checker.check_schedule(p, s.transfers)
+
+
+def test_dist_pick_random_problems(pk):
+    """heterogeneous links give many distinct c.dist values (one class per chunk in the extreme); nodes with more than
+    8 in-links are refused"""
+    ran = 0
+    for i in range(60):
+        p = _random_problem(i)
+        try:
+            o = oracle.synthesize(*p.args(), relay=oracle.RELAY_THIN_DIST_PICK)
+        except oracle.OracleError:
+            continue
+        try:
+            s = gpu_run(pk, p, pk.PCCL_FLAG_DIST_PICK | pk.PCCL_FLAG_KEEP_ON_DEVICE)
+        except pk.PcclError as e:
+            assert e.code == pk.PCCL_ERR_UNSUPPORTED
+            indeg = np.bincount(p.links["dst"], minlength=p.n_npus).max()
+            outdeg = np.bincount(p.links["src"], minlength=p.n_npus).max()
+            assert max(indeg, outdeg) > 8, p.name
+            continue
+        assert_same(p, s, o)
+        ran += 1
+    assert ran >= 10
+
+
+@pytest.mark.slow
+def test_dist_pick_config4_full_size(pk):
+    p = wl.config4(0)
+    o = oracle.synthesize(*p.args(), relay=oracle.RELAY_THIN_DIST_PICK)
+    s = gpu_run(pk, p, pk.PCCL_FLAG_DIST_PICK | pk.PCCL_FLAG_KEEP_ON_DEVICE)
+    assert_same(p, s, o)
+    with pytest.raises(pk.PcclError) as e:
+        gpu_run(pk, wl.config3(0), pk.PCCL_FLAG_DIST_PICK)          # 15-in-link switches
+    assert e.value.code == pk.PCCL_ERR_UNSUPPORTED
