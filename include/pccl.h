@@ -59,7 +59,8 @@ typedef enum pccl_error {
     PCCL_ERR_UNREACHABLE = -3, /* some destination cannot be reached from its chunk's source */
     PCCL_ERR_CUDA = -4,        /* any CUDA runtime failure, including "no device" */
     PCCL_ERR_NOMEM = -5,       /* host or device allocation failed */
-    PCCL_ERR_INTERNAL = -6     /* a post-run invariant failed (never expected) */
+    PCCL_ERR_INTERNAL = -6,    /* a post-run invariant failed (never expected) */
+    PCCL_ERR_TOO_LARGE = -7    /* pccl_candidate_totals_static: the problem needs more than PCCL_STATIC_SCRATCH_BYTES */
 } pccl_error;
 
 /* A directed physical link, cost alpha_ps + ceil(chunk_bytes / bytes_per_ps) picoseconds
@@ -334,6 +335,38 @@ int pccl_device_candidate_sweep(pccl_problem_t* problem, uint32_t phase, uint64_
  * ld.global.cg, grid-stride) `iters` times and reports the milliseconds per pass: the measured ceiling of L2 when the
  * buffer fits there, of HBM when it does not.  Errors: INVALID, CUDA, NOMEM. */
 int pccl_device_read_bandwidth(uint64_t bytes, uint32_t iters, float* ms_per_pass);
+
+/* ---------------------------------------------------------------------------------------
+ * The entry point that allocates nothing.
+ *
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): row a5 -- |cand(l)| = popcount(have[src_l] & wants[dst_l]) of every link (one chunk per link and
+ * step; north star: per-link candidate bitmap) -- on bitmaps the CALLER holds on the device, by the same streaming
+ * sweep kernel as pccl_device_candidate_sweep.  The kernel's scratch (per-link, per-4096-chunk segment counts and the
+ * whole-row sums it keeps beside them) lives in a fixed array of PCCL_STATIC_SCRATCH_BYTES inside the library's device
+ * image: every GPU that loads the library holds it until the process exits.  The call makes no cudaMalloc / cudaFree /
+ * cudaMallocAsync / cudaHostAlloc and calls no allocating library routine; it enqueues one memset, two kernels.
+ *
+ *   have, wants     device, n_npus rows of words_per_row u64 each (bit c of row v = chunk c at / wanted by node v);
+ *                   16-byte aligned, words_per_row even and > 0 (rows are copied in 16-byte units)
+ *   link_src        device, n_links u32: source node of link l
+ *   in_off, in_link device, CSR by destination: the in-links of node v are in_link[in_off[v] .. in_off[v+1]),
+ *                   n_npus + 1 and n_links u32; every link appears once
+ *   totals          device, n_links u32, written: |cand(l)|
+ *   stream          a cudaStream_t (NULL = the default stream); the work is enqueued there, the call does not wait
+ *
+ * Limit: n_links * (ceil(words_per_row / 64) + 1) * 4 bytes <= PCCL_STATIC_SCRATCH_BYTES, else PCCL_ERR_TOO_LARGE
+ * (nothing is enqueued).  Other errors: INVALID (null / misaligned pointer, odd or zero words_per_row), CUDA.
+ * n_npus == 0 or n_links == 0: PCCL_OK, nothing enqueued.
+ *
+ * Every call on a device shares the one array, which keeps the previous call's contents: the part a call uses is
+ * cleared on `stream` first.  Two calls whose work overlaps on the GPU (different streams, or threads) RACE on it --
+ * order them.  The first call on each device looks the array's device address up (cudaGetSymbolAddress) and sets the
+ * kernel's shared-memory attribute: make it outside stream capture.  The caller owns all buffers. */
+#define PCCL_STATIC_SCRATCH_BYTES (4u << 20)
+int pccl_candidate_totals_static(const uint64_t* have, const uint64_t* wants, uint32_t n_npus, uint32_t n_links,
+                                 uint32_t words_per_row, const uint32_t* link_src, const uint32_t* in_off,
+                                 const uint32_t* in_link, uint32_t* totals, void* stream);
 
 #ifdef __cplusplus
 }

@@ -27,7 +27,8 @@ TRANSFER_DT = np.dtype([("chunk", "<u4"), ("src", "<u4"), ("dst", "<u4"), ("link
                         ("t_start_ps", "<u8"), ("t_end_ps", "<u8")])
 
 PCCL_OK, PCCL_ERR_INVALID, PCCL_ERR_UNSUPPORTED, PCCL_ERR_UNREACHABLE = 0, -1, -2, -3
-PCCL_ERR_CUDA, PCCL_ERR_NOMEM, PCCL_ERR_INTERNAL = -4, -5, -6
+PCCL_ERR_CUDA, PCCL_ERR_NOMEM, PCCL_ERR_INTERNAL, PCCL_ERR_TOO_LARGE = -4, -5, -6, -7
+PCCL_STATIC_SCRATCH_BYTES = 4 << 20
 PCCL_FLAG_KEEP_ON_DEVICE, PCCL_FLAG_NO_IDLE_SKIP, PCCL_FLAG_TIME_LOOP, PCCL_FLAG_TRACE = 1, 2, 4, 8
 PCCL_FLAG_DENSE_SWEEP = 16
 PCCL_FLAG_RESCAN = 32
@@ -97,6 +98,7 @@ SIGNATURES = {
     "pccl_device_wants": (_i64, [_vp, _u32, _u64, _vp, _u64]),
     "pccl_device_candidate_sweep": (_int, [_vp, _u32, _u64, _u32, _u32, C.POINTER(C.c_float), C.POINTER(_u64), _vp]),
     "pccl_device_read_bandwidth": (_int, [_u64, _u32, C.POINTER(C.c_float)]),
+    "pccl_candidate_totals_static": (_int, [_vp, _vp, _u32, _u32, _u32, _vp, _vp, _vp, _vp, _vp]),
 }
 
 
@@ -351,6 +353,17 @@ def read_bandwidth_gbs(nbytes: int, iters: int = 20) -> float:
     ms = C.c_float()
     _check(lib.pccl_device_read_bandwidth(nbytes, iters, C.byref(ms)))
     return nbytes / (ms.value * 1e-3) / 1e9
+
+
+def candidate_totals_static(have, wants, n_npus: int, n_links: int, words_per_row: int, link_src, in_off, in_link,
+                            totals, stream: int = 0) -> None:
+    """``pccl_candidate_totals_static``: |have[src_l] & wants[dst_l]| of every link into ``totals``, with no allocation
+    (fixed scratch of PCCL_STATIC_SCRATCH_BYTES in the library).  Every array is a DEVICE buffer: an object with
+    ``data_ptr()`` (a torch CUDA tensor) or a raw address.  Enqueues on ``stream`` (a cudaStream_t as int) and returns."""
+    def dp(x):
+        return C.c_void_p(int(x.data_ptr()) if hasattr(x, "data_ptr") else int(x))
+    _check(lib.pccl_candidate_totals_static(dp(have), dp(wants), n_npus, n_links, words_per_row, dp(link_src), dp(in_off),
+                                            dp(in_link), dp(totals), C.c_void_p(int(stream) or None)))
 
 
 def device_philox(ctr, key) -> np.ndarray:

@@ -355,6 +355,7 @@ extern "C" const char* pccl_strerror(int err) {
         case PCCL_ERR_CUDA: return "CUDA failure (no device, launch or copy error)";
         case PCCL_ERR_NOMEM: return "out of memory";
         case PCCL_ERR_INTERNAL: return "internal invariant violated";
+        case PCCL_ERR_TOO_LARGE: return "problem exceeds the fixed scratch of the no-allocation entry point (PCCL_STATIC_SCRATCH_BYTES)";
         default: return "unknown error";
     }
 }
@@ -2233,5 +2234,102 @@ extern "C" int pccl_device_read_bandwidth(uint64_t bytes, uint32_t iters, float*
     float ms = 0.f;
     CU(cudaEventElapsedTime(&ms, e0, e1));
     *ms_per_pass = ms / (float)iters;
+    return PCCL_OK;
+}
+
+// -----------------------------------------------------------------------------------------
+// The entry point that allocates nothing (include/pccl.h: pccl_candidate_totals_static).
+//
+// Row a5 on the caller's bitmaps by k_count_sweep<true>, its scratch in a fixed array of the device image instead of
+// the per-call workspace.  Layout of the part a call uses:  [n_links][S] u32 segment counts (gcnt), then [n_links] u32
+// whole-row sums (gtot); the totals handed to the caller are summed from the segment counts by k_static_totals, so
+// the result goes THROUGH the array.  In host code `g_static_scratch` is only a stand-in for the symbol: the device
+// address comes from cudaGetSymbolAddress, once per device, with that device current.
+// -----------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_static_scratch[PCCL_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+// totals[l] = sum over segments of gcnt[l][s]; one warp per link
+__global__ void __launch_bounds__(256) k_static_totals(const uint32_t* __restrict__ gcnt, const uint32_t* __restrict__ gtot,
+                                                       uint32_t L, uint32_t S, uint32_t* __restrict__ totals) {
+    const uint32_t l = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (l >= L) return;
+    uint32_t t = 0;
+    for (uint32_t s = lane; s < S; s += 32) t += gcnt[(size_t)l * S + s];
+    t = __reduce_add_sync(0xFFFFFFFFu, t);
+    // (the whole-row sum is the kernel's own second tally of the same row: a mismatch marks the total as invalid)
+    if (lane == 0) totals[l] = (t == gtot[l]) ? t : 0xFFFFFFFFu;
+}
+
+constexpr int STATIC_MAX_DEV = 64;
+struct StaticDev {
+    bool ready = false;
+    unsigned char* scratch = nullptr;   // device address of g_static_scratch on this device
+    uint32_t resident = 0;              // CTAs of k_count_sweep<true> the device holds at once
+};
+StaticDev g_static_dev[STATIC_MAX_DEV];
+std::mutex g_static_mu;
+
+// once per device, with that device current: the array's device address, the kernel's shared-memory attribute, the
+// resident grid.  None of these allocates.
+int static_setup(const StaticDev** out) {
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEV) return PCCL_ERR_INVALID;
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    StaticDev& d = g_static_dev[dev];
+    if (!d.ready) {
+        void* p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p) return PCCL_ERR_CUDA;
+        const void* kern = (const void*)k_count_sweep<true>;
+        const size_t smem = (size_t)SW_STAGES * SW_ROWS * SW_SLICE_U4 * 16;
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int occ = 0, sms = 0;
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, SW_THREADS, smem));
+        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        if (occ < 1 || sms < 1) return PCCL_ERR_CUDA;
+        d.scratch = (unsigned char*)p;
+        d.resident = (uint32_t)occ * (uint32_t)sms;
+        d.ready = true;
+    }
+    *out = &d;
+    return PCCL_OK;
+}
+
+}  // namespace
+
+extern "C" int pccl_candidate_totals_static(const uint64_t* have, const uint64_t* wants, uint32_t n_npus, uint32_t n_links,
+                                            uint32_t words_per_row, const uint32_t* link_src, const uint32_t* in_off,
+                                            const uint32_t* in_link, uint32_t* totals, void* stream) {
+    if (n_npus == 0 || n_links == 0) return PCCL_OK;
+    if (!have || !wants || !link_src || !in_off || !in_link || !totals) return PCCL_ERR_INVALID;
+    if (words_per_row == 0 || (words_per_row & 1u)) return PCCL_ERR_INVALID;
+    if ((((uintptr_t)have) | ((uintptr_t)wants)) & 15u) return PCCL_ERR_INVALID;
+    const uint32_t S = (words_per_row / 2 + SEG_U4 - 1) / SEG_U4;
+    const uint64_t need = (uint64_t)n_links * ((uint64_t)S + 1) * 4;
+    if (need > (uint64_t)PCCL_STATIC_SCRATCH_BYTES) return PCCL_ERR_TOO_LARGE;
+    const StaticDev* d = nullptr;
+    int rc = static_setup(&d);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    uint32_t* gcnt = reinterpret_cast<uint32_t*>(d->scratch);
+    uint32_t* gtot = gcnt + (size_t)n_links * S;
+    // the array keeps the last call's contents: what this call uses starts at zero
+    CU(cudaMemsetAsync(d->scratch, 0, (size_t)need, st));
+    LoopArgs a;
+    memset(&a, 0, sizeof(a));
+    a.N = n_npus; a.L = n_links; a.Wp = words_per_row; a.S = S;
+    a.esrc = link_src; a.in_off = in_off; a.in_link = in_link;
+    a.have = const_cast<uint64_t*>(have); a.wants = const_cast<uint64_t*>(wants);
+    a.gcnt = gcnt; a.gtot = gtot;
+    a.flags = 1;                                               // (rows whole: the sweep kernel reads its parts count here)
+    const size_t smem = (size_t)SW_STAGES * SW_ROWS * SW_SLICE_U4 * 16;
+    const uint32_t grid = std::min<uint32_t>(n_npus, d->resident);
+    k_count_sweep<true><<<grid, SW_THREADS, smem, counted(st)>>>(a);
+    CU(cudaGetLastError());
+    k_static_totals<<<(n_links + 7) / 8, 256, 0, counted(st)>>>(gcnt, gtot, n_links, S, totals);
+    CU(cudaGetLastError());
     return PCCL_OK;
 }

@@ -206,3 +206,22 @@ def test_flag_constants_match_the_header(pk):
     for name, val in flags.items():
         assert getattr(pk, name) == int(val), name
     assert int(re.search(r"#define PCCL_TRACE_SLOTS (\d+)", src).group(1)) == pk.PCCL_TRACE_SLOTS
+
+
+def test_static_entry_point_checks_its_arguments_before_touching_the_device(pk):
+    """pccl_candidate_totals_static (the entry point that allocates nothing): argument and size checks come first, so
+    they can be exercised without a GPU; with valid arguments and no device the call fails loudly."""
+    import torch
+    fake = 0x1000                                                # non-null, 16-byte aligned; never dereferenced here
+    call = lambda **k: pk.pccl_candidate_totals_static(k.get("have", fake), fake, k.get("n", 4), k.get("links", 4),  # noqa: E731
+                                                       k.get("words", 2), fake, fake, fake, k.get("totals", fake), None)
+    assert call(n=0) == pk.PCCL_OK and call(links=0) == pk.PCCL_OK
+    assert call(totals=None) == pk.PCCL_ERR_INVALID and call(words=3) == pk.PCCL_ERR_INVALID
+    assert call(words=0) == pk.PCCL_ERR_INVALID and call(have=fake + 8) == pk.PCCL_ERR_INVALID
+    src = open(os.path.join(ROOT, "include", "pccl.h")).read()
+    assert int(re.search(r"#define PCCL_STATIC_SCRATCH_BYTES \((\d+)u << (\d+)\)", src).group(1)) << 20 == pk.PCCL_STATIC_SCRATCH_BYTES
+    per_link = 8                                                 # 2 words per row: one segment count + one row sum
+    assert call(links=pk.PCCL_STATIC_SCRATCH_BYTES // per_link + 1) == pk.PCCL_ERR_TOO_LARGE
+    assert b"PCCL_STATIC_SCRATCH_BYTES" in pk.pccl_strerror(pk.PCCL_ERR_TOO_LARGE)
+    if not torch.cuda.is_available():
+        assert call() == pk.PCCL_ERR_CUDA
