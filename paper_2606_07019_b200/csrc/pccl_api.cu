@@ -15,6 +15,13 @@
 #include <mutex>
 #include <new>
 #include <atomic>
+#if defined(__x86_64__)
+#include <immintrin.h>
+#endif
+#include <chrono>
+#include <condition_variable>
+#include <functional>
+#include <thread>
 #include <unordered_set>
 #include <vector>
 
@@ -55,6 +62,9 @@ struct Globals {
     // polling host thread watches
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t loop_done = nullptr;
+    // the barrier-free loop's emitter runs in windows on a stream of its own while the loop is going
+    cudaStream_t emit_stream = nullptr;
+    cudaEvent_t win_done = nullptr, pre_loop = nullptr;
     std::atomic<uint64_t> launches{0};   // kernels launched by the library (pccl_launch_count)
     // process-wide options (pccl_set_option); 0 = default
     std::atomic<uint64_t> opt_bfs_window{0}, opt_bfs_rows{0}, opt_dyn_records{0};
@@ -109,18 +119,25 @@ int ensure_device() {
     CU(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
     if (!coop) return PCCL_ERR_CUDA;
     void* mb = nullptr;
-    cudaStream_t cs = nullptr;
-    cudaEvent_t ev = nullptr;
+    cudaStream_t cs = nullptr, es = nullptr;
+    cudaEvent_t ev = nullptr, ev2 = nullptr, ev3 = nullptr;
     if (cudaHostAlloc(&mb, 4096, cudaHostAllocDefault) != cudaSuccess ||
         cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess ||
-        cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) {
+        cudaStreamCreateWithFlags(&es, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ev2, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ev3, cudaEventDisableTiming) != cudaSuccess) {
         (void)cudaGetLastError();
+        if (ev3) (void)cudaEventDestroy(ev3);
+        if (ev2) (void)cudaEventDestroy(ev2);
         if (ev) (void)cudaEventDestroy(ev);
+        if (es) (void)cudaStreamDestroy(es);
         if (cs) (void)cudaStreamDestroy(cs);
         if (mb) (void)cudaFreeHost(mb);
         return PCCL_ERR_CUDA;
     }
     G.mailbox = mb; G.copy_stream = cs; G.loop_done = ev;
+    G.emit_stream = es; G.win_done = ev2; G.pre_loop = ev3;
     G.sm_count = sms;
     G.dev = dev;
     return PCCL_OK;
@@ -573,9 +590,95 @@ void finish_phase(Phase& ph, uint32_t N) {
     index_phase(ph, N, is_src, is_dst);
 }
 
-// The common large case in one streaming pass over the caller's arrays: both pair lists already ordered by chunk,
-// exactly one pre-holder per chunk (COPY mode), post-holders of a chunk strictly ascending.  Returns false on ANY
-// deviation (including invalid input) without touching P: the general path below then decides, errors included.
+// A few host threads kept for the life of the process (the normaliser's passes over millions of pairs): run(n, f) calls
+// f(0) on the caller and f(1) .. f(n-1) on the workers and returns when all are done.  Workers are created on first
+// use; if none can be created everything runs on the caller.
+class HostPool2 {
+    std::vector<std::thread> th_;
+    std::mutex mu_;
+    std::condition_variable cv_, done_;
+    const std::function<void(int)>* job_ = nullptr;
+    int want_ = 0, left_ = 0;
+    uint64_t gen_ = 0;
+    bool stop_ = false;
+    void worker(int id) {
+        uint64_t seen = 0;
+        for (;;) {
+            const std::function<void(int)>* f = nullptr;
+            {
+                std::unique_lock<std::mutex> lk(mu_);
+                cv_.wait(lk, [&] { return stop_ || (gen_ != seen && id < want_); });
+                if (stop_) return;
+                seen = gen_;
+                f = job_;
+            }
+            (*f)(id);
+            {
+                std::lock_guard<std::mutex> lk(mu_);
+                if (--left_ == 0) done_.notify_one();
+            }
+        }
+    }
+public:
+    static constexpr int MAX_THREADS = 8;
+    int capacity() {
+        std::lock_guard<std::mutex> lk(mu_);
+        if (th_.empty()) {
+            const int hw = (int)std::thread::hardware_concurrency();
+            const int n = std::max(1, std::min(MAX_THREADS, hw / 2));
+            try {
+                for (int i = 1; i < n; ++i) th_.emplace_back([this, i] { worker(i); });
+            } catch (const std::system_error&) {
+            }
+        }
+        return (int)th_.size() + 1;
+    }
+    void run(int n, const std::function<void(int)>& f) {
+        n = std::min(n, capacity());
+        if (n > 1) {
+            std::lock_guard<std::mutex> lk(mu_);
+            job_ = &f; want_ = n; left_ = n - 1; ++gen_;
+        }
+        if (n > 1) cv_.notify_all();
+        f(0);
+        if (n > 1) {
+            std::unique_lock<std::mutex> lk(mu_);
+            done_.wait(lk, [&] { return left_ == 0; });
+            want_ = 0;
+        }
+    }
+    ~HostPool2() {
+        {
+            std::lock_guard<std::mutex> lk(mu_);
+            stop_ = true;
+        }
+        cv_.notify_all();
+        for (auto& t : th_) t.join();
+    }
+};
+HostPool2 g_threads;
+std::mutex g_threads_mu;   // one parallel region at a time
+
+// stores that bypass the caches (x86-64: movnti), for arrays written once, front to back, and read next by DMA
+#if defined(__x86_64__)
+inline void nt_store32(uint32_t* p, uint32_t v) { _mm_stream_si32((int*)p, (int)v); }
+inline void nt_store64(uint64_t* p, uint64_t v) { _mm_stream_si64((long long*)p, (long long)v); }
+inline void nt_fence() { _mm_sfence(); }
+inline void cpu_relax() { _mm_pause(); }
+#else
+inline void cpu_relax() { std::this_thread::yield(); }
+inline void nt_store32(uint32_t* p, uint32_t v) { *p = v; }
+inline void nt_store64(uint64_t* p, uint64_t v) { *p = v; }
+inline void nt_fence() {}
+#endif
+
+// The common large case straight from the caller's arrays: both pair lists already ordered by chunk, exactly one
+// pre-holder per chunk (COPY mode), post-holders of a chunk strictly ascending.  Returns false on ANY deviation
+// (including invalid input) without touching P: the general path below then decides, errors included.
+// Two passes over slices of the chunk range, one slice per host thread: count and validate, then write at the offsets
+// the counts give.  A slice starts at the first post pair whose chunk is >= its first chunk (binary search, right if
+// the list is ordered) and must end exactly where the next slice starts -- together with the pair-by-pair check inside
+// a slice that proves the order the search assumed.
 bool normalise_ordered_copy(const pccl_condition_t* pre, const pccl_condition_t* post, uint32_t C, uint32_t N,
                             const std::vector<char>& member, Phase& cp) {
     if (pre->n_pairs != C || post->n_pairs < C) return false;
@@ -583,45 +686,131 @@ bool normalise_ordered_copy(const pccl_condition_t* pre, const pccl_condition_t*
     const pccl_pair_t* __restrict__ qp = post->pairs;
     const uint64_t nq = post->n_pairs;
     const char* mem = member.data();
-    cp.cond_src.resize(C);
-    cp.dest_off.resize((size_t)C + 1);
-    cp.dests.resize(nq);
-    cp.dchunk.resize(nq);
-    uint32_t* __restrict__ o_src = cp.cond_src.data();
-    uint64_t* __restrict__ o_off = cp.dest_off.data();
-    uint32_t* __restrict__ o_dst = cp.dests.data();
-    uint32_t* __restrict__ o_chk = cp.dchunk.data();
-    std::vector<uint32_t> f_src(N, 0), f_dst(N, 0);
-    o_off[0] = 0;
-    uint64_t k = 0, nd = 0;
-    for (uint32_t c = 0; c < C; ++c) {
-        const pccl_pair_t a = pp[c];
-        if (a.chunk != c || a.npu >= N || !mem[a.npu]) return false;
-        const uint32_t src = a.npu;
-        if (k >= nq || qp[k].chunk != c) return false;   // no post-holder, or not ordered
-        const uint64_t first = nd;
-        uint32_t prev = 0;
-        bool have_prev = false;
-        while (k < nq && qp[k].chunk == c) {
-            const uint32_t d = qp[k].npu;
-            if (d >= N || !mem[d] || (have_prev && d <= prev)) return false;
-            prev = d;
-            have_prev = true;
-            ++k;
-            if (d == src) continue;
-            o_dst[nd] = d;
-            o_chk[nd] = c;
-            f_dst[d] = 1;
-            ++nd;
-        }
-        o_src[c] = src;
-        o_off[c + 1] = nd;
-        if (nd > first) f_src[src] = 1;
+    std::unique_lock<std::mutex> region(g_threads_mu, std::defer_lock);
+    int T = 1;
+    if (nq >= (1u << 15)) {
+        region.lock();
+        T = std::min<int>(g_threads.capacity(), (int)std::min<uint64_t>(HostPool2::MAX_THREADS, nq >> 14));
     }
-    if (k != nq) return false;   // pairs of a chunk id >= C, or out of order
-    cp.dests.resize(nd);
-    cp.dchunk.resize(nd);
-    index_phase(cp, N, std::vector<char>(f_src.begin(), f_src.end()), std::vector<char>(f_dst.begin(), f_dst.end()));
+    struct Slice {
+        uint32_t c_lo, c_hi;
+        uint64_t k_lo, k_end, nd;
+        bool ok;
+        std::vector<uint32_t> f_src, f_dst;
+    };
+    std::vector<Slice> sl((size_t)T);
+    for (int t = 0; t < T; ++t) {
+        sl[t].c_lo = (uint32_t)((uint64_t)C * t / T);
+        sl[t].c_hi = (uint32_t)((uint64_t)C * (t + 1) / T);
+        sl[t].f_src.assign(N, 0);
+        sl[t].f_dst.assign(N, 0);
+    }
+    // pass 1: validate, count the destinations (post-holders other than the source), mark sources and destinations
+    const std::function<void(int)> pass1 = [&](int t) {
+        Slice& s = sl[t];
+        s.ok = false;
+        uint64_t lo = 0, hi = nq;                                  // first pair with chunk >= c_lo
+        while (lo < hi) {
+            const uint64_t mid = (lo + hi) >> 1;
+            if (qp[mid].chunk < s.c_lo) lo = mid + 1; else hi = mid;
+        }
+        s.k_lo = lo;
+        uint64_t k = lo, nd = 0;
+        uint32_t* f_src = s.f_src.data();
+        uint32_t* f_dst = s.f_dst.data();
+        for (uint32_t c = s.c_lo; c < s.c_hi; ++c) {
+            const pccl_pair_t a = pp[c];
+            if (a.chunk != c || a.npu >= N || !mem[a.npu]) return;
+            const uint32_t src = a.npu;
+            if (k >= nq || qp[k].chunk != c) return;               // no post-holder, or not ordered
+            const uint64_t first = nd;
+            uint32_t prev = 0;
+            bool have_prev = false;
+            while (k < nq && qp[k].chunk == c) {
+                const uint32_t d = qp[k].npu;
+                if (d >= N || !mem[d] || (have_prev && d <= prev)) return;
+                prev = d;
+                have_prev = true;
+                ++k;
+                if (d == src) continue;
+                f_dst[d] = 1;
+                ++nd;
+            }
+            if (nd > first) f_src[src] = 1;
+        }
+        s.k_end = k;
+        s.nd = nd;
+        s.ok = true;
+    };
+    // between the passes, thread 0 checks that the slices tile the list, sizes the arrays and hands out the offsets;
+    // the other threads (awake anyway) spin for those few microseconds instead of going back to sleep
+    uint32_t* o_src = nullptr;
+    uint64_t* o_off = nullptr;
+    uint32_t* o_dst = nullptr;
+    uint32_t* o_chk = nullptr;
+    std::vector<uint64_t> nd_base((size_t)T, 0);
+    std::atomic<int> arrived{0}, go{0};                          // go: 1 write, 2 give up (not the ordered form), 3 out of memory
+    auto between = [&]() -> int {
+        uint64_t nd_total = 0;
+        for (int t = 0; t < T; ++t) {
+            if (!sl[t].ok) return 2;
+            if (sl[t].k_lo != (t == 0 ? 0 : sl[t - 1].k_end)) return 2;   // the slices tile the list
+            nd_total += sl[t].nd;
+        }
+        if (sl[T - 1].k_end != nq) return 2;                     // pairs of a chunk id >= C, or out of order
+        try {
+            cp.cond_src.resize(C);
+            cp.dest_off.resize((size_t)C + 1);
+            cp.dests.resize(nd_total);
+            cp.dchunk.resize(nd_total);
+        } catch (const std::bad_alloc&) {
+            return 3;
+        }
+        o_src = cp.cond_src.data(); o_off = cp.dest_off.data(); o_dst = cp.dests.data(); o_chk = cp.dchunk.data();
+        o_off[0] = 0;
+        for (int t = 1; t < T; ++t) nd_base[t] = nd_base[t - 1] + sl[t - 1].nd;
+        return 1;
+    };
+    // pass 2: write (everything was validated).  The four arrays go to the device next, by DMA from these very
+    // (page-locked) blocks: non-temporal stores put them in memory instead of leaving dirty lines in the caches of
+    // whichever cores the slices ran on (measured on the B200 host: DMA of lines that sit modified in other cores'
+    // caches ran at 7 GB/s instead of 55).
+    const std::function<void(int)> pass2 = [&](int t) {
+        const Slice& s = sl[t];
+        uint64_t k = s.k_lo, nd = nd_base[t];
+        for (uint32_t c = s.c_lo; c < s.c_hi; ++c) {
+            const uint32_t src = pp[c].npu;
+            while (k < nq && qp[k].chunk == c) {
+                const uint32_t d = qp[k].npu;
+                ++k;
+                if (d == src) continue;
+                nt_store32(o_dst + nd, d);
+                nt_store32(o_chk + nd, c);
+                ++nd;
+            }
+            nt_store32(o_src + c, src);
+            nt_store64(o_off + c + 1, nd);
+        }
+        nt_fence();
+    };
+    const std::function<void(int)> both = [&](int t) {
+        pass1(t);
+        arrived.fetch_add(1, std::memory_order_acq_rel);
+        if (t == 0) {
+            while (arrived.load(std::memory_order_acquire) < T) cpu_relax();
+            go.store(between(), std::memory_order_release);
+        } else {
+            while (go.load(std::memory_order_acquire) == 0) cpu_relax();
+        }
+        if (go.load(std::memory_order_acquire) == 1) pass2(t);
+    };
+    g_threads.run(T, both);
+    if (go.load() == 3) throw std::bad_alloc();
+    if (go.load() != 1) return false;
+    std::vector<char> f_src(N, 0), f_dst(N, 0);
+    for (int t = 0; t < T; ++t)
+        for (uint32_t v = 0; v < N; ++v) { f_src[v] |= (char)sl[t].f_src[v]; f_dst[v] |= (char)sl[t].f_dst[v]; }
+    index_phase(cp, N, f_src, f_dst);
     return true;
 }
 
@@ -767,7 +956,7 @@ int normalise(const pccl_topology* topo, const uint32_t* group, uint32_t n_membe
     return PCCL_OK;
 }
 
-int phase_upload(Phase& ph, uint32_t N) {
+int phase_upload(Phase& ph, uint32_t N, bool sync = true) {
     if (ph.blob) return PCCL_OK;
     const size_t C = ph.cond_src.size(), ND = ph.dests.size(), NS = ph.sources.size();
     Carver c;
@@ -794,7 +983,8 @@ int phase_upload(Phase& ph, uint32_t N) {
     up(o_si, ph.sidx.data(), (size_t)N * 4);
     up(o_or, ph.orig.data(), ph.orig.size() * 4);
     up(o_cl, ph.cls.data(), ph.cls.size() * 4);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(G.stream);
+    // (sync == false: the caller's next work is on the same stream and it synchronises before the arrays can go away)
+    if (e == cudaSuccess && sync) e = cudaStreamSynchronize(G.stream);
     if (e != cudaSuccess) {
         (void)cudaGetLastError();
         (void)cudaStreamSynchronize(G.stream);
@@ -840,20 +1030,23 @@ extern "C" void pccl_problem_destroy(pccl_problem_t* P) {
     delete P;
 }
 
-extern "C" int pccl_problem_upload(pccl_problem_t* P) {
+// sync == false: the copies are only enqueued (from the problem's own page-locked arrays); the caller goes on working
+// on the same stream and synchronises it before it returns
+static int problem_upload(pccl_problem_t* P, bool sync) {
     SERIALISE;
     if (!P) return PCCL_ERR_INVALID;
     if (P->uploaded) return PCCL_OK;
     int rc = topo_upload(const_cast<pccl_topology*>(P->topo));
     if (rc) return rc;
     try {
-        for (Phase& ph : P->phases) { rc = phase_upload(ph, P->topo->N); if (rc) return rc; }
+        for (Phase& ph : P->phases) { rc = phase_upload(ph, P->topo->N, sync); if (rc) return rc; }
     } catch (const std::bad_alloc&) {
         return PCCL_ERR_NOMEM;
     }
     P->uploaded = true;
     return PCCL_OK;
 }
+extern "C" int pccl_problem_upload(pccl_problem_t* P) { return problem_upload(P, true); }
 
 extern "C" int pccl_problem_mode(const pccl_problem_t* P) { return P ? P->mode : PCCL_ERR_INVALID; }
 extern "C" uint32_t pccl_problem_n_chunks(const pccl_problem_t* P) { return P ? P->C : 0; }
@@ -1121,8 +1314,11 @@ int reverse_sorted(Rec* raw, uint64_t M, uint64_t T, uint32_t L, Rec* out, bool 
 // steps D..E without a grid barrier (pccl_loop2.cuh): setup of the per-destination entry lists and translation
 // tables, the loop, and the ranking of the logged claims into canonical order.  `raw_only`: leave the records in log
 // order (a transposed phase sorts them after the reversal anyway).
+// host_out (optional, pinned, out_cap records): the emitter's windows run on a second stream while the loop is going
+// and this thread copies the finished prefix of the records there meanwhile; *streamed says whether all of them went.
 int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t seed, uint32_t flags, Rec* out,
-                     uint64_t out_cap, uint64_t t_offset, bool raw_only, LoopResult* res, Timers* tm) {
+                     uint64_t out_cap, uint64_t t_offset, bool raw_only, LoopResult* res, Timers* tm,
+                     Rec* host_out = nullptr, bool* streamed = nullptr) {
     const pccl_topology* t = P.topo;
     const PhaseView pv = view_of(t, ph.transposed);
     const uint32_t N = t->N, L = t->L;
@@ -1149,6 +1345,7 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     const size_t o_log = c.take(M * 16), o_tk = c.take((size_t)a.tcap * 8);
     const size_t o_zero = c.cur;                                 // cleared
     const size_t o_tc = c.take((size_t)a.tcap * 4), o_tf = c.take((size_t)a.tcap * 4), o_bm = c.take((size_t)a.ecap * W.nLw * 8);
+    const size_t o_wc = c.take((size_t)N * 4), o_wn = c.take((size_t)N * 4), o_win = c.take(sizeof(A2Win));
     void* blob = nullptr;
     int rc = dev_alloc(c.cur, &blob);
     if (rc) return rc;
@@ -1160,6 +1357,8 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     a.wbase = (uint32_t*)(b + o_wb); a.trank = (uint32_t*)(b + o_tr); a.log = (U128*)(b + o_log);
     a.tkey = (unsigned long long*)(b + o_tk); a.tcnt = (uint32_t*)(b + o_tc); a.tflag = (uint32_t*)(b + o_tf);
     a.bm = (unsigned long long*)(b + o_bm);
+    a.wcur = (uint32_t*)(b + o_wc); a.wnext = (uint32_t*)(b + o_wn); a.win = (A2Win*)(b + o_win);
+    a.progress = nullptr;
     CU(cudaMemsetAsync(b + o_ff, 0xFF, o_zero - o_ff, st));
     CU(cudaMemsetAsync(b + o_zero, 0, c.cur - o_zero, st));
     // entries, translation tables, private images (once per phase)
@@ -1175,21 +1374,88 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kloop2, threads, smem));
     if (occ < 1 || (uint64_t)occ * (uint64_t)G.sm_count < W.a2_grid) return PCCL_ERR_INTERNAL;   // (checked by the caller's plan)
     void* args[] = {(void*)&a};
+    // one window of the emitter (pccl_loop2.cuh): the claims that start before the global virtual time -- or all that
+    // are left (final) -- ranked and written behind the records of the earlier windows
+    auto window = [&](cudaStream_t s, int final) -> cudaError_t {
+        k_win_begin<<<1, 1024, 0, counted(s)>>>(a, final);
+        k_win_times<<<N, 256, 0, counted(s)>>>(a);
+        if (!raw_only) {
+            k_win_rank<<<(a.ecap + 255) / 256, 256, 0, counted(s)>>>(a);
+            k_win_base<<<1, 1024, 0, counted(s)>>>(a);
+            k_win_bits<<<N, 256, 0, counted(s)>>>(a);
+            k_win_wbase<<<std::min<uint32_t>((a.ecap + 7) / 8, 256u), 256, 0, counted(s)>>>(a);
+            k_win_write<<<N, 256, 0, counted(s)>>>(a);
+            k_win_end<<<1, 1, 0, counted(s)>>>(a);
+        } else {
+            k_emit_raw<<<N, 256, 0, counted(s)>>>(a);
+        }
+        return cudaGetLastError();
+    };
+    // streaming: the progress word lives in the pinned mailbox (mapped: k_win_end stores to it directly)
+    volatile unsigned long long* progress = (volatile unsigned long long*)((unsigned char*)G.mailbox + 2048);
+    const bool stream_out = host_out != nullptr && !raw_only && out_cap > 0;
+    uint64_t copied = 0;
+    struct Drain {   // whatever happens, nothing of this call is left running on the side streams
+        bool on;
+        ~Drain() {
+            if (!on) return;
+            (void)cudaStreamSynchronize(G.emit_stream);
+            (void)cudaStreamSynchronize(G.copy_stream);
+            (void)cudaGetLastError();
+        }
+    } drain{stream_out};
+    if (stream_out) {
+        *progress = 0;
+        void* dp = nullptr;
+        CU(cudaHostGetDevicePointer(&dp, (void*)progress, 0));
+        a.progress = (unsigned long long*)dp;
+        CU(cudaEventRecord(G.pre_loop, st));                      // headers, logs and tables are initialised
+        CU(cudaStreamWaitEvent(G.emit_stream, G.pre_loop, 0));
+    }
     if (tm) { tm->setup.stop(); tm->loop.start(); }
     CU(cudaLaunchCooperativeKernel(kloop2, dim3(W.a2_grid), dim3(threads), args, smem, counted(st)));
-    if (tm) { tm->loop.stop(); tm->emit.start(); }
-    // emit
-    k_emit_times<<<N, 256, 0, counted(st)>>>(a);
-    if (!raw_only) {
-        k_emit_rank<<<(a.ecap + 255) / 256, 256, 0, counted(st)>>>(a);
-        k_emit_base<<<1, 1024, 0, counted(st)>>>(a);
-        k_emit_bits<<<N, 256, 0, counted(st)>>>(a);
-        k_emit_wbase<<<(a.ecap + 7) / 8, 256, 0, counted(st)>>>(a);
-        k_emit_write<<<N, 256, 0, counted(st)>>>(a);
-    } else {
-        k_emit_raw<<<N, 256, 0, counted(st)>>>(a);
+    if (tm) tm->loop.stop();
+    if (stream_out) {
+        // windows on the emit stream while the loop runs (it never waits for them; they read headers and logs only);
+        // finished records leave in pieces of >= 2 MB on the copy stream.  Both streams are drained before anything
+        // can fail or return.
+        constexpr uint64_t PIECE = 1u << 16;
+        bool in_flight = false, any = false;
+        cudaError_t e = cudaEventRecord(G.loop_done, st), q = cudaErrorNotReady;
+        while (e == cudaSuccess && (q = cudaEventQuery(G.loop_done)) == cudaErrorNotReady) {
+            if (in_flight && cudaEventQuery(G.win_done) != cudaErrorNotReady) in_flight = false;
+            if (in_flight) continue;
+            const uint64_t p = std::min<uint64_t>(*progress, out_cap);
+            if (p >= copied + PIECE) {
+                e = cudaMemcpyAsync(host_out + copied, out + copied, (p - copied) * sizeof(Rec), cudaMemcpyDeviceToHost,
+                                    G.copy_stream);
+                copied = p;
+            }
+            if (e == cudaSuccess) e = window(G.emit_stream, 0);
+            if (e == cudaSuccess) e = cudaEventRecord(G.win_done, G.emit_stream);
+            in_flight = any = true;
+        }
+        if (e == cudaSuccess && q != cudaSuccess) e = q;
+        if (e == cudaSuccess && any) e = cudaStreamWaitEvent(st, G.win_done, 0);   // the last window before the final one
+        if (e != cudaSuccess) {
+            (void)cudaGetLastError();
+            (void)cudaStreamSynchronize(G.emit_stream);
+            (void)cudaStreamSynchronize(G.copy_stream);
+            (void)cudaStreamSynchronize(st);
+            (void)cudaGetLastError();
+            return PCCL_ERR_CUDA;
+        }
     }
-    CU(cudaGetLastError());
+    if (tm) tm->emit.start();
+    {
+        const cudaError_t e = window(st, 1);
+        if (e != cudaSuccess) {
+            (void)cudaStreamSynchronize(G.copy_stream);
+            (void)cudaStreamSynchronize(st);
+            (void)cudaGetLastError();
+            return PCCL_ERR_CUDA;
+        }
+    }
     if (tm) tm->emit.stop();
     LoopCtrl* mb = (LoopCtrl*)G.mailbox;
     A2Ctrl* mb2 = (A2Ctrl*)((unsigned char*)G.mailbox + 1024);
@@ -1221,6 +1487,13 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
         if (rc) return rc;
         if (e != cudaSuccess) { (void)cudaGetLastError(); return PCCL_ERR_CUDA; }
     }
+    if (stream_out && !(mb2->err & 1u) && mb2->total <= out_cap) {   // the tail (after a fall-back sort nothing was streamed)
+        if (mb2->total > copied)
+            CU(cudaMemcpyAsync(host_out + copied, out + copied, (mb2->total - copied) * sizeof(Rec), cudaMemcpyDeviceToHost,
+                               G.copy_stream));
+        CU(cudaStreamSynchronize(G.copy_stream));
+        if (streamed) *streamed = true;
+    }
     res->total = mb2->total; res->tmax = mb2->tmax;
     res->events = (uint64_t)mb2->n_end + 1;   // event times = {0} and every distinct t_end (each free time is visited)
     res->rows = mb2->actions; res->links = mb2->picks; res->slow = mb2->slow; res->bytes = mb2->bytes;
@@ -1237,7 +1510,7 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
     const bool dynamic = (flags & PCCL_FLAG_DYNAMIC_RELAY) != 0;
     if (W.a2_planned && out_cap > 0 && out_cap <= 0xFFFFFFFFull && W.a2.smem_need <= 220 * 1024 &&
         ((flags & (PCCL_FLAG_ASYNC | PCCL_FLAG_DIST_PICK)) || W.a2.w_max / 16 <= W.a2.w_min))
-        return phase_loop_async(P, ph, W, seed, flags, out, out_cap, t_offset, ph.transposed, res, tm);
+        return phase_loop_async(P, ph, W, seed, flags, out, out_cap, t_offset, ph.transposed, res, tm, host_out, streamed);
     if ((flags & PCCL_FLAG_DIST_PICK) && out_cap > 0) return PCCL_ERR_UNSUPPORTED;   // the c.dist pick lives in the barrier-free loop
     // the dynamic rule keeps the counts current too: wants bits are only dropped where a neighbour holds the chunk
     // (holder lists, dyn_shrink_wants); DENSE_SWEEP / RESCAN recount instead and drop every bit at once
@@ -1717,10 +1990,10 @@ int bfs_phase(const pccl_problem& P, const Phase& ph, uint64_t seed, uint64_t t_
 extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_t flags, pccl_schedule_t** out) {
     SERIALISE;
     if (!P || !out) return PCCL_ERR_INVALID;
-    int rc = pccl_problem_upload(P);
+    int rc = problem_upload(P, false);
     if (rc) return rc;
     pccl_schedule* S = new (std::nothrow) pccl_schedule();
-    if (!S) return PCCL_ERR_NOMEM;
+    if (!S) { if (cudaStreamSynchronize(G.stream) != cudaSuccess) (void)cudaGetLastError(); return PCCL_ERR_NOMEM; }
     memset(&S->stats, 0, sizeof(S->stats));
     S->stats.mode = (uint32_t)P->mode;
     Timers tm;

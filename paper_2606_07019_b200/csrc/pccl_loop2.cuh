@@ -32,9 +32,10 @@
 // new log entries of its sources (one L2 round trip), the table words of the arrivals (a second one), and
 // stores its own claims and header.
 //
-// The records are ranked afterwards (k_emit_*): start times are hashed into a small table, the distinct ones
-// ranked, and a per-event link bitmap gives the position  base(event) + rank(link)  -- the same canonical
-// (t_start, link) order the barrier loops emit.
+// The records are ranked after the fact (k_win_*), in windows of start times behind the global virtual time -- on a
+// second stream while the loop runs when the host is streaming them out, else in one window after it: start times
+// are hashed into a small table, the distinct ones ranked, and a per-event link bitmap gives the position
+// base(event) + rank(link)  -- the same canonical (t_start, link) order the barrier loops emit.
 // =========================================================================================
 #pragma once
 #include "pccl_device.cuh"
@@ -82,6 +83,14 @@ struct A2Ctrl {                      // read back once by the host after the pla
     uint32_t err;                    // 1 table or bitmap capacity exceeded (the host falls back to the radix sort)
     uint32_t pad;
     unsigned long long prof[8];      // -DPCCL_A2_PROFILE: SM cycles per phase, summed over the warps
+};
+
+// state of the windowed emitter (device memory, cleared before the first window)
+struct A2Win {
+    unsigned long long gvt;           // this window takes the claims that start before gvt
+    unsigned long long emitted;       // records written by the earlier windows
+    unsigned long long emitted_next;  //   ... and by this one
+    uint32_t used0, pad;              // this window's distinct start times are used[used0 .. n_start)
 };
 
 // per-destination fixed part of the warp's shared memory
@@ -148,6 +157,10 @@ struct A2Args {
     uint32_t tcap, ecap;
     Rec* out;
     uint64_t out_cap, t_offset;
+    // windows of the emitter
+    A2Win* win;
+    uint32_t *wcur, *wnext;           // [N] log entries of node v below wcur are emitted; the window ends at wnext
+    unsigned long long* progress;     // mapped host word: records that are final (null: nobody is streaming them out)
 };
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -818,7 +831,17 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// emit: rank the logged claims into canonical (t_start, link) order (a8/a9)
+// emit: rank the logged claims into canonical (t_start, link) order (a8/a9) -- in WINDOWS of start times.
+//
+// A window takes every claim that starts before a bound `gvt` and has not been emitted yet.  With gvt = the smallest
+// header time over all nodes (the simulation's global virtual time) those claims are final -- every node has logged
+// all its claims that start before its own header time -- and all of them start at or after the previous window's
+// bound, so their ranks simply continue where the previous window stopped: the windows can run on a second stream
+// WHILE k_loop2 is still going (they only read headers and logs, k_loop2 never waits for them), and the host copies
+// the finished prefix of the records out meanwhile.  A last window with gvt = inf after the loop takes the rest; a run
+// that does not stream uses that window alone.  Per window: start times are hashed into a small table, the new
+// distinct ones ranked, and a per-event link bitmap gives the position  base(event) + rank(link).
+// A node's log is in time order, so a window's claims are the log entries [wcur, wnext) of each node.
 // ---------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t a2_time_slot(const A2Args& a, unsigned long long t) {
     const uint32_t mask = a.tcap - 1;
@@ -836,16 +859,42 @@ __device__ __forceinline__ uint32_t a2_time_slot(const A2Args& a, unsigned long 
     return 0;
 }
 
-// block per node: hash every claim's start and end time; count the records per start time
-__global__ void __launch_bounds__(256) k_emit_times(A2Args a) {
+// one block: the window's bound and the first of its distinct start times
+__global__ void __launch_bounds__(1024) k_win_begin(A2Args a, int final) {
+    __shared__ unsigned long long sm[32];
+    unsigned long long g = T_INF;
+    if (!final)
+        for (uint32_t v = threadIdx.x; v < a.N; v += 1024) g = min(g, ld128(a.hdr + v).lo);
+    for (int o = 16; o; o >>= 1) g = min(g, __shfl_xor_sync(0xFFFFFFFFu, g, o));
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = g;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        g = sm[threadIdx.x];
+        for (int o = 16; o; o >>= 1) g = min(g, __shfl_xor_sync(0xFFFFFFFFu, g, o));
+        if (threadIdx.x == 0) { a.win->gvt = g; a.win->used0 = min(a.ctrl->n_start, a.ecap); }
+    }
+}
+
+// block per node: hash the start and end time of every claim of the window; count the records per start time
+__global__ void __launch_bounds__(256) k_win_times(A2Args a) {
+    __shared__ uint32_t s_n;
     const uint32_t v = blockIdx.x;
-    const U128 h = ld128(a.hdr + v);
-    const uint32_t cnt = (uint32_t)h.hi;
+    const unsigned long long gvt = a.win->gvt;
+    const uint32_t cnt = (uint32_t)ld128(a.hdr + v).hi, c0 = a.wcur[v];
     const unsigned long long base = a.nbase[v];
     const uint32_t e0 = a.in_off[v];
+    if (threadIdx.x == 0) s_n = 0;
+    __syncthreads();
     unsigned long long tmax = 0;
-    for (uint32_t i = threadIdx.x; i < cnt; i += blockDim.x) {
-        const U128 en = a.log[base + i];
+    uint32_t mine = 0;
+    for (uint32_t i = c0 + threadIdx.x; i < cnt; i += blockDim.x) {
+        U128 en = ld128(a.log + base + i);
+        for (uint32_t spins = 0; en.hi == T_INF; ++spins) {       // counted by the header, the store is on its way
+            if (spins > (1u << 22)) { atomicOr(a.abort_flag, 256u); break; }
+            en = ld128(a.log + base + i);
+        }
+        if (en.lo >= gvt) break;                                  // (log in time order: so are the later ones)
+        ++mine;
         const uint32_t l = a.in_link[e0 + ((uint32_t)(en.hi >> 32) & 7u)];
         const unsigned long long te = en.lo + a.w[l];
         tmax = max(tmax, te);
@@ -859,86 +908,95 @@ __global__ void __launch_bounds__(256) k_emit_times(A2Args a) {
         const uint32_t s2 = a2_time_slot(a, te);
         if (!(atomicOr(&a.tflag[s2], 1u) & 1u)) atomicAdd(&a.ctrl->n_end, 1u);
     }
+    if (mine) atomicAdd(&s_n, mine);
     for (int o = 16; o; o >>= 1) tmax = max(tmax, __shfl_xor_sync(0xFFFFFFFFu, tmax, o));
-    if (threadIdx.x == 0 && cnt) atomicAdd(&a.ctrl->total, (unsigned long long)cnt);
     if ((threadIdx.x & 31) == 0) {
         if (tmax) atomicMax(&a.ctrl->tmax, tmax);
         if (2u * (a.ctrl->n_start + a.ctrl->n_end) > a.tcap) atomicOr(&a.ctrl->err, 1u);   // keep the table half empty
     }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        a.wnext[v] = c0 + s_n;
+        if (s_n) atomicAdd(&a.ctrl->total, (unsigned long long)s_n);
+    }
 }
 
-// rank of every distinct start time (a thread per time, all times compared through shared-memory tiles)
-__global__ void __launch_bounds__(256) k_emit_rank(A2Args a) {
+// rank of every distinct start time of the window (a thread per time, all times compared through shared-memory tiles)
+__global__ void __launch_bounds__(256) k_win_rank(A2Args a) {
     __shared__ unsigned long long tile[256];
-    const uint32_t n = min(a.ctrl->n_start, a.ecap);
+    const uint32_t u0 = a.win->used0, n = min(a.ctrl->n_start, a.ecap) - u0;
     const uint32_t i = blockIdx.x * 256 + threadIdx.x;
     if (blockIdx.x * 256 >= n) return;
-    const uint32_t slot = i < n ? a.used[i] : 0u;
+    const uint32_t slot = i < n ? a.used[u0 + i] : 0u;
     const unsigned long long mine = i < n ? a.tkey[slot] : T_INF;
     uint32_t rank = 0;
     for (uint32_t b = 0; b < n; b += 256) {
         __syncthreads();
-        tile[threadIdx.x] = b + threadIdx.x < n ? a.tkey[a.used[b + threadIdx.x]] : T_INF;
+        tile[threadIdx.x] = b + threadIdx.x < n ? a.tkey[a.used[u0 + b + threadIdx.x]] : T_INF;
         __syncthreads();
         const uint32_t m = min(256u, n - b);
         for (uint32_t k = 0; k < m; ++k) rank += tile[k] < mine;
     }
-    if (i < n) { a.trank[slot] = rank; a.cnt_sorted[rank] = a.tcnt[slot]; }
+    if (i < n) { a.trank[slot] = u0 + rank; a.cnt_sorted[u0 + rank] = a.tcnt[slot]; }
 }
 
-// first record of every start time (one block)
-__global__ void __launch_bounds__(1024) k_emit_base(A2Args a) {
+// first record of every start time of the window (one block)
+__global__ void __launch_bounds__(1024) k_win_base(A2Args a) {
     __shared__ unsigned long long sm[33];
-    const uint32_t n = min(a.ctrl->n_start, a.ecap);
-    unsigned long long carry = 0, tot;
+    const uint32_t u0 = a.win->used0, n = min(a.ctrl->n_start, a.ecap) - u0;
+    unsigned long long carry = a.win->emitted, tot;
     for (uint32_t b = 0; b < n; b += 1024) {
         const uint32_t i = b + threadIdx.x;
-        const unsigned long long x = i < n ? a.cnt_sorted[i] : 0ull;
+        const unsigned long long x = i < n ? a.cnt_sorted[u0 + i] : 0ull;
         const unsigned long long ex = block_excl_scan_1024(x, &tot, sm);
-        if (i < n) a.ebase[i] = carry + ex;
+        if (i < n) a.ebase[u0 + i] = carry + ex;
         carry += tot;
     }
+    if (threadIdx.x == 0) a.win->emitted_next = carry;
 }
 
-// the links matched at every start time
-__global__ void __launch_bounds__(256) k_emit_bits(A2Args a) {
+// the links matched at every start time of the window
+__global__ void __launch_bounds__(256) k_win_bits(A2Args a) {
     if (a.ctrl->err & 1u) return;   // the table or the bitmaps overflowed: ranks are not valid, the host sorts instead
     const uint32_t v = blockIdx.x;
-    const uint32_t cnt = (uint32_t)ld128(a.hdr + v).hi;
+    const uint32_t c0 = a.wcur[v], c1 = a.wnext[v];
     const unsigned long long base = a.nbase[v];
     const uint32_t e0 = a.in_off[v];
-    for (uint32_t i = threadIdx.x; i < cnt; i += blockDim.x) {
-        const U128 en = a.log[base + i];
+    for (uint32_t i = c0 + threadIdx.x; i < c1; i += blockDim.x) {
+        const U128 en = ld128(a.log + base + i);
         const uint32_t l = a.in_link[e0 + ((uint32_t)(en.hi >> 32) & 7u)];
         const uint32_t r = a.trank[a.eslot[base + i]];
         atomicOr(a.bm + (size_t)r * a.nLw + (l >> 6), 1ull << (l & 63));
     }
 }
 
-// matched links before each 64-link word of every start time's row (a warp per row)
-__global__ void __launch_bounds__(256) k_emit_wbase(A2Args a) {
-    const uint32_t n = min(a.ctrl->n_start, a.ecap);
-    const uint32_t r = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (r >= n) return;
-    uint32_t run = 0;
-    for (uint32_t wb = 0; wb < a.nLw; wb += 32) {
-        const uint32_t wi = wb + lane;
-        const uint32_t pc = wi < a.nLw ? __popcll(a.bm[(size_t)r * a.nLw + wi]) : 0u;
-        const uint32_t incl = warp_incl_scan(pc, lane);
-        if (wi < a.nLw) a.wbase[(size_t)r * a.nLw + wi] = run + incl - pc;
-        run += __shfl_sync(0xFFFFFFFFu, incl, 31);
+// matched links before each 64-link word of every start time's row (a warp per row of the window)
+__global__ void __launch_bounds__(256) k_win_wbase(A2Args a) {
+    const uint32_t u0 = a.win->used0, u1 = min(a.ctrl->n_start, a.ecap);
+    const uint32_t lane = threadIdx.x & 31;
+    for (uint32_t r = u0 + blockIdx.x * 8 + (threadIdx.x >> 5); r < u1; r += gridDim.x * 8) {
+        uint32_t run = 0;
+        for (uint32_t wb = 0; wb < a.nLw; wb += 32) {
+            const uint32_t wi = wb + lane;
+            const uint32_t pc = wi < a.nLw ? __popcll(a.bm[(size_t)r * a.nLw + wi]) : 0u;
+            const uint32_t incl = warp_incl_scan(pc, lane);
+            if (wi < a.nLw) a.wbase[(size_t)r * a.nLw + wi] = run + incl - pc;
+            run += __shfl_sync(0xFFFFFFFFu, incl, 31);
+        }
     }
 }
 
-__global__ void __launch_bounds__(256) k_emit_write(A2Args a) {
-    if (a.ctrl->err & 1u) return;
+__global__ void __launch_bounds__(256) k_win_write(A2Args a) {
     const uint32_t v = blockIdx.x;
-    const uint32_t cnt = (uint32_t)ld128(a.hdr + v).hi;
+    const uint32_t c0 = a.wcur[v], c1 = a.wnext[v];
+    __syncthreads();
+    if (threadIdx.x == 0) a.wcur[v] = c1;                        // the next window starts here
+    if (a.ctrl->err & 1u) return;
     const unsigned long long base = a.nbase[v];
     const uint32_t e0 = a.in_off[v];
     const uint32_t* ids = a.ids + base;
-    for (uint32_t i = threadIdx.x; i < cnt; i += blockDim.x) {
-        const U128 en = a.log[base + i];
+    for (uint32_t i = c0 + threadIdx.x; i < c1; i += blockDim.x) {
+        const U128 en = ld128(a.log + base + i);
         const uint32_t l = a.in_link[e0 + ((uint32_t)(en.hi >> 32) & 7u)];
         const uint32_t r = a.trank[a.eslot[base + i]];
         const unsigned long long word = a.bm[(size_t)r * a.nLw + (l >> 6)];
@@ -949,6 +1007,16 @@ __global__ void __launch_bounds__(256) k_emit_write(A2Args a) {
         const uint32_t ch = ids[(uint32_t)en.hi];
         o[0] = make_uint4(a.orig != nullptr ? a.orig[ch] : ch, a.psrc[l], a.pdst[l], l);
         o[1] = make_uint4((uint32_t)ts, (uint32_t)(ts >> 32), (uint32_t)te, (uint32_t)(te >> 32));
+    }
+}
+
+// the window is written: records [0, emitted) are final (and told to the host when it is streaming them out)
+__global__ void k_win_end(A2Args a) {
+    const unsigned long long e = a.win->emitted_next;
+    a.win->emitted = e;
+    if (a.progress != nullptr && !(a.ctrl->err & 3u)) {
+        __threadfence_system();
+        *(volatile unsigned long long*)a.progress = e;
     }
 }
 

@@ -225,3 +225,47 @@ def test_static_entry_point_checks_its_arguments_before_touching_the_device(pk):
     assert b"PCCL_STATIC_SCRATCH_BYTES" in pk.pccl_strerror(pk.PCCL_ERR_TOO_LARGE)
     if not torch.cuda.is_available():
         assert call() == pk.PCCL_ERR_CUDA
+
+
+def test_step_R_threaded_one_pass_normaliser_at_full_size(pk):
+    """From 2^15 post pairs on, the one-pass normaliser works on slices of the chunk range, one per host thread (count
+    and validate, then write).  Config 5 at full size (0.48 M post pairs, uneven chunks per NPU): the conditions against
+    the definition, computed here with numpy; a deviation from the chunk order in the middle of the list must fall back
+    to the general path with the same result, and an invalid pair in a late slice must be refused."""
+    p = wl.config5(0)
+    assert len(p.post) >= 1 << 17
+
+    def conditions(pre, post):
+        pr = pk.Problem(pk.Topology(p.n_npus, p.links), p.group, p.n_chunks, pre, post, p.chunk_bytes)
+        assert pr.mode == 0
+        cs = np.random.default_rng(3).integers(0, p.n_chunks, 4000)
+        cs = np.concatenate([cs, np.arange(64), np.arange(p.n_chunks - 64, p.n_chunks),
+                             (np.arange(1, 8)[:, None] * p.n_chunks // 8 + np.arange(-3, 4)).ravel()])
+        return pr, {int(c): (lambda sd: (sd[0], tuple(sd[1].tolist())))(pr.condition(0, int(c))) for c in cs}
+
+    src = np.zeros(p.n_chunks, dtype=np.int64)
+    src[p.pre["chunk"]] = p.pre["npu"]
+    order = np.lexsort((p.post["npu"], p.post["chunk"]))
+    pc, pn = p.post["chunk"][order].astype(np.int64), p.post["npu"][order].astype(np.int64)
+    keep = pn != src[pc]
+    pc, pn = pc[keep], pn[keep]
+    off = np.concatenate([[0], np.cumsum(np.bincount(pc, minlength=p.n_chunks))])
+    pr, got = conditions(p.pre, p.post)
+    for c, (s, d) in got.items():
+        assert s == src[c] and d == tuple(pn[off[c]:off[c + 1]].tolist()), c
+    # total number of destinations = what the device would be given
+    n = pk.lib.pccl_problem_condition(pr.handle, 0, p.n_chunks - 1, None, None, 0)
+    assert n == off[-1] - off[-2]
+    # two adjacent pairs of different chunks swapped in the middle: not chunk-ordered any more -> general path, same result
+    post2 = p.post.copy()
+    m = len(post2) // 2
+    while post2["chunk"][m] == post2["chunk"][m + 1]:
+        m += 1
+    post2[[m, m + 1]] = post2[[m + 1, m]]
+    assert conditions(p.pre, post2)[1] == got
+    # an out-of-range NPU near the end
+    post3 = p.post.copy()
+    post3["npu"][-7] = p.n_npus
+    with pytest.raises(pk.PcclError) as e:
+        conditions(p.pre, post3)
+    assert e.value.code == pk.PCCL_ERR_INVALID

@@ -427,6 +427,22 @@ def test_full_size_schedule_equals_the_oracles_digest(pk, case, mode):
     checker.check_structure(p, s.transfers)
 
 
+@pytest.mark.slow
+@pytest.mark.parametrize("case,runs", [("cfg4:thin", 6), ("cfg5:thin", 3)], ids=lambda x: str(x))
+def test_full_size_streamed_schedule_equals_the_oracles_digest(pk, case, runs):
+    """The e2e path (pccl_synthesize, host buffers): the emitter ranks the claims in windows behind the global virtual
+    time on a second stream WHILE the barrier-free loop runs, and the host copies the finished prefix out meanwhile.
+    Where the windows fall depends on timing, the records must not: several runs, each against the oracle's digest."""
+    g = _golden(case)
+    if g is None:
+        pytest.skip(f"no oracle digest for {case}")
+    p = {"cfg4": wl.config4, "cfg5": wl.config5}[case.split(":")[0]](g["seed"])
+    for i in range(runs):
+        s = pk.synthesize(*p.args())
+        _assert_digest(s, g, f"{case} streamed, run {i}")
+        s.close()
+
+
 def test_dynamic_relay_record_buffer_rerun(pk):
     """The dynamic rule's record buffer is sized from the static relay tree's transfer count; when it is short the run
     still finishes (records past the end are dropped, the count goes on) and the phase is rerun with the exact count.
