@@ -73,39 +73,52 @@ class ClockSampler:
     def __init__(self, index: int):
         self.index, self.rows, self.stop, self.th = index, [], threading.Event(), None
 
-    def _run_nvml(self):
+    def _init_nvml(self):
+        """NVML is initialised by the caller's thread BEFORE the timed region starts (nvmlInit alone can take longer than
+        the whole region), so the sampling thread only reads."""
         import pynvml
         pynvml.nvmlInit()
         h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
         mx = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
         get_reasons = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
             pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+        pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)      # fail here, not in the thread
+        int(get_reasons(h))
+        self.nvml = (pynvml, h, mx, get_reasons)
+
+    def _sample_nvml(self):
+        pynvml, h, mx, get_reasons = self.nvml
         bits = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40}
-        while not self.stop.is_set():
-            sm = pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)
-            r = int(get_reasons(h))
-            row = [str(sm), str(mx), "0"] + [("Active" if r & bits[n] else "Not Active")
-                                            for n in ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")]
-            self.rows.append(row)
-            self.stop.wait(0.002)
+        sm = pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)
+        r = int(get_reasons(h))
+        self.rows.append([str(sm), str(mx), "0"] + [("Active" if r & bits[n] else "Not Active")
+                                                    for n in ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")])
+
+    def _sample_smi(self):
+        out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                              "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+        for line in out.strip().splitlines():
+            self.rows.append([x.strip() for x in line.split(",")])
 
     def _run(self):
-        try:
-            self._run_nvml()          # NVML: a sample every ~2 ms (the timed region is ~50 ms long)
-            return
-        except Exception:
-            pass
-        while not self.stop.is_set():
+        # NVML: a sample every ~2 ms (the timed region is some tens of ms long); nvidia-smi (~100 ms a call) otherwise
+        while True:
             try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
-                for line in out.strip().splitlines():
-                    self.rows.append([x.strip() for x in line.split(",")])
+                if self.nvml is not None:
+                    self._sample_nvml()
+                else:
+                    self._sample_smi()
             except Exception:
                 pass
-            self.stop.wait(0.1)
+            if self.stop.wait(0.002 if self.nvml is not None else 0.1):
+                return
 
     def __enter__(self):
+        self.nvml = None
+        try:
+            self._init_nvml()
+        except Exception:
+            self.nvml = None
         self.th = threading.Thread(target=self._run, daemon=True)
         self.th.start()
         return self

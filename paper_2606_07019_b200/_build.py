@@ -35,7 +35,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile if missing or older than its sources.  Returns the path of libpccl.so."""
     if force or stale():
         tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [nvcc_path(), *NVCC_FLAGS, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
+        extra = os.environ.get("PCCL_NVCC_EXTRA", "").split()   # e.g. -DPCCL_DEBUG_CU, -DPCCL_A2_PROFILE, -DPCCL_BFS_PROFILE
+        cmd = [nvcc_path(), *NVCC_FLAGS, *extra, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
         res = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or res.returncode != 0:
             print(" ".join(cmd))

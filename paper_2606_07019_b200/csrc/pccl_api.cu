@@ -76,10 +76,16 @@ inline cudaStream_t counted(cudaStream_t s) { G.launches.fetch_add(1, std::memor
 
 #define SERIALISE std::lock_guard<std::recursive_mutex> call_lock__(G.call_mu)
 
+#ifdef PCCL_DEBUG_CU   /* debugging build: say which call failed */
+#define CU_REPORT(e) fprintf(stderr, "[pccl] line %d: %s\n", __LINE__, cudaGetErrorString(e))
+#else
+#define CU_REPORT(e) ((void)0)
+#endif
 #define CU(call)                                   \
     do {                                           \
         cudaError_t e__ = (call);                  \
         if (e__ != cudaSuccess) {                  \
+            CU_REPORT(e__);                        \
             (void)cudaGetLastError();              \
             return PCCL_ERR_CUDA;                  \
         }                                          \
@@ -1376,15 +1382,18 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     void* args[] = {(void*)&a};
     // one window of the emitter (pccl_loop2.cuh): the claims that start before the global virtual time -- or all that
     // are left (final) -- ranked and written behind the records of the earlier windows
-    auto window = [&](cudaStream_t s, int final) -> cudaError_t {
-        k_win_begin<<<1, 1024, 0, counted(s)>>>(a, final);
-        k_win_times<<<N, 256, 0, counted(s)>>>(a);
+    // `pad` bytes of (unused) dynamic shared memory keep a window's CTAs off the SMs where a CTA of the loop is resident:
+    // beside the loop's latency-bound warps they cost it 0.18 ms at config 4 (measured); on the SMs the loop leaves free
+    // they cost it nothing
+    auto window = [&](cudaStream_t s, int final, size_t pad) -> cudaError_t {
+        k_win_begin<<<1, 1024, pad, counted(s)>>>(a, final);
+        k_win_times<<<N, 256, pad, counted(s)>>>(a);
         if (!raw_only) {
-            k_win_rank<<<(a.ecap + 255) / 256, 256, 0, counted(s)>>>(a);
-            k_win_base<<<1, 1024, 0, counted(s)>>>(a);
-            k_win_bits<<<N, 256, 0, counted(s)>>>(a);
-            k_win_wbase<<<std::min<uint32_t>((a.ecap + 7) / 8, 256u), 256, 0, counted(s)>>>(a);
-            k_win_write<<<N, 256, 0, counted(s)>>>(a);
+            k_win_rank<<<(a.ecap + 255) / 256, 256, pad, counted(s)>>>(a);
+            k_win_base<<<1, 1024, pad, counted(s)>>>(a);
+            k_win_bits<<<N, 256, pad, counted(s)>>>(a);
+            k_win_wbase<<<std::min<uint32_t>((a.ecap + 7) / 8, 256u), 256, pad, counted(s)>>>(a);
+            k_win_write<<<N, 256, pad, counted(s)>>>(a);
             k_win_end<<<1, 1, 0, counted(s)>>>(a);
         } else {
             k_emit_raw<<<N, 256, 0, counted(s)>>>(a);
@@ -1393,7 +1402,25 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     };
     // streaming: the progress word lives in the pinned mailbox (mapped: k_win_end stores to it directly)
     volatile unsigned long long* progress = (volatile unsigned long long*)((unsigned char*)G.mailbox + 2048);
-    const bool stream_out = host_out != nullptr && !raw_only && out_cap > 0;
+    // Early windows -- the emitter running on a second stream while the loop is going -- in two cases.  (i) The records
+    // leave for the host: the download then overlaps the loop.  (ii) They stay on the device and the loop leaves SMs free
+    // (config 4: 128 CTAs on 148 SMs): what is left for the window after the loop is only the tail of the schedule.  Window
+    // CTAs resident BESIDE the loop's latency-bound warps cost it 0.1-0.18 ms at config 4 (measured): worth it for (i), not
+    // for (ii) -- there `win_pad` bytes of unused dynamic shared memory keep them on the SMs without a CTA of the loop
+    // (loop + emit 2.52 -> 2.41 ms at config 4; with the pad in case (i) the windows fall behind the download: 3.4 -> 4.1 ms).
+    const bool stream_out = !raw_only && out_cap > 0 && host_out != nullptr;
+    size_t win_pad = 0;
+    if (!stream_out && !raw_only && out_cap > 0 && (uint32_t)G.sm_count >= W.a2_grid + 16u && W.a2.smem_need + 218 * 1024 > 227 * 1024) {
+        win_pad = 216 * 1024;
+        static std::atomic<int> padded_dev{-1};      // the attribute is per device function: set once per device in use
+        if (padded_dev.load() != G.dev) {
+            const void* ks[] = {(const void*)k_win_begin, (const void*)k_win_times, (const void*)k_win_rank, (const void*)k_win_base,
+                                (const void*)k_win_bits, (const void*)k_win_wbase, (const void*)k_win_write};
+            for (const void* k : ks) CU(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)win_pad));
+            padded_dev.store(G.dev);
+        }
+    }
+    const bool early = stream_out || win_pad != 0;
     uint64_t copied = 0;
     struct Drain {   // whatever happens, nothing of this call is left running on the side streams
         bool on;
@@ -1403,19 +1430,21 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
             (void)cudaStreamSynchronize(G.copy_stream);
             (void)cudaGetLastError();
         }
-    } drain{stream_out};
-    if (stream_out) {
-        *progress = 0;
-        void* dp = nullptr;
-        CU(cudaHostGetDevicePointer(&dp, (void*)progress, 0));
-        a.progress = (unsigned long long*)dp;
+    } drain{early};
+    if (early) {
+        if (stream_out) {
+            *progress = 0;
+            void* dp = nullptr;
+            CU(cudaHostGetDevicePointer(&dp, (void*)progress, 0));
+            a.progress = (unsigned long long*)dp;
+        }
         CU(cudaEventRecord(G.pre_loop, st));                      // headers, logs and tables are initialised
         CU(cudaStreamWaitEvent(G.emit_stream, G.pre_loop, 0));
     }
     if (tm) { tm->setup.stop(); tm->loop.start(); }
     CU(cudaLaunchCooperativeKernel(kloop2, dim3(W.a2_grid), dim3(threads), args, smem, counted(st)));
     if (tm) tm->loop.stop();
-    if (stream_out) {
+    if (early) {
         // windows on the emit stream while the loop runs (it never waits for them; they read headers and logs only);
         // finished records leave in pieces of >= 2 MB on the copy stream.  Both streams are drained before anything
         // can fail or return.
@@ -1425,13 +1454,13 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
         while (e == cudaSuccess && (q = cudaEventQuery(G.loop_done)) == cudaErrorNotReady) {
             if (in_flight && cudaEventQuery(G.win_done) != cudaErrorNotReady) in_flight = false;
             if (in_flight) continue;
-            const uint64_t p = std::min<uint64_t>(*progress, out_cap);
+            const uint64_t p = stream_out ? std::min<uint64_t>(*progress, out_cap) : 0;
             if (p >= copied + PIECE) {
                 e = cudaMemcpyAsync(host_out + copied, out + copied, (p - copied) * sizeof(Rec), cudaMemcpyDeviceToHost,
                                     G.copy_stream);
                 copied = p;
             }
-            if (e == cudaSuccess) e = window(G.emit_stream, 0);
+            if (e == cudaSuccess) e = window(G.emit_stream, 0, win_pad);
             if (e == cudaSuccess) e = cudaEventRecord(G.win_done, G.emit_stream);
             in_flight = any = true;
         }
@@ -1448,7 +1477,7 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     }
     if (tm) tm->emit.start();
     {
-        const cudaError_t e = window(st, 1);
+        const cudaError_t e = window(st, 1, 0);
         if (e != cudaSuccess) {
             (void)cudaStreamSynchronize(G.copy_stream);
             (void)cudaStreamSynchronize(st);
@@ -1604,7 +1633,7 @@ int phase_loop(const pccl_problem& P, const Phase& ph, const Work& W, uint64_t s
         uint64_t copied = 0;
         cudaError_t e = cudaEventRecord(G.loop_done, st), q = cudaErrorNotReady;
         while (e == cudaSuccess && (q = cudaEventQuery(G.loop_done)) == cudaErrorNotReady) {
-            const uint64_t p = std::min<uint64_t>(*progress, out_cap);
+            const uint64_t p = stream_out ? std::min<uint64_t>(*progress, out_cap) : 0;
             if (p >= copied + PIECE) {
                 e = cudaMemcpyAsync(host_out + copied, out + copied, (p - copied) * sizeof(Rec), cudaMemcpyDeviceToHost,
                                     G.copy_stream);

@@ -384,7 +384,8 @@ struct LoopArgs {
 
 constexpr uint32_t HOLD_ROW = 32, HOLD_CAP = 31;
 constexpr int TRACE_SLOTS = 12;  // 0 loop top, 1 links phase, 2 barrier 1, 3 in-link list, 4 count, 5 pick, 6 commit,
-                                 // 7 barrier 2, 8 summary scan, 9 work list, 10 unused, 11 unused
+                                 // 7 barrier 2, 8 summary scan, 9 work list, 10 conflict resolve, 11 dynamic rule: the
+                                 // wants-shrink of the event before (stamped between 0 and 1)
 __device__ __forceinline__ void trace_stamp(const LoopArgs& a, uint32_t step, int slot) {
     if (a.trace != nullptr && blockIdx.x == 0 && threadIdx.x == 0 && step < a.trace_cap) {
         unsigned long long ns;
@@ -477,6 +478,8 @@ __device__ __forceinline__ bool dyn_still_wants(const LoopArgs& a, uint32_t u, u
     return false;
 }
 
+__device__ __forceinline__ void dyn_drop(const LoopArgs& a, uint32_t u, uint32_t c, uint64_t t);
+
 // ---- P1: ordered emit of the previous event's matches (a8) + arrivals at time t (a3) ---------------
 template <bool DYN>
 __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t step, uint64_t t,
@@ -545,11 +548,10 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
                 const uint32_t o = a.out_link[off + k], v2 = a.out_far[off + k];
                 if ((ldcg64(a.wants + (size_t)v2 * a.Wp + (c >> 6)) >> (c & 63)) & 1ull) {
                     if (DYN && a.hold != nullptr && !dyn_still_wants(a, v2, c)) {
-                        // lazy dynamic rule: v2 stopped wanting c while no neighbour held it; the bit goes now, and no
-                        // count can include it (a neighbour that held c would have had it cleared at the tightening)
-                        const unsigned long long bit = 1ull << (c & 63);
-                        if (atomicAnd((unsigned long long*)&a.wants[(size_t)v2 * a.Wp + (c >> 6)], ~bit) & bit)
-                            atomicSub(&a.wants_cnt[v2], 1u);
+                        // lazy dynamic rule: v2 stopped wanting c -- either long ago, while no neighbour held it (then no
+                        // count includes it), or at the event before this one (the shrink of that event runs beside
+                        // these arrivals: whoever clears the bit takes the candidate away from the earlier holders)
+                        dyn_drop(a, v2, c, t);
                     } else {
                         atomicAdd(&a.gcnt[(size_t)o * a.S + (c >> 12)], 1u);
                         atomicAdd(&a.gtot[o], 1u);
@@ -565,13 +567,21 @@ __device__ __forceinline__ void loop_phase_links(const LoopArgs& a, uint32_t ste
 }
 
 // ---- dynamic relay rule, end of an event (Q18).  Every claim (c, v) of the event has tightened
-// best[p] = min(best[p], dist(v -> d_p)) for the pairs p of c at commit; after the event's barrier, for every
+// best[p] = min(best[p], dist(v -> d_p)) for the pairs p of c at commit; after the event's second barrier, for every
 // claimed chunk, each node that is no longer strictly closer to some dest than the best holder stops wanting it
-// (and, with kept counts, its in-links lose the candidate).  A barrier follows: arrivals read wants.
+// (and, with kept counts, its in-links lose the candidate).  No barrier of its own: the phase runs BESIDE the
+// arrivals of the next event time t (loop_phase_links), which read wants and set have bits -- both sides evaluate
+// the same rule on the same best[] (nothing commits between the two barriers), the one that clears a bit does the
+// whole upkeep, and "the source held c" below means "before the arrivals of time t".
 // v stops wanting c (dynamic rule): clear the bit once, and with kept counts take the candidate away from every
-// in-link of u whose source holds c
-__device__ __forceinline__ void dyn_drop(const LoopArgs& a, uint32_t u, uint32_t c) {
+// in-link of u whose source held c before time t.  A source that receives c at t itself (an in-link of it has
+// inflight == c and free_t == t; its have bit may or may not be stored yet) never counted the candidate: its own
+// arrival thread sees the bit cleared, or sees the rule fail.
+__device__ __forceinline__ void dyn_drop(const LoopArgs& a, uint32_t u, uint32_t c, uint64_t t) {
     const unsigned long long bit = 1ull << (c & 63);
+#ifdef PCCL_DEBUG_COUNTS
+    if (u >= a.N || c >= a.Wp * 64u) { printf("[dbg] drop u %u c %u\n", u, c); return; }
+#endif
     if (!(atomicAnd((unsigned long long*)&a.wants[(size_t)u * a.Wp + (c >> 6)], ~bit) & bit)) return;   // once per (u, c)
     atomicSub(&a.wants_cnt[u], 1u);
     if (a.gcnt == nullptr) return;
@@ -590,6 +600,19 @@ __device__ __forceinline__ void dyn_drop(const LoopArgs& a, uint32_t u, uint32_t
 #pragma unroll
         for (int k = 0; k < 4; ++k)
             if ((hw[k] >> (c & 63)) & 1ull) {
+                bool now = false;                          // is c arriving at the source right now?
+                const uint32_t f1 = a.in_off[u2[k] + 1];
+                for (uint32_t f0 = a.in_off[u2[k]]; f0 < f1; f0 += 8) {   // eight in-links of the source per round trip
+                    uint32_t li[8], ci[8];
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) li[q] = f0 + q < f1 ? a.in_link[f0 + q] : NONE32;
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) ci[q] = li[q] != NONE32 ? ldcg32(a.inflight + li[q]) : NONE32;
+#pragma unroll
+                    for (int q = 0; q < 8; ++q)
+                        if (li[q] != NONE32 && ci[q] == c && ldcg64(a.free_t + li[q]) == t) now = true;
+                }
+                if (now) continue;
                 atomicSub(&a.gcnt[(size_t)l2[k] * a.S + (c >> 12)], 1u);
                 atomicSub(&a.gtot[l2[k]], 1u);
             }
@@ -597,7 +620,7 @@ __device__ __forceinline__ void dyn_drop(const LoopArgs& a, uint32_t u, uint32_t
 }
 
 // every node that no longer wants claimed chunk c loses the bit (whole warp; scans all nodes)
-__device__ __forceinline__ void dyn_shrink_chunk(const LoopArgs& a, uint32_t c, uint32_t lane) {
+__device__ __forceinline__ void dyn_shrink_chunk(const LoopArgs& a, uint32_t c, uint32_t lane, uint64_t t) {
     const uint64_t p0 = a.dest_off[c], p1 = a.dest_off[c + 1];
     const unsigned long long bit = 1ull << (c & 63);
     if (p1 - p0 <= 32) {
@@ -624,12 +647,12 @@ __device__ __forceinline__ void dyn_shrink_chunk(const LoopArgs& a, uint32_t c, 
             }
 #pragma unroll
             for (int k = 0; k < 4; ++k)
-                if (need[k] && !keep[k]) dyn_drop(a, ub + 32 * k + lane, c);
+                if (need[k] && !keep[k]) dyn_drop(a, ub + 32 * k + lane, c, t);
         }
     } else {
         for (uint32_t u = lane; u < a.N; u += 32) {
             if (!(ldcg64(a.wants + (size_t)u * a.Wp + (c >> 6)) & bit)) continue;
-            if (!dyn_still_wants(a, u, c)) dyn_drop(a, u, c);
+            if (!dyn_still_wants(a, u, c)) dyn_drop(a, u, c, t);
         }
     }
 }
@@ -639,21 +662,29 @@ __device__ __forceinline__ void dyn_shrink_chunk(const LoopArgs& a, uint32_t c, 
 // bits of all other nodes may stay stale until a neighbour receives the chunk -- the arrival then applies the rule
 // (loop_phase_links).  A chunk with more than HOLD_CAP arrivals falls back to the scan over all nodes, which is
 // exact whatever was skipped before.
-__device__ __forceinline__ void dyn_shrink_wants(const LoopArgs& a, uint32_t step) {
+// `step` is the event whose claims are applied, t the time of the event after it (whose arrivals run beside this).
+__device__ __forceinline__ void dyn_shrink_wants(const LoopArgs& a, uint32_t step, uint64_t t) {
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nW = (gridDim.x * blockDim.x) >> 5;
     const uint64_t* mb = a.matchbits + (size_t)(step & 1) * a.nLw;
     for (uint32_t l = gw; l < a.L; l += nW) {   // a warp per link matched at this event
         if (!((ldcg64(mb + (l >> 6)) >> (l & 63)) & 1ull)) continue;
         const uint32_t c = ldcg32(a.inflight + l);
-        if (a.hold == nullptr) { dyn_shrink_chunk(a, c, lane); continue; }
+#ifdef PCCL_DEBUG_COUNTS
+        if (c >= a.Wp * 64u) { if (lane == 0) printf("[dbg] shrink step %u link %u: inflight %u\n", step, l, c); continue; }
+#endif
+        if (a.hold == nullptr) { dyn_shrink_chunk(a, c, lane, t); continue; }
         // everything keyed on c in one round trip: the arrival count, the pairs, the holder slots (slots past the
         // count hold garbage and are masked below).  Lane 0: the source, lanes 1..nh: the arrival nodes
-        const uint32_t nh = ldcg32(a.hold_cnt + c);
+        // (the count moves while this runs -- the arrivals of time t append their nodes: ONE read for the whole warp)
+        const uint32_t nh = __shfl_sync(0xFFFFFFFFu, ldcg32(a.hold_cnt + c), 0);
         const uint64_t p0 = a.dest_off[c], p1 = a.dest_off[c + 1];
         uint32_t u = (lane == 0) ? a.csrc[c] : ldcg32(a.hold + (size_t)c * HOLD_ROW + lane);
-        if (nh > HOLD_CAP || p1 - p0 > 32) { dyn_shrink_chunk(a, c, lane); continue; }
-        if (lane > nh) u = NONE32;
+        if (nh > HOLD_CAP || p1 - p0 > 32) { dyn_shrink_chunk(a, c, lane, t); continue; }
+        // (a slot of an arrival that is being appended right now may not be stored yet: whatever it holds, a node id is
+        // revisited harmlessly -- the rule decides -- and anything else is skipped; the arrival's own thread applies the
+        // rule to that node's out-neighbours)
+        if (lane > nh || u >= a.N) u = NONE32;
         const uint32_t np = (uint32_t)(p1 - p0);
         uint32_t row = 0;               // lane q: pair q of c (row of its dest in Dto, current best)
         unsigned long long bst = 0;
@@ -680,7 +711,7 @@ __device__ __forceinline__ void dyn_shrink_wants(const LoopArgs& a, uint32_t ste
                 const unsigned long long b = __shfl_sync(0xFFFFFFFFu, bst, q);
                 if (need && !keep) keep = a.Dto[(size_t)r * a.N + v2] < b;
             }
-            if (need && !keep) dyn_drop(a, v2, c);
+            if (need && !keep) dyn_drop(a, v2, c, t);
         }
     }
 }
@@ -1317,11 +1348,38 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop(const Loop
     __shared__ unsigned long long s_next[2];   // one thread per CTA reads the two hot words after a barrier
     for (;;) {
         trace_stamp(a, step, 0);
+        // dynamic rule: the wants-shrink of the event before runs beside this event's arrivals (no barrier between
+        // them, see dyn_drop); best[] is final since that event's second barrier
+        if (DYN && a.best != nullptr && step > 0) {
+            dyn_shrink_wants(a, step - 1, t);
+            trace_stamp(a, step, 11);
+        }
         loop_phase_links<DYN>(a, step, t, emit_base);
         emit_base = total_now;
         trace_stamp(a, step, 1);
         grid.sync();
         trace_stamp(a, step, 2);
+#ifdef PCCL_DEBUG_COUNTS   /* debugging build: the kept counts against a recount of have[src] & wants[dst] */
+        if (a.gtot != nullptr) {
+            const uint32_t lane = threadIdx.x & 31;
+            const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nW = (gridDim.x * blockDim.x) >> 5;
+            for (uint32_t l = gw; l < a.L; l += nW) {
+                uint32_t n = 0;
+                for (uint32_t wi = lane; wi < a.Wp; wi += 32)
+                    n += __popcll(ldcg64(a.have + (size_t)a.esrc[l] * a.Wp + wi) & ldcg64(a.wants + (size_t)a.edst[l] * a.Wp + wi));
+                n = __reduce_add_sync(0xFFFFFFFFu, n);
+                const uint32_t g = ldcg32(a.gtot + l);
+                if (lane == 0 && g != n) {
+                    printf("[counts] step %u t %llu link %u (%u -> %u): kept %u actual %u\n", step, (unsigned long long)t, l, a.esrc[l], a.edst[l], g, n);
+                    for (uint32_t wi = 0; wi < a.Wp; ++wi) {
+                        const unsigned long long x = ldcg64(a.have + (size_t)a.esrc[l] * a.Wp + wi) & ldcg64(a.wants + (size_t)a.edst[l] * a.Wp + wi);
+                        if (x) printf("[counts]   link %u word %u: %llx\n", l, wi, x);
+                    }
+                }
+            }
+            grid.sync();
+        }
+#endif
         {
             uint32_t k = 0;
             for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x, ++k)
@@ -1339,12 +1397,6 @@ __global__ void __launch_bounds__(NBT * 32, 1024 / (NBT * 32)) k_loop(const Loop
         t = s_next[0];
         total_now = s_next[1];
         __syncthreads();
-        if (DYN && a.best != nullptr && t != T_INF) {   // (the last event never has claims)
-            dyn_shrink_wants(a, step);
-            trace_stamp(a, step, 10);
-            grid.sync();
-            trace_stamp(a, step, 11);
-        }
         ++step;
         if (t == T_INF) break;
     }
