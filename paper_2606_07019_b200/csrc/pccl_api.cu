@@ -1198,9 +1198,11 @@ int phase_setup(const pccl_problem& P, const Phase& ph, Work& W, uint64_t seed, 
     if (C) k_have<<<(C + 255) / 256, 256, 0, counted(st)>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
     const uint64_t ND = ph.dests.size();
     if (ND) {
-        k_wants<<<(unsigned)((ND + 127) / 128), 128, 0, counted(st)>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, ND, pv.esrc, pv.in_off,
+        const size_t wants_smem = (size_t)N * 8 <= 32 * 1024 ? (size_t)N * 8 : 0;   // the staged distance row (k_wants)
+        k_wants<<<(unsigned)((ND + 127) / 128), 128, wants_smem, counted(st)>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, ND, pv.esrc, pv.in_off,
                                                           pv.in_link, W.w, ph.d_sidx, W.D, N, W.Wp, W.SWp, k0, k1, W.wants,
-                                                          W.wsum, W.wants_cnt, &W.ctrl->err, ph.d_orig);
+                                                          W.wsum, W.wants_cnt, &W.ctrl->err, ph.d_orig, wants_smem ? 1u : 0u);
+        k_wants_finish<<<N, 256, 0, counted(st)>>>(W.wants, W.Wp, W.SWp, W.wsum, W.wants_cnt);
     }
     k_sum_u32<<<1, 1024, 0, counted(st)>>>(W.wants_cnt, N, &W.ctrl->wants_total);
     W.a2_planned = false;

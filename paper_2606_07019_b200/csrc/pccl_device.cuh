@@ -140,31 +140,42 @@ __global__ void k_have(const uint32_t* __restrict__ cond_src, uint32_t C, uint32
 // in-link (ascending link id), j = (Philox(c, cur, 0, 1)[0] * |tight|) >> 32.  The choice is
 // keyed on (c, cur) only, so walks of one chunk merge into a tree whatever order they run in;
 // a walk stops at the first node already marked for its chunk.
-__global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* __restrict__ dests,
+__global__ void __launch_bounds__(128, 12) k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* __restrict__ dests,
                         const uint32_t* __restrict__ dchunk, uint64_t n_pairs,
                         const uint32_t* __restrict__ esrc, const uint32_t* __restrict__ in_off,
                         const uint32_t* __restrict__ in_link, const uint64_t* __restrict__ w,
                         const uint32_t* __restrict__ sidx, const uint64_t* __restrict__ D, uint32_t N,
                         uint32_t Wp, uint32_t SWp, uint32_t k0, uint32_t k1, uint64_t* __restrict__ wants,
                         uint64_t* __restrict__ wsum, uint32_t* __restrict__ wants_cnt, uint32_t* __restrict__ err,
-                        const uint32_t* __restrict__ orig = nullptr) {   // orig: the caller's id of a relabelled chunk (keys the draw)
+                        const uint32_t* __restrict__ orig, uint32_t stage) {   // orig: the caller's id of a relabelled chunk (keys the draw)
+    // stage != 0 (N * 8 bytes of dynamic shared memory): the distance row of the block's FIRST pair's source is copied to
+    // shared memory.  Collectives list their chunks source by source, so nearly every pair of the block walks on that
+    // row (config 4: 511 consecutive pairs per source) and its ~40 distance loads hit shared memory instead of L2;
+    // a pair of another source reads its row from global memory as before.
+    extern __shared__ uint64_t s_row[];
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t staged = NONE32;
+    if (stage) {
+        staged = sidx[cond_src[dchunk[(uint64_t)blockIdx.x * blockDim.x]]];
+        const uint64_t* row = D + (size_t)staged * N;
+        for (uint32_t i = threadIdx.x; i < N; i += blockDim.x) s_row[i] = row[i];
+        __syncthreads();
+    }
     if (p >= n_pairs) return;
     const uint32_t c = dchunk[p];
     const uint32_t ck = orig != nullptr ? orig[c] : c;
     const uint32_t s = cond_src[c];
-    const uint64_t* Ds = D + (size_t)sidx[s] * N;
+    const uint32_t si = sidx[s];
+    const uint64_t* Ds = si == staged ? s_row : D + (size_t)si * N;
     uint32_t cur = dests[p];
     if (Ds[cur] == T_INF) { atomicOr(err, 1u); return; }
     const unsigned long long bit = 1ull << (c & 63);
     while (cur != s) {
-        // the node's tables are loaded before the mark's round trip is waited for
+        // the mark's round trip (a third of the kernel's stall samples when it was waited for first) runs beside the
+        // choice of the predecessor: `old` is only looked at once the next node is known
         const uint64_t dcur = Ds[cur];
         const uint32_t e0 = in_off[cur], e1 = in_off[cur + 1];
         const unsigned long long old = atomicOr((unsigned long long*)&wants[(size_t)cur * Wp + (c >> 6)], bit);
-        if (old & bit) break;
-        atomicOr((unsigned long long*)&wsum[(size_t)cur * SWp + (c >> 14)], 1ull << ((c >> 8) & 63));
-        atomicAdd(&wants_cnt[cur], 1u);
         uint32_t nxt = cur;
         if (e1 - e0 <= 32) {
             // one pass: tight in-links as a bit mask (ascending link id = ascending bit), then the j-th set bit
@@ -196,7 +207,41 @@ __global__ void k_wants(const uint32_t* __restrict__ cond_src, const uint32_t* _
                 }
             }
         }
+        if (old & bit) break;                    // another walk of this chunk marked the node: it also goes on from here
         cur = nxt;
+    }
+}
+
+// wants_cnt[v] = popcount of the wants row, wsum[v] = its sector summary: one streaming pass over the rows after the
+// walks.  (Counted by the walks themselves these were 2 atomics per mark on N and N * C / 16384 hot addresses --
+// same-address atomics are served one after the other: k_wants 180 -> ... us at config 4.)  One block per node.
+__global__ void __launch_bounds__(256) k_wants_finish(const uint64_t* __restrict__ wants, uint32_t Wp, uint32_t SWp,
+                                                      uint64_t* __restrict__ wsum, uint32_t* __restrict__ wants_cnt) {
+    const uint32_t v = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint64_t* row = wants + (size_t)v * Wp;
+    __shared__ uint32_t s_cnt[8];
+    uint32_t cnt = 0;
+    for (uint32_t sw = warp; sw < SWp; sw += 8) {          // a warp per summary word: 64 sectors of 4 words
+        bool any[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const uint32_t w0 = (sw * 64 + h * 32 + lane) * 4;
+            uint64_t x[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) x[k] = w0 + k < Wp ? row[w0 + k] : 0ull;
+            any[h] = (x[0] | x[1] | x[2] | x[3]) != 0ull;
+            cnt += __popcll(x[0]) + __popcll(x[1]) + __popcll(x[2]) + __popcll(x[3]);
+        }
+        const uint32_t lo = __ballot_sync(0xFFFFFFFFu, any[0]), hi = __ballot_sync(0xFFFFFFFFu, any[1]);
+        if (lane == 0) wsum[(size_t)v * SWp + sw] = ((uint64_t)hi << 32) | lo;
+    }
+    cnt = __reduce_add_sync(0xFFFFFFFFu, cnt);
+    if (lane == 0) s_cnt[warp] = cnt;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t t = 0;
+        for (int k = 0; k < 8; ++k) t += s_cnt[k];
+        wants_cnt[v] = t;
     }
 }
 
