@@ -14,6 +14,7 @@
 #include <system_error>
 #include <mutex>
 #include <new>
+#include <memory>
 #include <atomic>
 #if defined(__x86_64__)
 #include <immintrin.h>
@@ -76,6 +77,18 @@ inline cudaStream_t counted(cudaStream_t s) { G.launches.fetch_add(1, std::memor
 
 #define SERIALISE std::lock_guard<std::recursive_mutex> call_lock__(G.call_mu)
 
+#ifdef PCCL_DEBUG_TIMELINE   /* debugging build: host-side time between marks of one call, to stderr */
+static thread_local std::chrono::steady_clock::time_point dbgt_last__;
+#define DBGT(label)                                                                                              \
+    do {                                                                                                         \
+        const auto now__ = std::chrono::steady_clock::now();                                                     \
+        fprintf(stderr, "[t] %-28s %8.1f us\n", label,                                                           \
+                std::chrono::duration<double, std::micro>(now__ - dbgt_last__).count());                         \
+        dbgt_last__ = now__;                                                                                     \
+    } while (0)
+#else
+#define DBGT(label) ((void)0)
+#endif
 #ifdef PCCL_DEBUG_CU   /* debugging build: say which call failed */
 #define CU_REPORT(e) fprintf(stderr, "[pccl] line %d: %s\n", __LINE__, cudaGetErrorString(e))
 #else
@@ -596,34 +609,54 @@ void finish_phase(Phase& ph, uint32_t N) {
     index_phase(ph, N, is_src, is_dst);
 }
 
-// A few host threads kept for the life of the process (the normaliser's passes over millions of pairs): run(n, f) calls
-// f(0) on the caller and f(1) .. f(n-1) on the workers and returns when all are done.  Workers are created on first
-// use; if none can be created everything runs on the caller.
+// A few host threads kept for the life of the process (the normaliser's passes over millions of pairs).
+// parallel_for(n, f) runs f(0) .. f(n-1), each once: the caller and whichever workers are awake CLAIM indices from a
+// shared counter, and the call returns when every claimed index is done.  Nobody ever waits for a worker to wake up: on
+// the GPU box (a VM) a condition-variable wake-up took up to a millisecond, which the earlier one-slice-per-thread form
+// paid on every call (normalise 0.24 ms or 1.1 ms at config 4, depending on the run); a worker that wakes late finds
+// nothing left to claim and goes back to sleep.  After a job a worker polls for the next one for a short while (the
+// normaliser's second pass follows its first within microseconds) before it sleeps.
 class HostPool2 {
+    struct Job {
+        std::function<void(int)> fn;
+        int n = 0;
+        std::atomic<int> next{0}, done{0};
+    };
     std::vector<std::thread> th_;
     std::mutex mu_;
-    std::condition_variable cv_, done_;
-    const std::function<void(int)>* job_ = nullptr;
-    int want_ = 0, left_ = 0;
-    uint64_t gen_ = 0;
+    std::condition_variable cv_;
+    std::shared_ptr<Job> job_;                 // (kept alive by every worker that holds it: a late one only reads next/n)
+    std::atomic<uint64_t> gen_{0};
     bool stop_ = false;
-    void worker(int id) {
+    static void drain(Job& j) {
+        for (;;) {
+            const int i = j.next.fetch_add(1, std::memory_order_relaxed);
+            if (i >= j.n) return;
+            j.fn(i);
+            j.done.fetch_add(1, std::memory_order_release);
+        }
+    }
+    void worker() {
         uint64_t seen = 0;
         for (;;) {
-            const std::function<void(int)>* f = nullptr;
+            std::shared_ptr<Job> j;
+            for (int spin = 0; spin < 2000 && gen_.load(std::memory_order_acquire) == seen; ++spin) cpu_relax_();
             {
                 std::unique_lock<std::mutex> lk(mu_);
-                cv_.wait(lk, [&] { return stop_ || (gen_ != seen && id < want_); });
+                cv_.wait(lk, [&] { return stop_ || gen_.load(std::memory_order_relaxed) != seen; });
                 if (stop_) return;
-                seen = gen_;
-                f = job_;
+                seen = gen_.load(std::memory_order_relaxed);
+                j = job_;
             }
-            (*f)(id);
-            {
-                std::lock_guard<std::mutex> lk(mu_);
-                if (--left_ == 0) done_.notify_one();
-            }
+            if (j) drain(*j);
         }
+    }
+    static void cpu_relax_() {
+#if defined(__x86_64__)
+        _mm_pause();
+#else
+        std::this_thread::yield();
+#endif
     }
 public:
     static constexpr int MAX_THREADS = 8;
@@ -633,25 +666,30 @@ public:
             const int hw = (int)std::thread::hardware_concurrency();
             const int n = std::max(1, std::min(MAX_THREADS, hw / 2));
             try {
-                for (int i = 1; i < n; ++i) th_.emplace_back([this, i] { worker(i); });
+                for (int i = 1; i < n; ++i) th_.emplace_back([this] { worker(); });
             } catch (const std::system_error&) {
             }
         }
         return (int)th_.size() + 1;
     }
-    void run(int n, const std::function<void(int)>& f) {
-        n = std::min(n, capacity());
-        if (n > 1) {
+    void parallel_for(int n, const std::function<void(int)>& f) {
+        if (n <= 0) return;
+        if (n == 1 || capacity() == 1) {
+            for (int i = 0; i < n; ++i) f(i);
+            return;
+        }
+        std::shared_ptr<Job> j = std::make_shared<Job>();
+        j->fn = f; j->n = n;
+        {
             std::lock_guard<std::mutex> lk(mu_);
-            job_ = &f; want_ = n; left_ = n - 1; ++gen_;
+            job_ = j;
+            gen_.fetch_add(1, std::memory_order_release);
         }
-        if (n > 1) cv_.notify_all();
-        f(0);
-        if (n > 1) {
-            std::unique_lock<std::mutex> lk(mu_);
-            done_.wait(lk, [&] { return left_ == 0; });
-            want_ = 0;
-        }
+        cv_.notify_all();
+        drain(*j);
+        while (j->done.load(std::memory_order_acquire) < n) cpu_relax_();   // indices claimed by workers that are running
+        std::lock_guard<std::mutex> lk(mu_);
+        if (job_ == j) job_.reset();
     }
     ~HostPool2() {
         {
@@ -693,28 +731,29 @@ bool normalise_ordered_copy(const pccl_condition_t* pre, const pccl_condition_t*
     const uint64_t nq = post->n_pairs;
     const char* mem = member.data();
     std::unique_lock<std::mutex> region(g_threads_mu, std::defer_lock);
-    int T = 1;
+    int T = 1;                                                     // slices of the chunk range (>= 2^13 post pairs each)
     if (nq >= (1u << 15)) {
         region.lock();
-        T = std::min<int>(g_threads.capacity(), (int)std::min<uint64_t>(HostPool2::MAX_THREADS, nq >> 14));
+        if (g_threads.capacity() > 1) T = (int)std::min<uint64_t>(64, nq >> 13);
     }
     struct Slice {
         uint32_t c_lo, c_hi;
         uint64_t k_lo, k_end, nd;
         bool ok;
-        std::vector<uint32_t> f_src, f_dst;
     };
     std::vector<Slice> sl((size_t)T);
     for (int t = 0; t < T; ++t) {
         sl[t].c_lo = (uint32_t)((uint64_t)C * t / T);
         sl[t].c_hi = (uint32_t)((uint64_t)C * (t + 1) / T);
-        sl[t].f_src.assign(N, 0);
-        sl[t].f_dst.assign(N, 0);
+        sl[t].ok = false;
     }
+    // marks "is a source" / "is a destination", shared by the slices (every store writes 1: relaxed atomic byte stores)
+    std::vector<unsigned char> f_src(N, 0), f_dst(N, 0);
+    unsigned char* fs = f_src.data();
+    unsigned char* fd = f_dst.data();
     // pass 1: validate, count the destinations (post-holders other than the source), mark sources and destinations
     const std::function<void(int)> pass1 = [&](int t) {
         Slice& s = sl[t];
-        s.ok = false;
         uint64_t lo = 0, hi = nq;                                  // first pair with chunk >= c_lo
         while (lo < hi) {
             const uint64_t mid = (lo + hi) >> 1;
@@ -722,8 +761,6 @@ bool normalise_ordered_copy(const pccl_condition_t* pre, const pccl_condition_t*
         }
         s.k_lo = lo;
         uint64_t k = lo, nd = 0;
-        uint32_t* f_src = s.f_src.data();
-        uint32_t* f_dst = s.f_dst.data();
         for (uint32_t c = s.c_lo; c < s.c_hi; ++c) {
             const pccl_pair_t a = pp[c];
             if (a.chunk != c || a.npu >= N || !mem[a.npu]) return;
@@ -739,44 +776,35 @@ bool normalise_ordered_copy(const pccl_condition_t* pre, const pccl_condition_t*
                 have_prev = true;
                 ++k;
                 if (d == src) continue;
-                f_dst[d] = 1;
+                if (!__atomic_load_n(fd + d, __ATOMIC_RELAXED)) __atomic_store_n(fd + d, (unsigned char)1, __ATOMIC_RELAXED);
                 ++nd;
             }
-            if (nd > first) f_src[src] = 1;
+            if (nd > first && !__atomic_load_n(fs + src, __ATOMIC_RELAXED)) __atomic_store_n(fs + src, (unsigned char)1, __ATOMIC_RELAXED);
         }
         s.k_end = k;
         s.nd = nd;
         s.ok = true;
     };
-    // between the passes, thread 0 checks that the slices tile the list, sizes the arrays and hands out the offsets;
-    // the other threads (awake anyway) spin for those few microseconds instead of going back to sleep
-    uint32_t* o_src = nullptr;
-    uint64_t* o_off = nullptr;
-    uint32_t* o_dst = nullptr;
-    uint32_t* o_chk = nullptr;
+    g_threads.parallel_for(T, pass1);
+    // between the passes: the slices must tile the list; size the arrays, hand out the offsets
     std::vector<uint64_t> nd_base((size_t)T, 0);
-    std::atomic<int> arrived{0}, go{0};                          // go: 1 write, 2 give up (not the ordered form), 3 out of memory
-    auto between = [&]() -> int {
-        uint64_t nd_total = 0;
-        for (int t = 0; t < T; ++t) {
-            if (!sl[t].ok) return 2;
-            if (sl[t].k_lo != (t == 0 ? 0 : sl[t - 1].k_end)) return 2;   // the slices tile the list
-            nd_total += sl[t].nd;
-        }
-        if (sl[T - 1].k_end != nq) return 2;                     // pairs of a chunk id >= C, or out of order
-        try {
-            cp.cond_src.resize(C);
-            cp.dest_off.resize((size_t)C + 1);
-            cp.dests.resize(nd_total);
-            cp.dchunk.resize(nd_total);
-        } catch (const std::bad_alloc&) {
-            return 3;
-        }
-        o_src = cp.cond_src.data(); o_off = cp.dest_off.data(); o_dst = cp.dests.data(); o_chk = cp.dchunk.data();
-        o_off[0] = 0;
-        for (int t = 1; t < T; ++t) nd_base[t] = nd_base[t - 1] + sl[t - 1].nd;
-        return 1;
-    };
+    uint64_t nd_total = 0;
+    for (int t = 0; t < T; ++t) {
+        if (!sl[t].ok) return false;
+        if (sl[t].k_lo != (t == 0 ? 0 : sl[t - 1].k_end)) return false;
+        nd_base[t] = nd_total;
+        nd_total += sl[t].nd;
+    }
+    if (sl[T - 1].k_end != nq) return false;                     // pairs of a chunk id >= C, or out of order
+    cp.cond_src.resize(C);                                       // (std::bad_alloc is the caller's to turn into NOMEM)
+    cp.dest_off.resize((size_t)C + 1);
+    cp.dests.resize(nd_total);
+    cp.dchunk.resize(nd_total);
+    uint32_t* o_src = cp.cond_src.data();
+    uint64_t* o_off = cp.dest_off.data();
+    uint32_t* o_dst = cp.dests.data();
+    uint32_t* o_chk = cp.dchunk.data();
+    o_off[0] = 0;
     // pass 2: write (everything was validated).  The four arrays go to the device next, by DMA from these very
     // (page-locked) blocks: non-temporal stores put them in memory instead of leaving dirty lines in the caches of
     // whichever cores the slices ran on (measured on the B200 host: DMA of lines that sit modified in other cores'
@@ -799,24 +827,10 @@ bool normalise_ordered_copy(const pccl_condition_t* pre, const pccl_condition_t*
         }
         nt_fence();
     };
-    const std::function<void(int)> both = [&](int t) {
-        pass1(t);
-        arrived.fetch_add(1, std::memory_order_acq_rel);
-        if (t == 0) {
-            while (arrived.load(std::memory_order_acquire) < T) cpu_relax();
-            go.store(between(), std::memory_order_release);
-        } else {
-            while (go.load(std::memory_order_acquire) == 0) cpu_relax();
-        }
-        if (go.load(std::memory_order_acquire) == 1) pass2(t);
-    };
-    g_threads.run(T, both);
-    if (go.load() == 3) throw std::bad_alloc();
-    if (go.load() != 1) return false;
-    std::vector<char> f_src(N, 0), f_dst(N, 0);
-    for (int t = 0; t < T; ++t)
-        for (uint32_t v = 0; v < N; ++v) { f_src[v] |= (char)sl[t].f_src[v]; f_dst[v] |= (char)sl[t].f_dst[v]; }
-    index_phase(cp, N, f_src, f_dst);
+    g_threads.parallel_for(T, pass2);
+    std::vector<char> f_src_c(N, 0), f_dst_c(N, 0);
+    for (uint32_t v = 0; v < N; ++v) { f_src_c[v] = (char)f_src[v]; f_dst_c[v] = (char)f_dst[v]; }
+    index_phase(cp, N, f_src_c, f_dst_c);
     return true;
 }
 
@@ -1387,15 +1401,15 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     // `pad` bytes of (unused) dynamic shared memory keep a window's CTAs off the SMs where a CTA of the loop is resident:
     // beside the loop's latency-bound warps they cost it 0.18 ms at config 4 (measured); on the SMs the loop leaves free
     // they cost it nothing
-    auto window = [&](cudaStream_t s, int final, size_t pad) -> cudaError_t {
+    auto window = [&](cudaStream_t s, int final, size_t pad, uint32_t wgrid) -> cudaError_t {
         k_win_begin<<<1, 1024, pad, counted(s)>>>(a, final);
-        k_win_times<<<N, 256, pad, counted(s)>>>(a);
+        k_win_times<<<wgrid, 256, pad, counted(s)>>>(a);
         if (!raw_only) {
             k_win_rank<<<(a.ecap + 255) / 256, 256, pad, counted(s)>>>(a);
             k_win_base<<<1, 1024, pad, counted(s)>>>(a);
-            k_win_bits<<<N, 256, pad, counted(s)>>>(a);
+            k_win_bits<<<wgrid, 256, pad, counted(s)>>>(a);
             k_win_wbase<<<std::min<uint32_t>((a.ecap + 7) / 8, 256u), 256, pad, counted(s)>>>(a);
-            k_win_write<<<N, 256, pad, counted(s)>>>(a);
+            k_win_write<<<wgrid, 256, pad, counted(s)>>>(a);
             k_win_end<<<1, 1, 0, counted(s)>>>(a);
         } else {
             k_emit_raw<<<N, 256, 0, counted(s)>>>(a);
@@ -1406,23 +1420,20 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     volatile unsigned long long* progress = (volatile unsigned long long*)((unsigned char*)G.mailbox + 2048);
     // Early windows -- the emitter running on a second stream while the loop is going -- in two cases.  (i) The records
     // leave for the host: the download then overlaps the loop.  (ii) They stay on the device and the loop leaves SMs free
-    // (config 4: 128 CTAs on 148 SMs): what is left for the window after the loop is only the tail of the schedule.  Window
-    // CTAs resident BESIDE the loop's latency-bound warps cost it 0.1-0.18 ms at config 4 (measured): worth it for (i), not
-    // for (ii) -- there `win_pad` bytes of unused dynamic shared memory keep them on the SMs without a CTA of the loop
-    // (loop + emit 2.52 -> 2.41 ms at config 4; with the pad in case (i) the windows fall behind the download: 3.4 -> 4.1 ms).
+    // (config 4: 128 CTAs on 148 SMs): what is left for the window after the loop is only the tail of the schedule.
+    // Window CTAs resident BESIDE the loop's latency-bound warps cost it 0.1-0.18 ms at config 4 (measured).  When the
+    // loop leaves at least 16 SMs free, an early window is therefore launched with only as many CTAs as fit on those SMs
+    // (8 of 256 threads each; the block scheduler fills idle SMs first) striding over the nodes, and 24 KB of unused
+    // dynamic shared memory per CTA keeps it at 8 per SM: loop + emit 2.52 -> 2.41 ms at config 4 with the records kept
+    // on the device, end to end 3.8 -> 3.7 ms in the same process.  (One CTA per free SM, forced by a 216 KB pad, is too
+    // slow: the windows fall behind the download, 3.4 -> 4.1 ms.)  With fewer free SMs (config 5: one) case (i) uses the
+    // full grid and case (ii) has no early windows.
     const bool stream_out = !raw_only && out_cap > 0 && host_out != nullptr;
-    size_t win_pad = 0;
-    if (!stream_out && !raw_only && out_cap > 0 && (uint32_t)G.sm_count >= W.a2_grid + 16u && W.a2.smem_need + 218 * 1024 > 227 * 1024) {
-        win_pad = 216 * 1024;
-        static std::atomic<int> padded_dev{-1};      // the attribute is per device function: set once per device in use
-        if (padded_dev.load() != G.dev) {
-            const void* ks[] = {(const void*)k_win_begin, (const void*)k_win_times, (const void*)k_win_rank, (const void*)k_win_base,
-                                (const void*)k_win_bits, (const void*)k_win_wbase, (const void*)k_win_write};
-            for (const void* k : ks) CU(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)win_pad));
-            padded_dev.store(G.dev);
-        }
-    }
-    const bool early = stream_out || win_pad != 0;
+    const uint32_t free_sms = (uint32_t)G.sm_count > W.a2_grid ? (uint32_t)G.sm_count - W.a2_grid : 0u;
+    const bool shielded = !raw_only && out_cap > 0 && free_sms >= 16u;
+    const size_t win_pad = shielded ? 24 * 1024 : 0;
+    const uint32_t wgrid_early = shielded ? std::min<uint32_t>(N, free_sms * 8u) : N;
+    const bool early = stream_out || shielded;
     uint64_t copied = 0;
     struct Drain {   // whatever happens, nothing of this call is left running on the side streams
         bool on;
@@ -1444,8 +1455,10 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
         CU(cudaStreamWaitEvent(G.emit_stream, G.pre_loop, 0));
     }
     if (tm) { tm->setup.stop(); tm->loop.start(); }
+    DBGT("  a2 setup enqueued");
     CU(cudaLaunchCooperativeKernel(kloop2, dim3(W.a2_grid), dim3(threads), args, smem, counted(st)));
     if (tm) tm->loop.stop();
+    DBGT("  loop launched");
     if (early) {
         // windows on the emit stream while the loop runs (it never waits for them; they read headers and logs only);
         // finished records leave in pieces of >= 2 MB on the copy stream.  Both streams are drained before anything
@@ -1462,7 +1475,7 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
                                     G.copy_stream);
                 copied = p;
             }
-            if (e == cudaSuccess) e = window(G.emit_stream, 0, win_pad);
+            if (e == cudaSuccess) e = window(G.emit_stream, 0, win_pad, wgrid_early);
             if (e == cudaSuccess) e = cudaEventRecord(G.win_done, G.emit_stream);
             in_flight = any = true;
         }
@@ -1477,9 +1490,10 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
             return PCCL_ERR_CUDA;
         }
     }
+    DBGT("  loop done (polling)");
     if (tm) tm->emit.start();
     {
-        const cudaError_t e = window(st, 1, 0);
+        const cudaError_t e = window(st, 1, 0, N);
         if (e != cudaSuccess) {
             (void)cudaStreamSynchronize(G.copy_stream);
             (void)cudaStreamSynchronize(st);
@@ -1493,6 +1507,7 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     CU(cudaMemcpyAsync(mb, W.ctrl, sizeof(LoopCtrl), cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(mb2, W.a2ctrl, sizeof(A2Ctrl), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    DBGT("  final window synced");
 #ifdef PCCL_A2_PROFILE
     fprintf(stderr, "[a2 profile] actions %llu polls %llu | cycles per action: philox %.0f poll %.0f apply %.0f pick %.0f commit %.0f next %.0f | per poll: load wait %.0f evaluate %.0f\n",
             mb2->actions, mb2->polls, (double)mb2->prof[0] / mb2->actions, (double)mb2->prof[1] / mb2->actions,
@@ -1523,6 +1538,7 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
             CU(cudaMemcpyAsync(host_out + copied, out + copied, (mb2->total - copied) * sizeof(Rec), cudaMemcpyDeviceToHost,
                                G.copy_stream));
         CU(cudaStreamSynchronize(G.copy_stream));
+        DBGT("  tail copy synced");
         if (streamed) *streamed = true;
     }
     res->total = mb2->total; res->tmax = mb2->tmax;
@@ -2022,6 +2038,7 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
     SERIALISE;
     if (!P || !out) return PCCL_ERR_INVALID;
     int rc = problem_upload(P, false);
+    DBGT("upload enqueued");
     if (rc) return rc;
     pccl_schedule* S = new (std::nothrow) pccl_schedule();
     if (!S) { if (cudaStreamSynchronize(G.stream) != cudaSuccess) (void)cudaGetLastError(); return PCCL_ERR_NOMEM; }
@@ -2125,7 +2142,9 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
             rc = phase_setup(*P, ph, W, seed, &M_thin, false, false);
             if (rc) return fail(rc);
         }
+        DBGT("before phase_setup");
         rc = phase_setup(*P, ph, W, seed, &M, dynamic, plan_async);
+        DBGT("phase_setup (synced)");
         if (rc) return fail(rc);
         t_setup.stop();
         S->stats.wants_total += M;
@@ -2186,7 +2205,9 @@ extern "C" int pccl_problem_synthesize(pccl_problem_t* P, uint64_t seed, uint32_
                     S->h_bytes = cap * sizeof(Rec);
                     S->h_recs = pinned_get(S->h_bytes);   // null: no streaming, the download reports the failure
                 }
+                DBGT("before phase_loop");
                 rc = phase_loop(*P, ph, W, seed, flags, out_recs + base, cap, toff, &lr, &tm, &S->trace, (Rec*)S->h_recs, &streamed);
+                DBGT("phase_loop returns");
                 if (rc == PCCL_ERR_NOMEM && dynamic && attempt == 0 && lr.total > cap && lr.total <= M) {
                     dev_free(out_recs); out_recs = nullptr;
                     cap = lr.total;
@@ -2226,12 +2247,16 @@ extern "C" int pccl_synthesize(const pccl_topology_t* topo, const uint32_t* grou
                                const pccl_condition_t* pre, const pccl_condition_t* post, uint64_t chunk_bytes,
                                uint64_t seed, pccl_schedule_t** out) {
     if (!out) return PCCL_ERR_INVALID;
+    DBGT("-- pccl_synthesize");
     pccl_problem_t* P = nullptr;
     int rc = pccl_problem_create(topo, group_members, n_members, pre, post, chunk_bytes, &P);
+    DBGT("problem_create (normalise)");
     if (rc) return rc;
     pccl_schedule_t* S = nullptr;
     rc = pccl_problem_synthesize(P, seed, 0, &S);
+    DBGT("problem_synthesize returns");
     pccl_problem_destroy(P);
+    DBGT("problem_destroy");
     if (rc) return rc;
     *out = S;
     return PCCL_OK;

@@ -878,14 +878,15 @@ __global__ void __launch_bounds__(1024) k_win_begin(A2Args a, int final) {
 // block per node: hash the start and end time of every claim of the window; count the records per start time
 __global__ void __launch_bounds__(256) k_win_times(A2Args a) {
     __shared__ uint32_t s_n;
-    const uint32_t v = blockIdx.x;
     const unsigned long long gvt = a.win->gvt;
+    unsigned long long tmax = 0;
+  for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x) {   // (a block per node, or fewer blocks striding over the nodes)
     const uint32_t cnt = (uint32_t)ld128(a.hdr + v).hi, c0 = a.wcur[v];
     const unsigned long long base = a.nbase[v];
     const uint32_t e0 = a.in_off[v];
+    __syncthreads();
     if (threadIdx.x == 0) s_n = 0;
     __syncthreads();
-    unsigned long long tmax = 0;
     uint32_t mine = 0;
     for (uint32_t i = c0 + threadIdx.x; i < cnt; i += blockDim.x) {
         U128 en = ld128(a.log + base + i);
@@ -909,15 +910,16 @@ __global__ void __launch_bounds__(256) k_win_times(A2Args a) {
         if (!(atomicOr(&a.tflag[s2], 1u) & 1u)) atomicAdd(&a.ctrl->n_end, 1u);
     }
     if (mine) atomicAdd(&s_n, mine);
-    for (int o = 16; o; o >>= 1) tmax = max(tmax, __shfl_xor_sync(0xFFFFFFFFu, tmax, o));
-    if ((threadIdx.x & 31) == 0) {
-        if (tmax) atomicMax(&a.ctrl->tmax, tmax);
-        if (2u * (a.ctrl->n_start + a.ctrl->n_end) > a.tcap) atomicOr(&a.ctrl->err, 1u);   // keep the table half empty
-    }
     __syncthreads();
     if (threadIdx.x == 0) {
         a.wnext[v] = c0 + s_n;
         if (s_n) atomicAdd(&a.ctrl->total, (unsigned long long)s_n);
+    }
+  }
+    for (int o = 16; o; o >>= 1) tmax = max(tmax, __shfl_xor_sync(0xFFFFFFFFu, tmax, o));
+    if ((threadIdx.x & 31) == 0) {
+        if (tmax) atomicMax(&a.ctrl->tmax, tmax);
+        if (2u * (a.ctrl->n_start + a.ctrl->n_end) > a.tcap) atomicOr(&a.ctrl->err, 1u);   // keep the table half empty
     }
 }
 
@@ -958,15 +960,16 @@ __global__ void __launch_bounds__(1024) k_win_base(A2Args a) {
 // the links matched at every start time of the window
 __global__ void __launch_bounds__(256) k_win_bits(A2Args a) {
     if (a.ctrl->err & 1u) return;   // the table or the bitmaps overflowed: ranks are not valid, the host sorts instead
-    const uint32_t v = blockIdx.x;
-    const uint32_t c0 = a.wcur[v], c1 = a.wnext[v];
-    const unsigned long long base = a.nbase[v];
-    const uint32_t e0 = a.in_off[v];
-    for (uint32_t i = c0 + threadIdx.x; i < c1; i += blockDim.x) {
-        const U128 en = ld128(a.log + base + i);
-        const uint32_t l = a.in_link[e0 + ((uint32_t)(en.hi >> 32) & 7u)];
-        const uint32_t r = a.trank[a.eslot[base + i]];
-        atomicOr(a.bm + (size_t)r * a.nLw + (l >> 6), 1ull << (l & 63));
+    for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x) {
+        const uint32_t c0 = a.wcur[v], c1 = a.wnext[v];
+        const unsigned long long base = a.nbase[v];
+        const uint32_t e0 = a.in_off[v];
+        for (uint32_t i = c0 + threadIdx.x; i < c1; i += blockDim.x) {
+            const U128 en = ld128(a.log + base + i);
+            const uint32_t l = a.in_link[e0 + ((uint32_t)(en.hi >> 32) & 7u)];
+            const uint32_t r = a.trank[a.eslot[base + i]];
+            atomicOr(a.bm + (size_t)r * a.nLw + (l >> 6), 1ull << (l & 63));
+        }
     }
 }
 
@@ -987,11 +990,12 @@ __global__ void __launch_bounds__(256) k_win_wbase(A2Args a) {
 }
 
 __global__ void __launch_bounds__(256) k_win_write(A2Args a) {
-    const uint32_t v = blockIdx.x;
+  const bool bad = (a.ctrl->err & 1u) != 0u;
+  for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x) {
     const uint32_t c0 = a.wcur[v], c1 = a.wnext[v];
     __syncthreads();
     if (threadIdx.x == 0) a.wcur[v] = c1;                        // the next window starts here
-    if (a.ctrl->err & 1u) return;
+    if (bad) continue;
     const unsigned long long base = a.nbase[v];
     const uint32_t e0 = a.in_off[v];
     const uint32_t* ids = a.ids + base;
@@ -1008,6 +1012,7 @@ __global__ void __launch_bounds__(256) k_win_write(A2Args a) {
         o[0] = make_uint4(a.orig != nullptr ? a.orig[ch] : ch, a.psrc[l], a.pdst[l], l);
         o[1] = make_uint4((uint32_t)ts, (uint32_t)(ts >> 32), (uint32_t)te, (uint32_t)(te >> 32));
     }
+  }
 }
 
 // the window is written: records [0, emitted) are final (and told to the host when it is streaming them out)
