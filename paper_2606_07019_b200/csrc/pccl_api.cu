@@ -1360,11 +1360,11 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     a.out = out; a.out_cap = out_cap; a.t_offset = t_offset;
     Carver c;
     const size_t o_ids = c.take(M * 4), o_rp = c.take((size_t)N * W.Wp * 4), o_xm = c.take(W.a2.xmap_total * 4),
-                 o_pr = c.take(W.a2.priv_total * 4), o_hdr = c.take((size_t)N * 16), o_es = c.take(M * 4),
+                 o_pr = c.take(W.a2.priv_total * 4), o_hdr = c.take((size_t)N * 16 * A2_HDR_STRIDE), o_es = c.take(M * 4),
                  o_us = c.take((size_t)a.ecap * 4), o_cs = c.take((size_t)a.ecap * 4), o_eb = c.take((size_t)a.ecap * 8),
                  o_wb = c.take((size_t)a.ecap * W.nLw * 4), o_tr = c.take((size_t)a.tcap * 4);
     const size_t o_ff = c.cur;                                   // filled with 0xFF: the log and the time keys
-    const size_t o_log = c.take(M * 16), o_tk = c.take((size_t)a.tcap * 8);
+    const size_t o_log = c.take(M * 16 * A2_LOG_STRIDE), o_tk = c.take((size_t)a.tcap * 8);
     const size_t o_zero = c.cur;                                 // cleared
     const size_t o_tc = c.take((size_t)a.tcap * 4), o_tf = c.take((size_t)a.tcap * 4), o_bm = c.take((size_t)a.ecap * W.nLw * 8);
     const size_t o_wc = c.take((size_t)N * 4), o_wn = c.take((size_t)N * 4), o_win = c.take(sizeof(A2Win));

@@ -69,6 +69,14 @@ __device__ __forceinline__ void ld128x2(const U128* p0, bool on0, const U128* p1
 }
 
 constexpr int A2_MAX_IN = 8;         // in-links per node (one quad of lanes each)
+#ifndef A2_HDR_STRIDE
+#define A2_HDR_STRIDE 8              // U128 units between two nodes' headers: one header per 128-byte line
+#endif
+#define A2_HDR(a, v) ((a).hdr + (size_t)(v) * A2_HDR_STRIDE)
+#ifndef A2_LOG_STRIDE
+#define A2_LOG_STRIDE 1              // U128 units between two log entries (a sector or a line per entry was tried: no gain)
+#endif
+#define A2_LOG(a, i) ((a).log + (size_t)(i) * A2_LOG_STRIDE)
 constexpr int A2_MAX_WARPS = 16;     // destinations per CTA
 
 struct A2Ctrl {                      // read back once by the host after the plan kernel / after the loop
@@ -306,7 +314,7 @@ __global__ void __launch_bounds__(128) k_a2_priv(A2Args a) {
     const uint32_t v = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const uint32_t W = a.wants_cnt[v];
     const uint32_t e0 = a.in_off[v], nin = a.in_off[v + 1] - e0;
-    if (threadIdx.x == 0) st128(a.hdr + v, W ? 0ull : T_INF, 0ull);
+    if (threadIdx.x == 0) st128(A2_HDR(a, v), W ? 0ull : T_INF, 0ull);
     if (W == 0) return;
     const uint32_t Wd = (W + 31) >> 5, G = (Wd + 31) >> 5;
     uint32_t* live = a.priv + a.poff[v];
@@ -565,7 +573,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
     __syncwarp();
     const uint32_t nsrc = f.nsrc;
     const int nslots = nsrc > 4 ? 2 : 1;                             // sources 4..7 use the second item of every lane
-    U128* mylog = a.log + a.nbase[v];
+    U128* mylog = A2_LOG(a, a.nbase[v]);
     const uint32_t my_link = lane < nin ? f.link[lane] : 0u;
     // the two items of this lane in a poll: (source s0 = lane / 8, k = lane % 8) and (source s0 + 4, k); k = 0 is the
     // source's header, k = 1..7 its log entries cur + k - 1.  Everything static about the two sources sits in registers.
@@ -583,7 +591,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
         p_W[sl] = p_act[sl] ? f.s_W[s] : 0u;
         p_cur[sl] = 0;
         p_xm[sl] = a.xmap + (p_act[sl] ? f.s_xbase[s] : 0ull);
-        p_ptr[sl] = !p_act[sl] ? a.hdr : (kq == 0 ? a.hdr + f.s_node[s] : a.log + f.s_logbase[s] + (kq - 1));
+        p_ptr[sl] = !p_act[sl] ? a.hdr : (kq == 0 ? A2_HDR(a, f.s_node[s]) : A2_LOG(a, f.s_logbase[s] + (kq - 1)));
     }
     unsigned long long t = 0;
     uint32_t cnt = 0, remaining = W;
@@ -613,7 +621,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
                 const uint32_t s0 = lane >> 3, s1 = 4 + s0;
                 const bool on0 = p_act[0] && ((need >> s0) & 1u) && (kq == 0 || p_cur[0] + kq - 1 < p_W[0]);
                 const bool on1 = nslots == 2 && p_act[1] && ((need >> s1) & 1u) && (kq == 0 || p_cur[1] + kq - 1 < p_W[1]);
-                ld128x2(p_ptr[0] + (kq == 0 ? 0u : p_cur[0]), on0, p_ptr[1] + (kq == 0 ? 0u : p_cur[1]), on1, it[0], it[1]);
+                ld128x2(p_ptr[0] + (kq == 0 ? 0u : p_cur[0] * A2_LOG_STRIDE), on0, p_ptr[1] + (kq == 0 ? 0u : p_cur[1] * A2_LOG_STRIDE), on1, it[0], it[1]);
             }
             if (!have_r) {   // the pick's draw depends on (t, link) only: computed while the loads are in flight
                 if (lane < nin) r_mine = philox_draw((uint32_t)t, (uint32_t)(t >> 32), my_link, 0u, a.k0, a.k1);
@@ -767,7 +775,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
             const bool stand = on && j4 < first_bad;
             const uint32_t smask = __ballot_sync(0xFFFFFFFFu, stand && q4 == 0);        // bit 4j
             if (stand && e_spec == NONE32) { atomicOr(a.abort_flag, 4u); return; }      // cannot happen
-            U128* slot = mylog + cnt + __popc(smask & ((1u << (4 * j4)) - 1u));
+            U128* slot = mylog + (size_t)(cnt + __popc(smask & ((1u << (4 * j4)) - 1u))) * A2_LOG_STRIDE;
             claims = (uint32_t)__popc(smask);
             if (first_bad >= nin) {
                 // the common case: every pick stands.  Publish first -- the claims, then the header with the next event
@@ -781,7 +789,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
                     const uint32_t ml = __reduce_min_sync(0xFFFFFFFFu, hi == mh ? (uint32_t)nt_o : 0xFFFFFFFFu);
                     nt = ((unsigned long long)mh << 32) | ml;
                 }
-                if (lane == 0) st128(a.hdr + v, remaining == claims ? T_INF : nt, (unsigned long long)(cnt + claims));
+                if (lane == 0) st128(A2_HDR(a, v), remaining == claims ? T_INF : nt, (unsigned long long)(cnt + claims));
                 a2_commit(f, live, cb, grp, nin, Wd, G, stand, e_spec, j4, q4, t, nullptr);
                 __syncwarp();
             } else {
@@ -795,7 +803,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
                     const uint32_t e2 = a2_pick<PRIO>(cb + j * Wd, grp + j * G, Wd, G, n2, r2, j4 == j, q4, lane, pb, W);
                     const uint32_t e = __shfl_sync(0xFFFFFFFFu, e2, 4 * j);
                     if (e == NONE32) { if (lane == 0) atomicOr(a.abort_flag, 4u); return; }   // cannot happen
-                    a2_commit(f, live, cb, grp, nin, Wd, G, j4 == j, e, j4, q4, t, mylog + cnt + claims);
+                    a2_commit(f, live, cb, grp, nin, Wd, G, j4 == j, e, j4, q4, t, mylog + (size_t)(cnt + claims) * A2_LOG_STRIDE);
                     ++claims;
                     ++st_slow;
                     __syncwarp();
@@ -806,7 +814,7 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
                     const uint32_t ml = __reduce_min_sync(0xFFFFFFFFu, hi == mh ? (uint32_t)nt_o : 0xFFFFFFFFu);
                     nt = ((unsigned long long)mh << 32) | ml;
                 }
-                if (lane == 0) st128(a.hdr + v, remaining == claims ? T_INF : nt, (unsigned long long)(cnt + claims));
+                if (lane == 0) st128(A2_HDR(a, v), remaining == claims ? T_INF : nt, (unsigned long long)(cnt + claims));
             }
         }
         A2_TICK(4)
@@ -864,7 +872,7 @@ __global__ void __launch_bounds__(1024) k_win_begin(A2Args a, int final) {
     __shared__ unsigned long long sm[32];
     unsigned long long g = T_INF;
     if (!final)
-        for (uint32_t v = threadIdx.x; v < a.N; v += 1024) g = min(g, ld128(a.hdr + v).lo);
+        for (uint32_t v = threadIdx.x; v < a.N; v += 1024) g = min(g, ld128(A2_HDR(a, v)).lo);
     for (int o = 16; o; o >>= 1) g = min(g, __shfl_xor_sync(0xFFFFFFFFu, g, o));
     if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = g;
     __syncthreads();
@@ -881,7 +889,7 @@ __global__ void __launch_bounds__(256) k_win_times(A2Args a) {
     const unsigned long long gvt = a.win->gvt;
     unsigned long long tmax = 0;
   for (uint32_t v = blockIdx.x; v < a.N; v += gridDim.x) {   // (a block per node, or fewer blocks striding over the nodes)
-    const uint32_t cnt = (uint32_t)ld128(a.hdr + v).hi, c0 = a.wcur[v];
+    const uint32_t cnt = (uint32_t)ld128(A2_HDR(a, v)).hi, c0 = a.wcur[v];
     const unsigned long long base = a.nbase[v];
     const uint32_t e0 = a.in_off[v];
     __syncthreads();
@@ -889,10 +897,10 @@ __global__ void __launch_bounds__(256) k_win_times(A2Args a) {
     __syncthreads();
     uint32_t mine = 0;
     for (uint32_t i = c0 + threadIdx.x; i < cnt; i += blockDim.x) {
-        U128 en = ld128(a.log + base + i);
+        U128 en = ld128(A2_LOG(a, base + i));
         for (uint32_t spins = 0; en.hi == T_INF; ++spins) {       // counted by the header, the store is on its way
             if (spins > (1u << 22)) { atomicOr(a.abort_flag, 256u); break; }
-            en = ld128(a.log + base + i);
+            en = ld128(A2_LOG(a, base + i));
         }
         if (en.lo >= gvt) break;                                  // (log in time order: so are the later ones)
         ++mine;
@@ -965,7 +973,7 @@ __global__ void __launch_bounds__(256) k_win_bits(A2Args a) {
         const unsigned long long base = a.nbase[v];
         const uint32_t e0 = a.in_off[v];
         for (uint32_t i = c0 + threadIdx.x; i < c1; i += blockDim.x) {
-            const U128 en = ld128(a.log + base + i);
+            const U128 en = ld128(A2_LOG(a, base + i));
             const uint32_t l = a.in_link[e0 + ((uint32_t)(en.hi >> 32) & 7u)];
             const uint32_t r = a.trank[a.eslot[base + i]];
             atomicOr(a.bm + (size_t)r * a.nLw + (l >> 6), 1ull << (l & 63));
@@ -1000,7 +1008,7 @@ __global__ void __launch_bounds__(256) k_win_write(A2Args a) {
     const uint32_t e0 = a.in_off[v];
     const uint32_t* ids = a.ids + base;
     for (uint32_t i = c0 + threadIdx.x; i < c1; i += blockDim.x) {
-        const U128 en = ld128(a.log + base + i);
+        const U128 en = ld128(A2_LOG(a, base + i));
         const uint32_t l = a.in_link[e0 + ((uint32_t)(en.hi >> 32) & 7u)];
         const uint32_t r = a.trank[a.eslot[base + i]];
         const unsigned long long word = a.bm[(size_t)r * a.nLw + (l >> 6)];
@@ -1029,12 +1037,12 @@ __global__ void k_win_end(A2Args a) {
 // the time table or the per-event bitmaps are too small
 __global__ void __launch_bounds__(256) k_emit_raw(A2Args a) {
     const uint32_t v = blockIdx.x;
-    const uint32_t cnt = (uint32_t)ld128(a.hdr + v).hi;
+    const uint32_t cnt = (uint32_t)ld128(A2_HDR(a, v)).hi;
     const unsigned long long base = a.nbase[v];
     const uint32_t e0 = a.in_off[v];
     const uint32_t* ids = a.ids + base;
     for (uint32_t i = threadIdx.x; i < cnt; i += blockDim.x) {
-        const U128 en = a.log[base + i];
+        const U128 en = *A2_LOG(a, base + i);
         const uint32_t l = a.in_link[e0 + ((uint32_t)(en.hi >> 32) & 7u)];
         if (base + i >= a.out_cap) { atomicOr(&a.ctrl->err, 2u); continue; }
         const unsigned long long ts = en.lo + a.t_offset, te = en.lo + a.w[l] + a.t_offset;
