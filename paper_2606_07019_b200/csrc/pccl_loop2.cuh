@@ -613,6 +613,10 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
         uint32_t need = (1u << nsrc) - 1u;           // sources not settled yet
         uint32_t spins = 0, r_mine = 0;
         bool have_r = false;
+        // what this lane saw in the last evaluated poll of this event: a header is identified by its time (every header a
+        // node stores carries a later time than the one before), a log entry by its second word (write-once)
+        unsigned long long seen0 = 0, seen1 = 0;
+        bool have_seen = false;
         uint32_t xh[2] = {NONE32, NONE32}, xv[2] = {NONE32, NONE32};   // consumed entry whose table word is still in flight
         unsigned long long xte[2] = {0, 0};
         while (need) {
@@ -629,6 +633,20 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
             }
             ++st_polls;
             st_bytes += 128u * (uint32_t)__popc(need);
+            {   // nothing new since the last poll (same sources polled, same words back): evaluating it again would change
+                // nothing -- poll again at once, so that the change is seen a whole evaluation earlier
+                const unsigned long long now0 = kq == 0 ? it[0].lo : it[0].hi, now1 = kq == 0 ? it[1].lo : it[1].hi;
+                const bool same = have_seen && now0 == seen0 && now1 == seen1;
+                seen0 = now0; seen1 = now1;
+                if (__all_sync(0xFFFFFFFFu, same)) {
+                    if ((++spins & 63u) == 0u) {
+                        if (ldcg32(a.abort_flag) != 0u) return;
+                        if (spins > (1u << 24)) { if (lane == 0) atomicOr(a.abort_flag, 64u); return; }
+                    }
+                    continue;
+                }
+                have_seen = true;
+            }
 #ifdef PCCL_A2_PROFILE
             const long long q0 = clock64();
             { const unsigned long long z = __shfl_sync(0xFFFFFFFFu, it[0].lo ^ it[1].lo, 0); if (z == 0x1234567ull) ++st_polls; }
@@ -694,32 +712,12 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
                 }
             }
         }
-        // ---- arrivals at the sources at time t become candidates (a3, a5): the entries consumed just now that arrive
-        //      now are applied by the lane that consumed them, the others wait in the pending table ----
+        // ---- arrivals at the sources at time t become candidates (a3, a5).  First the pending table (arrivals consumed at
+        //      earlier events), then the entries consumed just now: their table words are the last loads issued, and their
+        //      round trip (about 800 cycles when an entry and its header became visible in the same poll) runs beside the
+        //      table scan.  An entry that arrives later waits in the pending table ----
         ++st_actions;
         A2_TICK(1)
-#pragma unroll
-        for (int sl = 0; sl < 2; ++sl) {
-            if (xh[sl] != NONE32) {
-                if (xte[sl] <= t) {
-                    const uint32_t e = xv[sl];
-                    if (e != NONE32 && ((live[e >> 5] >> (e & 31)) & 1u)) {
-                        uint32_t m = f.s_mask[xh[sl] >> 3];
-                        while (m) {
-                            const uint32_t j = __ffs(m) - 1;
-                            m &= m - 1;
-                            atomicOr(&cb[j * Wd + (e >> 5)], 1u << (e & 31));
-                            atomicAdd(&grp[j * G + (e >> 10)], 1u);
-                            atomicAdd(&f.n[j], 1u);
-                        }
-                    }
-                } else {
-                    f.pend_e[xh[sl]] = xv[sl];
-                    f.pend_te[xh[sl]] = xte[sl];
-                }
-            }
-        }
-        __syncwarp();
         unsigned long long nt_o = min(lane_lb[0], lane_lb[1]);     // this lane's share of the next event time
 #pragma unroll
         for (int sl = 0; sl < 2; ++sl) {
@@ -741,6 +739,29 @@ __global__ void __launch_bounds__(A2_MAX_WARPS * 32, 1) k_loop2(const A2Args a) 
                     }
                 } else {
                     nt_o = min(nt_o, te);
+                }
+            }
+        }
+        __syncwarp();                                               // (a slot is scanned before a new entry may take it)
+#pragma unroll
+        for (int sl = 0; sl < 2; ++sl) {
+            if (xh[sl] != NONE32) {
+                if (xte[sl] <= t) {
+                    const uint32_t e = xv[sl];
+                    if (e != NONE32 && ((live[e >> 5] >> (e & 31)) & 1u)) {
+                        uint32_t m = f.s_mask[xh[sl] >> 3];
+                        while (m) {
+                            const uint32_t j = __ffs(m) - 1;
+                            m &= m - 1;
+                            atomicOr(&cb[j * Wd + (e >> 5)], 1u << (e & 31));
+                            atomicAdd(&grp[j * G + (e >> 10)], 1u);
+                            atomicAdd(&f.n[j], 1u);
+                        }
+                    }
+                } else {
+                    f.pend_e[xh[sl]] = xv[sl];
+                    f.pend_te[xh[sl]] = xte[sl];
+                    nt_o = min(nt_o, xte[sl]);
                 }
             }
         }
