@@ -344,6 +344,10 @@ __device__ void bfs_search(const BfsArgs& a, uint32_t chunk, unsigned long long*
                 const uint32_t l = os.x, v = os.y;
                 if (v == src && !serial) continue;
                 const uint64_t wl = ((uint64_t)os.w << 32) | os.z;
+                // a transfer over l ends no earlier than au + w(l): past the arrival at the last dest it can neither lie on
+                // a kept path nor tie with one (only the paths to the dests are kept), so it is not looked up
+                // and its far end is not expanded -- the search ends with the sweep that reaches the last dest
+                if (!SW && au + wl > bound) continue;
                 const ulonglong2* row = a.runs + (size_t)l * a.R;
                 uint64_t cand;
                 const uint32_t sr = SW ? a.swidx[v] : NONE32;
