@@ -1214,8 +1214,8 @@ int phase_setup(const pccl_problem& P, const Phase& ph, Work& W, uint64_t seed, 
     if (ND) {
         const size_t wants_smem = (size_t)N * 8 <= 32 * 1024 ? (size_t)N * 8 : 0;   // the staged distance row (k_wants)
         k_wants<<<(unsigned)((ND + 127) / 128), 128, wants_smem, counted(st)>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, ND, pv.esrc, pv.in_off,
-                                                          pv.in_link, W.w, ph.d_sidx, W.D, N, W.Wp, W.SWp, k0, k1, W.wants,
-                                                          W.wsum, W.wants_cnt, &W.ctrl->err, ph.d_orig, wants_smem ? 1u : 0u);
+                                                          pv.in_link, W.w, ph.d_sidx, W.D, N, W.Wp, k0, k1, W.wants,
+                                                          &W.ctrl->err, ph.d_orig, wants_smem ? 1u : 0u);
         k_wants_finish<<<N, 256, 0, counted(st)>>>(W.wants, W.Wp, W.SWp, W.wsum, W.wants_cnt);
     }
     k_sum_u32<<<1, 1024, 0, counted(st)>>>(W.wants_cnt, N, &W.ctrl->wants_total);
@@ -1386,8 +1386,14 @@ int phase_loop_async(const pccl_problem& P, const Phase& ph, const Work& W, uint
     // entries, translation tables, private images (once per phase)
     if (tm) tm->setup.start();
     k_a2_entries<<<N, 256, 0, counted(st)>>>(a);
+    // the translation tables and the private images only depend on the entry lists: side by side on two streams
+    // (config 4: 45 + 36 us one after the other)
+    CU(cudaEventRecord(G.loop_done, st));
+    CU(cudaStreamWaitEvent(G.emit_stream, G.loop_done, 0));
+    k_a2_priv<<<N, 128, 0, counted(G.emit_stream)>>>(a);
+    CU(cudaEventRecord(G.win_done, G.emit_stream));
     if (L) k_a2_xmap<<<L, 128, 0, counted(st)>>>(a);
-    k_a2_priv<<<N, 128, 0, counted(st)>>>(a);
+    CU(cudaStreamWaitEvent(st, G.win_done, 0));
     const size_t smem = (size_t)W.a2.smem_need;
     const int threads = (int)W.a2_wpc * 32;
     const void* kloop2 = ph.ncls ? (const void*)k_loop2<true> : (const void*)k_loop2<false>;

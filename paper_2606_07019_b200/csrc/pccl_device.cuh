@@ -145,8 +145,7 @@ __global__ void __launch_bounds__(128, 12) k_wants(const uint32_t* __restrict__ 
                         const uint32_t* __restrict__ esrc, const uint32_t* __restrict__ in_off,
                         const uint32_t* __restrict__ in_link, const uint64_t* __restrict__ w,
                         const uint32_t* __restrict__ sidx, const uint64_t* __restrict__ D, uint32_t N,
-                        uint32_t Wp, uint32_t SWp, uint32_t k0, uint32_t k1, uint64_t* __restrict__ wants,
-                        uint64_t* __restrict__ wsum, uint32_t* __restrict__ wants_cnt, uint32_t* __restrict__ err,
+                        uint32_t Wp, uint32_t k0, uint32_t k1, uint64_t* __restrict__ wants, uint32_t* __restrict__ err,
                         const uint32_t* __restrict__ orig, uint32_t stage) {   // orig: the caller's id of a relabelled chunk (keys the draw)
     // stage != 0 (N * 8 bytes of dynamic shared memory): the distance row of the block's FIRST pair's source is copied to
     // shared memory.  Collectives list their chunks source by source, so nearly every pair of the block walks on that
