@@ -1184,7 +1184,7 @@ int phase_setup(const pccl_problem& P, const Phase& ph, Work& W, uint64_t seed, 
         const size_t smem = (size_t)N * 8;
         if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        if (NDS) k_distances<<<NDS, 256, smem, counted(st)>>>(pv.edst, pv.esrc, W.w, N, L, ph.d_dsts, W.D);
+        if (NDS) k_distances<<<NDS, 512, smem, counted(st)>>>(pv.edst, pv.esrc, W.w, N, L, ph.d_dsts, W.D);
         if (NP) k_best_init<<<(unsigned)((NP + 255) / 256), 256, 0, counted(st)>>>(ph.d_cond_src, ph.d_dests, ph.d_dchunk, NP, ph.d_didx,
                                                                          W.D, N, W.best, W.drow, &W.ctrl->err);
         if (C) k_have<<<(C + 255) / 256, 256, 0, counted(st)>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
@@ -1207,7 +1207,7 @@ int phase_setup(const pccl_problem& P, const Phase& ph, Work& W, uint64_t seed, 
         const size_t smem = (size_t)N * 8;
         if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        k_distances<<<NS, 256, smem, counted(st)>>>(pv.esrc, pv.edst, W.w, N, L, ph.d_sources, W.D);
+        k_distances<<<NS, 512, smem, counted(st)>>>(pv.esrc, pv.edst, W.w, N, L, ph.d_sources, W.D);
     }
     if (C) k_have<<<(C + 255) / 256, 256, 0, counted(st)>>>(ph.d_cond_src, C, W.Wp, W.SWp, W.have, W.hsum);
     const uint64_t ND = ph.dests.size();
@@ -1780,7 +1780,7 @@ int prio_prepare(pccl_problem& P) {
                     const size_t smem = (size_t)N * 8;
                     if (smem > 200 * 1024) return PCCL_ERR_UNSUPPORTED;
                     if (smem > 48 * 1024) CU(cudaFuncSetAttribute(k_distances, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                    k_distances<<<NS, 256, smem, counted(st)>>>(pv.esrc, pv.edst, (uint64_t*)(b + o_w), N, L, ph.d_sources, (uint64_t*)(b + o_D));
+                    k_distances<<<NS, 512, smem, counted(st)>>>(pv.esrc, pv.edst, (uint64_t*)(b + o_w), N, L, ph.d_sources, (uint64_t*)(b + o_D));
                 }
                 k_cdist<<<(C + 255) / 256, 256, 0, counted(st)>>>(ph.d_cond_src, ph.d_dest_off, ph.d_dests, C, ph.d_sidx, (uint64_t*)(b + o_D), N,
                                                                   (uint64_t*)(b + o_cd), keys[0], vals[0]);
